@@ -1,0 +1,337 @@
+"""Pins for the fp64 oracle (CPU only).  Each test checks ``oracle/`` against something the paper or the
+mathematics fixes -- a printed value, a closed form, an invariant, a brute force written along a DIFFERENT
+route (explicit matrices in the PAPER's column convention) -- never against a retyped copy of its own loop.
+
+P-numbers refer to DESIGN.md "Oracle pins".
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import GATE_CHANNEL, GATE_SCALAR
+
+RNG = np.random.default_rng(20260701)
+
+
+def _rand_inputs(L, H, dk, dv, gate, rng, g_lo=-0.1, normalise=True, beta_hi=1.0):
+    k = rng.standard_normal((L, H, dk)).astype(np.float32)
+    if normalise:
+        k /= np.linalg.norm(k, axis=-1, keepdims=True)
+    v = rng.standard_normal((L, H, dv)).astype(np.float32)
+    gshape = (L, H) if gate == GATE_SCALAR else (L, H, dk)
+    g = (rng.random(gshape) * g_lo).astype(np.float32)
+    beta = (rng.random((L, H)) * beta_hi).astype(np.float32)
+    return k, v, g, beta
+
+
+def _cu(lens):
+    return np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# P4: brute force from explicitly built matrices, in the PAPER's convention (column vectors, left-multiplying;
+# PAPER.md:84 Eq. 2, Table 1), then transposed.  Also pins reading A1 (row vs column convention),
+# G1 (u_i = beta k v^T), G3 (ordered product, later tokens on the left) and A3 (decay-then-erase order).
+# ---------------------------------------------------------------------------------------------------------
+def _paper_convention_bruteforce(k, v, g, beta, gate, S0_paper=None):
+    """k:[L,dk] v:[L,dv] float64.  Returns (S_L paper [dk,dv], T_C paper [dk,dk])."""
+    L, dk = k.shape
+    dv = v.shape[1]
+    I = np.eye(dk)
+    S = np.zeros((dk, dv)) if S0_paper is None else S0_paper.copy()
+    Tc = np.eye(dk)
+    for i in range(L):
+        ki = k[i][:, None]
+        if gate == GATE_SCALAR:  # GDN: T_i = g_i (I - beta_i k_i k_i^T)
+            Ti = np.exp(g[i]) * (I - beta[i] * (ki @ ki.T))
+        else:  # KDA: T_i = (I - beta_i k_i k_i^T) diag(g_i)
+            Ti = (I - beta[i] * (ki @ ki.T)) @ np.diag(np.exp(g[i]))
+        ui = beta[i] * (ki @ v[i][None, :])
+        S = Ti @ S + ui
+        Tc = Ti @ Tc  # prod_{i=n}^{1}: later tokens on the left
+    return S, Tc
+
+
+@pytest.mark.parametrize("gate", [GATE_SCALAR, GATE_CHANNEL])
+@pytest.mark.parametrize("L,dk,dv", [(4, 4, 4), (4, 4, 3), (7, 5, 6)])
+def test_P4_bruteforce_paper_convention(gate, L, dk, dv):
+    rng = np.random.default_rng(100 + L + dk + 7 * gate)
+    k, v, g, beta = _rand_inputs(L, 1, dk, dv, gate, rng, g_lo=-0.5, normalise=False)
+    E, T = oracle.segment_encode(k, v, g, beta, _cu([L]), gate)
+    S_p, T_p = _paper_convention_bruteforce(k[:, 0].astype(np.float64), v[:, 0].astype(np.float64),
+                                            g[:, 0].astype(np.float64), beta[:, 0].astype(np.float64), gate)
+    np.testing.assert_allclose(E[0, 0], S_p.T, rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(T[0, 0], T_p.T, rtol=1e-12, atol=1e-14)
+
+
+def test_P4_unrolled_sum_of_products():
+    """E = sum_t beta_t v_t k_t^T A_{t+1}...A_L and T = A_1 A_2 A_3 A_4 with A_t = alpha_t (I - beta_t k_t k_t^T)
+    (row convention, Eq. 2 unrolled): 4 tokens, dk = dv = 4, matrices built explicitly."""
+    rng = np.random.default_rng(4)
+    L, d = 4, 4
+    k, v, g, beta = _rand_inputs(L, 1, d, d, GATE_SCALAR, rng, g_lo=-0.3, normalise=False)
+    E, T = oracle.segment_encode(k, v, g, beta, _cu([L]))
+    kk, vv = k[:, 0].astype(np.float64), v[:, 0].astype(np.float64)
+    A = [np.exp(float(g[t, 0])) * (np.eye(d) - float(beta[t, 0]) * np.outer(kk[t], kk[t])) for t in range(L)]
+    T_ref = A[0] @ A[1] @ A[2] @ A[3]
+    E_ref = np.zeros((d, d))
+    for t in range(L):
+        # the write enters AFTER token t's own decay/erase: S_t = S_{t-1} A_t + beta_t v_t k_t^T
+        tail = np.eye(d)
+        for s in range(t + 1, L):
+            tail = tail @ A[s]
+        E_ref += float(beta[t, 0]) * np.outer(vv[t], kk[t]) @ tail
+    np.testing.assert_allclose(T[0, 0], T_ref, rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(E[0, 0], E_ref, rtol=1e-12, atol=1e-14)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# P1: compose(encode(C_1..C_n); S_in) == sequential recurrence over the concatenation (Eq. 4/6, Insight 1)
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gate", [GATE_SCALAR, GATE_CHANNEL])
+@pytest.mark.parametrize("lens", [[128, 128], [1, 63, 64, 65, 7], [50, 0, 33], [200]])
+@pytest.mark.parametrize("zero_start", [True, False])
+def test_P1_compose_equals_sequential(gate, lens, zero_start):
+    rng = np.random.default_rng(sum(lens) + 13 * gate + zero_start)
+    H, dk, dv = 2, 16, 12
+    L = sum(lens)
+    k, v, g, beta = _rand_inputs(L, H, dk, dv, gate, rng)
+    E, T = oracle.segment_encode(k, v, g, beta, _cu(lens), gate)
+    S_in = None if zero_start else 0.1 * rng.standard_normal((1, H, dv, dk))
+    ids = np.arange(len(lens), dtype=np.int32)
+    S_comp = oracle.compose(S_in, E, T, ids, np.array([0, len(lens)], dtype=np.int32))
+    S_seq = oracle.sequential(S_in, k, v, g, beta, np.array([0, L], dtype=np.int32), gate)
+    assert oracle.rel_fro(S_comp, S_seq) < 1e-12
+
+
+def test_P1_compose_is_order_sensitive():
+    """Non-commutativity (reading S10): swapping two segments changes the result, and the swapped composition
+    equals the sequential recurrence over the swapped token order."""
+    rng = np.random.default_rng(77)
+    H, d = 1, 8
+    lens = [20, 30]
+    k, v, g, beta = _rand_inputs(50, H, d, d, GATE_SCALAR, rng)
+    E, T = oracle.segment_encode(k, v, g, beta, _cu(lens))
+    cu1 = np.array([0, 2], dtype=np.int32)
+    S01 = oracle.compose(None, E, T, np.array([0, 1], dtype=np.int32), cu1)
+    S10 = oracle.compose(None, E, T, np.array([1, 0], dtype=np.int32), cu1)
+    assert oracle.rel_fro(S10, S01) > 1e-3
+    perm = np.concatenate([np.arange(20, 50), np.arange(0, 20)])
+    S_seq = oracle.sequential(None, k[perm], v[perm], g[perm], beta[perm], np.array([0, 50], dtype=np.int32))
+    assert oracle.rel_fro(S10, S_seq) < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------------------
+# P2: beta = 0  =>  T = (prod alpha) I  (scalar) / diag(prod_t alpha_{t,c}) (per-channel), E = 0  (Table 3)
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gate", [GATE_SCALAR, GATE_CHANNEL])
+def test_P2_beta_zero_closed_form(gate):
+    rng = np.random.default_rng(2 + gate)
+    L, H, dk, dv = 90, 3, 8, 6
+    k, v, g, beta = _rand_inputs(L, H, dk, dv, gate, rng)
+    beta[:] = 0.0
+    E, T = oracle.segment_encode(k, v, g, beta, _cu([L]), gate)
+    assert np.all(E == 0.0)
+    for h in range(H):
+        if gate == GATE_SCALAR:
+            ref = np.exp(g[:, h].astype(np.float64).sum()) * np.eye(dk)
+        else:
+            ref = np.diag(np.exp(g[:, h].astype(np.float64).sum(axis=0)))
+        np.testing.assert_allclose(T[0, h], ref, rtol=1e-12, atol=1e-300)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# P3: Table 2's nine printed values from the oracle's T with constant decay, beta = 0
+# ---------------------------------------------------------------------------------------------------------
+def test_P3_table2_printed_values(golden_dir):
+    rows = []
+    with open(os.path.join(golden_dir, "table2_naive_addition_error.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                e, n, val = line.split()
+                rows.append((int(e), int(n), float(val)))
+    assert len(rows) == 9
+    rng = np.random.default_rng(3)
+    dk, dv = 8, 5
+    S1 = rng.standard_normal((dv, dk))  # stands for S_{C1|0}
+    for e, n, printed in rows:
+        gamma = 1.0 - 2.0 ** e
+        k, v, _, beta = _rand_inputs(n, 1, dk, dv, GATE_SCALAR, rng)
+        beta[:] = 0.0  # RetNet: T_i = gamma I, no delta-rule term
+        g = np.full((n, 1), np.log(gamma), dtype=np.float32)
+        gamma_eff = float(np.exp(np.float64(g[0, 0])))  # the fp32-rounded log-decay the oracle actually sees
+        _, T = oracle.segment_encode(k, v, g, beta, _cu([n]))
+        delta = S1 @ T[0, 0] - S1  # (T_{C2} - I) applied to S_{C1|0}, Eq. 5 (row convention)
+        ratio = np.linalg.norm(delta) / np.linalg.norm(S1)
+        assert abs(ratio - (1.0 - gamma_eff ** n)) < 1e-12
+        assert abs(ratio - printed) <= 5.1e-4, (e, n, ratio, printed)  # printed to 3 decimals
+
+
+# ---------------------------------------------------------------------------------------------------------
+# P5: T(C1 C2) = T(C1) T(C2);  E(C1 C2) = E(C1) T(C2) + E(C2)     (Eq. 4; independence of prefix)
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gate", [GATE_SCALAR, GATE_CHANNEL])
+def test_P5_concatenation_law(gate):
+    rng = np.random.default_rng(5 + gate)
+    H, dk, dv = 2, 10, 7
+    l1, l2 = 37, 91
+    k, v, g, beta = _rand_inputs(l1 + l2, H, dk, dv, gate, rng)
+    E12, T12 = oracle.segment_encode(k, v, g, beta, _cu([l1 + l2]), gate)
+    E, T = oracle.segment_encode(k, v, g, beta, _cu([l1, l2]), gate)
+    for h in range(H):
+        np.testing.assert_allclose(T12[0, h], T[0, h] @ T[1, h], rtol=1e-11, atol=1e-14)
+        np.testing.assert_allclose(E12[0, h], E[0, h] @ T[1, h] + E[1, h], rtol=1e-11, atol=1e-13)
+    # T and E of the second segment do not depend on what precedes it
+    E2, T2 = oracle.segment_encode(k[l1:], v[l1:], g[l1:], beta[l1:], _cu([l2]), gate)
+    assert np.array_equal(E2[0], E[1]) and np.array_equal(T2[0], T[1])
+
+
+# ---------------------------------------------------------------------------------------------------------
+# P6: orthonormal keys k_t = e_{pi(t)} (L <= dk): factors commute; closed form
+# ---------------------------------------------------------------------------------------------------------
+def test_P6_orthonormal_keys_closed_form():
+    rng = np.random.default_rng(6)
+    dk, dv, L = 12, 9, 8
+    pi = rng.permutation(dk)[:L]
+    k = np.zeros((L, 1, dk), dtype=np.float32)
+    k[np.arange(L), 0, pi] = 1.0
+    v = rng.standard_normal((L, 1, dv)).astype(np.float32)
+    g = (rng.random((L, 1)) * -0.3).astype(np.float32)
+    beta = rng.random((L, 1)).astype(np.float32)
+    E, T = oracle.segment_encode(k, v, g, beta, _cu([L]))
+    a = np.exp(g[:, 0].astype(np.float64))
+    b = beta[:, 0].astype(np.float64)
+    T_ref = np.eye(dk)
+    for t in range(L):
+        T_ref[pi[t], pi[t]] -= b[t]
+    T_ref *= a.prod()
+    E_ref = np.zeros((dv, dk))
+    for t in range(L):
+        E_ref[:, pi[t]] += b[t] * a[t + 1:].prod() * v[t, 0].astype(np.float64)
+    np.testing.assert_allclose(T[0, 0], T_ref, rtol=1e-12, atol=1e-15)
+    np.testing.assert_allclose(E[0, 0], E_ref, rtol=1e-12, atol=1e-15)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# P7: one repeated unit key, alpha = 1: T = I - (1 - prod(1-beta_t)) k k^T; constant v: E k = (1 - prod(1-beta)) v
+# ---------------------------------------------------------------------------------------------------------
+def test_P7_repeated_key_lms_convergence():
+    rng = np.random.default_rng(7)
+    dk, dv, L = 9, 5, 25
+    kd = rng.standard_normal(dk)
+    kd /= np.linalg.norm(kd)
+    k32 = kd.astype(np.float32)
+    k = np.tile(k32[None, None, :], (L, 1, 1))
+    v0 = rng.standard_normal(dv).astype(np.float32)
+    v = np.tile(v0[None, None, :], (L, 1, 1))
+    g = np.zeros((L, 1), dtype=np.float32)
+    beta = (rng.random((L, 1)) * 0.9).astype(np.float32)
+    E, T = oracle.segment_encode(k, v, g, beta, _cu([L]))
+    kk = k32.astype(np.float64)
+    n2 = kk @ kk  # fp32-rounded key is not exactly unit: use the general closed form with |k|^2
+    resid = np.prod(1.0 - beta[:, 0].astype(np.float64) * n2)
+    T_ref = np.eye(dk) - (1.0 - resid) * np.outer(kk, kk) / n2
+    np.testing.assert_allclose(T[0, 0], T_ref, rtol=1e-12, atol=1e-15)
+    np.testing.assert_allclose(E[0, 0] @ kk, (1.0 - resid) * v0.astype(np.float64), rtol=1e-12, atol=1e-15)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# P8: the paper's two-invocation route: the E recurrence with dv := dk, v = 0, S_0 = I gives T
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gate", [GATE_SCALAR, GATE_CHANNEL])
+def test_P8_two_invocation_route(gate):
+    rng = np.random.default_rng(8 + gate)
+    L, H, dk = 70, 2, 12
+    k, _, g, beta = _rand_inputs(L, H, dk, dk, gate, rng)
+    v0 = np.zeros((L, H, dk), dtype=np.float32)
+    _, T = oracle.segment_encode(k, v0, g, beta, _cu([L]), gate)
+    S_I = np.tile(np.eye(dk)[None, None], (1, H, 1, 1))
+    S_end = oracle.sequential(S_I, k, v0, g, beta, np.array([0, L], dtype=np.int32), gate)
+    np.testing.assert_allclose(S_end[0], T[0], rtol=1e-13, atol=1e-300)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# P9: det T = prod_t alpha_t^{dk} (1 - beta_t |k_t|^2)   (per-channel: prod_t (prod_c alpha_{t,c}) (1 - beta_t |k_t|^2))
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gate", [GATE_SCALAR, GATE_CHANNEL])
+def test_P9_determinant(gate):
+    rng = np.random.default_rng(9 + gate)
+    L, dk, dv = 11, 6, 4
+    k, v, g, beta = _rand_inputs(L, 1, dk, dv, gate, rng, normalise=False, beta_hi=0.1)
+    _, T = oracle.segment_encode(k, v, g, beta, _cu([L]), gate)
+    sign, logdet = np.linalg.slogdet(T[0, 0])
+    k64, b64, g64 = k[:, 0].astype(np.float64), beta[:, 0].astype(np.float64), g[:, 0].astype(np.float64)
+    fac = 1.0 - b64 * (k64 * k64).sum(-1)
+    log_ref = np.log(np.abs(fac)).sum() + (dk * g64.sum() if gate == GATE_SCALAR else g64.sum())
+    assert sign == np.prod(np.sign(fac))
+    assert abs(logdet - log_ref) < 1e-10
+
+
+# ---------------------------------------------------------------------------------------------------------
+# P10: beta_L = 1, |k_L| = 1  =>  T k_L = 0 and E k_L = v_L;  ||T||_2 <= prod alpha_t for beta |k|^2 in [0,2]
+# ---------------------------------------------------------------------------------------------------------
+def test_P10_last_pair_recalled_and_contraction():
+    rng = np.random.default_rng(10)
+    L, dk, dv = 40, 8, 6
+    k, v, g, beta = _rand_inputs(L, 1, dk, dv, GATE_SCALAR, rng)
+    k[-1, 0] = 0.0
+    k[-1, 0, 3] = 1.0  # exactly unit in fp32
+    beta[-1, 0] = 1.0
+    E, T = oracle.segment_encode(k, v, g, beta, _cu([L]))
+    kL = k[-1, 0].astype(np.float64)
+    assert np.abs(T[0, 0] @ kL).max() < 1e-15
+    np.testing.assert_allclose(E[0, 0] @ kL, v[-1, 0].astype(np.float64), rtol=1e-13)
+    # contraction bound on a run with beta |k|^2 in (0, 1]
+    k2, v2, g2, b2 = _rand_inputs(L, 1, dk, dv, GATE_SCALAR, rng)
+    _, T2 = oracle.segment_encode(k2, v2, g2, b2, _cu([L]))
+    assert np.linalg.norm(T2[0, 0], 2) <= np.exp(g2.astype(np.float64).sum()) * (1 + 1e-6)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Degenerate cases and layout
+# ---------------------------------------------------------------------------------------------------------
+def test_empty_segment_is_identity():
+    rng = np.random.default_rng(11)
+    k, v, g, beta = _rand_inputs(5, 2, 4, 3, GATE_SCALAR, rng)
+    E, T = oracle.segment_encode(k, v, g, beta, _cu([0, 5, 0]))
+    for s in (0, 2):
+        assert np.all(E[s] == 0)
+        assert np.array_equal(T[s], np.tile(np.eye(4)[None], (2, 1, 1)))
+
+
+def test_compose_empty_list_copies_s_in_and_f32_pools_match_f64():
+    rng = np.random.default_rng(12)
+    P, H, dk, dv = 5, 2, 6, 4
+    E = rng.standard_normal((P, H, dv, dk)).astype(np.float32)
+    T = (rng.standard_normal((P, H, dk, dk)) * 0.3).astype(np.float32)
+    S_in = rng.standard_normal((2, H, dv, dk))
+    ids = np.array([3, 1, 4], dtype=np.int32)
+    cu = np.array([0, 0, 3], dtype=np.int32)
+    out = oracle.compose(S_in, E, T, ids, cu)
+    assert np.array_equal(out[0], S_in[0])  # empty list
+    out64 = oracle.compose(S_in, E.astype(np.float64), T.astype(np.float64), ids, cu)
+    assert np.array_equal(out, out64)
+    # explicit fold with numpy matmul for request 1
+    for h in range(H):
+        S = S_in[1, h].copy()
+        for i in ids:
+            S = S @ T[i, h].astype(np.float64) + E[i, h].astype(np.float64)
+        np.testing.assert_allclose(out[1, h], S, rtol=1e-13, atol=1e-15)
+
+
+def test_heads_and_segments_are_independent_units():
+    """Layout pin: unit (s,h) of a packed multi-head batch equals the same tokens run alone (catches a wrong
+    stride / index in the packed [Ttot,H,d] addressing)."""
+    rng = np.random.default_rng(13)
+    lens, H, dk, dv = [9, 17, 4], 3, 6, 5
+    k, v, g, beta = _rand_inputs(sum(lens), H, dk, dv, GATE_CHANNEL, rng)
+    E, T = oracle.segment_encode(k, v, g, beta, _cu(lens), GATE_CHANNEL)
+    cu = _cu(lens)
+    for s in range(len(lens)):
+        for h in range(H):
+            sl = slice(cu[s], cu[s + 1])
+            e1, t1 = oracle.segment_encode(k[sl, h:h + 1], v[sl, h:h + 1], g[sl, h:h + 1], beta[sl, h:h + 1],
+                                           _cu([lens[s]]), GATE_CHANNEL)
+            assert np.array_equal(e1[0, 0], E[s, h]) and np.array_equal(t1[0, 0], T[s, h])
