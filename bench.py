@@ -1,0 +1,449 @@
+#!/usr/bin/env python
+"""bench.py -- HYPIC hot path (segment encode + composition) on B200, through the C ABI of libhypic.so.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--layers L]
+
+A "step" is one pass of the whole hot path (rows a0..a6 of SURVEY.md section 8(a)) over the RAG-shaped request
+of BASELINE.json configs[2] (cfg2): for each of the `--layers` (default 36) independent linear layers, encode
+the 20 x 4096-token segments (H=32, dk=dv=128, bf16 k/v, fp32 g/beta) into (E, T), then compose the 20 segments
+per head.  cfg2 is the configuration the encode target of north_star is judged on;
+configs[1] (cfg1, 12 us of ideal work) and configs[4] (cfg4, the compose stress) are timed beside it and
+reported in the "extra" object.  Metric: tokens/s, a token being one sequence position of one layer (all H
+heads).  Inputs are synthetic and seeded (paper_2607_01299_b200/workloads.py); every layer has its own
+buffers, so one step streams 49 GB of inputs -- far larger than the 126 MB L2 -- and no flush is needed.
+
+N > 1 (torchrun): weak scaling, one request (its own seeds) per rank, no data-path collective (DESIGN.md
+"Multi-GPU"); value = tokens of all ranks / max-over-ranks time.
+
+--impl reference: the fp64 CPU oracle (oracle/), as it stands, on the host cores, on a bounded sample of the
+same workload per step (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2607_01299_b200 import workloads as wl  # noqa: E402
+
+METRIC = "cfg2 segment-encode + compose tokens/s (token = one position of one layer, all H heads)"
+UNIT = "tokens/s"
+SEG_LEN, N_SEG, H, D = 4096, 20, 32, 128
+ENC_FLOP_PER_TOKEN_HEAD = 4 * D * (D + D) + 64 * D + 64 * (D + D)  # 155,648 at d=128, C=64
+ENC_BYTES_PER_TOKEN_HEAD = 2 * D + 2 * D + 4 + 4                   # bf16 k, v + fp32 g, beta = 520 B
+COMPOSE_BYTES_PER_STEP = 4 * (D * D + D * D)                       # T_i + E_i fp32 = 131,072 B
+COMPOSE_FLOP_PER_STEP = 2 * D * D * D
+FP32_ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12              # 148 SMs x 128 FMA lanes x max clock
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return {"hbm_gbs": p["hbm_gbs"], "bf16_tflops": p["bf16_tflops"],
+                "bf16_tflops_sustained": p.get("bf16_tflops_sustained"), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.lines:
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx = float(parts[1])
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+# ------------------------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline of our arm, and the whole --impl reference arm).  The only place bench.py
+# touches oracle/.
+# ------------------------------------------------------------------------------------------------------------
+def oracle_sample_rates(units_per_core: int = 2, chains_per_core: int = 2):
+    """Time the oracle, as it stands, on a bounded sample of cfg2: `cores * units_per_core` (segment, head)
+    units of 4096 tokens for encode, and `cores * chains_per_core` (layer, head) chains of 20 steps for compose.
+    Returns token-heads/s, compose head-steps/s, cores, and a description of the sample."""
+    import numpy as np
+
+    import oracle
+
+    cores = oracle.num_threads()
+    n_units = max(1, cores * units_per_core)
+    inp = wl.make_encode_inputs([SEG_LEN] * n_units, 1, D, D, kv_dtype=torch.bfloat16, g_lo=-0.05,
+                                beta_kind="sigmoid", seed=wl.seed_for(2, 0), device="cpu")
+    kf, vf = inp.k.float().numpy(), inp.v.float().numpy()
+    t0 = time.perf_counter()
+    E, T = oracle.segment_encode(kf, vf, inp.g.numpy(), inp.beta.numpy(), inp.cu_seqlens.numpy(), gate=inp.gate)
+    t_enc = time.perf_counter() - t0
+    n_chains = max(1, cores * chains_per_core)
+    rng = np.random.default_rng(7)
+    Ep = rng.standard_normal((N_SEG, n_chains, D, D)).astype(np.float32)
+    Tp = (rng.standard_normal((N_SEG, n_chains, D, D)) * 0.05).astype(np.float32)
+    ids = np.arange(N_SEG, dtype=np.int32)
+    cu = np.array([0, N_SEG], dtype=np.int32)
+    t0 = time.perf_counter()
+    oracle.compose(None, Ep, Tp, ids, cu)
+    t_cmp = time.perf_counter() - t0
+    return {
+        "token_heads_per_s": n_units * SEG_LEN / t_enc,
+        "head_steps_per_s": n_chains * N_SEG / t_cmp,
+        "cores": cores,
+        "sample": (f"encode: {n_units} (segment, head) units x {SEG_LEN} tokens of cfg2 in {t_enc:.2f} s; compose: "
+                   f"{n_chains} head-chains x {N_SEG} steps in {t_cmp:.2f} s; combined per layer as "
+                   f"t = {N_SEG * SEG_LEN * H} token-heads / rate_enc + {N_SEG * H} head-steps / rate_cmp"),
+        "seconds": t_enc + t_cmp,
+    }
+
+
+def tokens_per_s_from_rates(r):
+    t_layer = N_SEG * SEG_LEN * H / r["token_heads_per_s"] + N_SEG * H / r["head_steps_per_s"]
+    return N_SEG * SEG_LEN / t_layer
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    for _ in range(args.warmup):
+        oracle_sample_rates(1, 1)
+    vals, secs, last = [], 0.0, None
+    for _ in range(args.steps):
+        last = oracle_sample_rates(1, 1)
+        vals.append(tokens_per_s_from_rates(last))
+        secs += last["seconds"]
+    value = sum(vals) / len(vals)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "cfg2 (BASELINE.json configs[2]): bounded per-step sample, see cpu_baseline.sample",
+                   "layers": args.layers, "segments": N_SEG, "seg_len": SEG_LEN, "H": H, "dk": D, "dv": D},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": last["cores"], "kind": "oracle",
+                         "sample": last["sample"]},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------------------
+# GPU arm
+# ------------------------------------------------------------------------------------------------------------
+class Cfg2Request:
+    """One RAG-shaped request (cfg2) resident in HBM: per-layer inputs, (E, T) pools, composed state."""
+
+    def __init__(self, hb, n_layers: int, seed_base: int, device):
+        self.hb = hb
+        self.layers = [wl.cfg2_layer(seed_base + l, device=device) for l in range(n_layers)]
+        self.E = [torch.empty((N_SEG, H, D, D), dtype=torch.float32, device=device) for _ in range(n_layers)]
+        self.T = [torch.empty((N_SEG, H, D, D), dtype=torch.float32, device=device) for _ in range(n_layers)]
+        self.S = [torch.empty((1, H, D, D), dtype=torch.float32, device=device) for _ in range(n_layers)]
+        self.ids = torch.arange(N_SEG, dtype=torch.int32, device=device)
+        self.cu = torch.tensor([0, N_SEG], dtype=torch.int32, device=device)
+        need = hb.hypic_segment_encode_workspace(N_SEG, N_SEG * SEG_LEN, H, D, D, hb.HYPIC_DT_BF16, hb.HYPIC_GATE_SCALAR)
+        self.ws = torch.empty(max(need, 16), dtype=torch.uint8, device=device)
+        self.launches = 0
+
+    def encode(self, l, inp=None):
+        x = inp if inp is not None else self.layers[l]
+        self.hb.hypic_segment_encode(x.k, x.v, x.g, x.beta, x.cu_seqlens, x.gate, E=self.E[l], T=self.T[l],
+                                     workspace=self.ws)
+        self.launches += self.hb.hypic_last_launch_count()
+
+    def compose(self, l):
+        self.hb.hypic_compose(None, self.E[l], self.T[l], self.ids, self.cu, total_steps=N_SEG, S_out=self.S[l])
+        self.launches += self.hb.hypic_last_launch_count()
+
+    def step(self, events=None):
+        for l in range(len(self.layers)):
+            if events is not None:
+                events[l][0].record()
+            self.encode(l)
+            if events is not None:
+                events[l][1].record()
+            self.compose(l)
+            if events is not None:
+                events[l][2].record()
+
+
+def time_extra_cfg1(hb, device, reps=20):
+    """cfg1 (H=16, 4 x 2048): encode + compose; 4 rotating input copies (272 MB > L2) so inputs come from HBM."""
+    copies = [wl.make_encode_inputs([2048] * 4, 16, D, D, kv_dtype=torch.bfloat16, g_lo=-0.05, beta_kind="sigmoid",
+                                    seed=wl.seed_for(1, i), device=device) for i in range(4)]
+    ids = torch.arange(4, dtype=torch.int32, device=device)
+    cu = torch.tensor([0, 4], dtype=torch.int32, device=device)
+    E = torch.empty((4, 16, D, D), dtype=torch.float32, device=device)
+    T = torch.empty_like(E)
+    S = torch.empty((1, 16, D, D), dtype=torch.float32, device=device)
+    ws = torch.empty(max(16, hb.hypic_segment_encode_workspace(4, 8192, 16, D, D, hb.HYPIC_DT_BF16, 0)),
+                     dtype=torch.uint8, device=device)
+
+    def one(i):
+        x = copies[i % 4]
+        hb.hypic_segment_encode(x.k, x.v, x.g, x.beta, x.cu_seqlens, x.gate, E=E, T=T, workspace=ws)
+        hb.hypic_compose(None, E, T, ids, cu, total_steps=4, S_out=S)
+
+    for i in range(4):
+        one(i)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(reps):
+        one(i)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    return {"workload": "cfg1: H=16, 4 x 2048, encode + compose", "ms": ms, "tokens_per_s": 8192 / (ms * 1e-3),
+            "tc_frac_of_bf16_peak": None}
+
+
+def time_extra_cfg4(hb, device, peaks, iters=48):
+    """cfg4 compose stress: pool P=1024 resident (4.3 GB, reading S7), 48 layer-iterations with their own request
+    lists (R=128, n_r ~ U{16..64}); compose only is timed."""
+    pin = wl.cfg4_pool_inputs(device=device)
+    E_tmp, T = hb.hypic_segment_encode(pin.k, pin.v, pin.g, pin.beta, pin.cu_seqlens, pin.gate)
+    del pin, E_tmp
+    E = wl.cfg4_pool_E(device=device)
+    reqs = [wl.cfg4_requests(device=device, layer=i) for i in range(iters)]
+    S_out = torch.empty_like(reqs[0].S_in)
+    for i in range(3):
+        hb.hypic_compose(reqs[i].S_in, E, T, reqs[i].seg_ids, reqs[i].cu_segs, S_out=S_out)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for rq in reqs:
+        hb.hypic_compose(rq.S_in, E, T, rq.seg_ids, rq.cu_segs, S_out=S_out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    head_steps = sum(r.n_steps for r in reqs) * H
+    gbs = head_steps * COMPOSE_BYTES_PER_STEP / (ms * 1e-3) / 1e9
+    fam = hb.hypic_compose_impl_for(H, D, D)
+    return {"workload": f"cfg4: P=1024, H=32, R=128, n~U{{16..64}}, {iters} layer-iterations, compose only",
+            "ms_total": ms, "head_steps": head_steps, "compose_ops_per_s": head_steps / (ms * 1e-3),
+            "request_layer_ops_per_s": head_steps / H / (ms * 1e-3),
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                         "frac": gbs / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"]},
+            "kernel_family": "tensor" if fam == hb.HYPIC_IMPL_TENSOR else "simt"}
+
+
+def run_ours(args):
+    from paper_2607_01299_b200 import binding as hb
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libhypic has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+    hb.load_library()
+    peaks = load_peaks()
+    L = args.layers
+
+    # weak scaling: every rank owns one full request with its own seeds (layer index offset by rank)
+    req = Cfg2Request(hb, L, seed_base=L * rank, device=device)
+    for _ in range(args.warmup):
+        req.step()
+    torch.cuda.synchronize()
+
+    events = [[[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(L)] for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    req.launches = 0
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for s in range(args.steps):
+        req.step(events[s])
+    t1.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = t0.elapsed_time(t1)
+    launches = req.launches
+    if dist is not None:
+        tt = torch.tensor([ms_total], device=device, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    ms_step = ms_total / args.steps
+    tokens_per_step = L * N_SEG * SEG_LEN * world
+    value = tokens_per_step / (ms_step * 1e-3)
+
+    # per-kernel durations measured live inside the timed region (CUDA events on the launching stream)
+    enc_ms = [ev[0].elapsed_time(ev[1]) for st in events for ev in st]
+    cmp_ms = [ev[1].elapsed_time(ev[2]) for st in events for ev in st]
+    enc_avg, cmp_avg = sum(enc_ms) / len(enc_ms), sum(cmp_ms) / len(cmp_ms)
+    th_per_launch = N_SEG * SEG_LEN * H
+    enc_family = hb.hypic_encode_impl_for(H, D, D, hb.HYPIC_DT_BF16, hb.HYPIC_GATE_SCALAR)
+    enc_tflops = th_per_launch * ENC_FLOP_PER_TOKEN_HEAD / (enc_avg * 1e-3) / 1e12
+    enc_gbs = (th_per_launch * ENC_BYTES_PER_TOKEN_HEAD + N_SEG * H * COMPOSE_BYTES_PER_STEP) / (enc_avg * 1e-3) / 1e9
+    if enc_family == hb.HYPIC_IMPL_TENSOR:
+        roofline = {"bound": "tensor", "achieved": enc_tflops, "peak": peaks["bf16_tflops_sustained"],
+                    "unit": "TFLOP/s", "frac": enc_tflops / peaks["bf16_tflops_sustained"], "traffic": None,
+                    "peak_kind": f"bf16 dense, sustained, {peaks['source']} (burst {peaks['bf16_tflops']})"}
+    else:
+        roofline = {"bound": "alu", "achieved": enc_tflops, "peak": FP32_ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
+                    "frac": enc_tflops / FP32_ALU_PEAK_TFLOPS, "traffic": None,
+                    "peak_kind": "fp32 FMA: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md)"}
+    roofline.update({"kernel": "segment encode (" + ("tensor" if enc_family == hb.HYPIC_IMPL_TENSOR else "simt") +
+                     " family)", "avg_launch_ms": enc_avg, "share_of_step": enc_avg * L / ms_step,
+                     "frac_of_bf16_burst_peak": enc_tflops / peaks["bf16_tflops"], "hbm_gbs": enc_gbs,
+                     "hbm_frac": enc_gbs / peaks["hbm_gbs"]})
+
+    if rank != 0:
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    # ---- end to end: pinned host inputs -> H2D -> C-ABI calls -> D2H of the composed state, every step
+    Le = min(L, args.e2e_layers)
+    host = []
+    for l in range(Le):
+        x = req.layers[l]
+        host.append([t.cpu().pin_memory() for t in (x.k, x.v, x.g, x.beta)])
+    stage = req.layers[0]
+    s_host = torch.empty((1, H, D, D), dtype=torch.float32).pin_memory()
+    h2d = sum(t.numel() * t.element_size() for t in host[0])
+    d2h = s_host.numel() * 4
+
+    def e2e_step():
+        for l in range(Le):
+            for dst, src in zip((stage.k, stage.v, stage.g, stage.beta), host[l]):
+                dst.copy_(src, non_blocking=True)
+            req.encode(0, stage)
+            req.compose(0)
+            s_host.copy_(req.S[0], non_blocking=True)
+        torch.cuda.synchronize()
+
+    e2e_step()
+    torch.cuda.synchronize()
+    w0 = time.perf_counter()
+    n_e2e = max(2, min(args.steps, 5))
+    for _ in range(n_e2e):
+        e2e_step()
+    e2e_s = (time.perf_counter() - w0) / n_e2e
+    e2e = {"value": Le * N_SEG * SEG_LEN / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d * Le,
+           "d2h_bytes_per_step": d2h * Le, "layers_per_step": Le,
+           "note": "pinned host k/v/g/beta -> device per layer, encode + compose via the C ABI, composed S -> host"}
+    del host
+
+    extra = {}
+    if not args.no_extra:
+        del req
+        torch.cuda.empty_cache()
+        extra["cfg1"] = time_extra_cfg1(hb, device)
+        extra["cfg4_compose"] = time_extra_cfg4(hb, device, peaks)
+        extra["cfg2_compose"] = {"avg_launch_ms": cmp_avg, "compose_ops_per_s": N_SEG * H / (cmp_avg * 1e-3),
+                                 "hbm_gbs": N_SEG * H * COMPOSE_BYTES_PER_STEP / (cmp_avg * 1e-3) / 1e9}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        r = oracle_sample_rates(2, 2)
+        cpu = {"value": tokens_per_s_from_rates(r), "unit": UNIT, "cores": r["cores"], "kind": "oracle",
+               "sample": r["sample"], "token_heads_per_s": r["token_heads_per_s"],
+               "compose_head_steps_per_s": r["head_steps_per_s"]}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic",
+        "config": {"workload": "cfg2 (BASELINE.json configs[2]): RAG-shaped request, encode all segments then compose "
+                               "per layer", "layers": L, "segments": N_SEG, "seg_len": SEG_LEN, "H": H, "dk": D,
+                   "dv": D, "kv_dtype": "bf16", "gate": "scalar", "requests_per_gpu": 1,
+                   "l2": "inputs larger than L2 (1.35 GB per layer, own buffers per layer); no flush needed",
+                   "token_heads_per_s": value * H},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+        "extra": extra,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--layers", type=int, default=36, help="linear layers of the cfg2 request (36 = as written)")
+    ap.add_argument("--e2e-layers", type=int, default=4, help="layers per end-to-end step (bounds pinned host memory)")
+    ap.add_argument("--no-extra", action="store_true", help="skip the cfg1 / cfg4 side measurements")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,136 @@
+/*
+ * hypic.h -- C ABI of libhypic.so: the linear-attention hot path of HYPIC (arxiv/paper_2607_01299, C1)
+ * on one NVIDIA B200 (sm_100a).
+ *
+ * Conventions (row convention of BASELINE.json:north_star; the paper writes the transpose, PAPER.md:80-90,
+ * DESIGN.md reading A1).  Per attention head:
+ *     state S in R^{dv x dk};  token step  S <- S diag(alpha_t);  S <- S + beta_t (v_t - S k_t) k_t^T,
+ *     alpha_t = exp(g_t)   (Eq. 2 with Table 1's dense family)
+ *     T_C = prod_{t in C} diag(alpha_t)(I - beta_t k_t k_t^T), first token leftmost
+ *     E_C = S after the tokens of C, started from S = 0                  ("S_{C|0}")
+ *     compose: S <- S T_i + E_i over a request's ordered segment list     (Eq. 4, 182 Eq. 6)
+ *
+ * General rules for every entry point:
+ *   - Every pointer is a DEVICE pointer unless its comment says HOST.  The caller owns every buffer; the
+ *     library allocates nothing, keeps no state between calls and never synchronises the host.  Work is
+ *     enqueued on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *   - All tensors are dense, row-major, innermost dimension last; pointers must be 16-byte aligned.
+ *   - Return value: a hypic_status_t as int.  No exceptions, no abort, nothing printed.  Host-visible
+ *     arguments are validated BEFORE any CUDA call (so validation errors are returned on a box with no GPU).
+ *     Device-side contents (cu_seqlens, seg_ids, cu_segs) are trusted.  Asynchronous device faults surface
+ *     at the caller's next synchronisation, as with any kernel launch.
+ *   - There is no CPU fallback: without a usable sm_100 device the compute calls return HYPIC_ERR_CUDA.
+ */
+#ifndef HYPIC_H_
+#define HYPIC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HYPIC_VERSION 100 /* 0.1.0 */
+
+typedef enum {
+  HYPIC_OK = 0,
+  HYPIC_ERR_INVALID_ARG = 1, /* null / negative / inconsistent host-visible argument */
+  HYPIC_ERR_UNSUPPORTED = 2, /* shape or dtype outside the built envelope (see each call) */
+  HYPIC_ERR_WORKSPACE = 3,   /* workspace NULL or smaller than *_workspace() says */
+  HYPIC_ERR_CUDA = 4         /* a CUDA runtime/driver call failed (no device, launch error, ...) */
+} hypic_status_t;
+
+typedef enum { HYPIC_DT_F32 = 0, HYPIC_DT_BF16 = 1 } hypic_dtype_t;          /* dtype of k and v */
+typedef enum { HYPIC_GATE_SCALAR = 0, HYPIC_GATE_CHANNEL = 1 } hypic_gate_t; /* g:[Ttot,H] or [Ttot,H,dk] */
+
+/* Kernel families behind the two operations.  AUTO picks the fastest one built for the shape. */
+typedef enum {
+  HYPIC_IMPL_AUTO = 0,
+  HYPIC_IMPL_SIMT = 1,   /* fp32 CUDA-core kernels: token-by-token scan / FFMA compose; any dk in {64,128} */
+  HYPIC_IMPL_TENSOR = 2  /* tcgen05/TMEM kernels (dk = dv = 128) */
+} hypic_impl_t;
+
+/*
+ * hypic_set_impl / hypic_get_impl: process-wide selection of the kernel family (default AUTO).  A forced
+ * family that does not cover a call's shape makes that call return HYPIC_ERR_UNSUPPORTED.  This is the only
+ * global the library keeps; it exists so that tests can check every kernel family against the oracle.
+ */
+int hypic_set_impl(int impl);
+int hypic_get_impl(void);
+
+/*
+ * hypic_segment_encode_workspace: bytes of device scratch hypic_segment_encode needs for these arguments
+ * (0 is possible).  Returns 0 for arguments the encode call would reject.  Pure host arithmetic.
+ */
+size_t hypic_segment_encode_workspace(int32_t n_seg, int32_t t_total, int32_t H, int32_t dk, int32_t dv,
+                                      int kv_dtype, int gate);
+
+/*
+ * hypic_segment_encode: for every segment s (tokens [cu_seqlens[s], cu_seqlens[s+1])) and head h, the
+ * zero-start end-state E[s,h] = S_{C|0} (dv x dk) and the segment-cumulative transition
+ * T[s,h] = T_C (dk x dk; Eq. 4), both from one pass over the segment's tokens.
+ *
+ *   k        [t_total, H, dk]   kv_dtype (bf16 or fp32), packed by cu_seqlens
+ *   v        [t_total, H, dv]   kv_dtype
+ *   g        [t_total, H] (HYPIC_GATE_SCALAR, GDN) or [t_total, H, dk] (HYPIC_GATE_CHANNEL, KDA), fp32
+ *            log-decay: alpha = exp(g) (Table 1; reading A2)
+ *   beta     [t_total, H] fp32
+ *   cu_seqlens  int32 [n_seg+1] on the DEVICE, cu[0] = 0, non-decreasing, cu[n_seg] = t_total (trusted)
+ *   E        out [n_seg, H, dv, dk] fp32       T   out [n_seg, H, dk, dk] fp32
+ *   workspace / workspace_bytes: device scratch of at least hypic_segment_encode_workspace(...) bytes
+ *            (may be NULL when that is 0).  Contents are undefined before and after the call.
+ *
+ * A zero-length segment yields E = 0, T = I.  n_seg = 0 or t_total = 0 with n_seg > 0 are valid.
+ * Built envelope: dk in {64, 128}; dv in [1, 1024] for the SIMT family, dv = dk = 128 for the tensor family;
+ * H, n_seg, lengths arbitrary.  Inputs are only read; E and T are fully overwritten.
+ */
+int hypic_segment_encode(const void* k, const void* v, const float* g, const float* beta,
+                         const int32_t* cu_seqlens, int32_t n_seg, int32_t t_total, int32_t H, int32_t dk,
+                         int32_t dv, int kv_dtype, int gate, float* E, float* T, void* workspace,
+                         size_t workspace_bytes, void* stream);
+
+/*
+ * hypic_compose: for every request r and head h, fold  S <- S T_i + E_i  (Eq. 6, evaluated as
+ * the chain of Eq. 4 steps it abbreviates) over the request's ordered list of pool ids
+ * seg_ids[cu_segs[r] .. cu_segs[r+1]) starting from S_in[r,h].  Composition is not commutative: the order
+ * is the list order.  An empty list copies S_in (or writes zeros).
+ *
+ *   S_in     [R, H, dv, dk] fp32, or NULL (= zeros)
+ *   E_pool   [P, H, dv, dk] fp32        T_pool  [P, H, dk, dk] fp32  (exactly the E/T layout of encode)
+ *   seg_ids  int32 [cu_segs[R]] on the DEVICE, values in [0, P) (trusted)
+ *   cu_segs  int32 [R+1] on the DEVICE, cu_segs[0] = 0, non-decreasing (trusted)
+ *   total_steps  HOST value of cu_segs[R] (>= 0); used only to size the launch / skip empty work
+ *   S_out    out [R, H, dv, dk] fp32; may alias S_in exactly (same pointer), no partial overlap
+ *
+ * Built envelope: dk in {64, 128}, dv in [1, 1024] (SIMT family); dv = dk = 128 (tensor family).
+ */
+int hypic_compose(const float* S_in, const float* E_pool, const float* T_pool, const int32_t* seg_ids,
+                  const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
+                  int32_t dv, float* S_out, void* stream);
+
+/*
+ * hypic_encode_impl_for / hypic_compose_impl_for: which kernel family (HYPIC_IMPL_SIMT or HYPIC_IMPL_TENSOR)
+ * a call with this shape would run under the current hypic_set_impl setting, or a negative hypic_status_t
+ * (-HYPIC_ERR_UNSUPPORTED / -HYPIC_ERR_INVALID_ARG) if the call would be rejected.  Pure host arithmetic;
+ * bench.py uses it to name the roofline that bounds the kernel it timed.
+ */
+int hypic_encode_impl_for(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate);
+int hypic_compose_impl_for(int32_t H, int32_t dk, int32_t dv);
+
+/* hypic_status_string: static, NUL-terminated description of a status code (never NULL). */
+const char* hypic_status_string(int status);
+
+/* hypic_version: HYPIC_VERSION of the built library. */
+int hypic_version(void);
+
+/*
+ * hypic_last_launch_count: number of kernel launches the most recent compute call on this thread enqueued
+ * (bench.py reports it as gpu_launches).  Pure host bookkeeping.
+ */
+int hypic_last_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HYPIC_H_ */

@@ -1,0 +1,213 @@
+"""Thin Python binding of libhypic.so (include/hypic.h): argument marshalling only.
+
+Same names as the C ABI.  Every step of the path runs in the CUDA kernels behind the library; torch is used
+for device memory and streams.  There is NO CPU fallback: if the shared library is missing or a tensor is not
+on a CUDA device, the call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Tuple
+
+import torch
+
+HYPIC_OK = 0
+HYPIC_ERR_INVALID_ARG = 1
+HYPIC_ERR_UNSUPPORTED = 2
+HYPIC_ERR_WORKSPACE = 3
+HYPIC_ERR_CUDA = 4
+HYPIC_DT_F32 = 0
+HYPIC_DT_BF16 = 1
+HYPIC_GATE_SCALAR = 0
+HYPIC_GATE_CHANNEL = 1
+HYPIC_IMPL_AUTO = 0
+HYPIC_IMPL_SIMT = 1
+HYPIC_IMPL_TENSOR = 2
+
+EXPORTS = (
+    "hypic_set_impl", "hypic_get_impl", "hypic_segment_encode_workspace", "hypic_segment_encode", "hypic_compose",
+    "hypic_status_string", "hypic_version", "hypic_last_launch_count", "hypic_encode_impl_for",
+    "hypic_compose_impl_for",
+)
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhypic.so")
+_lib = None
+
+
+class HypicError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = int(status)
+        super().__init__(f"{where} failed: status {status} ({hypic_status_string(status)})")
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libhypic.so (built by ``python -m paper_2607_01299_b200.build``) and declare the prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2607_01299_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    i32, vp, sz = ctypes.c_int32, ctypes.c_void_p, ctypes.c_size_t
+    lib.hypic_set_impl.argtypes = [ctypes.c_int]
+    lib.hypic_set_impl.restype = ctypes.c_int
+    lib.hypic_get_impl.argtypes = []
+    lib.hypic_get_impl.restype = ctypes.c_int
+    lib.hypic_segment_encode_workspace.argtypes = [i32, i32, i32, i32, i32, ctypes.c_int, ctypes.c_int]
+    lib.hypic_segment_encode_workspace.restype = sz
+    lib.hypic_segment_encode.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, ctypes.c_int, ctypes.c_int, vp,
+                                         vp, vp, sz, vp]
+    lib.hypic_segment_encode.restype = ctypes.c_int
+    lib.hypic_compose.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp, vp]
+    lib.hypic_compose.restype = ctypes.c_int
+    lib.hypic_status_string.argtypes = [ctypes.c_int]
+    lib.hypic_status_string.restype = ctypes.c_char_p
+    lib.hypic_version.argtypes = []
+    lib.hypic_version.restype = ctypes.c_int
+    lib.hypic_last_launch_count.argtypes = []
+    lib.hypic_last_launch_count.restype = ctypes.c_int
+    lib.hypic_encode_impl_for.argtypes = [i32, i32, i32, ctypes.c_int, ctypes.c_int]
+    lib.hypic_encode_impl_for.restype = ctypes.c_int
+    lib.hypic_compose_impl_for.argtypes = [i32, i32, i32]
+    lib.hypic_compose_impl_for.restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def hypic_status_string(status: int) -> str:
+    return load_library().hypic_status_string(int(status)).decode()
+
+
+def hypic_version() -> int:
+    return int(load_library().hypic_version())
+
+
+def hypic_set_impl(impl: int) -> None:
+    rc = load_library().hypic_set_impl(int(impl))
+    if rc != HYPIC_OK:
+        raise HypicError(rc, "hypic_set_impl")
+
+
+def hypic_get_impl() -> int:
+    return int(load_library().hypic_get_impl())
+
+
+def hypic_encode_impl_for(H: int, dk: int, dv: int, kv_dtype: int, gate: int) -> int:
+    return int(load_library().hypic_encode_impl_for(H, dk, dv, kv_dtype, gate))
+
+
+def hypic_compose_impl_for(H: int, dk: int, dv: int) -> int:
+    return int(load_library().hypic_compose_impl_for(H, dk, dv))
+
+
+def hypic_last_launch_count() -> int:
+    return int(load_library().hypic_last_launch_count())
+
+
+def _dev_ptr(t: Optional[torch.Tensor], name: str, dtype=None) -> Optional[int]:
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"{name} must be {dtype}, got {t.dtype}")
+    return t.data_ptr() if t.numel() > 0 else None
+
+
+def _stream_handle(stream: Optional[torch.cuda.Stream]) -> int:
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def hypic_segment_encode_workspace(n_seg: int, t_total: int, H: int, dk: int, dv: int, kv_dtype: int,
+                                   gate: int) -> int:
+    return int(load_library().hypic_segment_encode_workspace(n_seg, t_total, H, dk, dv, kv_dtype, gate))
+
+
+def hypic_segment_encode(k: torch.Tensor, v: torch.Tensor, g: torch.Tensor, beta: torch.Tensor,
+                         cu_seqlens: torch.Tensor, gate: int = HYPIC_GATE_SCALAR, *,
+                         E: Optional[torch.Tensor] = None, T: Optional[torch.Tensor] = None,
+                         workspace: Optional[torch.Tensor] = None,
+                         stream: Optional[torch.cuda.Stream] = None) -> Tuple[torch.Tensor, torch.Tensor]:
+    """E:[n_seg,H,dv,dk], T:[n_seg,H,dk,dk] fp32 for packed k:[Ttot,H,dk], v:[Ttot,H,dv] (bf16 or fp32),
+    g:[Ttot,H] or [Ttot,H,dk] fp32, beta:[Ttot,H] fp32, cu_seqlens:int32[n_seg+1] (device)."""
+    lib = load_library()
+    for name, t in (("k", k), ("v", v), ("g", g), ("beta", beta), ("cu_seqlens", cu_seqlens)):
+        if not t.is_cuda:
+            raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if k.dim() != 3 or v.dim() != 3 or k.shape[:2] != v.shape[:2] or k.dtype != v.dtype:
+        raise ValueError("k:[Ttot,H,dk] and v:[Ttot,H,dv] must agree in Ttot, H and dtype")
+    t_total, H, dk = (int(x) for x in k.shape)
+    dv = int(v.shape[2])
+    if k.dtype == torch.bfloat16:
+        kv_dtype = HYPIC_DT_BF16
+    elif k.dtype == torch.float32:
+        kv_dtype = HYPIC_DT_F32
+    else:
+        raise ValueError(f"k/v must be bf16 or fp32, got {k.dtype}")
+    want_g = (t_total, H) if gate == HYPIC_GATE_SCALAR else (t_total, H, dk)
+    if tuple(g.shape) != want_g or tuple(beta.shape) != (t_total, H):
+        raise ValueError(f"g must be {want_g} and beta {(t_total, H)}; got {tuple(g.shape)}, {tuple(beta.shape)}")
+    n_seg = int(cu_seqlens.numel()) - 1
+    if n_seg < 0:
+        raise ValueError("cu_seqlens must have n_seg+1 >= 1 entries")
+    dev = k.device
+    if E is None:
+        E = torch.empty((n_seg, H, dv, dk), dtype=torch.float32, device=dev)
+    if T is None:
+        T = torch.empty((n_seg, H, dk, dk), dtype=torch.float32, device=dev)
+    if tuple(E.shape) != (n_seg, H, dv, dk) or tuple(T.shape) != (n_seg, H, dk, dk):
+        raise ValueError("E / T have the wrong shape")
+    need = int(lib.hypic_segment_encode_workspace(n_seg, t_total, H, dk, dv, kv_dtype, gate))
+    if need > 0 and (workspace is None or workspace.numel() * workspace.element_size() < need):
+        workspace = torch.empty(need, dtype=torch.uint8, device=dev)
+    ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    with torch.cuda.device(dev):
+        rc = lib.hypic_segment_encode(
+            _dev_ptr(k, "k"), _dev_ptr(v, "v"), _dev_ptr(g, "g", torch.float32), _dev_ptr(beta, "beta", torch.float32),
+            _dev_ptr(cu_seqlens, "cu_seqlens", torch.int32), n_seg, t_total, H, dk, dv, kv_dtype, int(gate),
+            _dev_ptr(E, "E", torch.float32), _dev_ptr(T, "T", torch.float32), _dev_ptr(workspace, "workspace"),
+            ws_bytes, _stream_handle(stream))
+    if rc != HYPIC_OK:
+        raise HypicError(rc, "hypic_segment_encode")
+    return E, T
+
+
+def hypic_compose(S_in: Optional[torch.Tensor], E_pool: torch.Tensor, T_pool: torch.Tensor, seg_ids: torch.Tensor,
+                  cu_segs: torch.Tensor, *, total_steps: Optional[int] = None, S_out: Optional[torch.Tensor] = None,
+                  stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """S_out[r,h] = fold of S <- S T_i + E_i over seg_ids[cu_segs[r]:cu_segs[r+1]] from S_in[r,h] (None = 0)."""
+    lib = load_library()
+    for name, t in (("E_pool", E_pool), ("T_pool", T_pool), ("seg_ids", seg_ids), ("cu_segs", cu_segs)):
+        if not t.is_cuda:
+            raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if E_pool.dim() != 4 or T_pool.dim() != 4:
+        raise ValueError("E_pool:[P,H,dv,dk], T_pool:[P,H,dk,dk]")
+    P, H, dv, dk = (int(x) for x in E_pool.shape)
+    if tuple(T_pool.shape) != (P, H, dk, dk):
+        raise ValueError("T_pool must be [P,H,dk,dk]")
+    R = int(cu_segs.numel()) - 1
+    if R < 0:
+        raise ValueError("cu_segs must have R+1 >= 1 entries")
+    if total_steps is None:
+        total_steps = int(seg_ids.numel())  # shape metadata, no device sync
+    if S_in is not None and tuple(S_in.shape) != (R, H, dv, dk):
+        raise ValueError("S_in must be [R,H,dv,dk]")
+    if S_out is None:
+        S_out = torch.empty((R, H, dv, dk), dtype=torch.float32, device=E_pool.device)
+    if tuple(S_out.shape) != (R, H, dv, dk):
+        raise ValueError("S_out must be [R,H,dv,dk]")
+    with torch.cuda.device(E_pool.device):
+        rc = lib.hypic_compose(
+            _dev_ptr(S_in, "S_in", torch.float32), _dev_ptr(E_pool, "E_pool", torch.float32),
+            _dev_ptr(T_pool, "T_pool", torch.float32), _dev_ptr(seg_ids, "seg_ids", torch.int32),
+            _dev_ptr(cu_segs, "cu_segs", torch.int32), R, P, int(total_steps), H, dk, dv,
+            _dev_ptr(S_out, "S_out", torch.float32), _stream_handle(stream))
+    if rc != HYPIC_OK:
+        raise HypicError(rc, "hypic_compose")
+    return S_out

@@ -1,0 +1,71 @@
+// common.cuh -- shared host/device helpers of libhypic (product code; nothing here is used by oracle/).
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/hypic.h"
+
+namespace hypic {
+
+// Launch bookkeeping behind hypic_last_launch_count().
+extern thread_local int g_launch_count;
+inline void note_launch(int n = 1) { g_launch_count += n; }
+
+#define HYPIC_CUDA_OK(expr)                        \
+  do {                                             \
+    cudaError_t _e = (expr);                       \
+    if (_e != cudaSuccess) return HYPIC_ERR_CUDA;  \
+  } while (0)
+
+struct EncodeArgs {
+  const void* k;
+  const void* v;
+  const float* g;
+  const float* beta;
+  const int32_t* cu_seqlens;
+  int32_t n_seg, t_total, H, dk, dv;
+  int kv_dtype, gate;
+  float* E;
+  float* T;
+  void* workspace;
+  size_t workspace_bytes;
+  cudaStream_t stream;
+};
+
+struct ComposeArgs {
+  const float* S_in;
+  const float* E_pool;
+  const float* T_pool;
+  const int32_t* seg_ids;
+  const int32_t* cu_segs;
+  int32_t R, P, total_steps, H, dk, dv;
+  float* S_out;
+  cudaStream_t stream;
+};
+
+// Kernel families (each returns a hypic_status_t; UNSUPPORTED when the shape is outside its envelope).
+int encode_simt(const EncodeArgs& a);
+int compose_simt(const ComposeArgs& a);
+bool encode_tensor_shape_ok(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate);
+inline bool encode_tensor_supported(const EncodeArgs& a) {
+  return encode_tensor_shape_ok(a.H, a.dk, a.dv, a.kv_dtype, a.gate);
+}
+size_t encode_tensor_workspace(int32_t n_seg, int32_t t_total, int32_t H, int32_t dk, int32_t dv, int kv_dtype,
+                               int gate);
+int encode_tensor(const EncodeArgs& a);
+bool compose_tensor_shape_ok(int32_t H, int32_t dk, int32_t dv);
+inline bool compose_tensor_supported(const ComposeArgs& a) { return compose_tensor_shape_ok(a.H, a.dk, a.dv); }
+int compose_tensor(const ComposeArgs& a);
+
+// Device properties cached per process (SM count, opt-in shared memory).
+struct DeviceInfo {
+  int ok;  // 0 = not queried / failed
+  int device;
+  int sm_count;
+  int cc_major, cc_minor;
+  int max_smem_optin;
+};
+const DeviceInfo& device_info();
+
+}  // namespace hypic

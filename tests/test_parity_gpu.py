@@ -1,0 +1,273 @@
+"""GPU parity: libhypic (through the C ABI via the thin binding) vs the fp64 oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json:north_star's (parity_util.TOL_*).  Every kernel family is
+checked (AUTO = what bench.py times, SIMT, TENSOR); a family that does not cover a shape is skipped."""
+import contextlib
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2607_01299_b200 import binding as hb
+from paper_2607_01299_b200 import workloads as wl
+from parity_util import (TOL_BF16, TOL_F32, check_E, check_T, oracle_compose_units, oracle_encode,
+                         oracle_encode_units)
+
+pytestmark = pytest.mark.gpu
+
+IMPLS = [("auto", hb.HYPIC_IMPL_AUTO), ("simt", hb.HYPIC_IMPL_SIMT), ("tensor", hb.HYPIC_IMPL_TENSOR)]
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_cuda():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    hb.load_library()  # fail loudly if the extension is missing
+    yield
+    hb.hypic_set_impl(hb.HYPIC_IMPL_AUTO)
+
+
+@contextlib.contextmanager
+def impl_family(impl):
+    hb.hypic_set_impl(impl)
+    try:
+        yield
+    except hb.HypicError as e:
+        if e.status == hb.HYPIC_ERR_UNSUPPORTED and impl == hb.HYPIC_IMPL_TENSOR:
+            pytest.skip("tensor family does not cover this shape")
+        raise
+    finally:
+        hb.hypic_set_impl(hb.HYPIC_IMPL_AUTO)
+
+
+def gpu_encode(inp, impl):
+    with impl_family(impl):
+        E, T = hb.hypic_segment_encode(inp.k, inp.v, inp.g, inp.beta, inp.cu_seqlens, inp.gate)
+        torch.cuda.synchronize()
+    return E, T
+
+
+def gpu_compose(S_in, E, T, ids, cu, impl, **kw):
+    with impl_family(impl):
+        out = hb.hypic_compose(S_in, E, T, ids, cu, **kw)
+        torch.cuda.synchronize()
+    return out
+
+
+# ------------------------------------------------------------------------------------------------ cfg0
+@pytest.mark.parametrize("name,impl", IMPLS)
+def test_cfg0_fp32_encode_and_compose_vs_sequential(name, impl):
+    """cfg0: 1 head, d=64, fp32, 2 x 128 tokens; E,T per segment; compose from 0 and from N(0,0.1) must equal
+    the sequential recurrence over all 256 tokens (Eq. 4)."""
+    inp = wl.cfg0("cuda")
+    E, T = gpu_encode(inp, impl)
+    E_ref, T_ref = oracle_encode(inp)
+    check_E(E, E_ref, TOL_F32)
+    check_T(T, T_ref, TOL_F32)
+    s_in = wl.cfg0_s_in("cuda")
+    ids = torch.tensor([0, 1, 0, 1], dtype=torch.int32, device="cuda")
+    cu = torch.tensor([0, 2, 4], dtype=torch.int32, device="cuda")
+    S_in = torch.cat([torch.zeros_like(s_in), s_in], 0)
+    S = gpu_compose(S_in, E, T, ids, cu, impl)
+    c = inp.cpu()
+    seq = oracle.sequential(S_in.cpu().numpy().astype(np.float64), torch.cat([c.k, c.k]), torch.cat([c.v, c.v]),
+                            torch.cat([c.g, c.g]), torch.cat([c.beta, c.beta]),
+                            np.array([0, 256, 512], dtype=np.int32), gate=c.gate)
+    check_E(S, seq, TOL_F32, "S_out vs sequential")
+    # S_in = NULL is the same as zeros
+    S0 = gpu_compose(None, E, T, ids[:2].contiguous(), cu[:2].contiguous(), impl)
+    check_E(S0, seq[:1], TOL_F32, "S_out (S_in=NULL) vs sequential")
+
+
+# ------------------------------------------------------------------------- ragged / edge-case encodes
+RAGGED = [200, 64, 65, 1, 0, 63, 333, 128, 0, 2]
+
+
+@pytest.mark.parametrize("name,impl", IMPLS)
+@pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
+@pytest.mark.parametrize("kv,d,tol", [(torch.bfloat16, 128, TOL_BF16), (torch.float32, 128, TOL_F32),
+                                      (torch.float32, 64, TOL_F32), (torch.bfloat16, 64, TOL_BF16)])
+def test_encode_ragged_segments(name, impl, gate, kv, d, tol):
+    """Lengths spanning several 64-token chunks with ragged tails, plus length 0 / 1 / 63 / 64 / 65."""
+    inp = wl.make_encode_inputs(RAGGED, 3, d, d, kv_dtype=kv, gate=gate, g_lo=-0.05, seed=wl.seed_for(1, 11),
+                                device="cuda")
+    E, T = gpu_encode(inp, impl)
+    E_ref, T_ref = oracle_encode(inp)
+    check_E(E, E_ref, tol)
+    check_T(T, T_ref, tol)
+    # empty segments: E = 0, T = I exactly
+    for s, L in enumerate(RAGGED):
+        if L == 0:
+            assert torch.count_nonzero(E[s]) == 0
+            assert torch.equal(T[s], torch.eye(d, device="cuda").expand_as(T[s]))
+
+
+@pytest.mark.parametrize("name,impl", IMPLS)
+def test_encode_dv_not_equal_dk(name, impl):
+    inp = wl.make_encode_inputs([70, 129], 2, 64, 96, kv_dtype=torch.float32, seed=wl.seed_for(0, 3), device="cuda")
+    E, T = gpu_encode(inp, impl)
+    E_ref, T_ref = oracle_encode(inp)
+    check_E(E, E_ref, TOL_F32)
+    check_T(T, T_ref, TOL_F32)
+
+
+@pytest.mark.parametrize("name,impl", IMPLS)
+def test_encode_degenerate_inputs(name, impl):
+    """beta = 0 => T = (prod alpha) I, E = 0; n_seg = 0; all segments empty."""
+    inp = wl.make_encode_inputs([130, 64], 2, 128, 128, kv_dtype=torch.bfloat16, seed=5, device="cuda")
+    inp.beta.zero_()
+    E, T = gpu_encode(inp, impl)
+    assert torch.count_nonzero(E) == 0
+    g = inp.g.double().cpu()
+    for s, (a, b) in enumerate([(0, 130), (130, 194)]):
+        for h in range(2):
+            want = torch.exp(g[a:b, h].sum()) * torch.eye(128, dtype=torch.float64)
+            assert torch.allclose(T[s, h].double().cpu(), want, rtol=2e-5, atol=0)
+    empty = wl.make_encode_inputs([], 2, 128, 128, kv_dtype=torch.bfloat16, seed=5, device="cuda")
+    E0, T0 = gpu_encode(empty, impl)
+    assert E0.shape == (0, 2, 128, 128) and T0.shape == (0, 2, 128, 128)
+    zeros = wl.make_encode_inputs([0, 0], 2, 128, 128, kv_dtype=torch.bfloat16, seed=5, device="cuda")
+    E1, T1 = gpu_encode(zeros, impl)
+    assert torch.count_nonzero(E1) == 0 and torch.equal(T1, torch.eye(128, device="cuda").expand_as(T1))
+
+
+# ------------------------------------------------------------------------------------------ compose
+@pytest.mark.parametrize("name,impl", IMPLS)
+@pytest.mark.parametrize("d", [128, 64])
+def test_compose_near_unit_pool(name, impl, d):
+    """Reading S9: pool with ||T||_F = O(1..10) (short segments, weak decay), so S.T is not negligible; fp32
+    pools vs fp64 compose of the same pools -> 1e-5.  Lists of length 0, 1 and up to 40; unsorted ids."""
+    P, H = 24, 3
+    pin = wl.near_unit_pool_inputs(P, H, device="cuda", d=d, kv_dtype=torch.float32)
+    hb.hypic_set_impl(hb.HYPIC_IMPL_SIMT)
+    E, T = hb.hypic_segment_encode(pin.k, pin.v, pin.g, pin.beta, pin.cu_seqlens, pin.gate)
+    hb.hypic_set_impl(hb.HYPIC_IMPL_AUTO)
+    assert float(T.norm(dim=(-1, -2)).min()) > 0.5
+    req = wl.make_compose_requests(9, P, H, d, d, n_lo=0, n_hi=24, seed=77, device="cuda", s_in_std=1.0)
+    # force an empty list and a singleton
+    cu = req.cu_segs.cpu().clone()
+    S = gpu_compose(req.S_in, E, T, req.seg_ids, req.cu_segs, impl)
+    ref = oracle.compose(req.S_in.cpu().numpy(), E.cpu().numpy(), T.cpu().numpy(), req.seg_ids.cpu().numpy(),
+                         cu.numpy())
+    check_E(S, ref, TOL_F32, "S_out")
+    # long chain that repeats ids (40 steps)
+    gen = torch.Generator().manual_seed(123)
+    ids = torch.randint(0, P, (40,), generator=gen, dtype=torch.int32).cuda()
+    cu2 = torch.tensor([0, 0, 1, 40], dtype=torch.int32, device="cuda")  # empty, singleton, 39-long
+    S_in2 = torch.randn(3, H, d, d, device="cuda")
+    S2 = gpu_compose(S_in2, E, T, ids, cu2, impl)
+    ref2 = oracle.compose(S_in2.cpu().numpy(), E.cpu().numpy(), T.cpu().numpy(), ids.cpu().numpy(),
+                          cu2.cpu().numpy())
+    check_E(S2, ref2, TOL_F32, "S_out (chain)")
+    assert torch.equal(S2[0], S_in2[0])  # empty list copies S_in
+    # in-place: S_out aliases S_in
+    S3 = S_in2.clone()
+    gpu_compose(S3, E, T, ids, cu2, impl, S_out=S3)
+    assert torch.equal(S3, S2)
+    # S_in = NULL
+    S4 = gpu_compose(None, E, T, ids, cu2, impl)
+    ref4 = oracle.compose(None, E.cpu().numpy(), T.cpu().numpy(), ids.cpu().numpy(), cu2.cpu().numpy())
+    check_E(S4, ref4, TOL_F32, "S_out (NULL S_in)")
+    assert torch.count_nonzero(S4[0]) == 0
+
+
+@pytest.mark.parametrize("name,impl", IMPLS)
+def test_compose_order_matters(name, impl):
+    pin = wl.near_unit_pool_inputs(4, 1, device="cuda", d=128, kv_dtype=torch.float32, seed_off=3)
+    hb.hypic_set_impl(hb.HYPIC_IMPL_SIMT)
+    E, T = hb.hypic_segment_encode(pin.k, pin.v, pin.g, pin.beta, pin.cu_seqlens, pin.gate)
+    hb.hypic_set_impl(hb.HYPIC_IMPL_AUTO)
+    ids = torch.tensor([0, 1, 2, 3, 3, 2, 1, 0], dtype=torch.int32, device="cuda")
+    cu = torch.tensor([0, 4, 8], dtype=torch.int32, device="cuda")
+    S = gpu_compose(None, E, T, ids, cu, impl)
+    ref = oracle.compose(None, E.cpu().numpy(), T.cpu().numpy(), ids.cpu().numpy(), cu.cpu().numpy())
+    check_E(S, ref, TOL_F32)
+    assert oracle.rel_fro(S[0].cpu().numpy(), ref[1]) > 1e-2  # the two orders really differ
+
+
+# ------------------------------------------------------------- end to end at bf16: encode -> compose
+@pytest.mark.parametrize("name,impl", IMPLS)
+def test_cfg1_small_end_to_end_vs_sequential(name, impl):
+    """cfg1 scaled down (H=4, 4 x 320 tokens): GPU encode (bf16) -> GPU compose vs the fp64 sequential
+    recurrence over the concatenation -> 3e-3 (reading S8)."""
+    inp = wl.cfg1("cuda", seg_len=320, n_seg=4, H=4)
+    E, T = gpu_encode(inp, impl)
+    E_ref, T_ref = oracle_encode(inp)
+    check_E(E, E_ref, TOL_BF16)
+    check_T(T, T_ref, TOL_BF16)
+    ids = torch.arange(4, dtype=torch.int32, device="cuda")
+    cu = torch.tensor([0, 4], dtype=torch.int32, device="cuda")
+    S = gpu_compose(None, E, T, ids, cu, impl)
+    c = inp.cpu()
+    seq = oracle.sequential(None, c.k, c.v, c.g, c.beta, np.array([0, 1280], dtype=np.int32), gate=c.gate)
+    check_E(S, seq, TOL_BF16, "S_out vs sequential")
+
+
+# ------------------------------------------- full sizes, bench.py's launch configuration (AUTO family)
+def _sample_units(n_a, n_b, n, seed):
+    gen = np.random.default_rng(seed)
+    return sorted({(int(gen.integers(n_a)), int(gen.integers(n_b))) for _ in range(n)})
+
+
+def test_cfg1_full_size():
+    """cfg1 as written (H=16, 4 x 2048, bf16): every unit against the oracle, then compose the 4 in order."""
+    inp = wl.cfg1("cuda")
+    E, T = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
+    E_ref, T_ref = oracle_encode(inp)
+    check_E(E, E_ref, TOL_BF16)
+    check_T(T, T_ref, TOL_BF16)
+    ids = torch.arange(4, dtype=torch.int32, device="cuda")
+    cu = torch.tensor([0, 4], dtype=torch.int32, device="cuda")
+    S = gpu_compose(None, E, T, ids, cu, hb.HYPIC_IMPL_AUTO)
+    ref = oracle.compose(None, E.cpu().numpy(), T.cpu().numpy(), ids.cpu().numpy(), cu.cpu().numpy())
+    check_E(S, ref, TOL_F32, "S_out vs fp64 compose of the same pools")
+    ref_e2e = oracle.compose(None, E_ref, T_ref, ids.cpu().numpy(), cu.cpu().numpy())
+    check_E(S, ref_e2e, TOL_BF16, "S_out end to end")
+
+
+def test_cfg2_one_layer_sampled_units():
+    """cfg2, one of the 36 layers at full size (20 x 4096, H=32): sampled (segment, head) units one by one."""
+    inp = wl.cfg2_layer(0, "cuda")
+    E, T = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
+    units = _sample_units(20, 32, 6, 2)
+    E_ref, T_ref = oracle_encode_units(inp, units)
+    sel_s = torch.tensor([u[0] for u in units]), torch.tensor([u[1] for u in units])
+    check_E(E[sel_s[0], sel_s[1]][:, None], E_ref, TOL_BF16)
+    check_T(T[sel_s[0], sel_s[1]][:, None], T_ref, TOL_BF16)  # 4096 tokens: T underflows -> absolute criterion
+    assert torch.isfinite(E).all() and torch.isfinite(T).all()
+    # compose the 20 segments per head, sampled heads, vs fp64 compose of the same fp32 pools
+    ids = torch.arange(20, dtype=torch.int32, device="cuda")
+    cu = torch.tensor([0, 20], dtype=torch.int32, device="cuda")
+    S = gpu_compose(None, E, T, ids, cu, hb.HYPIC_IMPL_AUTO)
+    heads = [(0, h) for h in (0, 13, 31)]
+    ref = oracle_compose_units(None, E, T, ids, cu, heads)
+    check_E(S[0, [0, 13, 31]][:, None], ref, TOL_F32, "S_out")
+
+
+def test_cfg3_varlen_channel_gate_sampled_units():
+    """cfg3 (64 varlen segments, per-channel gate) at a reduced head count to bound memory; sampled units
+    including the shortest and the longest segment."""
+    inp = wl.cfg3("cuda", H=4)
+    E, T = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
+    lens = inp.seg_lens
+    units = [(int(np.argmin(lens)), 1), (int(np.argmax(lens)), 2)] + _sample_units(64, 4, 3, 3)
+    E_ref, T_ref = oracle_encode_units(inp, units)
+    si, hi = torch.tensor([u[0] for u in units]), torch.tensor([u[1] for u in units])
+    check_E(E[si, hi][:, None], E_ref, TOL_BF16)
+    check_T(T[si, hi][:, None], T_ref, TOL_BF16)
+    assert torch.isfinite(E).all() and torch.isfinite(T).all()
+
+
+def test_cfg4_compose_stress_sampled_requests():
+    """cfg4 at full size for one layer-iteration (P=1024, H=32, R=128, n_r ~ U{16..64}): sampled (request,
+    head) chains against the fp64 compose of the same fp32 pools."""
+    pin = wl.cfg4_pool_inputs(device="cuda")
+    _, T = gpu_encode(pin, hb.HYPIC_IMPL_AUTO)
+    del pin
+    E = wl.cfg4_pool_E(device="cuda")
+    req = wl.cfg4_requests(device="cuda")
+    S = gpu_compose(req.S_in, E, T, req.seg_ids, req.cu_segs, hb.HYPIC_IMPL_AUTO)
+    assert torch.isfinite(S).all()
+    units = _sample_units(128, 32, 8, 4)
+    ref = oracle_compose_units(req.S_in, E, T, req.seg_ids, req.cu_segs, units)
+    ri, hi = torch.tensor([u[0] for u in units]), torch.tensor([u[1] for u in units])
+    check_E(S[ri, hi][:, None], ref, TOL_F32, "S_out")
