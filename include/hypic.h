@@ -118,6 +118,14 @@ int hypic_compose(const float* S_in, const float* E_pool, const float* T_pool, c
 int hypic_encode_impl_for(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate);
 int hypic_compose_impl_for(int32_t H, int32_t dk, int32_t dv);
 
+/*
+ * hypic_debug_timeout_count: the tensor-family kernels never spin forever on an mbarrier; a wait that expires
+ * (a protocol bug, never expected) bumps a device counter instead of hanging the GPU.  This call synchronises
+ * the device and returns the counter since library load (0 = healthy; 0xffffffff = the query itself failed).
+ * Test / diagnostics only.
+ */
+unsigned int hypic_debug_timeout_count(void);
+
 /* hypic_status_string: static, NUL-terminated description of a status code (never NULL). */
 const char* hypic_status_string(int status);
 

@@ -28,7 +28,7 @@ HYPIC_IMPL_TENSOR = 2
 EXPORTS = (
     "hypic_set_impl", "hypic_get_impl", "hypic_segment_encode_workspace", "hypic_segment_encode", "hypic_compose",
     "hypic_status_string", "hypic_version", "hypic_last_launch_count", "hypic_encode_impl_for",
-    "hypic_compose_impl_for",
+    "hypic_compose_impl_for", "hypic_debug_timeout_count",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -73,6 +73,8 @@ def load_library() -> ctypes.CDLL:
     lib.hypic_encode_impl_for.restype = ctypes.c_int
     lib.hypic_compose_impl_for.argtypes = [i32, i32, i32]
     lib.hypic_compose_impl_for.restype = ctypes.c_int
+    lib.hypic_debug_timeout_count.argtypes = []
+    lib.hypic_debug_timeout_count.restype = ctypes.c_uint
     _lib = lib
     return lib
 
@@ -101,6 +103,10 @@ def hypic_encode_impl_for(H: int, dk: int, dv: int, kv_dtype: int, gate: int) ->
 
 def hypic_compose_impl_for(H: int, dk: int, dv: int) -> int:
     return int(load_library().hypic_compose_impl_for(H, dk, dv))
+
+
+def hypic_debug_timeout_count() -> int:
+    return int(load_library().hypic_debug_timeout_count())
 
 
 def hypic_last_launch_count() -> int:

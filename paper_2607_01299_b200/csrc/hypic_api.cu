@@ -139,6 +139,8 @@ const char* hypic_status_string(int status) {
 
 int hypic_version(void) { return HYPIC_VERSION; }
 
+unsigned int hypic_debug_timeout_count(void) { return debug_timeout_count(); }
+
 int hypic_last_launch_count(void) { return g_launch_count; }
 
 }  // extern "C"

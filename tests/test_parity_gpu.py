@@ -24,6 +24,7 @@ def _need_cuda():
     hb.load_library()  # fail loudly if the extension is missing
     yield
     hb.hypic_set_impl(hb.HYPIC_IMPL_AUTO)
+    assert hb.hypic_debug_timeout_count() == 0, "a tensor-family kernel hit a bounded-wait timeout"
 
 
 @contextlib.contextmanager
