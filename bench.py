@@ -224,7 +224,7 @@ class Cfg2Request:
                 events[l][2].record()
 
 
-def time_extra_cfg1(hb, device, reps=20):
+def time_extra_cfg1(hb, device, peaks, reps=20):
     """cfg1 (H=16, 4 x 2048): encode + compose; 4 rotating input copies (272 MB > L2) so inputs come from HBM."""
     copies = [wl.make_encode_inputs([2048] * 4, 16, D, D, kv_dtype=torch.bfloat16, g_lo=-0.05, beta_kind="sigmoid",
                                     seed=wl.seed_for(1, i), device=device) for i in range(4)]
@@ -252,7 +252,7 @@ def time_extra_cfg1(hb, device, reps=20):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / reps
     return {"workload": "cfg1: H=16, 4 x 2048, encode + compose", "ms": ms, "tokens_per_s": 8192 / (ms * 1e-3),
-            "tc_frac_of_bf16_peak": None}
+            "tc_frac_of_bf16_burst_peak": 8192 * 16 * ENC_FLOP_PER_TOKEN_HEAD / (ms * 1e-3) / 1e12 / peaks["bf16_tflops"]}
 
 
 def time_extra_cfg4(hb, device, peaks, iters=48):
@@ -350,8 +350,15 @@ def run_ours(args):
         roofline = {"bound": "alu", "achieved": enc_tflops, "peak": FP32_ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
                     "frac": enc_tflops / FP32_ALU_PEAK_TFLOPS, "traffic": None,
                     "peak_kind": "fp32 FMA: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md)"}
-    roofline.update({"kernel": "segment encode (" + ("tensor" if enc_family == hb.HYPIC_IMPL_TENSOR else "simt") +
-                     " family)", "avg_launch_ms": enc_avg, "share_of_step": enc_avg * L / ms_step,
+    fam = "tensor" if enc_family == hb.HYPIC_IMPL_TENSOR else "simt"
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")  # dram bytes per launch from the committed ncu capture
+    if os.path.exists(tpath):
+        roofline["traffic"] = json.load(open(tpath)).get(f"encode_{fam}_cfg2_layer_dram_bytes")
+    roofline.update({"kernel": ("hypic_segment_encode = chunk_offsets_kernel + prep_kernel + scan_kernel (tensor "
+                                "family; scan_kernel dominates, see profiles/)") if fam == "tensor" else
+                     "hypic_segment_encode = encode_simt_kernel (simt family)",
+                     "units_per_launch": f"{th_per_launch} token-heads x {ENC_FLOP_PER_TOKEN_HEAD} flop",
+                     "avg_launch_ms": enc_avg, "share_of_step": enc_avg * L / ms_step,
                      "frac_of_bf16_burst_peak": enc_tflops / peaks["bf16_tflops"], "hbm_gbs": enc_gbs,
                      "hbm_frac": enc_gbs / peaks["hbm_gbs"]})
 
@@ -397,7 +404,7 @@ def run_ours(args):
     if not args.no_extra:
         del req
         torch.cuda.empty_cache()
-        extra["cfg1"] = time_extra_cfg1(hb, device)
+        extra["cfg1"] = time_extra_cfg1(hb, device, peaks)
         extra["cfg4_compose"] = time_extra_cfg4(hb, device, peaks)
         extra["cfg2_compose"] = {"avg_launch_ms": cmp_avg, "compose_ops_per_s": N_SEG * H / (cmp_avg * 1e-3),
                                  "hbm_gbs": N_SEG * H * COMPOSE_BYTES_PER_STEP / (cmp_avg * 1e-3) / 1e9}
