@@ -9,10 +9,15 @@
 //     each slab into T_hi / T_lo in the 32-bit MN-major "128B swizzle, 32B base" layout (B operand);
 //   * 3xTF32:  D = S_hi T_hi + S_lo T_hi + S_hi T_lo  (fp32 accumulate in TMEM; the hardware truncates tf32
 //     operands, which is why hi is rounded in software and lo carries the remainder);
-//   * round-trip warps read D (tcgen05.ld), add E_i (staged in padded smem rows by per-row bulk copies), and
-//     write the next S_hi / S_lo (tcgen05.st), or S_out after the last step.
+//   * round-trip warps (two per TMEM lane quarter) read D (tcgen05.ld), add E_i (staged by TMA tensor boxes of
+//     32 rows x 128 B with the 128B swizzle, so that row-per-thread reads are bank-conflict free; per-row bulk
+//     copies were measured to cost ~46 cycles of TMA issue each and dominated the step), and write the next
+//     S_hi / S_lo (tcgen05.st), or S_out after the last step.
 // S_in enters as "step -1" (D = 0, E = S_in).  All waits are bounded: a protocol error raises the timeout
 // counter (hypic_debug_timeout_count) instead of hanging the GPU.
+#include <cuda.h>
+#include <string.h>
+
 #include "common.cuh"
 #include "sm100_ptx.cuh"
 
@@ -27,9 +32,8 @@ constexpr int kD = 128;
 constexpr int kSlabBytes = 32 * kD * 4;  // 32 rows of T (or E): 16 KB
 constexpr int kNRaw = 3;                 // raw T slabs in flight
 constexpr int kNHl = 3;                  // converted (hi, lo) slab pairs
-constexpr int kEPitch = 528;             // padded row pitch of an E slot (conflict-free row-per-thread reads)
-constexpr int kESlotBytes = 32 * kEPitch;
-constexpr int kThreads = 352;            // warp 0 T producer, 1 MMA, 2 E producer, 3-6 converters, 7-10 round trip
+constexpr int kESlotBytes = kSlabBytes;  // 4 TMA boxes of 32 rows x 128 B (128B swizzle: conflict-free row reads)
+constexpr int kThreads = 480;            // warp 0 T producer, 1 MMA, 2 E producer, 3-6 converters, 7-14 round trip
 
 constexpr int kOffHl = 0;
 constexpr int kOffRaw = kOffHl + kNHl * 2 * kSlabBytes;
@@ -61,9 +65,42 @@ __device__ __forceinline__ float rna_tf32(float x) {
   return __uint_as_float(r);
 }
 
+__device__ __forceinline__ void tma_load_2d(void* dst_smem, const CUtensorMap* tm, int c0, int c1, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+          smem_u32(dst_smem)),
+      "l"(reinterpret_cast<uint64_t>(tm)), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+      : "memory");
+}
+
+// [rows][128] fp32 row-major viewed as a 2-D tensor; box = 32 columns (128 B) x 32 rows, 128B swizzle.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int make_rows_tensor_map(CUtensorMap* tm, const float* base, uint64_t rows) {
+  static EncodeTiledFn fn = nullptr;
+  if (fn == nullptr) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess || p == nullptr)
+      return HYPIC_ERR_CUDA;
+    fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  const cuuint64_t dims[2] = {(cuuint64_t)kD, (cuuint64_t)rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)kD * 4};
+  const cuuint32_t box[2] = {32, 32};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? HYPIC_OK : HYPIC_ERR_CUDA;
+}
+
 __global__ void __launch_bounds__(kThreads, 1)
-    compose_tensor_kernel(const float* __restrict__ S_in, const float* __restrict__ E_pool,
-                          const float* __restrict__ T_pool, const int32_t* __restrict__ seg_ids,
+    compose_tensor_kernel(const __grid_constant__ CUtensorMap tmE, const __grid_constant__ CUtensorMap tmS,
+                          const float* __restrict__ S_in, const float* __restrict__ T_pool, const int32_t* __restrict__ seg_ids,
                           const int32_t* __restrict__ cu_segs, int H, float* __restrict__ S_out) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -81,9 +118,9 @@ __global__ void __launch_bounds__(kThreads, 1)
   if (tid == 32) {
     for (int i = 0; i < kNRaw; ++i) { mbar_init(&bars->raw_full[i], 1); mbar_init(&bars->raw_empty[i], 4); }
     for (int i = 0; i < kNHl; ++i) { mbar_init(&bars->hl_full[i], 4); mbar_init(&bars->hl_empty[i], 1); }
-    for (int i = 0; i < 4; ++i) { mbar_init(&bars->e_full[i], 1); mbar_init(&bars->e_empty[i], 1); }
+    for (int i = 0; i < 4; ++i) { mbar_init(&bars->e_full[i], 1); mbar_init(&bars->e_empty[i], 2); }
     mbar_init(&bars->d_full, 1);
-    mbar_init(&bars->a_ready, 4);
+    mbar_init(&bars->a_ready, 8);
     bars->abort_flag = 0;
     fence_barrier_init();
   }
@@ -138,24 +175,28 @@ __global__ void __launch_bounds__(kThreads, 1)
       }
     }
   } else if (warp == 2) {
-    // ---------------------------------------------------------------- E producer: one 512 B row per lane, padded
-    uint32_t ecount = 0;
-    for (int s = -1; s < n; ++s) {
-      const float* src;
-      if (s < 0) {
-        if (S_in == nullptr) continue;
-        src = S_in + (size_t)unit * mat;
-      } else {
-        src = E_pool + ((size_t)seg_ids[seg_begin + s] * H + h) * mat;
+    // ---------------------------------------------------------------- E producer: 4 TMA boxes (32 x 32 fp32) per slab
+    if (lane < 4) {
+      uint32_t ecount = 0;
+      for (int s = -1; s < n; ++s) {
+        const CUtensorMap* tm;
+        int row0;
+        if (s < 0) {
+          if (S_in == nullptr) continue;
+          tm = &tmS;
+          row0 = unit * kD;
+        } else {
+          tm = &tmE;
+          row0 = (seg_ids[seg_begin + s] * H + h) * kD;
+        }
+        for (int q = 0; q < 4; ++q) {
+          wait_or_abort(&bars->e_empty[q], (ecount & 1) ^ 1, abort_flag);
+          if (lane == 0) mbar_expect_tx(&bars->e_full[q], kSlabBytes);
+          __syncwarp(0xf);
+          tma_load_2d(smem + kOffE + q * kESlotBytes + lane * 4096, tm, 32 * lane, row0 + 32 * q, &bars->e_full[q]);
+        }
+        ++ecount;
       }
-      for (int q = 0; q < 4; ++q) {
-        wait_or_abort(&bars->e_empty[q], (ecount & 1) ^ 1, abort_flag);
-        if (lane == 0) mbar_expect_tx(&bars->e_full[q], kSlabBytes);
-        __syncwarp();
-        bulk_g2s(smem + kOffE + q * kESlotBytes + lane * kEPitch, src + (size_t)(32 * q + lane) * kD, kD * 4,
-                 &bars->e_full[q]);
-      }
-      ++ecount;
     }
   } else if (warp < 7) {
     // ---------------------------------------------------------------- converters: raw slab -> (hi, lo) tiles
@@ -195,10 +236,11 @@ __global__ void __launch_bounds__(kThreads, 1)
     }
   } else {
     // ---------------------------------------------------------------- round trip: D (+E) -> next S_hi/S_lo or S_out
-    const int q = warp & 3;  // TMEM lane quarter this warp may touch
+    const int q = warp & 3;            // TMEM lane quarter this warp may touch
+    const int half = (warp - 7) >> 2;  // which 64 columns of the quarter this warp handles
     const uint32_t lane_base = (uint32_t)(32 * q) << 16;
     const int row = 32 * q + lane;
-    const uint8_t* erow = smem + kOffE + q * kESlotBytes + lane * kEPitch;
+    const uint8_t* erow = smem + kOffE + q * kESlotBytes + lane * 128;
     float* out_row = S_out + (size_t)unit * mat + (size_t)row * kD;
     uint32_t ecount = 0;
     for (int s = -1; s < n; ++s) {
@@ -210,7 +252,7 @@ __global__ void __launch_bounds__(kThreads, 1)
       }
       if (have_e) wait_or_abort(&bars->e_full[q], ecount & 1, abort_flag);
 #pragma unroll 1
-      for (int cb = 0; cb < 4; ++cb) {
+      for (int cb = 2 * half; cb < 2 * half + 2; ++cb) {
         uint32_t d[32];
         if (s >= 0) {
           tmem_ld32(tD + lane_base + 32 * cb, d);
@@ -223,10 +265,10 @@ __global__ void __launch_bounds__(kThreads, 1)
 #pragma unroll
         for (int c = 0; c < 32; ++c) xv[c] = __uint_as_float(d[c]);
         if (have_e) {
-          const float4* e4 = reinterpret_cast<const float4*>(erow + cb * 128);
+          const uint8_t* eb = erow + cb * 4096;
 #pragma unroll
           for (int u = 0; u < 8; ++u) {
-            const float4 e = e4[u];
+            const float4 e = *reinterpret_cast<const float4*>(eb + ((u ^ (lane & 7)) * 16));
             xv[4 * u] += e.x, xv[4 * u + 1] += e.y, xv[4 * u + 2] += e.z, xv[4 * u + 3] += e.w;
           }
         }
@@ -279,7 +321,20 @@ int compose_tensor(const ComposeArgs& a) {
   }
   const long long units = (long long)a.R * a.H;
   if (units > 0x7fffffffLL) return HYPIC_ERR_UNSUPPORTED;
-  compose_tensor_kernel<<<(unsigned)units, kThreads, kSmemBytes, a.stream>>>(a.S_in, a.E_pool, a.T_pool, a.seg_ids,
+  CUtensorMap tmE, tmS;
+  if (a.total_steps > 0 || a.S_in != nullptr) {
+    const int rc = make_rows_tensor_map(&tmE, a.total_steps > 0 ? a.E_pool : a.S_in,
+                                        a.total_steps > 0 ? (uint64_t)a.P * a.H * kD : (uint64_t)units * kD);
+    if (rc != HYPIC_OK) return rc;
+  } else {
+    memset(&tmE, 0, sizeof(tmE));
+  }
+  tmS = tmE;
+  if (a.S_in != nullptr) {
+    const int rc = make_rows_tensor_map(&tmS, a.S_in, (uint64_t)units * kD);
+    if (rc != HYPIC_OK) return rc;
+  }
+  compose_tensor_kernel<<<(unsigned)units, kThreads, kSmemBytes, a.stream>>>(tmE, tmS, a.S_in, a.T_pool, a.seg_ids,
                                                                             a.cu_segs, a.H, a.S_out);
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
