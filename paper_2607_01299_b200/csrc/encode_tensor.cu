@@ -13,6 +13,9 @@
 //                      K-major 128B-swizzled UMMA B tiles, plus the gate record (d_j, gamma_C).
 //   K2 scan          : one CTA per (segment, head, row block of X), sequential over chunks; every contraction is
 //                      a tcgen05.mma with the state block resident in TMEM (see the kernel's comment).
+#include <cuda.h>
+#include <stdlib.h>
+
 #include "common.cuh"
 #include "sm100_ptx.cuh"
 
@@ -166,28 +169,33 @@ __global__ void __launch_bounds__(kPrepThreads)
           const int j = 8 * nt + 2 * tq + (i & 1);
           float v = 0.f;
           if (j < r) v = s_b[r] * expf(s_g[r] - s_g[j]) * acc[mt][nt][i];
-          s_l[r * kLPitch + j] = v;
+          s_l[j * kLPitch + r] = v;  // stored transposed: Lt[j][r]
         }
   }
   __syncthreads();
 
-  // ---- a3: A = (I + L)^-1 by forward substitution; thread c owns column c (fp32 throughout)
+  // ---- a3: A = (I + L)^-1, column c per thread, right-looking (column-oriented) forward substitution in fp32:
+  // a_j = t_j is final once columns < j have been applied; then t_r -= L_rj a_j for r > j (independent FMAs).
+  // Column c of A is zero above row c, so a warp skips the steps below its first column.
   float a[kC];
   {
     const int c = tid;
 #pragma unroll
-    for (int r = 0; r < kC; ++r) {
-      float acc = (r == c) ? 1.f : 0.f;
-      const float4* lrow = reinterpret_cast<const float4*>(s_l + r * kLPitch);
+    for (int r = 0; r < kC; ++r) a[r] = (r == c) ? 1.f : 0.f;
 #pragma unroll
-      for (int j4 = 0; j4 < (r + 3) / 4; ++j4) {
-        const float4 l = lrow[j4];
-        if (4 * j4 + 0 < r) acc = fmaf(-l.x, a[4 * j4 + 0], acc);
-        if (4 * j4 + 1 < r) acc = fmaf(-l.y, a[4 * j4 + 1], acc);
-        if (4 * j4 + 2 < r) acc = fmaf(-l.z, a[4 * j4 + 2], acc);
-        if (4 * j4 + 3 < r) acc = fmaf(-l.w, a[4 * j4 + 3], acc);
+    for (int j = 0; j < kC - 1; ++j) {
+      if (j >= 32 * warp) {
+        const float aj = a[j];
+        const float4* lcol = reinterpret_cast<const float4*>(s_l + j * kLPitch);
+#pragma unroll
+        for (int r4 = (j + 1) / 4; r4 < kC / 4; ++r4) {
+          const float4 l = lcol[r4];
+          if (4 * r4 + 0 > j) a[4 * r4 + 0] = fmaf(-l.x, aj, a[4 * r4 + 0]);
+          if (4 * r4 + 1 > j) a[4 * r4 + 1] = fmaf(-l.y, aj, a[4 * r4 + 1]);
+          if (4 * r4 + 2 > j) a[4 * r4 + 2] = fmaf(-l.z, aj, a[4 * r4 + 2]);
+          if (4 * r4 + 3 > j) a[4 * r4 + 3] = fmaf(-l.w, aj, a[4 * r4 + 3]);
+        }
       }
-      a[r] = acc;
     }
   }
   // A_b = A diag(beta) staged as fp32 [r][c] in the (now dead) K buffer
@@ -518,6 +526,34 @@ __global__ void __launch_bounds__(kScanThreads, 1)
   if (warp == 0) tmem_dealloc(tmem, 512);
 }
 
+#include "encode_scan_ws.cuh"
+
+// k / v viewed as 3-D bf16 tensors [t_total][H][128]; box = 64 elements (128 B) x 1 head x 64 tokens, 128B swizzle:
+// the box lands as one MN-major UMMA chunk (8-token atoms of 1 KB), two boxes per 64 x 128 tile.
+typedef CUresult (*EncodeTiledFn3)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int make_kv_tensor_map(CUtensorMap* tm, const void* base, int32_t t_total, int32_t H) {
+  static EncodeTiledFn3 fn = nullptr;
+  if (fn == nullptr) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess || p == nullptr)
+      return HYPIC_ERR_CUDA;
+    fn = reinterpret_cast<EncodeTiledFn3>(p);
+  }
+  const cuuint64_t dims[3] = {(cuuint64_t)kD, (cuuint64_t)H, (cuuint64_t)t_total};
+  const cuuint64_t strides[2] = {(cuuint64_t)kD * 2, (cuuint64_t)H * kD * 2};
+  const cuuint32_t box[3] = {64, 1, 64};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  const CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? HYPIC_OK : HYPIC_ERR_CUDA;
+}
+
 }  // namespace
 
 bool encode_tensor_shape_ok(int32_t, int32_t dk, int32_t dv, int kv_dtype, int gate) {
@@ -555,8 +591,26 @@ int encode_tensor(const EncodeArgs& a) {
                                                                          a.n_seg, a.H, ab, gate);
     note_launch();
   }
-  scan_kernel<<<dim3(2, a.H, a.n_seg), kScanThreads, kScanSmem, a.stream>>>(kp, vp, a.cu_seqlens, chunk_off, a.H, ab,
+  static const bool use_v1 = [] {
+    const char* e = getenv("HYPIC_SCAN_V1");  // diagnostics: the lock-step 128-thread scan kernel
+    return e != nullptr && e[0] == '1';
+  }();
+  if (use_v1 || a.t_total == 0) {
+    scan_kernel<<<dim3(2, a.H, a.n_seg), kScanThreads, kScanSmem, a.stream>>>(kp, vp, a.cu_seqlens, chunk_off, a.H, ab,
+                                                                              gate, a.E, a.T);
+  } else {
+    static bool configured_ws = false;
+    if (!configured_ws) {
+      HYPIC_CUDA_OK(cudaFuncSetAttribute(scan_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kWsSmem));
+      configured_ws = true;
+    }
+    CUtensorMap tmK, tmV;
+    int rc = make_kv_tensor_map(&tmK, a.k, a.t_total, a.H);
+    if (rc == HYPIC_OK) rc = make_kv_tensor_map(&tmV, a.v, a.t_total, a.H);
+    if (rc != HYPIC_OK) return rc;
+    scan_ws_kernel<<<dim3(2, a.H, a.n_seg), kWsThreads, kWsSmem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, a.H, ab,
                                                                             gate, a.E, a.T);
+  }
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
   return HYPIC_OK;
