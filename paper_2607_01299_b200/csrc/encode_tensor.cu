@@ -8,12 +8,13 @@
 //     X <- gamma_C X + ([U^t ; 0] - X W^t) diag(d) K          for the stacked state X = [E ; T].
 // Three launches:
 //   K0 chunk_offsets : prefix sum of ceil(L_s / 64) (cu_seqlens lives on the device; no host sync).
-//   K1 prep          : per (chunk, head), state-independent: Gram (mma.sync bf16), L, A by forward substitution
-//                      (fp32), then A_b and A_b diag(gamma) split into bf16 hi + lo and stored as ready-made
-//                      K-major 128B-swizzled UMMA B tiles, plus the gate record (d_j, gamma_C).
-//   K2 scan          : one CTA per (segment, head, row block of X), sequential over chunks; every contraction is
-//                      a tcgen05.mma with the state block resident in TMEM (see the kernel's comment).
+//   K1 prep          : per (chunk, head), state-independent: Gram (mma.sync), L, A by forward substitution (fp32),
+//                      W (mma.sync, fp16 out) and A_b (bf16 hi + lo), stored as ready-made K-major 128B-swizzled
+//                      UMMA B tiles, plus the gate record (d_j, gamma_C).
+//   K2 scan          : one CTA per (segment, head), sequential over chunks, both row blocks of X resident in TMEM;
+//                      every state contraction is a tcgen05.mma (see encode_scan2.cuh).
 #include <cuda.h>
+#include <cuda_fp16.h>
 #include <stdlib.h>
 
 #include "common.cuh"
@@ -25,19 +26,15 @@ using namespace ptx;
 
 constexpr int kC = 64;                  // chunk length (north_star)
 constexpr int kD = 128;                 // dk = dv
-constexpr int kTileB = kC * kC * 2;     // one bf16 64x64 B tile: 8 KB
-constexpr int kAbBytes = 4 * kTileB;    // A_b hi, A_b lo, A_bg hi, A_bg lo
+constexpr int kTileB = kC * kC * 2;     // one 16-bit 64x64 tile: 8 KB
+constexpr int kRecW = 0;                // record: -W (fp16, [token][dk], two 64-wide boxes) 16 KB
+constexpr int kRecAb = 2 * kTileB;      //         A_b hi, A_b lo (bf16, [token][token]) 2 x 8 KB
+constexpr int kRecBytes = 4 * kTileB;   // 32 KB per (chunk, head)
 constexpr int kGateFloats = 72;         // d_j[64], gamma_C, pad (288 B = 18 x 16 B)
 constexpr int kGateBytes = kGateFloats * 4;
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
-
-struct Workspace {
-  int32_t* chunk_off;  // [n_seg + 1]
-  uint8_t* ab;         // [n_chunk_cap][H][kAbBytes]
-  float* gate;         // [n_chunk_cap][H][kGateFloats]
-};
-__host__ __device__ inline size_t ws_off_ab(int32_t n_seg) { return align_up(4 * ((size_t)n_seg + 1), 1024); }
+__host__ __device__ inline size_t ws_off_rec(int32_t n_seg) { return align_up(4 * ((size_t)n_seg + 1), 1024); }
 __host__ __device__ inline size_t chunk_cap(int32_t n_seg, int32_t t_total) { return (size_t)t_total / kC + n_seg; }
 
 // ------------------------------------------------------------------------------------------------ K0
@@ -69,29 +66,40 @@ __global__ void chunk_offsets_kernel(const int32_t* __restrict__ cu_seqlens, int
 
 // ------------------------------------------------------------------------------------------------ K1
 constexpr int kPrepThreads = 64;
-constexpr int kKsPitch = kD + 8;  // bf16 elements per row of the staged K chunk (conflict-free fragment loads)
+constexpr int kKsPitch = kD + 8;  // 16-bit elements per row of the staged K chunk (conflict-free fragment loads)
 constexpr int kLPitch = 68;       // floats per row of L / A
 
-__device__ __forceinline__ void mma_bf16_16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
-                                               uint32_t b0, uint32_t b1) {
+__device__ __forceinline__ void mma_f16_16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                              uint32_t b0, uint32_t b1) {
   asm volatile(
-      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
       : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
       : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
-
+__device__ __forceinline__ void ldmatrix_x4_trans(uint32_t (&r)[4], uint32_t saddr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "r"(saddr));
+}
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   __nv_bfloat162 p = __floats2bfloat162_rn(lo, hi);
   return *reinterpret_cast<uint32_t*>(&p);
 }
+__device__ __forceinline__ uint32_t pack_f16(float lo, float hi) {
+  __half2 p = __floats2half2_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&p);
+}
 
+// K is staged as fp16 (exact for bf16 values with |x| in [2^-14, 65504]; smaller magnitudes lose bits below
+// 2^-24 absolute), so that the Gram and W contractions run as f16 mma.sync with an 11-bit A operand.
 __global__ void __launch_bounds__(kPrepThreads)
     prep_kernel(const __nv_bfloat16* __restrict__ k, const float* __restrict__ g, const float* __restrict__ beta,
                 const int32_t* __restrict__ cu_seqlens, const int32_t* __restrict__ chunk_off, int n_seg, int H,
-                uint8_t* __restrict__ ab, float* __restrict__ gate) {
-  __shared__ __align__(16) uint8_t s_k[kC * kKsPitch * 2];  // K chunk (bf16), later reused for A (fp32)
-  __shared__ __align__(16) float s_l[kC * kLPitch];
-  __shared__ float s_g[kC], s_b[kC];
+                uint8_t* __restrict__ rec, float* __restrict__ gate) {
+  __shared__ __align__(16) uint8_t s_k[kC * kKsPitch * 2];  // K chunk (fp16); later the staged W tile
+  __shared__ __align__(16) float s_l[kC * kLPitch];         // L^t; later A_b
+  __shared__ float s_g[kC], s_b[kC], s_gam[kC];
+  __shared__ float s_wsum;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int x = blockIdx.x, h = blockIdx.y;
   if (x >= chunk_off[n_seg]) return;
@@ -105,29 +113,38 @@ __global__ void __launch_bounds__(kPrepThreads)
   const int t0 = cu_seqlens[s] + (x - chunk_off[s]) * kC;
   const int valid = min(kC, cu_seqlens[s + 1] - t0);
 
-  __nv_bfloat16* ks = reinterpret_cast<__nv_bfloat16*>(s_k);
+  __half* ks = reinterpret_cast<__half*>(s_k);
   for (int idx = tid; idx < kC * (kD / 8); idx += kPrepThreads) {
     const int r = idx / (kD / 8), c8 = idx % (kD / 8);
     uint4 val = make_uint4(0, 0, 0, 0);
-    if (r < valid) val = *reinterpret_cast<const uint4*>(k + ((size_t)(t0 + r) * H + h) * kD + c8 * 8);
+    if (r < valid) {
+      const uint4 raw = *reinterpret_cast<const uint4*>(k + ((size_t)(t0 + r) * H + h) * kD + c8 * 8);
+      const uint32_t w[4] = {raw.x, raw.y, raw.z, raw.w};
+      uint32_t o[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) o[i] = pack_f16(__uint_as_float(w[i] << 16), __uint_as_float(w[i] & 0xffff0000u));
+      val = make_uint4(o[0], o[1], o[2], o[3]);
+    }
     *reinterpret_cast<uint4*>(ks + r * kKsPitch + c8 * 8) = val;
   }
-  {
+  {  // a1: inclusive cumulative log-decay by a two-warp shuffle scan
     const bool ok = tid < valid;
-    s_g[tid] = ok ? g[(size_t)(t0 + tid) * H + h] : 0.f;
+    float gv = ok ? g[(size_t)(t0 + tid) * H + h] : 0.f;
     s_b[tid] = ok ? beta[(size_t)(t0 + tid) * H + h] : 0.f;
-  }
-  __syncthreads();
-  if (tid == 0) {  // inclusive cumulative log-decay (a1)
-    float run = 0.f;
-    for (int r = 0; r < kC; ++r) {
-      run += s_g[r];
-      s_g[r] = run;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const float up = __shfl_up_sync(0xffffffffu, gv, o);
+      if (lane >= o) gv += up;
     }
+    if (tid == 31) s_wsum = gv;
+    __syncthreads();
+    if (warp == 1) gv += s_wsum;
+    s_g[tid] = gv;
+    s_gam[tid] = expf(gv);
   }
   __syncthreads();
 
-  // ---- a2: Gram K K^t with mma.sync (bf16 in, fp32 accumulate); warp w owns rows [32w, 32w+32)
+  // ---- a2: Gram K K^t with mma.sync (fp16 in, fp32 accumulate); warp w owns rows [32w, 32w+32)
   {
     const int gq = lane >> 2, tq = lane & 3;
     float acc[2][8][4];
@@ -152,10 +169,11 @@ __global__ void __launch_bounds__(kPrepThreads)
       }
 #pragma unroll
       for (int nt = 0; nt < 8; ++nt) {
+        if (nt > 4 * warp + 3) continue;  // strictly above the diagonal for every row of this warp
         const int n0 = 8 * nt + gq;
         const uint32_t b0 = kw[n0 * pw + 8 * kk + tq], b1 = kw[n0 * pw + 8 * kk + 4 + tq];
-        mma_bf16_16816(acc[0][nt], a[0][0], a[0][1], a[0][2], a[0][3], b0, b1);
-        mma_bf16_16816(acc[1][nt], a[1][0], a[1][1], a[1][2], a[1][3], b0, b1);
+        mma_f16_16816(acc[0][nt], a[0][0], a[0][1], a[0][2], a[0][3], b0, b1);
+        mma_f16_16816(acc[1][nt], a[1][0], a[1][1], a[1][2], a[1][3], b0, b1);
       }
     }
     // L_rj = beta_r exp(G_r - G_j) (k_r.k_j) for j < r, else 0
@@ -168,7 +186,7 @@ __global__ void __launch_bounds__(kPrepThreads)
           const int r = 32 * warp + 16 * mt + gq + ((i >> 1) ? 8 : 0);
           const int j = 8 * nt + 2 * tq + (i & 1);
           float v = 0.f;
-          if (j < r) v = s_b[r] * expf(s_g[r] - s_g[j]) * acc[mt][nt][i];
+          if (j < r) v = s_b[r] * __expf(s_g[r] - s_g[j]) * acc[mt][nt][i];
           s_l[j * kLPitch + r] = v;  // stored transposed: Lt[j][r]
         }
   }
@@ -177,8 +195,8 @@ __global__ void __launch_bounds__(kPrepThreads)
   // ---- a3: A = (I + L)^-1, column c per thread, right-looking (column-oriented) forward substitution in fp32:
   // a_j = t_j is final once columns < j have been applied; then t_r -= L_rj a_j for r > j (independent FMAs).
   // Column c of A is zero above row c, so a warp skips the steps below its first column.
-  float a[kC];
   {
+    float a[kC];
     const int c = tid;
 #pragma unroll
     for (int r = 0; r < kC; ++r) a[r] = (r == c) ? 1.f : 0.f;
@@ -197,336 +215,102 @@ __global__ void __launch_bounds__(kPrepThreads)
         }
       }
     }
-  }
-  // A_b = A diag(beta) staged as fp32 [r][c] in the (now dead) K buffer
-  float* s_a = reinterpret_cast<float*>(s_k);
-  {
+    __syncthreads();  // every column is done reading L
+    // A_b = A diag(beta) as fp32 [r][c] in the (now dead) L buffer
     const float bc = s_b[tid];
 #pragma unroll
-    for (int r = 0; r < kC; ++r) s_a[r * kLPitch + tid] = a[r] * bc;
+    for (int r = 0; r < kC; ++r) s_l[r * kLPitch + tid] = a[r] * bc;
   }
   __syncthreads();
+  const float* s_a = s_l;
 
-  // ---- emit the four bf16 B tiles (K-major, 128B swizzle: row r, 16-byte chunk j8 at ((j8 ^ (r & 7)) * 16))
-  uint8_t* out = ab + ((size_t)x * H + h) * kAbBytes;
+  // ---- W = (A_b diag(gamma)) K with mma.sync: M = 64 tokens (warp w: rows [32w, 32w+32)), N = 128, K = 64 tokens
+  float wacc[2][16][4];
+  {
+    const int gq = lane >> 2, tq = lane & 3;
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+      for (int nt = 0; nt < 16; ++nt)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) wacc[mt][nt][i] = 0.f;
+    const uint32_t ks_base = smem_u32(s_k);
+#pragma unroll
+    for (int kk = 0; kk < kC / 16; ++kk) {
+      if (kk > 2 * warp + 1) continue;  // A_b is lower triangular: rows < 32(w+1) have no columns >= 32(w+1)
+      uint32_t a[2][4];
+      const int c0 = 16 * kk + 2 * tq;
+      const float g0 = s_gam[c0], g1 = s_gam[c0 + 1], g8 = s_gam[c0 + 8], g9 = s_gam[c0 + 9];
+#pragma unroll
+      for (int mt = 0; mt < 2; ++mt) {
+        const int r0 = 32 * warp + 16 * mt + gq;
+        const float2 p0 = *reinterpret_cast<const float2*>(s_a + r0 * kLPitch + c0);
+        const float2 p1 = *reinterpret_cast<const float2*>(s_a + (r0 + 8) * kLPitch + c0);
+        const float2 p2 = *reinterpret_cast<const float2*>(s_a + r0 * kLPitch + c0 + 8);
+        const float2 p3 = *reinterpret_cast<const float2*>(s_a + (r0 + 8) * kLPitch + c0 + 8);
+        a[mt][0] = pack_f16(p0.x * g0, p0.y * g1);
+        a[mt][1] = pack_f16(p1.x * g0, p1.y * g1);
+        a[mt][2] = pack_f16(p2.x * g8, p2.y * g9);
+        a[mt][3] = pack_f16(p3.x * g8, p3.y * g9);
+      }
+      // B fragments (k = token, n = dk) by transposing ldmatrix over the [token][dk] tile, two n-tiles at a time
+      const int tok = 16 * kk + (lane & 7) + ((lane >> 3) & 1) * 8;
+#pragma unroll
+      for (int np = 0; np < 8; ++np) {
+        uint32_t b[4];
+        ldmatrix_x4_trans(b, ks_base + (uint32_t)(tok * kKsPitch + 8 * (2 * np + (lane >> 4))) * 2u);
+        mma_f16_16816(wacc[0][2 * np], a[0][0], a[0][1], a[0][2], a[0][3], b[0], b[1]);
+        mma_f16_16816(wacc[1][2 * np], a[1][0], a[1][1], a[1][2], a[1][3], b[0], b[1]);
+        mma_f16_16816(wacc[0][2 * np + 1], a[0][0], a[0][1], a[0][2], a[0][3], b[2], b[3]);
+        mma_f16_16816(wacc[1][2 * np + 1], a[1][0], a[1][1], a[1][2], a[1][3], b[2], b[3]);
+      }
+    }
+  }
+  __syncthreads();  // K is dead: stage W over it, already in the K-major 128B-swizzled two-box layout
+  {
+    const int gq = lane >> 2, tq = lane & 3;
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+      for (int nt = 0; nt < 16; ++nt)
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+          const int r = 32 * warp + 16 * mt + gq + 8 * hh;
+          const int col = 8 * nt + 2 * tq;
+          const uint32_t off = (col >> 6) * 8192 + (r >> 3) * 1024 + (r & 7) * 128 + ((((col & 63) >> 3) ^ (r & 7)) * 16) +
+                               (col & 7) * 2;
+          *reinterpret_cast<uint32_t*>(s_k + off) = pack_f16(-wacc[mt][nt][2 * hh], -wacc[mt][nt][2 * hh + 1]);  // -W
+        }
+  }
+  __syncthreads();
+  uint8_t* out = rec + ((size_t)x * H + h) * kRecBytes;
+  for (int idx = tid; idx < 2 * kTileB / 16; idx += kPrepThreads)
+    *reinterpret_cast<uint4*>(out + kRecW + idx * 16) = *reinterpret_cast<const uint4*>(s_k + idx * 16);
+
+  // ---- A_b as bf16 hi + lo B tiles (K-major, 128B swizzle: row r, 16-byte chunk j8 at ((j8 ^ (r & 7)) * 16))
   for (int idx = tid; idx < kC * 8; idx += kPrepThreads) {
     const int r = idx >> 3, j8 = idx & 7;
-    float v[8], vg[8];
+    float v[8];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      v[i] = s_a[r * kLPitch + 8 * j8 + i];
-      vg[i] = v[i] * expf(s_g[8 * j8 + i]);
-    }
-    uint32_t hi[4], lo[4], ghi[4], glo[4];
+    for (int i = 0; i < 8; ++i) v[i] = s_a[r * kLPitch + 8 * j8 + i];
+    uint32_t hi[4], lo[4];
 #pragma unroll
     for (int p = 0; p < 4; ++p) {
-      const float h0 = __bfloat162float(__float2bfloat16_rn(v[2 * p])), h1 = __bfloat162float(__float2bfloat16_rn(v[2 * p + 1]));
-      hi[p] = pack_bf16(h0, h1);
-      lo[p] = pack_bf16(v[2 * p] - h0, v[2 * p + 1] - h1);
-      const float q0 = __bfloat162float(__float2bfloat16_rn(vg[2 * p])), q1 = __bfloat162float(__float2bfloat16_rn(vg[2 * p + 1]));
-      ghi[p] = pack_bf16(q0, q1);
-      glo[p] = pack_bf16(vg[2 * p] - q0, vg[2 * p + 1] - q1);
+      hi[p] = pack_bf16(v[2 * p], v[2 * p + 1]);
+      lo[p] = pack_bf16(v[2 * p] - __uint_as_float(hi[p] << 16), v[2 * p + 1] - __uint_as_float(hi[p] & 0xffff0000u));
     }
     const uint32_t off = (r >> 3) * 1024 + (r & 7) * 128 + ((j8 ^ (r & 7)) * 16);
-    *reinterpret_cast<uint4*>(out + 0 * kTileB + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-    *reinterpret_cast<uint4*>(out + 1 * kTileB + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
-    *reinterpret_cast<uint4*>(out + 2 * kTileB + off) = make_uint4(ghi[0], ghi[1], ghi[2], ghi[3]);
-    *reinterpret_cast<uint4*>(out + 3 * kTileB + off) = make_uint4(glo[0], glo[1], glo[2], glo[3]);
+    *reinterpret_cast<uint4*>(out + kRecAb + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+    *reinterpret_cast<uint4*>(out + kRecAb + kTileB + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
   }
   float* go = gate + ((size_t)x * H + h) * kGateFloats;
   go[tid] = expf(s_g[kC - 1] - s_g[tid]);
-  if (tid < kGateFloats - kC) go[kC + tid] = (tid == 0) ? expf(s_g[kC - 1]) : 0.f;
-}
-
-// ------------------------------------------------------------------------------------------------ K2
-// One CTA per (row block b of X, head, segment): b = 0 is E (dv = 128 rows), b = 1 is T (dk = 128 rows); rows of
-// X evolve independently given the chunk operators, so the two blocks share nothing but their inputs.
-// TMEM columns: X [0,128) fp32 state block (pre-scaled by gamma_C before the chunk's update), Xr [128,256) =
-// rna_tf32(X) (the hardware truncates tf32 operands), DY [256,320), Wt [320,384).  Per chunk:
-//   (2) Wt  = K^t  A_bg^t        bf16, A = K tile (MN-major), B = A_bg hi/lo tiles           -> TMEM
-//   (1) DY  = V^t  A_b^t         bf16 (E block only)                                          -> TMEM
-//       Wt -> registers -> -rna_tf32 -> smem as the MN-major (32B-base swizzle) B tile of (3)
-//   (3) DY += Xr (-W)^t          tf32, A = Xr from TMEM
-//       DY -> registers -> * d_j -> bf16 hi/lo -> smem K-major A tiles of (4)
-//   (4) X  += U'' K              bf16, B = K tile (MN-major)
-constexpr int kScanThreads = 128;
-constexpr int kStK = 0, kStV = 16384, kStAb = 32768, kStGate = 65536;
-constexpr int kStageBytes = 65536 + 1024;
-constexpr int kOffW = 2 * kStageBytes;
-constexpr int kOffUhi = kOffW + 32768;
-constexpr int kOffUlo = kOffUhi + 16384;
-constexpr int kOffBar = kOffUlo + 16384;
-constexpr int kScanSmem = kOffBar + 64 + 1024;
-
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool valid) {
-  const int sz = valid ? 16 : 0;
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(sz) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-__device__ __forceinline__ float rna_tf32f(float x) {
-  uint32_t r;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
-  return __uint_as_float(r);
+  if (tid < kGateFloats - kC) go[kC + tid] = (tid == 0) ? s_gam[kC - 1] : 0.f;
 }
 
 __device__ unsigned int g_timeout_count_enc = 0;
 
-__global__ void __launch_bounds__(kScanThreads, 1)
-    scan_kernel(const __nv_bfloat16* __restrict__ k, const __nv_bfloat16* __restrict__ v,
-                const int32_t* __restrict__ cu_seqlens, const int32_t* __restrict__ chunk_off, int H,
-                const uint8_t* __restrict__ ab, const float* __restrict__ gate, float* __restrict__ E,
-                float* __restrict__ T) {
-  extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(smem + kOffBar);
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + kOffBar + 16);
-  const int tid = threadIdx.x, warp = tid >> 5;
-  const int blk = blockIdx.x, h = blockIdx.y, s = blockIdx.z;
-  const bool is_e = (blk == 0);
-  const int seg_begin = cu_seqlens[s], seg_end = cu_seqlens[s + 1];
-  const int nc = (seg_end - seg_begin + kC - 1) / kC;
-  const int chunk0 = chunk_off[s];
-
-  if (warp == 0) tmem_alloc(tmem_slot, 512);
-  if (tid == 32) {
-    mbar_init(mbar, 1);
-    fence_barrier_init();
-  }
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = *tmem_slot;
-  const uint32_t lane_base = (uint32_t)(32 * warp) << 16;
-  const uint32_t tX = tmem + lane_base, tXr = tmem + 128 + lane_base, tDY = tmem + 256 + lane_base,
-                 tWt = tmem + 320 + lane_base;
-  const uint32_t smem_base = smem_u32(smem);
-  const int row = tid;  // row of the state block (and dk index in the Wt conversion)
-
-  auto load_stage = [&](int c, int st) {
-    const int t0 = seg_begin + c * kC;
-    const int valid = min(kC, seg_end - t0);
-    const uint32_t sb = smem_base + st * kStageBytes;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const int idx = tid + kScanThreads * i;
-      const int r = idx >> 4, c16 = idx & 15;
-      const uint32_t off = (c16 >> 3) * 8192 + (r >> 3) * 1024 + (r & 7) * 128 + (((c16 & 7) ^ (r & 7)) * 16);
-      const bool ok = r < valid;
-      const size_t goff = ((size_t)(t0 + (ok ? r : 0)) * H + h) * kD + c16 * 8;
-      cp_async16(sb + kStK + off, k + goff, ok);
-      if (is_e) cp_async16(sb + kStV + off, v + goff, ok);
-    }
-    const uint8_t* abg = ab + ((size_t)(chunk0 + c) * H + h) * kAbBytes;
-#pragma unroll
-    for (int i = 0; i < kAbBytes / 16 / kScanThreads; ++i) {
-      const int idx = tid + kScanThreads * i;
-      cp_async16(sb + kStAb + idx * 16, abg + (size_t)idx * 16, true);
-    }
-    if (tid < kGateBytes / 16)
-      cp_async16(sb + kStGate + tid * 16, gate + ((size_t)(chunk0 + c) * H + h) * kGateFloats + tid * 4, true);
-    cp_async_commit();
-  };
-
-  uint32_t ph = 0;
-  bool dead = false;
-  auto wait_mma = [&]() {
-    if (!dead && !mbar_wait(mbar, ph & 1, 4000000u)) {
-      dead = true;
-      if (tid == 0) atomicAdd(&g_timeout_count_enc, 1u);
-    }
-    ++ph;
-    tc_fence_after();
-  };
-
-  if (nc > 0) load_stage(0, 0);
-  for (int c = 0; c < nc; ++c) {
-    const int st = c & 1;
-    if (c + 1 < nc) {
-      load_stage(c + 1, st ^ 1);
-      cp_async_wait<1>();
-    } else {
-      cp_async_wait<0>();
-    }
-    fence_proxy_async();
-    __syncthreads();
-    const uint8_t* stg = smem + st * kStageBytes;
-    const float* gt = reinterpret_cast<const float*>(stg + kStGate);
-    const uint32_t sb = smem_base + st * kStageBytes;
-
-    // ---- pass: Xr = rna_tf32(X); X <- gamma_C X  (c = 0: X is its initial value, 0 or I)
-    {
-      const float gC = gt[kC];
-#pragma unroll 1
-      for (int cb = 0; cb < 4; ++cb) {
-        uint32_t x[32];
-        if (c > 0) {
-          tmem_ld32(tX + 32 * cb, x);
-          tmem_ld_wait();
-        } else {
-#pragma unroll
-          for (int i = 0; i < 32; ++i) x[i] = (!is_e && 32 * cb + i == row) ? __float_as_uint(1.f) : 0u;
-        }
-        uint32_t xr[32], xs[32];
-#pragma unroll
-        for (int i = 0; i < 32; ++i) {
-          const float f = __uint_as_float(x[i]);
-          xr[i] = __float_as_uint(rna_tf32f(f));
-          xs[i] = __float_as_uint(f * gC);
-        }
-        tmem_st32(tXr + 32 * cb, xr);
-        tmem_st32(tX + 32 * cb, xs);
-      }
-      tmem_st_wait();
-    }
-    tc_fence_before();
-    __syncthreads();
-
-    // ---- (2) Wt = K^t A_bg^t, (1) DY = V^t A_b^t
-    if (tid == 0) {
-      tc_fence_after();
-      constexpr uint32_t id12 = make_idesc(1u, 128, 64, 1, 0);
-#pragma unroll
-      for (int hl = 0; hl < 2; ++hl)
-#pragma unroll
-        for (int ks = 0; ks < 4; ++ks) {
-          const uint64_t ad = make_desc(sb + kStK + ks * 2048, 8192, 1024, 2);
-          const uint64_t bd = make_desc(sb + kStAb + (2 + hl) * kTileB + ks * 32, 16, 1024, 2);
-          mma_f16_ss(tmem + 320, ad, bd, id12, (hl | ks) > 0);
-        }
-      if (is_e) {
-#pragma unroll
-        for (int hl = 0; hl < 2; ++hl)
-#pragma unroll
-          for (int ks = 0; ks < 4; ++ks) {
-            const uint64_t ad = make_desc(sb + kStV + ks * 2048, 8192, 1024, 2);
-            const uint64_t bd = make_desc(sb + kStAb + hl * kTileB + ks * 32, 16, 1024, 2);
-            mma_f16_ss(tmem + 256, ad, bd, id12, (hl | ks) > 0);
-          }
-      }
-      mma_commit(mbar);
-    }
-    __syncthreads();
-    wait_mma();
-
-    // ---- Wt -> -rna_tf32 -> smem B tile of (3): [k = dk row][n = token], 32-bit MN-major, 32B-base swizzle
-    {
-      uint8_t* wt = smem + kOffW;
-#pragma unroll 1
-      for (int nch = 0; nch < 2; ++nch) {
-        uint32_t w[32];
-        tmem_ld32(tWt + 32 * nch, w);
-        tmem_ld_wait();
-        uint8_t* base = wt + nch * 16384 + (row >> 2) * 512 + (row & 3) * 128;
-#pragma unroll
-        for (int q8 = 0; q8 < 4; ++q8) {
-          float4 lo4, hi4;
-          lo4.x = -rna_tf32f(__uint_as_float(w[8 * q8 + 0])), lo4.y = -rna_tf32f(__uint_as_float(w[8 * q8 + 1]));
-          lo4.z = -rna_tf32f(__uint_as_float(w[8 * q8 + 2])), lo4.w = -rna_tf32f(__uint_as_float(w[8 * q8 + 3]));
-          hi4.x = -rna_tf32f(__uint_as_float(w[8 * q8 + 4])), hi4.y = -rna_tf32f(__uint_as_float(w[8 * q8 + 5]));
-          hi4.z = -rna_tf32f(__uint_as_float(w[8 * q8 + 6])), hi4.w = -rna_tf32f(__uint_as_float(w[8 * q8 + 7]));
-          uint8_t* p = base + ((q8 ^ (row & 3)) * 32);
-          *reinterpret_cast<float4*>(p) = lo4;
-          *reinterpret_cast<float4*>(p + 16) = hi4;
-        }
-      }
-    }
-    fence_proxy_async();
-    tc_fence_before();
-    __syncthreads();
-
-    // ---- (3) DY (+)= Xr (-W)^t
-    if (tid == 0) {
-      tc_fence_after();
-      constexpr uint32_t id3 = make_idesc(2u, 128, 64, 0, 1);
-#pragma unroll
-      for (int ks = 0; ks < 16; ++ks) {
-        const uint64_t bd = make_desc(smem_base + kOffW + ks * 1024, 16384, 512, 1);
-        mma_tf32_ts(tmem + 256, tmem + 128 + ks * 8, bd, id3, (is_e || ks > 0) ? 1u : 0u);
-      }
-      mma_commit(mbar);
-    }
-    __syncthreads();
-    wait_mma();
-
-    // ---- DY * d_j -> bf16 hi/lo -> K-major A tiles of (4)
-    {
-      uint8_t* uhi = smem + kOffUhi + (row >> 3) * 1024 + (row & 7) * 128;
-      uint8_t* ulo = smem + kOffUlo + (row >> 3) * 1024 + (row & 7) * 128;
-#pragma unroll 1
-      for (int half = 0; half < 2; ++half) {
-        uint32_t y[32];
-        tmem_ld32(tDY + 32 * half, y);
-        tmem_ld_wait();
-#pragma unroll
-        for (int j8 = 0; j8 < 4; ++j8) {
-          uint32_t hi[4], lo[4];
-#pragma unroll
-          for (int p = 0; p < 4; ++p) {
-            const int j = 32 * half + 8 * j8 + 2 * p;
-            const float u0 = __uint_as_float(y[8 * j8 + 2 * p]) * gt[j];
-            const float u1 = __uint_as_float(y[8 * j8 + 2 * p + 1]) * gt[j + 1];
-            const float h0 = __bfloat162float(__float2bfloat16_rn(u0)), h1 = __bfloat162float(__float2bfloat16_rn(u1));
-            hi[p] = pack_bf16(h0, h1);
-            lo[p] = pack_bf16(u0 - h0, u1 - h1);
-          }
-          const int chunk = 4 * half + j8;
-          const uint32_t sw = ((chunk ^ (row & 7)) * 16);
-          *reinterpret_cast<uint4*>(uhi + sw) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-          *reinterpret_cast<uint4*>(ulo + sw) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
-        }
-      }
-    }
-    fence_proxy_async();
-    tc_fence_before();
-    __syncthreads();
-
-    // ---- (4) X += U'' K
-    if (tid == 0) {
-      tc_fence_after();
-      constexpr uint32_t id4 = make_idesc(1u, 128, 128, 0, 1);
-#pragma unroll
-      for (int hl = 0; hl < 2; ++hl)
-#pragma unroll
-        for (int ks = 0; ks < 4; ++ks) {
-          const uint64_t ad = make_desc(smem_base + (hl ? kOffUlo : kOffUhi) + ks * 32, 16, 1024, 2);
-          const uint64_t bd = make_desc(sb + kStK + ks * 2048, 8192, 1024, 2);
-          mma_f16_ss(tmem, ad, bd, id4, 1u);
-        }
-      mma_commit(mbar);
-    }
-    __syncthreads();
-    wait_mma();
-  }
-
-  // ---- a5: write the block out (thread = row)
-  {
-    float* dst = (is_e ? E : T) + (((size_t)s * H + h) * kD + row) * kD;
-#pragma unroll 1
-    for (int cb = 0; cb < 4; ++cb) {
-      uint32_t x[32];
-      if (nc > 0) {
-        tmem_ld32(tX + 32 * cb, x);
-        tmem_ld_wait();
-      } else {
-#pragma unroll
-        for (int i = 0; i < 32; ++i) x[i] = (!is_e && 32 * cb + i == row) ? __float_as_uint(1.f) : 0u;
-      }
-      float4* d4 = reinterpret_cast<float4*>(dst + 32 * cb);
-#pragma unroll
-      for (int u = 0; u < 8; ++u)
-        d4[u] = make_float4(__uint_as_float(x[4 * u]), __uint_as_float(x[4 * u + 1]), __uint_as_float(x[4 * u + 2]),
-                            __uint_as_float(x[4 * u + 3]));
-    }
-  }
-  tc_fence_before();
-  __syncthreads();
-  if (warp == 0) tmem_dealloc(tmem, 512);
-}
-
-#include "encode_scan_ws.cuh"
+#include "encode_scan2.cuh"
 
 // k / v viewed as 3-D bf16 tensors [t_total][H][128]; box = 64 elements (128 B) x 1 head x 64 tokens, 128B swizzle:
 // the box lands as one MN-major UMMA chunk (8-token atoms of 1 KB), two boxes per 64 x 128 tile.
@@ -554,6 +338,16 @@ int make_kv_tensor_map(CUtensorMap* tm, const void* base, int32_t t_total, int32
   return r == CUDA_SUCCESS ? HYPIC_OK : HYPIC_ERR_CUDA;
 }
 
+// E = 0, T = I for every (segment, head) when the call carries no tokens at all (no tensor map can be built).
+__global__ void identity_fill_kernel(float* __restrict__ E, float* __restrict__ T, size_t n_units) {
+  const size_t n = n_units * kD * kD;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    E[i] = 0.f;
+    const size_t e = i % (kD * kD);
+    T[i] = (e / kD == e % kD) ? 1.f : 0.f;
+  }
+}
+
 }  // namespace
 
 bool encode_tensor_shape_ok(int32_t, int32_t dk, int32_t dv, int kv_dtype, int gate) {
@@ -564,7 +358,7 @@ size_t encode_tensor_workspace(int32_t n_seg, int32_t t_total, int32_t H, int32_
                                int gate) {
   if (!encode_tensor_shape_ok(H, dk, dv, kv_dtype, gate)) return 0;
   const size_t cap = chunk_cap(n_seg, t_total);
-  return ws_off_ab(n_seg) + cap * H * ((size_t)kAbBytes + kGateBytes);
+  return ws_off_rec(n_seg) + cap * H * ((size_t)kRecBytes + kGateBytes);
 }
 
 int encode_tensor(const EncodeArgs& a) {
@@ -573,44 +367,33 @@ int encode_tensor(const EncodeArgs& a) {
   if (a.H > 65535 || a.n_seg > 65535) return HYPIC_ERR_UNSUPPORTED;
   const size_t cap = chunk_cap(a.n_seg, a.t_total);
   if (cap > 0x7fffffffULL) return HYPIC_ERR_UNSUPPORTED;
+  if (a.t_total == 0) {
+    identity_fill_kernel<<<296, 256, 0, a.stream>>>(a.E, a.T, (size_t)a.n_seg * a.H);
+    note_launch();
+    HYPIC_CUDA_OK(cudaGetLastError());
+    return HYPIC_OK;
+  }
   uint8_t* ws = static_cast<uint8_t*>(a.workspace);
   int32_t* chunk_off = reinterpret_cast<int32_t*>(ws);
-  uint8_t* ab = ws + ws_off_ab(a.n_seg);
-  float* gate = reinterpret_cast<float*>(ab + cap * a.H * (size_t)kAbBytes);
+  uint8_t* rec = ws + ws_off_rec(a.n_seg);
+  float* gate = reinterpret_cast<float*>(rec + cap * a.H * (size_t)kRecBytes);
   static bool configured = false;
   if (!configured) {
-    HYPIC_CUDA_OK(cudaFuncSetAttribute(scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kScanSmem));
+    HYPIC_CUDA_OK(cudaFuncSetAttribute(scan2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kS2Smem));
     configured = true;
   }
   const auto* kp = static_cast<const __nv_bfloat16*>(a.k);
-  const auto* vp = static_cast<const __nv_bfloat16*>(a.v);
+  CUtensorMap tmK, tmV;
+  int rc = make_kv_tensor_map(&tmK, a.k, a.t_total, a.H);
+  if (rc == HYPIC_OK) rc = make_kv_tensor_map(&tmV, a.v, a.t_total, a.H);
+  if (rc != HYPIC_OK) return rc;
   chunk_offsets_kernel<<<1, 1024, 0, a.stream>>>(a.cu_seqlens, a.n_seg, chunk_off);
   note_launch();
-  if (cap > 0) {
-    prep_kernel<<<dim3((unsigned)cap, a.H), kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, a.cu_seqlens, chunk_off,
-                                                                         a.n_seg, a.H, ab, gate);
-    note_launch();
-  }
-  static const bool use_v1 = [] {
-    const char* e = getenv("HYPIC_SCAN_V1");  // diagnostics: the lock-step 128-thread scan kernel
-    return e != nullptr && e[0] == '1';
-  }();
-  if (use_v1 || a.t_total == 0) {
-    scan_kernel<<<dim3(2, a.H, a.n_seg), kScanThreads, kScanSmem, a.stream>>>(kp, vp, a.cu_seqlens, chunk_off, a.H, ab,
-                                                                              gate, a.E, a.T);
-  } else {
-    static bool configured_ws = false;
-    if (!configured_ws) {
-      HYPIC_CUDA_OK(cudaFuncSetAttribute(scan_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kWsSmem));
-      configured_ws = true;
-    }
-    CUtensorMap tmK, tmV;
-    int rc = make_kv_tensor_map(&tmK, a.k, a.t_total, a.H);
-    if (rc == HYPIC_OK) rc = make_kv_tensor_map(&tmV, a.v, a.t_total, a.H);
-    if (rc != HYPIC_OK) return rc;
-    scan_ws_kernel<<<dim3(2, a.H, a.n_seg), kWsThreads, kWsSmem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, a.H, ab,
-                                                                            gate, a.E, a.T);
-  }
+  prep_kernel<<<dim3((unsigned)cap, a.H), kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, a.cu_seqlens, chunk_off,
+                                                                       a.n_seg, a.H, rec, gate);
+  note_launch();
+  scan2_kernel<<<dim3(a.H, a.n_seg), kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, a.H, rec, gate,
+                                                                     a.E, a.T);
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
   return HYPIC_OK;
