@@ -17,6 +17,18 @@
 // DY_T [448,512).  All waits are bounded; a protocol error bumps g_timeout_count_enc instead of hanging the GPU.
 #pragma once
 
+// Diagnostics only (-DHYPIC_TIMELINE, never in the shipped library): per-chunk clock stamps of CTA (0, 0).
+#ifdef HYPIC_TIMELINE
+__device__ long long g_s2_timeline[3 * 64 * 8];
+#define S2_STAMP(role, c, k)                                                                   \
+  do {                                                                                         \
+    if (blockIdx.x == 0 && blockIdx.y == 0 && (c) < 64 && (threadIdx.x & 31) == 0 && ((threadIdx.x >> 5) & 3) == ((role) == 2 ? 1 : 0)) \
+      g_s2_timeline[((role) * 64 + (c)) * 8 + (k)] = clock64();                                \
+  } while (0)
+#else
+#define S2_STAMP(role, c, k) do {} while (0)
+#endif
+
 constexpr int kS2Threads = 384;
 constexpr int kS2StK = 0, kS2StV = 16384, kS2StRec = 32768, kS2StGate = 65536;
 constexpr int kS2StageBytes = 65536 + 1024;
@@ -101,6 +113,7 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     s2_wait(&bars->st_full[c & 1], (c >> 1) & 1, abort_flag);
     if (c > 0) s2_wait(&bars->m4_done[b], (c - 1) & 1, abort_flag);
     tc_fence_after();
+    S2_STAMP(b, c, 0);
     const float gC = gt[kC];
     // ---- pass: Xh = fp16(X 2^-s) (A operand of (3)), X <- gamma_C X
     float inv_scale = 1.f;
@@ -156,11 +169,13 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     tmem_st_wait();
     tc_fence_before();
     __syncwarp();
+    S2_STAMP(b, c, 1);
     if (lane == 0) mbar_arrive(&bars->xh_ready[b]);
 
     // ---- epilogue: U''[:, j] = DY[:, j] d_j 2^s -> bf16 hi + lo, K-major 128B swizzle (A operand of (4))
     s2_wait(&bars->m3_done[b], c & 1, abort_flag);
     tc_fence_after();
+    S2_STAMP(b, c, 2);
 #pragma unroll
     for (int half = 0; half < 2; ++half) {
       uint32_t y[32];
@@ -189,6 +204,7 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     fence_proxy_async();
     tc_fence_before();
     __syncwarp();
+    S2_STAMP(b, c, 3);
     if (lane == 0) mbar_arrive(&bars->u_ready[b]);
   }
 
@@ -310,21 +326,25 @@ __global__ void __launch_bounds__(kS2Threads, 1)
           const int c = cc[b];
           if (c >= nc) continue;
           if (at3[b]) {
-            if (!mbar_try_wait(&bars->xh_ready[b], c & 1)) continue;
+            if (!mbar_test_wait(&bars->xh_ready[b], c & 1)) continue;
             if (c > seen) {
               ok = s2_wait(&bars->st_full[c & 1], (c >> 1) & 1, abort_flag);
               seen = c;
             }
             tc_fence_after();
+            S2_STAMP(2, c, 0 + 4 * b);
             issue3(b, c);
             mma_commit(&bars->m3_done[b]);
+            S2_STAMP(2, c, 1 + 4 * b);
             at3[b] = false;
             progress = true;
           } else {
-            if (!mbar_try_wait(&bars->u_ready[b], c & 1)) continue;
+            if (!mbar_test_wait(&bars->u_ready[b], c & 1)) continue;
             tc_fence_after();
+            S2_STAMP(2, c, 2 + 4 * b);
             issue4(b, c);
             mma_commit(&bars->m4_done[b]);
+            S2_STAMP(2, c, 3 + 4 * b);
             if (cc[b ^ 1] > c) mma_commit(&bars->st_free[c & 1]);  // the other chain is already past this chunk
             cc[b] = c + 1;
             at3[b] = true;

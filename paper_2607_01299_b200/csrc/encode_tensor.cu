@@ -399,6 +399,12 @@ int encode_tensor(const EncodeArgs& a) {
   return HYPIC_OK;
 }
 
+#ifdef HYPIC_TIMELINE
+extern "C" int hypic_debug_timeline(long long* out, int n) {
+  return cudaMemcpyFromSymbol(out, g_s2_timeline, sizeof(long long) * (size_t)n) == cudaSuccess ? 0 : 1;
+}
+#endif
+
 unsigned int debug_timeout_count_encode() {
   unsigned int v = 0;
   if (cudaMemcpyFromSymbol(&v, g_timeout_count_enc, sizeof(v)) != cudaSuccess) return 0xffffffffu;
