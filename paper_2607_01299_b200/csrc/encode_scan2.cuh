@@ -2,16 +2,26 @@
 // Included by encode_tensor.cu inside namespace hypic::{anonymous}; uses its constants and helpers.
 //
 // One CTA per (segment, head), sequential over the segment's 64-token chunks; both row blocks of the stacked state
-// X = [E ; T] (128 rows each) stay in TMEM as fp32 for the whole segment.  12 warps:
-//   warp 0       loader      TMA tensor boxes for the K / V chunk tiles, bulk copies for the prep record (W, A_b hi/lo)
-//                            and the gate record; two stages, one mbarrier per stage
-//   warp 1       MMA issuer  one thread, polls the two chains and issues whichever step is ready:
-//                              (1)_c  DY_E  = V^t A_b^t               bf16 hi + lo                  (E block only)
-//                              (3)_c  DY_b += Xh_b W^t                fp16, A = Xh_b from TMEM, B = W from smem
-//                              (4)_c  X_b  += U''_b K                 bf16 hi + lo, B = the K tile
-//   warps 4-7    E chain     thread = row of E:  pass: Xh = fp16(X), X <- gamma_C X;  epilogue: DY d_j -> U'' hi/lo
-//   warps 8-11   T chain     same for T, with a per-row power-of-two scale so that fp16(T 2^-s) keeps 11 significant
-//                            bits however far the row has decayed; the scale is undone in the epilogue (fp32).
+// X = [E ; T] (128 rows each) stay in TMEM as fp32 for the whole segment.  Every contraction is a single-pass
+// tcgen05.mma kind::f16 on fp16 operands (11 significant bits, like tf32, at the full 16-bit rate):
+//     (1)_c  DY_E  = V^t A_b^t              A = the V tile (MN-major), B = A_b from the prep record   (E block only)
+//     (3)_c  DY_b += Xh_b (-W)^t            A = Xh_b = fp16(X_b) read from TMEM, B = -W from the prep record
+//     (4)_c  X_b  += U''_b K                A = U''_b = fp16(DY_b d_j) from smem, B = the K tile (MN-major)
+// fp16 has a narrow exponent range, so the T block is held row-normalised: row r of the TMEM copy is T_r 2^s_r with
+// s_r re-chosen in every pass so that the row maximum sits in [2^14, 2^15); since (3) and (4) are linear in the row
+// the factor never has to be undone before the final write-out.  E rows live on the scale of v and stay unscaled.
+// k / v arrive as bf16 and are converted to fp16 in place in shared memory (exact for |x| in [2^-14, 65504]).
+//
+// 20 warps:
+// (the warp scheduler favours the highest warp id of an SM sub-partition, so the latency-critical single-thread
+// roles sit at the top):
+//   warps 0-7     E chain     thread = (row of E, 64-column half): pass  Xh = fp16(X), X <- gamma_C X;
+//                             epilogue  U'' = fp16(DY d_j)
+//   warps 8-15    T chain     same for T plus the row re-normalisation
+//   warps 16-17   converters  K (warp 16) and V (warp 17) tile bf16 -> fp16 in place; warp 16 also owns TMEM alloc
+//   warp 18       loader      TMA tensor boxes for the K / V chunk tiles, bulk copies for the prep record (-W, A_b)
+//                             and the gate record; three stages
+//   warp 19       MMA issuer  one thread; polls the two chains and issues whichever step is ready
 // The two chains only share read-only operands, so while one is in its element-wise phase the tensor pipe runs the
 // other one's MMAs.  TMEM columns: X_E [0,128), X_T [128,256), Xh_E [256,320), Xh_T [320,384), DY_E [384,448),
 // DY_T [448,512).  All waits are bounded; a protocol error bumps g_timeout_count_enc instead of hanging the GPU.
@@ -19,25 +29,34 @@
 
 // Diagnostics only (-DHYPIC_TIMELINE, never in the shipped library): per-chunk clock stamps of CTA (0, 0).
 #ifdef HYPIC_TIMELINE
-__device__ long long g_s2_timeline[3 * 64 * 8];
-#define S2_STAMP(role, c, k)                                                                   \
-  do {                                                                                         \
-    if (blockIdx.x == 0 && blockIdx.y == 0 && (c) < 64 && (threadIdx.x & 31) == 0 && ((threadIdx.x >> 5) & 3) == ((role) == 2 ? 1 : 0)) \
-      g_s2_timeline[((role) * 64 + (c)) * 8 + (k)] = clock64();                                \
+__device__ long long g_s2_timeline[4 * 64 * 8];
+#define S2_STAMP(role, c, k)                                                                              \
+  do {                                                                                                    \
+    if (blockIdx.x == 0 && blockIdx.y == 0 && (c) < 64 && (threadIdx.x & 31) == 0 &&                      \
+        (threadIdx.x >> 5) == ((role) >= 2 ? 19 : ((role) == 0 ? 0 : 8)))                                 \
+      g_s2_timeline[((role) * 64 + (c)) * 8 + (k)] = clock64();                                           \
+  } while (0)
+#define S2_STAMPW(w, role, c, k)                                                                          \
+  do {                                                                                                    \
+    if (blockIdx.x == 0 && blockIdx.y == 0 && (c) < 64 && (threadIdx.x & 31) == 0 && (threadIdx.x >> 5) == (w)) \
+      g_s2_timeline[((role) * 64 + (c)) * 8 + (k)] = clock64();                                           \
   } while (0)
 #else
 #define S2_STAMP(role, c, k) do {} while (0)
+#define S2_STAMPW(w, role, c, k) do {} while (0)
 #endif
 
-constexpr int kS2Threads = 384;
-constexpr int kS2StK = 0, kS2StV = 16384, kS2StRec = 32768, kS2StGate = 65536;
-constexpr int kS2StageBytes = 65536 + 1024;
-constexpr int kS2OffU = 2 * kS2StageBytes;         // per block b: U'' hi (16 KB) | lo (16 KB)
-constexpr int kS2OffBar = kS2OffU + 2 * 32768;
+constexpr int kS2Threads = 640;
+constexpr int kS2Stages = 3;
+constexpr int kS2StK = 0, kS2StV = 16384, kS2StRec = 32768, kS2StGate = 32768 + kRecBytes;
+constexpr int kS2StageBytes = 32768 + kRecBytes + 1024;
+constexpr int kS2OffU = kS2Stages * kS2StageBytes;  // per block b: U'' (fp16, 16 KB)
+constexpr int kS2OffXch = kS2OffU + 2 * 16384;      // T chain: row maxima of the two column halves
+constexpr int kS2OffBar = kS2OffXch + 1024;
 constexpr int kS2Smem = kS2OffBar + 256 + 1024;
 
 struct S2Bars {
-  uint64_t st_full[2], st_free[2];
+  uint64_t st_full[kS2Stages], st_conv[kS2Stages], st_free[kS2Stages];
   uint64_t xh_ready[2], m3_done[2], u_ready[2], m4_done[2];  // [block]: 0 = E, 1 = T
   uint32_t tmem_base;
   int abort_flag;
@@ -54,9 +73,9 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst_smem, const CUtensorMap
 
 __device__ __noinline__ bool s2_wait(uint64_t* bar, uint32_t parity, volatile int* abort_flag) {
 #pragma unroll 1
-  for (uint32_t i = 0; i < 4000000u; ++i) {
-    if (mbar_try_wait(bar, parity)) return true;
-    if ((i & 1023u) == 1023u && *abort_flag) return false;
+  for (uint32_t i = 0; i < 400000u; ++i) {
+    if (mbar_try_wait_hint(bar, parity, 20000u)) return true;
+    if ((i & 63u) == 63u && *abort_flag) return false;
   }
   if (!*abort_flag) {
     *abort_flag = 1;
@@ -73,132 +92,135 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
       "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
       : "memory");
 }
-// (a, b) <- (a, b) * s  as one packed fp32x2 multiply
-__device__ __forceinline__ void mul2(uint32_t& a, uint32_t& b, float s) {
-  asm("{\n\t.reg .b64 t, u;\n\tmov.b64 t, {%0, %1};\n\tmov.b64 u, {%2, %2};\n\tmul.rn.f32x2 t, t, u;\n\tmov.b64 {%0, %1}, t;\n\t}"
-      : "+r"(a), "+r"(b)
-      : "r"(__float_as_uint(s)));
-}
+// (a, b) <- (a, b) * (s0, s1)  as one packed fp32x2 multiply
 __device__ __forceinline__ void mul2v(uint32_t& a, uint32_t& b, float s0, float s1) {
   asm("{\n\t.reg .b64 t, u;\n\tmov.b64 t, {%0, %1};\n\tmov.b64 u, {%2, %3};\n\tmul.rn.f32x2 t, t, u;\n\tmov.b64 {%0, %1}, t;\n\t}"
       : "+r"(a), "+r"(b)
       : "r"(__float_as_uint(s0)), "r"(__float_as_uint(s1)));
 }
+__device__ __forceinline__ void mul2(uint32_t& a, uint32_t& b, float s) { mul2v(a, b, s, s); }
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ float pow2i(int e) { return __uint_as_float((uint32_t)(127 + e) << 23); }  // e in [-126, 127]
 
 template <bool kIsT>
-__device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile int* abort_flag, uint32_t tmem, int warp,
-                                         int lane, int nc, float* __restrict__ dst_row) {
+__device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile int* abort_flag, uint32_t tmem, int cw,
+                                         int lane, int nc, float* __restrict__ dst_block) {
   constexpr int b = kIsT ? 1 : 0;
   constexpr uint32_t cX = kIsT ? 128 : 0, cH = kIsT ? 320 : 256, cD = kIsT ? 448 : 384;
-  const int q = warp & 3;
+  const int q = cw & 3, hf = cw >> 2;  // TMEM lane quarter; column half
   const int row = 32 * q + lane;
   const uint32_t lane_base = (uint32_t)(32 * q) << 16;
-  const uint32_t tX = tmem + cX + lane_base, tH = tmem + cH + lane_base, tD = tmem + cD + lane_base;
-  uint8_t* uhi = smem + kS2OffU + b * 32768 + (row >> 3) * 1024 + (row & 7) * 128;
-  uint8_t* ulo = uhi + 16384;
+  const uint32_t tX = tmem + cX + lane_base + 64 * hf, tH = tmem + cH + lane_base + 32 * hf,
+                 tD = tmem + cD + lane_base + 32 * hf;
+  uint8_t* urow = smem + kS2OffU + b * 16384 + (row >> 3) * 1024 + (row & 7) * 128;
+  float* xch = reinterpret_cast<float*>(smem + kS2OffXch);
+  int s_exp = 0;  // T chain: the TMEM copy of this row is T_row * 2^s_exp
 
   // X_0 = [0 ; I]
 #pragma unroll
-  for (int cb = 0; cb < 4; ++cb) {
+  for (int cb = 0; cb < 2; ++cb) {
     uint32_t x[32];
 #pragma unroll
-    for (int i = 0; i < 32; ++i) x[i] = (kIsT && 32 * cb + i == row) ? __float_as_uint(1.f) : 0u;
+    for (int i = 0; i < 32; ++i) x[i] = (kIsT && 64 * hf + 32 * cb + i == row) ? __float_as_uint(1.f) : 0u;
     tmem_st32(tX + 32 * cb, x);
   }
   tmem_st_wait();
 
 #pragma unroll 1
   for (int c = 0; c < nc; ++c) {
-    const float* gt = reinterpret_cast<const float*>(smem + (c & 1) * kS2StageBytes + kS2StGate);
-    s2_wait(&bars->st_full[c & 1], (c >> 1) & 1, abort_flag);
+    const int st = c % kS2Stages;
+    const float* gt = reinterpret_cast<const float*>(smem + st * kS2StageBytes + kS2StGate);
+    s2_wait(&bars->st_full[st], (c / kS2Stages) & 1, abort_flag);
     if (c > 0) s2_wait(&bars->m4_done[b], (c - 1) & 1, abort_flag);
     tc_fence_after();
     S2_STAMP(b, c, 0);
     const float gC = gt[kC];
-    // ---- pass: Xh = fp16(X 2^-s) (A operand of (3)), X <- gamma_C X
-    float inv_scale = 1.f;
-    float scale = 1.f;
-    if (kIsT) {
-      float m = 0.f;
-#pragma unroll
-      for (int hb = 0; hb < 2; ++hb) {
-        uint32_t x0[32], x1[32];
-        tmem_ld32(tX + 64 * hb, x0);
-        tmem_ld32(tX + 64 * hb + 32, x1);
-        tmem_ld_wait();
+    // ---- pass: Xh = fp16(X) (A operand of (3)), X <- gamma_C X; T rows are re-normalised on the way
+    {
+      uint32_t x0[32], x1[32];
+      tmem_ld32(tX, x0);
+      tmem_ld32(tX + 32, x1);
+      tmem_ld_wait();
+      S2_STAMP(b, c, 4);
+      float f = gC;
+      if (kIsT) {
+        float m = 0.f;
 #pragma unroll
         for (int i = 0; i < 32; ++i) m = fmaxf(m, fmaxf(fabsf(__uint_as_float(x0[i])), fabsf(__uint_as_float(x1[i]))));
-      }
-      // row maximum in [2^(e-127), 2^(e-126)): scale it into [2^14, 2^15)
-      uint32_t e = __float_as_uint(m) >> 23;
-      e = e < 14u ? 14u : e;
-      scale = __uint_as_float((268u - e) << 23);
-      inv_scale = __uint_as_float((e - 14u) << 23);
-    }
-#pragma unroll
-    for (int hb = 0; hb < 2; ++hb) {
-      uint32_t x0[32], x1[32], hh[32];
-      tmem_ld32(tX + 64 * hb, x0);
-      tmem_ld32(tX + 64 * hb + 32, x1);
-      tmem_ld_wait();
-      if (kIsT) {
+        xch[2 * row + hf] = m;
+        named_bar_sync(1 + q, 64);
+        m = fmaxf(m, xch[2 * row + (hf ^ 1)]);
+        S2_STAMP(b, c, 5);
+        // row maximum in [2^(e-127), 2^(e-126)): move it to [2^14, 2^15)
+        const int e = (int)(__float_as_uint(m) >> 23);
+        int dlt = (e == 0) ? 0 : 141 - e;
+        dlt = max(-100, min(100, dlt));
+        s_exp += dlt;
+        const float sc = pow2i(dlt);
+        f = gC * sc;
+        uint32_t hh[16];
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
-          uint32_t a0 = x0[2 * j], a1 = x0[2 * j + 1], b0 = x1[2 * j], b1 = x1[2 * j + 1];
-          mul2(a0, a1, scale);
-          mul2(b0, b1, scale);
+          uint32_t a0 = x0[2 * j], a1 = x0[2 * j + 1];
+          mul2(a0, a1, sc);
           hh[j] = pack_f16(__uint_as_float(a0), __uint_as_float(a1));
-          hh[16 + j] = pack_f16(__uint_as_float(b0), __uint_as_float(b1));
         }
-      } else {
+        tmem_st16(tH, hh);
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
-          hh[j] = pack_f16(__uint_as_float(x0[2 * j]), __uint_as_float(x0[2 * j + 1]));
-          hh[16 + j] = pack_f16(__uint_as_float(x1[2 * j]), __uint_as_float(x1[2 * j + 1]));
+          uint32_t a0 = x1[2 * j], a1 = x1[2 * j + 1];
+          mul2(a0, a1, sc);
+          hh[j] = pack_f16(__uint_as_float(a0), __uint_as_float(a1));
         }
+        tmem_st16(tH + 16, hh);
+      } else {
+        uint32_t hh[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x0[2 * j]), __uint_as_float(x0[2 * j + 1]));
+        tmem_st16(tH, hh);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x1[2 * j]), __uint_as_float(x1[2 * j + 1]));
+        tmem_st16(tH + 16, hh);
       }
-      tmem_st32(tH + 32 * hb, hh);
 #pragma unroll
       for (int j = 0; j < 16; ++j) {
-        mul2(x0[2 * j], x0[2 * j + 1], gC);
-        mul2(x1[2 * j], x1[2 * j + 1], gC);
+        mul2(x0[2 * j], x0[2 * j + 1], f);
+        mul2(x1[2 * j], x1[2 * j + 1], f);
       }
-      tmem_st32(tX + 64 * hb, x0);
-      tmem_st32(tX + 64 * hb + 32, x1);
+      tmem_st32(tX, x0);
+      tmem_st32(tX + 32, x1);
+      S2_STAMP(b, c, 6);
+      tmem_st_wait();
     }
-    tmem_st_wait();
     tc_fence_before();
     __syncwarp();
     S2_STAMP(b, c, 1);
     if (lane == 0) mbar_arrive(&bars->xh_ready[b]);
 
-    // ---- epilogue: U''[:, j] = DY[:, j] d_j 2^s -> bf16 hi + lo, K-major 128B swizzle (A operand of (4))
+    // ---- epilogue: U''[:, j] = fp16(DY[:, j] d_j), K-major 128B swizzle (A operand of (4)); tokens [32 hf, 32 hf + 32)
     s2_wait(&bars->m3_done[b], c & 1, abort_flag);
     tc_fence_after();
     S2_STAMP(b, c, 2);
-#pragma unroll
-    for (int half = 0; half < 2; ++half) {
+    {
       uint32_t y[32];
-      tmem_ld32(tD + 32 * half, y);
+      tmem_ld32(tD, y);
       tmem_ld_wait();
+      S2_STAMP(b, c, 7);
 #pragma unroll
       for (int j8 = 0; j8 < 4; ++j8) {
-        const float4 d0 = *reinterpret_cast<const float4*>(gt + 32 * half + 8 * j8);
-        const float4 d1 = *reinterpret_cast<const float4*>(gt + 32 * half + 8 * j8 + 4);
+        const float4 d0 = *reinterpret_cast<const float4*>(gt + 32 * hf + 8 * j8);
+        const float4 d1 = *reinterpret_cast<const float4*>(gt + 32 * hf + 8 * j8 + 4);
         const float dd[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
-        uint32_t hi[4], lo[4];
+        uint32_t u[4];
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
           uint32_t u0 = y[8 * j8 + 2 * p], u1 = y[8 * j8 + 2 * p + 1];
-          if (kIsT) mul2(u0, u1, inv_scale);
           mul2v(u0, u1, dd[2 * p], dd[2 * p + 1]);
-          hi[p] = pack_bf16(__uint_as_float(u0), __uint_as_float(u1));
-          lo[p] = pack_bf16(__uint_as_float(u0) - __uint_as_float(hi[p] << 16),
-                            __uint_as_float(u1) - __uint_as_float(hi[p] & 0xffff0000u));
+          u[p] = pack_f16(__uint_as_float(u0), __uint_as_float(u1));
         }
-        const uint32_t sw = (((4 * half + j8) ^ (row & 7)) * 16);
-        *reinterpret_cast<uint4*>(uhi + sw) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-        *reinterpret_cast<uint4*>(ulo + sw) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+        *reinterpret_cast<uint4*>(urow + (((4 * hf + j8) ^ (row & 7)) * 16)) = make_uint4(u[0], u[1], u[2], u[3]);
       }
     }
     fence_proxy_async();
@@ -208,21 +230,32 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     if (lane == 0) mbar_arrive(&bars->u_ready[b]);
   }
 
-  // ---- a5: write the row out
+  // ---- a5: write this thread's 64 columns of its row (T: undo the row normalisation, in two exact steps)
   if (nc > 0) {
     s2_wait(&bars->m4_done[b], (nc - 1) & 1, abort_flag);
     tc_fence_after();
   }
+  const int se = max(-250, min(250, s_exp));
+  const float f0 = pow2i(-(se / 2)), f1 = pow2i(-(se - se / 2));
+  float* dst = dst_block + (size_t)row * kD + 64 * hf;
 #pragma unroll 1
-  for (int cb = 0; cb < 4; ++cb) {
+  for (int cb = 0; cb < 2; ++cb) {
     uint32_t x[32];
     tmem_ld32(tX + 32 * cb, x);
     tmem_ld_wait();
-    float4* d4 = reinterpret_cast<float4*>(dst_row + 32 * cb);
+    float4* d4 = reinterpret_cast<float4*>(dst + 32 * cb);
 #pragma unroll
-    for (int u = 0; u < 8; ++u)
-      d4[u] = make_float4(__uint_as_float(x[4 * u]), __uint_as_float(x[4 * u + 1]), __uint_as_float(x[4 * u + 2]),
-                          __uint_as_float(x[4 * u + 3]));
+    for (int u = 0; u < 8; ++u) {
+      float4 o = make_float4(__uint_as_float(x[4 * u]), __uint_as_float(x[4 * u + 1]), __uint_as_float(x[4 * u + 2]),
+                             __uint_as_float(x[4 * u + 3]));
+      if (kIsT) {
+        o.x = o.x * f0 * f1;
+        o.y = o.y * f0 * f1;
+        o.z = o.z * f0 * f1;
+        o.w = o.w * f0 * f1;
+      }
+      d4[u] = o;
+    }
   }
 }
 
@@ -241,14 +274,17 @@ __global__ void __launch_bounds__(kS2Threads, 1)
   const int nc = (seg_end - seg_begin + kC - 1) / kC;
   const int chunk0 = chunk_off[s];
 
-  if (warp == 2) tmem_alloc(&bars->tmem_base, 512);
+  if (warp == 16) tmem_alloc(&bars->tmem_base, 512);
   if (tid == 0) {
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < kS2Stages; ++i) {
       mbar_init(&bars->st_full[i], 1);
+      mbar_init(&bars->st_conv[i], 2);
       mbar_init(&bars->st_free[i], 1);
-      mbar_init(&bars->xh_ready[i], 4);
+    }
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(&bars->xh_ready[i], 8);
       mbar_init(&bars->m3_done[i], 1);
-      mbar_init(&bars->u_ready[i], 4);
+      mbar_init(&bars->u_ready[i], 8);
       mbar_init(&bars->m4_done[i], 1);
     }
     bars->abort_flag = 0;
@@ -260,14 +296,15 @@ __global__ void __launch_bounds__(kS2Threads, 1)
   const uint32_t tmem = bars->tmem_base;
   const uint32_t smem_base = smem_u32(smem);
 
-  if (warp == 0) {
+  if (warp == 18) {
     // ------------------------------------------------------------------------------------------- loader
     if (lane == 0) {
       constexpr uint32_t bytes = 32768u + (uint32_t)kRecBytes + (uint32_t)kGateBytes;
 #pragma unroll 1
       for (int c = 0; c < nc; ++c) {
-        const int st = c & 1;
-        s2_wait(&bars->st_free[st], ((c >> 1) & 1) ^ 1, abort_flag);
+        const int st = c % kS2Stages;
+        s2_wait(&bars->st_free[st], ((c / kS2Stages) & 1) ^ 1, abort_flag);
+        S2_STAMPW(18, 3, c, 5);
         const uint32_t sb = smem_base + st * kS2StageBytes;
         const int t0 = seg_begin + c * kC;
         mbar_expect_tx(&bars->st_full[st], bytes);
@@ -280,23 +317,21 @@ __global__ void __launch_bounds__(kS2Threads, 1)
         bulk_g2s(smem + st * kS2StageBytes + kS2StGate, gate + r * kGateFloats, kGateBytes, &bars->st_full[st]);
       }
     }
-  } else if (warp == 1) {
+  } else if (warp == 19) {
     // ------------------------------------------------------------------------------------------- MMA issuer
     if (lane == 0 && nc > 0) {
-      constexpr uint32_t id1 = make_idesc(1u, 128, 64, 1, 0);    // bf16, A MN-major (V tile), B K-major (A_b)
-      constexpr uint32_t id3 = make_idesc(0u, 128, 64, 0, 0);    // fp16, A from TMEM, B K-major (W)
-      constexpr uint32_t id4 = make_idesc(1u, 128, 128, 0, 1);   // bf16, A K-major (U''), B MN-major (K tile)
+      constexpr uint32_t id1 = make_idesc(0u, 128, 64, 1, 0);    // fp16, A MN-major (V tile), B K-major (A_b)
+      constexpr uint32_t id3 = make_idesc(0u, 128, 64, 0, 0);    // fp16, A from TMEM, B K-major (-W)
+      constexpr uint32_t id4 = make_idesc(0u, 128, 128, 0, 1);   // fp16, A K-major (U''), B MN-major (K tile)
       auto issue1 = [&](int c) {  // DY_E = V^t A_b^t
-        const uint32_t sb = smem_base + (c & 1) * kS2StageBytes;
+        const uint32_t sb = smem_base + (c % kS2Stages) * kS2StageBytes;
 #pragma unroll
-        for (int hl = 0; hl < 2; ++hl)
-#pragma unroll
-          for (int ks = 0; ks < 4; ++ks)
-            mma_f16_ss(tmem + 384, make_desc(sb + kS2StV + ks * 2048, 8192, 1024, 2),
-                       make_desc(sb + kS2StRec + kRecAb + hl * kTileB + ks * 32, 16, 1024, 2), id1, (hl | ks) > 0);
+        for (int ks = 0; ks < 4; ++ks)
+          mma_f16_ss(tmem + 384, make_desc(sb + kS2StV + ks * 2048, 8192, 1024, 2),
+                     make_desc(sb + kS2StRec + kRecAb + ks * 32, 16, 1024, 2), id1, ks > 0);
       };
-      auto issue3 = [&](int b, int c) {  // DY_b (+)= Xh_b W^t
-        const uint32_t sb = smem_base + (c & 1) * kS2StageBytes;
+      auto issue3 = [&](int b, int c) {  // DY_b (+)= Xh_b (-W)^t
+        const uint32_t sb = smem_base + (c % kS2Stages) * kS2StageBytes;
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks)
           mma_f16_ts(tmem + 384 + 64 * b, tmem + 256 + 64 * b + 8 * ks,
@@ -304,19 +339,24 @@ __global__ void __launch_bounds__(kS2Threads, 1)
                      (b == 0 || ks > 0) ? 1u : 0u);
       };
       auto issue4 = [&](int b, int c) {  // X_b += U''_b K
-        const uint32_t sb = smem_base + (c & 1) * kS2StageBytes;
+        const uint32_t sb = smem_base + (c % kS2Stages) * kS2StageBytes;
 #pragma unroll
-        for (int hl = 0; hl < 2; ++hl)
-#pragma unroll
-          for (int ks = 0; ks < 4; ++ks)
-            mma_f16_ss(tmem + 128 * b, make_desc(smem_base + kS2OffU + b * 32768 + hl * 16384 + ks * 32, 16, 1024, 2),
-                       make_desc(sb + kS2StK + ks * 2048, 8192, 1024, 2), id4, 1u);
+        for (int ks = 0; ks < 4; ++ks)
+          mma_f16_ss(tmem + 128 * b, make_desc(smem_base + kS2OffU + b * 16384 + ks * 32, 16, 1024, 2),
+                     make_desc(sb + kS2StK + ks * 2048, 8192, 1024, 2), id4, 1u);
       };
       int cc[2] = {0, 0};          // current chunk of each chain
       bool at3[2] = {true, true};  // next step of each chain: (3) or (4)
-      int seen = 0;                // stages up to chunk `seen` have been observed full by this thread
-      bool ok = s2_wait(&bars->st_full[0], 0, abort_flag);
-      tc_fence_after();
+      int seen = -1;               // converted stages observed by this thread: chunks <= seen
+      bool ok = true;
+      auto need_stage = [&](int c) {
+        while (ok && seen < c) {
+          ++seen;
+          ok = s2_wait(&bars->st_conv[seen % kS2Stages], (seen / kS2Stages) & 1, abort_flag);
+        }
+        tc_fence_after();
+      };
+      need_stage(0);
       issue1(0);
       uint32_t spins = 0;
       while (ok && (cc[0] < nc || cc[1] < nc)) {
@@ -327,11 +367,7 @@ __global__ void __launch_bounds__(kS2Threads, 1)
           if (c >= nc) continue;
           if (at3[b]) {
             if (!mbar_test_wait(&bars->xh_ready[b], c & 1)) continue;
-            if (c > seen) {
-              ok = s2_wait(&bars->st_full[c & 1], (c >> 1) & 1, abort_flag);
-              seen = c;
-            }
-            tc_fence_after();
+            need_stage(c);
             S2_STAMP(2, c, 0 + 4 * b);
             issue3(b, c);
             mma_commit(&bars->m3_done[b]);
@@ -345,17 +381,16 @@ __global__ void __launch_bounds__(kS2Threads, 1)
             issue4(b, c);
             mma_commit(&bars->m4_done[b]);
             S2_STAMP(2, c, 3 + 4 * b);
-            if (cc[b ^ 1] > c) mma_commit(&bars->st_free[c & 1]);  // the other chain is already past this chunk
+            if (cc[b ^ 1] > c) mma_commit(&bars->st_free[c % kS2Stages]);  // the other chain is already past this chunk
             cc[b] = c + 1;
             at3[b] = true;
             progress = true;
             if (b == 0 && c + 1 < nc) {
-              if (c + 1 > seen) {
-                ok = s2_wait(&bars->st_full[(c + 1) & 1], ((c + 1) >> 1) & 1, abort_flag);
-                seen = c + 1;
-              }
-              tc_fence_after();
+              S2_STAMP(3, c, 0);
+              need_stage(c + 1);
+              S2_STAMP(3, c, 1);
               issue1(c + 1);
+              S2_STAMP(3, c, 2);
             }
           }
         }
@@ -370,12 +405,35 @@ __global__ void __launch_bounds__(kS2Threads, 1)
         }
       }
     }
-  } else if (warp >= 4 && warp < 8) {
-    s2_chain<false>(smem, bars, abort_flag, tmem, warp, lane, nc, E + (((size_t)s * H + h) * kD + 32 * (warp & 3) + lane) * kD);
-  } else if (warp >= 8) {
-    s2_chain<true>(smem, bars, abort_flag, tmem, warp, lane, nc, T + (((size_t)s * H + h) * kD + 32 * (warp & 3) + lane) * kD);
+  } else if (warp >= 16) {
+    // ------------------------------------------------------------------------------------------- converters
+    // bf16 -> fp16 in place (element-wise on 16-bit lanes, so the 128B swizzle of the TMA boxes is untouched)
+#pragma unroll 1
+    for (int c = 0; c < nc; ++c) {
+      const int st = c % kS2Stages;
+      s2_wait(&bars->st_full[st], (c / kS2Stages) & 1, abort_flag);
+      S2_STAMPW(16, 3, c, 3);
+      uint4* tile = reinterpret_cast<uint4*>(smem + st * kS2StageBytes + (warp == 16 ? kS2StK : kS2StV));
+#pragma unroll 4
+      for (int it = 0; it < 32; ++it) {
+        uint4 w = tile[it * 32 + lane];
+        w.x = pack_f16(__uint_as_float(w.x << 16), __uint_as_float(w.x & 0xffff0000u));
+        w.y = pack_f16(__uint_as_float(w.y << 16), __uint_as_float(w.y & 0xffff0000u));
+        w.z = pack_f16(__uint_as_float(w.z << 16), __uint_as_float(w.z & 0xffff0000u));
+        w.w = pack_f16(__uint_as_float(w.w << 16), __uint_as_float(w.w & 0xffff0000u));
+        tile[it * 32 + lane] = w;
+      }
+      fence_proxy_async();
+      __syncwarp();
+      S2_STAMPW(16, 3, c, 4);
+      if (lane == 0) mbar_arrive(&bars->st_conv[st]);
+    }
+  } else if (warp < 8) {
+    s2_chain<false>(smem, bars, abort_flag, tmem, warp, lane, nc, E + ((size_t)s * H + h) * kD * kD);
+  } else {
+    s2_chain<true>(smem, bars, abort_flag, tmem, warp - 8, lane, nc, T + ((size_t)s * H + h) * kD * kD);
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 2) tmem_dealloc(tmem, 512);
+  if (warp == 16) tmem_dealloc(tmem, 512);
 }

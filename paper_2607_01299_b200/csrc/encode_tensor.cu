@@ -9,7 +9,7 @@
 // Three launches:
 //   K0 chunk_offsets : prefix sum of ceil(L_s / 64) (cu_seqlens lives on the device; no host sync).
 //   K1 prep          : per (chunk, head), state-independent: Gram (mma.sync), L, A by forward substitution (fp32),
-//                      W (mma.sync, fp16 out) and A_b (bf16 hi + lo), stored as ready-made K-major 128B-swizzled
+//                      -W (mma.sync, fp16 out) and A_b (fp16), stored as ready-made K-major 128B-swizzled
 //                      UMMA B tiles, plus the gate record (d_j, gamma_C).
 //   K2 scan          : one CTA per (segment, head), sequential over chunks, both row blocks of X resident in TMEM;
 //                      every state contraction is a tcgen05.mma (see encode_scan2.cuh).
@@ -28,8 +28,8 @@ constexpr int kC = 64;                  // chunk length (north_star)
 constexpr int kD = 128;                 // dk = dv
 constexpr int kTileB = kC * kC * 2;     // one 16-bit 64x64 tile: 8 KB
 constexpr int kRecW = 0;                // record: -W (fp16, [token][dk], two 64-wide boxes) 16 KB
-constexpr int kRecAb = 2 * kTileB;      //         A_b hi, A_b lo (bf16, [token][token]) 2 x 8 KB
-constexpr int kRecBytes = 4 * kTileB;   // 32 KB per (chunk, head)
+constexpr int kRecAb = 2 * kTileB;      //         A_b (fp16, [token][token]) 8 KB
+constexpr int kRecBytes = 3 * kTileB;   // 24 KB per (chunk, head)
 constexpr int kGateFloats = 72;         // d_j[64], gamma_C, pad (288 B = 18 x 16 B)
 constexpr int kGateBytes = kGateFloats * 4;
 
@@ -287,21 +287,14 @@ __global__ void __launch_bounds__(kPrepThreads)
   for (int idx = tid; idx < 2 * kTileB / 16; idx += kPrepThreads)
     *reinterpret_cast<uint4*>(out + kRecW + idx * 16) = *reinterpret_cast<const uint4*>(s_k + idx * 16);
 
-  // ---- A_b as bf16 hi + lo B tiles (K-major, 128B swizzle: row r, 16-byte chunk j8 at ((j8 ^ (r & 7)) * 16))
+  // ---- A_b as an fp16 B tile (K-major, 128B swizzle: row r, 16-byte chunk j8 at ((j8 ^ (r & 7)) * 16))
   for (int idx = tid; idx < kC * 8; idx += kPrepThreads) {
     const int r = idx >> 3, j8 = idx & 7;
-    float v[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) v[i] = s_a[r * kLPitch + 8 * j8 + i];
-    uint32_t hi[4], lo[4];
-#pragma unroll
-    for (int p = 0; p < 4; ++p) {
-      hi[p] = pack_bf16(v[2 * p], v[2 * p + 1]);
-      lo[p] = pack_bf16(v[2 * p] - __uint_as_float(hi[p] << 16), v[2 * p + 1] - __uint_as_float(hi[p] & 0xffff0000u));
-    }
+    const float4 v0 = *reinterpret_cast<const float4*>(s_a + r * kLPitch + 8 * j8);
+    const float4 v1 = *reinterpret_cast<const float4*>(s_a + r * kLPitch + 8 * j8 + 4);
     const uint32_t off = (r >> 3) * 1024 + (r & 7) * 128 + ((j8 ^ (r & 7)) * 16);
-    *reinterpret_cast<uint4*>(out + kRecAb + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-    *reinterpret_cast<uint4*>(out + kRecAb + kTileB + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+    *reinterpret_cast<uint4*>(out + kRecAb + off) =
+        make_uint4(pack_f16(v0.x, v0.y), pack_f16(v0.z, v0.w), pack_f16(v1.x, v1.y), pack_f16(v1.z, v1.w));
   }
   float* go = gate + ((size_t)x * H + h) * kGateFloats;
   go[tid] = expf(s_g[kC - 1] - s_g[tid]);
