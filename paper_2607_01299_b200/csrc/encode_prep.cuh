@@ -1,0 +1,328 @@
+// encode_prep.cuh -- the prep kernel (K1) of the tensor-family segment encode: everything of a chunk that does not
+// depend on the running state.  Included by encode_tensor.cu inside namespace hypic::{anonymous}.
+//
+// One CTA (4 warps) per (chunk, head).  Rows a1..a3 of SURVEY.md section 8(a):
+//   a1  G_r = inclusive cumulative log-decay, gamma_r = exp(G_r), d_j = exp(G_C - G_j)
+//   a2  L_rj = beta_r exp(G_r - G_j) (k_r.k_j) for j < r            Gram by mma.sync (fp16 operands, fp32 accumulate)
+//   a3  A = (I + L)^-1, blocked 4 x 4 in 16 x 16 blocks: the diagonal blocks by forward substitution in fp32 (one
+//       column per lane), the off-diagonal ones by the 2 x 2 block inverse formula A21 = -A22 L21 A11 applied at block
+//       sizes 16 and 32; their 16^3 products run on mma.sync with both operands split in fp16 hi + lo (three passes,
+//       ~2^-22 relative), so A stays at fp32 quality although the flops sit on the tensor pipe
+//   out -W = -(A diag(beta gamma)) K  (mma.sync, fp16 out, K-major 128B-swizzled UMMA B tile of two 64-wide boxes),
+//       A_b = A diag(beta) (fp16, K-major 128B-swizzled UMMA B tile), gate record (d_j, gamma_C).
+// K is staged as fp16 (exact for bf16 values with |x| in [2^-14, 65504]; smaller magnitudes lose bits below 2^-24
+// absolute), so that the Gram and W contractions run as f16 mma.sync with an 11-bit second operand.
+#pragma once
+
+constexpr int kPrepThreads = 128;
+constexpr int kKsPitch = kD + 8;  // 16-bit elements per row of the staged K chunk (conflict-free ldmatrix rows)
+constexpr int kLPitch = 68;       // floats per row of L / A
+constexpr int kMPitch = 36;       // floats per row of the 32 x 32 temporary of the last merge
+
+__device__ __forceinline__ void mma_f16_16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                              uint32_t b0, uint32_t b1) {
+  asm volatile(
+      "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], uint32_t saddr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "r"(saddr));
+}
+__device__ __forceinline__ void ldmatrix_x4_trans(uint32_t (&r)[4], uint32_t saddr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "r"(saddr));
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  __nv_bfloat162 p = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&p);
+}
+__device__ __forceinline__ uint32_t pack_f16(float lo, float hi) {
+  __half2 p = __floats2half2_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&p);
+}
+// (x0, x1) -> packed fp16 hi and packed fp16 lo = fp16(x - hi)
+__device__ __forceinline__ void split_f16(float x0, float x1, uint32_t& hi, uint32_t& lo) {
+  const __half2 h = __floats2half2_rn(x0, x1);
+  const float2 hf = __half22float2(h);
+  hi = *reinterpret_cast<const uint32_t*>(&h);
+  lo = pack_f16(x0 - hf.x, x1 - hf.y);
+}
+
+// acc (16 x 16, two n-tiles of the m16n8 C fragment) += X Y with X = xs[0..16)[0..16), Y = ys[0..16)[0..16), both fp32
+// row-major in shared memory with the given pitches; operands split in fp16 hi + lo, three passes (hh, lh, hl).
+__device__ __forceinline__ void block_mma_16(float (&acc)[2][4], const float* xs, int xp, const float* ys, int yp,
+                                             int lane) {
+  const int gq = lane >> 2, tq = lane & 3;
+  uint32_t ah[4], al[4];
+  {
+    const float2 p0 = *reinterpret_cast<const float2*>(xs + gq * xp + 2 * tq);
+    const float2 p1 = *reinterpret_cast<const float2*>(xs + (gq + 8) * xp + 2 * tq);
+    const float2 p2 = *reinterpret_cast<const float2*>(xs + gq * xp + 2 * tq + 8);
+    const float2 p3 = *reinterpret_cast<const float2*>(xs + (gq + 8) * xp + 2 * tq + 8);
+    split_f16(p0.x, p0.y, ah[0], al[0]);
+    split_f16(p1.x, p1.y, ah[1], al[1]);
+    split_f16(p2.x, p2.y, ah[2], al[2]);
+    split_f16(p3.x, p3.y, ah[3], al[3]);
+  }
+#pragma unroll
+  for (int nt = 0; nt < 2; ++nt) {
+    const int n = 8 * nt + gq;
+    uint32_t bh[2], bl[2];
+    split_f16(ys[(2 * tq) * yp + n], ys[(2 * tq + 1) * yp + n], bh[0], bl[0]);
+    split_f16(ys[(2 * tq + 8) * yp + n], ys[(2 * tq + 9) * yp + n], bh[1], bl[1]);
+    mma_f16_16816(acc[nt], ah[0], ah[1], ah[2], ah[3], bh[0], bh[1]);
+    mma_f16_16816(acc[nt], al[0], al[1], al[2], al[3], bh[0], bh[1]);
+    mma_f16_16816(acc[nt], ah[0], ah[1], ah[2], ah[3], bl[0], bl[1]);
+  }
+}
+// store sign * acc as a 16 x 16 fp32 block
+__device__ __forceinline__ void block_store_16(const float (&acc)[2][4], float sign, float* dst, int dp, int lane) {
+  const int gq = lane >> 2, tq = lane & 3;
+#pragma unroll
+  for (int nt = 0; nt < 2; ++nt) {
+    *reinterpret_cast<float2*>(dst + gq * dp + 8 * nt + 2 * tq) = make_float2(sign * acc[nt][0], sign * acc[nt][1]);
+    *reinterpret_cast<float2*>(dst + (gq + 8) * dp + 8 * nt + 2 * tq) = make_float2(sign * acc[nt][2], sign * acc[nt][3]);
+  }
+}
+__device__ __forceinline__ void block_zero(float (&acc)[2][4]) {
+#pragma unroll
+  for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+    for (int i = 0; i < 4; ++i) acc[nt][i] = 0.f;
+}
+
+__global__ void __launch_bounds__(kPrepThreads)
+    prep_kernel(const __nv_bfloat16* __restrict__ k, const float* __restrict__ g, const float* __restrict__ beta,
+                const int32_t* __restrict__ cu_seqlens, const int32_t* __restrict__ chunk_off, int n_seg, int H,
+                uint8_t* __restrict__ rec, float* __restrict__ gate) {
+  __shared__ __align__(16) uint8_t s_k[kC * kKsPitch * 2];  // K chunk (fp16); later the staged -W tile
+  __shared__ __align__(16) float s_a[kC * kLPitch];         // L, inverted in place to A
+  __shared__ __align__(16) float s_m[32 * kMPitch];         // temporaries of the block merges
+  __shared__ __align__(16) float s_g[kC], s_b[kC], s_bg[kC];
+  __shared__ float s_wsum;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int gq = lane >> 2, tq = lane & 3;
+  const int x = blockIdx.x, h = blockIdx.y;
+  if (x >= chunk_off[n_seg]) return;
+  // segment of this chunk: last s with chunk_off[s] <= x
+  int lo = 0, hi = n_seg - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (chunk_off[mid] <= x) lo = mid; else hi = mid - 1;
+  }
+  const int s = lo;
+  const int t0 = cu_seqlens[s] + (x - chunk_off[s]) * kC;
+  const int valid = min(kC, cu_seqlens[s + 1] - t0);
+
+  __half* ks = reinterpret_cast<__half*>(s_k);
+#pragma unroll
+  for (int it = 0; it < kC * (kD / 8) / kPrepThreads; ++it) {
+    const int idx = tid + it * kPrepThreads;
+    const int r = idx / (kD / 8), c8 = idx % (kD / 8);
+    uint4 val = make_uint4(0, 0, 0, 0);
+    if (r < valid) {
+      const uint4 raw = *reinterpret_cast<const uint4*>(k + ((size_t)(t0 + r) * H + h) * kD + c8 * 8);
+      val.x = pack_f16(__uint_as_float(raw.x << 16), __uint_as_float(raw.x & 0xffff0000u));
+      val.y = pack_f16(__uint_as_float(raw.y << 16), __uint_as_float(raw.y & 0xffff0000u));
+      val.z = pack_f16(__uint_as_float(raw.z << 16), __uint_as_float(raw.z & 0xffff0000u));
+      val.w = pack_f16(__uint_as_float(raw.w << 16), __uint_as_float(raw.w & 0xffff0000u));
+    }
+    *reinterpret_cast<uint4*>(ks + r * kKsPitch + c8 * 8) = val;
+  }
+  {  // a1: inclusive cumulative log-decay by a two-warp shuffle scan (warps 0 and 1 hold the 64 tokens)
+    float gv = 0.f, bv = 0.f;
+    if (tid < valid) {
+      gv = g[(size_t)(t0 + tid) * H + h];
+      bv = beta[(size_t)(t0 + tid) * H + h];
+    }
+    if (warp < 2) {
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const float up = __shfl_up_sync(0xffffffffu, gv, o);
+        if (lane >= o) gv += up;
+      }
+      if (tid == 31) s_wsum = gv;
+    }
+    __syncthreads();
+    if (warp < 2) {
+      if (warp == 1) gv += s_wsum;
+      s_g[tid] = gv;
+      s_b[tid] = bv;
+      s_bg[tid] = bv * expf(gv);
+    }
+  }
+  __syncthreads();
+  const uint32_t ks_base = smem_u32(s_k);
+
+  // ---- a2: Gram K K^t (lower block triangle): warp w owns rows [16w, 16w+16), n-tile pairs p <= w
+  {
+    float acc[8][4];
+#pragma unroll
+    for (int nt = 0; nt < 8; ++nt)
+#pragma unroll
+      for (int i = 0; i < 4; ++i) acc[nt][i] = 0.f;
+    const int arow = 16 * warp + (lane & 7) + 8 * ((lane >> 3) & 1);
+#pragma unroll
+    for (int kk = 0; kk < kD / 16; ++kk) {
+      uint32_t a[4];
+      ldmatrix_x4(a, ks_base + (uint32_t)(arow * kKsPitch + 16 * kk + 8 * (lane >> 4)) * 2u);
+#pragma unroll
+      for (int p = 0; p < 4; ++p) {
+        if (p > warp) continue;
+        uint32_t b[4];
+        const int nrow = 16 * p + (lane & 7) + 8 * (lane >> 4);
+        ldmatrix_x4(b, ks_base + (uint32_t)(nrow * kKsPitch + 16 * kk + 8 * ((lane >> 3) & 1)) * 2u);
+        mma_f16_16816(acc[2 * p], a[0], a[1], a[2], a[3], b[0], b[1]);
+        mma_f16_16816(acc[2 * p + 1], a[0], a[1], a[2], a[3], b[2], b[3]);
+      }
+    }
+    // L_rj = beta_r exp(G_r - G_j) (k_r.k_j) for j < r, else 0 (the upper blocks are zero-filled: the A_b tile reads them)
+#pragma unroll
+    for (int hh = 0; hh < 2; ++hh) {
+      const int r = 16 * warp + gq + 8 * hh;
+      const float br = s_b[r], gr = s_g[r];
+#pragma unroll
+      for (int nt = 0; nt < 8; ++nt) {
+        const int j = 8 * nt + 2 * tq;
+        float v0 = 0.f, v1 = 0.f;
+        if (nt <= 2 * warp + 1) {
+          if (j < r) v0 = br * __expf(gr - s_g[j]) * acc[nt][2 * hh];
+          if (j + 1 < r) v1 = br * __expf(gr - s_g[j + 1]) * acc[nt][2 * hh + 1];
+        }
+        *reinterpret_cast<float2*>(s_a + r * kLPitch + j) = make_float2(v0, v1);
+      }
+    }
+  }
+  __syncthreads();
+
+  // ---- a3 (i): diagonal blocks D_w = (I + L_ww)^-1 in place, lane c < 16 = column c, row-oriented substitution
+  {
+    float* blk = s_a + (16 * warp) * kLPitch + 16 * warp;
+    float a[16];
+    const int c = lane & 15;
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+      float sum = (r == c) ? 1.f : 0.f;
+#pragma unroll
+      for (int j4 = 0; j4 < (r + 3) / 4; ++j4) {
+        const float4 l = *reinterpret_cast<const float4*>(blk + r * kLPitch + 4 * j4);
+        if (4 * j4 + 0 < r) sum = fmaf(-l.x, a[4 * j4 + 0], sum);
+        if (4 * j4 + 1 < r) sum = fmaf(-l.y, a[4 * j4 + 1], sum);
+        if (4 * j4 + 2 < r) sum = fmaf(-l.z, a[4 * j4 + 2], sum);
+        if (4 * j4 + 3 < r) sum = fmaf(-l.w, a[4 * j4 + 3], sum);
+      }
+      a[r] = sum;
+    }
+    __syncwarp();
+    if (lane < 16) {
+#pragma unroll
+      for (int r = 0; r < 16; ++r) blk[r * kLPitch + c] = a[r];
+    }
+  }
+  __syncthreads();
+  auto B = [&](int i, int j) { return s_a + (16 * i) * kLPitch + 16 * j; };
+
+  // ---- a3 (ii): A10 = -D1 (L10 D0) (warp 0), A32 = -D3 (L32 D2) (warp 1)
+  if (warp < 2) {
+    const int i = 2 * warp + 1, j = 2 * warp;
+    float* tmp = s_m + (16 * warp) * kMPitch;
+    float acc[2][4];
+    block_zero(acc);
+    block_mma_16(acc, B(i, j), kLPitch, B(j, j), kLPitch, lane);
+    block_store_16(acc, 1.f, tmp, kMPitch, lane);
+    __syncwarp();
+    block_zero(acc);
+    block_mma_16(acc, B(i, i), kLPitch, tmp, kMPitch, lane);
+    __syncwarp();
+    block_store_16(acc, -1.f, B(i, j), kLPitch, lane);
+  }
+  __syncthreads();
+  // ---- a3 (iii): the 32 x 32 block A[2:4, 0:2] = -A[2:4, 2:4] (L[2:4, 0:2] A[0:2, 0:2]); warp -> block (2 + w/2, w%2)
+  {
+    const int i = 2 + (warp >> 1), j = warp & 1;
+    float acc[2][4];
+    block_zero(acc);
+    if (j == 0) block_mma_16(acc, B(i, 0), kLPitch, B(0, 0), kLPitch, lane);
+    block_mma_16(acc, B(i, 1), kLPitch, B(1, j), kLPitch, lane);
+    block_store_16(acc, 1.f, s_m + (16 * (i - 2)) * kMPitch + 16 * j, kMPitch, lane);
+    __syncthreads();
+    block_zero(acc);
+    block_mma_16(acc, B(i, 2), kLPitch, s_m + 16 * j, kMPitch, lane);
+    if (i == 3) block_mma_16(acc, B(3, 3), kLPitch, s_m + 16 * kMPitch + 16 * j, kMPitch, lane);
+    block_store_16(acc, -1.f, B(i, j), kLPitch, lane);
+  }
+  __syncthreads();
+
+  // ---- -W = -(A diag(beta gamma)) K with mma.sync: warp w rows [16w, 16w+16), k-steps kk <= w (A is lower triangular)
+  float wacc[16][4];
+#pragma unroll
+  for (int nt = 0; nt < 16; ++nt)
+#pragma unroll
+    for (int i = 0; i < 4; ++i) wacc[nt][i] = 0.f;
+#pragma unroll
+  for (int kk = 0; kk < 4; ++kk) {
+    if (kk > warp) continue;
+    uint32_t a[4];
+    {
+      const int r0 = 16 * warp + gq, c0 = 16 * kk + 2 * tq;
+      const float g0 = s_bg[c0], g1 = s_bg[c0 + 1], g8 = s_bg[c0 + 8], g9 = s_bg[c0 + 9];
+      const float2 p0 = *reinterpret_cast<const float2*>(s_a + r0 * kLPitch + c0);
+      const float2 p1 = *reinterpret_cast<const float2*>(s_a + (r0 + 8) * kLPitch + c0);
+      const float2 p2 = *reinterpret_cast<const float2*>(s_a + r0 * kLPitch + c0 + 8);
+      const float2 p3 = *reinterpret_cast<const float2*>(s_a + (r0 + 8) * kLPitch + c0 + 8);
+      a[0] = pack_f16(p0.x * g0, p0.y * g1);
+      a[1] = pack_f16(p1.x * g0, p1.y * g1);
+      a[2] = pack_f16(p2.x * g8, p2.y * g9);
+      a[3] = pack_f16(p3.x * g8, p3.y * g9);
+    }
+    // B fragments (k = token, n = dk) by transposing ldmatrix over the [token][dk] tile, two n-tiles at a time
+    const int tok = 16 * kk + (lane & 7) + ((lane >> 3) & 1) * 8;
+#pragma unroll
+    for (int np = 0; np < 8; ++np) {
+      uint32_t b[4];
+      ldmatrix_x4_trans(b, ks_base + (uint32_t)(tok * kKsPitch + 8 * (2 * np + (lane >> 4))) * 2u);
+      mma_f16_16816(wacc[2 * np], a[0], a[1], a[2], a[3], b[0], b[1]);
+      mma_f16_16816(wacc[2 * np + 1], a[0], a[1], a[2], a[3], b[2], b[3]);
+    }
+  }
+
+  // ---- A_b = A diag(beta) as an fp16 B tile (K-major, 128B swizzle: row r, 16-byte chunk j8 at ((j8 ^ (r & 7)) * 16))
+  uint8_t* out = rec + ((size_t)x * H + h) * kRecBytes;
+#pragma unroll
+  for (int it = 0; it < kC * 8 / kPrepThreads; ++it) {
+    const int idx = tid + it * kPrepThreads;
+    const int r = idx >> 3, j8 = idx & 7;
+    const float4 v0 = *reinterpret_cast<const float4*>(s_a + r * kLPitch + 8 * j8);
+    const float4 v1 = *reinterpret_cast<const float4*>(s_a + r * kLPitch + 8 * j8 + 4);
+    const float4 b0 = *reinterpret_cast<const float4*>(s_b + 8 * j8);
+    const float4 b1 = *reinterpret_cast<const float4*>(s_b + 8 * j8 + 4);
+    const uint32_t off = (r >> 3) * 1024 + (r & 7) * 128 + ((j8 ^ (r & 7)) * 16);
+    *reinterpret_cast<uint4*>(out + kRecAb + off) =
+        make_uint4(pack_f16(v0.x * b0.x, v0.y * b0.y), pack_f16(v0.z * b0.z, v0.w * b0.w),
+                   pack_f16(v1.x * b1.x, v1.y * b1.y), pack_f16(v1.z * b1.z, v1.w * b1.w));
+  }
+  __syncthreads();  // K is dead: stage -W over it, already in the K-major 128B-swizzled two-box layout
+#pragma unroll
+  for (int nt = 0; nt < 16; ++nt)
+#pragma unroll
+    for (int hh = 0; hh < 2; ++hh) {
+      const int r = 16 * warp + gq + 8 * hh;
+      const int col = 8 * nt + 2 * tq;
+      const uint32_t off = (col >> 6) * 8192 + (r >> 3) * 1024 + (r & 7) * 128 + ((((col & 63) >> 3) ^ (r & 7)) * 16) +
+                           (col & 7) * 2;
+      *reinterpret_cast<uint32_t*>(s_k + off) = pack_f16(-wacc[nt][2 * hh], -wacc[nt][2 * hh + 1]);
+    }
+  __syncthreads();
+#pragma unroll
+  for (int it = 0; it < 2 * kTileB / 16 / kPrepThreads; ++it) {
+    const int idx = tid + it * kPrepThreads;
+    *reinterpret_cast<uint4*>(out + kRecW + idx * 16) = *reinterpret_cast<const uint4*>(s_k + idx * 16);
+  }
+  float* go = gate + ((size_t)x * H + h) * kGateFloats;
+  if (tid < kC) go[tid] = expf(s_g[kC - 1] - s_g[tid]);
+  else if (tid < kGateFloats) go[tid] = (tid == kC) ? expf(s_g[kC - 1]) : 0.f;
+}

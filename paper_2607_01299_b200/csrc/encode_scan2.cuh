@@ -73,15 +73,20 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst_smem, const CUtensorMap
 
 __device__ __noinline__ bool s2_wait(uint64_t* bar, uint32_t parity, volatile int* abort_flag) {
 #pragma unroll 1
-  for (uint32_t i = 0; i < 400000u; ++i) {
-    if (mbar_try_wait_hint(bar, parity, 20000u)) return true;
-    if ((i & 63u) == 63u && *abort_flag) return false;
+  for (uint32_t i = 0; i < 4000000u; ++i) {
+    if (mbar_try_wait(bar, parity)) return true;
+    __nanosleep(20);  // back off: a tight try_wait loop floods the shared-memory pipeline the working warps need
+    if ((i & 1023u) == 1023u && *abort_flag) return false;
   }
   if (!*abort_flag) {
     *abort_flag = 1;
     atomicAdd(&g_timeout_count_enc, 1u);
   }
   return false;
+}
+
+__device__ __forceinline__ void s2_wait_warp(uint64_t* bar, uint32_t parity, volatile int* abort_flag, int) {
+  s2_wait(bar, parity, abort_flag);
 }
 
 // 32 lanes x 16 columns
@@ -132,8 +137,8 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
   for (int c = 0; c < nc; ++c) {
     const int st = c % kS2Stages;
     const float* gt = reinterpret_cast<const float*>(smem + st * kS2StageBytes + kS2StGate);
-    s2_wait(&bars->st_full[st], (c / kS2Stages) & 1, abort_flag);
-    if (c > 0) s2_wait(&bars->m4_done[b], (c - 1) & 1, abort_flag);
+    s2_wait_warp(&bars->st_full[st], (c / kS2Stages) & 1, abort_flag, lane);
+    if (c > 0) s2_wait_warp(&bars->m4_done[b], (c - 1) & 1, abort_flag, lane);
     tc_fence_after();
     S2_STAMP(b, c, 0);
     const float gC = gt[kC];
@@ -200,7 +205,7 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     if (lane == 0) mbar_arrive(&bars->xh_ready[b]);
 
     // ---- epilogue: U''[:, j] = fp16(DY[:, j] d_j), K-major 128B swizzle (A operand of (4)); tokens [32 hf, 32 hf + 32)
-    s2_wait(&bars->m3_done[b], c & 1, abort_flag);
+    s2_wait_warp(&bars->m3_done[b], c & 1, abort_flag, lane);
     tc_fence_after();
     S2_STAMP(b, c, 2);
     {
@@ -232,7 +237,7 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
 
   // ---- a5: write this thread's 64 columns of its row (T: undo the row normalisation, in two exact steps)
   if (nc > 0) {
-    s2_wait(&bars->m4_done[b], (nc - 1) & 1, abort_flag);
+    s2_wait_warp(&bars->m4_done[b], (nc - 1) & 1, abort_flag, lane);
     tc_fence_after();
   }
   const int se = max(-250, min(250, s_exp));
@@ -411,9 +416,10 @@ __global__ void __launch_bounds__(kS2Threads, 1)
 #pragma unroll 1
     for (int c = 0; c < nc; ++c) {
       const int st = c % kS2Stages;
-      s2_wait(&bars->st_full[st], (c / kS2Stages) & 1, abort_flag);
+      s2_wait_warp(&bars->st_full[st], (c / kS2Stages) & 1, abort_flag, lane);
       S2_STAMPW(16, 3, c, 3);
       uint4* tile = reinterpret_cast<uint4*>(smem + st * kS2StageBytes + (warp == 16 ? kS2StK : kS2StV));
+#ifndef HYPIC_EXP_NOCONV
 #pragma unroll 4
       for (int it = 0; it < 32; ++it) {
         uint4 w = tile[it * 32 + lane];
@@ -423,6 +429,7 @@ __global__ void __launch_bounds__(kS2Threads, 1)
         w.w = pack_f16(__uint_as_float(w.w << 16), __uint_as_float(w.w & 0xffff0000u));
         tile[it * 32 + lane] = w;
       }
+#endif
       fence_proxy_async();
       __syncwarp();
       S2_STAMPW(16, 3, c, 4);
