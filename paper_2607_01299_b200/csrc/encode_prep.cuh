@@ -95,9 +95,9 @@ __device__ __forceinline__ void block_zero(float (&acc)[2][4]) {
     for (int i = 0; i < 4; ++i) acc[nt][i] = 0.f;
 }
 
-__global__ void __launch_bounds__(kPrepThreads)
+__global__ void __launch_bounds__(kPrepThreads, 5)
     prep_kernel(const __nv_bfloat16* __restrict__ k, const float* __restrict__ g, const float* __restrict__ beta,
-                const int32_t* __restrict__ cu_seqlens, const int32_t* __restrict__ chunk_off, int n_seg, int H,
+                const int2* __restrict__ chunk_meta, int H,
                 uint8_t* __restrict__ rec, float* __restrict__ gate) {
   __shared__ __align__(16) uint8_t s_k[kC * kKsPitch * 2];  // K chunk (fp16); later the staged -W tile
   __shared__ __align__(16) float s_a[kC * kLPitch];         // L, inverted in place to A
@@ -107,16 +107,9 @@ __global__ void __launch_bounds__(kPrepThreads)
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int gq = lane >> 2, tq = lane & 3;
   const int x = blockIdx.x, h = blockIdx.y;
-  if (x >= chunk_off[n_seg]) return;
-  // segment of this chunk: last s with chunk_off[s] <= x
-  int lo = 0, hi = n_seg - 1;
-  while (lo < hi) {
-    const int mid = (lo + hi + 1) >> 1;
-    if (chunk_off[mid] <= x) lo = mid; else hi = mid - 1;
-  }
-  const int s = lo;
-  const int t0 = cu_seqlens[s] + (x - chunk_off[s]) * kC;
-  const int valid = min(kC, cu_seqlens[s + 1] - t0);
+  const int2 meta = chunk_meta[x];  // (first token, valid tokens); (0, 0) beyond the last chunk of the call
+  const int t0 = meta.x, valid = meta.y;
+  if (valid == 0) return;
 
   __half* ks = reinterpret_cast<__half*>(s_k);
 #pragma unroll

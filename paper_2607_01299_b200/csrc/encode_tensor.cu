@@ -34,11 +34,16 @@ constexpr int kGateFloats = 72;         // d_j[64], gamma_C, pad (288 B = 18 x 1
 constexpr int kGateBytes = kGateFloats * 4;
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
-__host__ __device__ inline size_t ws_off_rec(int32_t n_seg) { return align_up(4 * ((size_t)n_seg + 1), 1024); }
+// workspace: chunk_off int32[n_seg + 1] | chunk_meta int2[cap] | records [cap][H][kRecBytes] | gate [cap][H][kGateFloats]
 __host__ __device__ inline size_t chunk_cap(int32_t n_seg, int32_t t_total) { return (size_t)t_total / kC + n_seg; }
+__host__ __device__ inline size_t ws_off_meta(int32_t n_seg) { return align_up(4 * ((size_t)n_seg + 1), 1024); }
+__host__ __device__ inline size_t ws_off_rec(int32_t n_seg, size_t cap) { return ws_off_meta(n_seg) + align_up(8 * cap, 1024); }
 
 // ------------------------------------------------------------------------------------------------ K0
-__global__ void chunk_offsets_kernel(const int32_t* __restrict__ cu_seqlens, int n_seg, int32_t* __restrict__ chunk_off) {
+// chunk_meta[x] = (first token, number of valid tokens) of global chunk x, (0, 0) for the unused tail of the table:
+// the prep CTAs read one entry instead of searching chunk_off (a chain of dependent global loads).
+__global__ void chunk_offsets_kernel(const int32_t* __restrict__ cu_seqlens, int n_seg, int32_t* __restrict__ chunk_off,
+                                     int2* __restrict__ chunk_meta, int cap) {
   __shared__ int part[1024];
   const int tid = threadIdx.x;
   const int per = (n_seg + 1023) / 1024;
@@ -60,8 +65,15 @@ __global__ void chunk_offsets_kernel(const int32_t* __restrict__ cu_seqlens, int
   int run = part[tid];
   for (int s = lo; s < hi; ++s) {
     chunk_off[s] = run;
-    run += (cu_seqlens[s + 1] - cu_seqlens[s] + kC - 1) / kC;
+    const int b = cu_seqlens[s], e = cu_seqlens[s + 1];
+    const int n = (e - b + kC - 1) / kC;
+    for (int c = 0; c < n; ++c) chunk_meta[run + c] = make_int2(b + c * kC, min(kC, e - b - c * kC));
+    run += n;
   }
+  __shared__ int total;
+  if (tid == 1023) total = run;  // the last thread ends at the grand total
+  __syncthreads();
+  for (int x = total + tid; x < cap; x += 1024) chunk_meta[x] = make_int2(0, 0);
 }
 
 // ------------------------------------------------------------------------------------------------ K1, K2
@@ -117,7 +129,7 @@ size_t encode_tensor_workspace(int32_t n_seg, int32_t t_total, int32_t H, int32_
                                int gate) {
   if (!encode_tensor_shape_ok(H, dk, dv, kv_dtype, gate)) return 0;
   const size_t cap = chunk_cap(n_seg, t_total);
-  return ws_off_rec(n_seg) + cap * H * ((size_t)kRecBytes + kGateBytes);
+  return ws_off_rec(n_seg, cap) + cap * H * ((size_t)kRecBytes + kGateBytes);
 }
 
 int encode_tensor(const EncodeArgs& a) {
@@ -134,7 +146,8 @@ int encode_tensor(const EncodeArgs& a) {
   }
   uint8_t* ws = static_cast<uint8_t*>(a.workspace);
   int32_t* chunk_off = reinterpret_cast<int32_t*>(ws);
-  uint8_t* rec = ws + ws_off_rec(a.n_seg);
+  int2* chunk_meta = reinterpret_cast<int2*>(ws + ws_off_meta(a.n_seg));
+  uint8_t* rec = ws + ws_off_rec(a.n_seg, cap);
   float* gate = reinterpret_cast<float*>(rec + cap * a.H * (size_t)kRecBytes);
   static bool configured = false;
   if (!configured) {
@@ -146,10 +159,9 @@ int encode_tensor(const EncodeArgs& a) {
   int rc = make_kv_tensor_map(&tmK, a.k, a.t_total, a.H);
   if (rc == HYPIC_OK) rc = make_kv_tensor_map(&tmV, a.v, a.t_total, a.H);
   if (rc != HYPIC_OK) return rc;
-  chunk_offsets_kernel<<<1, 1024, 0, a.stream>>>(a.cu_seqlens, a.n_seg, chunk_off);
+  chunk_offsets_kernel<<<1, 1024, 0, a.stream>>>(a.cu_seqlens, a.n_seg, chunk_off, chunk_meta, (int)cap);
   note_launch();
-  prep_kernel<<<dim3((unsigned)cap, a.H), kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, a.cu_seqlens, chunk_off,
-                                                                       a.n_seg, a.H, rec, gate);
+  prep_kernel<<<dim3((unsigned)cap, a.H), kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, chunk_meta, a.H, rec, gate);
   note_launch();
   scan2_kernel<<<dim3(a.H, a.n_seg), kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, a.H, rec, gate,
                                                                      a.E, a.T);
