@@ -327,9 +327,8 @@ def run_ours(args):
     ms_total = t0.elapsed_time(t1)
     launches = req.launches
     if dist is not None:
-        tt = torch.tensor([ms_total], device=device, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
+        from paper_2607_01299_b200 import sharding
+        ms_total = sharding.max_over_ranks(ms_total, device=device)
     ms_step = ms_total / args.steps
     tokens_per_step = L * N_SEG * SEG_LEN * world
     value = tokens_per_step / (ms_step * 1e-3)
@@ -354,8 +353,8 @@ def run_ours(args):
     tpath = os.path.join(ROOT, "profiles", "traffic.json")  # dram bytes per launch from the committed ncu capture
     if os.path.exists(tpath):
         roofline["traffic"] = json.load(open(tpath)).get(f"encode_{fam}_cfg2_layer_dram_bytes")
-    roofline.update({"kernel": ("hypic_segment_encode = chunk_offsets_kernel + prep_kernel + scan_kernel (tensor "
-                                "family; scan_kernel dominates, see profiles/)") if fam == "tensor" else
+    roofline.update({"kernel": ("hypic_segment_encode = chunk_offsets_kernel + prep_kernel + scan2_kernel (tensor "
+                                "family; prep and scan share the call about evenly, see profiles/)") if fam == "tensor" else
                      "hypic_segment_encode = encode_simt_kernel (simt family)",
                      "units_per_launch": f"{th_per_launch} token-heads x {ENC_FLOP_PER_TOKEN_HEAD} flop",
                      "avg_launch_ms": enc_avg, "share_of_step": enc_avg * L / ms_step,

@@ -82,7 +82,9 @@ size_t hypic_segment_encode_workspace(int32_t n_seg, int32_t t_total, int32_t H,
  *            (may be NULL when that is 0).  Contents are undefined before and after the call.
  *
  * A zero-length segment yields E = 0, T = I.  n_seg = 0 or t_total = 0 with n_seg > 0 are valid.
- * Built envelope: dk in {64, 128}; dv in [1, 1024] for the SIMT family, dv = dk = 128 for the tensor family;
+ * Built envelope: dk in {64, 128}; dv in [1, 1024] for the SIMT family, dv = dk = 128 for the tensor family
+ * (bf16 k/v, scalar gate; its tensor-core operands are fp16, so it additionally assumes finite |k|, |v| <= 65504 and
+ * beta |k|^2 within the stable range of the recurrence -- callers outside that range select HYPIC_IMPL_SIMT);
  * H, n_seg, lengths arbitrary.  Inputs are only read; E and T are fully overwritten.
  */
 int hypic_segment_encode(const void* k, const void* v, const float* g, const float* beta,

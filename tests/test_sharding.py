@@ -1,0 +1,85 @@
+"""N > 1 host logic on CPU: LPT segment partition (Eq. 9), head split, and the max-over-ranks
+timing reduction over a world_size-2 gloo group.  Also: encoding a shard of the segments and composing per head
+with the oracle gives the same state as the unsharded run (the path shards with no data-path collective)."""
+import os
+import socket
+
+import numpy as np
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+import oracle
+from paper_2607_01299_b200 import sharding
+from paper_2607_01299_b200 import workloads as wl
+
+
+def test_lpt_partition_covers_and_balances():
+    lens = wl.cfg3_seg_lens()
+    for world in (1, 2, 3, 8):
+        parts = sharding.lpt_partition(lens, world)
+        assert sorted(i for p in parts for i in p) == list(range(len(lens)))
+        loads = sharding.shard_loads(lens, parts)
+        # greedy list scheduling: the fullest worker, minus the last segment it was given, is no fuller than the mean
+        assert max(loads) <= sum(lens) / world + max(lens)
+        if world == 1:
+            assert loads == [sum(lens)]
+    assert sharding.lpt_partition([], 4) == [[], [], [], []]
+    assert sharding.lpt_partition([5, 5, 5], 2) == [[0, 2], [1]]
+
+
+def test_head_range_is_a_partition():
+    for H in (1, 16, 32, 33):
+        for world in (1, 2, 3, 8):
+            spans = [sharding.head_range(H, r, world) for r in range(world)]
+            assert spans[0][0] == 0 and spans[-1][1] == H
+            assert all(spans[i][1] == spans[i + 1][0] for i in range(world - 1))
+            sizes = [e - b for b, e in spans]
+            assert max(sizes) - min(sizes) <= 1
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out_dir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        inp = wl.make_encode_inputs([70, 33, 129, 64, 5], 2, 16, 16, kv_dtype=torch.float32, seed=wl.seed_for(0, 9))
+        parts = sharding.lpt_partition(inp.seg_lens, world)
+        mine = parts[rank]
+        # every rank derives the same partition on its own
+        gathered = [None] * world
+        dist.all_gather_object(gathered, parts)
+        assert all(g == parts for g in gathered)
+        # encode my segments only (oracle stands in for the device on the CPU box); no collective on the data path
+        E_all, T_all = oracle.segment_encode(inp.k, inp.v, inp.g, inp.beta, inp.cu_seqlens, gate=inp.gate)
+        cu = inp.cu_seqlens.numpy()
+        for s in mine:
+            sl = slice(int(cu[s]), int(cu[s + 1]))
+            E, T = oracle.segment_encode(inp.k[sl], inp.v[sl], inp.g[sl], inp.beta[sl],
+                                         np.array([0, sl.stop - sl.start], dtype=np.int32), gate=inp.gate)
+            assert np.array_equal(E[0], E_all[s]) and np.array_equal(T[0], T_all[s])
+        # compose is sharded by heads: my heads of the composed state equal the same heads of the full run
+        b, e = sharding.head_range(2, rank, world)
+        ids = np.arange(5, dtype=np.int32)
+        cu_r = np.array([0, 5], dtype=np.int32)
+        S_full = oracle.compose(None, E_all, T_all, ids, cu_r)
+        S_mine = oracle.compose(None, E_all[:, b:e], T_all[:, b:e], ids, cu_r)
+        assert np.array_equal(S_mine, S_full[:, b:e])
+        # timing reduction: max over ranks
+        t = sharding.max_over_ranks(10.0 + rank)
+        assert t == 10.0 + world - 1
+        with open(os.path.join(out_dir, f"ok{rank}"), "w") as f:
+            f.write("ok")
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_rank_gloo_sharding(tmp_path):
+    world = 2
+    mp.spawn(_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    assert all((tmp_path / f"ok{r}").exists() for r in range(world))
