@@ -12,7 +12,7 @@
 // the factor never has to be undone before the final write-out.  E rows live on the scale of v and stay unscaled.
 // k / v arrive as bf16 and are converted to fp16 in place in shared memory (exact for |x| in [2^-14, 65504]).
 //
-// 20 warps:
+// 19 warps:
 // (the warp scheduler favours the highest warp id of an SM sub-partition, so the latency-critical single-thread
 // roles sit at the top):
 //   warps 0-7     E chain     thread = (row of E, 64-column half): pass  Xh = fp16(X), X <- gamma_C X;
@@ -21,7 +21,9 @@
 //   warps 16-17   converters  K (warp 16) and V (warp 17) tile bf16 -> fp16 in place; warp 16 also owns TMEM alloc
 //   warp 18       loader      TMA tensor boxes for the K / V chunk tiles, bulk copies for the prep record (-W, A_b)
 //                             and the gate record; three stages
-//   warp 19       MMA issuer  one thread; polls the two chains and issues whichever step is ready
+// There is no separate MMA-issuer role: after a chain-wide named barrier, one elected thread of the chain issues the
+// chain's next batch itself (a dedicated issuer thread that polled both chains reacted 450-800 cycles late per batch,
+// starved by the busy chain warps of its SM sub-partition) and commits it to the mbarrier the chain then waits on.
 // The two chains only share read-only operands, so while one is in its element-wise phase the tensor pipe runs the
 // other one's MMAs.  TMEM columns: X_E [0,128), X_T [128,256), Xh_E [256,320), Xh_T [320,384), DY_E [384,448),
 // DY_T [448,512).  All waits are bounded; a protocol error bumps g_timeout_count_enc instead of hanging the GPU.
@@ -33,7 +35,7 @@ __device__ long long g_s2_timeline[4 * 64 * 8];
 #define S2_STAMP(role, c, k)                                                                              \
   do {                                                                                                    \
     if (blockIdx.x == 0 && blockIdx.y == 0 && (c) < 64 && (threadIdx.x & 31) == 0 &&                      \
-        (threadIdx.x >> 5) == ((role) >= 2 ? 19 : ((role) == 0 ? 0 : 8)))                                 \
+        (threadIdx.x >> 5) == ((role) == 0 ? 0 : 8))                                 \
       g_s2_timeline[((role) * 64 + (c)) * 8 + (k)] = clock64();                                           \
   } while (0)
 #define S2_STAMPW(w, role, c, k)                                                                          \
@@ -46,7 +48,7 @@ __device__ long long g_s2_timeline[4 * 64 * 8];
 #define S2_STAMPW(w, role, c, k) do {} while (0)
 #endif
 
-constexpr int kS2Threads = 640;
+constexpr int kS2Threads = 608;
 constexpr int kS2Stages = 3;
 constexpr int kS2StK = 0, kS2StV = 16384, kS2StRec = 32768, kS2StGate = 32768 + kRecBytes;
 constexpr int kS2StageBytes = 32768 + kRecBytes + 1024;
@@ -57,7 +59,7 @@ constexpr int kS2Smem = kS2OffBar + 256 + 1024;
 
 struct S2Bars {
   uint64_t st_full[kS2Stages], st_conv[kS2Stages], st_free[kS2Stages];
-  uint64_t xh_ready[2], m3_done[2], u_ready[2], m4_done[2];  // [block]: 0 = E, 1 = T
+  uint64_t m3_done[2], m4_done[2];  // [block]: 0 = E, 1 = T
   uint32_t tmem_base;
   int abort_flag;
 };
@@ -109,6 +111,30 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 }
 __device__ __forceinline__ float pow2i(int e) { return __uint_as_float((uint32_t)(127 + e) << 23); }  // e in [-126, 127]
 
+// MMA batches of one chunk; each is issued by one elected thread of the chain that produced its operands.
+__device__ __forceinline__ void s2_issue1(uint32_t tmem, uint32_t sb) {  // DY_E = V^t A_b^t
+  constexpr uint32_t id1 = make_idesc(0u, 128, 64, 1, 0);  // fp16, A MN-major (V tile), B K-major (A_b)
+#pragma unroll
+  for (int ks = 0; ks < 4; ++ks)
+    mma_f16_ss(tmem + 384, make_desc(sb + kS2StV + ks * 2048, 8192, 1024, 2),
+               make_desc(sb + kS2StRec + kRecAb + ks * 32, 16, 1024, 2), id1, ks > 0);
+}
+__device__ __forceinline__ void s2_issue3(uint32_t tmem, uint32_t sb, int b) {  // DY_b (+)= Xh_b (-W)^t
+  constexpr uint32_t id3 = make_idesc(0u, 128, 64, 0, 0);  // fp16, A from TMEM, B K-major (-W)
+#pragma unroll
+  for (int ks = 0; ks < 8; ++ks)
+    mma_f16_ts(tmem + 384 + 64 * b, tmem + 256 + 64 * b + 8 * ks,
+               make_desc(sb + kS2StRec + kRecW + (ks >> 2) * 8192 + (ks & 3) * 32, 16, 1024, 2), id3,
+               (b == 0 || ks > 0) ? 1u : 0u);
+}
+__device__ __forceinline__ void s2_issue4(uint32_t tmem, uint32_t sb, uint32_t su, int b) {  // X_b += U''_b K
+  constexpr uint32_t id4 = make_idesc(0u, 128, 128, 0, 1);  // fp16, A K-major (U''), B MN-major (K tile)
+#pragma unroll
+  for (int ks = 0; ks < 4; ++ks)
+    mma_f16_ss(tmem + 128 * b, make_desc(su + ks * 32, 16, 1024, 2), make_desc(sb + kS2StK + ks * 2048, 8192, 1024, 2),
+               id4, 1u);
+}
+
 template <bool kIsT>
 __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile int* abort_flag, uint32_t tmem, int cw,
                                          int lane, int nc, float* __restrict__ dst_block) {
@@ -132,6 +158,13 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     tmem_st32(tX + 32 * cb, x);
   }
   tmem_st_wait();
+  const uint32_t smem_base = smem_u32(smem);
+  const bool issuer = (cw == 0 && lane == 0);  // this chain's MMA-issuing thread
+  if (!kIsT && issuer && nc > 0) {
+    s2_wait(&bars->st_conv[0], 0, abort_flag);
+    tc_fence_after();
+    s2_issue1(tmem, smem_base);
+  }
 
 #pragma unroll 1
   for (int c = 0; c < nc; ++c) {
@@ -200,9 +233,15 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
       tmem_st_wait();
     }
     tc_fence_before();
-    __syncwarp();
+    named_bar_sync(5 + b, 256);  // the whole chain has written Xh / X
     S2_STAMP(b, c, 1);
-    if (lane == 0) mbar_arrive(&bars->xh_ready[b]);
+    if (issuer) {
+      if (kIsT) s2_wait(&bars->st_conv[st], (c / kS2Stages) & 1, abort_flag);  // (E saw it before its (1)_c)
+      tc_fence_after();
+      s2_issue3(tmem, smem_base + st * kS2StageBytes, b);
+      mma_commit(&bars->m3_done[b]);
+    }
+    __syncwarp();
 
     // ---- epilogue: U''[:, j] = fp16(DY[:, j] d_j), K-major 128B swizzle (A operand of (4)); tokens [32 hf, 32 hf + 32)
     s2_wait_warp(&bars->m3_done[b], c & 1, abort_flag, lane);
@@ -230,9 +269,20 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     }
     fence_proxy_async();
     tc_fence_before();
-    __syncwarp();
+    named_bar_sync(5 + b, 256);  // the whole chain has written U''
     S2_STAMP(b, c, 3);
-    if (lane == 0) mbar_arrive(&bars->u_ready[b]);
+    if (issuer) {
+      tc_fence_after();
+      s2_issue4(tmem, smem_base + st * kS2StageBytes, smem_base + kS2OffU + b * 16384, b);
+      mma_commit(&bars->m4_done[b]);
+      mma_commit(&bars->st_free[st]);  // count 2: released when both chains' (4) of this chunk have completed
+      if (!kIsT && c + 1 < nc) {
+        s2_wait(&bars->st_conv[(c + 1) % kS2Stages], ((c + 1) / kS2Stages) & 1, abort_flag);
+        tc_fence_after();
+        s2_issue1(tmem, smem_base + ((c + 1) % kS2Stages) * kS2StageBytes);
+      }
+    }
+    __syncwarp();
   }
 
   // ---- a5: write this thread's 64 columns of its row (T: undo the row normalisation, in two exact steps)
@@ -284,12 +334,10 @@ __global__ void __launch_bounds__(kS2Threads, 1)
     for (int i = 0; i < kS2Stages; ++i) {
       mbar_init(&bars->st_full[i], 1);
       mbar_init(&bars->st_conv[i], 2);
-      mbar_init(&bars->st_free[i], 1);
+      mbar_init(&bars->st_free[i], 2);
     }
     for (int i = 0; i < 2; ++i) {
-      mbar_init(&bars->xh_ready[i], 8);
       mbar_init(&bars->m3_done[i], 1);
-      mbar_init(&bars->u_ready[i], 8);
       mbar_init(&bars->m4_done[i], 1);
     }
     bars->abort_flag = 0;
@@ -320,94 +368,6 @@ __global__ void __launch_bounds__(kS2Threads, 1)
         const size_t r = (size_t)(chunk0 + c) * H + h;
         bulk_g2s(smem + st * kS2StageBytes + kS2StRec, rec + r * kRecBytes, kRecBytes, &bars->st_full[st]);
         bulk_g2s(smem + st * kS2StageBytes + kS2StGate, gate + r * kGateFloats, kGateBytes, &bars->st_full[st]);
-      }
-    }
-  } else if (warp == 19) {
-    // ------------------------------------------------------------------------------------------- MMA issuer
-    if (lane == 0 && nc > 0) {
-      constexpr uint32_t id1 = make_idesc(0u, 128, 64, 1, 0);    // fp16, A MN-major (V tile), B K-major (A_b)
-      constexpr uint32_t id3 = make_idesc(0u, 128, 64, 0, 0);    // fp16, A from TMEM, B K-major (-W)
-      constexpr uint32_t id4 = make_idesc(0u, 128, 128, 0, 1);   // fp16, A K-major (U''), B MN-major (K tile)
-      auto issue1 = [&](int c) {  // DY_E = V^t A_b^t
-        const uint32_t sb = smem_base + (c % kS2Stages) * kS2StageBytes;
-#pragma unroll
-        for (int ks = 0; ks < 4; ++ks)
-          mma_f16_ss(tmem + 384, make_desc(sb + kS2StV + ks * 2048, 8192, 1024, 2),
-                     make_desc(sb + kS2StRec + kRecAb + ks * 32, 16, 1024, 2), id1, ks > 0);
-      };
-      auto issue3 = [&](int b, int c) {  // DY_b (+)= Xh_b (-W)^t
-        const uint32_t sb = smem_base + (c % kS2Stages) * kS2StageBytes;
-#pragma unroll
-        for (int ks = 0; ks < 8; ++ks)
-          mma_f16_ts(tmem + 384 + 64 * b, tmem + 256 + 64 * b + 8 * ks,
-                     make_desc(sb + kS2StRec + kRecW + (ks >> 2) * 8192 + (ks & 3) * 32, 16, 1024, 2), id3,
-                     (b == 0 || ks > 0) ? 1u : 0u);
-      };
-      auto issue4 = [&](int b, int c) {  // X_b += U''_b K
-        const uint32_t sb = smem_base + (c % kS2Stages) * kS2StageBytes;
-#pragma unroll
-        for (int ks = 0; ks < 4; ++ks)
-          mma_f16_ss(tmem + 128 * b, make_desc(smem_base + kS2OffU + b * 16384 + ks * 32, 16, 1024, 2),
-                     make_desc(sb + kS2StK + ks * 2048, 8192, 1024, 2), id4, 1u);
-      };
-      int cc[2] = {0, 0};          // current chunk of each chain
-      bool at3[2] = {true, true};  // next step of each chain: (3) or (4)
-      int seen = -1;               // converted stages observed by this thread: chunks <= seen
-      bool ok = true;
-      auto need_stage = [&](int c) {
-        while (ok && seen < c) {
-          ++seen;
-          ok = s2_wait(&bars->st_conv[seen % kS2Stages], (seen / kS2Stages) & 1, abort_flag);
-        }
-        tc_fence_after();
-      };
-      need_stage(0);
-      issue1(0);
-      uint32_t spins = 0;
-      while (ok && (cc[0] < nc || cc[1] < nc)) {
-        bool progress = false;
-#pragma unroll
-        for (int b = 0; b < 2; ++b) {
-          const int c = cc[b];
-          if (c >= nc) continue;
-          if (at3[b]) {
-            if (!mbar_test_wait(&bars->xh_ready[b], c & 1)) continue;
-            need_stage(c);
-            S2_STAMP(2, c, 0 + 4 * b);
-            issue3(b, c);
-            mma_commit(&bars->m3_done[b]);
-            S2_STAMP(2, c, 1 + 4 * b);
-            at3[b] = false;
-            progress = true;
-          } else {
-            if (!mbar_test_wait(&bars->u_ready[b], c & 1)) continue;
-            tc_fence_after();
-            S2_STAMP(2, c, 2 + 4 * b);
-            issue4(b, c);
-            mma_commit(&bars->m4_done[b]);
-            S2_STAMP(2, c, 3 + 4 * b);
-            if (cc[b ^ 1] > c) mma_commit(&bars->st_free[c % kS2Stages]);  // the other chain is already past this chunk
-            cc[b] = c + 1;
-            at3[b] = true;
-            progress = true;
-            if (b == 0 && c + 1 < nc) {
-              S2_STAMP(3, c, 0);
-              need_stage(c + 1);
-              S2_STAMP(3, c, 1);
-              issue1(c + 1);
-              S2_STAMP(3, c, 2);
-            }
-          }
-        }
-        if (progress) {
-          spins = 0;
-        } else if (++spins > 8000000u || ((spins & 4095u) == 0 && *abort_flag)) {
-          if (!*abort_flag) {
-            *abort_flag = 1;
-            atomicAdd(&g_timeout_count_enc, 1u);
-          }
-          break;
-        }
       }
     }
   } else if (warp >= 16) {
