@@ -6,7 +6,8 @@
 // tcgen05.mma kind::f16 on fp16 operands (11 significant bits, like tf32, at the full 16-bit rate):
 //     (1)_c  DY_E  = V^t A_b^t              A = the V tile (MN-major), B = A_b from the prep record   (E block only)
 //     (3)_c  DY_b += Xh_b (-W)^t            A = Xh_b = fp16(X_b) read from TMEM, B = -W from the prep record
-//     (4)_c  X_b  += U''_b K                A = U''_b = fp16(DY_b d_j) from smem, B = the K tile (MN-major)
+//     (4)_c  X_b  += U''_b K                A = U''_b = fp16(DY_b d_j) read from TMEM (it takes over the columns of
+//                                           Xh_b, dead once (3)_c has completed), B = the K tile (MN-major)
 // fp16 has a narrow exponent range, so the T block is held row-normalised: row r of the TMEM copy is T_r 2^s_r with
 // s_r re-chosen in every pass so that the row maximum sits in [2^14, 2^15); since (3) and (4) are linear in the row
 // the factor never has to be undone before the final write-out.  E rows live on the scale of v and stay unscaled.
@@ -52,8 +53,7 @@ constexpr int kS2Threads = 608;
 constexpr int kS2Stages = 3;
 constexpr int kS2StK = 0, kS2StV = 16384, kS2StRec = 32768, kS2StGate = 32768 + kRecBytes;
 constexpr int kS2StageBytes = 32768 + kRecBytes + 1024;
-constexpr int kS2OffU = kS2Stages * kS2StageBytes;  // per block b: U'' (fp16, 16 KB)
-constexpr int kS2OffXch = kS2OffU + 2 * 16384;      // T chain: row maxima of the two column halves
+constexpr int kS2OffXch = kS2Stages * kS2StageBytes;  // T chain: row maxima of the two column halves
 constexpr int kS2OffBar = kS2OffXch + 1024;
 constexpr int kS2Smem = kS2OffBar + 256 + 1024;
 
@@ -127,12 +127,11 @@ __device__ __forceinline__ void s2_issue3(uint32_t tmem, uint32_t sb, int b) {  
                make_desc(sb + kS2StRec + kRecW + (ks >> 2) * 8192 + (ks & 3) * 32, 16, 1024, 2), id3,
                (b == 0 || ks > 0) ? 1u : 0u);
 }
-__device__ __forceinline__ void s2_issue4(uint32_t tmem, uint32_t sb, uint32_t su, int b) {  // X_b += U''_b K
-  constexpr uint32_t id4 = make_idesc(0u, 128, 128, 0, 1);  // fp16, A K-major (U''), B MN-major (K tile)
+__device__ __forceinline__ void s2_issue4(uint32_t tmem, uint32_t sb, int b) {  // X_b += U''_b K
+  constexpr uint32_t id4 = make_idesc(0u, 128, 128, 0, 1);  // fp16, A from TMEM (U''), B MN-major (K tile)
 #pragma unroll
   for (int ks = 0; ks < 4; ++ks)
-    mma_f16_ss(tmem + 128 * b, make_desc(su + ks * 32, 16, 1024, 2), make_desc(sb + kS2StK + ks * 2048, 8192, 1024, 2),
-               id4, 1u);
+    mma_f16_ts(tmem + 128 * b, tmem + 256 + 64 * b + 8 * ks, make_desc(sb + kS2StK + ks * 2048, 8192, 1024, 2), id4, 1u);
 }
 
 template <bool kIsT>
@@ -145,7 +144,6 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
   const uint32_t lane_base = (uint32_t)(32 * q) << 16;
   const uint32_t tX = tmem + cX + lane_base + 64 * hf, tH = tmem + cH + lane_base + 32 * hf,
                  tD = tmem + cD + lane_base + 32 * hf;
-  uint8_t* urow = smem + kS2OffU + b * 16384 + (row >> 3) * 1024 + (row & 7) * 128;
   float* xch = reinterpret_cast<float*>(smem + kS2OffXch);
   int s_exp = 0;  // T chain: the TMEM copy of this row is T_row * 2^s_exp
 
@@ -243,7 +241,7 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     }
     __syncwarp();
 
-    // ---- epilogue: U''[:, j] = fp16(DY[:, j] d_j), K-major 128B swizzle (A operand of (4)); tokens [32 hf, 32 hf + 32)
+    // ---- epilogue: U''[:, j] = fp16(DY[:, j] d_j) -> TMEM (A operand of (4)); this thread: tokens [32 hf, 32 hf + 32)
     s2_wait_warp(&bars->m3_done[b], c & 1, abort_flag, lane);
     tc_fence_after();
     S2_STAMP(b, c, 2);
@@ -257,23 +255,22 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
         const float4 d0 = *reinterpret_cast<const float4*>(gt + 32 * hf + 8 * j8);
         const float4 d1 = *reinterpret_cast<const float4*>(gt + 32 * hf + 8 * j8 + 4);
         const float dd[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
-        uint32_t u[4];
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
           uint32_t u0 = y[8 * j8 + 2 * p], u1 = y[8 * j8 + 2 * p + 1];
           mul2v(u0, u1, dd[2 * p], dd[2 * p + 1]);
-          u[p] = pack_f16(__uint_as_float(u0), __uint_as_float(u1));
+          y[4 * j8 + p] = pack_f16(__uint_as_float(u0), __uint_as_float(u1));  // packed in place: slot 4 j8 + p < 8 j8 + 2 p
         }
-        *reinterpret_cast<uint4*>(urow + (((4 * hf + j8) ^ (row & 7)) * 16)) = make_uint4(u[0], u[1], u[2], u[3]);
       }
+      tmem_st16(tH - 16 * hf, y);  // columns [16 hf, 16 hf + 16) of the (dead) Xh region: tokens [32 hf, 32 hf + 32)
+      tmem_st_wait();
     }
-    fence_proxy_async();
     tc_fence_before();
     named_bar_sync(5 + b, 256);  // the whole chain has written U''
     S2_STAMP(b, c, 3);
     if (issuer) {
       tc_fence_after();
-      s2_issue4(tmem, smem_base + st * kS2StageBytes, smem_base + kS2OffU + b * 16384, b);
+      s2_issue4(tmem, smem_base + st * kS2StageBytes, b);
       mma_commit(&bars->m4_done[b]);
       mma_commit(&bars->st_free[st]);  // count 2: released when both chains' (4) of this chunk have completed
       if (!kIsT && c + 1 < nc) {
