@@ -95,9 +95,14 @@ __device__ __forceinline__ void block_zero(float (&acc)[2][4]) {
     for (int i = 0; i < 4; ++i) acc[nt][i] = 0.f;
 }
 
-__global__ void __launch_bounds__(kPrepThreads, 5)
+// Each CTA works through kPrepChunksPerCta consecutive chunks of one head and keeps the next chunk's k rows, g and
+// beta in flight in registers while it computes the current one: with one chunk per CTA 45 % of all stall samples
+// sat on the first global loads (profiles/r01b), which 5 CTAs per SM cannot hide.
+constexpr int kPrepChunksPerCta = 4;
+
+__global__ void __launch_bounds__(kPrepThreads, 4)
     prep_kernel(const __nv_bfloat16* __restrict__ k, const float* __restrict__ g, const float* __restrict__ beta,
-                const int2* __restrict__ chunk_meta, int H,
+                const int2* __restrict__ chunk_meta, int cap, int H,
                 uint8_t* __restrict__ rec, float* __restrict__ gate) {
   __shared__ __align__(16) uint8_t s_k[kC * kKsPitch * 2];  // K chunk (fp16); later the staged -W tile
   __shared__ __align__(16) float s_a[kC * kLPitch];         // L, inverted in place to A
@@ -106,19 +111,41 @@ __global__ void __launch_bounds__(kPrepThreads, 5)
   __shared__ float s_wsum;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int gq = lane >> 2, tq = lane & 3;
-  const int x = blockIdx.x, h = blockIdx.y;
-  const int2 meta = chunk_meta[x];  // (first token, valid tokens); (0, 0) beyond the last chunk of the call
-  const int t0 = meta.x, valid = meta.y;
-  if (valid == 0) return;
-
+  const int x0 = blockIdx.x * kPrepChunksPerCta, h = blockIdx.y;
+  int2 metas[kPrepChunksPerCta];  // (first token, valid tokens); (0, 0) beyond the last chunk of the call
+#pragma unroll
+  for (int i = 0; i < kPrepChunksPerCta; ++i) metas[i] = (x0 + i < cap) ? chunk_meta[x0 + i] : make_int2(0, 0);
+  uint4 kreg[kC * (kD / 8) / kPrepThreads];
+  float greg = 0.f, breg = 0.f;
+  auto prefetch = [&](int2 m) {  // rows >= valid are not read; their registers are ignored at the store
+#pragma unroll
+    for (int it = 0; it < kC * (kD / 8) / kPrepThreads; ++it) {
+      const int idx = tid + it * kPrepThreads;
+      const int r = idx / (kD / 8), c8 = idx % (kD / 8);
+      if (r < m.y) kreg[it] = *reinterpret_cast<const uint4*>(k + ((size_t)(m.x + r) * H + h) * kD + c8 * 8);
+    }
+    greg = 0.f, breg = 0.f;
+    if (tid < m.y) {
+      greg = g[(size_t)(m.x + tid) * H + h];
+      breg = beta[(size_t)(m.x + tid) * H + h];
+    }
+  };
+  if (metas[0].y > 0) prefetch(metas[0]);
   __half* ks = reinterpret_cast<__half*>(s_k);
+  const uint32_t ks_base = smem_u32(s_k);
+
+#pragma unroll 1
+  for (int ci = 0; ci < kPrepChunksPerCta; ++ci) {
+  const int x = x0 + ci;
+  const int valid = metas[ci].y;
+  if (valid == 0) break;
 #pragma unroll
   for (int it = 0; it < kC * (kD / 8) / kPrepThreads; ++it) {
     const int idx = tid + it * kPrepThreads;
     const int r = idx / (kD / 8), c8 = idx % (kD / 8);
     uint4 val = make_uint4(0, 0, 0, 0);
     if (r < valid) {
-      const uint4 raw = *reinterpret_cast<const uint4*>(k + ((size_t)(t0 + r) * H + h) * kD + c8 * 8);
+      const uint4 raw = kreg[it];
       val.x = pack_f16(__uint_as_float(raw.x << 16), __uint_as_float(raw.x & 0xffff0000u));
       val.y = pack_f16(__uint_as_float(raw.y << 16), __uint_as_float(raw.y & 0xffff0000u));
       val.z = pack_f16(__uint_as_float(raw.z << 16), __uint_as_float(raw.z & 0xffff0000u));
@@ -127,11 +154,8 @@ __global__ void __launch_bounds__(kPrepThreads, 5)
     *reinterpret_cast<uint4*>(ks + r * kKsPitch + c8 * 8) = val;
   }
   {  // a1: inclusive cumulative log-decay by a two-warp shuffle scan (warps 0 and 1 hold the 64 tokens)
-    float gv = 0.f, bv = 0.f;
-    if (tid < valid) {
-      gv = g[(size_t)(t0 + tid) * H + h];
-      bv = beta[(size_t)(t0 + tid) * H + h];
-    }
+    float gv = greg, bv = breg;
+    if (ci + 1 < kPrepChunksPerCta && metas[ci + 1].y > 0) prefetch(metas[ci + 1]);  // in flight during this chunk
     if (warp < 2) {
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
@@ -149,7 +173,6 @@ __global__ void __launch_bounds__(kPrepThreads, 5)
     }
   }
   __syncthreads();
-  const uint32_t ks_base = smem_u32(s_k);
 
   // ---- a2: Gram K K^t (lower block triangle): warp w owns rows [16w, 16w+16), n-tile pairs p <= w
   {
@@ -318,4 +341,6 @@ __global__ void __launch_bounds__(kPrepThreads, 5)
   float* go = gate + ((size_t)x * H + h) * kGateFloats;
   if (tid < kC) go[tid] = expf(s_g[kC - 1] - s_g[tid]);
   else if (tid < kGateFloats) go[tid] = (tid == kC) ? expf(s_g[kC - 1]) : 0.f;
+  __syncthreads();  // s_k (staged -W), s_a, s_g are free for the next chunk
+  }
 }

@@ -161,7 +161,8 @@ int encode_tensor(const EncodeArgs& a) {
   if (rc != HYPIC_OK) return rc;
   chunk_offsets_kernel<<<1, 1024, 0, a.stream>>>(a.cu_seqlens, a.n_seg, chunk_off, chunk_meta, (int)cap);
   note_launch();
-  prep_kernel<<<dim3((unsigned)cap, a.H), kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, chunk_meta, a.H, rec, gate);
+  prep_kernel<<<dim3((unsigned)((cap + kPrepChunksPerCta - 1) / kPrepChunksPerCta), a.H), kPrepThreads, 0, a.stream>>>(
+      kp, a.g, a.beta, chunk_meta, (int)cap, a.H, rec, gate);
   note_launch();
   scan2_kernel<<<dim3(a.H, a.n_seg), kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, a.H, rec, gate,
                                                                      a.E, a.T);
