@@ -84,7 +84,8 @@ size_t hypic_segment_encode_workspace(int32_t n_seg, int32_t t_total, int32_t H,
  * A zero-length segment yields E = 0, T = I.  n_seg = 0 or t_total = 0 with n_seg > 0 are valid.
  * Built envelope: dk in {64, 128}; dv in [1, 1024] for the SIMT family, dv = dk = 128 for the tensor family
  * (bf16 k/v, scalar gate; its tensor-core operands are fp16, so it additionally assumes finite |k|, |v| <= 65504 and
- * beta |k|^2 within the stable range of the recurrence -- callers outside that range select HYPIC_IMPL_SIMT);
+ * beta |k|^2 within the stable range of the recurrence and a per-chunk log-decay >= -9, see
+ * hypic_envelope_violation_count -- callers outside that range select HYPIC_IMPL_SIMT);
  * H, n_seg, lengths arbitrary.  Inputs are only read; E and T are fully overwritten.
  */
 int hypic_segment_encode(const void* k, const void* v, const float* g, const float* beta,
@@ -127,6 +128,16 @@ int hypic_compose_impl_for(int32_t H, int32_t dk, int32_t dv);
  * Test / diagnostics only.
  */
 unsigned int hypic_debug_timeout_count(void);
+
+/*
+ * hypic_envelope_violation_count: the tensor-family encode computes in fp16 operands and therefore assumes that the
+ * cumulative log-decay of every 64-token chunk stays above -9 (gamma >= 1.2e-4 inside a chunk; the benchmark
+ * distributions stay above -6.4) and that g and beta are finite.  Its prep kernel counts the (chunk, head) pairs that
+ * break this since library load; such pairs may come out with a relative error above the family's tolerance, and the
+ * caller should re-run the call with HYPIC_IMPL_SIMT, which has no such limit.  Synchronises the device; 0 = never
+ * violated; 0xffffffff = the query itself failed.
+ */
+unsigned int hypic_envelope_violation_count(void);
 
 /* hypic_status_string: static, NUL-terminated description of a status code (never NULL). */
 const char* hypic_status_string(int status);

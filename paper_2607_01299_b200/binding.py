@@ -28,7 +28,7 @@ HYPIC_IMPL_TENSOR = 2
 EXPORTS = (
     "hypic_set_impl", "hypic_get_impl", "hypic_segment_encode_workspace", "hypic_segment_encode", "hypic_compose",
     "hypic_status_string", "hypic_version", "hypic_last_launch_count", "hypic_encode_impl_for",
-    "hypic_compose_impl_for", "hypic_debug_timeout_count",
+    "hypic_compose_impl_for", "hypic_debug_timeout_count", "hypic_envelope_violation_count",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -75,6 +75,8 @@ def load_library() -> ctypes.CDLL:
     lib.hypic_compose_impl_for.restype = ctypes.c_int
     lib.hypic_debug_timeout_count.argtypes = []
     lib.hypic_debug_timeout_count.restype = ctypes.c_uint
+    lib.hypic_envelope_violation_count.argtypes = []
+    lib.hypic_envelope_violation_count.restype = ctypes.c_uint
     _lib = lib
     return lib
 
@@ -103,6 +105,10 @@ def hypic_encode_impl_for(H: int, dk: int, dv: int, kv_dtype: int, gate: int) ->
 
 def hypic_compose_impl_for(H: int, dk: int, dv: int) -> int:
     return int(load_library().hypic_compose_impl_for(H, dk, dv))
+
+
+def hypic_envelope_violation_count() -> int:
+    return int(load_library().hypic_envelope_violation_count())
 
 
 def hypic_debug_timeout_count() -> int:

@@ -58,6 +58,7 @@ bool compose_tensor_shape_ok(int32_t H, int32_t dk, int32_t dv);
 inline bool compose_tensor_supported(const ComposeArgs& a) { return compose_tensor_shape_ok(a.H, a.dk, a.dv); }
 int compose_tensor(const ComposeArgs& a);
 unsigned int debug_timeout_count_encode();
+unsigned int envelope_violation_count_encode();
 unsigned int debug_timeout_count();  // bounded-wait expiries in the tensor kernels since load (0 = healthy)
 
 // Device properties cached per process (SM count, opt-in shared memory).

@@ -339,6 +339,7 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
     *reinterpret_cast<uint4*>(out + kRecW + idx * 16) = *reinterpret_cast<const uint4*>(s_k + idx * 16);
   }
   float* go = gate + ((size_t)x * H + h) * kGateFloats;
+  if (tid == 0 && !(s_g[kC - 1] >= -9.f && s_g[kC - 1] <= 0.f)) atomicAdd(&g_envelope_count_enc, 1u);  // also NaN
   if (tid < kC) go[tid] = expf(s_g[kC - 1] - s_g[tid]);
   else if (tid < kGateFloats) go[tid] = (tid == kC) ? expf(s_g[kC - 1]) : 0.f;
   __syncthreads();  // s_k (staged -W), s_a, s_g are free for the next chunk

@@ -77,9 +77,10 @@ __global__ void chunk_offsets_kernel(const int32_t* __restrict__ cu_seqlens, int
 }
 
 // ------------------------------------------------------------------------------------------------ K1, K2
-#include "encode_prep.cuh"
-
 __device__ unsigned int g_timeout_count_enc = 0;
+__device__ unsigned int g_envelope_count_enc = 0;  // (chunk, head) pairs outside the fp16 envelope (hypic.h)
+
+#include "encode_prep.cuh"
 
 #include "encode_scan2.cuh"
 
@@ -176,6 +177,13 @@ extern "C" int hypic_debug_timeline(long long* out, int n) {
   return cudaMemcpyFromSymbol(out, g_s2_timeline, sizeof(long long) * (size_t)n) == cudaSuccess ? 0 : 1;
 }
 #endif
+
+unsigned int envelope_violation_count_encode() {
+  unsigned int v = 0;
+  if (cudaDeviceSynchronize() != cudaSuccess) return 0xffffffffu;
+  if (cudaMemcpyFromSymbol(&v, g_envelope_count_enc, sizeof(v)) != cudaSuccess) return 0xffffffffu;
+  return v;
+}
 
 unsigned int debug_timeout_count_encode() {
   unsigned int v = 0;

@@ -141,6 +141,8 @@ int hypic_version(void) { return HYPIC_VERSION; }
 
 unsigned int hypic_debug_timeout_count(void) { return debug_timeout_count(); }
 
+unsigned int hypic_envelope_violation_count(void) { return envelope_violation_count_encode(); }
+
 int hypic_last_launch_count(void) { return g_launch_count; }
 
 }  // extern "C"

@@ -272,3 +272,46 @@ def test_cfg4_compose_stress_sampled_requests():
     ref = oracle_compose_units(req.S_in, E, T, req.seg_ids, req.cu_segs, units)
     ri, hi = torch.tensor([u[0] for u in units]), torch.tensor([u[1] for u in units])
     check_E(S[ri, hi][:, None], ref, TOL_F32, "S_out")
+
+
+# ------------------------------------------------- tensor family: range handling of the fp16 operands
+@pytest.mark.parametrize("case", ["strong_erasure", "no_gate_long", "v_x100", "v_x0.01", "gate_x2"])
+def test_tensor_family_operand_range(case):
+    """The tensor family feeds fp16 operands to tcgen05.mma; T rows are held row-normalised in TMEM.
+    Cases that move T, E or the gate far from the benchmark distributions must still meet the bf16 tolerance:
+    beta = 1 (every key is fully erased, T decays by projections alone), g = 0 over 1536 tokens (no gate decay at
+    all, T shrinks only through the delta rule), v scaled by 100 and by 0.01, and g ~ U(-1, 0) (T underflows fp32
+    within a few hundred tokens: absolute criterion of reading S6)."""
+    lens = [1536, 200] if case == "no_gate_long" else [384, 130, 64]
+    inp = wl.make_encode_inputs(lens, 2, 128, 128, kv_dtype=torch.bfloat16, g_lo=-0.05, seed=wl.seed_for(1, 31),
+                                device="cuda")
+    if case == "strong_erasure":
+        inp.beta.fill_(1.0)
+    elif case == "no_gate_long":
+        inp.g.zero_()
+    elif case == "v_x100":
+        inp.v.mul_(100.0)
+    elif case == "v_x0.01":
+        inp.v.mul_(0.01)
+    elif case == "gate_x2":
+        inp.g.mul_(2.0)
+    before = hb.hypic_envelope_violation_count()
+    E, T = gpu_encode(inp, hb.HYPIC_IMPL_TENSOR)
+    E_ref, T_ref = oracle_encode(inp)
+    check_E(E, E_ref, TOL_BF16)
+    check_T(T, T_ref, TOL_BF16)
+    assert hb.hypic_envelope_violation_count() == before
+
+
+def test_tensor_family_envelope_guard():
+    """g ~ U(-1, 0): the cumulative log-decay of a chunk (~ -32) is far outside the fp16 envelope of the tensor family
+    (hypic.h); its prep kernel must count the violation, and the SIMT family must still match the oracle."""
+    inp = wl.make_encode_inputs([130, 64], 2, 128, 128, kv_dtype=torch.bfloat16, g_lo=-1.0, seed=wl.seed_for(1, 32),
+                                device="cuda")
+    before = hb.hypic_envelope_violation_count()
+    gpu_encode(inp, hb.HYPIC_IMPL_TENSOR)
+    assert hb.hypic_envelope_violation_count() > before
+    E, T = gpu_encode(inp, hb.HYPIC_IMPL_SIMT)
+    E_ref, T_ref = oracle_encode(inp)
+    check_E(E, E_ref, TOL_BF16)
+    check_T(T, T_ref, TOL_BF16)
