@@ -3,19 +3,23 @@
 // Row a6 of SURVEY.md section 8(a):  S <- S T_i + E_i  (Eq. 6 as the chain of Eq. 4 steps) for one
 // (request, head) chain per CTA.  The chain is HBM-bound (128 KB of (T_i, E_i) per 4.2 MFLOP step), so the kernel
 // is a streaming pipeline; tensor cores only keep the fp32-accurate GEMM off the critical path:
-//   * S lives in TMEM for the whole chain as two tf32 operands S_hi = rna_tf32(S), S_lo = S - S_hi
-//     (A operand of tcgen05.mma kind::tf32 read from TMEM: lane = row of S, column = k);
-//   * T_i streams HBM -> smem in 32-row slabs (1-D bulk async copies on mbarriers), converter warps split
-//     each slab into T_hi / T_lo in the 32-bit MN-major "128B swizzle, 32B base" layout (B operand);
-//   * 3xTF32:  D = S_hi T_hi + S_lo T_hi + S_hi T_lo  (fp32 accumulate in TMEM; the hardware truncates tf32
-//     operands, which is why hi is rounded in software and lo carries the remainder);
-//   * round-trip warps (two per TMEM lane quarter) read D (tcgen05.ld), add E_i (staged by TMA tensor boxes of
-//     32 rows x 128 B with the 128B swizzle, so that row-per-thread reads are bank-conflict free; per-row bulk
-//     copies were measured to cost ~46 cycles of TMA issue each and dominated the step), and write the next
-//     S_hi / S_lo (tcgen05.st), or S_out after the last step.
+//   * S lives in TMEM for the whole chain as two fp16 operands of a two-term split: row m is normalised by a power
+//     of two 2^-r_m (row maximum in [2^13, 2^14)), S_hi = fp16(S 2^-r), S_lo = fp16(S 2^-r - S_hi), packed two per
+//     column (A operand of tcgen05.mma kind::f16 read from TMEM: lane = row of S);
+//   * T_i streams HBM -> smem in 32-row slabs (1-D bulk async copies on mbarriers), converter warps split each slab
+//     into T_hi = fp16(2^14 T), T_lo = fp16(2^14 T - T_hi) in the 16-bit MN-major 128B-swizzle layout (B operand);
+//     the constant 2^14 keeps T_lo out of fp16's subnormals down to |t| ~ 1e-5 (|t| < 4 is the envelope: T of a
+//     stable recurrence has spectral norm <= 1);
+//   * D = S_hi T_hi + S_lo T_hi + S_hi T_lo: 22 significant bits per product, fp32 accumulate in TMEM, at the
+//     16-bit rate (K = 16 per instruction: half the MMA time of the 3xTF32 scheme this replaces, half the
+//     shared-memory and TMEM traffic);
+//   * round-trip warps (two per TMEM lane quarter) read D (tcgen05.ld), undo the scales (2^(r_m - 14), fp32), add E_i
+//     (staged by TMA tensor boxes of 32 rows x 128 B with the 128B swizzle, so that row-per-thread reads are
+//     bank-conflict free), and write the next S_hi / S_lo (tcgen05.st), or S_out after the last step.
 // S_in enters as "step -1" (D = 0, E = S_in).  All waits are bounded: a protocol error raises the timeout
 // counter (hypic_debug_timeout_count) instead of hanging the GPU.
 #include <cuda.h>
+#include <cuda_fp16.h>
 #include <string.h>
 
 #include "common.cuh"
@@ -30,15 +34,18 @@ using namespace ptx;
 
 constexpr int kD = 128;
 constexpr int kSlabBytes = 32 * kD * 4;  // 32 rows of T (or E): 16 KB
-constexpr int kNRaw = 3;                 // raw T slabs in flight
-constexpr int kNHl = 3;                  // converted (hi, lo) slab pairs
+constexpr int kNRaw = 6;                 // raw T slabs in flight
+constexpr int kNHl = 3;                  // converted (hi, lo) slab pairs (fp16: 8 KB + 8 KB)
+constexpr int kHlBytes = kSlabBytes;     // one converted pair
+constexpr float kTScale = 16384.f;       // 2^14, applied to T before the fp16 split
 constexpr int kESlotBytes = kSlabBytes;  // 4 TMA boxes of 32 rows x 128 B (128B swizzle: conflict-free row reads)
 constexpr int kThreads = 480;            // warp 0 T producer, 1 MMA, 2 E producer, 3-6 converters, 7-14 round trip
 
 constexpr int kOffHl = 0;
-constexpr int kOffRaw = kOffHl + kNHl * 2 * kSlabBytes;
+constexpr int kOffRaw = kOffHl + kNHl * kHlBytes;
 constexpr int kOffE = kOffRaw + kNRaw * kSlabBytes;
-constexpr int kOffBar = kOffE + 4 * kESlotBytes;
+constexpr int kOffXch = kOffE + 4 * kESlotBytes;  // row maxima of the two column halves (round trip)
+constexpr int kOffBar = kOffXch + 1024;
 constexpr int kSmemBytes = kOffBar + 256 + 1024;  // + barriers + alignment slack
 
 struct Bars {
@@ -59,10 +66,23 @@ __device__ __forceinline__ bool wait_or_abort(uint64_t* bar, uint32_t parity, vo
   return false;
 }
 
-__device__ __forceinline__ float rna_tf32(float x) {
-  uint32_t r;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
-  return __uint_as_float(r);
+// (x0, x1) -> packed fp16 hi and packed fp16 lo = fp16(x - hi)
+__device__ __forceinline__ void split_f16(float x0, float x1, uint32_t& hi, uint32_t& lo) {
+  const __half2 h = __floats2half2_rn(x0, x1);
+  const float2 hf = __half22float2(h);
+  const __half2 l = __floats2half2_rn(x0 - hf.x, x1 - hf.y);
+  hi = *reinterpret_cast<const uint32_t*>(&h);
+  lo = *reinterpret_cast<const uint32_t*>(&l);
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
+      "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+      "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+      : "memory");
 }
 
 __device__ __forceinline__ void tma_load_2d(void* dst_smem, const CUtensorMap* tm, int c0, int c1, uint64_t* bar) {
@@ -128,7 +148,7 @@ __global__ void __launch_bounds__(kThreads, 1)
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = bars->tmem_base;
-  const uint32_t tD = tmem, tAhi = tmem + 128, tAlo = tmem + 256;
+  const uint32_t tD = tmem, tAhi = tmem + 128, tAlo = tmem + 192;  // D fp32 128 columns; S_hi, S_lo fp16 64 each
 
   if (warp == 0) {
     // ---------------------------------------------------------------- T producer: 16 KB slabs into the raw ring
@@ -148,7 +168,7 @@ __global__ void __launch_bounds__(kThreads, 1)
   } else if (warp == 1) {
     // ---------------------------------------------------------------- MMA issuer (one thread)
     if (lane == 0) {
-      constexpr uint32_t idesc = make_idesc(2u, 128, 128, 0, 1);  // tf32, M = N = 128, B MN-major
+      constexpr uint32_t idesc = make_idesc(0u, 128, 128, 0, 1);  // fp16, M = N = 128, A from TMEM, B MN-major
       uint32_t it = 0;
       for (int i = 0; i < n; ++i) {
         wait_or_abort(&bars->a_ready, i & 1, abort_flag);
@@ -157,17 +177,17 @@ __global__ void __launch_bounds__(kThreads, 1)
           const uint32_t slot = it % kNHl, ph = (it / kNHl) & 1;
           wait_or_abort(&bars->hl_full[slot], ph, abort_flag);
           tc_fence_after();
-          const uint32_t hi_addr = smem_u32(smem + kOffHl + slot * 2 * kSlabBytes);
-          const uint32_t lo_addr = hi_addr + kSlabBytes;
+          const uint32_t hi_addr = smem_u32(smem + kOffHl + slot * kHlBytes);
+          const uint32_t lo_addr = hi_addr + kHlBytes / 2;
 #pragma unroll
-          for (int ks = 0; ks < 4; ++ks) {
-            // 8 rows of T per instruction = two 4-row atoms of 512 B; 32-column chunks are 4 KB apart
-            const uint64_t bhi = make_desc(hi_addr + ks * 1024, 4096, 512, 1);
-            const uint64_t blo = make_desc(lo_addr + ks * 1024, 4096, 512, 1);
-            const uint32_t acol = j * 32 + ks * 8;
-            mma_tf32_ts(tD, tAhi + acol, bhi, idesc, (j | ks) > 0);
-            mma_tf32_ts(tD, tAlo + acol, bhi, idesc, 1);
-            mma_tf32_ts(tD, tAhi + acol, blo, idesc, 1);
+          for (int ks = 0; ks < 2; ++ks) {
+            // 16 rows of T per instruction = two 8-row atoms of 1 KB; the two 64-column boxes are 4 KB apart
+            const uint64_t bhi = make_desc(hi_addr + ks * 2048, 4096, 1024, 2);
+            const uint64_t blo = make_desc(lo_addr + ks * 2048, 4096, 1024, 2);
+            const uint32_t acol = j * 16 + ks * 8;
+            mma_f16_ts(tD, tAhi + acol, bhi, idesc, (j | ks) > 0);
+            mma_f16_ts(tD, tAlo + acol, bhi, idesc, 1);
+            mma_f16_ts(tD, tAhi + acol, blo, idesc, 1);
           }
           mma_commit(&bars->hl_empty[slot]);
         }
@@ -212,19 +232,19 @@ __global__ void __launch_bounds__(kThreads, 1)
 #pragma unroll
         for (int u = 0; u < 8; ++u) x[u] = raw[ctid + 128 * u];
         wait_or_abort(&bars->hl_empty[hslot], hph ^ 1, abort_flag);
-        uint8_t* hi_t = smem + kOffHl + hslot * 2 * kSlabBytes;
-        uint8_t* lo_t = hi_t + kSlabBytes;
+        uint8_t* hi_t = smem + kOffHl + hslot * kHlBytes;
+        uint8_t* lo_t = hi_t + kHlBytes / 2;
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
           const int idx = ctid + 128 * u;
           const int k = idx >> 5, n0 = (idx & 31) * 4;  // row of the slab, first of 4 columns
-          const uint32_t off = (n0 >> 5) * 4096 + (k >> 2) * 512 + (k & 3) * 128 +
-                               ((((n0 & 31) >> 3) ^ (k & 3)) * 32) + ((n0 & 7) * 4);
-          float4 hi, lo;
-          hi.x = rna_tf32(x[u].x), hi.y = rna_tf32(x[u].y), hi.z = rna_tf32(x[u].z), hi.w = rna_tf32(x[u].w);
-          lo.x = x[u].x - hi.x, lo.y = x[u].y - hi.y, lo.z = x[u].z - hi.z, lo.w = x[u].w - hi.w;
-          *reinterpret_cast<float4*>(hi_t + off) = hi;
-          *reinterpret_cast<float4*>(lo_t + off) = lo;
+          const uint32_t off = (n0 >> 6) * 4096 + (k >> 3) * 1024 + (k & 7) * 128 + ((((n0 & 63) >> 3) ^ (k & 7)) * 16) +
+                               (n0 & 7) * 2;
+          uint2 hi, lo;
+          split_f16(x[u].x * kTScale, x[u].y * kTScale, hi.x, lo.x);
+          split_f16(x[u].z * kTScale, x[u].w * kTScale, hi.y, lo.y);
+          *reinterpret_cast<uint2*>(hi_t + off) = hi;
+          *reinterpret_cast<uint2*>(lo_t + off) = lo;
         }
         fence_proxy_async();
         __syncwarp();
@@ -243,6 +263,8 @@ __global__ void __launch_bounds__(kThreads, 1)
     const uint8_t* erow = smem + kOffE + q * kESlotBytes + lane * 128;
     float* out_row = S_out + (size_t)unit * mat + (size_t)row * kD;
     uint32_t ecount = 0;
+    float* xch = reinterpret_cast<float*>(smem + kOffXch);
+    float unscale = 1.f;  // D of step s holds 2^(14 - r_m) (S T): r_m = this row's normalisation chosen after step s - 1
     for (int s = -1; s < n; ++s) {
       const bool have_e = (s >= 0) || (S_in != nullptr);
       const bool last = (s == n - 1);
@@ -251,41 +273,28 @@ __global__ void __launch_bounds__(kThreads, 1)
         tc_fence_after();
       }
       if (have_e) wait_or_abort(&bars->e_full[q], ecount & 1, abort_flag);
-#pragma unroll 1
-      for (int cb = 2 * half; cb < 2 * half + 2; ++cb) {
-        uint32_t d[32];
+      float xv[64];
+#pragma unroll
+      for (int cc = 0; cc < 2; ++cc) {
+        const int cb = 2 * half + cc;
         if (s >= 0) {
+          uint32_t d[32];
           tmem_ld32(tD + lane_base + 32 * cb, d);
           tmem_ld_wait();
+#pragma unroll
+          for (int c = 0; c < 32; ++c) xv[32 * cc + c] = __uint_as_float(d[c]) * unscale;
         } else {
 #pragma unroll
-          for (int c = 0; c < 32; ++c) d[c] = 0u;
+          for (int c = 0; c < 32; ++c) xv[32 * cc + c] = 0.f;
         }
-        float xv[32];
-#pragma unroll
-        for (int c = 0; c < 32; ++c) xv[c] = __uint_as_float(d[c]);
         if (have_e) {
           const uint8_t* eb = erow + cb * 4096;
 #pragma unroll
           for (int u = 0; u < 8; ++u) {
             const float4 e = *reinterpret_cast<const float4*>(eb + ((u ^ (lane & 7)) * 16));
-            xv[4 * u] += e.x, xv[4 * u + 1] += e.y, xv[4 * u + 2] += e.z, xv[4 * u + 3] += e.w;
+            xv[32 * cc + 4 * u] += e.x, xv[32 * cc + 4 * u + 1] += e.y, xv[32 * cc + 4 * u + 2] += e.z,
+                xv[32 * cc + 4 * u + 3] += e.w;
           }
-        }
-        if (last) {
-          float4* o4 = reinterpret_cast<float4*>(out_row + 32 * cb);
-#pragma unroll
-          for (int u = 0; u < 8; ++u) o4[u] = make_float4(xv[4 * u], xv[4 * u + 1], xv[4 * u + 2], xv[4 * u + 3]);
-        } else {
-          uint32_t hi[32], lo[32];
-#pragma unroll
-          for (int c = 0; c < 32; ++c) {
-            const float hf = rna_tf32(xv[c]);
-            hi[c] = __float_as_uint(hf);
-            lo[c] = __float_as_uint(xv[c] - hf);
-          }
-          tmem_st32(tAhi + lane_base + 32 * cb, hi);
-          tmem_st32(tAlo + lane_base + 32 * cb, lo);
         }
       }
       if (have_e) {
@@ -293,7 +302,28 @@ __global__ void __launch_bounds__(kThreads, 1)
         if (lane == 0) mbar_arrive(&bars->e_empty[q]);
         ++ecount;
       }
-      if (!last) {
+      if (last) {
+        float4* o4 = reinterpret_cast<float4*>(out_row + 64 * half);
+#pragma unroll
+        for (int u = 0; u < 16; ++u) o4[u] = make_float4(xv[4 * u], xv[4 * u + 1], xv[4 * u + 2], xv[4 * u + 3]);
+      } else {
+        // row normalisation: maximum of the whole row (both column halves) into [2^13, 2^14)
+        float m = 0.f;
+#pragma unroll
+        for (int c = 0; c < 64; c += 2) m = fmaxf(m, fmaxf(fabsf(xv[c]), fabsf(xv[c + 1])));
+        xch[2 * row + half] = m;
+        named_bar_sync(1 + q, 64);
+        m = fmaxf(m, xch[2 * row + (half ^ 1)]);
+        const int e = (int)(__float_as_uint(m) >> 23);
+        int r = (e == 0) ? 0 : e - 140;  // max in [2^(e-127), 2^(e-126)) -> 2^-r max in [2^13, 2^14)
+        r = max(-100, min(100, r));
+        const float sc = __uint_as_float((uint32_t)(127 - r) << 23);
+        unscale = __uint_as_float((uint32_t)(127 + r - 14) << 23);
+        uint32_t hi[32], lo[32];
+#pragma unroll
+        for (int c = 0; c < 32; ++c) split_f16(xv[2 * c] * sc, xv[2 * c + 1] * sc, hi[c], lo[c]);
+        tmem_st32(tAhi + lane_base + 32 * half, hi);
+        tmem_st32(tAlo + lane_base + 32 * half, lo);
         tmem_st_wait();
         tc_fence_before();
         __syncwarp();
