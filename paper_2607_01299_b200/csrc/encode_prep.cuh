@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
     prep_kernel(const __nv_bfloat16* __restrict__ k, const float* __restrict__ g, const float* __restrict__ beta,
                 const int2* __restrict__ chunk_meta, int cap, int H,
                 uint8_t* __restrict__ rec, float* __restrict__ gate) {
-  __shared__ __align__(16) uint8_t s_k[kC * kKsPitch * 2];  // K chunk (fp16); later the staged -W tile
+  __shared__ __align__(16) uint8_t s_k[kC * kKsPitch * 2];  // K chunk (fp16)
   __shared__ __align__(16) float s_a[kC * kLPitch];         // L, inverted in place to A
   __shared__ __align__(16) float s_m[32 * kMPitch];         // temporaries of the block merges
   __shared__ __align__(16) float s_g[kC], s_b[kC], s_bg[kC];
@@ -273,41 +273,54 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
   }
   __syncthreads();
 
-  // ---- -W = -(A diag(beta gamma)) K with mma.sync: warp w rows [16w, 16w+16), k-steps kk <= w (A is lower triangular)
-  float wacc[16][4];
+  // ---- -W = -(A diag(beta gamma)) K with mma.sync: warp w rows [16w, 16w+16), k-steps kk <= w (A is lower
+  // triangular), in two halves of 64 columns; the fp16 fragments go straight to the record in its K-major
+  // 128B-swizzled two-box layout (4-byte stores; each 16-byte chunk is completed by the four lanes of a quad)
+  uint8_t* out = rec + ((size_t)x * H + h) * kRecBytes;
+#pragma unroll 1
+  for (int nh = 0; nh < 2; ++nh) {
+    float wacc[8][4];
 #pragma unroll
-  for (int nt = 0; nt < 16; ++nt)
+    for (int nt = 0; nt < 8; ++nt)
 #pragma unroll
-    for (int i = 0; i < 4; ++i) wacc[nt][i] = 0.f;
+      for (int i = 0; i < 4; ++i) wacc[nt][i] = 0.f;
 #pragma unroll
-  for (int kk = 0; kk < 4; ++kk) {
-    if (kk > warp) continue;
-    uint32_t a[4];
-    {
-      const int r0 = 16 * warp + gq, c0 = 16 * kk + 2 * tq;
-      const float g0 = s_bg[c0], g1 = s_bg[c0 + 1], g8 = s_bg[c0 + 8], g9 = s_bg[c0 + 9];
-      const float2 p0 = *reinterpret_cast<const float2*>(s_a + r0 * kLPitch + c0);
-      const float2 p1 = *reinterpret_cast<const float2*>(s_a + (r0 + 8) * kLPitch + c0);
-      const float2 p2 = *reinterpret_cast<const float2*>(s_a + r0 * kLPitch + c0 + 8);
-      const float2 p3 = *reinterpret_cast<const float2*>(s_a + (r0 + 8) * kLPitch + c0 + 8);
-      a[0] = pack_f16(p0.x * g0, p0.y * g1);
-      a[1] = pack_f16(p1.x * g0, p1.y * g1);
-      a[2] = pack_f16(p2.x * g8, p2.y * g9);
-      a[3] = pack_f16(p3.x * g8, p3.y * g9);
+    for (int kk = 0; kk < 4; ++kk) {
+      if (kk > warp) continue;
+      uint32_t a[4];
+      {
+        const int r0 = 16 * warp + gq, c0 = 16 * kk + 2 * tq;
+        const float g0 = s_bg[c0], g1 = s_bg[c0 + 1], g8 = s_bg[c0 + 8], g9 = s_bg[c0 + 9];
+        const float2 p0 = *reinterpret_cast<const float2*>(s_a + r0 * kLPitch + c0);
+        const float2 p1 = *reinterpret_cast<const float2*>(s_a + (r0 + 8) * kLPitch + c0);
+        const float2 p2 = *reinterpret_cast<const float2*>(s_a + r0 * kLPitch + c0 + 8);
+        const float2 p3 = *reinterpret_cast<const float2*>(s_a + (r0 + 8) * kLPitch + c0 + 8);
+        a[0] = pack_f16(p0.x * g0, p0.y * g1);
+        a[1] = pack_f16(p1.x * g0, p1.y * g1);
+        a[2] = pack_f16(p2.x * g8, p2.y * g9);
+        a[3] = pack_f16(p3.x * g8, p3.y * g9);
+      }
+      // B fragments (k = token, n = dk) by transposing ldmatrix over the [token][dk] tile, two n-tiles at a time
+      const int tok = 16 * kk + (lane & 7) + ((lane >> 3) & 1) * 8;
+#pragma unroll
+      for (int np = 0; np < 4; ++np) {
+        uint32_t b[4];
+        ldmatrix_x4_trans(b, ks_base + (uint32_t)(tok * kKsPitch + 64 * nh + 8 * (2 * np + (lane >> 4))) * 2u);
+        mma_f16_16816(wacc[2 * np], a[0], a[1], a[2], a[3], b[0], b[1]);
+        mma_f16_16816(wacc[2 * np + 1], a[0], a[1], a[2], a[3], b[2], b[3]);
+      }
     }
-    // B fragments (k = token, n = dk) by transposing ldmatrix over the [token][dk] tile, two n-tiles at a time
-    const int tok = 16 * kk + (lane & 7) + ((lane >> 3) & 1) * 8;
 #pragma unroll
-    for (int np = 0; np < 8; ++np) {
-      uint32_t b[4];
-      ldmatrix_x4_trans(b, ks_base + (uint32_t)(tok * kKsPitch + 8 * (2 * np + (lane >> 4))) * 2u);
-      mma_f16_16816(wacc[2 * np], a[0], a[1], a[2], a[3], b[0], b[1]);
-      mma_f16_16816(wacc[2 * np + 1], a[0], a[1], a[2], a[3], b[2], b[3]);
-    }
+    for (int nt = 0; nt < 8; ++nt)
+#pragma unroll
+      for (int hh = 0; hh < 2; ++hh) {
+        const int r = 16 * warp + gq + 8 * hh;
+        const uint32_t off = nh * 8192 + (r >> 3) * 1024 + (r & 7) * 128 + ((nt ^ (r & 7)) * 16) + tq * 4;
+        *reinterpret_cast<uint32_t*>(out + kRecW + off) = pack_f16(-wacc[nt][2 * hh], -wacc[nt][2 * hh + 1]);
+      }
   }
 
   // ---- A_b = A diag(beta) as an fp16 B tile (K-major, 128B swizzle: row r, 16-byte chunk j8 at ((j8 ^ (r & 7)) * 16))
-  uint8_t* out = rec + ((size_t)x * H + h) * kRecBytes;
 #pragma unroll
   for (int it = 0; it < kC * 8 / kPrepThreads; ++it) {
     const int idx = tid + it * kPrepThreads;
@@ -321,27 +334,10 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
         make_uint4(pack_f16(v0.x * b0.x, v0.y * b0.y), pack_f16(v0.z * b0.z, v0.w * b0.w),
                    pack_f16(v1.x * b1.x, v1.y * b1.y), pack_f16(v1.z * b1.z, v1.w * b1.w));
   }
-  __syncthreads();  // K is dead: stage -W over it, already in the K-major 128B-swizzled two-box layout
-#pragma unroll
-  for (int nt = 0; nt < 16; ++nt)
-#pragma unroll
-    for (int hh = 0; hh < 2; ++hh) {
-      const int r = 16 * warp + gq + 8 * hh;
-      const int col = 8 * nt + 2 * tq;
-      const uint32_t off = (col >> 6) * 8192 + (r >> 3) * 1024 + (r & 7) * 128 + ((((col & 63) >> 3) ^ (r & 7)) * 16) +
-                           (col & 7) * 2;
-      *reinterpret_cast<uint32_t*>(s_k + off) = pack_f16(-wacc[nt][2 * hh], -wacc[nt][2 * hh + 1]);
-    }
-  __syncthreads();
-#pragma unroll
-  for (int it = 0; it < 2 * kTileB / 16 / kPrepThreads; ++it) {
-    const int idx = tid + it * kPrepThreads;
-    *reinterpret_cast<uint4*>(out + kRecW + idx * 16) = *reinterpret_cast<const uint4*>(s_k + idx * 16);
-  }
   float* go = gate + ((size_t)x * H + h) * kGateFloats;
   if (tid == 0 && !(s_g[kC - 1] >= -9.f && s_g[kC - 1] <= 0.f)) atomicAdd(&g_envelope_count_enc, 1u);  // also NaN
   if (tid < kC) go[tid] = expf(s_g[kC - 1] - s_g[tid]);
   else if (tid < kGateFloats) go[tid] = (tid == kC) ? expf(s_g[kC - 1]) : 0.f;
-  __syncthreads();  // s_k (staged -W), s_a, s_g are free for the next chunk
+  __syncthreads();  // s_k, s_a, s_g are free for the next chunk
   }
 }
