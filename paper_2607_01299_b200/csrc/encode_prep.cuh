@@ -100,14 +100,16 @@ __device__ __forceinline__ void block_zero(float (&acc)[2][4]) {
 // sat on the first global loads (profiles/r01b), which 5 CTAs per SM cannot hide.
 constexpr int kPrepChunksPerCta = 4;
 
-__global__ void __launch_bounds__(kPrepThreads, 4)
+template <bool kCh>
+__global__ void __launch_bounds__(kPrepThreads, kCh ? 3 : 4)
     prep_kernel(const __nv_bfloat16* __restrict__ k, const float* __restrict__ g, const float* __restrict__ beta,
                 const int2* __restrict__ chunk_meta, int cap, int H,
                 uint8_t* __restrict__ rec, float* __restrict__ gate) {
   __shared__ __align__(16) uint8_t s_k[kC * kKsPitch * 2];  // K chunk (fp16)
-  __shared__ __align__(16) float s_a[kC * kLPitch];         // L, inverted in place to A
+  __shared__ __align__(16) float s_a[kC * kLPitch];         // L, inverted in place to A (per-channel gate: first K (/) Gamma)
+  uint8_t* s_k2 = reinterpret_cast<uint8_t*>(s_a);           // fp16 [64][kKsPitch]: exactly the size of s_a
   __shared__ __align__(16) float s_m[32 * kMPitch];         // temporaries of the block merges
-  __shared__ __align__(16) float s_g[kC], s_b[kC], s_bg[kC];
+  __shared__ __align__(16) float s_g[kCh ? kD : kC], s_b[kC], s_bg[kC];  // s_g: G_r per token (scalar) or G_C per channel
   __shared__ float s_wsum;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int gq = lane >> 2, tq = lane & 3;
@@ -126,7 +128,7 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
     }
     greg = 0.f, breg = 0.f;
     if (tid < m.y) {
-      greg = g[(size_t)(m.x + tid) * H + h];
+      if (!kCh) greg = g[(size_t)(m.x + tid) * H + h];
       breg = beta[(size_t)(m.x + tid) * H + h];
     }
   };
@@ -156,23 +158,63 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
   {  // a1: inclusive cumulative log-decay by a two-warp shuffle scan (warps 0 and 1 hold the 64 tokens)
     float gv = greg, bv = breg;
     if (ci + 1 < kPrepChunksPerCta && metas[ci + 1].y > 0) prefetch(metas[ci + 1]);  // in flight during this chunk
-    if (warp < 2) {
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const float up = __shfl_up_sync(0xffffffffu, gv, o);
-        if (lane >= o) gv += up;
+    if (kCh) {
+      // per-channel gate: thread = channel c; G_j[c] = cumulative log-decay down the chunk's tokens; the K chunk is
+      // rewritten as K (.) Gamma (s_k) and K (/) Gamma (s_k2), both fp16 (Gamma in [e^-9, 1] inside the envelope)
+      if (tid < kC) s_b[tid] = bv;
+      __syncthreads();  // the K chunk is in s_k
+      const int t0c = metas[ci].x;
+      __half* k2 = reinterpret_cast<__half*>(s_k2);
+      float run = 0.f;
+#pragma unroll 4
+      for (int j = 0; j < kC; ++j) {
+        if (j < valid) run += g[((size_t)(t0c + j) * H + h) * kD + tid];
+        const float kv = __half2float(ks[j * kKsPitch + tid]);
+        const float e = __expf(run);
+        ks[j * kKsPitch + tid] = __float2half_rn(kv * e);
+        k2[j * kKsPitch + tid] = __float2half_rn(__fdividef(kv, e));
       }
-      if (tid == 31) s_wsum = gv;
-    }
-    __syncthreads();
-    if (warp < 2) {
-      if (warp == 1) gv += s_wsum;
-      s_g[tid] = gv;
-      s_b[tid] = bv;
-      s_bg[tid] = bv * expf(gv);
+      s_g[tid] = run;
+    } else {
+      if (warp < 2) {
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const float up = __shfl_up_sync(0xffffffffu, gv, o);
+          if (lane >= o) gv += up;
+        }
+        if (tid == 31) s_wsum = gv;
+      }
+      __syncthreads();
+      if (warp < 2) {
+        if (warp == 1) gv += s_wsum;
+        s_g[tid] = gv;
+        s_b[tid] = bv;
+        s_bg[tid] = bv * expf(gv);
+      }
     }
   }
   __syncthreads();
+  const uint32_t k2_base = smem_u32(kCh ? s_k2 : s_k);  // second Gram operand
+  uint8_t* out = rec + ((size_t)x * H + h) * (kCh ? kRecBytesCh : kRecBytes);
+  if (kCh) {
+    // K~_j = k_j (.) (Gamma_C (/) Gamma_j) = (K (/) Gamma)_j (.) Gamma_C, fp16, laid out like a K tile ([token][dk], two
+    // 64-wide boxes, 128B swizzle): the B operand of (4)
+    const __half* k2 = reinterpret_cast<const __half*>(s_k2);
+#pragma unroll
+    for (int it = 0; it < kC * (kD / 8) / kPrepThreads; ++it) {
+      const int idx = tid + it * kPrepThreads;
+      const int j = idx / (kD / 8), c8 = idx % (kD / 8);
+      uint32_t w[4];
+#pragma unroll
+      for (int p = 0; p < 4; ++p) {
+        const int c = 8 * c8 + 2 * p;
+        w[p] = pack_f16(__half2float(k2[j * kKsPitch + c]) * __expf(s_g[c]),
+                        __half2float(k2[j * kKsPitch + c + 1]) * __expf(s_g[c + 1]));
+      }
+      const uint32_t off = (c8 >> 3) * 8192 + (j >> 3) * 1024 + (j & 7) * 128 + (((c8 & 7) ^ (j & 7)) * 16);
+      *reinterpret_cast<uint4*>(out + kRecKt + off) = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+  }
 
   // ---- a2: Gram K K^t (lower block triangle): warp w owns rows [16w, 16w+16), n-tile pairs p <= w
   {
@@ -191,23 +233,24 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
         if (p > warp) continue;
         uint32_t b[4];
         const int nrow = 16 * p + (lane & 7) + 8 * (lane >> 4);
-        ldmatrix_x4(b, ks_base + (uint32_t)(nrow * kKsPitch + 16 * kk + 8 * ((lane >> 3) & 1)) * 2u);
+        ldmatrix_x4(b, k2_base + (uint32_t)(nrow * kKsPitch + 16 * kk + 8 * ((lane >> 3) & 1)) * 2u);
         mma_f16_16816(acc[2 * p], a[0], a[1], a[2], a[3], b[0], b[1]);
         mma_f16_16816(acc[2 * p + 1], a[0], a[1], a[2], a[3], b[2], b[3]);
       }
     }
+    if (kCh) __syncthreads();  // every warp is done with K (/) Gamma: L takes over its buffer
     // L_rj = beta_r exp(G_r - G_j) (k_r.k_j) for j < r, else 0 (the upper blocks are zero-filled: the A_b tile reads them)
 #pragma unroll
     for (int hh = 0; hh < 2; ++hh) {
       const int r = 16 * warp + gq + 8 * hh;
-      const float br = s_b[r], gr = s_g[r];
+      const float br = s_b[r], gr = kCh ? 0.f : s_g[r];
 #pragma unroll
       for (int nt = 0; nt < 8; ++nt) {
         const int j = 8 * nt + 2 * tq;
         float v0 = 0.f, v1 = 0.f;
         if (nt <= 2 * warp + 1) {
-          if (j < r) v0 = br * __expf(gr - s_g[j]) * acc[nt][2 * hh];
-          if (j + 1 < r) v1 = br * __expf(gr - s_g[j + 1]) * acc[nt][2 * hh + 1];
+          if (j < r) v0 = br * (kCh ? 1.f : __expf(gr - s_g[j])) * acc[nt][2 * hh];
+          if (j + 1 < r) v1 = br * (kCh ? 1.f : __expf(gr - s_g[j + 1])) * acc[nt][2 * hh + 1];
         }
         *reinterpret_cast<float2*>(s_a + r * kLPitch + j) = make_float2(v0, v1);
       }
@@ -276,7 +319,6 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
   // ---- -W = -(A diag(beta gamma)) K with mma.sync: warp w rows [16w, 16w+16), k-steps kk <= w (A is lower
   // triangular), in two halves of 64 columns; the fp16 fragments go straight to the record in its K-major
   // 128B-swizzled two-box layout (4-byte stores; each 16-byte chunk is completed by the four lanes of a quad)
-  uint8_t* out = rec + ((size_t)x * H + h) * kRecBytes;
 #pragma unroll 1
   for (int nh = 0; nh < 2; ++nh) {
     float wacc[8][4];
@@ -290,7 +332,8 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
       uint32_t a[4];
       {
         const int r0 = 16 * warp + gq, c0 = 16 * kk + 2 * tq;
-        const float g0 = s_bg[c0], g1 = s_bg[c0 + 1], g8 = s_bg[c0 + 8], g9 = s_bg[c0 + 9];
+        const float* sc = kCh ? s_b : s_bg;  // per-channel gate: Gamma already sits in the K (.) Gamma operand
+        const float g0 = sc[c0], g1 = sc[c0 + 1], g8 = sc[c0 + 8], g9 = sc[c0 + 9];
         const float2 p0 = *reinterpret_cast<const float2*>(s_a + r0 * kLPitch + c0);
         const float2 p1 = *reinterpret_cast<const float2*>(s_a + (r0 + 8) * kLPitch + c0);
         const float2 p2 = *reinterpret_cast<const float2*>(s_a + r0 * kLPitch + c0 + 8);
@@ -334,10 +377,18 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
         make_uint4(pack_f16(v0.x * b0.x, v0.y * b0.y), pack_f16(v0.z * b0.z, v0.w * b0.w),
                    pack_f16(v1.x * b1.x, v1.y * b1.y), pack_f16(v1.z * b1.z, v1.w * b1.w));
   }
-  float* go = gate + ((size_t)x * H + h) * kGateFloats;
-  if (tid == 0 && !(s_g[kC - 1] >= -9.f && s_g[kC - 1] <= 0.f)) atomicAdd(&g_envelope_count_enc, 1u);  // also NaN
-  if (tid < kC) go[tid] = expf(s_g[kC - 1] - s_g[tid]);
-  else if (tid < kGateFloats) go[tid] = (tid == kC) ? expf(s_g[kC - 1]) : 0.f;
+  if (kCh) {
+    float* go = gate + ((size_t)x * H + h) * kGateFloatsCh;
+    const float gc = s_g[tid];
+    go[tid] = expf(gc);
+    if (tid < kGateFloatsCh - kD) go[kD + tid] = 0.f;
+    if (!(gc >= -9.f && gc <= 0.f)) atomicAdd(&g_envelope_count_enc, 1u);  // also NaN
+  } else {
+    float* go = gate + ((size_t)x * H + h) * kGateFloats;
+    if (tid == 0 && !(s_g[kC - 1] >= -9.f && s_g[kC - 1] <= 0.f)) atomicAdd(&g_envelope_count_enc, 1u);  // also NaN
+    if (tid < kC) go[tid] = expf(s_g[kC - 1] - s_g[tid]);
+    else if (tid < kGateFloats) go[tid] = (tid == kC) ? expf(s_g[kC - 1]) : 0.f;
+  }
   __syncthreads();  // s_k, s_a, s_g are free for the next chunk
   }
 }

@@ -134,7 +134,7 @@ __device__ __forceinline__ void s2_issue4(uint32_t tmem, uint32_t sb, int b) {  
     mma_f16_ts(tmem + 128 * b, tmem + 256 + 64 * b + 8 * ks, make_desc(sb + kS2StK + ks * 2048, 8192, 1024, 2), id4, 1u);
 }
 
-template <bool kIsT>
+template <bool kIsT, bool kCh>
 __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile int* abort_flag, uint32_t tmem, int cw,
                                          int lane, int nc, float* __restrict__ dst_block) {
   constexpr int b = kIsT ? 1 : 0;
@@ -172,7 +172,7 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     if (c > 0) s2_wait_warp(&bars->m4_done[b], (c - 1) & 1, abort_flag, lane);
     tc_fence_after();
     S2_STAMP(b, c, 0);
-    const float gC = gt[kC];
+    const float gC = kCh ? 1.f : gt[kC];  // scalar gate: gamma_C; per-channel gate: Gamma_C[col] = gt[col], applied below
     // ---- pass: Xh = fp16(X) (A operand of (3)), X <- gamma_C X; T rows are re-normalised on the way
     {
       uint32_t x0[32], x1[32];
@@ -220,10 +220,22 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
         for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x1[2 * j]), __uint_as_float(x1[2 * j + 1]));
         tmem_st16(tH + 16, hh);
       }
+      if (kCh) {
+        const float4* gv = reinterpret_cast<const float4*>(gt + 64 * hf);
 #pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        mul2(x0[2 * j], x0[2 * j + 1], f);
-        mul2(x1[2 * j], x1[2 * j + 1], f);
+        for (int j4 = 0; j4 < 8; ++j4) {
+          const float4 a = gv[j4], b4 = gv[8 + j4];
+          mul2v(x0[4 * j4], x0[4 * j4 + 1], f * a.x, f * a.y);
+          mul2v(x0[4 * j4 + 2], x0[4 * j4 + 3], f * a.z, f * a.w);
+          mul2v(x1[4 * j4], x1[4 * j4 + 1], f * b4.x, f * b4.y);
+          mul2v(x1[4 * j4 + 2], x1[4 * j4 + 3], f * b4.z, f * b4.w);
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+          mul2(x0[2 * j], x0[2 * j + 1], f);
+          mul2(x1[2 * j], x1[2 * j + 1], f);
+        }
       }
       tmem_st32(tX, x0);
       tmem_st32(tX + 32, x1);
@@ -252,13 +264,16 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
       S2_STAMP(b, c, 7);
 #pragma unroll
       for (int j8 = 0; j8 < 4; ++j8) {
-        const float4 d0 = *reinterpret_cast<const float4*>(gt + 32 * hf + 8 * j8);
-        const float4 d1 = *reinterpret_cast<const float4*>(gt + 32 * hf + 8 * j8 + 4);
+        float4 d0 = make_float4(1.f, 1.f, 1.f, 1.f), d1 = d0;  // per-channel gate: the decay ratios sit in the K~ tile
+        if (!kCh) {
+          d0 = *reinterpret_cast<const float4*>(gt + 32 * hf + 8 * j8);
+          d1 = *reinterpret_cast<const float4*>(gt + 32 * hf + 8 * j8 + 4);
+        }
         const float dd[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
           uint32_t u0 = y[8 * j8 + 2 * p], u1 = y[8 * j8 + 2 * p + 1];
-          mul2v(u0, u1, dd[2 * p], dd[2 * p + 1]);
+          if (!kCh) mul2v(u0, u1, dd[2 * p], dd[2 * p + 1]);
           y[4 * j8 + p] = pack_f16(__uint_as_float(u0), __uint_as_float(u1));  // packed in place: slot 4 j8 + p < 8 j8 + 2 p
         }
       }
@@ -311,6 +326,7 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
   }
 }
 
+template <bool kCh>
 __global__ void __launch_bounds__(kS2Threads, 1)
     scan2_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
                  const int32_t* __restrict__ cu_seqlens, const int32_t* __restrict__ chunk_off, int H,
@@ -349,7 +365,7 @@ __global__ void __launch_bounds__(kS2Threads, 1)
   if (warp == 18) {
     // ------------------------------------------------------------------------------------------- loader
     if (lane == 0) {
-      constexpr uint32_t bytes = 32768u + (uint32_t)kRecBytes + (uint32_t)kGateBytes;
+      constexpr uint32_t bytes = 32768u + (uint32_t)kRecBytes + (uint32_t)(kCh ? kGateBytesCh : kGateBytes);
 #pragma unroll 1
       for (int c = 0; c < nc; ++c) {
         const int st = c % kS2Stages;
@@ -358,13 +374,19 @@ __global__ void __launch_bounds__(kS2Threads, 1)
         const uint32_t sb = smem_base + st * kS2StageBytes;
         const int t0 = seg_begin + c * kC;
         mbar_expect_tx(&bars->st_full[st], bytes);
-        tma_load_3d(sb + kS2StK, &tmK, 0, h, t0, &bars->st_full[st]);
-        tma_load_3d(sb + kS2StK + 8192, &tmK, 64, h, t0, &bars->st_full[st]);
+        const size_t r = (size_t)(chunk0 + c) * H + h;
+        if (kCh) {  // the K~ tile of the prep record (fp16, same layout as a K tile) takes the K slot
+          bulk_g2s(smem + st * kS2StageBytes + kS2StK, rec + r * kRecBytesCh + kRecKt, 2 * kTileB, &bars->st_full[st]);
+        } else {
+          tma_load_3d(sb + kS2StK, &tmK, 0, h, t0, &bars->st_full[st]);
+          tma_load_3d(sb + kS2StK + 8192, &tmK, 64, h, t0, &bars->st_full[st]);
+        }
         tma_load_3d(sb + kS2StV, &tmV, 0, h, t0, &bars->st_full[st]);
         tma_load_3d(sb + kS2StV + 8192, &tmV, 64, h, t0, &bars->st_full[st]);
-        const size_t r = (size_t)(chunk0 + c) * H + h;
-        bulk_g2s(smem + st * kS2StageBytes + kS2StRec, rec + r * kRecBytes, kRecBytes, &bars->st_full[st]);
-        bulk_g2s(smem + st * kS2StageBytes + kS2StGate, gate + r * kGateFloats, kGateBytes, &bars->st_full[st]);
+        bulk_g2s(smem + st * kS2StageBytes + kS2StRec, rec + r * (kCh ? kRecBytesCh : kRecBytes), kRecBytes,
+                 &bars->st_full[st]);
+        bulk_g2s(smem + st * kS2StageBytes + kS2StGate, gate + r * (kCh ? kGateFloatsCh : kGateFloats),
+                 kCh ? kGateBytesCh : kGateBytes, &bars->st_full[st]);
       }
     }
   } else if (warp >= 16) {
@@ -376,7 +398,7 @@ __global__ void __launch_bounds__(kS2Threads, 1)
       s2_wait_warp(&bars->st_full[st], (c / kS2Stages) & 1, abort_flag, lane);
       S2_STAMPW(16, 3, c, 3);
       uint4* tile = reinterpret_cast<uint4*>(smem + st * kS2StageBytes + (warp == 16 ? kS2StK : kS2StV));
-#ifndef HYPIC_EXP_NOCONV
+      if (!(kCh && warp == 16)) {  // the K~ tile of the per-channel gate arrives as fp16
 #pragma unroll 4
       for (int it = 0; it < 32; ++it) {
         uint4 w = tile[it * 32 + lane];
@@ -386,16 +408,16 @@ __global__ void __launch_bounds__(kS2Threads, 1)
         w.w = pack_f16(__uint_as_float(w.w << 16), __uint_as_float(w.w & 0xffff0000u));
         tile[it * 32 + lane] = w;
       }
-#endif
+      }
       fence_proxy_async();
       __syncwarp();
       S2_STAMPW(16, 3, c, 4);
       if (lane == 0) mbar_arrive(&bars->st_conv[st]);
     }
   } else if (warp < 8) {
-    s2_chain<false>(smem, bars, abort_flag, tmem, warp, lane, nc, E + ((size_t)s * H + h) * kD * kD);
+    s2_chain<false, kCh>(smem, bars, abort_flag, tmem, warp, lane, nc, E + ((size_t)s * H + h) * kD * kD);
   } else {
-    s2_chain<true>(smem, bars, abort_flag, tmem, warp - 8, lane, nc, T + ((size_t)s * H + h) * kD * kD);
+    s2_chain<true, kCh>(smem, bars, abort_flag, tmem, warp - 8, lane, nc, T + ((size_t)s * H + h) * kD * kD);
   }
   tc_fence_before();
   __syncthreads();

@@ -32,6 +32,12 @@ constexpr int kRecAb = 2 * kTileB;      //         A_b (fp16, [token][token]) 8 
 constexpr int kRecBytes = 3 * kTileB;   // 24 KB per (chunk, head)
 constexpr int kGateFloats = 72;         // d_j[64], gamma_C, pad (288 B = 18 x 16 B)
 constexpr int kGateBytes = kGateFloats * 4;
+// per-channel gate (KDA row of Table 1): the record also carries K~_j = k_j (.) (Gamma_C (/) Gamma_j) (fp16,
+// laid out like a K tile) and the gate record is Gamma_C[128]
+constexpr int kRecKt = 3 * kTileB;
+constexpr int kRecBytesCh = 5 * kTileB;  // 40 KB per (chunk, head)
+constexpr int kGateFloatsCh = 144;       // Gamma_C[128], pad (576 B = 36 x 16 B)
+constexpr int kGateBytesCh = kGateFloatsCh * 4;
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 // workspace: chunk_off int32[n_seg + 1] | chunk_meta int2[cap] | records [cap][H][kRecBytes] | gate [cap][H][kGateFloats]
@@ -123,14 +129,15 @@ __global__ void identity_fill_kernel(float* __restrict__ E, float* __restrict__ 
 }  // namespace
 
 bool encode_tensor_shape_ok(int32_t, int32_t dk, int32_t dv, int kv_dtype, int gate) {
-  return dk == kD && dv == kD && kv_dtype == HYPIC_DT_BF16 && gate == HYPIC_GATE_SCALAR;
+  return dk == kD && dv == kD && kv_dtype == HYPIC_DT_BF16 && (gate == HYPIC_GATE_SCALAR || gate == HYPIC_GATE_CHANNEL);
 }
 
 size_t encode_tensor_workspace(int32_t n_seg, int32_t t_total, int32_t H, int32_t dk, int32_t dv, int kv_dtype,
                                int gate) {
   if (!encode_tensor_shape_ok(H, dk, dv, kv_dtype, gate)) return 0;
   const size_t cap = chunk_cap(n_seg, t_total);
-  return ws_off_rec(n_seg, cap) + cap * H * ((size_t)kRecBytes + kGateBytes);
+  const bool ch = gate == HYPIC_GATE_CHANNEL;
+  return ws_off_rec(n_seg, cap) + cap * H * ((size_t)(ch ? kRecBytesCh : kRecBytes) + (ch ? kGateBytesCh : kGateBytes));
 }
 
 int encode_tensor(const EncodeArgs& a) {
@@ -149,10 +156,12 @@ int encode_tensor(const EncodeArgs& a) {
   int32_t* chunk_off = reinterpret_cast<int32_t*>(ws);
   int2* chunk_meta = reinterpret_cast<int2*>(ws + ws_off_meta(a.n_seg));
   uint8_t* rec = ws + ws_off_rec(a.n_seg, cap);
-  float* gate = reinterpret_cast<float*>(rec + cap * a.H * (size_t)kRecBytes);
+  const bool ch = a.gate == HYPIC_GATE_CHANNEL;
+  float* gate = reinterpret_cast<float*>(rec + cap * a.H * (size_t)(ch ? kRecBytesCh : kRecBytes));
   static bool configured = false;
   if (!configured) {
-    HYPIC_CUDA_OK(cudaFuncSetAttribute(scan2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kS2Smem));
+    HYPIC_CUDA_OK(cudaFuncSetAttribute(scan2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kS2Smem));
+    HYPIC_CUDA_OK(cudaFuncSetAttribute(scan2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kS2Smem));
     configured = true;
   }
   const auto* kp = static_cast<const __nv_bfloat16*>(a.k);
@@ -162,11 +171,16 @@ int encode_tensor(const EncodeArgs& a) {
   if (rc != HYPIC_OK) return rc;
   chunk_offsets_kernel<<<1, 1024, 0, a.stream>>>(a.cu_seqlens, a.n_seg, chunk_off, chunk_meta, (int)cap);
   note_launch();
-  prep_kernel<<<dim3((unsigned)((cap + kPrepChunksPerCta - 1) / kPrepChunksPerCta), a.H), kPrepThreads, 0, a.stream>>>(
-      kp, a.g, a.beta, chunk_meta, (int)cap, a.H, rec, gate);
-  note_launch();
-  scan2_kernel<<<dim3(a.H, a.n_seg), kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, a.H, rec, gate,
-                                                                     a.E, a.T);
+  const dim3 pgrid((unsigned)((cap + kPrepChunksPerCta - 1) / kPrepChunksPerCta), a.H), sgrid(a.H, a.n_seg);
+  if (ch) {
+    prep_kernel<true><<<pgrid, kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, chunk_meta, (int)cap, a.H, rec, gate);
+    note_launch();
+    scan2_kernel<true><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, a.H, rec, gate, a.E, a.T);
+  } else {
+    prep_kernel<false><<<pgrid, kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, chunk_meta, (int)cap, a.H, rec, gate);
+    note_launch();
+    scan2_kernel<false><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, a.H, rec, gate, a.E, a.T);
+  }
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
   return HYPIC_OK;
