@@ -255,6 +255,40 @@ def time_extra_cfg1(hb, device, peaks, reps=20):
             "tc_frac_of_bf16_burst_peak": 8192 * 16 * ENC_FLOP_PER_TOKEN_HEAD / (ms * 1e-3) / 1e12 / peaks["bf16_tflops"]}
 
 
+def time_extra_cfg3(hb, device, peaks, reps=3):
+    """cfg3 (64 varlen segments ~ U[512,16384], H=32, per-channel gate): encode only; HBM-bound by its 1,028 B per
+    token-head, so the binding fraction is reported against the measured HBM peak."""
+    inp = wl.cfg3(device=device)
+    n_seg, ttot = inp.n_seg, inp.t_total
+    E = torch.empty((n_seg, H, D, D), dtype=torch.float32, device=device)
+    T = torch.empty_like(E)
+    ws = torch.empty(max(16, hb.hypic_segment_encode_workspace(n_seg, ttot, H, D, D, hb.HYPIC_DT_BF16,
+                                                               hb.HYPIC_GATE_CHANNEL)), dtype=torch.uint8, device=device)
+
+    def one():
+        hb.hypic_segment_encode(inp.k, inp.v, inp.g, inp.beta, inp.cu_seqlens, inp.gate, E=E, T=T, workspace=ws)
+
+    one()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        one()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    th = ttot * H
+    gbs = (th * (2 * D + 2 * D + 4 * D + 4) + n_seg * H * COMPOSE_BYTES_PER_STEP) / (ms * 1e-3) / 1e9
+    tfl = th * ENC_FLOP_PER_TOKEN_HEAD / (ms * 1e-3) / 1e12
+    fam = hb.hypic_encode_impl_for(H, D, D, hb.HYPIC_DT_BF16, hb.HYPIC_GATE_CHANNEL)
+    return {"workload": f"cfg3: {n_seg} varlen segments, {ttot} tokens, H=32, per-channel gate, encode only (17.8 GB of "
+                        "inputs: larger than L2)", "ms": ms, "tokens_per_s": ttot / (ms * 1e-3),
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                         "frac": gbs / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"]},
+            "tc_frac_of_bf16_burst_peak": tfl / peaks["bf16_tflops"],
+            "kernel_family": "tensor" if fam == hb.HYPIC_IMPL_TENSOR else "simt"}
+
+
 def time_extra_cfg4(hb, device, peaks, iters=48):
     """cfg4 compose stress: pool P=1024 resident (4.3 GB, reading S7), 48 layer-iterations with their own request
     lists (R=128, n_r ~ U{16..64}); compose only is timed."""
@@ -405,6 +439,8 @@ def run_ours(args):
         torch.cuda.empty_cache()
         extra["cfg1"] = time_extra_cfg1(hb, device, peaks)
         extra["cfg4_compose"] = time_extra_cfg4(hb, device, peaks)
+        torch.cuda.empty_cache()
+        extra["cfg3_encode"] = time_extra_cfg3(hb, device, peaks)
         extra["cfg2_compose"] = {"avg_launch_ms": cmp_avg, "compose_ops_per_s": N_SEG * H / (cmp_avg * 1e-3),
                                  "hbm_gbs": N_SEG * H * COMPOSE_BYTES_PER_STEP / (cmp_avg * 1e-3) / 1e9}
 
