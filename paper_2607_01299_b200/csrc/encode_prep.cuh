@@ -166,13 +166,20 @@ __global__ void __launch_bounds__(kPrepThreads, kCh ? 3 : 4)
       const int t0c = metas[ci].x;
       __half* k2 = reinterpret_cast<__half*>(s_k2);
       float run = 0.f;
-#pragma unroll 4
-      for (int j = 0; j < kC; ++j) {
-        if (j < valid) run += g[((size_t)(t0c + j) * H + h) * kD + tid];
-        const float kv = __half2float(ks[j * kKsPitch + tid]);
-        const float e = __expf(run);
-        ks[j * kKsPitch + tid] = __float2half_rn(kv * e);
-        k2[j * kKsPitch + tid] = __float2half_rn(__fdividef(kv, e));
+#pragma unroll 1
+      for (int jb = 0; jb < kC; jb += 16) {
+        float gl[16];  // 16 independent loads in flight per thread
+#pragma unroll
+        for (int i = 0; i < 16; ++i) gl[i] = (jb + i < valid) ? g[((size_t)(t0c + jb + i) * H + h) * kD + tid] : 0.f;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          const int j = jb + i;
+          run += gl[i];
+          const float kv = __half2float(ks[j * kKsPitch + tid]);
+          const float e = __expf(run);
+          ks[j * kKsPitch + tid] = __float2half_rn(kv * e);
+          k2[j * kKsPitch + tid] = __float2half_rn(__fdividef(kv, e));
+        }
       }
       s_g[tid] = run;
     } else {
