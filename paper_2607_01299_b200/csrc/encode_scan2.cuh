@@ -329,15 +329,15 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
 template <bool kCh>
 __global__ void __launch_bounds__(kS2Threads, 1)
     scan2_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
-                 const int32_t* __restrict__ cu_seqlens, const int32_t* __restrict__ chunk_off, int H,
-                 const uint8_t* __restrict__ rec, const float* __restrict__ gate, float* __restrict__ E,
+                 const int32_t* __restrict__ cu_seqlens, const int32_t* __restrict__ chunk_off,
+                 const int32_t* __restrict__ seg_order, int H, const uint8_t* __restrict__ rec, const float* __restrict__ gate, float* __restrict__ E,
                  float* __restrict__ T) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   S2Bars* bars = reinterpret_cast<S2Bars*>(smem + kS2OffBar);
   volatile int* abort_flag = &bars->abort_flag;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int h = blockIdx.x, s = blockIdx.y;
+  const int h = blockIdx.x, s = seg_order[blockIdx.y];  // longest segments first
   const int seg_begin = cu_seqlens[s], seg_end = cu_seqlens[s + 1];
   const int nc = (seg_end - seg_begin + kC - 1) / kC;
   const int chunk0 = chunk_off[s];

@@ -40,16 +40,18 @@ constexpr int kGateFloatsCh = 144;       // Gamma_C[128], pad (576 B = 36 x 16 B
 constexpr int kGateBytesCh = kGateFloatsCh * 4;
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
-// workspace: chunk_off int32[n_seg + 1] | chunk_meta int2[cap] | records [cap][H][kRecBytes] | gate [cap][H][kGateFloats]
+// workspace: chunk_off int32[n_seg + 1], seg_order int32[n_seg] | chunk_meta int2[cap] | records [cap][H][kRecBytes] | gate [cap][H][kGateFloats]
 __host__ __device__ inline size_t chunk_cap(int32_t n_seg, int32_t t_total) { return (size_t)t_total / kC + n_seg; }
-__host__ __device__ inline size_t ws_off_meta(int32_t n_seg) { return align_up(4 * ((size_t)n_seg + 1), 1024); }
+__host__ __device__ inline size_t ws_off_meta(int32_t n_seg) { return align_up(8 * ((size_t)n_seg + 1), 1024); }
 __host__ __device__ inline size_t ws_off_rec(int32_t n_seg, size_t cap) { return ws_off_meta(n_seg) + align_up(8 * cap, 1024); }
 
 // ------------------------------------------------------------------------------------------------ K0
 // chunk_meta[x] = (first token, number of valid tokens) of global chunk x, (0, 0) for the unused tail of the table:
 // the prep CTAs read one entry instead of searching chunk_off (a chain of dependent global loads).
+// seg_order = the segments by decreasing length (the paper's LPT rule, used here as the launch order of
+// the scan CTAs so that the longest sequential scans start first); identity beyond 8192 segments.
 __global__ void chunk_offsets_kernel(const int32_t* __restrict__ cu_seqlens, int n_seg, int32_t* __restrict__ chunk_off,
-                                     int2* __restrict__ chunk_meta, int cap) {
+                                     int32_t* __restrict__ seg_order, int2* __restrict__ chunk_meta, int cap) {
   __shared__ int part[1024];
   const int tid = threadIdx.x;
   const int per = (n_seg + 1023) / 1024;
@@ -80,6 +82,18 @@ __global__ void chunk_offsets_kernel(const int32_t* __restrict__ cu_seqlens, int
   if (tid == 1023) total = run;  // the last thread ends at the grand total
   __syncthreads();
   for (int x = total + tid; x < cap; x += 1024) chunk_meta[x] = make_int2(0, 0);
+  for (int sg = tid; sg < n_seg; sg += 1024) {
+    int rank = sg;
+    if (n_seg <= 8192) {
+      const int len = cu_seqlens[sg + 1] - cu_seqlens[sg];
+      rank = 0;
+      for (int t = 0; t < n_seg; ++t) {
+        const int lt = cu_seqlens[t + 1] - cu_seqlens[t];
+        rank += (lt > len || (lt == len && t < sg)) ? 1 : 0;
+      }
+    }
+    seg_order[rank] = sg;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ K1, K2
@@ -154,6 +168,7 @@ int encode_tensor(const EncodeArgs& a) {
   }
   uint8_t* ws = static_cast<uint8_t*>(a.workspace);
   int32_t* chunk_off = reinterpret_cast<int32_t*>(ws);
+  int32_t* seg_order = chunk_off + a.n_seg + 1;
   int2* chunk_meta = reinterpret_cast<int2*>(ws + ws_off_meta(a.n_seg));
   uint8_t* rec = ws + ws_off_rec(a.n_seg, cap);
   const bool ch = a.gate == HYPIC_GATE_CHANNEL;
@@ -169,17 +184,17 @@ int encode_tensor(const EncodeArgs& a) {
   int rc = make_kv_tensor_map(&tmK, a.k, a.t_total, a.H);
   if (rc == HYPIC_OK) rc = make_kv_tensor_map(&tmV, a.v, a.t_total, a.H);
   if (rc != HYPIC_OK) return rc;
-  chunk_offsets_kernel<<<1, 1024, 0, a.stream>>>(a.cu_seqlens, a.n_seg, chunk_off, chunk_meta, (int)cap);
+  chunk_offsets_kernel<<<1, 1024, 0, a.stream>>>(a.cu_seqlens, a.n_seg, chunk_off, seg_order, chunk_meta, (int)cap);
   note_launch();
   const dim3 pgrid((unsigned)((cap + kPrepChunksPerCta - 1) / kPrepChunksPerCta), a.H), sgrid(a.H, a.n_seg);
   if (ch) {
     prep_kernel<true><<<pgrid, kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, chunk_meta, (int)cap, a.H, rec, gate);
     note_launch();
-    scan2_kernel<true><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, a.H, rec, gate, a.E, a.T);
+    scan2_kernel<true><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, seg_order, a.H, rec, gate, a.E, a.T);
   } else {
     prep_kernel<false><<<pgrid, kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, chunk_meta, (int)cap, a.H, rec, gate);
     note_launch();
-    scan2_kernel<false><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, a.H, rec, gate, a.E, a.T);
+    scan2_kernel<false><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, seg_order, a.H, rec, gate, a.E, a.T);
   }
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
