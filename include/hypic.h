@@ -48,7 +48,7 @@ typedef enum { HYPIC_GATE_SCALAR = 0, HYPIC_GATE_CHANNEL = 1 } hypic_gate_t; /* 
 typedef enum {
   HYPIC_IMPL_AUTO = 0,
   HYPIC_IMPL_SIMT = 1,   /* fp32 CUDA-core kernels: token-by-token scan / FFMA compose; any dk in {64,128} */
-  HYPIC_IMPL_TENSOR = 2  /* tcgen05/TMEM kernels (dk = dv = 128) */
+  HYPIC_IMPL_TENSOR = 2  /* tcgen05/TMEM kernels (dk = dv = 128; encode: bf16 k/v) */
 } hypic_impl_t;
 
 /*
@@ -83,7 +83,7 @@ size_t hypic_segment_encode_workspace(int32_t n_seg, int32_t t_total, int32_t H,
  *
  * A zero-length segment yields E = 0, T = I.  n_seg = 0 or t_total = 0 with n_seg > 0 are valid.
  * Built envelope: dk in {64, 128}; dv in [1, 1024] for the SIMT family, dv = dk = 128 for the tensor family
- * (bf16 k/v, scalar gate; its tensor-core operands are fp16, so it additionally assumes finite |k|, |v| <= 65504 and
+ * (bf16 k/v, scalar or per-channel gate; its tensor-core operands are fp16, so it additionally assumes finite |k|, |v| <= 65504 and
  * beta |k|^2 within the stable range of the recurrence and a per-chunk log-decay >= -9, see
  * hypic_envelope_violation_count -- callers outside that range select HYPIC_IMPL_SIMT);
  * H, n_seg, lengths arbitrary.  Inputs are only read; E and T are fully overwritten.
@@ -106,7 +106,9 @@ int hypic_segment_encode(const void* k, const void* v, const float* g, const flo
  *   total_steps  HOST value of cu_segs[R] (>= 0); used only to size the launch / skip empty work
  *   S_out    out [R, H, dv, dk] fp32; may alias S_in exactly (same pointer), no partial overlap
  *
- * Built envelope: dk in {64, 128}, dv in [1, 1024] (SIMT family); dv = dk = 128 (tensor family).
+ * Built envelope: dk in {64, 128}, dv in [1, 1024] (SIMT family); dv = dk = 128 (tensor family, which multiplies
+ * two-term fp16 splits and assumes finite pools with |T entries| < 4 -- a transition of a stable recurrence has
+ * spectral norm <= 1 -- and |S|, |E| below 1e30; other pools: HYPIC_IMPL_SIMT).
  */
 int hypic_compose(const float* S_in, const float* E_pool, const float* T_pool, const int32_t* seg_ids,
                   const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
