@@ -19,7 +19,8 @@
 //   warps 0-7     E chain     thread = (row of E, 64-column half): pass  Xh = fp16(X), X <- gamma_C X;
 //                             epilogue  U'' = fp16(DY d_j)
 //   warps 8-15    T chain     same for T plus the row re-normalisation
-//   warps 16-17   converters  K (warp 16) and V (warp 17) tile bf16 -> fp16 in place; warp 16 also owns TMEM alloc
+//   warps 16-17   converters  K (warp 16) and V (warp 17) tile bf16 -> fp16 in place; warp 16 also owns TMEM alloc;
+//                             warp 17 issues (1) for the tile it has just converted
 //   warp 18       loader      TMA tensor boxes for the K / V chunk tiles, bulk copies for the prep record (-W, A_b)
 //                             and the gate record; three stages
 // There is no separate MMA-issuer role: after a chain-wide named barrier, one elected thread of the chain issues the
@@ -60,6 +61,7 @@ constexpr int kS2Smem = kS2OffBar + 256 + 1024;
 struct S2Bars {
   uint64_t st_full[kS2Stages], st_conv[kS2Stages], st_free[kS2Stages];
   uint64_t m3_done[2], m4_done[2];  // [block]: 0 = E, 1 = T
+  uint64_t dy_free, issued1;        // E chain <-> V converter, which issues (1): DY_E may be overwritten / (1)_c is in the pipe
   uint32_t tmem_base;
   int abort_flag;
 };
@@ -158,17 +160,12 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
   tmem_st_wait();
   const uint32_t smem_base = smem_u32(smem);
   const bool issuer = (cw == 0 && lane == 0);  // this chain's MMA-issuing thread
-  if (!kIsT && issuer && nc > 0) {
-    s2_wait(&bars->st_conv[0], 0, abort_flag);
-    tc_fence_after();
-    s2_issue1(tmem, smem_base);
-  }
 
 #pragma unroll 1
   for (int c = 0; c < nc; ++c) {
     const int st = c % kS2Stages;
     const float* gt = reinterpret_cast<const float*>(smem + st * kS2StageBytes + kS2StGate);
-    s2_wait_warp(&bars->st_full[st], (c / kS2Stages) & 1, abort_flag, lane);
+    s2_wait_warp(&bars->st_conv[st], (c / kS2Stages) & 1, abort_flag, lane);  // converted, hence also landed
     if (c > 0) s2_wait_warp(&bars->m4_done[b], (c - 1) & 1, abort_flag, lane);
     tc_fence_after();
     S2_STAMP(b, c, 0);
@@ -246,7 +243,7 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     named_bar_sync(5 + b, 256);  // the whole chain has written Xh / X
     S2_STAMP(b, c, 1);
     if (issuer) {
-      if (kIsT) s2_wait(&bars->st_conv[st], (c / kS2Stages) & 1, abort_flag);  // (E saw it before its (1)_c)
+      if (!kIsT) s2_wait(&bars->issued1, c & 1, abort_flag);  // (1)_c is ahead of (3)_c in the tensor pipe
       tc_fence_after();
       s2_issue3(tmem, smem_base + st * kS2StageBytes, b);
       mma_commit(&bars->m3_done[b]);
@@ -284,15 +281,11 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     named_bar_sync(5 + b, 256);  // the whole chain has written U''
     S2_STAMP(b, c, 3);
     if (issuer) {
+      if (!kIsT) mbar_arrive(&bars->dy_free);  // DY_E has been read: the V converter may issue (1) of the next chunk
       tc_fence_after();
       s2_issue4(tmem, smem_base + st * kS2StageBytes, b);
       mma_commit(&bars->m4_done[b]);
       mma_commit(&bars->st_free[st]);  // count 2: released when both chains' (4) of this chunk have completed
-      if (!kIsT && c + 1 < nc) {
-        s2_wait(&bars->st_conv[(c + 1) % kS2Stages], ((c + 1) / kS2Stages) & 1, abort_flag);
-        tc_fence_after();
-        s2_issue1(tmem, smem_base + ((c + 1) % kS2Stages) * kS2StageBytes);
-      }
     }
     __syncwarp();
   }
@@ -347,6 +340,7 @@ __global__ void __launch_bounds__(kS2Threads, 1)
     for (int i = 0; i < kS2Stages; ++i) {
       mbar_init(&bars->st_full[i], 1);
       mbar_init(&bars->st_conv[i], 2);
+      if (i == 0) { mbar_init(&bars->dy_free, 1); mbar_init(&bars->issued1, 1); }
       mbar_init(&bars->st_free[i], 2);
     }
     for (int i = 0; i < 2; ++i) {
@@ -413,6 +407,16 @@ __global__ void __launch_bounds__(kS2Threads, 1)
       __syncwarp();
       S2_STAMPW(16, 3, c, 4);
       if (lane == 0) mbar_arrive(&bars->st_conv[st]);
+      if (warp == 17 && lane == 0) {
+        // (1)_c = V^t A_b^t is issued here, off the E chain's critical path: its V operand was just converted by this
+        // warp, A_b landed with the stage, and DY_E is free once the E chain has read it for chunk c - 1.
+        if (c > 0) s2_wait(&bars->dy_free, (c - 1) & 1, abort_flag);
+        tc_fence_after();
+        s2_issue1(tmem, smem_base + st * kS2StageBytes);
+        tc_fence_before();
+        mbar_arrive(&bars->issued1);
+      }
+      __syncwarp();
     }
   } else if (warp < 8) {
     s2_chain<false, kCh>(smem, bars, abort_flag, tmem, warp, lane, nc, E + ((size_t)s * H + h) * kD * kD);
