@@ -59,9 +59,13 @@ constexpr int kS2OffBar = kS2OffXch + 1024;
 constexpr int kS2Smem = kS2OffBar + 256 + 1024;
 
 struct S2Bars {
-  uint64_t st_full[kS2Stages], st_conv[kS2Stages], st_free[kS2Stages];
+  uint64_t st_full[kS2Stages], st_free[kS2Stages];
   uint64_t m3_done[2], m4_done[2];  // [block]: 0 = E, 1 = T
-  uint64_t dy_free, issued1;        // E chain <-> V converter, which issues (1): DY_E may be overwritten / (1)_c is in the pipe
+  uint64_t dy_free;                 // E chain -> V converter (which issues (1)): DY_E may be overwritten
+  // Progress counters read with plain acquire loads: an mbarrier probe costs ~380 cycles in this kernel even when the
+  // phase completed long ago, and these two sit on the chains' critical path once per chunk.
+  int conv_cnt[2];                  // chunks converted by warp 16 (K) / 17 (V); both > c: stage c landed and converted
+  int issued1_cnt;                  // chunks whose (1) is in the tensor pipe
   uint32_t tmem_base;
   int abort_flag;
 };
@@ -91,6 +95,27 @@ __device__ __noinline__ bool s2_wait(uint64_t* bar, uint32_t parity, volatile in
 
 __device__ __forceinline__ void s2_wait_warp(uint64_t* bar, uint32_t parity, volatile int* abort_flag, int) {
   s2_wait(bar, parity, abort_flag);
+}
+
+__device__ __forceinline__ void flag_release(int* p, int v) {
+  asm volatile("st.release.cta.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ int flag_acquire(const int* p) {
+  int v;
+  asm volatile("ld.acquire.cta.shared::cta.b32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+  return v;
+}
+// bounded spin until *p > c
+__device__ __forceinline__ void s2_wait_count(const int* p, int c, volatile int* abort_flag) {
+#pragma unroll 1
+  for (uint32_t i = 0; i < 40000000u; ++i) {
+    if (flag_acquire(p) > c) return;
+    if ((i & 4095u) == 4095u && *abort_flag) return;
+  }
+  if (!*abort_flag) {
+    *abort_flag = 1;
+    atomicAdd(&g_timeout_count_enc, 1u);
+  }
 }
 
 // 32 lanes x 16 columns
@@ -165,7 +190,8 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
   for (int c = 0; c < nc; ++c) {
     const int st = c % kS2Stages;
     const float* gt = reinterpret_cast<const float*>(smem + st * kS2StageBytes + kS2StGate);
-    s2_wait_warp(&bars->st_conv[st], (c / kS2Stages) & 1, abort_flag, lane);  // converted, hence also landed
+    s2_wait_count(&bars->conv_cnt[0], c, abort_flag);  // converted, hence also landed
+    s2_wait_count(&bars->conv_cnt[1], c, abort_flag);
     if (c > 0) s2_wait_warp(&bars->m4_done[b], (c - 1) & 1, abort_flag, lane);
     tc_fence_after();
     S2_STAMP(b, c, 0);
@@ -243,7 +269,7 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     named_bar_sync(5 + b, 256);  // the whole chain has written Xh / X
     S2_STAMP(b, c, 1);
     if (issuer) {
-      if (!kIsT) s2_wait(&bars->issued1, c & 1, abort_flag);  // (1)_c is ahead of (3)_c in the tensor pipe
+      if (!kIsT) s2_wait_count(&bars->issued1_cnt, c, abort_flag);  // (1)_c is ahead of (3)_c in the tensor pipe
       tc_fence_after();
       s2_issue3(tmem, smem_base + st * kS2StageBytes, b);
       mma_commit(&bars->m3_done[b]);
@@ -339,8 +365,7 @@ __global__ void __launch_bounds__(kS2Threads, 1)
   if (tid == 0) {
     for (int i = 0; i < kS2Stages; ++i) {
       mbar_init(&bars->st_full[i], 1);
-      mbar_init(&bars->st_conv[i], 2);
-      if (i == 0) { mbar_init(&bars->dy_free, 1); mbar_init(&bars->issued1, 1); }
+      if (i == 0) mbar_init(&bars->dy_free, 1);
       mbar_init(&bars->st_free[i], 2);
     }
     for (int i = 0; i < 2; ++i) {
@@ -348,6 +373,7 @@ __global__ void __launch_bounds__(kS2Threads, 1)
       mbar_init(&bars->m4_done[i], 1);
     }
     bars->abort_flag = 0;
+    bars->conv_cnt[0] = bars->conv_cnt[1] = bars->issued1_cnt = 0;
     fence_barrier_init();
   }
   tc_fence_before();
@@ -406,7 +432,7 @@ __global__ void __launch_bounds__(kS2Threads, 1)
       fence_proxy_async();
       __syncwarp();
       S2_STAMPW(16, 3, c, 4);
-      if (lane == 0) mbar_arrive(&bars->st_conv[st]);
+      if (lane == 0) flag_release(&bars->conv_cnt[warp - 16], c + 1);
       if (warp == 17 && lane == 0) {
         // (1)_c = V^t A_b^t is issued here, off the E chain's critical path: its V operand was just converted by this
         // warp, A_b landed with the stage, and DY_E is free once the E chain has read it for chunk c - 1.
@@ -414,7 +440,7 @@ __global__ void __launch_bounds__(kS2Threads, 1)
         tc_fence_after();
         s2_issue1(tmem, smem_base + st * kS2StageBytes);
         tc_fence_before();
-        mbar_arrive(&bars->issued1);
+        flag_release(&bars->issued1_cnt, c + 1);
       }
       __syncwarp();
     }
