@@ -94,6 +94,9 @@ __device__ __noinline__ bool s2_wait(uint64_t* bar, uint32_t parity, volatile in
 }
 
 __device__ __forceinline__ void s2_wait_warp(uint64_t* bar, uint32_t parity, volatile int* abort_flag, int) {
+#pragma unroll 1
+  for (int i = 0; i < 64; ++i)  // inline fast path: the chains' waits are on the critical path of every chunk
+    if (mbar_try_wait(bar, parity)) return;
   s2_wait(bar, parity, abort_flag);
 }
 
