@@ -223,43 +223,66 @@ __global__ void __launch_bounds__(kPrepThreads, kCh ? 3 : 4)
     }
   }
 
-  // ---- a2: Gram K K^t (lower block triangle): warp w owns rows [16w, 16w+16), n-tile pairs p <= w
+  // ---- a2: Gram K K^t, lower block triangle = 10 blocks of 16 x 16 (block row m, block column p <= m), dealt to the
+  // warps as 3 + 2 + 3 + 2 so that no warp carries the whole last block row
   {
-    float acc[8][4];
+    // warp 0: (3,0) (3,1) (0,0)   warp 1: (3,2) (3,3)   warp 2: (2,0) (2,1) (2,2)   warp 3: (1,0) (1,1)
+    const int m0 = (warp == 0 || warp == 1) ? 3 : (warp == 2 ? 2 : 1);  // block row of units 0 and 1
+    const int p0 = (warp == 1) ? 2 : 0;                                 // block columns p0, p0 + 1
+    const int nun = (warp & 1) ? 2 : 3;                                 // third unit: warp 0 -> (0,0), warp 2 -> (2,2)
+    const int m2 = (warp == 0) ? 0 : 2, p2 = (warp == 0) ? 0 : 2;
+    float acc[3][2][4];
 #pragma unroll
-    for (int nt = 0; nt < 8; ++nt)
+    for (int u = 0; u < 3; ++u)
 #pragma unroll
-      for (int i = 0; i < 4; ++i) acc[nt][i] = 0.f;
-    const int arow = 16 * warp + (lane & 7) + 8 * ((lane >> 3) & 1);
+      for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) acc[u][nt][i] = 0.f;
+    const int lrow = (lane & 7) + 8 * ((lane >> 3) & 1), lcol = 8 * (lane >> 4);  // A operand: ldmatrix lane -> (row, k)
+    const int brow = (lane & 7) + 8 * (lane >> 4), bcol = 8 * ((lane >> 3) & 1);  // B operand
 #pragma unroll
     for (int kk = 0; kk < kD / 16; ++kk) {
-      uint32_t a[4];
-      ldmatrix_x4(a, ks_base + (uint32_t)(arow * kKsPitch + 16 * kk + 8 * (lane >> 4)) * 2u);
-#pragma unroll
-      for (int p = 0; p < 4; ++p) {
-        if (p > warp) continue;
-        uint32_t b[4];
-        const int nrow = 16 * p + (lane & 7) + 8 * (lane >> 4);
-        ldmatrix_x4(b, k2_base + (uint32_t)(nrow * kKsPitch + 16 * kk + 8 * ((lane >> 3) & 1)) * 2u);
-        mma_f16_16816(acc[2 * p], a[0], a[1], a[2], a[3], b[0], b[1]);
-        mma_f16_16816(acc[2 * p + 1], a[0], a[1], a[2], a[3], b[2], b[3]);
+      uint32_t a[4], b[4];
+      ldmatrix_x4(a, ks_base + (uint32_t)((16 * m0 + lrow) * kKsPitch + 16 * kk + lcol) * 2u);
+      ldmatrix_x4(b, k2_base + (uint32_t)((16 * p0 + brow) * kKsPitch + 16 * kk + bcol) * 2u);
+      mma_f16_16816(acc[0][0], a[0], a[1], a[2], a[3], b[0], b[1]);
+      mma_f16_16816(acc[0][1], a[0], a[1], a[2], a[3], b[2], b[3]);
+      ldmatrix_x4(b, k2_base + (uint32_t)((16 * (p0 + 1) + brow) * kKsPitch + 16 * kk + bcol) * 2u);
+      mma_f16_16816(acc[1][0], a[0], a[1], a[2], a[3], b[0], b[1]);
+      mma_f16_16816(acc[1][1], a[0], a[1], a[2], a[3], b[2], b[3]);
+      if (nun == 3) {
+        if (warp == 0) ldmatrix_x4(a, ks_base + (uint32_t)((16 * m2 + lrow) * kKsPitch + 16 * kk + lcol) * 2u);
+        ldmatrix_x4(b, k2_base + (uint32_t)((16 * p2 + brow) * kKsPitch + 16 * kk + bcol) * 2u);
+        mma_f16_16816(acc[2][0], a[0], a[1], a[2], a[3], b[0], b[1]);
+        mma_f16_16816(acc[2][1], a[0], a[1], a[2], a[3], b[2], b[3]);
       }
     }
     if (kCh) __syncthreads();  // every warp is done with K (/) Gamma: L takes over its buffer
-    // L_rj = beta_r exp(G_r - G_j) (k_r.k_j) for j < r, else 0 (the upper blocks are zero-filled: the A_b tile reads them)
+    // the strictly upper blocks are zero (the A_b tile reads them): 6 blocks of 16 x 16 = 384 float4
 #pragma unroll
-    for (int hh = 0; hh < 2; ++hh) {
-      const int r = 16 * warp + gq + 8 * hh;
-      const float br = s_b[r], gr = kCh ? 0.f : s_g[r];
+    for (int it = 0; it < 3; ++it) {
+      const int idx = tid + it * kPrepThreads;       // 0..383
+      const int blk = idx >> 6, e = idx & 63;        // block (i, j) with j > i, 64 float4 each
+      const int bi = blk < 3 ? 0 : (blk < 5 ? 1 : 2), bj = blk < 3 ? blk + 1 : (blk < 5 ? blk - 1 : 3);
+      *reinterpret_cast<float4*>(s_a + (16 * bi + (e >> 2)) * kLPitch + 16 * bj + 4 * (e & 3)) = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    // L_rj = beta_r exp(G_r - G_j) (k_r.k_j) for j < r, else 0
 #pragma unroll
-      for (int nt = 0; nt < 8; ++nt) {
-        const int j = 8 * nt + 2 * tq;
-        float v0 = 0.f, v1 = 0.f;
-        if (nt <= 2 * warp + 1) {
-          if (j < r) v0 = br * (kCh ? 1.f : __expf(gr - s_g[j])) * acc[nt][2 * hh];
-          if (j + 1 < r) v1 = br * (kCh ? 1.f : __expf(gr - s_g[j + 1])) * acc[nt][2 * hh + 1];
+    for (int u = 0; u < 3; ++u) {
+      if (u == 2 && nun < 3) continue;
+      const int mm = (u < 2) ? m0 : m2, pp = (u < 2) ? p0 + u : p2;
+#pragma unroll
+      for (int hh = 0; hh < 2; ++hh) {
+        const int r = 16 * mm + gq + 8 * hh;
+        const float br = s_b[r], gr = kCh ? 0.f : s_g[r];
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt) {
+          const int j = 16 * pp + 8 * nt + 2 * tq;
+          float v0 = 0.f, v1 = 0.f;
+          if (j < r) v0 = br * (kCh ? 1.f : __expf(gr - s_g[j])) * acc[u][nt][2 * hh];
+          if (j + 1 < r) v1 = br * (kCh ? 1.f : __expf(gr - s_g[j + 1])) * acc[u][nt][2 * hh + 1];
+          *reinterpret_cast<float2*>(s_a + r * kLPitch + j) = make_float2(v0, v1);
         }
-        *reinterpret_cast<float2*>(s_a + r * kLPitch + j) = make_float2(v0, v1);
       }
     }
   }
@@ -272,15 +295,16 @@ __global__ void __launch_bounds__(kPrepThreads, kCh ? 3 : 4)
     const int c = lane & 15;
 #pragma unroll
     for (int r = 0; r < 16; ++r) {
-      float sum = (r == c) ? 1.f : 0.f;
+      float part[4] = {(r == c) ? 1.f : 0.f, 0.f, 0.f, 0.f};  // one partial sum per float4 of the row: short chains
 #pragma unroll
       for (int j4 = 0; j4 < (r + 3) / 4; ++j4) {
         const float4 l = *reinterpret_cast<const float4*>(blk + r * kLPitch + 4 * j4);
-        if (4 * j4 + 0 < r) sum = fmaf(-l.x, a[4 * j4 + 0], sum);
-        if (4 * j4 + 1 < r) sum = fmaf(-l.y, a[4 * j4 + 1], sum);
-        if (4 * j4 + 2 < r) sum = fmaf(-l.z, a[4 * j4 + 2], sum);
-        if (4 * j4 + 3 < r) sum = fmaf(-l.w, a[4 * j4 + 3], sum);
+        if (4 * j4 + 0 < r) part[j4] = fmaf(-l.x, a[4 * j4 + 0], part[j4]);
+        if (4 * j4 + 1 < r) part[j4] = fmaf(-l.y, a[4 * j4 + 1], part[j4]);
+        if (4 * j4 + 2 < r) part[j4] = fmaf(-l.z, a[4 * j4 + 2], part[j4]);
+        if (4 * j4 + 3 < r) part[j4] = fmaf(-l.w, a[4 * j4 + 3], part[j4]);
       }
+      const float sum = (part[0] + part[1]) + (part[2] + part[3]);
       a[r] = sum;
     }
     __syncwarp();
