@@ -101,7 +101,7 @@ __device__ __forceinline__ void block_zero(float (&acc)[2][4]) {
 constexpr int kPrepChunksPerCta = 4;
 
 template <bool kCh>
-__global__ void __launch_bounds__(kPrepThreads, kCh ? 3 : 4)
+__global__ void __launch_bounds__(kPrepThreads, 4)
     prep_kernel(const __nv_bfloat16* __restrict__ k, const float* __restrict__ g, const float* __restrict__ beta,
                 const int2* __restrict__ chunk_meta, int cap, int H,
                 uint8_t* __restrict__ rec, float* __restrict__ gate) {
