@@ -215,29 +215,38 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
         named_bar_sync(1 + q, 64);
         m = fmaxf(m, xch[2 * row + (hf ^ 1)]);
         S2_STAMP(b, c, 5);
-        // row maximum in [2^(e-127), 2^(e-126)): move it to [2^14, 2^15)
+        // row maximum in [2^(e-127), 2^(e-126)): move it to [2^14, 2^15) -- in place, the row stays normalised
         const int e = (int)(__float_as_uint(m) >> 23);
         int dlt = (e == 0) ? 0 : 141 - e;
         dlt = max(-100, min(100, dlt));
         s_exp += dlt;
         const float sc = pow2i(dlt);
         f = gC * sc;
-        uint32_t hh[16];
+        if (kCh) {  // per-channel gate: normalise in place, the per-column decay follows below
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          uint32_t a0 = x0[2 * j], a1 = x0[2 * j + 1];
-          mul2(a0, a1, sc);
-          hh[j] = pack_f16(__uint_as_float(a0), __uint_as_float(a1));
-        }
-        tmem_st16(tH, hh);
+          for (int j = 0; j < 16; ++j) {
+            mul2(x0[2 * j], x0[2 * j + 1], sc);
+            mul2(x1[2 * j], x1[2 * j + 1], sc);
+          }
+        } else {    // scalar gate: Xh from x sc, then one multiply by gamma_C sc below
+          uint32_t hh[16];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          uint32_t a0 = x1[2 * j], a1 = x1[2 * j + 1];
-          mul2(a0, a1, sc);
-          hh[j] = pack_f16(__uint_as_float(a0), __uint_as_float(a1));
+          for (int j = 0; j < 16; ++j) {
+            uint32_t a0 = x0[2 * j], a1 = x0[2 * j + 1];
+            mul2(a0, a1, sc);
+            hh[j] = pack_f16(__uint_as_float(a0), __uint_as_float(a1));
+          }
+          tmem_st16(tH, hh);
+#pragma unroll
+          for (int j = 0; j < 16; ++j) {
+            uint32_t a0 = x1[2 * j], a1 = x1[2 * j + 1];
+            mul2(a0, a1, sc);
+            hh[j] = pack_f16(__uint_as_float(a0), __uint_as_float(a1));
+          }
+          tmem_st16(tH + 16, hh);
         }
-        tmem_st16(tH + 16, hh);
-      } else {
+      }
+      if (!kIsT || kCh) {
         uint32_t hh[16];
 #pragma unroll
         for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x0[2 * j]), __uint_as_float(x0[2 * j + 1]));
@@ -251,10 +260,10 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
 #pragma unroll
         for (int j4 = 0; j4 < 8; ++j4) {
           const float4 a = gv[j4], b4 = gv[8 + j4];
-          mul2v(x0[4 * j4], x0[4 * j4 + 1], f * a.x, f * a.y);
-          mul2v(x0[4 * j4 + 2], x0[4 * j4 + 3], f * a.z, f * a.w);
-          mul2v(x1[4 * j4], x1[4 * j4 + 1], f * b4.x, f * b4.y);
-          mul2v(x1[4 * j4 + 2], x1[4 * j4 + 3], f * b4.z, f * b4.w);
+          mul2v(x0[4 * j4], x0[4 * j4 + 1], a.x, a.y);
+          mul2v(x0[4 * j4 + 2], x0[4 * j4 + 3], a.z, a.w);
+          mul2v(x1[4 * j4], x1[4 * j4 + 1], b4.x, b4.y);
+          mul2v(x1[4 * j4 + 2], x1[4 * j4 + 3], b4.z, b4.w);
         }
       } else {
 #pragma unroll
