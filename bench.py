@@ -311,7 +311,25 @@ def time_extra_cfg4(hb, device, peaks, iters=48):
     head_steps = sum(r.n_steps for r in reqs) * H
     gbs = head_steps * COMPOSE_BYTES_PER_STEP / (ms * 1e-3) / 1e9
     fam = hb.hypic_compose_impl_for(H, D, D)
+    # the same requests over fp16-stored pools (hypic_compose_f16; the paper's cache precision)
+    Eh, Th = hb.hypic_tuple_pack_f16(E), hb.hypic_tuple_pack_f16(T)
+    del E, T
+    for i in range(3):
+        hb.hypic_compose_f16(reqs[i].S_in, Eh, Th, reqs[i].seg_ids, reqs[i].cu_segs, S_out=S_out)
+    torch.cuda.synchronize()
+    e0.record()
+    for rq in reqs:
+        hb.hypic_compose_f16(rq.S_in, Eh, Th, rq.seg_ids, rq.cu_segs, S_out=S_out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms16 = e0.elapsed_time(e1)
+    gbs16 = head_steps * (COMPOSE_BYTES_PER_STEP // 2) / (ms16 * 1e-3) / 1e9
+    f16 = {"ms_total": ms16, "compose_ops_per_s": head_steps / (ms16 * 1e-3),
+           "roofline": {"bound": "hbm", "achieved": gbs16, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                        "frac": gbs16 / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"]},
+           "note": "hypic_compose_f16: 65,536 B of fp16 (T_i, E_i) per head-step"}
     return {"workload": f"cfg4: P=1024, H=32, R=128, n~U{{16..64}}, {iters} layer-iterations, compose only",
+            "fp16_pools": f16,
             "ms_total": ms, "head_steps": head_steps, "compose_ops_per_s": head_steps / (ms * 1e-3),
             "request_layer_ops_per_s": head_steps / H / (ms * 1e-3),
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",

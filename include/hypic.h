@@ -115,6 +115,26 @@ int hypic_compose(const float* S_in, const float* E_pool, const float* T_pool, c
                   int32_t dv, float* S_out, void* stream);
 
 /*
+ * hypic_compose_f16: hypic_compose over pools stored in fp16 -- the precision the paper keeps its cached tuples in
+ * (32 KB per T at dk = dv = 128: Table 3).  Same fold, same argument meaning and error behaviour as
+ * hypic_compose; the differences:
+ *   E_pool   [P, H, dv, dk] fp16 (IEEE binary16), T_pool [P, H, dk, dk] fp16; S_in / S_out stay fp32
+ *   the stored fp16 values are taken as exact inputs (the result is the fp32-accurate fold of THOSE tuples; what is
+ *   lost by storing a tuple in fp16 is lost when it is packed, see hypic_tuple_pack_f16)
+ * Built envelope: dv = dk = 128 (tcgen05/TMEM kernel only; there is no SIMT variant), |S| below 1e30.
+ */
+int hypic_compose_f16(const float* S_in, const void* E_pool, const void* T_pool, const int32_t* seg_ids,
+                      const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk, int32_t dv,
+                      float* S_out, void* stream);
+
+/*
+ * hypic_tuple_pack_f16: dst[i] = fp16(src[i]) (round to nearest even; overflow to +-inf, underflow through fp16
+ * subnormals to zero, as IEEE conversion does) for i < count: packs the fp32 E / T tensors of hypic_segment_encode into
+ * the fp16 pools of hypic_compose_f16.  src fp32 [count], dst fp16 [count], both 16-byte aligned, no overlap.
+ */
+int hypic_tuple_pack_f16(const float* src, void* dst, size_t count, void* stream);
+
+/*
  * hypic_encode_impl_for / hypic_compose_impl_for: which kernel family (HYPIC_IMPL_SIMT or HYPIC_IMPL_TENSOR)
  * a call with this shape would run under the current hypic_set_impl setting, or a negative hypic_status_t
  * (-HYPIC_ERR_UNSUPPORTED / -HYPIC_ERR_INVALID_ARG) if the call would be rejected.  Pure host arithmetic;

@@ -28,7 +28,8 @@ HYPIC_IMPL_TENSOR = 2
 EXPORTS = (
     "hypic_set_impl", "hypic_get_impl", "hypic_segment_encode_workspace", "hypic_segment_encode", "hypic_compose",
     "hypic_status_string", "hypic_version", "hypic_last_launch_count", "hypic_encode_impl_for",
-    "hypic_compose_impl_for", "hypic_debug_timeout_count", "hypic_envelope_violation_count",
+    "hypic_compose_impl_for", "hypic_debug_timeout_count", "hypic_envelope_violation_count", "hypic_compose_f16",
+    "hypic_tuple_pack_f16",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -63,6 +64,10 @@ def load_library() -> ctypes.CDLL:
     lib.hypic_segment_encode.restype = ctypes.c_int
     lib.hypic_compose.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp, vp]
     lib.hypic_compose.restype = ctypes.c_int
+    lib.hypic_compose_f16.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp, vp]
+    lib.hypic_compose_f16.restype = ctypes.c_int
+    lib.hypic_tuple_pack_f16.argtypes = [vp, vp, sz, vp]
+    lib.hypic_tuple_pack_f16.restype = ctypes.c_int
     lib.hypic_status_string.argtypes = [ctypes.c_int]
     lib.hypic_status_string.restype = ctypes.c_char_p
     lib.hypic_version.argtypes = []
@@ -223,3 +228,57 @@ def hypic_compose(S_in: Optional[torch.Tensor], E_pool: torch.Tensor, T_pool: to
     if rc != HYPIC_OK:
         raise HypicError(rc, "hypic_compose")
     return S_out
+
+
+def hypic_compose_f16(S_in: Optional[torch.Tensor], E_pool: torch.Tensor, T_pool: torch.Tensor, seg_ids: torch.Tensor,
+                      cu_segs: torch.Tensor, *, total_steps: Optional[int] = None,
+                      S_out: Optional[torch.Tensor] = None,
+                      stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """hypic_compose over fp16-stored pools (E_pool, T_pool: torch.float16); S_in / S_out stay fp32."""
+    lib = load_library()
+    for name, t in (("E_pool", E_pool), ("T_pool", T_pool), ("seg_ids", seg_ids), ("cu_segs", cu_segs)):
+        if not t.is_cuda:
+            raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if E_pool.dim() != 4 or T_pool.dim() != 4:
+        raise ValueError("E_pool:[P,H,dv,dk], T_pool:[P,H,dk,dk]")
+    P, H, dv, dk = (int(x) for x in E_pool.shape)
+    if tuple(T_pool.shape) != (P, H, dk, dk):
+        raise ValueError("T_pool must be [P,H,dk,dk]")
+    R = int(cu_segs.numel()) - 1
+    if R < 0:
+        raise ValueError("cu_segs must have R+1 >= 1 entries")
+    if total_steps is None:
+        total_steps = int(seg_ids.numel())  # shape metadata, no device sync
+    if S_in is not None and tuple(S_in.shape) != (R, H, dv, dk):
+        raise ValueError("S_in must be [R,H,dv,dk]")
+    if S_out is None:
+        S_out = torch.empty((R, H, dv, dk), dtype=torch.float32, device=E_pool.device)
+    if tuple(S_out.shape) != (R, H, dv, dk):
+        raise ValueError("S_out must be [R,H,dv,dk]")
+    with torch.cuda.device(E_pool.device):
+        rc = lib.hypic_compose_f16(
+            _dev_ptr(S_in, "S_in", torch.float32), _dev_ptr(E_pool, "E_pool", torch.float16),
+            _dev_ptr(T_pool, "T_pool", torch.float16), _dev_ptr(seg_ids, "seg_ids", torch.int32),
+            _dev_ptr(cu_segs, "cu_segs", torch.int32), R, P, int(total_steps), H, dk, dv,
+            _dev_ptr(S_out, "S_out", torch.float32), _stream_handle(stream))
+    if rc != HYPIC_OK:
+        raise HypicError(rc, "hypic_compose_f16")
+    return S_out
+
+
+def hypic_tuple_pack_f16(src: torch.Tensor, dst: Optional[torch.Tensor] = None,
+                         stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """dst = fp16(src), round to nearest even: packs fp32 E / T tensors into the fp16 pools of hypic_compose_f16."""
+    lib = load_library()
+    if not src.is_cuda:
+        raise ValueError("src must be a CUDA tensor (no CPU fallback)")
+    if dst is None:
+        dst = torch.empty(src.shape, dtype=torch.float16, device=src.device)
+    if dst.numel() != src.numel():
+        raise ValueError("dst must have as many elements as src")
+    with torch.cuda.device(src.device):
+        rc = lib.hypic_tuple_pack_f16(_dev_ptr(src, "src", torch.float32), _dev_ptr(dst, "dst", torch.float16),
+                                      int(src.numel()), _stream_handle(stream))
+    if rc != HYPIC_OK:
+        raise HypicError(rc, "hypic_tuple_pack_f16")
+    return dst

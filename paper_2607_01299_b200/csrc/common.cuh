@@ -44,6 +44,17 @@ struct ComposeArgs {
   cudaStream_t stream;
 };
 
+struct ComposeF16Args {
+  const float* S_in;
+  const void* E_pool;  // fp16
+  const void* T_pool;  // fp16
+  const int32_t* seg_ids;
+  const int32_t* cu_segs;
+  int32_t R, P, total_steps, H, dk, dv;
+  float* S_out;
+  cudaStream_t stream;
+};
+
 // Kernel families (each returns a hypic_status_t; UNSUPPORTED when the shape is outside its envelope).
 int encode_simt(const EncodeArgs& a);
 int compose_simt(const ComposeArgs& a);
@@ -57,6 +68,10 @@ int encode_tensor(const EncodeArgs& a);
 bool compose_tensor_shape_ok(int32_t H, int32_t dk, int32_t dv);
 inline bool compose_tensor_supported(const ComposeArgs& a) { return compose_tensor_shape_ok(a.H, a.dk, a.dv); }
 int compose_tensor(const ComposeArgs& a);
+bool compose_f16_shape_ok(int32_t H, int32_t dk, int32_t dv);
+int compose_f16(const ComposeF16Args& a);
+int pack_f16(const float* src, void* dst, size_t n, cudaStream_t stream);
+unsigned int debug_timeout_count_compose_f16();
 unsigned int debug_timeout_count_encode();
 unsigned int envelope_violation_count_encode();
 unsigned int debug_timeout_count();  // bounded-wait expiries in the tensor kernels since load (0 = healthy)

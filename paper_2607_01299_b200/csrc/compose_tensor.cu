@@ -374,8 +374,8 @@ int compose_tensor(const ComposeArgs& a) {
 unsigned int debug_timeout_count() {
   unsigned int v = 0;
   if (cudaMemcpyFromSymbol(&v, g_timeout_count, sizeof(v)) != cudaSuccess) return 0xffffffffu;
-  const unsigned int e = debug_timeout_count_encode();
-  return e == 0xffffffffu ? e : v + e;
+  const unsigned int e = debug_timeout_count_encode(), f = debug_timeout_count_compose_f16();
+  return (e == 0xffffffffu || f == 0xffffffffu) ? 0xffffffffu : v + e + f;
 }
 
 }  // namespace hypic

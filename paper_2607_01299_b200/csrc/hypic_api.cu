@@ -106,6 +106,27 @@ int hypic_compose(const float* S_in, const float* E_pool, const float* T_pool, c
   return compose_simt(a);
 }
 
+int hypic_compose_f16(const float* S_in, const void* E_pool, const void* T_pool, const int32_t* seg_ids,
+                      const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk, int32_t dv,
+                      float* S_out, void* stream) {
+  g_launch_count = 0;
+  if (R < 0 || P < 0 || total_steps < 0 || H <= 0 || dk <= 0 || dv <= 0) return HYPIC_ERR_INVALID_ARG;
+  if (!cu_segs) return HYPIC_ERR_INVALID_ARG;
+  if (R > 0 && !S_out) return HYPIC_ERR_INVALID_ARG;
+  if (total_steps > 0 && (!E_pool || !T_pool || !seg_ids || P == 0)) return HYPIC_ERR_INVALID_ARG;
+  if (!aligned16(S_in) || !aligned16(E_pool) || !aligned16(T_pool) || !aligned16(S_out)) return HYPIC_ERR_INVALID_ARG;
+  if (!compose_f16_shape_ok(H, dk, dv)) return HYPIC_ERR_UNSUPPORTED;
+  ComposeF16Args a{S_in, E_pool, T_pool, seg_ids, cu_segs, R, P, total_steps, H, dk, dv, S_out, (cudaStream_t)stream};
+  return compose_f16(a);
+}
+
+int hypic_tuple_pack_f16(const float* src, void* dst, size_t count, void* stream) {
+  g_launch_count = 0;
+  if (count > 0 && (!src || !dst)) return HYPIC_ERR_INVALID_ARG;
+  if (!aligned16(src) || !aligned16(dst)) return HYPIC_ERR_INVALID_ARG;
+  return pack_f16(src, dst, count, (cudaStream_t)stream);
+}
+
 int hypic_encode_impl_for(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate) {
   const int vs = validate_encode_shape(0, 0, H, dk, dv, kv_dtype, gate);
   if (vs != HYPIC_OK) return -vs;

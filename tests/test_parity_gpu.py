@@ -315,3 +315,68 @@ def test_tensor_family_envelope_guard():
     E_ref, T_ref = oracle_encode(inp)
     check_E(E, E_ref, TOL_BF16)
     check_T(T, T_ref, TOL_BF16)
+
+
+# ------------------------------------------------------------- fp16-stored tuples
+def test_tuple_pack_f16_is_ieee_rne():
+    """hypic_tuple_pack_f16 = IEEE fp32 -> fp16 conversion, bit for bit (numpy's astype is the definition): normal
+    values, fp16 subnormals, overflow to inf, signed zeros, a ragged tail."""
+    gen = torch.Generator().manual_seed(5)
+    x = torch.randn(4099, generator=gen) * torch.pow(10.0, torch.randint(-9, 6, (4099,), generator=gen).float())
+    x[:6] = torch.tensor([0.0, -0.0, 65504.0, 65520.0, -1e-8, 6.0e-8])
+    got = hb.hypic_tuple_pack_f16(x.cuda()).cpu().numpy()
+    with np.errstate(over="ignore"):
+        want = x.numpy().astype(np.float16)
+    assert np.array_equal(got.view(np.uint16), want.view(np.uint16))
+    assert hb.hypic_tuple_pack_f16(torch.empty(0, device="cuda")).numel() == 0
+
+
+def test_compose_f16_pools_vs_oracle():
+    """hypic_compose_f16: pools stored in fp16 (as the paper caches them) are exact inputs; the fold
+    must match the fp64 compose of the same stored values to the fp32-input tolerance.  Near-unit pool (reading S9),
+    lists of length 0, 1 and 39, repeated and unsorted ids, NULL and in-place S."""
+    P, H, d = 24, 3, 128
+    pin = wl.near_unit_pool_inputs(P, H, device="cuda", d=d, kv_dtype=torch.float32)
+    hb.hypic_set_impl(hb.HYPIC_IMPL_SIMT)
+    E, T = hb.hypic_segment_encode(pin.k, pin.v, pin.g, pin.beta, pin.cu_seqlens, pin.gate)
+    hb.hypic_set_impl(hb.HYPIC_IMPL_AUTO)
+    Eh, Th = hb.hypic_tuple_pack_f16(E), hb.hypic_tuple_pack_f16(T)
+    E64, T64 = Eh.cpu().numpy().astype(np.float32), Th.cpu().numpy().astype(np.float32)
+    gen = torch.Generator().manual_seed(321)
+    ids = torch.randint(0, P, (40,), generator=gen, dtype=torch.int32).cuda()
+    cu = torch.tensor([0, 0, 1, 40], dtype=torch.int32, device="cuda")
+    S_in = torch.randn(3, H, d, d, device="cuda")
+    S = hb.hypic_compose_f16(S_in, Eh, Th, ids, cu)
+    torch.cuda.synchronize()
+    ref = oracle.compose(S_in.cpu().numpy(), E64, T64, ids.cpu().numpy(), cu.cpu().numpy())
+    check_E(S, ref, TOL_F32, "S_out (fp16 pools)")
+    assert torch.equal(S[0], S_in[0])  # empty list copies S_in
+    S0 = hb.hypic_compose_f16(None, Eh, Th, ids, cu)
+    ref0 = oracle.compose(None, E64, T64, ids.cpu().numpy(), cu.cpu().numpy())
+    check_E(S0, ref0, TOL_F32, "S_out (fp16 pools, NULL S_in)")
+    S3 = S_in.clone()
+    hb.hypic_compose_f16(S3, Eh, Th, ids, cu, S_out=S3)
+    assert torch.equal(S3, S)
+    # what fp16 storage costs against the fp32 tuples (context: the paper reports 6e-5 at layer 0, PAPER.md:216)
+    ref32 = oracle.compose(S_in.cpu().numpy(), E.cpu().numpy(), T.cpu().numpy(), ids.cpu().numpy(), cu.cpu().numpy())
+    assert oracle.rel_fro(S.cpu().numpy()[2], ref32[2]) < 2e-3
+    with pytest.raises(hb.HypicError):
+        hb.hypic_compose_f16(None, Eh[..., :64, :64].contiguous(), Th[..., :64, :64].contiguous(), ids, cu)
+
+
+def test_cfg4_compose_f16_sampled_requests():
+    """cfg4 at full size for one layer-iteration with fp16-stored pools: sampled chains against the fp64 compose of
+    the stored values."""
+    pin = wl.cfg4_pool_inputs(device="cuda")
+    _, T = gpu_encode(pin, hb.HYPIC_IMPL_AUTO)
+    del pin
+    Th = hb.hypic_tuple_pack_f16(T)
+    del T
+    Eh = hb.hypic_tuple_pack_f16(wl.cfg4_pool_E(device="cuda"))
+    req = wl.cfg4_requests(device="cuda")
+    S = hb.hypic_compose_f16(req.S_in, Eh, Th, req.seg_ids, req.cu_segs)
+    assert torch.isfinite(S).all()
+    units = _sample_units(128, 32, 6, 5)
+    ref = oracle_compose_units(req.S_in, Eh.float(), Th.float(), req.seg_ids, req.cu_segs, units)
+    ri, hi = torch.tensor([u[0] for u in units]), torch.tensor([u[1] for u in units])
+    check_E(S[ri, hi][:, None], ref, TOL_F32, "S_out")
