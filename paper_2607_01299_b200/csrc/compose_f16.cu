@@ -26,15 +26,16 @@ using namespace ptx;
 
 constexpr int kD = 128;
 constexpr int kTSlab = 32 * kD * 2;   // 32 rows of T in fp16: 8 KB = two boxes of 4 KB
-constexpr int kNT = 8;                // T slabs in flight (two full matrices)
+constexpr int kTMat = 4 * kTSlab;     // one T matrix: 32 KB
+constexpr int kNT = 3;                // T matrices in flight (one mbarrier probe per step: a probe costs ~380 cycles)
 constexpr int kEQuarter = 32 * kD * 2;  // 32 rows of E in fp16: 8 KB = two boxes
 constexpr int kNE = 8;                // E quarter slots: two buffers x 4 TMEM lane quarters
-constexpr int kThreads = 352;         // warp 0 T producer, 1 MMA issuer, 2 E producer, 3-10 round trip
+constexpr int kThreads = 608;         // warp 0 T producer, 1 MMA issuer, 2 E producer, 3-18 round trip
 
 constexpr int kOffT = 0;
-constexpr int kOffE = kOffT + kNT * kTSlab;
+constexpr int kOffE = kOffT + kNT * kTMat;
 constexpr int kOffXch = kOffE + kNE * kEQuarter;
-constexpr int kOffBar = kOffXch + 1024;
+constexpr int kOffBar = kOffXch + 2048;
 constexpr int kSmemBytes = kOffBar + 512 + 1024;
 
 struct Bars {
@@ -63,6 +64,13 @@ __device__ __forceinline__ void split_f16(float x0, float x1, uint32_t& hi, uint
 }
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
+      "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+      "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+      : "memory");
 }
 __device__ __forceinline__ void tma_load_2d(void* dst_smem, const CUtensorMap* tm, int c0, int c1, uint64_t* bar) {
   asm volatile(
@@ -116,9 +124,9 @@ __global__ void __launch_bounds__(kThreads, 1)
   if (warp == 0) tmem_alloc(&bars->tmem_base, 256);
   if (tid == 32) {
     for (int i = 0; i < kNT; ++i) { mbar_init(&bars->t_full[i], 1); mbar_init(&bars->t_empty[i], 1); }
-    for (int i = 0; i < kNE; ++i) { mbar_init(&bars->e_full[i], 1); mbar_init(&bars->e_empty[i], 2); }
+    for (int i = 0; i < kNE; ++i) { mbar_init(&bars->e_full[i], 1); mbar_init(&bars->e_empty[i], 4); }
     mbar_init(&bars->d_full, 1);
-    mbar_init(&bars->a_ready, 8);
+    mbar_init(&bars->a_ready, 16);
     bars->abort_flag = 0;
     fence_barrier_init();
   }
@@ -134,13 +142,15 @@ __global__ void __launch_bounds__(kThreads, 1)
       uint32_t it = 0;
       for (int i = 0; i < n; ++i) {
         const int row0 = (seg_ids[seg_begin + i] * H + h) * kD;
-        for (int j = 0; j < 4; ++j, ++it) {
-          const uint32_t slot = it % kNT, ph = (it / kNT) & 1;
-          wait_or_abort(&bars->t_empty[slot], ph ^ 1, abort_flag);
-          mbar_expect_tx(&bars->t_full[slot], kTSlab);
-          tma_load_2d(smem + kOffT + slot * kTSlab, &tmT, 0, row0 + 32 * j, &bars->t_full[slot]);
-          tma_load_2d(smem + kOffT + slot * kTSlab + kTSlab / 2, &tmT, 64, row0 + 32 * j, &bars->t_full[slot]);
+        const uint32_t slot = it % kNT, ph = (it / kNT) & 1;
+        wait_or_abort(&bars->t_empty[slot], ph ^ 1, abort_flag);
+        mbar_expect_tx(&bars->t_full[slot], kTMat);
+        for (int j = 0; j < 4; ++j) {
+          uint8_t* dst = smem + kOffT + slot * kTMat + j * kTSlab;
+          tma_load_2d(dst, &tmT, 0, row0 + 32 * j, &bars->t_full[slot]);
+          tma_load_2d(dst + kTSlab / 2, &tmT, 64, row0 + 32 * j, &bars->t_full[slot]);
         }
+        ++it;
       }
     }
   } else if (warp == 1) {
@@ -149,13 +159,13 @@ __global__ void __launch_bounds__(kThreads, 1)
       constexpr uint32_t idesc = make_idesc(0u, 128, 128, 0, 1);  // fp16, M = N = 128, A from TMEM, B MN-major
       uint32_t it = 0;
       for (int i = 0; i < n; ++i) {
+        const uint32_t slot = it % kNT, ph = (it / kNT) & 1;
+        wait_or_abort(&bars->t_full[slot], ph, abort_flag);  // T runs ahead of the state: probe it first
         wait_or_abort(&bars->a_ready, i & 1, abort_flag);
         tc_fence_after();
-        for (int j = 0; j < 4; ++j, ++it) {
-          const uint32_t slot = it % kNT, ph = (it / kNT) & 1;
-          wait_or_abort(&bars->t_full[slot], ph, abort_flag);
-          tc_fence_after();
-          const uint32_t t_addr = smem_u32(smem + kOffT + slot * kTSlab);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t t_addr = smem_u32(smem + kOffT + slot * kTMat + j * kTSlab);
 #pragma unroll
           for (int ks = 0; ks < 2; ++ks) {
             // 16 rows of T per instruction = two 8-row atoms of 1 KB; the two 64-column boxes are 4 KB apart
@@ -164,8 +174,9 @@ __global__ void __launch_bounds__(kThreads, 1)
             mma_f16_ts(tD, tAhi + acol, bd, idesc, (j | ks) > 0);
             mma_f16_ts(tD, tAlo + acol, bd, idesc, 1);
           }
-          mma_commit(&bars->t_empty[slot]);
         }
+        mma_commit(&bars->t_empty[slot]);
+        ++it;
         mma_commit(&bars->d_full);
       }
     }
@@ -187,44 +198,41 @@ __global__ void __launch_bounds__(kThreads, 1)
   } else {
     // ---------------------------------------------------------------- round trip: D (+E) -> next S_hi/S_lo or S_out
     const int q = warp & 3;            // TMEM lane quarter this warp may touch
-    const int half = (warp - 3) >> 2;  // which 64 columns of the quarter this warp handles
+    const int part = (warp - 3) >> 2;  // which 32 columns of the quarter this warp handles (4 warps per quarter)
     const uint32_t lane_base = (uint32_t)(32 * q) << 16;
     const int row = 32 * q + lane;
-    float* out_row = S_out + (size_t)unit * mat + (size_t)row * kD + 64 * half;
+    float* out_row = S_out + (size_t)unit * mat + (size_t)row * kD + 32 * part;
     float* xch = reinterpret_cast<float*>(smem + kOffXch);
     float unscale = 1.f;  // D of step s holds 2^-r_m (S T): r_m = this row's normalisation chosen after step s - 1
     for (int s = -1; s < n; ++s) {
       const bool last = (s == n - 1);
-      float xv[64];
+      float xv[32];
       if (s >= 0) {
+        const uint32_t eslot = (uint32_t)(4 * s + q) % kNE, eph = ((uint32_t)(4 * s + q) / kNE) & 1;
+        wait_or_abort(&bars->e_full[eslot], eph, abort_flag);  // E runs ahead: its probe overlaps the MMAs
         wait_or_abort(&bars->d_full, s & 1, abort_flag);
         tc_fence_after();
-        const uint32_t eslot = (uint32_t)(4 * s + q) % kNE, eph = ((uint32_t)(4 * s + q) / kNE) & 1;
-        wait_or_abort(&bars->e_full[eslot], eph, abort_flag);
-        const uint8_t* eb = smem + kOffE + eslot * kEQuarter + half * (kEQuarter / 2) + lane * 128;
+        const uint8_t* eb = smem + kOffE + eslot * kEQuarter + (part >> 1) * (kEQuarter / 2) + lane * 128;
+        uint32_t d[32];
+        tmem_ld32(tD + lane_base + 32 * part, d);
+        tmem_ld_wait();
 #pragma unroll
-        for (int cc = 0; cc < 2; ++cc) {
-          uint32_t d[32];
-          tmem_ld32(tD + lane_base + 64 * half + 32 * cc, d);
-          tmem_ld_wait();
+        for (int u = 0; u < 4; ++u) {  // 8 columns per 16-byte chunk
+          const uint4 e = *reinterpret_cast<const uint4*>(eb + (((4 * (part & 1) + u) ^ (lane & 7)) * 16));
+          const uint32_t ew[4] = {e.x, e.y, e.z, e.w};
 #pragma unroll
-          for (int u = 0; u < 4; ++u) {  // 8 columns per 16-byte chunk
-            const uint4 e = *reinterpret_cast<const uint4*>(eb + (((4 * cc + u) ^ (lane & 7)) * 16));
-            const uint32_t ew[4] = {e.x, e.y, e.z, e.w};
-#pragma unroll
-            for (int p = 0; p < 4; ++p) {
-              const float2 ef = __half22float2(*reinterpret_cast<const __half2*>(&ew[p]));
-              xv[32 * cc + 8 * u + 2 * p] = fmaf(__uint_as_float(d[8 * u + 2 * p]), unscale, ef.x);
-              xv[32 * cc + 8 * u + 2 * p + 1] = fmaf(__uint_as_float(d[8 * u + 2 * p + 1]), unscale, ef.y);
-            }
+          for (int p = 0; p < 4; ++p) {
+            const float2 ef = __half22float2(*reinterpret_cast<const __half2*>(&ew[p]));
+            xv[8 * u + 2 * p] = fmaf(__uint_as_float(d[8 * u + 2 * p]), unscale, ef.x);
+            xv[8 * u + 2 * p + 1] = fmaf(__uint_as_float(d[8 * u + 2 * p + 1]), unscale, ef.y);
           }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&bars->e_empty[eslot]);
       } else {
-        const float4* src = reinterpret_cast<const float4*>(S_in + (size_t)unit * mat + (size_t)row * kD + 64 * half);
+        const float4* src = reinterpret_cast<const float4*>(S_in + (size_t)unit * mat + (size_t)row * kD + 32 * part);
 #pragma unroll
-        for (int u = 0; u < 16; ++u) {
+        for (int u = 0; u < 8; ++u) {
           const float4 v = (S_in != nullptr) ? src[u] : make_float4(0.f, 0.f, 0.f, 0.f);
           xv[4 * u] = v.x, xv[4 * u + 1] = v.y, xv[4 * u + 2] = v.z, xv[4 * u + 3] = v.w;
         }
@@ -232,25 +240,26 @@ __global__ void __launch_bounds__(kThreads, 1)
       if (last) {
         float4* o4 = reinterpret_cast<float4*>(out_row);
 #pragma unroll
-        for (int u = 0; u < 16; ++u) o4[u] = make_float4(xv[4 * u], xv[4 * u + 1], xv[4 * u + 2], xv[4 * u + 3]);
+        for (int u = 0; u < 8; ++u) o4[u] = make_float4(xv[4 * u], xv[4 * u + 1], xv[4 * u + 2], xv[4 * u + 3]);
       } else {
-        // row normalisation: maximum of the whole row (both column halves) into [2^13, 2^14)
+        // row normalisation: maximum of the whole row (all four column parts) into [2^13, 2^14)
         float m = 0.f;
 #pragma unroll
-        for (int c = 0; c < 64; c += 2) m = fmaxf(m, fmaxf(fabsf(xv[c]), fabsf(xv[c + 1])));
-        xch[2 * row + half] = m;
-        named_bar_sync(1 + q, 64);
-        m = fmaxf(m, xch[2 * row + (half ^ 1)]);
+        for (int c = 0; c < 32; c += 2) m = fmaxf(m, fmaxf(fabsf(xv[c]), fabsf(xv[c + 1])));
+        xch[4 * row + part] = m;
+        named_bar_sync(1 + q, 128);
+        const float4 mm = *reinterpret_cast<const float4*>(xch + 4 * row);
+        m = fmaxf(fmaxf(mm.x, mm.y), fmaxf(mm.z, mm.w));
         const int e = (int)(__float_as_uint(m) >> 23);
         int rs = (e == 0) ? 0 : e - 140;  // max in [2^(e-127), 2^(e-126)) -> 2^-rs max in [2^13, 2^14)
         rs = max(-100, min(100, rs));
         const float sc = __uint_as_float((uint32_t)(127 - rs) << 23);
         unscale = __uint_as_float((uint32_t)(127 + rs) << 23);
-        uint32_t hi[32], lo[32];
+        uint32_t hi[16], lo[16];
 #pragma unroll
-        for (int c = 0; c < 32; ++c) split_f16(xv[2 * c] * sc, xv[2 * c + 1] * sc, hi[c], lo[c]);
-        tmem_st32(tAhi + lane_base + 32 * half, hi);
-        tmem_st32(tAlo + lane_base + 32 * half, lo);
+        for (int c = 0; c < 16; ++c) split_f16(xv[2 * c] * sc, xv[2 * c + 1] * sc, hi[c], lo[c]);
+        tmem_st16(tAhi + lane_base + 16 * part, hi);
+        tmem_st16(tAlo + lane_base + 16 * part, lo);
         tmem_st_wait();
         tc_fence_before();
         __syncwarp();
