@@ -52,6 +52,8 @@ def _load():
         lib.hypic_oracle_segment_encode.restype = i32
         lib.hypic_oracle_sequential.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp]
         lib.hypic_oracle_sequential.restype = i32
+        lib.hypic_oracle_seam_window.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]
+        lib.hypic_oracle_seam_window.restype = i32
         lib.hypic_oracle_compose.argtypes = [vp, vp, vp, i32, vp, vp, i32, i32, i32, i32, i32, vp]
         lib.hypic_oracle_compose.restype = i32
         _lib = lib
@@ -133,6 +135,28 @@ def sequential(S_in, k, v, g, beta, cu_tokens, gate: int = GATE_SCALAR):
     if rc != 0:
         raise ValueError(f"hypic_oracle_sequential failed with code {rc}")
     return S_out
+
+
+def seam_window(S_in, q, k, v, g, beta, cu_tokens, gate: int = GATE_SCALAR):
+    """Seam-window step: token recurrence from S_in over each request's window tokens with the
+    per-token read-out o_t = S_t q_t (row convention).  q:[Ttot,H,dk].  Returns (S_out:[R,H,dv,dk],
+    o:[Ttot,H,dv]) float64; rows of o for tokens outside every request are NaN."""
+    k, v, g, beta, ttot, H, dk, dv = _check_inputs(k, v, g, beta, gate)
+    q = _f32(q)
+    assert q.shape == (ttot, H, dk)
+    cu = _i32(cu_tokens)
+    R = cu.shape[0] - 1
+    assert np.all(np.diff(cu) >= 0) and cu[0] >= 0 and cu[-1] <= ttot
+    if S_in is not None:
+        S_in = np.ascontiguousarray(S_in, dtype=np.float64)
+        assert S_in.shape == (R, H, dv, dk)
+    S_out = np.empty((R, H, dv, dk), dtype=np.float64)
+    o = np.full((ttot, H, dv), np.nan, dtype=np.float64)
+    rc = _load().hypic_oracle_seam_window(_ptr(S_in), _ptr(q), _ptr(k), _ptr(v), _ptr(g), _ptr(beta), _ptr(cu), R, H,
+                                          dk, dv, gate, _ptr(S_out), _ptr(o))
+    if rc != 0:
+        raise ValueError(f"hypic_oracle_seam_window failed with code {rc}")
+    return S_out, o
 
 
 def compose(S_in, E_pool, T_pool, seg_ids, cu_segs):

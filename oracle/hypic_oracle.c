@@ -20,9 +20,11 @@
  *       first token is the LEFTMOST factor in the row convention):  T <- T diag(a_t) (I - beta_t k_t k_t^T)
  *   zero-start end-state: E = S after the segment's tokens, started from S = 0
  *   composition (Eq. 4, Eq. 6):  S <- S T_i + E_i, i in list order
+ *   seam-window step (Fig. 8): token steps from a given running state, with the read-out
+ *       of PAPER.md:86-90 (Eq. 2) after each step:  paper o_i = q_i^T S_i;  here o_t = S_t q_t
  *
  * There is no chunking, blocking, fusion or reordering here: one token at a time, one row at a time.
- * All pins are in tests/test_oracle_pins.py (P1..P10 of DESIGN.md); no function here is "parity unpinned".
+ * All pins are in tests/test_oracle_pins.py (P1..P10 and W1..W4 of DESIGN.md); no function here is "parity unpinned".
  *
  * Build: gcc -O3 -march=native -fopenmp -shared -fPIC hypic_oracle.c -o libhypic_oracle.so -lm
  */
@@ -155,6 +157,42 @@ int hypic_oracle_sequential(const double* S_in, const float* k, const float* v, 
     else
       memset(Su, 0, sizeof(double) * (size_t)dv * dk);
     scan_unit(k, v, g, beta, cu_tokens[r], cu_tokens[r + 1], h, H, dk, dv, gate, Su, NULL);
+  }
+  return 0;
+}
+
+/*
+ * hypic_oracle_seam_window: the seam-window step of PAPER.md:232-234 (section 4.3, Fig. 8): a few uncached tokens
+ * are run through a linear layer on the fly, from the running state in front of them, and their per-token outputs are
+ * emitted.  For each request r and head h: S = S_in[r,h] (NULL = zeros); for every token t of
+ * [cu_tokens[r], cu_tokens[r+1]): one token step (Eq. 2, as in hypic_oracle_sequential), then the read-out
+ * of PAPER.md:86-90 (Eq. 2, "o_i = q_i^T S_i") in the row convention:  o_t = S_t q_t  (a dv-vector; the state AFTER
+ * token t's update is read).  q:[Ttot,H,dk] float32, o:[Ttot,H,dv] doubles (rows of tokens outside every request are
+ * left untouched), S_out:[R,H,dv,dk] doubles.  Returns 0, or 1 on a bad argument.
+ */
+int hypic_oracle_seam_window(const double* S_in, const float* q, const float* k, const float* v, const float* g,
+                             const float* beta, const int32_t* cu_tokens, int R, int H, int dk, int dv, int gate,
+                             double* S_out, double* o) {
+  if (R < 0 || H <= 0 || dk <= 0 || dv <= 0 || !cu_tokens || !S_out || !o) return 1;
+  if (gate != HYPIC_ORACLE_GATE_SCALAR && gate != HYPIC_ORACLE_GATE_CHANNEL) return 1;
+  const long n_units = (long)R * H;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (long u = 0; u < n_units; ++u) {
+    const int r = (int)(u / H), h = (int)(u % H);
+    double* Su = S_out + (size_t)u * dv * dk;
+    if (S_in)
+      memcpy(Su, S_in + (size_t)u * dv * dk, sizeof(double) * (size_t)dv * dk);
+    else
+      memset(Su, 0, sizeof(double) * (size_t)dv * dk);
+    for (int t = cu_tokens[r]; t < cu_tokens[r + 1]; ++t) {
+      scan_unit(k, v, g, beta, t, t + 1, h, H, dk, dv, gate, Su, NULL); /* one token step */
+      const size_t th = (size_t)t * H + h;
+      for (int i = 0; i < dv; ++i) {
+        double acc = 0.0;
+        for (int c = 0; c < dk; ++c) acc += Su[(size_t)i * dk + c] * (double)q[th * dk + c];
+        o[th * dv + i] = acc;
+      }
+    }
   }
   return 0;
 }

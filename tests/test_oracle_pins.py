@@ -335,3 +335,83 @@ def test_heads_and_segments_are_independent_units():
             e1, t1 = oracle.segment_encode(k[sl, h:h + 1], v[sl, h:h + 1], g[sl, h:h + 1], beta[sl, h:h + 1],
                                            _cu([lens[s]]), GATE_CHANNEL)
             assert np.array_equal(e1[0, 0], E[s, h]) and np.array_equal(t1[0, 0], T[s, h])
+
+
+# ---------------------------------------------------------------------------------------------------------
+# W-pins: seam-window step (Fig. 8): token recurrence from a non-zero running state with the
+# per-token read-out o_i = q_i^T S_i (Eq. 2).
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gate", [GATE_SCALAR, GATE_CHANNEL])
+@pytest.mark.parametrize("w,dk,dv", [(1, 4, 4), (3, 4, 5), (8, 6, 3)])
+def test_W1_seam_bruteforce_paper_convention(gate, w, dk, dv):
+    """Explicit T_i, u_i matrices in the paper's column convention, S_0 = S_in^T, o_i = q_i^T S_i read AFTER the
+    update of token i (a read before the update, a transposed S or q on the wrong side all fail)."""
+    rng = np.random.default_rng(4100 + w + dk + 7 * gate)
+    k, v, g, beta = _rand_inputs(w, 1, dk, dv, gate, rng, g_lo=-0.5, normalise=False)
+    q = rng.standard_normal((w, 1, dk)).astype(np.float32)
+    S_in = rng.standard_normal((1, 1, dv, dk))
+    S_out, o = oracle.seam_window(S_in, q, k, v, g, beta, _cu([w]), gate)
+    for i in range(w):
+        S_p, _ = _paper_convention_bruteforce(k[:i + 1, 0].astype(np.float64), v[:i + 1, 0].astype(np.float64),
+                                              g[:i + 1, 0].astype(np.float64), beta[:i + 1, 0].astype(np.float64),
+                                              gate, S0_paper=S_in[0, 0].T)
+        o_p = q[i, 0].astype(np.float64)[None, :] @ S_p  # 1 x dv
+        np.testing.assert_allclose(o[i, 0], o_p[0], rtol=1e-12, atol=1e-13)
+    np.testing.assert_allclose(S_out[0, 0], S_p.T, rtol=1e-12, atol=1e-13)
+
+
+@pytest.mark.parametrize("gate", [GATE_SCALAR, GATE_CHANNEL])
+def test_W2_seam_via_composition_law(gate):
+    """the seam's own (T, S) inserted into Eq. 6.  For every prefix 1..t of the window,
+    o_t = (S_in T_{1..t} + E_{1..t}) q_t with (E, T) from segment_encode + compose (pinned by P1-P10), and the
+    state handed on equals hypic_oracle_sequential's."""
+    rng = np.random.default_rng(4200 + gate)
+    w, H, dk, dv = 8, 2, 16, 12
+    k, v, g, beta = _rand_inputs(w, H, dk, dv, gate, rng, g_lo=-0.3)
+    q = rng.standard_normal((w, H, dk)).astype(np.float32)
+    S_in = rng.standard_normal((1, H, dv, dk))
+    S_out, o = oracle.seam_window(S_in, q, k, v, g, beta, _cu([w]), gate)
+    for t in range(1, w + 1):
+        E, T = oracle.segment_encode(k[:t], v[:t], g[:t], beta[:t], _cu([t]), gate)
+        S_t = oracle.compose(S_in, E, T, np.array([0], dtype=np.int32), _cu([1]))
+        o_t = np.einsum("hic,hc->hi", S_t[0], q[t - 1].astype(np.float64))
+        np.testing.assert_allclose(o[t - 1], o_t, rtol=1e-11, atol=1e-12)
+    S_seq = oracle.sequential(S_in, k, v, g, beta, _cu([w]), gate)
+    np.testing.assert_allclose(S_out, S_seq, rtol=0, atol=0)
+
+
+@pytest.mark.parametrize("gate", [GATE_SCALAR, GATE_CHANNEL])
+def test_W3_seam_recall_closed_form(gate):
+    """Delta rule closed form: with beta_t ||k_t||^2 = 1 the write makes S_t k_t = v_t whatever S_{t-1} and the
+    gate were, so q_t = k_t reads back o_t = v_t exactly (a read-out taken before the write fails)."""
+    rng = np.random.default_rng(4300 + gate)
+    w, H, dk, dv = 8, 3, 8, 5
+    k, v, g, _ = _rand_inputs(w, H, dk, dv, gate, rng, g_lo=-1.0, normalise=False)
+    beta = (1.0 / np.sum(k.astype(np.float64) ** 2, axis=-1))
+    beta32 = beta.astype(np.float32)
+    S_in = 10.0 * rng.standard_normal((1, H, dv, dk))
+    _, o = oracle.seam_window(S_in, k, k, v, g, beta32, _cu([w]), gate)
+    # beta is rounded to float32, so beta ||k||^2 = 1 + O(2^-24): the residual is that relative error times |S k|
+    np.testing.assert_allclose(o, v.astype(np.float64), rtol=0, atol=2e-5)
+
+
+def test_W4_seam_requests_are_independent_and_empty_window_copies():
+    rng = np.random.default_rng(4400)
+    H, dk, dv = 2, 8, 8
+    lens = [3, 0, 8, 1]
+    ttot = sum(lens) + 2  # two trailing tokens belong to no request
+    k, v, g, beta = _rand_inputs(ttot, H, dk, dv, GATE_SCALAR, rng)
+    q = rng.standard_normal((ttot, H, dk)).astype(np.float32)
+    S_in = rng.standard_normal((len(lens), H, dv, dk))
+    cu = _cu(lens)
+    S_out, o = oracle.seam_window(S_in, q, k, v, g, beta, cu, GATE_SCALAR)
+    assert np.array_equal(S_out[1], S_in[1])  # empty window: state handed on unchanged
+    assert np.all(np.isnan(o[cu[-1]:])) and not np.any(np.isnan(o[:cu[-1]]))
+    for r, L in enumerate(lens):
+        sl = slice(int(cu[r]), int(cu[r + 1]))
+        S_r, o_r = oracle.seam_window(S_in[r:r + 1], q[sl], k[sl], v[sl], g[sl], beta[sl], _cu([L]), GATE_SCALAR)
+        assert np.array_equal(S_r[0], S_out[r]) and np.array_equal(o_r, o[sl])
+    # S_in = None is the zero state
+    S0, o0 = oracle.seam_window(None, q, k, v, g, beta, cu, GATE_SCALAR)
+    Sz, oz = oracle.seam_window(np.zeros_like(S_in), q, k, v, g, beta, cu, GATE_SCALAR)
+    assert np.array_equal(S0, Sz) and np.array_equal(o0[:cu[-1]], oz[:cu[-1]])
