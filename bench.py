@@ -337,6 +337,39 @@ def time_extra_cfg4(hb, device, peaks, iters=48):
             "kernel_family": "tensor" if fam == hb.HYPIC_IMPL_TENSOR else "simt"}
 
 
+def time_extra_seam(hb, device, peaks, reps=20, w=8):
+    """Seam-window step (hypic_seam_window): one seam of w = 8 tokens per request of cfg4's batch
+    (R = 128, H = 32, dk = dv = 128, bf16 q/k/v).  S_in + S_out are 537 MB per call (larger than L2), so the state is
+    read from and written to HBM every call; algorithmic bytes per (request, head): 2 * 64 KiB of state +
+    w * (3 * 256 B of q, k, v + 8 B of g, beta + 512 B of o)."""
+    si = wl.seam_cfg(w=w, device=device)
+    e = si.enc
+    R = si.S_in.shape[0]
+    S_out = torch.empty_like(si.S_in)
+    o = torch.empty((e.t_total, H, D), dtype=torch.float32, device=device)
+
+    def one():
+        hb.hypic_seam_window(si.S_in, si.q, e.k, e.v, e.g, e.beta, e.cu_seqlens, e.gate, S_out=S_out, o=o)
+
+    for _ in range(3):
+        one()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        one()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    unit_bytes = 2 * D * D * 4 + w * (3 * D * 2 + 8 + D * 4)
+    gbs = R * H * unit_bytes / (ms * 1e-3) / 1e9
+    return {"workload": f"seam window: R={R}, H=32, w={w}, bf16 q/k/v, S_in/S_out fp32 (537 MB: larger than L2)",
+            "ms": ms, "seam_tokens_per_s": R * w / (ms * 1e-3), "request_layer_ops_per_s": R / (ms * 1e-3),
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                         "frac": gbs / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"]},
+            "kernel_family": "simt"}
+
+
 def run_ours(args):
     from paper_2607_01299_b200 import binding as hb
 
@@ -459,6 +492,8 @@ def run_ours(args):
         extra["cfg4_compose"] = time_extra_cfg4(hb, device, peaks)
         torch.cuda.empty_cache()
         extra["cfg3_encode"] = time_extra_cfg3(hb, device, peaks)
+        torch.cuda.empty_cache()
+        extra["seam_window"] = time_extra_seam(hb, device, peaks)
         extra["cfg2_compose"] = {"avg_launch_ms": cmp_avg, "compose_ops_per_s": N_SEG * H / (cmp_avg * 1e-3),
                                  "hbm_gbs": N_SEG * H * COMPOSE_BYTES_PER_STEP / (cmp_avg * 1e-3) / 1e9}
 

@@ -135,6 +135,31 @@ int hypic_compose_f16(const float* S_in, const void* E_pool, const void* T_pool,
 int hypic_tuple_pack_f16(const float* src, void* dst, size_t count, void* stream);
 
 /*
+ * hypic_seam_window: the seam-window step of PAPER.md:232-234 (section 4.3, Fig. 8).  The first w tokens of an
+ * interior segment are left out of the cached tuple and, at reuse time, run through the linear layer on the fly from
+ * the running state in front of them, which both advances that state and emits every seam token's output for the layer
+ * above.  For every request r and head h:  S = S_in[r,h];  for each token t of [cu_tokens[r], cu_tokens[r+1]) in
+ * order: one token step of PAPER.md:84 Eq. 2 (the recurrence hypic_segment_encode accumulates; decay, then erase and
+ * write), then the read-out of PAPER.md:86-90 taken AFTER that step:  o[t,h,:] = S_t q_t  (the paper's o_i = q_i^T S_i
+ * in the row convention);  S_out[r,h] = S after the last token.  Composing the rest of the segment is hypic_compose
+ * on S_out.
+ *
+ *   q, k     [t_total, H, dk]   kv_dtype (bf16 or fp32)        v   [t_total, H, dv]  kv_dtype
+ *   g        [t_total, H] (HYPIC_GATE_SCALAR) or [t_total, H, dk] (HYPIC_GATE_CHANNEL) fp32 log-decay, beta [t_total, H] fp32
+ *   cu_tokens  int32 [R+1] on the DEVICE, non-decreasing, 0 <= cu_tokens[0], cu_tokens[R] <= t_total (trusted); windows of
+ *            any length are accepted (w = 8 is the paper's default); tokens outside every window are ignored
+ *   S_in     [R, H, dv, dk] fp32, or NULL (= zeros)            S_out  out [R, H, dv, dk] fp32, may alias S_in exactly
+ *   o        out [t_total, H, dv] fp32; rows of tokens outside every window are left untouched
+ *
+ * An empty window copies S_in to S_out.  fp32 arithmetic on the CUDA cores (the step moves 8 dk bytes of state per 6 w dk
+ * flops, so it is bound by HBM, not by arithmetic); there is no tensor-core variant and hypic_set_impl does not affect
+ * it.  Built envelope: dk in {64, 128}, dv in [1, 1024]; R, H <= 65535.
+ */
+int hypic_seam_window(const void* q, const void* k, const void* v, const float* g, const float* beta,
+                      const int32_t* cu_tokens, int32_t R, int32_t t_total, int32_t H, int32_t dk, int32_t dv,
+                      int kv_dtype, int gate, const float* S_in, float* S_out, float* o, void* stream);
+
+/*
  * hypic_encode_impl_for / hypic_compose_impl_for: which kernel family (HYPIC_IMPL_SIMT or HYPIC_IMPL_TENSOR)
  * a call with this shape would run under the current hypic_set_impl setting, or a negative hypic_status_t
  * (-HYPIC_ERR_UNSUPPORTED / -HYPIC_ERR_INVALID_ARG) if the call would be rejected.  Pure host arithmetic;

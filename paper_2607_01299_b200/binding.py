@@ -29,7 +29,7 @@ EXPORTS = (
     "hypic_set_impl", "hypic_get_impl", "hypic_segment_encode_workspace", "hypic_segment_encode", "hypic_compose",
     "hypic_status_string", "hypic_version", "hypic_last_launch_count", "hypic_encode_impl_for",
     "hypic_compose_impl_for", "hypic_debug_timeout_count", "hypic_envelope_violation_count", "hypic_compose_f16",
-    "hypic_tuple_pack_f16",
+    "hypic_tuple_pack_f16", "hypic_seam_window",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -68,6 +68,9 @@ def load_library() -> ctypes.CDLL:
     lib.hypic_compose_f16.restype = ctypes.c_int
     lib.hypic_tuple_pack_f16.argtypes = [vp, vp, sz, vp]
     lib.hypic_tuple_pack_f16.restype = ctypes.c_int
+    lib.hypic_seam_window.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, ctypes.c_int, ctypes.c_int, vp,
+                                      vp, vp, vp]
+    lib.hypic_seam_window.restype = ctypes.c_int
     lib.hypic_status_string.argtypes = [ctypes.c_int]
     lib.hypic_status_string.restype = ctypes.c_char_p
     lib.hypic_version.argtypes = []
@@ -282,3 +285,52 @@ def hypic_tuple_pack_f16(src: torch.Tensor, dst: Optional[torch.Tensor] = None,
     if rc != HYPIC_OK:
         raise HypicError(rc, "hypic_tuple_pack_f16")
     return dst
+
+
+def hypic_seam_window(S_in: Optional[torch.Tensor], q: torch.Tensor, k: torch.Tensor, v: torch.Tensor, g: torch.Tensor,
+                      beta: torch.Tensor, cu_tokens: torch.Tensor, gate: int = HYPIC_GATE_SCALAR, *,
+                      S_out: Optional[torch.Tensor] = None, o: Optional[torch.Tensor] = None,
+                      stream: Optional[torch.cuda.Stream] = None) -> Tuple[torch.Tensor, torch.Tensor]:
+    """Seam-window step: token recurrence over each request's window [cu_tokens[r], cu_tokens[r+1]) from S_in[r]
+    (None = 0) with per-token read-out o[t,h] = S_t q_t.  Returns (S_out:[R,H,dv,dk], o:[Ttot,H,dv]) fp32; rows of o
+    for tokens outside every window are left as they were (zeros when o is allocated here)."""
+    lib = load_library()
+    for name, t in (("q", q), ("k", k), ("v", v), ("g", g), ("beta", beta), ("cu_tokens", cu_tokens)):
+        if not t.is_cuda:
+            raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if k.dim() != 3 or v.dim() != 3 or k.shape[:2] != v.shape[:2] or k.dtype != v.dtype:
+        raise ValueError("k:[Ttot,H,dk] and v:[Ttot,H,dv] must agree in Ttot, H and dtype")
+    if q.shape != k.shape or q.dtype != k.dtype:
+        raise ValueError("q must have k's shape and dtype")
+    t_total, H, dk = (int(x) for x in k.shape)
+    dv = int(v.shape[2])
+    if k.dtype == torch.bfloat16:
+        kv_dtype = HYPIC_DT_BF16
+    elif k.dtype == torch.float32:
+        kv_dtype = HYPIC_DT_F32
+    else:
+        raise ValueError(f"q/k/v must be bf16 or fp32, got {k.dtype}")
+    want_g = (t_total, H) if gate == HYPIC_GATE_SCALAR else (t_total, H, dk)
+    if tuple(g.shape) != want_g or tuple(beta.shape) != (t_total, H):
+        raise ValueError(f"g must be {want_g} and beta {(t_total, H)}; got {tuple(g.shape)}, {tuple(beta.shape)}")
+    R = int(cu_tokens.numel()) - 1
+    if R < 0:
+        raise ValueError("cu_tokens must have R+1 >= 1 entries")
+    dev = k.device
+    if S_in is not None and tuple(S_in.shape) != (R, H, dv, dk):
+        raise ValueError("S_in must be [R,H,dv,dk]")
+    if S_out is None:
+        S_out = torch.empty((R, H, dv, dk), dtype=torch.float32, device=dev)
+    if o is None:
+        o = torch.zeros((t_total, H, dv), dtype=torch.float32, device=dev)
+    if tuple(S_out.shape) != (R, H, dv, dk) or tuple(o.shape) != (t_total, H, dv):
+        raise ValueError("S_out / o have the wrong shape")
+    with torch.cuda.device(dev):
+        rc = lib.hypic_seam_window(
+            _dev_ptr(q, "q"), _dev_ptr(k, "k"), _dev_ptr(v, "v"), _dev_ptr(g, "g", torch.float32),
+            _dev_ptr(beta, "beta", torch.float32), _dev_ptr(cu_tokens, "cu_tokens", torch.int32), R, t_total, H, dk,
+            dv, kv_dtype, int(gate), _dev_ptr(S_in, "S_in", torch.float32), _dev_ptr(S_out, "S_out", torch.float32),
+            _dev_ptr(o, "o", torch.float32), _stream_handle(stream))
+    if rc != HYPIC_OK:
+        raise HypicError(rc, "hypic_seam_window")
+    return S_out, o

@@ -55,9 +55,25 @@ struct ComposeF16Args {
   cudaStream_t stream;
 };
 
+struct SeamArgs {
+  const void* q;
+  const void* k;
+  const void* v;
+  const float* g;
+  const float* beta;
+  const int32_t* cu_tokens;
+  int32_t R, t_total, H, dk, dv;
+  int kv_dtype, gate;
+  const float* S_in;
+  float* S_out;
+  float* o;
+  cudaStream_t stream;
+};
+
 // Kernel families (each returns a hypic_status_t; UNSUPPORTED when the shape is outside its envelope).
 int encode_simt(const EncodeArgs& a);
 int compose_simt(const ComposeArgs& a);
+int seam_simt(const SeamArgs& a);
 bool encode_tensor_shape_ok(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate);
 inline bool encode_tensor_supported(const EncodeArgs& a) {
   return encode_tensor_shape_ok(a.H, a.dk, a.dv, a.kv_dtype, a.gate);

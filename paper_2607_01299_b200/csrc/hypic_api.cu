@@ -127,6 +127,25 @@ int hypic_tuple_pack_f16(const float* src, void* dst, size_t count, void* stream
   return pack_f16(src, dst, count, (cudaStream_t)stream);
 }
 
+int hypic_seam_window(const void* q, const void* k, const void* v, const float* g, const float* beta,
+                      const int32_t* cu_tokens, int32_t R, int32_t t_total, int32_t H, int32_t dk, int32_t dv,
+                      int kv_dtype, int gate, const float* S_in, float* S_out, float* o, void* stream) {
+  g_launch_count = 0;
+  if (R < 0 || t_total < 0 || H <= 0 || dk <= 0 || dv <= 0) return HYPIC_ERR_INVALID_ARG;
+  if (kv_dtype != HYPIC_DT_F32 && kv_dtype != HYPIC_DT_BF16) return HYPIC_ERR_INVALID_ARG;
+  if (gate != HYPIC_GATE_SCALAR && gate != HYPIC_GATE_CHANNEL) return HYPIC_ERR_INVALID_ARG;
+  if (!cu_tokens) return HYPIC_ERR_INVALID_ARG;
+  if (R > 0 && !S_out) return HYPIC_ERR_INVALID_ARG;
+  if (t_total > 0 && (!q || !k || !v || !g || !beta || !o)) return HYPIC_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(g) || !aligned16(beta) || !aligned16(S_in) ||
+      !aligned16(S_out) || !aligned16(o))
+    return HYPIC_ERR_INVALID_ARG;
+  if (dk != 64 && dk != 128) return HYPIC_ERR_UNSUPPORTED;
+  if (dv > 1024) return HYPIC_ERR_UNSUPPORTED;
+  SeamArgs a{q, k, v, g, beta, cu_tokens, R, t_total, H, dk, dv, kv_dtype, gate, S_in, S_out, o, (cudaStream_t)stream};
+  return seam_simt(a);
+}
+
 int hypic_encode_impl_for(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate) {
   const int vs = validate_encode_shape(0, 0, H, dk, dv, kv_dtype, gate);
   if (vs != HYPIC_OK) return -vs;

@@ -210,3 +210,31 @@ def near_unit_pool_inputs(P: int, H: int, device: str = "cpu", d: int = 128, kv_
     lens = [int(x) for x in torch.randint(16, 65, (P,), generator=gen)]
     return make_encode_inputs(lens, H, d, d, kv_dtype=kv_dtype, g_lo=-0.01, beta_kind="sigmoid",
                               seed=seed_for(4, 78) + seed_off, device=device)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Seam-window step: R windows of w tokens each (w = 8 default),
+# one per request, with queries and a non-zero running state in front of every window.
+# ---------------------------------------------------------------------------------------------------------
+@dataclasses.dataclass
+class SeamInputs:
+    enc: EncodeInputs        # k, v, g, beta of the window tokens; enc.cu_seqlens = cu_tokens of the R windows
+    q: torch.Tensor          # [Ttot, H, dk], L2-normalised like k (the layers normalise q and k alike), kv dtype
+    S_in: torch.Tensor       # [R, H, dv, dk] fp32 ~ N(0, 1): stands in for the composed state in front of the seam
+
+
+def make_seam_inputs(win_lens: Sequence[int], H: int, dk: int, dv: int, *, kv_dtype: torch.dtype,
+                     gate: int = GATE_SCALAR, g_lo: float = -0.05, seed: int = BASE_SEED,
+                     device: str = "cpu") -> SeamInputs:
+    enc = make_encode_inputs(win_lens, H, dk, dv, kv_dtype=kv_dtype, gate=gate, g_lo=g_lo, seed=seed, device=device)
+    gen = torch.Generator(device=device)
+    gen.manual_seed(int(seed) + 500_000)
+    q = torch.randn((enc.t_total, H, dk), generator=gen, device=device, dtype=torch.float32)
+    q = (q / q.norm(dim=-1, keepdim=True).clamp_min(1e-20)).to(kv_dtype)
+    S_in = torch.randn((len(win_lens), H, dv, dk), generator=gen, device=device, dtype=torch.float32)
+    return SeamInputs(enc=enc, q=q, S_in=S_in)
+
+
+def seam_cfg(R: int = 128, H: int = 32, w: int = 8, device: str = "cpu", layer: int = 0) -> SeamInputs:
+    """One seam per request of cfg4's batch (R = 128 requests, H = 32 heads, dk = dv = 128, bf16 q/k/v, w = 8)."""
+    return make_seam_inputs([w] * R, H, 128, 128, kv_dtype=torch.bfloat16, seed=seed_for(5, layer), device=device)

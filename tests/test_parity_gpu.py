@@ -380,3 +380,122 @@ def test_cfg4_compose_f16_sampled_requests():
     ref = oracle_compose_units(req.S_in, Eh.float(), Th.float(), req.seg_ids, req.cu_segs, units)
     ri, hi = torch.tensor([u[0] for u in units]), torch.tensor([u[1] for u in units])
     check_E(S[ri, hi][:, None], ref, TOL_F32, "S_out")
+
+
+# ------------------------------------------------------------------------------------------------ seam window
+def _oracle_seam(si):
+    c = si.enc.cpu()
+    return oracle.seam_window(si.S_in.cpu().numpy(), si.q.float().cpu().numpy(), c.k, c.v, c.g, c.beta, c.cu_seqlens,
+                              gate=c.gate)
+
+
+def _typical_readout(S_in, q, k, v, g, beta, cu, gate):
+    """||S_t||_F ||q_t||_2 / sqrt(dk) per (token, head): the size a read-out of the state S_t has for a query in general
+    position.  S_t comes from the oracle, one token at a time.  numpy inputs; S_in may be None."""
+    ttot, H, dk = q.shape
+    out = np.zeros((ttot, H))
+    for r in range(len(cu) - 1):
+        S = None if S_in is None else S_in[r:r + 1]
+        for t in range(int(cu[r]), int(cu[r + 1])):
+            sl = slice(t, t + 1)
+            S, _ = oracle.seam_window(S, q[sl], k[sl], v[sl], g[sl], beta[sl], np.array([0, 1], dtype=np.int32), gate=gate)
+            out[t] = np.sqrt((S[0] ** 2).sum(axis=(-1, -2))) * np.sqrt((q[t].astype(np.float64) ** 2).sum(-1)) / np.sqrt(dk)
+    return out
+
+
+def _check_o(o_gpu, o_ref, cu, tol, typical=None):
+    """DESIGN.md reading W2: per (token, head), ||o - o_ref||_2 <= tol * max(||o_ref||_2, ||S_t||_F ||q_t||_2 / sqrt(dk)).
+    The first term is the plain relative error; the second keeps the bound meaningful where q_t is nearly orthogonal to
+    the state (o_t = S_t q_t cancels and no fp32 evaluation can be relatively accurate).  Rows outside every window must
+    be left untouched."""
+    o_gpu = o_gpu.cpu().numpy().astype(np.float64)
+    inside = np.zeros(o_ref.shape[0], dtype=bool)
+    for r in range(len(cu) - 1):
+        inside[cu[r]:cu[r + 1]] = True
+    assert np.isfinite(o_gpu).all()
+    num = np.sqrt(((o_gpu[inside] - o_ref[inside]) ** 2).sum(-1))
+    den = np.sqrt((o_ref[inside] ** 2).sum(-1))
+    if typical is not None:
+        den = np.maximum(den, typical[inside])
+    worst = float((num / np.maximum(den, 1e-300)).max()) if inside.any() else 0.0
+    assert worst <= tol, f"o: max per-token rel. L2 error {worst:.3e} > {tol:.1e}"
+    assert np.all(o_gpu[~inside] == 0.0), "o rows outside every window must be left untouched"
+    return worst
+
+
+@pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
+@pytest.mark.parametrize("kv,d,dv", [(torch.bfloat16, 128, 128), (torch.float32, 128, 128), (torch.float32, 64, 64),
+                                     (torch.bfloat16, 128, 72), (torch.float32, 64, 33)])
+def test_seam_window_vs_oracle(gate, kv, d, dv):
+    """hypic_seam_window: windows of w = 8 (the default), 0, 1, 7, 9 (a ragged second tile), 16 and
+    37 tokens, from a non-zero running state, both gates, dv off the 32-row CTA tile."""
+    lens = [8, 0, 1, 7, 9, 16, 37, 8]
+    si = wl.make_seam_inputs(lens, 3, d, dv, kv_dtype=kv, gate=gate, g_lo=-0.3, seed=wl.seed_for(5, 1), device="cuda")
+    S_ref, o_ref = _oracle_seam(si)
+    e = si.enc
+    host = [t.float().cpu().numpy() for t in (si.q, e.k, e.v, e.g, e.beta)]
+    cu_h = e.cu_seqlens.cpu().numpy()
+    S, o = hb.hypic_seam_window(si.S_in, si.q, e.k, e.v, e.g, e.beta, e.cu_seqlens, e.gate)
+    torch.cuda.synchronize()
+    assert hb.hypic_last_launch_count() == 1
+    check_E(S, S_ref, TOL_F32, "S_out")
+    _check_o(o, o_ref, cu_h, TOL_F32, _typical_readout(si.S_in.cpu().numpy(), *host, cu_h, e.gate))
+    assert torch.equal(S[1], si.S_in[1])  # empty window hands the state on unchanged
+    # NULL S_in = zero state; in-place S; windows that skip tokens (cu_tokens[0] > 0, cu_tokens[R] < t_total)
+    S0, o0 = hb.hypic_seam_window(None, si.q, e.k, e.v, e.g, e.beta, e.cu_seqlens, e.gate)
+    S0_ref, o0_ref = oracle.seam_window(None, *host, cu_h, gate=e.gate)
+    check_E(S0, S0_ref, TOL_F32, "S_out (NULL S_in)")
+    _check_o(o0, o0_ref, cu_h, TOL_F32, _typical_readout(None, *host, cu_h, e.gate))
+    S2 = si.S_in.clone()
+    hb.hypic_seam_window(S2, si.q, e.k, e.v, e.g, e.beta, e.cu_seqlens, e.gate, S_out=S2)
+    assert torch.equal(S2, S)
+    cu_in = torch.tensor([3, 11, 11, 30], dtype=torch.int32, device="cuda")
+    S3, o3 = hb.hypic_seam_window(si.S_in[:3].contiguous(), si.q, e.k, e.v, e.g, e.beta, cu_in, e.gate)
+    S3_ref, o3_ref = oracle.seam_window(si.S_in[:3].cpu().numpy(), *host, cu_in.cpu().numpy(), gate=e.gate)
+    check_E(S3, S3_ref, TOL_F32, "S_out (inner windows)")
+    _check_o(o3, o3_ref, cu_in.cpu().numpy(), TOL_F32,
+             _typical_readout(si.S_in[:3].cpu().numpy(), *host, cu_in.cpu().numpy(), e.gate))
+
+
+def test_seam_then_compose_equals_sequential_over_the_whole_segment():
+    """PAPER.md:234 end to end: a segment whose first w tokens are left out of the cached tuple.  Seam step from the
+    running state, then hypic_compose with the tuple of the remaining tokens, equals the token recurrence over the whole
+    segment (oracle.sequential), and the seam outputs equal the recurrence's read-outs."""
+    w, L, H, d = 8, 200, 2, 128
+    full = wl.make_seam_inputs([L, L], H, d, d, kv_dtype=torch.float32, seed=wl.seed_for(5, 2), device="cuda")
+    e = full.enc
+    cu_seam = torch.tensor([0, w], dtype=torch.int32, device="cuda")
+    # request 0 only: seam = tokens [0, w), cached rest = tokens [w, L)
+    S_in = full.S_in[:1].contiguous()
+    S_mid, o = hb.hypic_seam_window(S_in, full.q, e.k, e.v, e.g, e.beta, cu_seam, e.gate)
+    cu_rest = torch.tensor([0, w, L], dtype=torch.int32, device="cuda")  # segment 0 = the seam (unused), 1 = the rest
+    with impl_family(hb.HYPIC_IMPL_SIMT):
+        E, T = hb.hypic_segment_encode(e.k[:L].contiguous(), e.v[:L].contiguous(), e.g[:L].contiguous(),
+                                       e.beta[:L].contiguous(), cu_rest, e.gate)
+        S = hb.hypic_compose(S_mid, E, T, torch.tensor([1], dtype=torch.int32, device="cuda"),
+                             torch.tensor([0, 1], dtype=torch.int32, device="cuda"))
+    torch.cuda.synchronize()
+    c = e.cpu()
+    S_ref = oracle.sequential(S_in.cpu().numpy(), c.k[:L], c.v[:L], c.g[:L], c.beta[:L],
+                              np.array([0, L], dtype=np.int32), gate=c.gate)
+    check_E(S, S_ref, TOL_F32, "S after seam + compose")
+    _, o_ref = oracle.seam_window(S_in.cpu().numpy(), full.q.float().cpu().numpy(), c.k, c.v, c.g, c.beta,
+                                  np.array([0, w], dtype=np.int32), gate=c.gate)
+    _check_o(o, o_ref, np.array([0, w]), TOL_F32)
+
+
+def test_seam_window_cfg_full_size_sampled_units():
+    """The launch bench.py times (128 windows of 8 tokens, 32 heads, bf16): sampled (request, head) units."""
+    si = wl.seam_cfg(device="cuda")
+    e = si.enc
+    S, o = hb.hypic_seam_window(si.S_in, si.q, e.k, e.v, e.g, e.beta, e.cu_seqlens, e.gate)
+    torch.cuda.synchronize()
+    assert torch.isfinite(S).all() and torch.isfinite(o).all()
+    cu = e.cu_seqlens.cpu().numpy()
+    for r, h in _sample_units(128, 32, 8, 9):
+        sl = slice(int(cu[r]), int(cu[r + 1]))
+        f = lambda t: t[sl, h:h + 1].float().cpu().numpy()
+        S_ref, o_ref = oracle.seam_window(si.S_in[r:r + 1, h:h + 1].cpu().numpy(), f(si.q), f(e.k), f(e.v), f(e.g),
+                                          f(e.beta), np.array([0, sl.stop - sl.start], dtype=np.int32), gate=e.gate)
+        check_E(S[r:r + 1, h:h + 1], S_ref, TOL_F32, "S_out")
+        _check_o(o[sl, h:h + 1], o_ref, np.array([0, sl.stop - sl.start]), TOL_F32)
