@@ -3,20 +3,26 @@
 // A handful of uncached tokens (w = 8 by default) are pushed through a linear-attention layer from
 // the running state in front of them: per token one step of PAPER.md:84 Eq. 2 and the read-out of PAPER.md:86-90,
 //     x <- x diag(a_t);   x <- x + beta_t (v_t[i] - x.k_t) k_t^T;   o_t[i] = x.q_t          (row i of S, row convention)
-// With w = 8 the state is read and written once (8 dk bytes per row) for 4 w dk = 32 dk fp32 operations per row, which
-// on B200 puts the HBM time, the FMA time and the shared-memory/shuffle (MIO) time within a factor 1.5 of each other,
-// so the layout is chosen to keep all three low (measured unit costs: LDS.128 = 4 cycles per warp whatever the address
-// pattern repeats, SHFL = 1 cycle per warp):
+// With w = 8 the state is read and written once (8 dk bytes per row) for about 3 w dk = 24 dk fp32 multiply-adds per
+// row, which on B200 puts the HBM time (83 us for the bench batch), the FMA-pipe time (~45 us) and the shared-memory /
+// shuffle (MIO) time (~50 us) within a factor two of each other, so the layout keeps all three low and overlaps them
+// (measured unit costs: LDS.128 = 4 cycles per warp whether or not quarter-warps repeat an address, SHFL = 1 cycle):
 //   * a thread owns a 4-row x (dk/8)-column block of S: 8 adjacent lanes share 4 rows, lane l holding the float4s
 //     l, l+8, .. of each.  Every warp load / store instruction covers 4 rows x 128 contiguous bytes (whole lines), and
 //     a token's k_t / q_t slices are fetched from shared memory once per 4 rows;
 //   * the 4 row sums x.k_t of a lane group are reduced by a 4-shuffle reduce-scatter (each lane ends with one row's
 //     sum), the write coefficient beta (v - x.k) is formed once per row and gathered back with 4 indexed shuffles; the
 //     read-outs x.q_t need only the reduce-scatter and sit off the recurrence's dependency chain;
-//   * k, q, a, beta, v of a tile of 8 tokens are staged in shared memory (double-buffered, so longer windows stream)
-//     and o is written back through shared memory as whole rows.
-// One CTA = 128 threads = 64 rows of one (request, head) unit; grid = ceil(dv / 64) x H x R.
+//   * the arithmetic is packed fp32 (FFMA2 / FMUL2: two columns per instruction, half the issue slots); with a scalar
+//     gate a tile of 8 tokens runs on y = x / gamma_t, which removes the per-token decay multiply (see FOLD below);
+//   * persistent CTAs (3-4 per SM) walk the (request, head, 64-row block) items: the next item's rows of S_in are
+//     prefetched into shared memory with cp.async while the current item computes (each thread refills only the slots
+//     it reads itself, so no barrier guards them), the next tile's k, q, v, g, beta are loaded into registers one tile
+//     ahead and converted / stored to shared memory when their turn comes, and o leaves through shared memory as
+//     whole rows.
+// One CTA = 128 threads; one item = 64 rows of one (request, head) unit.
 #include <algorithm>
+#include <type_traits>
 
 #include "common.cuh"
 
@@ -33,25 +39,6 @@ template <bool BF16>
 __device__ __forceinline__ float seam_load(const void* p, size_t idx) {
   if (BF16) return __bfloat162float(reinterpret_cast<const __nv_bfloat16*>(p)[idx]);
   return reinterpret_cast<const float*>(p)[idx];
-}
-
-// 8 consecutive elements starting at element index idx (a multiple of 8) -> fp32
-template <bool BF16>
-__device__ __forceinline__ void seam_load8(const void* p, size_t idx, float (&out)[8]) {
-  if (BF16) {
-    const uint4 u = __ldg(reinterpret_cast<const uint4*>(reinterpret_cast<const __nv_bfloat16*>(p) + idx));
-    const uint32_t w[4] = {u.x, u.y, u.z, u.w};
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      out[2 * i] = __uint_as_float(w[i] << 16);
-      out[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
-    }
-  } else {
-    const float4* f = reinterpret_cast<const float4*>(reinterpret_cast<const float*>(p) + idx);
-    const float4 a = __ldg(f), b = __ldg(f + 1);
-    out[0] = a.x, out[1] = a.y, out[2] = a.z, out[3] = a.w;
-    out[4] = b.x, out[5] = b.y, out[6] = b.z, out[7] = b.w;
-  }
 }
 
 // Reduce-scatter of 4 per-lane values over a group of 8 lanes (bits b0 b1 b2 of the lane): returns the full sum of
@@ -81,18 +68,17 @@ template <bool BF16, bool CHANNEL>
 struct SeamRaw {
   uint4 k[BF16 ? 1 : 2], q[BF16 ? 1 : 2];
   float4 g[CHANNEL ? 2 : 1];
-  float v[kSeamTT * kSeamRows / kSeamThreads];
+  uint32_t v[kSeamTT * kSeamRows / kSeamThreads];  // bf16 bits or fp32 bits
   float b, gs;
 };
 
 template <int DK, bool BF16, bool CHANNEL>
-__global__ void __launch_bounds__(kSeamThreads, 3)
+__global__ void __launch_bounds__(kSeamThreads, CHANNEL ? 3 : 4)
     seam_simt_kernel(const void* __restrict__ q, const void* __restrict__ k, const void* __restrict__ v,
                      const float* __restrict__ g, const float* __restrict__ beta, const int32_t* __restrict__ cu_tokens,
                      int H, int dv, int n_blk, int n_items, const float* S_in, float* S_out, float* __restrict__ o) {
   constexpr int AW = CHANNEL ? DK : 1;
   constexpr int NJ = DK / 32;                   // float4s of a row owned by one lane
-  constexpr int NS = kSeamRT * NJ;              // float4s of S owned by one thread
   constexpr int NV = kSeamTT * kSeamRows / kSeamThreads;
   constexpr int EPT = 8;                        // k / q channels per thread and staged tile
   static_assert(kSeamTT * DK / EPT <= kSeamThreads, "one staging pass");
@@ -103,6 +89,8 @@ __global__ void __launch_bounds__(kSeamThreads, 3)
   __shared__ __align__(16) float sa[kSeamTT][AW];
   __shared__ float sv[kSeamTT][kSeamRows];
   __shared__ float sb[kSeamTT];
+  __shared__ float sgam[kSeamTT], sgi[kSeamTT];  // scalar gate: gamma_t since the tile's first token, and 1 / gamma_t
+  __shared__ int s_fold;
   __shared__ float so[kSeamTT][kSeamRows];
 
   const int tid = threadIdx.x;
@@ -162,7 +150,11 @@ __global__ void __launch_bounds__(kSeamThreads, 3)
       const int idx = tid + n * kSeamThreads;
       const int tok = idx / kSeamRows, j = idx % kSeamRows;
       const int t = tbase + tok, row = blk * kSeamRows + j;
-      raw.v[n] = (t < t_end && row < dv) ? seam_load<BF16>(v, ((size_t)t * H + h) * dv + row) : 0.f;
+      raw.v[n] = 0u;
+      if (t < t_end && row < dv) {
+        const size_t e = ((size_t)t * H + h) * dv + row;
+        raw.v[n] = BF16 ? (uint32_t) reinterpret_cast<const uint16_t*>(v)[e] : reinterpret_cast<const uint32_t*>(v)[e];
+      }
     }
     raw.b = 0.f, raw.gs = 0.f;
     if (tid < kSeamTT && tbase + tid < t_end) {
@@ -208,11 +200,23 @@ __global__ void __launch_bounds__(kSeamThreads, 3)
 #pragma unroll
     for (int n = 0; n < NV; ++n) {
       const int idx = tid + n * kSeamThreads;
-      sv[idx / kSeamRows][idx % kSeamRows] = raw.v[n];
+      sv[idx / kSeamRows][idx % kSeamRows] = __uint_as_float(BF16 ? raw.v[n] << 16 : raw.v[n]);
     }
     if (tid < kSeamTT) {
       sb[tid] = raw.b;
-      if (!CHANNEL) sa[tid][0] = expf(raw.gs);
+      if (!CHANNEL) {
+        sa[tid][0] = expf(raw.gs);
+        float G = raw.gs;  // inclusive prefix sum of the log-decay over the tile's tokens (lanes 0..7 of warp 0)
+#pragma unroll
+        for (int sft = 1; sft < kSeamTT; sft *= 2) {
+          const float up = __shfl_up_sync((1u << kSeamTT) - 1u, G, sft);
+          if (tid >= sft) G += up;
+        }
+        sgam[tid] = expf(G);
+        sgi[tid] = expf(-G);
+        const int ok = __all_sync((1u << kSeamTT) - 1u, fabsf(G) <= 40.f);  // false for NaN as well
+        if (tid == 0) s_fold = ok;
+      }
     }
   };
 
@@ -255,78 +259,99 @@ __global__ void __launch_bounds__(kSeamThreads, 3)
       else if (next < n_items)
         load_raw(raw, next, 0, nt_begin, nt_end);
       const int n_tok = min(kSeamTT, L - tile * kSeamTT);
-#pragma unroll 1
-      for (int tok = 0; tok < n_tok; ++tok) {
-        const float b = sb[tok];
-        const float w = sv[tok][rloc0 + rho];
-        const float4* k4 = reinterpret_cast<const float4*>(&sk[tok][0]);
-        const float4* q4 = reinterpret_cast<const float4*>(&sq[tok][0]);
-        float4 kk[NJ], qq[NJ];
+      // FOLD (scalar gate only): the tile is run on y = x / gamma_t, gamma_t the decay accumulated since the tile's
+      // first token, so the per-token decay of the state (one multiply per element) disappears:
+      //     y += beta (v / gamma_t - y.k) k,   o_t = gamma_t (y.q),   x = gamma_8 y at the end of the tile.
+      // Taken only while gamma_8 >= e^-40 (store_raw decides per tile); otherwise the plain form below runs.
+      auto run_tokens = [&](auto fold_tag) {
+        constexpr bool FOLD = decltype(fold_tag)::value;
+#pragma unroll 2
+        for (int tok = 0; tok < n_tok; ++tok) {
+          const float b = sb[tok];
+          const float w = sv[tok][rloc0 + rho];
+          const float4* k4 = reinterpret_cast<const float4*>(&sk[tok][0]);
+          const float4* q4 = reinterpret_cast<const float4*>(&sq[tok][0]);
+          float4 kk[NJ], qq[NJ];
 #pragma unroll
-        for (int j = 0; j < NJ; ++j) kk[j] = k4[l + kSeamLanes * j];
+          for (int j = 0; j < NJ; ++j) kk[j] = k4[l + kSeamLanes * j];
 #pragma unroll
-        for (int j = 0; j < NJ; ++j) qq[j] = q4[l + kSeamLanes * j];
-        float a = 1.f;
-        if (CHANNEL) {
-          const float4* a4 = reinterpret_cast<const float4*>(&sa[tok][0]);
+          for (int j = 0; j < NJ; ++j) qq[j] = q4[l + kSeamLanes * j];
+          float a = 1.f;
+          if (CHANNEL) {
+            const float4* a4 = reinterpret_cast<const float4*>(&sa[tok][0]);
 #pragma unroll
-          for (int j = 0; j < NJ; ++j) {
-            const float4 aa = a4[l + kSeamLanes * j];
+            for (int j = 0; j < NJ; ++j) {
+              const float4 aa = a4[l + kSeamLanes * j];
 #pragma unroll
-            for (int i = 0; i < kSeamRT; ++i) {
-              x[i][j].x *= aa.x;
-              x[i][j].y *= aa.y;
-              x[i][j].z *= aa.z;
-              x[i][j].w *= aa.w;
+              for (int i = 0; i < kSeamRT; ++i) {
+                const float2 x01 = __fmul2_rn(make_float2(x[i][j].x, x[i][j].y), make_float2(aa.x, aa.y));
+                const float2 x23 = __fmul2_rn(make_float2(x[i][j].z, x[i][j].w), make_float2(aa.z, aa.w));
+                x[i][j] = make_float4(x01.x, x01.y, x23.x, x23.y);
+              }
             }
+          } else if (!FOLD) {
+            a = sa[tok][0];
           }
-        } else {
-          a = sa[tok][0];
-        }
-        float d[kSeamRT];
+          // packed fp32 (FFMA2): two columns per instruction, which halves the issue slots of the arithmetic
+          float d[kSeamRT];
 #pragma unroll
-        for (int i = 0; i < kSeamRT; ++i) {
-          float d0 = 0.f, d1 = 0.f;
+          for (int i = 0; i < kSeamRT; ++i) {
+            float2 d01 = make_float2(0.f, 0.f), d23 = make_float2(0.f, 0.f);
 #pragma unroll
-          for (int j = 0; j < NJ; ++j) {
-            d0 = fmaf(x[i][j].x, kk[j].x, d0);
-            d1 = fmaf(x[i][j].y, kk[j].y, d1);
-            d0 = fmaf(x[i][j].z, kk[j].z, d0);
-            d1 = fmaf(x[i][j].w, kk[j].w, d1);
-          }
-          d[i] = d0 + d1;
-        }
-        // decay first, then read the decayed state along k_t: (a x).k = a (x.k)  (a = 1 on the per-channel path,
-        // where the state was decayed above)
-        const float coef_own = b * (w - a * group8_reduce_scatter4(d, b0, b1));
-        float p[kSeamRT];
-#pragma unroll
-        for (int i = 0; i < kSeamRT; ++i) {
-          const float coef = __shfl_sync(0xffffffffu, coef_own, (i >> 1) + 2 * (i & 1), kSeamLanes);
-          float p0 = 0.f, p1 = 0.f;  // this lane's share of o_t[row] = S_t[row,:] . q_t, read AFTER token t's write
-#pragma unroll
-          for (int j = 0; j < NJ; ++j) {
-            if (CHANNEL) {
-              x[i][j].x = fmaf(coef, kk[j].x, x[i][j].x);
-              x[i][j].y = fmaf(coef, kk[j].y, x[i][j].y);
-              x[i][j].z = fmaf(coef, kk[j].z, x[i][j].z);
-              x[i][j].w = fmaf(coef, kk[j].w, x[i][j].w);
-            } else {
-              x[i][j].x = fmaf(coef, kk[j].x, a * x[i][j].x);
-              x[i][j].y = fmaf(coef, kk[j].y, a * x[i][j].y);
-              x[i][j].z = fmaf(coef, kk[j].z, a * x[i][j].z);
-              x[i][j].w = fmaf(coef, kk[j].w, a * x[i][j].w);
+            for (int j = 0; j < NJ; ++j) {
+              d01 = __ffma2_rn(make_float2(x[i][j].x, x[i][j].y), make_float2(kk[j].x, kk[j].y), d01);
+              d23 = __ffma2_rn(make_float2(x[i][j].z, x[i][j].w), make_float2(kk[j].z, kk[j].w), d23);
             }
-            p0 = fmaf(x[i][j].x, qq[j].x, p0);
-            p1 = fmaf(x[i][j].y, qq[j].y, p1);
-            p0 = fmaf(x[i][j].z, qq[j].z, p0);
-            p1 = fmaf(x[i][j].w, qq[j].w, p1);
+            d[i] = (d01.x + d01.y) + (d23.x + d23.y);
           }
-          p[i] = p0 + p1;
+          // decay first, then read the decayed state along k_t: (a x).k = a (x.k)  (a = 1 on the per-channel path,
+          // where the state was decayed above, and on the folded path, where v is divided by gamma_t instead)
+          const float dsum = group8_reduce_scatter4(d, b0, b1);
+          const float coef_own = FOLD ? b * (w * sgi[tok] - dsum) : b * (w - a * dsum);
+          const float2 a2 = make_float2(a, a);
+          float p[kSeamRT];
+#pragma unroll
+          for (int i = 0; i < kSeamRT; ++i) {
+            const float coef = __shfl_sync(0xffffffffu, coef_own, (i >> 1) + 2 * (i & 1), kSeamLanes);
+            const float2 c2 = make_float2(coef, coef);
+            // this lane's share of o_t[row] = S_t[row,:] . q_t, read AFTER token t's write
+            float2 p01 = make_float2(0.f, 0.f), p23 = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) {
+              float2 x01 = make_float2(x[i][j].x, x[i][j].y), x23 = make_float2(x[i][j].z, x[i][j].w);
+              if (!CHANNEL && !FOLD) {
+                x01 = __fmul2_rn(a2, x01);
+                x23 = __fmul2_rn(a2, x23);
+              }
+              x01 = __ffma2_rn(c2, make_float2(kk[j].x, kk[j].y), x01);
+              x23 = __ffma2_rn(c2, make_float2(kk[j].z, kk[j].w), x23);
+              p01 = __ffma2_rn(x01, make_float2(qq[j].x, qq[j].y), p01);
+              p23 = __ffma2_rn(x23, make_float2(qq[j].z, qq[j].w), p23);
+              x[i][j] = make_float4(x01.x, x01.y, x23.x, x23.y);
+            }
+            p[i] = (p01.x + p01.y) + (p23.x + p23.y);
+          }
+          float ot = group8_reduce_scatter4(p, b0, b1);
+          if (FOLD) ot *= sgam[tok];
+          if (l < 4) so[tok][rloc0 + rho] = ot;
         }
-        const float ot = group8_reduce_scatter4(p, b0, b1);
-        if (l < 4) so[tok][rloc0 + rho] = ot;
-      }
+        if (FOLD) {
+          const float gt = sgam[n_tok - 1];
+          const float2 g2 = make_float2(gt, gt);
+#pragma unroll
+          for (int i = 0; i < kSeamRT; ++i)
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) {
+              const float2 x01 = __fmul2_rn(g2, make_float2(x[i][j].x, x[i][j].y));
+              const float2 x23 = __fmul2_rn(g2, make_float2(x[i][j].z, x[i][j].w));
+              x[i][j] = make_float4(x01.x, x01.y, x23.x, x23.y);
+            }
+        }
+      };
+      if (!CHANNEL && s_fold)
+        run_tokens(std::true_type{});
+      else
+        run_tokens(std::false_type{});
       __syncthreads();
 #pragma unroll
       for (int n = 0; n < NV; ++n) {
@@ -365,7 +390,7 @@ int seam_launch(const SeamArgs& a) {
     HYPIC_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kDyn));
     attr_set = true;
   }
-  const int grid = (int)std::min<long long>(n_items, 3LL * di.sm_count);
+  const int grid = (int)std::min<long long>(n_items, (CHANNEL ? 3LL : 4LL) * di.sm_count);
   kern<<<grid, kSeamThreads, kDyn, a.stream>>>(a.q, a.k, a.v, a.g, a.beta, a.cu_tokens, a.H, a.dv, n_blk, (int)n_items,
                                                a.S_in, a.S_out, a.o);
   note_launch();

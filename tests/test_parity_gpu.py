@@ -457,6 +457,24 @@ def test_seam_window_vs_oracle(gate, kv, d, dv):
              _typical_readout(si.S_in[:3].cpu().numpy(), *host, cu_in.cpu().numpy(), e.gate))
 
 
+@pytest.mark.parametrize("g_lo", [-12.0, -40.0])
+def test_seam_window_strong_decay(g_lo):
+    """Scalar gate with a log-decay far below the benchmark's: some (g_lo = -12) or all (g_lo = -40) staged tiles
+    fall outside the range in which the kernel runs its decay-folded form, so both forms and the switch between them
+    are checked; the state in front of the window is forgotten almost completely."""
+    lens = [8, 24, 5, 64]
+    si = wl.make_seam_inputs(lens, 2, 128, 128, kv_dtype=torch.float32, g_lo=g_lo, seed=wl.seed_for(5, 3),
+                             device="cuda")
+    e = si.enc
+    S_ref, o_ref = _oracle_seam(si)
+    host = [t.float().cpu().numpy() for t in (si.q, e.k, e.v, e.g, e.beta)]
+    cu_h = e.cu_seqlens.cpu().numpy()
+    S, o = hb.hypic_seam_window(si.S_in, si.q, e.k, e.v, e.g, e.beta, e.cu_seqlens, e.gate)
+    torch.cuda.synchronize()
+    check_E(S, S_ref, TOL_F32, "S_out")
+    _check_o(o, o_ref, cu_h, TOL_F32, _typical_readout(si.S_in.cpu().numpy(), *host, cu_h, e.gate))
+
+
 def test_seam_then_compose_equals_sequential_over_the_whole_segment():
     """PAPER.md:234 end to end: a segment whose first w tokens are left out of the cached tuple.  Seam step from the
     running state, then hypic_compose with the tuple of the remaining tokens, equals the token recurrence over the whole
