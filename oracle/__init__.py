@@ -54,6 +54,12 @@ def _load():
         lib.hypic_oracle_sequential.restype = i32
         lib.hypic_oracle_seam_window.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]
         lib.hypic_oracle_seam_window.restype = i32
+        lib.hypic_oracle_diag_encode.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]
+        lib.hypic_oracle_diag_encode.restype = i32
+        lib.hypic_oracle_diag_sequential.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp]
+        lib.hypic_oracle_diag_sequential.restype = i32
+        lib.hypic_oracle_diag_compose.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp]
+        lib.hypic_oracle_diag_compose.restype = i32
         lib.hypic_oracle_compose.argtypes = [vp, vp, vp, i32, vp, vp, i32, i32, i32, i32, i32, vp]
         lib.hypic_oracle_compose.restype = i32
         _lib = lib
@@ -157,6 +163,71 @@ def seam_window(S_in, q, k, v, g, beta, cu_tokens, gate: int = GATE_SCALAR):
     if rc != 0:
         raise ValueError(f"hypic_oracle_seam_window failed with code {rc}")
     return S_out, o
+
+
+def _check_diag_inputs(k, v, g, gate):
+    k, v, g = _f32(k), _f32(v), _f32(g)
+    ttot, H, dk = k.shape
+    dv = v.shape[2]
+    assert v.shape[:2] == (ttot, H)
+    assert g.shape == ((ttot, H) if gate == GATE_SCALAR else (ttot, H, dk)), (g.shape, gate)
+    return k, v, g, ttot, H, dk, dv
+
+
+def diag_encode(k, v, g, cu_seqlens, gate: int = GATE_SCALAR):
+    """Scalar / diagonal families: (E:[n_seg,H,dv,dk], tvec:[n_seg,H] or [n_seg,H,dk])
+    float64 for the recurrence S <- S diag(exp(g_t)) + v_t k_t^T from S = 0; tvec = prod_t exp(g_t)."""
+    k, v, g, ttot, H, dk, dv = _check_diag_inputs(k, v, g, gate)
+    cu = _i32(cu_seqlens)
+    n_seg = cu.shape[0] - 1
+    assert cu[0] == 0 and cu[-1] == ttot and np.all(np.diff(cu) >= 0)
+    E = np.empty((n_seg, H, dv, dk), dtype=np.float64)
+    tvec = np.empty((n_seg, H) if gate == GATE_SCALAR else (n_seg, H, dk), dtype=np.float64)
+    rc = _load().hypic_oracle_diag_encode(_ptr(k), _ptr(v), _ptr(g), _ptr(cu), n_seg, H, dk, dv, gate, _ptr(E),
+                                          _ptr(tvec))
+    if rc != 0:
+        raise ValueError(f"hypic_oracle_diag_encode failed with code {rc}")
+    return E, tvec
+
+
+def diag_sequential(S_in, k, v, g, cu_tokens, gate: int = GATE_SCALAR):
+    """The same recurrence from S_in (None = zeros) over each request's tokens: S_out:[R,H,dv,dk] float64."""
+    k, v, g, ttot, H, dk, dv = _check_diag_inputs(k, v, g, gate)
+    cu = _i32(cu_tokens)
+    R = cu.shape[0] - 1
+    assert np.all(np.diff(cu) >= 0) and cu[0] >= 0 and cu[-1] <= ttot
+    if S_in is not None:
+        S_in = np.ascontiguousarray(S_in, dtype=np.float64)
+        assert S_in.shape == (R, H, dv, dk)
+    S_out = np.empty((R, H, dv, dk), dtype=np.float64)
+    rc = _load().hypic_oracle_diag_sequential(_ptr(S_in), _ptr(k), _ptr(v), _ptr(g), _ptr(cu), R, H, dk, dv, gate,
+                                              _ptr(S_out))
+    if rc != 0:
+        raise ValueError(f"hypic_oracle_diag_sequential failed with code {rc}")
+    return S_out
+
+
+def diag_compose(S_in, E_pool, t_pool, seg_ids, cu_segs):
+    """S <- S diag(t_i) + E_i over each request's ordered ids (Eq. 6 with Table 3's compressed T_C).
+    t_pool:[P,H] (scalar) or [P,H,dk]."""
+    E_pool = np.ascontiguousarray(E_pool, dtype=np.float64)
+    t_pool = np.ascontiguousarray(t_pool, dtype=np.float64)
+    P, H, dv, dk = E_pool.shape
+    gate = GATE_SCALAR if t_pool.ndim == 2 else GATE_CHANNEL
+    assert t_pool.shape == ((P, H) if gate == GATE_SCALAR else (P, H, dk))
+    ids, cu = _i32(seg_ids), _i32(cu_segs)
+    R = cu.shape[0] - 1
+    assert cu[0] == 0 and cu[-1] == ids.shape[0] and np.all(np.diff(cu) >= 0)
+    assert ids.size == 0 or (ids.min() >= 0 and ids.max() < P)
+    if S_in is not None:
+        S_in = np.ascontiguousarray(S_in, dtype=np.float64)
+        assert S_in.shape == (R, H, dv, dk)
+    S_out = np.empty((R, H, dv, dk), dtype=np.float64)
+    rc = _load().hypic_oracle_diag_compose(_ptr(S_in), _ptr(E_pool), _ptr(t_pool), _ptr(ids), _ptr(cu), R, H, dk, dv,
+                                           gate, _ptr(S_out))
+    if rc != 0:
+        raise ValueError(f"hypic_oracle_diag_compose failed with code {rc}")
+    return S_out
 
 
 def compose(S_in, E_pool, T_pool, seg_ids, cu_segs):

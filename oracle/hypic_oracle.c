@@ -20,11 +20,13 @@
  *       first token is the LEFTMOST factor in the row convention):  T <- T diag(a_t) (I - beta_t k_t k_t^T)
  *   zero-start end-state: E = S after the segment's tokens, started from S = 0
  *   composition (Eq. 4, Eq. 6):  S <- S T_i + E_i, i in list order
+ *   scalar / diagonal families (Table 1, Table 3): S <- S diag(a_t) + v_t k_t^T,
+ *       T_C = prod a_t kept as one scalar or a dk-vector, composition S <- S diag(t_i) + E_i  (hypic_oracle_diag_*)
  *   seam-window step (Fig. 8): token steps from a given running state, with the read-out
  *       of PAPER.md:86-90 (Eq. 2) after each step:  paper o_i = q_i^T S_i;  here o_t = S_t q_t
  *
  * There is no chunking, blocking, fusion or reordering here: one token at a time, one row at a time.
- * All pins are in tests/test_oracle_pins.py (P1..P10 and W1..W4 of DESIGN.md); no function here is "parity unpinned".
+ * All pins are in tests/test_oracle_pins.py (P1..P10, W1..W4 and D1..D5 of DESIGN.md); no function here is "parity unpinned".
  *
  * Build: gcc -O3 -march=native -fopenmp -shared -fPIC hypic_oracle.c -o libhypic_oracle.so -lm
  */
@@ -192,6 +194,104 @@ int hypic_oracle_seam_window(const double* S_in, const float* q, const float* k,
         for (int c = 0; c < dk; ++c) acc += Su[(size_t)i * dk + c] * (double)q[th * dk + c];
         o[th * dv + i] = acc;
       }
+    }
+  }
+  return 0;
+}
+
+/*
+ * Scalar and diagonal families of PAPER.md:57-61 (Table 1): T_i = a_i I (RetNet / Lightning-2 with a constant
+ * a_i = gamma, Mamba2 with a data-dependent scalar) or T_i = diag(g_i) (GLA); u_i = k_i v_i^T (no beta, no erase term).
+ * Row convention (state dv x dk):   S <- S diag(a_t) + v_t k_t^T,   a_t = exp(g_t)  (reading A2).
+ * PAPER.md:188-200 (Table 3): T_C = (prod_t a_t) I, stored as ONE scalar, or diag(prod_t g_t), stored as the
+ * dk-vector; applying it is an element-wise scaling of S.
+ *
+ * hypic_oracle_diag_encode: per (segment, head): E = end state from S = 0 (dv x dk) and tvec = prod_t a_t
+ * ([n_seg,H] for the scalar gate, [n_seg,H,dk] for the per-channel gate), the product taken token by token.
+ * A zero-length segment gives E = 0, tvec = 1.  g:[Ttot,H] or [Ttot,H,dk].
+ */
+int hypic_oracle_diag_encode(const float* k, const float* v, const float* g, const int32_t* cu_seqlens, int n_seg,
+                             int H, int dk, int dv, int gate, double* E, double* tvec) {
+  if (n_seg < 0 || H <= 0 || dk <= 0 || dv <= 0 || !cu_seqlens || !E || !tvec) return 1;
+  if (gate != HYPIC_ORACLE_GATE_SCALAR && gate != HYPIC_ORACLE_GATE_CHANNEL) return 1;
+  const int tw = gate == HYPIC_ORACLE_GATE_CHANNEL ? dk : 1;
+  const long n_units = (long)n_seg * H;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (long u = 0; u < n_units; ++u) {
+    const int s = (int)(u / H), h = (int)(u % H);
+    double* Eu = E + (size_t)u * dv * dk;
+    double* tu = tvec + (size_t)u * tw;
+    memset(Eu, 0, sizeof(double) * (size_t)dv * dk);
+    for (int c = 0; c < tw; ++c) tu[c] = 1.0;
+    for (int t = cu_seqlens[s]; t < cu_seqlens[s + 1]; ++t) {
+      const size_t th = (size_t)t * H + h;
+      for (int c = 0; c < tw; ++c) tu[c] *= exp((double)g[th * tw + c]);
+      for (int i = 0; i < dv; ++i)
+        for (int c = 0; c < dk; ++c) {
+          const double a = exp((double)g[th * tw + (tw == 1 ? 0 : c)]);
+          Eu[(size_t)i * dk + c] = Eu[(size_t)i * dk + c] * a + (double)v[th * dv + i] * (double)k[th * dk + c];
+        }
+    }
+  }
+  return 0;
+}
+
+/*
+ * hypic_oracle_diag_sequential: the same token recurrence from S_in (NULL = zeros) over each request's tokens
+ * [cu_tokens[r], cu_tokens[r+1]): what composing the request's segments must reproduce (Eq. 4).
+ */
+int hypic_oracle_diag_sequential(const double* S_in, const float* k, const float* v, const float* g,
+                                 const int32_t* cu_tokens, int R, int H, int dk, int dv, int gate, double* S_out) {
+  if (R < 0 || H <= 0 || dk <= 0 || dv <= 0 || !cu_tokens || !S_out) return 1;
+  if (gate != HYPIC_ORACLE_GATE_SCALAR && gate != HYPIC_ORACLE_GATE_CHANNEL) return 1;
+  const int tw = gate == HYPIC_ORACLE_GATE_CHANNEL ? dk : 1;
+  const long n_units = (long)R * H;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (long u = 0; u < n_units; ++u) {
+    const int r = (int)(u / H), h = (int)(u % H);
+    double* Su = S_out + (size_t)u * dv * dk;
+    if (S_in)
+      memcpy(Su, S_in + (size_t)u * dv * dk, sizeof(double) * (size_t)dv * dk);
+    else
+      memset(Su, 0, sizeof(double) * (size_t)dv * dk);
+    for (int t = cu_tokens[r]; t < cu_tokens[r + 1]; ++t) {
+      const size_t th = (size_t)t * H + h;
+      for (int i = 0; i < dv; ++i)
+        for (int c = 0; c < dk; ++c) {
+          const double a = exp((double)g[th * tw + (tw == 1 ? 0 : c)]);
+          Su[(size_t)i * dk + c] = Su[(size_t)i * dk + c] * a + (double)v[th * dv + i] * (double)k[th * dk + c];
+        }
+    }
+  }
+  return 0;
+}
+
+/*
+ * hypic_oracle_diag_compose: PAPER.md:182 (Eq. 6) with the compressed transitions of Table 3: for every request and
+ * head, S <- S diag(tvec_i) + E_i over the request's ordered pool ids (scalar gate: S <- tvec_i S + E_i).
+ * E_pool:[P,H,dv,dk], t_pool:[P,H] or [P,H,dk], doubles.
+ */
+int hypic_oracle_diag_compose(const double* S_in, const double* E_pool, const double* t_pool, const int32_t* seg_ids,
+                              const int32_t* cu_segs, int R, int H, int dk, int dv, int gate, double* S_out) {
+  if (R < 0 || H <= 0 || dk <= 0 || dv <= 0 || !cu_segs || !S_out) return 1;
+  if (gate != HYPIC_ORACLE_GATE_SCALAR && gate != HYPIC_ORACLE_GATE_CHANNEL) return 1;
+  const int tw = gate == HYPIC_ORACLE_GATE_CHANNEL ? dk : 1;
+  const long n_units = (long)R * H;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (long u = 0; u < n_units; ++u) {
+    const int r = (int)(u / H), h = (int)(u % H);
+    double* Su = S_out + (size_t)u * dv * dk;
+    if (S_in)
+      memcpy(Su, S_in + (size_t)u * dv * dk, sizeof(double) * (size_t)dv * dk);
+    else
+      memset(Su, 0, sizeof(double) * (size_t)dv * dk);
+    for (int j = cu_segs[r]; j < cu_segs[r + 1]; ++j) {
+      const size_t ph = (size_t)seg_ids[j] * H + h;
+      const double* Ei = E_pool + ph * dv * dk;
+      const double* ti = t_pool + ph * tw;
+      for (int i = 0; i < dv; ++i)
+        for (int c = 0; c < dk; ++c)
+          Su[(size_t)i * dk + c] = Su[(size_t)i * dk + c] * ti[tw == 1 ? 0 : c] + Ei[(size_t)i * dk + c];
     }
   }
   return 0;

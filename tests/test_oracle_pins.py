@@ -415,3 +415,126 @@ def test_W4_seam_requests_are_independent_and_empty_window_copies():
     S0, o0 = oracle.seam_window(None, q, k, v, g, beta, cu, GATE_SCALAR)
     Sz, oz = oracle.seam_window(np.zeros_like(S_in), q, k, v, g, beta, cu, GATE_SCALAR)
     assert np.array_equal(S0, Sz) and np.array_equal(o0[:cu[-1]], oz[:cu[-1]])
+
+
+# ---------------------------------------------------------------------------------------------------------
+# D-pins: scalar and diagonal families (Table 1; Table 3):
+# T_i = a_i I or diag(g_i), u_i = k_i v_i^T, T_C kept as one scalar / one dk-vector.
+# ---------------------------------------------------------------------------------------------------------
+def _paper_convention_diag(k, v, g, gate, S0_paper=None):
+    """Explicit T_i matrices in the paper's column convention: S_i = T_i S_{i-1} + k_i v_i^T (S: dk x dv)."""
+    L, dk = k.shape
+    S = np.zeros((dk, v.shape[1])) if S0_paper is None else S0_paper.copy()
+    Tc = np.eye(dk)
+    for i in range(L):
+        Ti = np.exp(g[i]) * np.eye(dk) if gate == GATE_SCALAR else np.diag(np.exp(g[i]))
+        S = Ti @ S + k[i][:, None] @ v[i][None, :]
+        Tc = Ti @ Tc
+    return S, Tc
+
+
+@pytest.mark.parametrize("gate", [GATE_SCALAR, GATE_CHANNEL])
+@pytest.mark.parametrize("L,dk,dv", [(1, 3, 2), (5, 4, 4), (9, 5, 7)])
+def test_D1_diag_bruteforce_paper_convention(gate, L, dk, dv):
+    rng = np.random.default_rng(5100 + L + 3 * dk + 7 * gate)
+    k, v, g, _ = _rand_inputs(L, 1, dk, dv, gate, rng, g_lo=-0.7, normalise=False)
+    E, tvec = oracle.diag_encode(k, v, g, _cu([L]), gate)
+    S_p, T_p = _paper_convention_diag(k[:, 0].astype(np.float64), v[:, 0].astype(np.float64),
+                                      g[:, 0].astype(np.float64), gate)
+    np.testing.assert_allclose(E[0, 0], S_p.T, rtol=1e-12, atol=1e-14)
+    full = tvec[0, 0] * np.eye(dk) if gate == GATE_SCALAR else np.diag(tvec[0, 0])
+    np.testing.assert_allclose(full, T_p.T, rtol=1e-12, atol=0)
+    # from a non-zero state
+    S0 = rng.standard_normal((1, 1, dv, dk))
+    S = oracle.diag_sequential(S0, k, v, g, _cu([L]), gate)
+    S_p2, _ = _paper_convention_diag(k[:, 0].astype(np.float64), v[:, 0].astype(np.float64),
+                                     g[:, 0].astype(np.float64), gate, S0_paper=S0[0, 0].T)
+    np.testing.assert_allclose(S[0, 0], S_p2.T, rtol=1e-12, atol=1e-14)
+
+
+def test_D2_table3_closed_forms():
+    """Table 3 (PAPER.md:192-194): RetNet / Lightning T_C = gamma^{|C|} I, Mamba2 (prod_t a_t) I, GLA diag(prod_t g_t);
+    and E = sum_t (prod_{s>t} a_s) v_t k_t^T written as one weighted matrix product."""
+    rng = np.random.default_rng(5200)
+    L, H, dk, dv = 50, 2, 6, 4
+    k, v, _, _ = _rand_inputs(L, H, dk, dv, GATE_SCALAR, rng, normalise=False)
+    gamma = 1.0 - 2.0 ** -5
+    g_const = np.full((L, H), np.log(gamma), dtype=np.float32)
+    g_eff = np.exp(np.float64(g_const[0, 0]))  # the decay the oracle actually sees (fp32-rounded log)
+    E, t = oracle.diag_encode(k, v, g_const, _cu([L]), GATE_SCALAR)
+    np.testing.assert_allclose(t, g_eff ** L, rtol=1e-12)
+    w = g_eff ** (L - 1 - np.arange(L))  # token t is decayed by the L-1-t tokens after it
+    for h in range(H):
+        ref = (v[:, h].astype(np.float64) * w[:, None]).T @ k[:, h].astype(np.float64)
+        np.testing.assert_allclose(E[0, h], ref, rtol=1e-11, atol=1e-13)
+    g_s = (rng.random((L, H)) * -0.4).astype(np.float32)
+    _, t_s = oracle.diag_encode(k, v, g_s, _cu([L]), GATE_SCALAR)
+    np.testing.assert_allclose(t_s[0], np.exp(g_s.astype(np.float64).sum(0)), rtol=1e-12)
+    g_c = (rng.random((L, H, dk)) * -0.4).astype(np.float32)
+    E_c, t_c = oracle.diag_encode(k, v, g_c, _cu([L]), GATE_CHANNEL)
+    np.testing.assert_allclose(t_c[0], np.exp(g_c.astype(np.float64).sum(0)), rtol=1e-12)
+    G = np.cumsum(g_c.astype(np.float64), axis=0)
+    wt = np.exp(G[-1][None] - G)  # [L,H,dk]: decay of channel c from token t to the end
+    for h in range(H):
+        ref = v[:, h].astype(np.float64).T @ (k[:, h].astype(np.float64) * wt[:, h])
+        np.testing.assert_allclose(E_c[0, h], ref, rtol=1e-11, atol=1e-13)
+
+
+@pytest.mark.parametrize("gate", [GATE_SCALAR, GATE_CHANNEL])
+@pytest.mark.parametrize("zero_start", [True, False])
+def test_D3_diag_compose_equals_sequential(gate, zero_start):
+    """PAPER.md:118 Eq. 4 / PAPER.md:182 Eq. 6 for the compressed transitions: composing the cached (E, tvec) of the
+    segments in order reproduces the recurrence over the concatenation; a different order does not."""
+    rng = np.random.default_rng(5300 + gate)
+    lens = [17, 1, 40, 0, 9]
+    H, dk, dv = 2, 8, 5
+    k, v, g, _ = _rand_inputs(sum(lens), H, dk, dv, gate, rng, g_lo=-0.2, normalise=False)
+    E, t = oracle.diag_encode(k, v, g, _cu(lens), gate)
+    S0 = None if zero_start else rng.standard_normal((1, H, dv, dk))
+    ids = np.arange(len(lens), dtype=np.int32)
+    S = oracle.diag_compose(S0, E, t, ids, _cu([len(lens)]))
+    S_seq = oracle.diag_sequential(S0, k, v, g, _cu([sum(lens)]), gate)
+    np.testing.assert_allclose(S, S_seq, rtol=1e-11, atol=1e-13)
+    S_rev = oracle.diag_compose(S0, E, t, ids[::-1].copy(), _cu([len(lens)]))
+    assert oracle.rel_fro(S_rev, S_seq) > 1e-3
+
+
+def test_D4_table2_printed_values_with_real_suffix(golden_dir):
+    """Table 2 on the scalar family itself: adding the two zero-start end-states instead of composing
+    them leaves the error Delta = (1 - gamma^{|C2|}) S_{C1|0}, whatever the suffix holds."""
+    rows = []
+    with open(os.path.join(golden_dir, "table2_naive_addition_error.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                e, n, val = line.split()
+                rows.append((int(e), int(n), float(val)))
+    rng = np.random.default_rng(5400)
+    H, dk, dv, l1 = 1, 6, 4, 30
+    for e, n, printed in rows:
+        gamma = 1.0 - 2.0 ** e
+        k, v, _, _ = _rand_inputs(l1 + n, H, dk, dv, GATE_SCALAR, rng, normalise=False)
+        g = np.full((l1 + n, H), np.log(gamma), dtype=np.float32)
+        E, t = oracle.diag_encode(k, v, g, _cu([l1, n]), GATE_SCALAR)
+        S_true = oracle.diag_compose(None, E, t, np.array([0, 1], dtype=np.int32), _cu([2]))
+        delta = (E[0] + E[1]) - S_true[0]
+        ratio = np.linalg.norm(delta) / np.linalg.norm(E[0])
+        assert abs(ratio - printed) <= 5.1e-4, (e, n, ratio, printed)
+
+
+def test_D5_diag_family_is_the_dense_family_without_erasure():
+    """Cross-family check against the pinned dense oracle: the dense token step with the erase term removed
+    (T_i = g_i (I - beta_i k_i k_i^T) -> g_i I) is linear in v, so for ORTHONORMAL keys in a segment
+    (k_s . k_t = 0: nothing is ever erased) and beta = 1 the dense end-state equals the scalar family's, and the dense
+    T equals tvec (I - sum_t k_t k_t^T)."""
+    rng = np.random.default_rng(5500)
+    L, dk, dv = 6, 8, 5
+    q, _ = np.linalg.qr(rng.standard_normal((dk, dk)))
+    k = q[:L][:, None, :].astype(np.float32)  # float32 rounding leaves k_s . k_t ~ 1e-8
+    v = rng.standard_normal((L, 1, dv)).astype(np.float32)
+    g = (rng.random((L, 1)) * -0.5).astype(np.float32)
+    beta = np.ones((L, 1), dtype=np.float32)
+    E_dense, T_dense = oracle.segment_encode(k, v, g, beta, _cu([L]), GATE_SCALAR)
+    E_diag, t = oracle.diag_encode(k, v, g, _cu([L]), GATE_SCALAR)
+    np.testing.assert_allclose(E_dense, E_diag, rtol=0, atol=1e-6)
+    kk = k[:, 0].astype(np.float64)
+    np.testing.assert_allclose(T_dense[0, 0], t[0, 0] * (np.eye(dk) - kk.T @ kk), rtol=0, atol=1e-6)
