@@ -160,6 +160,31 @@ int hypic_seam_window(const void* q, const void* k, const void* v, const float* 
                       int kv_dtype, int gate, const float* S_in, float* S_out, float* o, void* stream);
 
 /*
+ * Scalar and diagonal families (Table 1; compressed transitions of PAPER.md:188-200 Table 3).
+ * T_i = a_i I (RetNet / Lightning-2 with a constant a_i = gamma, Mamba2 with a data-dependent scalar) or diag(g_i)
+ * (GLA); u_i = k_i v_i^T (no beta).  Row convention: S <- S diag(a_t) + v_t k_t^T, a_t = exp(g_t) (A2).
+ *
+ * hypic_diag_encode: per segment and head, E[s,h] = the end state from S = 0 (dv x dk) and tvec[s,h] = prod_t a_t over
+ * the segment's tokens: T_C of Table 3 in its stored form -- ONE scalar for HYPIC_GATE_SCALAR, the dk-vector of the
+ * diagonal for HYPIC_GATE_CHANNEL.
+ *   k [t_total,H,dk], v [t_total,H,dv] kv_dtype; g [t_total,H] or [t_total,H,dk] fp32 log-decay; cu_seqlens as in
+ *   hypic_segment_encode; E out [n_seg,H,dv,dk] fp32; tvec out [n_seg,H] or [n_seg,H,dk] fp32.
+ * A zero-length segment yields E = 0, tvec = 1.  Built envelope: dk in {64, 128}, dv in [1, 1024], any gate value
+ * (the pre-weighting inside the kernel only multiplies by factors in (0, 1] when g <= 0).  No workspace.
+ *
+ * hypic_diag_compose: S <- S diag(tvec_i) + E_i (Eq. 6 with Table 3's "element-wise scaling" apply step;
+ * HYPIC_GATE_SCALAR: S <- tvec_i S + E_i) over each request's ordered id list; arguments as hypic_compose with
+ * t_pool [P,H] or [P,H,dk] fp32 in place of T_pool.  S_out may alias S_in exactly.  Built envelope: dk % 4 == 0,
+ * dk, dv <= 1024.
+ */
+int hypic_diag_encode(const void* k, const void* v, const float* g, const int32_t* cu_seqlens, int32_t n_seg,
+                      int32_t t_total, int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate, float* E, float* tvec,
+                      void* stream);
+int hypic_diag_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,
+                       const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
+                       int32_t dv, int gate, float* S_out, void* stream);
+
+/*
  * hypic_encode_impl_for / hypic_compose_impl_for: which kernel family (HYPIC_IMPL_SIMT or HYPIC_IMPL_TENSOR)
  * a call with this shape would run under the current hypic_set_impl setting, or a negative hypic_status_t
  * (-HYPIC_ERR_UNSUPPORTED / -HYPIC_ERR_INVALID_ARG) if the call would be rejected.  Pure host arithmetic;

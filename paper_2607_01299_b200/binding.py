@@ -29,7 +29,7 @@ EXPORTS = (
     "hypic_set_impl", "hypic_get_impl", "hypic_segment_encode_workspace", "hypic_segment_encode", "hypic_compose",
     "hypic_status_string", "hypic_version", "hypic_last_launch_count", "hypic_encode_impl_for",
     "hypic_compose_impl_for", "hypic_debug_timeout_count", "hypic_envelope_violation_count", "hypic_compose_f16",
-    "hypic_tuple_pack_f16", "hypic_seam_window",
+    "hypic_tuple_pack_f16", "hypic_seam_window", "hypic_diag_encode", "hypic_diag_compose",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -71,6 +71,10 @@ def load_library() -> ctypes.CDLL:
     lib.hypic_seam_window.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, ctypes.c_int, ctypes.c_int, vp,
                                       vp, vp, vp]
     lib.hypic_seam_window.restype = ctypes.c_int
+    lib.hypic_diag_encode.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, ctypes.c_int, ctypes.c_int, vp, vp, vp]
+    lib.hypic_diag_encode.restype = ctypes.c_int
+    lib.hypic_diag_compose.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, ctypes.c_int, vp, vp]
+    lib.hypic_diag_compose.restype = ctypes.c_int
     lib.hypic_status_string.argtypes = [ctypes.c_int]
     lib.hypic_status_string.restype = ctypes.c_char_p
     lib.hypic_version.argtypes = []
@@ -334,3 +338,88 @@ def hypic_seam_window(S_in: Optional[torch.Tensor], q: torch.Tensor, k: torch.Te
     if rc != HYPIC_OK:
         raise HypicError(rc, "hypic_seam_window")
     return S_out, o
+
+
+def hypic_diag_encode(k: torch.Tensor, v: torch.Tensor, g: torch.Tensor, cu_seqlens: torch.Tensor,
+                      gate: int = HYPIC_GATE_SCALAR, *, E: Optional[torch.Tensor] = None,
+                      tvec: Optional[torch.Tensor] = None,
+                      stream: Optional[torch.cuda.Stream] = None) -> Tuple[torch.Tensor, torch.Tensor]:
+    """Scalar / diagonal families: E:[n_seg,H,dv,dk] fp32 and tvec:[n_seg,H] (scalar gate) or [n_seg,H,dk] fp32 for
+    the recurrence S <- S diag(exp(g_t)) + v_t k_t^T over each segment from S = 0."""
+    lib = load_library()
+    for name, t in (("k", k), ("v", v), ("g", g), ("cu_seqlens", cu_seqlens)):
+        if not t.is_cuda:
+            raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if k.dim() != 3 or v.dim() != 3 or k.shape[:2] != v.shape[:2] or k.dtype != v.dtype:
+        raise ValueError("k:[Ttot,H,dk] and v:[Ttot,H,dv] must agree in Ttot, H and dtype")
+    t_total, H, dk = (int(x) for x in k.shape)
+    dv = int(v.shape[2])
+    if k.dtype == torch.bfloat16:
+        kv_dtype = HYPIC_DT_BF16
+    elif k.dtype == torch.float32:
+        kv_dtype = HYPIC_DT_F32
+    else:
+        raise ValueError(f"k/v must be bf16 or fp32, got {k.dtype}")
+    want_g = (t_total, H) if gate == HYPIC_GATE_SCALAR else (t_total, H, dk)
+    if tuple(g.shape) != want_g:
+        raise ValueError(f"g must be {want_g}; got {tuple(g.shape)}")
+    n_seg = int(cu_seqlens.numel()) - 1
+    if n_seg < 0:
+        raise ValueError("cu_seqlens must have n_seg+1 >= 1 entries")
+    dev = k.device
+    t_shape = (n_seg, H) if gate == HYPIC_GATE_SCALAR else (n_seg, H, dk)
+    if E is None:
+        E = torch.empty((n_seg, H, dv, dk), dtype=torch.float32, device=dev)
+    if tvec is None:
+        tvec = torch.empty(t_shape, dtype=torch.float32, device=dev)
+    if tuple(E.shape) != (n_seg, H, dv, dk) or tuple(tvec.shape) != t_shape:
+        raise ValueError("E / tvec have the wrong shape")
+    with torch.cuda.device(dev):
+        rc = lib.hypic_diag_encode(_dev_ptr(k, "k"), _dev_ptr(v, "v"), _dev_ptr(g, "g", torch.float32),
+                                   _dev_ptr(cu_seqlens, "cu_seqlens", torch.int32), n_seg, t_total, H, dk, dv,
+                                   kv_dtype, int(gate), _dev_ptr(E, "E", torch.float32),
+                                   _dev_ptr(tvec, "tvec", torch.float32), _stream_handle(stream))
+    if rc != HYPIC_OK:
+        raise HypicError(rc, "hypic_diag_encode")
+    return E, tvec
+
+
+def hypic_diag_compose(S_in: Optional[torch.Tensor], E_pool: torch.Tensor, t_pool: torch.Tensor,
+                       seg_ids: torch.Tensor, cu_segs: torch.Tensor, *, total_steps: Optional[int] = None,
+                       S_out: Optional[torch.Tensor] = None,
+                       stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """S_out[r,h] = fold of S <- S diag(t_i) + E_i over seg_ids[cu_segs[r]:cu_segs[r+1]] from S_in[r,h] (None = 0);
+    t_pool:[P,H] (scalar family) or [P,H,dk] (diagonal family)."""
+    lib = load_library()
+    for name, t in (("E_pool", E_pool), ("t_pool", t_pool), ("seg_ids", seg_ids), ("cu_segs", cu_segs)):
+        if not t.is_cuda:
+            raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if E_pool.dim() != 4:
+        raise ValueError("E_pool:[P,H,dv,dk]")
+    P, H, dv, dk = (int(x) for x in E_pool.shape)
+    if tuple(t_pool.shape) == (P, H):
+        gate = HYPIC_GATE_SCALAR
+    elif tuple(t_pool.shape) == (P, H, dk):
+        gate = HYPIC_GATE_CHANNEL
+    else:
+        raise ValueError("t_pool must be [P,H] or [P,H,dk]")
+    R = int(cu_segs.numel()) - 1
+    if R < 0:
+        raise ValueError("cu_segs must have R+1 >= 1 entries")
+    if total_steps is None:
+        total_steps = int(seg_ids.numel())
+    if S_in is not None and tuple(S_in.shape) != (R, H, dv, dk):
+        raise ValueError("S_in must be [R,H,dv,dk]")
+    if S_out is None:
+        S_out = torch.empty((R, H, dv, dk), dtype=torch.float32, device=E_pool.device)
+    if tuple(S_out.shape) != (R, H, dv, dk):
+        raise ValueError("S_out must be [R,H,dv,dk]")
+    with torch.cuda.device(E_pool.device):
+        rc = lib.hypic_diag_compose(
+            _dev_ptr(S_in, "S_in", torch.float32), _dev_ptr(E_pool, "E_pool", torch.float32),
+            _dev_ptr(t_pool, "t_pool", torch.float32), _dev_ptr(seg_ids, "seg_ids", torch.int32),
+            _dev_ptr(cu_segs, "cu_segs", torch.int32), R, P, int(total_steps), H, dk, dv, gate,
+            _dev_ptr(S_out, "S_out", torch.float32), _stream_handle(stream))
+    if rc != HYPIC_OK:
+        raise HypicError(rc, "hypic_diag_compose")
+    return S_out

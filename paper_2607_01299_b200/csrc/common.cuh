@@ -70,10 +70,36 @@ struct SeamArgs {
   cudaStream_t stream;
 };
 
+struct DiagEncodeArgs {
+  const void* k;
+  const void* v;
+  const float* g;
+  const int32_t* cu_seqlens;
+  int32_t n_seg, t_total, H, dk, dv;
+  int kv_dtype, gate;
+  float* E;
+  float* tvec;
+  cudaStream_t stream;
+};
+
+struct DiagComposeArgs {
+  const float* S_in;
+  const float* E_pool;
+  const float* t_pool;
+  const int32_t* seg_ids;
+  const int32_t* cu_segs;
+  int32_t R, P, total_steps, H, dk, dv;
+  int gate;
+  float* S_out;
+  cudaStream_t stream;
+};
+
 // Kernel families (each returns a hypic_status_t; UNSUPPORTED when the shape is outside its envelope).
 int encode_simt(const EncodeArgs& a);
 int compose_simt(const ComposeArgs& a);
 int seam_simt(const SeamArgs& a);
+int diag_encode(const DiagEncodeArgs& a);
+int diag_compose(const DiagComposeArgs& a);
 bool encode_tensor_shape_ok(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate);
 inline bool encode_tensor_supported(const EncodeArgs& a) {
   return encode_tensor_shape_ok(a.H, a.dk, a.dv, a.kv_dtype, a.gate);

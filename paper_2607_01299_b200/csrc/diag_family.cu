@@ -1,0 +1,252 @@
+// diag_family.cu -- scalar and diagonal families of PAPER.md:57-61 (Table 1) with the compressed transitions of
+// PAPER.md:188-200 (Table 3): T_i = a_i I (RetNet, Lightning-2, Mamba2) or diag(g_i) (GLA), u_i = k_i v_i^T.
+// Row convention (state dv x dk):   S <- S diag(a_t) + v_t k_t^T,  a_t = exp(g_t);
+//     encode:   E = end state from 0,  tvec = prod_t a_t   (one scalar, or a dk-vector, per (segment, head))
+//     compose:  S <- S diag(tvec_i) + E_i                   (element-wise: "O(dk dv)" apply cost of Table 3)
+//
+// diag_encode_simt_kernel (fp32 CUDA cores; the accurate path for fp32 inputs and any dk in {64,128}, dv <= 1024):
+//   one thread per row of E, dk-wide row in registers.  Tokens are staged in tiles of 16; inside a tile the keys are
+//   pre-weighted once per CTA with the decay from their token to the END of the tile, k~_t = k_t * exp(G_end - G_t)
+//   (a factor in (0, 1]: no overflow whatever the gate), so the row update is one FMA per element and token,
+//   x += v_t[i] k~_t, and the state is decayed once per tile, x *= exp(G_end - G_start).  tvec is the exponential of
+//   the log-decay summed in fp64 (4,096 fp32 terms would cost 1e-5 in fp32).
+// diag_compose_kernel: the fold is element-wise, so every thread owns 4 float4s of S for the whole chain and streams
+//   the E_i of its request through registers, one step prefetched ahead: bound by reading E_i from HBM.
+#include "common.cuh"
+
+namespace hypic {
+namespace {
+
+constexpr int kDgRows = 64;  // threads (= rows of E) per encode CTA
+constexpr int kDgTT = 16;    // tokens per staged tile
+
+template <bool BF16>
+__device__ __forceinline__ float dg_load(const void* p, size_t idx) {
+  if (BF16) return __bfloat162float(reinterpret_cast<const __nv_bfloat16*>(p)[idx]);
+  return reinterpret_cast<const float*>(p)[idx];
+}
+
+template <int DK, bool BF16, bool CHANNEL>
+__global__ void __launch_bounds__(kDgRows)
+    diag_encode_simt_kernel(const void* __restrict__ k, const void* __restrict__ v, const float* __restrict__ g,
+                            const int32_t* __restrict__ cu_seqlens, int H, int dv, float* __restrict__ E,
+                            float* __restrict__ tvec) {
+  constexpr int AW = CHANNEL ? DK : 1;
+  __shared__ __align__(16) float sk[2][kDgTT][DK];   // pre-weighted keys of the tile
+  __shared__ __align__(16) float sdec[2][AW];        // decay over the whole tile
+  __shared__ float sw[2][kDgTT][kDgRows];            // this CTA's value entries v_t[i]
+  __shared__ float sg[kDgTT][AW];                    // log-decays of the tile being staged
+
+  const int tid = threadIdx.x;
+  const int h = blockIdx.y, s = blockIdx.z;
+  const int row0 = blockIdx.x * kDgRows;
+  const int row = row0 + tid;
+  const int t_begin = cu_seqlens[s], t_end = cu_seqlens[s + 1];
+  const int L = t_end - t_begin;
+
+  float x[DK];
+#pragma unroll
+  for (int c = 0; c < DK; ++c) x[c] = 0.f;
+
+  // fp64 running sum of the log-decay: CTA 0 of the unit writes tvec.  Scalar gate: thread 0; channel gate: thread c
+  // and c + 64.
+  double gsum0 = 0.0, gsum1 = 0.0;
+
+  auto stage = [&](int buf, int tile) {
+    const int tbase = t_begin + tile * kDgTT;
+    const int n_tok = min(kDgTT, t_end - tbase);
+    // log-decays of the tile -> shared memory (zeros past the end of the segment)
+    for (int idx = tid; idx < kDgTT * AW; idx += kDgRows) {
+      const int tok = idx / AW, c = idx % AW;
+      sg[tok][c] = tok < n_tok ? g[((size_t)(tbase + tok) * H + h) * AW + c] : 0.f;
+    }
+    for (int idx = tid; idx < kDgTT * kDgRows; idx += kDgRows) {
+      const int tok = idx / kDgRows, j = idx % kDgRows;
+      float wv = 0.f;
+      if (tok < n_tok && row0 + j < dv) wv = dg_load<BF16>(v, ((size_t)(tbase + tok) * H + h) * dv + row0 + j);
+      sw[buf][tok][j] = wv;
+    }
+    __syncthreads();
+    // suffix sums inside the tile, one thread per channel (or thread 0): weight of token t = exp(sum_{s > t} g_s)
+    for (int c = tid; c < AW; c += kDgRows) {
+      float suf = 0.f;
+      double acc = 0.0;
+#pragma unroll
+      for (int tok = kDgTT - 1; tok >= 0; --tok) {
+        const float gv = sg[tok][c];
+        sg[tok][c] = suf;  // in place: now the log-weight of token tok
+        suf += gv;
+        acc += (double)gv;
+      }
+      sdec[buf][c] = expf(suf);
+      if (c < kDgRows) gsum0 += acc; else gsum1 += acc;
+    }
+    __syncthreads();
+    for (int idx = tid; idx < kDgTT * DK; idx += kDgRows) {
+      const int tok = idx / DK, c = idx % DK;
+      float kv = 0.f;
+      if (tok < n_tok) kv = dg_load<BF16>(k, ((size_t)(tbase + tok) * H + h) * DK + c) * expf(sg[tok][CHANNEL ? c : 0]);
+      sk[buf][tok][c] = kv;
+    }
+  };
+
+  const int n_tiles = (L + kDgTT - 1) / kDgTT;
+  if (n_tiles > 0) stage(0, 0);
+  __syncthreads();
+  for (int tile = 0; tile < n_tiles; ++tile) {
+    const int buf = tile & 1;
+    // decay of the state over this tile, then the tile's writes
+    if (CHANNEL) {
+      const float4* d4 = reinterpret_cast<const float4*>(&sdec[buf][0]);
+#pragma unroll
+      for (int c4 = 0; c4 < DK / 4; ++c4) {
+        const float4 dd = d4[c4];
+        x[4 * c4 + 0] *= dd.x;
+        x[4 * c4 + 1] *= dd.y;
+        x[4 * c4 + 2] *= dd.z;
+        x[4 * c4 + 3] *= dd.w;
+      }
+    } else {
+      const float dd = sdec[buf][0];
+#pragma unroll
+      for (int c = 0; c < DK; ++c) x[c] *= dd;
+    }
+    const int n_tok = min(kDgTT, L - tile * kDgTT);
+    for (int tok = 0; tok < n_tok; ++tok) {
+      const float w = sw[buf][tok][tid];
+      const float4* k4 = reinterpret_cast<const float4*>(&sk[buf][tok][0]);
+#pragma unroll
+      for (int c4 = 0; c4 < DK / 4; ++c4) {
+        const float4 kk = k4[c4];
+        x[4 * c4 + 0] = fmaf(w, kk.x, x[4 * c4 + 0]);
+        x[4 * c4 + 1] = fmaf(w, kk.y, x[4 * c4 + 1]);
+        x[4 * c4 + 2] = fmaf(w, kk.z, x[4 * c4 + 2]);
+        x[4 * c4 + 3] = fmaf(w, kk.w, x[4 * c4 + 3]);
+      }
+    }
+    __syncthreads();  // everyone is done with sg (staging scratch) and with buffer buf ^ 1 of the tile before
+    if (tile + 1 < n_tiles) stage(buf ^ 1, tile + 1);
+    __syncthreads();
+  }
+
+  if (row < dv) {
+    float4* d4 = reinterpret_cast<float4*>(E + (((size_t)s * H + h) * dv + row) * DK);
+#pragma unroll
+    for (int c4 = 0; c4 < DK / 4; ++c4) d4[c4] = make_float4(x[4 * c4], x[4 * c4 + 1], x[4 * c4 + 2], x[4 * c4 + 3]);
+  }
+  if (blockIdx.x == 0) {
+    float* tv = tvec + ((size_t)s * H + h) * AW;
+    if (tid < AW) tv[tid] = (float)exp(gsum0);
+    if (CHANNEL && tid + kDgRows < AW) tv[tid + kDgRows] = (float)exp(gsum1);
+  }
+}
+
+template <int DK, bool BF16, bool CHANNEL>
+int dg_launch(const DiagEncodeArgs& a) {
+  dim3 grid((a.dv + kDgRows - 1) / kDgRows, a.H, a.n_seg);
+  diag_encode_simt_kernel<DK, BF16, CHANNEL><<<grid, kDgRows, 0, a.stream>>>(a.k, a.v, a.g, a.cu_seqlens, a.H, a.dv,
+                                                                            a.E, a.tvec);
+  note_launch();
+  HYPIC_CUDA_OK(cudaGetLastError());
+  return HYPIC_OK;
+}
+
+template <int DK>
+int dg_dispatch(const DiagEncodeArgs& a) {
+  const bool bf = a.kv_dtype == HYPIC_DT_BF16, ch = a.gate == HYPIC_GATE_CHANNEL;
+  if (bf) return ch ? dg_launch<DK, true, true>(a) : dg_launch<DK, true, false>(a);
+  return ch ? dg_launch<DK, false, true>(a) : dg_launch<DK, false, false>(a);
+}
+
+// ------------------------------------------------------------------------------------------------ compose
+constexpr int kDcThreads = 256;
+constexpr int kDcV4 = 4;  // float4s of S per thread: a CTA owns 4,096 consecutive elements of one (request, head)
+
+template <bool CHANNEL>
+__global__ void __launch_bounds__(kDcThreads)
+    diag_compose_kernel(const float* __restrict__ S_in, const float* __restrict__ E_pool,
+                        const float* __restrict__ t_pool, const int32_t* __restrict__ seg_ids,
+                        const int32_t* __restrict__ cu_segs, int H, int dk, int unit_v4, float* __restrict__ S_out) {
+  const int tid = threadIdx.x;
+  const int h = blockIdx.y, r = blockIdx.z;
+  const size_t unit = (size_t)r * H + h;
+  int e4[kDcV4];  // float4 index inside the unit's dv x dk block
+  bool live[kDcV4];
+#pragma unroll
+  for (int i = 0; i < kDcV4; ++i) {
+    e4[i] = (blockIdx.x * kDcV4 + i) * kDcThreads + tid;
+    live[i] = e4[i] < unit_v4;
+  }
+  float4 x[kDcV4];
+#pragma unroll
+  for (int i = 0; i < kDcV4; ++i) {
+    x[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (live[i] && S_in) x[i] = __ldg(reinterpret_cast<const float4*>(S_in) + unit * unit_v4 + e4[i]);
+  }
+  const int dk4 = dk / 4;
+  const int j0 = cu_segs[r], j1 = cu_segs[r + 1];
+  float4 e_nxt[kDcV4], t_nxt[kDcV4];
+  auto fetch = [&](int j) {
+    const size_t ph = (size_t)seg_ids[j] * H + h;
+    const float4* Ei = reinterpret_cast<const float4*>(E_pool) + ph * unit_v4;
+#pragma unroll
+    for (int i = 0; i < kDcV4; ++i) {
+      if (live[i]) {
+        e_nxt[i] = __ldcs(Ei + e4[i]);
+        if (CHANNEL) {
+          t_nxt[i] = __ldg(reinterpret_cast<const float4*>(t_pool + ph * dk) + e4[i] % dk4);
+        } else {
+          const float ts = __ldg(t_pool + ph);
+          t_nxt[i] = make_float4(ts, ts, ts, ts);
+        }
+      }
+    }
+  };
+  if (j0 < j1) fetch(j0);
+  for (int j = j0; j < j1; ++j) {
+    float4 e_cur[kDcV4], t_cur[kDcV4];
+#pragma unroll
+    for (int i = 0; i < kDcV4; ++i) e_cur[i] = e_nxt[i], t_cur[i] = t_nxt[i];
+    if (j + 1 < j1) fetch(j + 1);
+#pragma unroll
+    for (int i = 0; i < kDcV4; ++i) {
+      x[i].x = fmaf(x[i].x, t_cur[i].x, e_cur[i].x);
+      x[i].y = fmaf(x[i].y, t_cur[i].y, e_cur[i].y);
+      x[i].z = fmaf(x[i].z, t_cur[i].z, e_cur[i].z);
+      x[i].w = fmaf(x[i].w, t_cur[i].w, e_cur[i].w);
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < kDcV4; ++i)
+    if (live[i]) __stcs(reinterpret_cast<float4*>(S_out) + unit * unit_v4 + e4[i], x[i]);
+}
+
+}  // namespace
+
+int diag_encode(const DiagEncodeArgs& a) {
+  if (a.H > 65535 || a.n_seg > 65535) return HYPIC_ERR_UNSUPPORTED;
+  if (a.dv < 1 || a.dv > 1024) return HYPIC_ERR_UNSUPPORTED;
+  if (a.n_seg == 0) return HYPIC_OK;
+  if (a.dk == 128) return dg_dispatch<128>(a);
+  if (a.dk == 64) return dg_dispatch<64>(a);
+  return HYPIC_ERR_UNSUPPORTED;
+}
+
+int diag_compose(const DiagComposeArgs& a) {
+  if (a.H > 65535 || a.R > 65535) return HYPIC_ERR_UNSUPPORTED;
+  if (a.dk % 4 != 0) return HYPIC_ERR_UNSUPPORTED;
+  if (a.R == 0) return HYPIC_OK;
+  const int unit_v4 = a.dv * a.dk / 4;
+  dim3 grid((unit_v4 + kDcThreads * kDcV4 - 1) / (kDcThreads * kDcV4), a.H, a.R);
+  if (a.gate == HYPIC_GATE_CHANNEL)
+    diag_compose_kernel<true><<<grid, kDcThreads, 0, a.stream>>>(a.S_in, a.E_pool, a.t_pool, a.seg_ids, a.cu_segs, a.H,
+                                                                 a.dk, unit_v4, a.S_out);
+  else
+    diag_compose_kernel<false><<<grid, kDcThreads, 0, a.stream>>>(a.S_in, a.E_pool, a.t_pool, a.seg_ids, a.cu_segs, a.H,
+                                                                  a.dk, unit_v4, a.S_out);
+  note_launch();
+  HYPIC_CUDA_OK(cudaGetLastError());
+  return HYPIC_OK;
+}
+
+}  // namespace hypic

@@ -146,6 +146,36 @@ int hypic_seam_window(const void* q, const void* k, const void* v, const float* 
   return seam_simt(a);
 }
 
+int hypic_diag_encode(const void* k, const void* v, const float* g, const int32_t* cu_seqlens, int32_t n_seg,
+                      int32_t t_total, int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate, float* E, float* tvec,
+                      void* stream) {
+  g_launch_count = 0;
+  const int vs = validate_encode_shape(n_seg, t_total, H, dk, dv, kv_dtype, gate);
+  if (vs != HYPIC_OK) return vs;
+  if (!cu_seqlens) return HYPIC_ERR_INVALID_ARG;
+  if (n_seg > 0 && (!E || !tvec)) return HYPIC_ERR_INVALID_ARG;
+  if (t_total > 0 && (!k || !v || !g)) return HYPIC_ERR_INVALID_ARG;
+  if (!aligned16(k) || !aligned16(v) || !aligned16(g) || !aligned16(E) || !aligned16(tvec)) return HYPIC_ERR_INVALID_ARG;
+  DiagEncodeArgs a{k, v, g, cu_seqlens, n_seg, t_total, H, dk, dv, kv_dtype, gate, E, tvec, (cudaStream_t)stream};
+  return diag_encode(a);
+}
+
+int hypic_diag_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,
+                       const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
+                       int32_t dv, int gate, float* S_out, void* stream) {
+  g_launch_count = 0;
+  if (R < 0 || P < 0 || total_steps < 0 || H <= 0 || dk <= 0 || dv <= 0) return HYPIC_ERR_INVALID_ARG;
+  if (gate != HYPIC_GATE_SCALAR && gate != HYPIC_GATE_CHANNEL) return HYPIC_ERR_INVALID_ARG;
+  if (!cu_segs) return HYPIC_ERR_INVALID_ARG;
+  if (R > 0 && !S_out) return HYPIC_ERR_INVALID_ARG;
+  if (total_steps > 0 && (!E_pool || !t_pool || !seg_ids || P == 0)) return HYPIC_ERR_INVALID_ARG;
+  if (!aligned16(S_in) || !aligned16(E_pool) || !aligned16(t_pool) || !aligned16(S_out)) return HYPIC_ERR_INVALID_ARG;
+  if (dk % 4 != 0 || dk > 1024 || dv > 1024) return HYPIC_ERR_UNSUPPORTED;
+  DiagComposeArgs a{S_in, E_pool, t_pool, seg_ids, cu_segs, R, P, total_steps, H, dk, dv, gate, S_out,
+                    (cudaStream_t)stream};
+  return diag_compose(a);
+}
+
 int hypic_encode_impl_for(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate) {
   const int vs = validate_encode_shape(0, 0, H, dk, dv, kv_dtype, gate);
   if (vs != HYPIC_OK) return -vs;

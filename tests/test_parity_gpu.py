@@ -517,3 +517,88 @@ def test_seam_window_cfg_full_size_sampled_units():
                                           f(e.beta), np.array([0, sl.stop - sl.start], dtype=np.int32), gate=e.gate)
         check_E(S[r:r + 1, h:h + 1], S_ref, TOL_F32, "S_out")
         _check_o(o[sl, h:h + 1], o_ref, np.array([0, sl.stop - sl.start]), TOL_F32)
+
+
+# ------------------------------------------------------------------------------------------------ scalar / diagonal families
+def _check_tvec(t_gpu, t_ref, tol):
+    t_gpu = t_gpu.cpu().numpy().astype(np.float64)
+    assert np.isfinite(t_gpu).all()
+    big = np.abs(t_ref) >= T_FLOOR_DIAG
+    err = np.abs(t_gpu - t_ref)[big] / np.abs(t_ref)[big]
+    worst = float(err.max()) if big.any() else 0.0
+    assert worst <= tol, f"tvec: max rel. error {worst:.3e} > {tol:.1e}"
+    if (~big).any():
+        assert np.abs(t_gpu[~big]).max() <= 2 * T_FLOOR_DIAG
+    return worst
+
+
+T_FLOOR_DIAG = 1e-30  # reading S6 carried over: below this the fp32 tvec may flush; absolute check
+
+
+@pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
+@pytest.mark.parametrize("kv,d,dv,tol", [(torch.float32, 128, 128, TOL_F32), (torch.bfloat16, 128, 128, TOL_F32),
+                                         (torch.float32, 64, 64, TOL_F32), (torch.float32, 128, 40, TOL_F32),
+                                         (torch.bfloat16, 64, 100, TOL_F32)])
+def test_diag_encode_ragged_segments(gate, kv, d, dv, tol):
+    """hypic_diag_encode (Table 1 scalar / diagonal families): ragged segments incl. empty, 1 token, a tile tail.
+    The SIMT kernel computes in fp32 from the exact input values, so bf16 inputs meet the fp32 tolerance too."""
+    lens = [70, 0, 1, 129, 16, 333, 15]
+    inp = wl.make_encode_inputs(lens, 3, d, dv, kv_dtype=kv, gate=gate, g_lo=-0.2, seed=wl.seed_for(6, 1), device="cuda")
+    E, tv = hb.hypic_diag_encode(inp.k, inp.v, inp.g, inp.cu_seqlens, inp.gate)
+    torch.cuda.synchronize()
+    assert hb.hypic_last_launch_count() == 1
+    c = inp.cpu()
+    E_ref, t_ref = oracle.diag_encode(c.k, c.v, c.g, c.cu_seqlens, gate=c.gate)
+    check_E(E, E_ref, tol, "E (diag family)")
+    _check_tvec(tv, t_ref, tol)
+    assert torch.all(E[1] == 0) and torch.all(tv[1] == 1)  # empty segment: E = 0, tvec = 1
+
+
+@pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
+def test_diag_encode_long_and_strong_decay(gate):
+    """A 5,000-token segment at the benchmark's decay (tvec ~ e^-125: far below 1 but representable) and a segment with
+    g ~ U(-30, 0): tvec underflows fp32 and E is set by the last few tokens only."""
+    for lens, g_lo in (([5000, 300], -0.05), ([200, 64], -30.0)):
+        inp = wl.make_encode_inputs(lens, 2, 128, 128, kv_dtype=torch.float32, gate=gate, g_lo=g_lo,
+                                    seed=wl.seed_for(6, 2), device="cuda")
+        E, tv = hb.hypic_diag_encode(inp.k, inp.v, inp.g, inp.cu_seqlens, inp.gate)
+        c = inp.cpu()
+        E_ref, t_ref = oracle.diag_encode(c.k, c.v, c.g, c.cu_seqlens, gate=c.gate)
+        check_E(E, E_ref, TOL_F32, f"E (g_lo={g_lo})")
+        _check_tvec(tv, t_ref, TOL_F32)
+
+
+@pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
+@pytest.mark.parametrize("d", [128, 64])
+def test_diag_compose_vs_oracle_and_sequential(gate, d):
+    """hypic_diag_compose: lists of length 0, 1 and 40 with repeated, unsorted ids; NULL and in-place S; and
+    encode -> compose in order equals the recurrence over the concatenation (oracle.diag_sequential)."""
+    P, H = 24, 3
+    lens = [int(x) for x in np.random.default_rng(61).integers(16, 65, P)]
+    pin = wl.make_encode_inputs(lens, H, d, d, kv_dtype=torch.float32, gate=gate, g_lo=-0.01, seed=wl.seed_for(6, 3),
+                                device="cuda")
+    E, tv = hb.hypic_diag_encode(pin.k, pin.v, pin.g, pin.cu_seqlens, pin.gate)
+    gen = torch.Generator().manual_seed(322)
+    ids = torch.randint(0, P, (41,), generator=gen, dtype=torch.int32).cuda()
+    cu = torch.tensor([0, 0, 1, 41], dtype=torch.int32, device="cuda")
+    S_in = torch.randn(3, H, d, d, device="cuda")
+    S = hb.hypic_diag_compose(S_in, E, tv, ids, cu)
+    torch.cuda.synchronize()
+    assert hb.hypic_last_launch_count() == 1
+    ref = oracle.diag_compose(S_in.cpu().numpy(), E.cpu().numpy(), tv.cpu().numpy(), ids.cpu().numpy(), cu.cpu().numpy())
+    check_E(S, ref, TOL_F32, "S_out (diag compose)")
+    assert torch.equal(S[0], S_in[0])
+    S0 = hb.hypic_diag_compose(None, E, tv, ids, cu)
+    ref0 = oracle.diag_compose(None, E.cpu().numpy(), tv.cpu().numpy(), ids.cpu().numpy(), cu.cpu().numpy())
+    check_E(S0, ref0, TOL_F32, "S_out (NULL S_in)")
+    S3 = S_in.clone()
+    hb.hypic_diag_compose(S3, E, tv, ids, cu, S_out=S3)
+    assert torch.equal(S3, S)
+    # all P segments in order from S_in[2] == the token recurrence over the concatenation
+    all_ids = torch.arange(P, dtype=torch.int32, device="cuda")
+    S_all = hb.hypic_diag_compose(S_in[2:3].contiguous(), E, tv, all_ids, torch.tensor([0, P], dtype=torch.int32,
+                                                                                       device="cuda"))
+    c = pin.cpu()
+    seq = oracle.diag_sequential(S_in[2:3].cpu().numpy(), c.k, c.v, c.g, np.array([0, sum(lens)], dtype=np.int32),
+                                 gate=c.gate)
+    check_E(S_all, seq, TOL_F32, "encode -> compose vs sequential")
