@@ -370,6 +370,59 @@ def time_extra_seam(hb, device, peaks, reps=20, w=8):
             "kernel_family": "simt"}
 
 
+def time_extra_diag(hb, device, peaks, iters=16):
+    """Scalar family (Table 1: RetNet / Mamba2-style scalar gate; compressed T_C of Table 3): hypic_diag_encode on one
+    cfg2-shaped layer (20 x 4096 tokens, H = 32, bf16 k/v) and hypic_diag_compose on cfg4's request lists over a
+    resident pool of P = 1024 end-states (2.1 GB) with one scalar per (segment, head)."""
+    inp = wl.cfg2_layer(0, device=device)
+    n_seg, ttot = inp.n_seg, inp.t_total
+    E = torch.empty((n_seg, H, D, D), dtype=torch.float32, device=device)
+    tv = torch.empty((n_seg, H), dtype=torch.float32, device=device)
+
+    def enc():
+        hb.hypic_diag_encode(inp.k, inp.v, inp.g, inp.cu_seqlens, hb.HYPIC_GATE_SCALAR, E=E, tvec=tv)
+
+    enc()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(3):
+        enc()
+    e1.record()
+    torch.cuda.synchronize()
+    ms_enc = e0.elapsed_time(e1) / 3
+    th = ttot * H
+    enc_gbs = th * (2 * D + 2 * D + 4) / (ms_enc * 1e-3) / 1e9
+    fam = hb.hypic_diag_encode_impl_for(H, D, D, hb.HYPIC_DT_BF16, hb.HYPIC_GATE_SCALAR)
+    del inp, E
+    E_pool = wl.cfg4_pool_E(device=device)
+    t_pool = torch.rand((E_pool.shape[0], H), device=device) * 0.5 + 0.5
+    reqs = [wl.cfg4_requests(device=device, layer=i) for i in range(iters)]
+    S_out = torch.empty_like(reqs[0].S_in)
+    for i in range(3):
+        hb.hypic_diag_compose(reqs[i].S_in, E_pool, t_pool, reqs[i].seg_ids, reqs[i].cu_segs, S_out=S_out)
+    torch.cuda.synchronize()
+    e0.record()
+    for rq in reqs:
+        hb.hypic_diag_compose(rq.S_in, E_pool, t_pool, rq.seg_ids, rq.cu_segs, S_out=S_out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    head_steps = sum(r.n_steps for r in reqs) * H
+    gbs = (head_steps * (D * D * 4 + 4) + iters * 128 * H * 2 * D * D * 4) / (ms * 1e-3) / 1e9
+    return {"workload": "scalar family: encode of one cfg2-shaped layer; compose over cfg4's request lists "
+                        f"({iters} layer-iterations, pool of 1024 end-states + one scalar each)",
+            "encode": {"ms": ms_enc, "tokens_per_s": ttot / (ms_enc * 1e-3),
+                       "kernel_family": "tensor" if fam == hb.HYPIC_IMPL_TENSOR else "simt",
+                       "roofline": {"bound": "hbm", "achieved": enc_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                    "frac": enc_gbs / peaks["hbm_gbs"], "traffic": None,
+                                    "peak_source": peaks["source"]}},
+            "compose": {"ms_total": ms, "compose_ops_per_s": head_steps / (ms * 1e-3),
+                        "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                     "frac": gbs / peaks["hbm_gbs"], "traffic": None,
+                                     "peak_source": peaks["source"]}}}
+
+
 def run_ours(args):
     from paper_2607_01299_b200 import binding as hb
 
@@ -494,6 +547,8 @@ def run_ours(args):
         extra["cfg3_encode"] = time_extra_cfg3(hb, device, peaks)
         torch.cuda.empty_cache()
         extra["seam_window"] = time_extra_seam(hb, device, peaks)
+        torch.cuda.empty_cache()
+        extra["diag_family"] = time_extra_diag(hb, device, peaks)
         extra["cfg2_compose"] = {"avg_launch_ms": cmp_avg, "compose_ops_per_s": N_SEG * H / (cmp_avg * 1e-3),
                                  "hbm_gbs": N_SEG * H * COMPOSE_BYTES_PER_STEP / (cmp_avg * 1e-3) / 1e9}
 

@@ -183,6 +183,10 @@ int hypic_diag_encode(const void* k, const void* v, const float* g, const int32_
 int hypic_diag_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,
                        const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
                        int32_t dv, int gate, float* S_out, void* stream);
+/* hypic_diag_encode_impl_for: as hypic_encode_impl_for, for hypic_diag_encode (the tcgen05 kernel covers the scalar
+ * gate with bf16 k/v at dk = dv = 128 and, like the dense tensor family, computes with fp16 operands: finite |k|, |v| <=
+ * 65504; everything else runs the fp32 CUDA-core kernel). */
+int hypic_diag_encode_impl_for(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate);
 
 /*
  * hypic_encode_impl_for / hypic_compose_impl_for: which kernel family (HYPIC_IMPL_SIMT or HYPIC_IMPL_TENSOR)

@@ -30,6 +30,7 @@ EXPORTS = (
     "hypic_status_string", "hypic_version", "hypic_last_launch_count", "hypic_encode_impl_for",
     "hypic_compose_impl_for", "hypic_debug_timeout_count", "hypic_envelope_violation_count", "hypic_compose_f16",
     "hypic_tuple_pack_f16", "hypic_seam_window", "hypic_diag_encode", "hypic_diag_compose",
+    "hypic_diag_encode_impl_for",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -75,6 +76,8 @@ def load_library() -> ctypes.CDLL:
     lib.hypic_diag_encode.restype = ctypes.c_int
     lib.hypic_diag_compose.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, ctypes.c_int, vp, vp]
     lib.hypic_diag_compose.restype = ctypes.c_int
+    lib.hypic_diag_encode_impl_for.argtypes = [i32, i32, i32, ctypes.c_int, ctypes.c_int]
+    lib.hypic_diag_encode_impl_for.restype = ctypes.c_int
     lib.hypic_status_string.argtypes = [ctypes.c_int]
     lib.hypic_status_string.restype = ctypes.c_char_p
     lib.hypic_version.argtypes = []
@@ -113,6 +116,10 @@ def hypic_get_impl() -> int:
 
 def hypic_encode_impl_for(H: int, dk: int, dv: int, kv_dtype: int, gate: int) -> int:
     return int(load_library().hypic_encode_impl_for(H, dk, dv, kv_dtype, gate))
+
+
+def hypic_diag_encode_impl_for(H: int, dk: int, dv: int, kv_dtype: int, gate: int) -> int:
+    return int(load_library().hypic_diag_encode_impl_for(H, dk, dv, kv_dtype, gate))
 
 
 def hypic_compose_impl_for(H: int, dk: int, dv: int) -> int:

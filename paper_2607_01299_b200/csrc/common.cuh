@@ -100,6 +100,8 @@ int compose_simt(const ComposeArgs& a);
 int seam_simt(const SeamArgs& a);
 int diag_encode(const DiagEncodeArgs& a);
 int diag_compose(const DiagComposeArgs& a);
+bool diag_encode_tensor_shape_ok(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate);
+int diag_encode_tensor(const DiagEncodeArgs& a);
 bool encode_tensor_shape_ok(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate);
 inline bool encode_tensor_supported(const EncodeArgs& a) {
   return encode_tensor_shape_ok(a.H, a.dk, a.dv, a.kv_dtype, a.gate);

@@ -104,6 +104,8 @@ __device__ unsigned int g_envelope_count_enc = 0;  // (chunk, head) pairs outsid
 
 #include "encode_scan2.cuh"
 
+#include "diag_scan.cuh"
+
 // k / v viewed as 3-D bf16 tensors [t_total][H][128]; box = 64 elements (128 B) x 1 head x 64 tokens, 128B swizzle:
 // the box lands as one MN-major UMMA chunk (8-token atoms of 1 KB), two boxes per 64 x 128 tile.
 typedef CUresult (*EncodeTiledFn3)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -196,6 +198,30 @@ int encode_tensor(const EncodeArgs& a) {
     note_launch();
     scan2_kernel<false><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, seg_order, a.H, rec, gate, a.E, a.T);
   }
+  note_launch();
+  HYPIC_CUDA_OK(cudaGetLastError());
+  return HYPIC_OK;
+}
+
+bool diag_encode_tensor_shape_ok(int32_t, int32_t dk, int32_t dv, int kv_dtype, int gate) {
+  return dk == kD && dv == kD && kv_dtype == HYPIC_DT_BF16 && gate == HYPIC_GATE_SCALAR;
+}
+
+// Scalar family on the tensor cores (diag_scan.cuh).  t_total > 0 (the tensor maps need a non-empty tensor).
+int diag_encode_tensor(const DiagEncodeArgs& a) {
+  if (!diag_encode_tensor_shape_ok(a.H, a.dk, a.dv, a.kv_dtype, a.gate) || a.t_total <= 0) return HYPIC_ERR_UNSUPPORTED;
+  if (a.n_seg == 0) return HYPIC_OK;
+  if (a.H > 65535 || a.n_seg > 65535) return HYPIC_ERR_UNSUPPORTED;
+  static bool configured = false;
+  if (!configured) {
+    HYPIC_CUDA_OK(cudaFuncSetAttribute(diag_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDtSmem));
+    configured = true;
+  }
+  CUtensorMap tmK, tmV;
+  int rc = make_kv_tensor_map(&tmK, a.k, a.t_total, a.H);
+  if (rc == HYPIC_OK) rc = make_kv_tensor_map(&tmV, a.v, a.t_total, a.H);
+  if (rc != HYPIC_OK) return rc;
+  diag_scan_kernel<<<dim3(a.H, a.n_seg), kDtThreads, kDtSmem, a.stream>>>(tmK, tmV, a.g, a.cu_seqlens, a.H, a.E, a.tvec);
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
   return HYPIC_OK;

@@ -157,7 +157,21 @@ int hypic_diag_encode(const void* k, const void* v, const float* g, const int32_
   if (t_total > 0 && (!k || !v || !g)) return HYPIC_ERR_INVALID_ARG;
   if (!aligned16(k) || !aligned16(v) || !aligned16(g) || !aligned16(E) || !aligned16(tvec)) return HYPIC_ERR_INVALID_ARG;
   DiagEncodeArgs a{k, v, g, cu_seqlens, n_seg, t_total, H, dk, dv, kv_dtype, gate, E, tvec, (cudaStream_t)stream};
+  const int impl = g_impl.load();
+  const bool tensor_ok = diag_encode_tensor_shape_ok(H, dk, dv, kv_dtype, gate);
+  if (impl == HYPIC_IMPL_TENSOR && !tensor_ok) return HYPIC_ERR_UNSUPPORTED;
+  if (tensor_ok && impl != HYPIC_IMPL_SIMT && t_total > 0) return diag_encode_tensor(a);
   return diag_encode(a);
+}
+
+int hypic_diag_encode_impl_for(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate) {
+  const int vs = validate_encode_shape(0, 0, H, dk, dv, kv_dtype, gate);
+  if (vs != HYPIC_OK) return -vs;
+  const int impl = g_impl.load();
+  const bool tensor_ok = diag_encode_tensor_shape_ok(H, dk, dv, kv_dtype, gate);
+  if (impl == HYPIC_IMPL_TENSOR) return tensor_ok ? HYPIC_IMPL_TENSOR : -HYPIC_ERR_UNSUPPORTED;
+  if (impl == HYPIC_IMPL_SIMT) return HYPIC_IMPL_SIMT;
+  return tensor_ok ? HYPIC_IMPL_TENSOR : HYPIC_IMPL_SIMT;
 }
 
 int hypic_diag_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,

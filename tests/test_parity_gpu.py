@@ -535,23 +535,58 @@ def _check_tvec(t_gpu, t_ref, tol):
 T_FLOOR_DIAG = 1e-30  # reading S6 carried over: below this the fp32 tvec may flush; absolute check
 
 
+def _diag_tol(inp, impl):
+    """fp32 CUDA-core kernel: 1e-5 whatever the input dtype (inputs are exact); tcgen05 kernel (fp16 operands): 3e-3."""
+    kv = hb.HYPIC_DT_BF16 if inp.k.dtype == torch.bfloat16 else hb.HYPIC_DT_F32
+    hb.hypic_set_impl(impl)
+    fam = hb.hypic_diag_encode_impl_for(inp.H, inp.dk, inp.dv, kv, inp.gate)
+    hb.hypic_set_impl(hb.HYPIC_IMPL_AUTO)
+    if fam < 0:
+        pytest.skip("tensor family does not cover this shape")
+    return TOL_BF16 if fam == hb.HYPIC_IMPL_TENSOR else TOL_F32
+
+
+def gpu_diag_encode(inp, impl):
+    with impl_family(impl):
+        E, tv = hb.hypic_diag_encode(inp.k, inp.v, inp.g, inp.cu_seqlens, inp.gate)
+        torch.cuda.synchronize()
+    return E, tv
+
+
+@pytest.mark.parametrize("name,impl", IMPLS)
 @pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
-@pytest.mark.parametrize("kv,d,dv,tol", [(torch.float32, 128, 128, TOL_F32), (torch.bfloat16, 128, 128, TOL_F32),
-                                         (torch.float32, 64, 64, TOL_F32), (torch.float32, 128, 40, TOL_F32),
-                                         (torch.bfloat16, 64, 100, TOL_F32)])
-def test_diag_encode_ragged_segments(gate, kv, d, dv, tol):
-    """hypic_diag_encode (Table 1 scalar / diagonal families): ragged segments incl. empty, 1 token, a tile tail.
-    The SIMT kernel computes in fp32 from the exact input values, so bf16 inputs meet the fp32 tolerance too."""
-    lens = [70, 0, 1, 129, 16, 333, 15]
+@pytest.mark.parametrize("kv,d,dv", [(torch.float32, 128, 128), (torch.bfloat16, 128, 128), (torch.float32, 64, 64),
+                                     (torch.float32, 128, 40), (torch.bfloat16, 64, 100)])
+def test_diag_encode_ragged_segments(name, impl, gate, kv, d, dv):
+    """hypic_diag_encode (Table 1 scalar / diagonal families): ragged segments incl. empty, 1 token, chunk tails, for
+    every kernel family that covers the shape."""
+    lens = [70, 0, 1, 129, 16, 333, 15, 64, 200]
     inp = wl.make_encode_inputs(lens, 3, d, dv, kv_dtype=kv, gate=gate, g_lo=-0.2, seed=wl.seed_for(6, 1), device="cuda")
-    E, tv = hb.hypic_diag_encode(inp.k, inp.v, inp.g, inp.cu_seqlens, inp.gate)
-    torch.cuda.synchronize()
+    tol = _diag_tol(inp, impl)
+    E, tv = gpu_diag_encode(inp, impl)
     assert hb.hypic_last_launch_count() == 1
     c = inp.cpu()
     E_ref, t_ref = oracle.diag_encode(c.k, c.v, c.g, c.cu_seqlens, gate=c.gate)
     check_E(E, E_ref, tol, "E (diag family)")
-    _check_tvec(tv, t_ref, tol)
+    _check_tvec(tv, t_ref, TOL_F32)
     assert torch.all(E[1] == 0) and torch.all(tv[1] == 1)  # empty segment: E = 0, tvec = 1
+
+
+def test_diag_encode_tensor_cfg2_layer_sampled_units():
+    """The launch bench.py times for the scalar family (one cfg2-shaped layer: 20 x 4096 tokens, H = 32, bf16) on the
+    tcgen05 kernel: sampled (segment, head) units against the oracle, every tvec against the fp64 sum."""
+    inp = wl.cfg2_layer(3, device="cuda")
+    assert hb.hypic_diag_encode_impl_for(inp.H, 128, 128, hb.HYPIC_DT_BF16, wl.GATE_SCALAR) == hb.HYPIC_IMPL_TENSOR
+    E, tv = gpu_diag_encode(inp, hb.HYPIC_IMPL_AUTO)
+    assert torch.isfinite(E).all()
+    cu = inp.cu_seqlens.cpu().numpy()
+    t_ref = np.stack([np.exp(inp.g[cu[s]:cu[s + 1]].double().sum(0).cpu().numpy()) for s in range(inp.n_seg)])
+    _check_tvec(tv, t_ref, TOL_F32)
+    for s, h in _sample_units(inp.n_seg, inp.H, 5, 11):
+        u = inp.unit(s, h)
+        E_ref, _ = oracle.diag_encode(u.k, u.v, u.g, u.cu_seqlens, gate=u.gate)
+        check_E(E[s:s + 1, h:h + 1], E_ref, TOL_BF16, "E (scalar family, tensor)")
+    assert hb.hypic_debug_timeout_count() == 0
 
 
 @pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
