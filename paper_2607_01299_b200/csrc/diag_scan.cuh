@@ -10,9 +10,9 @@
 // runs on tcgen05 (the fp32 CUDA-core kernel of diag_family.cu is FMA-bound, six times slower).
 //
 // Roles of a CTA (192 threads, one (segment, head) unit, two CTAs per SM, 128 TMEM columns each):
-//   warp 5      loader      TMA boxes of the bf16 K and V chunk tiles (64 tokens x 128 channels each), 3 stages
-//   warps 0-3   converters  weights of the chunk (warp 0: shuffle suffix scan of g, fp64 carry), then in place:
-//                           K~ = fp16(w_t k_t), V -> fp16, rows past the end of the segment zeroed; epilogue
+//   warp 5      loader      TMA boxes of the bf16 K and V chunk tiles (64 tokens x 128 channels each), 3 stages, and the
+//                           chunk's token weights (shuffle suffix scan of g, fp64 carry) -- up to 3 chunks ahead
+//   warps 0-3   converters  in place: K~ = fp16(w_t k_t), V -> fp16, rows past the end of the segment zeroed; epilogue
 //   warp 4      issuer      4 x tcgen05.mma (M = dv = 128, N = dk = 128, K = 16 tokens) per chunk, both operands
 //                           MN-major straight from the swizzled boxes; accumulator E (fp32) stays in TMEM throughout
 #pragma once
@@ -30,7 +30,24 @@ struct DtBars {
   int abort_flag;
 };
 
-__device__ __forceinline__ void named_bar_sync128(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
+// Single-thread wait of the loader / issuer: mbarrier.try_wait already suspends the thread for a hardware-chosen time, so
+// a plain retry loop reacts within tens of cycles; s2_wait's __nanosleep back-off (measured here: the loader woke up
+// ~2,400 cycles after the stage had been freed, once per chunk) is only the bounded fallback.
+__device__ __forceinline__ void dt_wait(uint64_t* bar, uint32_t parity, volatile int* abort_flag) {
+#pragma unroll 1
+  for (int i = 0; i < 4096; ++i)
+    if (mbar_try_wait(bar, parity)) return;
+  s2_wait(bar, parity, abort_flag);
+}
+
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
 
 __global__ void __launch_bounds__(kDtThreads, 2)
     diag_scan_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
@@ -56,7 +73,7 @@ __global__ void __launch_bounds__(kDtThreads, 2)
   if (warp == 4) tmem_alloc(&bars->tmem_base, 128);
   if (tid == 0) {
     for (int i = 0; i < kDtStages; ++i) {
-      mbar_init(&bars->full[i], 1);
+      mbar_init(&bars->full[i], 2);  // TMA bytes (expect_tx arrival) + the loader warp's weights
       mbar_init(&bars->conv[i], 4);
       mbar_init(&bars->free_[i], 1);
     }
@@ -71,21 +88,68 @@ __global__ void __launch_bounds__(kDtThreads, 2)
   const uint32_t smem_base = smem_u32(smem);
 
   if (warp == 5) {
-    // ----------------------------------------------------------------------------------------------- loader
-    if (lane == 0) {
+    // ------------------------------------------------------------------------------- loader + token weights
+    // Runs up to kDtStages chunks ahead of the converters, so neither the TMA latency nor the latency of the g loads
+    // sits on anybody's critical path.  full[st] completes on the TMA bytes AND this warp's second arrival (weights).
+    double carry = 0.0;   // log-decay of all tokens after the current chunk
+    double lane_sum = 0.0;  // this lane's share of the segment's total log-decay, fp64 (tvec sums thousands of terms)
+    // g of tokens 2 lane, 2 lane + 1 of a chunk, loaded two chunks ahead of its use
+    auto load_g = [&](int i, float& ga, float& gb) {
+      ga = gb = 0.f;
+      if (i < nc) {
+        const int ta = seg_begin + (nc - 1 - i) * kC + 2 * lane;
+        if (ta < seg_end) ga = __ldg(g + (size_t)ta * H + h);
+        if (ta + 1 < seg_end) gb = __ldg(g + (size_t)(ta + 1) * H + h);
+      }
+    };
+    float ga0, gb0, ga1, gb1;
+    load_g(0, ga0, gb0);
+    load_g(1, ga1, gb1);
 #pragma unroll 1
-      for (int i = 0; i < nc; ++i) {
-        const int st = i % kDtStages;
-        if (i >= kDtStages) s2_wait(&bars->free_[st], ((i / kDtStages) & 1) ^ 1, abort_flag);
+    for (int i = 0; i < nc; ++i) {
+      const int st = i % kDtStages;
+      const int t0 = seg_begin + (nc - 1 - i) * kC;  // last chunk first
+      const int ta = t0 + 2 * lane, tb = ta + 1;
+      S2_STAMPW(5, 0, i, 2);
+      const float ga = ga0, gb = gb0;
+      ga0 = ga1, gb0 = gb1;
+      load_g(i + 2, ga1, gb1);
+      S2_STAMPW(5, 0, i, 3);
+      if (i >= kDtStages) {
+        if (lane == 0) dt_wait(&bars->free_[st], ((i / kDtStages) & 1) ^ 1, abort_flag);
+        __syncwarp();
+      }
+      S2_STAMPW(5, 0, i, 0);
+      if (lane == 0) {
         const uint32_t sb = smem_base + st * kDtStageBytes;
-        const int t0 = seg_begin + (nc - 1 - i) * kC;  // last chunk first
         mbar_expect_tx(&bars->full[st], (uint32_t)kDtStageBytes);
         tma_load_3d(sb, &tmK, 0, h, t0, &bars->full[st]);
         tma_load_3d(sb + 8192, &tmK, 64, h, t0, &bars->full[st]);
         tma_load_3d(sb + 16384, &tmV, 0, h, t0, &bars->full[st]);
         tma_load_3d(sb + 24576, &tmV, 64, h, t0, &bars->full[st]);
       }
+      // exclusive suffix sums of g inside the chunk by a shuffle scan over the lane pairs
+      float suf = ga + gb;  // becomes the inclusive suffix sum over lanes >= lane
+#pragma unroll
+      for (int d = 1; d < 32; d *= 2) {
+        const float up = __shfl_down_sync(0xffffffffu, suf, d);
+        if (lane + d < 32) suf += up;
+      }
+      const float tot = __shfl_sync(0xffffffffu, suf, 0);
+      const float excl = suf - (ga + gb);  // tokens of the lanes above
+      const float cf = (float)carry;
+      float* w = sw + st * 64;
+      w[2 * lane + 1] = tb < seg_end ? __expf(cf + excl) : 0.f;
+      w[2 * lane] = ta < seg_end ? __expf(cf + excl + gb) : 0.f;
+      carry += (double)tot;
+      lane_sum += (double)ga + (double)gb;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars->full[st]);
+      S2_STAMPW(5, 0, i, 1);
     }
+#pragma unroll
+    for (int d = 16; d > 0; d /= 2) lane_sum += __shfl_xor_sync(0xffffffffu, lane_sum, d);
+    if (lane == 0) tvec[(size_t)s * H + h] = (float)exp(lane_sum);
   } else if (warp == 4) {
     // ----------------------------------------------------------------------------------------------- MMA issuer
     if (lane == 0) {
@@ -93,68 +157,47 @@ __global__ void __launch_bounds__(kDtThreads, 2)
 #pragma unroll 1
       for (int i = 0; i < nc; ++i) {
         const int st = i % kDtStages;
-        s2_wait(&bars->conv[st], (i / kDtStages) & 1, abort_flag);
+        dt_wait(&bars->conv[st], (i / kDtStages) & 1, abort_flag);
         tc_fence_after();
+        S2_STAMPW(4, 2, i, 0);
         const uint32_t sb = smem_base + st * kDtStageBytes;
 #pragma unroll
         for (int ks = 0; ks < 4; ++ks)
           mma_f16_ss(tmem, make_desc(sb + 16384 + ks * 2048, 8192, 1024, 2), make_desc(sb + ks * 2048, 8192, 1024, 2),
                      idesc, (i > 0 || ks > 0) ? 1u : 0u);
         mma_commit(&bars->free_[st]);
+        S2_STAMPW(4, 2, i, 1);
       }
       mma_commit(&bars->done);
     }
   } else {
     // ----------------------------------------------------------------------------------------------- converters
-    double carry = 0.0;  // warp 0: log-decay of all tokens after the current chunk (fp64: up to thousands of terms)
 #pragma unroll 1
     for (int i = 0; i < nc; ++i) {
       const int st = i % kDtStages;
       const int t0 = seg_begin + (nc - 1 - i) * kC;
-      float* w = sw + st * 64;
-      if (warp == 0) {
-        // tokens 2 lane, 2 lane + 1 of the chunk; exclusive suffix sums by a shuffle scan over the lane pairs
-        const int ta = t0 + 2 * lane, tb = ta + 1;
-        const float ga = ta < seg_end ? __ldg(g + (size_t)ta * H + h) : 0.f;
-        const float gb = tb < seg_end ? __ldg(g + (size_t)tb * H + h) : 0.f;
-        float suf = ga + gb;  // becomes the inclusive suffix sum over lanes >= lane
-        double tot = (double)ga + (double)gb;
-#pragma unroll
-        for (int d = 1; d < 32; d *= 2) {
-          const float up = __shfl_down_sync(0xffffffffu, suf, d);
-          const double upd = __shfl_xor_sync(0xffffffffu, tot, d);
-          if (lane + d < 32) suf += up;
-          tot += upd;
-        }
-        const float excl = suf - (ga + gb);  // tokens of the lanes above
-        const float cf = (float)carry;
-        // the stage's weights were read by the conversion of chunk i - kDtStages, which this warp finished long ago
-        w[2 * lane + 1] = tb < seg_end ? __expf(cf + excl) : 0.f;
-        w[2 * lane] = ta < seg_end ? __expf(cf + excl + gb) : 0.f;
-        carry += tot;
-      }
-      named_bar_sync128(1);
       s2_wait_warp(&bars->full[st], (i / kDtStages) & 1, abort_flag, lane);
-      uint4* tile = reinterpret_cast<uint4*>(smem + st * kDtStageBytes);
+      S2_STAMPW(0, 1, i, 0);
+      const float* w = sw + st * 64;
+      const uint32_t tile = smem_base + st * kDtStageBytes;
       // 2,048 16-byte vectors: K boxes [0, 1024), V boxes [1024, 2048); vector idx of a box sits in token row (idx % 512) / 8
-#pragma unroll 4
+#pragma unroll 8
       for (int it = 0; it < 16; ++it) {
         const int idx = it * 128 + tid;
         const int tok = (idx & 511) >> 3;
         const float m = it < 8 ? w[tok] : 1.f;
-        uint4 x = tile[idx];
+        uint4 x = lds128(tile + 16 * idx);
         x.x = pack_f16(m * __uint_as_float(x.x << 16), m * __uint_as_float(x.x & 0xffff0000u));
         x.y = pack_f16(m * __uint_as_float(x.y << 16), m * __uint_as_float(x.y & 0xffff0000u));
         x.z = pack_f16(m * __uint_as_float(x.z << 16), m * __uint_as_float(x.z & 0xffff0000u));
         x.w = pack_f16(m * __uint_as_float(x.w << 16), m * __uint_as_float(x.w & 0xffff0000u));
         if (t0 + tok >= seg_end) x = make_uint4(0u, 0u, 0u, 0u);  // rows past the segment hold other tokens' data
-        tile[idx] = x;
+        sts128(tile + 16 * idx, x);
       }
       fence_proxy_async();
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars->conv[st]);
-      // w[st] is rewritten kDtStages chunks later, behind at least one more named barrier that every converter only
-      // reaches after this conversion
+      S2_STAMPW(0, 1, i, 1);
     }
     // ----------------------------------------------------------------------------------------------- epilogue
     s2_wait_warp(&bars->done, 0, abort_flag, lane);
@@ -171,7 +214,6 @@ __global__ void __launch_bounds__(kDtThreads, 2)
         dst[8 * cb + u] = make_float4(__uint_as_float(x[4 * u]), __uint_as_float(x[4 * u + 1]), __uint_as_float(x[4 * u + 2]),
                                       __uint_as_float(x[4 * u + 3]));
     }
-    if (tid == 0) tvec[(size_t)s * H + h] = (float)exp(carry);
   }
   tc_fence_before();
   __syncthreads();
