@@ -9,15 +9,16 @@
 // 32,768 flop per token-head against 516 B of k, v, g: 64 flop/B, i.e. HBM-bound on B200 as long as the contraction
 // runs on tcgen05 (the fp32 CUDA-core kernel of diag_family.cu is FMA-bound, six times slower).
 //
-// Roles of a CTA (192 threads, one (segment, head) unit, two CTAs per SM, 128 TMEM columns each):
-//   warp 5      loader      TMA boxes of the bf16 K and V chunk tiles (64 tokens x 128 channels each), 3 stages, and the
+// Roles of a CTA (320 threads, one (segment, head) unit, two CTAs per SM, 128 TMEM columns each):
+//   warp 9      loader      TMA boxes of the bf16 K and V chunk tiles (64 tokens x 128 channels each), 3 stages, and the
 //                           chunk's token weights (shuffle suffix scan of g, fp64 carry) -- up to 3 chunks ahead
-//   warps 0-3   converters  in place: K~ = fp16(w_t k_t), V -> fp16, rows past the end of the segment zeroed; epilogue
-//   warp 4      issuer      4 x tcgen05.mma (M = dv = 128, N = dk = 128, K = 16 tokens) per chunk, both operands
+//   warps 0-7   converters  in place: K~ = fp16(w_t k_t), V -> fp16, rows past the end of the segment zeroed; epilogue
+//   warp 8      issuer      4 x tcgen05.mma (M = dv = 128, N = dk = 128, K = 16 tokens) per chunk, both operands
 //                           MN-major straight from the swizzled boxes; accumulator E (fp32) stays in TMEM throughout
 #pragma once
 
-constexpr int kDtThreads = 192;
+constexpr int kDtConvWarps = 8;
+constexpr int kDtThreads = 32 * (kDtConvWarps + 2);  // converters, then the MMA issuer warp, then the loader warp
 constexpr int kDtStages = 3;
 constexpr int kDtStageBytes = 32768;  // K tile (2 boxes of 8 KB) + V tile
 constexpr int kDtOffW = kDtStages * kDtStageBytes;        // per-stage token weights: float[kDtStages][64]
@@ -70,11 +71,11 @@ __global__ void __launch_bounds__(kDtThreads, 2)
     return;
   }
 
-  if (warp == 4) tmem_alloc(&bars->tmem_base, 128);
+  if (warp == kDtConvWarps) tmem_alloc(&bars->tmem_base, 128);
   if (tid == 0) {
     for (int i = 0; i < kDtStages; ++i) {
       mbar_init(&bars->full[i], 2);  // TMA bytes (expect_tx arrival) + the loader warp's weights
-      mbar_init(&bars->conv[i], 4);
+      mbar_init(&bars->conv[i], kDtConvWarps);
       mbar_init(&bars->free_[i], 1);
     }
     mbar_init(&bars->done, 1);
@@ -87,7 +88,7 @@ __global__ void __launch_bounds__(kDtThreads, 2)
   const uint32_t tmem = bars->tmem_base;
   const uint32_t smem_base = smem_u32(smem);
 
-  if (warp == 5) {
+  if (warp == kDtConvWarps + 1) {
     // ------------------------------------------------------------------------------- loader + token weights
     // Runs up to kDtStages chunks ahead of the converters, so neither the TMA latency nor the latency of the g loads
     // sits on anybody's critical path.  full[st] completes on the TMA bytes AND this warp's second arrival (weights).
@@ -110,16 +111,16 @@ __global__ void __launch_bounds__(kDtThreads, 2)
       const int st = i % kDtStages;
       const int t0 = seg_begin + (nc - 1 - i) * kC;  // last chunk first
       const int ta = t0 + 2 * lane, tb = ta + 1;
-      S2_STAMPW(5, 0, i, 2);
+      S2_STAMPW(kDtConvWarps + 1, 0, i, 2);
       const float ga = ga0, gb = gb0;
       ga0 = ga1, gb0 = gb1;
       load_g(i + 2, ga1, gb1);
-      S2_STAMPW(5, 0, i, 3);
+      S2_STAMPW(kDtConvWarps + 1, 0, i, 3);
       if (i >= kDtStages) {
         if (lane == 0) dt_wait(&bars->free_[st], ((i / kDtStages) & 1) ^ 1, abort_flag);
         __syncwarp();
       }
-      S2_STAMPW(5, 0, i, 0);
+      S2_STAMPW(kDtConvWarps + 1, 0, i, 0);
       if (lane == 0) {
         const uint32_t sb = smem_base + st * kDtStageBytes;
         mbar_expect_tx(&bars->full[st], (uint32_t)kDtStageBytes);
@@ -145,12 +146,12 @@ __global__ void __launch_bounds__(kDtThreads, 2)
       lane_sum += (double)ga + (double)gb;
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars->full[st]);
-      S2_STAMPW(5, 0, i, 1);
+      S2_STAMPW(kDtConvWarps + 1, 0, i, 1);
     }
 #pragma unroll
     for (int d = 16; d > 0; d /= 2) lane_sum += __shfl_xor_sync(0xffffffffu, lane_sum, d);
     if (lane == 0) tvec[(size_t)s * H + h] = (float)exp(lane_sum);
-  } else if (warp == 4) {
+  } else if (warp == kDtConvWarps) {
     // ----------------------------------------------------------------------------------------------- MMA issuer
     if (lane == 0) {
       constexpr uint32_t idesc = make_idesc(0u, 128, 128, 1, 1);  // fp16 x fp16 -> fp32, A (V tile) and B (K~ tile) MN-major
@@ -159,14 +160,14 @@ __global__ void __launch_bounds__(kDtThreads, 2)
         const int st = i % kDtStages;
         dt_wait(&bars->conv[st], (i / kDtStages) & 1, abort_flag);
         tc_fence_after();
-        S2_STAMPW(4, 2, i, 0);
+        S2_STAMPW(kDtConvWarps, 2, i, 0);
         const uint32_t sb = smem_base + st * kDtStageBytes;
 #pragma unroll
         for (int ks = 0; ks < 4; ++ks)
           mma_f16_ss(tmem, make_desc(sb + 16384 + ks * 2048, 8192, 1024, 2), make_desc(sb + ks * 2048, 8192, 1024, 2),
                      idesc, (i > 0 || ks > 0) ? 1u : 0u);
         mma_commit(&bars->free_[st]);
-        S2_STAMPW(4, 2, i, 1);
+        S2_STAMPW(kDtConvWarps, 2, i, 1);
       }
       mma_commit(&bars->done);
     }
@@ -181,11 +182,12 @@ __global__ void __launch_bounds__(kDtThreads, 2)
       const float* w = sw + st * 64;
       const uint32_t tile = smem_base + st * kDtStageBytes;
       // 2,048 16-byte vectors: K boxes [0, 1024), V boxes [1024, 2048); vector idx of a box sits in token row (idx % 512) / 8
-#pragma unroll 8
-      for (int it = 0; it < 16; ++it) {
-        const int idx = it * 128 + tid;
+      constexpr int kConvThreads = 32 * kDtConvWarps;
+#pragma unroll
+      for (int it = 0; it < 2048 / kConvThreads; ++it) {
+        const int idx = it * kConvThreads + tid;
         const int tok = (idx & 511) >> 3;
-        const float m = it < 8 ? w[tok] : 1.f;
+        const float m = it < 1024 / kConvThreads ? w[tok] : 1.f;
         uint4 x = lds128(tile + 16 * idx);
         x.x = pack_f16(m * __uint_as_float(x.x << 16), m * __uint_as_float(x.x & 0xffff0000u));
         x.y = pack_f16(m * __uint_as_float(x.y << 16), m * __uint_as_float(x.y & 0xffff0000u));
@@ -202,12 +204,14 @@ __global__ void __launch_bounds__(kDtThreads, 2)
     // ----------------------------------------------------------------------------------------------- epilogue
     s2_wait_warp(&bars->done, 0, abort_flag, lane);
     tc_fence_after();
-    const int row = 32 * warp + lane;  // dv index = TMEM lane
-    float4* dst = reinterpret_cast<float4*>(Eu + (size_t)row * kD);
+    const int q = warp & 3, hf = warp >> 2;  // TMEM lane quarter of this warp; column slice (two warps per quarter)
+    const int row = 32 * q + lane;           // dv index = TMEM lane
+    constexpr int kColsPerWarp = kD / (kDtConvWarps / 4);
+    float4* dst = reinterpret_cast<float4*>(Eu + (size_t)row * kD + kColsPerWarp * hf);
 #pragma unroll 1
-    for (int cb = 0; cb < 4; ++cb) {
+    for (int cb = 0; cb < kColsPerWarp / 32; ++cb) {
       uint32_t x[32];
-      tmem_ld32(tmem + ((uint32_t)(32 * warp) << 16) + 32 * cb, x);
+      tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + kColsPerWarp * hf + 32 * cb, x);
       tmem_ld_wait();
 #pragma unroll
       for (int u = 0; u < 8; ++u)
@@ -217,5 +221,5 @@ __global__ void __launch_bounds__(kDtThreads, 2)
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 4) tmem_dealloc(tmem, 128);
+  if (warp == kDtConvWarps) tmem_dealloc(tmem, 128);
 }
