@@ -19,7 +19,7 @@
 
 constexpr int kDtConvWarps = 8;
 constexpr int kDtThreads = 32 * (kDtConvWarps + 2);  // converters, then the MMA issuer warp, then the loader warp
-constexpr int kDtStages = 3;
+constexpr int kDtStages = 2;
 constexpr int kDtStageBytes = 32768;  // K tile (2 boxes of 8 KB) + V tile
 constexpr int kDtOffW = kDtStages * kDtStageBytes;        // per-stage token weights: float[kDtStages][64]
 constexpr int kDtOffBar = kDtOffW + kDtStages * 64 * 4;
@@ -50,7 +50,7 @@ __device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
   asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
-__global__ void __launch_bounds__(kDtThreads, 2)
+__global__ void __launch_bounds__(kDtThreads, 3)
     diag_scan_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
                      const float* __restrict__ g, const int32_t* __restrict__ cu_seqlens, int H, float* __restrict__ E,
                      float* __restrict__ tvec) {
