@@ -35,7 +35,7 @@ __global__ void __launch_bounds__(kDgRows)
   __shared__ __align__(16) float sk[2][kDgTT][DK];   // pre-weighted keys of the tile
   __shared__ __align__(16) float sdec[2][AW];        // decay over the whole tile
   __shared__ float sw[2][kDgTT][kDgRows];            // this CTA's value entries v_t[i]
-  __shared__ float sg[kDgTT][AW];                    // log-decays of the tile being staged
+  __shared__ __align__(16) float sg[kDgTT][CHANNEL ? DK : 4];  // log-decays of the tile being staged
 
   const int tid = threadIdx.x;
   const int h = blockIdx.y, s = blockIdx.z;
@@ -52,20 +52,54 @@ __global__ void __launch_bounds__(kDgRows)
   // and c + 64.
   double gsum0 = 0.0, gsum1 = 0.0;
 
+  // Staging of one tile: every global load of the tile is issued before anything waits (k stays in registers, raw,
+  // across the suffix-sum phase), so a tile costs one global round trip, not one per element.
+  constexpr int KV8 = kDgTT * DK / 8 / kDgRows;  // 8-channel groups of k per thread
+  constexpr int GV4 = CHANNEL ? kDgTT * DK / 4 / kDgRows : 1;
   auto stage = [&](int buf, int tile) {
     const int tbase = t_begin + tile * kDgTT;
     const int n_tok = min(kDgTT, t_end - tbase);
-    // log-decays of the tile -> shared memory (zeros past the end of the segment)
-    for (int idx = tid; idx < kDgTT * AW; idx += kDgRows) {
-      const int tok = idx / AW, c = idx % AW;
-      sg[tok][c] = tok < n_tok ? g[((size_t)(tbase + tok) * H + h) * AW + c] : 0.f;
+    uint4 kraw[KV8][BF16 ? 1 : 2];
+#pragma unroll
+    for (int n = 0; n < KV8; ++n) {
+      const int e8 = tid + n * kDgRows;
+      const int tok = (e8 * 8) / DK, c0 = (e8 * 8) % DK;
+#pragma unroll
+      for (int u = 0; u < (BF16 ? 1 : 2); ++u) kraw[n][u] = make_uint4(0u, 0u, 0u, 0u);
+      if (tok < n_tok) {
+        const size_t e0 = ((size_t)(tbase + tok) * H + h) * DK + c0;
+        if (BF16) {
+          kraw[n][0] = __ldg(reinterpret_cast<const uint4*>(reinterpret_cast<const __nv_bfloat16*>(k) + e0));
+        } else {
+#pragma unroll
+          for (int u = 0; u < (BF16 ? 1 : 2); ++u)
+            kraw[n][u] = __ldg(reinterpret_cast<const uint4*>(reinterpret_cast<const float*>(k) + e0) + u);
+        }
+      }
     }
-    for (int idx = tid; idx < kDgTT * kDgRows; idx += kDgRows) {
-      const int tok = idx / kDgRows, j = idx % kDgRows;
-      float wv = 0.f;
-      if (tok < n_tok && row0 + j < dv) wv = dg_load<BF16>(v, ((size_t)(tbase + tok) * H + h) * dv + row0 + j);
-      sw[buf][tok][j] = wv;
+    float vraw[kDgTT];
+#pragma unroll
+    for (int tok = 0; tok < kDgTT; ++tok)
+      vraw[tok] = (tok < n_tok && row < dv) ? dg_load<BF16>(v, ((size_t)(tbase + tok) * H + h) * dv + row) : 0.f;
+    if (CHANNEL) {
+      float4 graw[GV4];
+#pragma unroll
+      for (int n = 0; n < GV4; ++n) {
+        const int e4 = tid + n * kDgRows;
+        const int tok = (e4 * 4) / DK, c0 = (e4 * 4) % DK;
+        graw[n] = tok < n_tok ? __ldg(reinterpret_cast<const float4*>(g + ((size_t)(tbase + tok) * H + h) * DK + c0))
+                              : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int n = 0; n < GV4; ++n) {
+        const int e4 = tid + n * kDgRows;
+        *reinterpret_cast<float4*>(&sg[(e4 * 4) / DK][(e4 * 4) % DK]) = graw[n];
+      }
+    } else if (tid < kDgTT) {
+      sg[tid][0] = tid < n_tok ? g[(size_t)(tbase + tid) * H + h] : 0.f;
     }
+#pragma unroll
+    for (int tok = 0; tok < kDgTT; ++tok) sw[buf][tok][tid] = vraw[tok];
     __syncthreads();
     // suffix sums inside the tile, one thread per channel (or thread 0): weight of token t = exp(sum_{s > t} g_s)
     for (int c = tid; c < AW; c += kDgRows) {
@@ -82,11 +116,39 @@ __global__ void __launch_bounds__(kDgRows)
       if (c < kDgRows) gsum0 += acc; else gsum1 += acc;
     }
     __syncthreads();
-    for (int idx = tid; idx < kDgTT * DK; idx += kDgRows) {
-      const int tok = idx / DK, c = idx % DK;
-      float kv = 0.f;
-      if (tok < n_tok) kv = dg_load<BF16>(k, ((size_t)(tbase + tok) * H + h) * DK + c) * expf(sg[tok][CHANNEL ? c : 0]);
-      sk[buf][tok][c] = kv;
+#pragma unroll
+    for (int n = 0; n < KV8; ++n) {
+      const int e8 = tid + n * kDgRows;
+      const int tok = (e8 * 8) / DK, c0 = (e8 * 8) % DK;
+      float kv[8];
+      if (BF16) {
+        const uint32_t w4[4] = {kraw[n][0].x, kraw[n][0].y, kraw[n][0].z, kraw[n][0].w};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          kv[2 * u] = __uint_as_float(w4[u] << 16);
+          kv[2 * u + 1] = __uint_as_float(w4[u] & 0xffff0000u);
+        }
+      } else {
+#pragma unroll
+        for (int u = 0; u < (BF16 ? 1 : 2); ++u) {
+          kv[4 * u] = __uint_as_float(kraw[n][u].x), kv[4 * u + 1] = __uint_as_float(kraw[n][u].y);
+          kv[4 * u + 2] = __uint_as_float(kraw[n][u].z), kv[4 * u + 3] = __uint_as_float(kraw[n][u].w);
+        }
+      }
+      float wt[8];
+      if (CHANNEL) {
+        const float4 l0 = *reinterpret_cast<const float4*>(&sg[tok][c0]);
+        const float4 l1 = *reinterpret_cast<const float4*>(&sg[tok][c0 + 4]);
+        wt[0] = expf(l0.x), wt[1] = expf(l0.y), wt[2] = expf(l0.z), wt[3] = expf(l0.w);
+        wt[4] = expf(l1.x), wt[5] = expf(l1.y), wt[6] = expf(l1.z), wt[7] = expf(l1.w);
+      } else {
+        const float w1 = expf(sg[tok][0]);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) wt[u] = w1;
+      }
+      float4* d4 = reinterpret_cast<float4*>(&sk[buf][tok][c0]);
+      d4[0] = make_float4(kv[0] * wt[0], kv[1] * wt[1], kv[2] * wt[2], kv[3] * wt[3]);
+      d4[1] = make_float4(kv[4] * wt[4], kv[5] * wt[5], kv[6] * wt[6], kv[7] * wt[7]);
     }
   };
 
