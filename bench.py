@@ -394,6 +394,25 @@ def time_extra_diag(hb, device, peaks, iters=16):
     th = ttot * H
     enc_gbs = th * (2 * D + 2 * D + 4) / (ms_enc * 1e-3) / 1e9
     fam = hb.hypic_diag_encode_impl_for(H, D, D, hb.HYPIC_DT_BF16, hb.HYPIC_GATE_SCALAR)
+    del inp
+    # diagonal family (GLA): the same layer shape with a per-channel gate (1,028 B per token-head)
+    inp = wl.make_encode_inputs([4096] * 20, H, D, D, kv_dtype=torch.bfloat16, gate=wl.GATE_CHANNEL, g_lo=-0.05,
+                                seed=wl.seed_for(6, 0), device=device)
+    tvc = torch.empty((n_seg, H, D), dtype=torch.float32, device=device)
+
+    def enc_ch():
+        hb.hypic_diag_encode(inp.k, inp.v, inp.g, inp.cu_seqlens, hb.HYPIC_GATE_CHANNEL, E=E, tvec=tvc)
+
+    enc_ch()
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(3):
+        enc_ch()
+    e1.record()
+    torch.cuda.synchronize()
+    ms_ch = e0.elapsed_time(e1) / 3
+    ch_gbs = th * (2 * D + 2 * D + 4 * D) / (ms_ch * 1e-3) / 1e9
+    fam_ch = hb.hypic_diag_encode_impl_for(H, D, D, hb.HYPIC_DT_BF16, hb.HYPIC_GATE_CHANNEL)
     del inp, E
     E_pool = wl.cfg4_pool_E(device=device)
     t_pool = torch.rand((E_pool.shape[0], H), device=device) * 0.5 + 0.5
@@ -410,13 +429,18 @@ def time_extra_diag(hb, device, peaks, iters=16):
     ms = e0.elapsed_time(e1)
     head_steps = sum(r.n_steps for r in reqs) * H
     gbs = (head_steps * (D * D * 4 + 4) + iters * 128 * H * 2 * D * D * 4) / (ms * 1e-3) / 1e9
-    return {"workload": "scalar family: encode of one cfg2-shaped layer; compose over cfg4's request lists "
+    return {"workload": "scalar / diagonal families: encode of one cfg2-shaped layer; compose over cfg4's request lists "
                         f"({iters} layer-iterations, pool of 1024 end-states + one scalar each)",
             "encode": {"ms": ms_enc, "tokens_per_s": ttot / (ms_enc * 1e-3),
                        "kernel_family": "tensor" if fam == hb.HYPIC_IMPL_TENSOR else "simt",
                        "roofline": {"bound": "hbm", "achieved": enc_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                     "frac": enc_gbs / peaks["hbm_gbs"], "traffic": None,
                                     "peak_source": peaks["source"]}},
+            "encode_diagonal": {"ms": ms_ch, "tokens_per_s": ttot / (ms_ch * 1e-3),
+                                "kernel_family": "tensor" if fam_ch == hb.HYPIC_IMPL_TENSOR else "simt",
+                                "roofline": {"bound": "hbm", "achieved": ch_gbs, "peak": peaks["hbm_gbs"],
+                                             "unit": "GB/s", "frac": ch_gbs / peaks["hbm_gbs"], "traffic": None,
+                                             "peak_source": peaks["source"]}},
             "compose": {"ms_total": ms, "compose_ops_per_s": head_steps / (ms * 1e-3),
                         "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                      "frac": gbs / peaks["hbm_gbs"], "traffic": None,

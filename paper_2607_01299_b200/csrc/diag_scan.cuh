@@ -223,3 +223,203 @@ __global__ void __launch_bounds__(kDtThreads, 3)
   __syncthreads();
   if (warp == kDtConvWarps) tmem_dealloc(tmem, 128);
 }
+
+
+// ------------------------------------------------------------------------------------------------------------------
+// Diagonal family (GLA: T_i = diag(g_i)): the same reverse-streamed contraction with per-channel weights,
+//     E[i, c] = sum_t v_t[i] k_t[c] w_t[c],   w_t[c] = exp(sum_{s > t} g_s[c]),   tvec[c] = exp(sum_t g_t[c]).
+// The K / V tiles arrive by TMA as above; the 32 KB of fp32 log-decays per chunk are read straight from global memory by
+// the converter threads, one chunk ahead, into registers: thread (pair p, range r) owns channels 2p, 2p+1 of tokens
+// [16 r, 16 r + 16) of the chunk, scans its 16 tokens backwards, gets the totals of the later ranges through shared
+// memory (one named barrier per chunk), and folds exp(.) into its 16 x 2 entries of the K tile with 32-bit accesses.
+struct DtChShared {
+  float2 tot[2][4][64];   // [chunk parity][token range][channel pair]: log-decay summed over the range
+  double dsum[4][64][2];  // end of the segment: fp64 partial sums per (range, pair, channel of the pair)
+};
+constexpr int kDtChOffX = kDtOffBar + 128;
+constexpr int kDtChSmem = kDtChOffX + (int)sizeof(DtChShared) + 1024;
+
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void sts32(uint32_t addr, uint32_t v) {
+  asm volatile("st.shared.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+
+__global__ void __launch_bounds__(kDtThreads, 2)
+    diag_scan_ch_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                        const float* __restrict__ g, const int32_t* __restrict__ cu_seqlens, int H, float* __restrict__ E,
+                        float* __restrict__ tvec) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  DtBars* bars = reinterpret_cast<DtBars*>(smem + kDtOffBar);
+  DtChShared* xs = reinterpret_cast<DtChShared*>(smem + kDtChOffX);
+  volatile int* abort_flag = &bars->abort_flag;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int h = blockIdx.x, s = blockIdx.y;
+  const int seg_begin = cu_seqlens[s], seg_end = cu_seqlens[s + 1];
+  const int nc = (seg_end - seg_begin + kC - 1) / kC;
+  float* Eu = E + ((size_t)s * H + h) * kD * kD;
+  float* tv = tvec + ((size_t)s * H + h) * kD;
+
+  if (nc == 0) {  // empty segment: E = 0, tvec = 1
+    for (int i = tid; i < kD * kD / 4; i += kDtThreads) reinterpret_cast<float4*>(Eu)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (tid < kD) tv[tid] = 1.f;
+    return;
+  }
+
+  if (warp == kDtConvWarps) tmem_alloc(&bars->tmem_base, 128);
+  if (tid == 0) {
+    for (int i = 0; i < kDtStages; ++i) {
+      mbar_init(&bars->full[i], 1);
+      mbar_init(&bars->conv[i], kDtConvWarps);
+      mbar_init(&bars->free_[i], 1);
+    }
+    mbar_init(&bars->done, 1);
+    bars->abort_flag = 0;
+    fence_barrier_init();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = bars->tmem_base;
+  const uint32_t smem_base = smem_u32(smem);
+
+  if (warp == kDtConvWarps + 1) {
+    // ----------------------------------------------------------------------------------------------- loader
+    if (lane == 0) {
+#pragma unroll 1
+      for (int i = 0; i < nc; ++i) {
+        const int st = i % kDtStages;
+        if (i >= kDtStages) dt_wait(&bars->free_[st], ((i / kDtStages) & 1) ^ 1, abort_flag);
+        const uint32_t sb = smem_base + st * kDtStageBytes;
+        const int t0 = seg_begin + (nc - 1 - i) * kC;  // last chunk first
+        mbar_expect_tx(&bars->full[st], (uint32_t)kDtStageBytes);
+        tma_load_3d(sb, &tmK, 0, h, t0, &bars->full[st]);
+        tma_load_3d(sb + 8192, &tmK, 64, h, t0, &bars->full[st]);
+        tma_load_3d(sb + 16384, &tmV, 0, h, t0, &bars->full[st]);
+        tma_load_3d(sb + 24576, &tmV, 64, h, t0, &bars->full[st]);
+      }
+    }
+  } else if (warp == kDtConvWarps) {
+    // ----------------------------------------------------------------------------------------------- MMA issuer
+    if (lane == 0) {
+      constexpr uint32_t idesc = make_idesc(0u, 128, 128, 1, 1);
+#pragma unroll 1
+      for (int i = 0; i < nc; ++i) {
+        const int st = i % kDtStages;
+        dt_wait(&bars->conv[st], (i / kDtStages) & 1, abort_flag);
+        tc_fence_after();
+        const uint32_t sb = smem_base + st * kDtStageBytes;
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks)
+          mma_f16_ss(tmem, make_desc(sb + 16384 + ks * 2048, 8192, 1024, 2), make_desc(sb + ks * 2048, 8192, 1024, 2),
+                     idesc, (i > 0 || ks > 0) ? 1u : 0u);
+        mma_commit(&bars->free_[st]);
+      }
+      mma_commit(&bars->done);
+    }
+  } else {
+    // ----------------------------------------------------------------------------------------------- converters
+    static_assert(kDtConvWarps == 8, "thread map below: 64 channel pairs x 4 token ranges");
+    const int p = tid & 63, r = tid >> 6;
+    double carry0 = 0.0, carry1 = 0.0;  // log-decay of all tokens after the current chunk, channels 2p and 2p + 1
+    double dsum0 = 0.0, dsum1 = 0.0;    // this thread's tokens only, for tvec
+    float2 gn[16];
+    auto load_g = [&](int i) {
+      const int tb = seg_begin + (nc - 1 - i) * kC + 16 * r;
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        gn[j] = make_float2(0.f, 0.f);
+        if (i < nc && tb + j < seg_end) gn[j] = __ldg(reinterpret_cast<const float2*>(g + ((size_t)(tb + j) * H + h) * kD) + p);
+      }
+    };
+    load_g(0);
+    // K tile address of (token row 16 r + j, channel pair p): box p / 32, 128-byte rows, 16-byte chunks XOR-swizzled by row
+    const uint32_t k_box = (uint32_t)(p >> 5) * 8192u, k_chunk = (uint32_t)((p & 31) >> 2), k_in = (uint32_t)(p & 3) * 4u;
+#pragma unroll 1
+    for (int i = 0; i < nc; ++i) {
+      const int st = i % kDtStages;
+      const int t0 = seg_begin + (nc - 1 - i) * kC;
+      float lw0[16], lw1[16];
+      float s0 = 0.f, s1 = 0.f;
+#pragma unroll
+      for (int j = 15; j >= 0; --j) {  // exclusive suffix sums inside this thread's 16 tokens
+        lw0[j] = s0, lw1[j] = s1;
+        s0 += gn[j].x, s1 += gn[j].y;
+        dsum0 += (double)gn[j].x, dsum1 += (double)gn[j].y;
+      }
+      xs->tot[i & 1][r][p] = make_float2(s0, s1);
+      load_g(i + 1);  // next chunk's log-decays: in flight during this chunk's conversion
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      float later0 = 0.f, later1 = 0.f, all0 = 0.f, all1 = 0.f;
+#pragma unroll
+      for (int rr = 3; rr >= 0; --rr) {
+        const float2 t = xs->tot[i & 1][rr][p];
+        if (rr > r) later0 += t.x, later1 += t.y;
+        all0 += t.x, all1 += t.y;
+      }
+      const float b0 = (float)carry0 + later0, b1 = (float)carry1 + later1;
+      carry0 += (double)all0, carry1 += (double)all1;
+      s2_wait_warp(&bars->full[st], (i / kDtStages) & 1, abort_flag, lane);
+      const uint32_t tile = smem_base + st * kDtStageBytes;
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        const int tr = 16 * r + j;
+        const uint32_t addr = tile + k_box + (uint32_t)tr * 128u + ((k_chunk ^ (uint32_t)(tr & 7)) << 4) + k_in;
+        const uint32_t x = lds32(addr);
+        uint32_t y = 0u;
+        if (t0 + tr < seg_end)
+          y = pack_f16(__uint_as_float(x << 16) * __expf(b0 + lw0[j]), __uint_as_float(x & 0xffff0000u) * __expf(b1 + lw1[j]));
+        sts32(addr, y);
+      }
+      // V tile: bf16 -> fp16 in place, rows past the segment zeroed
+#pragma unroll
+      for (int it = 0; it < 4; ++it) {
+        const int idx = 1024 + it * 256 + tid;
+        const int tok = (idx & 511) >> 3;
+        uint4 x = lds128(tile + 16 * idx);
+        x.x = pack_f16(__uint_as_float(x.x << 16), __uint_as_float(x.x & 0xffff0000u));
+        x.y = pack_f16(__uint_as_float(x.y << 16), __uint_as_float(x.y & 0xffff0000u));
+        x.z = pack_f16(__uint_as_float(x.z << 16), __uint_as_float(x.z & 0xffff0000u));
+        x.w = pack_f16(__uint_as_float(x.w << 16), __uint_as_float(x.w & 0xffff0000u));
+        if (t0 + tok >= seg_end) x = make_uint4(0u, 0u, 0u, 0u);
+        sts128(tile + 16 * idx, x);
+      }
+      fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars->conv[st]);
+    }
+    // tvec: fp64 sums of the four token ranges of every channel
+    xs->dsum[r][p][0] = dsum0;
+    xs->dsum[r][p][1] = dsum1;
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    if (r == 0) {
+      const double a0 = xs->dsum[0][p][0] + xs->dsum[1][p][0] + xs->dsum[2][p][0] + xs->dsum[3][p][0];
+      const double a1 = xs->dsum[0][p][1] + xs->dsum[1][p][1] + xs->dsum[2][p][1] + xs->dsum[3][p][1];
+      *reinterpret_cast<float2*>(tv + 2 * p) = make_float2((float)exp(a0), (float)exp(a1));
+    }
+    // ----------------------------------------------------------------------------------------------- epilogue
+    s2_wait_warp(&bars->done, 0, abort_flag, lane);
+    tc_fence_after();
+    const int q = warp & 3, hf = warp >> 2;
+    const int row = 32 * q + lane;
+    constexpr int kColsPerWarp = kD / (kDtConvWarps / 4);
+    float4* dst = reinterpret_cast<float4*>(Eu + (size_t)row * kD + kColsPerWarp * hf);
+#pragma unroll 1
+    for (int cb = 0; cb < kColsPerWarp / 32; ++cb) {
+      uint32_t x[32];
+      tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + kColsPerWarp * hf + 32 * cb, x);
+      tmem_ld_wait();
+#pragma unroll
+      for (int u = 0; u < 8; ++u)
+        dst[8 * cb + u] = make_float4(__uint_as_float(x[4 * u]), __uint_as_float(x[4 * u + 1]), __uint_as_float(x[4 * u + 2]),
+                                      __uint_as_float(x[4 * u + 3]));
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == kDtConvWarps) tmem_dealloc(tmem, 128);
+}

@@ -204,7 +204,7 @@ int encode_tensor(const EncodeArgs& a) {
 }
 
 bool diag_encode_tensor_shape_ok(int32_t, int32_t dk, int32_t dv, int kv_dtype, int gate) {
-  return dk == kD && dv == kD && kv_dtype == HYPIC_DT_BF16 && gate == HYPIC_GATE_SCALAR;
+  return dk == kD && dv == kD && kv_dtype == HYPIC_DT_BF16 && (gate == HYPIC_GATE_SCALAR || gate == HYPIC_GATE_CHANNEL);
 }
 
 // Scalar family on the tensor cores (diag_scan.cuh).  t_total > 0 (the tensor maps need a non-empty tensor).
@@ -215,13 +215,18 @@ int diag_encode_tensor(const DiagEncodeArgs& a) {
   static bool configured = false;
   if (!configured) {
     HYPIC_CUDA_OK(cudaFuncSetAttribute(diag_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDtSmem));
+    HYPIC_CUDA_OK(cudaFuncSetAttribute(diag_scan_ch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDtChSmem));
     configured = true;
   }
   CUtensorMap tmK, tmV;
   int rc = make_kv_tensor_map(&tmK, a.k, a.t_total, a.H);
   if (rc == HYPIC_OK) rc = make_kv_tensor_map(&tmV, a.v, a.t_total, a.H);
   if (rc != HYPIC_OK) return rc;
-  diag_scan_kernel<<<dim3(a.H, a.n_seg), kDtThreads, kDtSmem, a.stream>>>(tmK, tmV, a.g, a.cu_seqlens, a.H, a.E, a.tvec);
+  if (a.gate == HYPIC_GATE_CHANNEL)
+    diag_scan_ch_kernel<<<dim3(a.H, a.n_seg), kDtThreads, kDtChSmem, a.stream>>>(tmK, tmV, a.g, a.cu_seqlens, a.H, a.E,
+                                                                                a.tvec);
+  else
+    diag_scan_kernel<<<dim3(a.H, a.n_seg), kDtThreads, kDtSmem, a.stream>>>(tmK, tmV, a.g, a.cu_seqlens, a.H, a.E, a.tvec);
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
   return HYPIC_OK;

@@ -572,6 +572,22 @@ def test_diag_encode_ragged_segments(name, impl, gate, kv, d, dv):
     assert torch.all(E[1] == 0) and torch.all(tv[1] == 1)  # empty segment: E = 0, tvec = 1
 
 
+def test_diag_encode_tensor_channel_gate_full_size_sampled_units():
+    """Diagonal family (GLA) on the tcgen05 kernel at the bench shape (20 x 4096 tokens, H = 32, per-channel gate with a
+    milder decay so that tvec stays representable): sampled units against the oracle, tvec of those units included."""
+    inp = wl.make_encode_inputs([4096] * 20, 32, 128, 128, kv_dtype=torch.bfloat16, gate=wl.GATE_CHANNEL, g_lo=-0.01,
+                                seed=wl.seed_for(6, 4), device="cuda")
+    assert hb.hypic_diag_encode_impl_for(32, 128, 128, hb.HYPIC_DT_BF16, wl.GATE_CHANNEL) == hb.HYPIC_IMPL_TENSOR
+    E, tv = gpu_diag_encode(inp, hb.HYPIC_IMPL_AUTO)
+    assert torch.isfinite(E).all() and torch.isfinite(tv).all()
+    for s, h in _sample_units(inp.n_seg, inp.H, 4, 12):
+        u = inp.unit(s, h)
+        E_ref, t_ref = oracle.diag_encode(u.k, u.v, u.g, u.cu_seqlens, gate=u.gate)
+        check_E(E[s:s + 1, h:h + 1], E_ref, TOL_BF16, "E (diagonal family, tensor)")
+        _check_tvec(tv[s:s + 1, h:h + 1], t_ref, TOL_F32)
+    assert hb.hypic_debug_timeout_count() == 0
+
+
 def test_diag_encode_tensor_cfg2_layer_sampled_units():
     """The launch bench.py times for the scalar family (one cfg2-shaped layer: 20 x 4096 tokens, H = 32, bf16) on the
     tcgen05 kernel: sampled (segment, head) units against the oracle, every tvec against the fp64 sum."""
