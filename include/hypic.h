@@ -169,8 +169,9 @@ int hypic_seam_window(const void* q, const void* k, const void* v, const float* 
  * diagonal for HYPIC_GATE_CHANNEL.
  *   k [t_total,H,dk], v [t_total,H,dv] kv_dtype; g [t_total,H] or [t_total,H,dk] fp32 log-decay; cu_seqlens as in
  *   hypic_segment_encode; E out [n_seg,H,dv,dk] fp32; tvec out [n_seg,H] or [n_seg,H,dk] fp32.
- * A zero-length segment yields E = 0, tvec = 1.  Built envelope: dk in {64, 128}, dv in [1, 1024], any gate value
- * (the pre-weighting inside the kernel only multiplies by factors in (0, 1] when g <= 0).  No workspace.
+ * A zero-length segment yields E = 0, tvec = 1.  Built envelope: dk in {64, 128}, dv in [1, 1024] (the pre-weighting
+ * inside the kernels only multiplies by factors in (0, 1] when g <= 0).  No workspace.  Kernel family as selected by
+ * hypic_set_impl, see hypic_diag_encode_impl_for.
  *
  * hypic_diag_compose: S <- S diag(tvec_i) + E_i (Eq. 6 with Table 3's "element-wise scaling" apply step;
  * HYPIC_GATE_SCALAR: S <- tvec_i S + E_i) over each request's ordered id list; arguments as hypic_compose with
@@ -183,9 +184,10 @@ int hypic_diag_encode(const void* k, const void* v, const float* g, const int32_
 int hypic_diag_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,
                        const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
                        int32_t dv, int gate, float* S_out, void* stream);
-/* hypic_diag_encode_impl_for: as hypic_encode_impl_for, for hypic_diag_encode (the tcgen05 kernel covers the scalar
- * gate with bf16 k/v at dk = dv = 128 and, like the dense tensor family, computes with fp16 operands: finite |k|, |v| <=
- * 65504; everything else runs the fp32 CUDA-core kernel). */
+/* hypic_diag_encode_impl_for: as hypic_encode_impl_for, for hypic_diag_encode.  The tcgen05 kernels cover bf16 k/v at
+ * dk = dv = 128 for both gates; like the dense tensor family they compute with fp16 operands (finite |k|, |v| <= 65504,
+ * g <= 0 so that every weight is <= 1; result within 3e-3 of the oracle, tvec within 1e-5); everything else, and
+ * HYPIC_IMPL_SIMT, runs the fp32 CUDA-core kernel (1e-5). */
 int hypic_diag_encode_impl_for(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate);
 
 /*
