@@ -429,7 +429,23 @@ def time_extra_diag(hb, device, peaks, iters=16):
     ms = e0.elapsed_time(e1)
     head_steps = sum(r.n_steps for r in reqs) * H
     gbs = (head_steps * (D * D * 4 + 4) + iters * 128 * H * 2 * D * D * 4) / (ms * 1e-3) / 1e9
-    return {"workload": "scalar / diagonal families: encode of one cfg2-shaped layer; compose over cfg4's request lists "
+    Eh = hb.hypic_tuple_pack_f16(E_pool)
+    del E_pool
+    for i in range(3):
+        hb.hypic_diag_compose(reqs[i].S_in, Eh, t_pool, reqs[i].seg_ids, reqs[i].cu_segs, S_out=S_out)
+    torch.cuda.synchronize()
+    e0.record()
+    for rq in reqs:
+        hb.hypic_diag_compose(rq.S_in, Eh, t_pool, rq.seg_ids, rq.cu_segs, S_out=S_out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms16 = e0.elapsed_time(e1)
+    gbs16 = (head_steps * (D * D * 2 + 4) + iters * 128 * H * 2 * D * D * 4) / (ms16 * 1e-3) / 1e9
+    return {"compose_f16": {"ms_total": ms16, "compose_ops_per_s": head_steps / (ms16 * 1e-3),
+                            "roofline": {"bound": "hbm", "achieved": gbs16, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                         "frac": gbs16 / peaks["hbm_gbs"], "traffic": None,
+                                         "peak_source": peaks["source"]}},
+            "workload": "scalar / diagonal families: encode of one cfg2-shaped layer; compose over cfg4's request lists "
                         f"({iters} layer-iterations, pool of 1024 end-states + one scalar each)",
             "encode": {"ms": ms_enc, "tokens_per_s": ttot / (ms_enc * 1e-3),
                        "kernel_family": "tensor" if fam == hb.HYPIC_IMPL_TENSOR else "simt",

@@ -184,6 +184,12 @@ int hypic_diag_encode(const void* k, const void* v, const float* g, const int32_
 int hypic_diag_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,
                        const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
                        int32_t dv, int gate, float* S_out, void* stream);
+/* hypic_diag_compose_f16: hypic_diag_compose over end-states stored in fp16 (hypic_tuple_pack_f16 of hypic_diag_encode's
+ * E; the paper's cache precision): E_pool [P,H,dv,dk] fp16, taken as exact inputs; t_pool stays fp32
+ * (4 B or 4 dk B per tuple: there is nothing to save, and a decay product rounded to fp16 would cost 5e-4 per step). */
+int hypic_diag_compose_f16(const float* S_in, const void* E_pool, const float* t_pool, const int32_t* seg_ids,
+                           const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
+                           int32_t dv, int gate, float* S_out, void* stream);
 /* hypic_diag_encode_impl_for: as hypic_encode_impl_for, for hypic_diag_encode.  The tcgen05 kernels cover bf16 k/v at
  * dk = dv = 128 for both gates; like the dense tensor family they compute with fp16 operands (finite |k|, |v| <= 65504,
  * g <= 0 so that every weight is <= 1; result within 3e-3 of the oracle, tvec within 1e-5); everything else, and

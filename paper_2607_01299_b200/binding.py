@@ -30,7 +30,7 @@ EXPORTS = (
     "hypic_status_string", "hypic_version", "hypic_last_launch_count", "hypic_encode_impl_for",
     "hypic_compose_impl_for", "hypic_debug_timeout_count", "hypic_envelope_violation_count", "hypic_compose_f16",
     "hypic_tuple_pack_f16", "hypic_seam_window", "hypic_diag_encode", "hypic_diag_compose",
-    "hypic_diag_encode_impl_for",
+    "hypic_diag_encode_impl_for", "hypic_diag_compose_f16",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -76,6 +76,8 @@ def load_library() -> ctypes.CDLL:
     lib.hypic_diag_encode.restype = ctypes.c_int
     lib.hypic_diag_compose.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, ctypes.c_int, vp, vp]
     lib.hypic_diag_compose.restype = ctypes.c_int
+    lib.hypic_diag_compose_f16.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, ctypes.c_int, vp, vp]
+    lib.hypic_diag_compose_f16.restype = ctypes.c_int
     lib.hypic_diag_encode_impl_for.argtypes = [i32, i32, i32, ctypes.c_int, ctypes.c_int]
     lib.hypic_diag_encode_impl_for.restype = ctypes.c_int
     lib.hypic_status_string.argtypes = [ctypes.c_int]
@@ -396,7 +398,7 @@ def hypic_diag_compose(S_in: Optional[torch.Tensor], E_pool: torch.Tensor, t_poo
                        S_out: Optional[torch.Tensor] = None,
                        stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
     """S_out[r,h] = fold of S <- S diag(t_i) + E_i over seg_ids[cu_segs[r]:cu_segs[r+1]] from S_in[r,h] (None = 0);
-    t_pool:[P,H] (scalar family) or [P,H,dk] (diagonal family)."""
+    t_pool:[P,H] (scalar family) or [P,H,dk] (diagonal family), fp32.  E_pool fp32, or fp16 (hypic_diag_compose_f16)."""
     lib = load_library()
     for name, t in (("E_pool", E_pool), ("t_pool", t_pool), ("seg_ids", seg_ids), ("cu_segs", cu_segs)):
         if not t.is_cuda:
@@ -421,9 +423,11 @@ def hypic_diag_compose(S_in: Optional[torch.Tensor], E_pool: torch.Tensor, t_poo
         S_out = torch.empty((R, H, dv, dk), dtype=torch.float32, device=E_pool.device)
     if tuple(S_out.shape) != (R, H, dv, dk):
         raise ValueError("S_out must be [R,H,dv,dk]")
+    f16 = E_pool.dtype == torch.float16
+    fn = lib.hypic_diag_compose_f16 if f16 else lib.hypic_diag_compose
     with torch.cuda.device(E_pool.device):
-        rc = lib.hypic_diag_compose(
-            _dev_ptr(S_in, "S_in", torch.float32), _dev_ptr(E_pool, "E_pool", torch.float32),
+        rc = fn(
+            _dev_ptr(S_in, "S_in", torch.float32), _dev_ptr(E_pool, "E_pool", torch.float16 if f16 else torch.float32),
             _dev_ptr(t_pool, "t_pool", torch.float32), _dev_ptr(seg_ids, "seg_ids", torch.int32),
             _dev_ptr(cu_segs, "cu_segs", torch.int32), R, P, int(total_steps), H, dk, dv, gate,
             _dev_ptr(S_out, "S_out", torch.float32), _stream_handle(stream))

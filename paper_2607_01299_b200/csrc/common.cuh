@@ -84,12 +84,13 @@ struct DiagEncodeArgs {
 
 struct DiagComposeArgs {
   const float* S_in;
-  const float* E_pool;
+  const void* E_pool;  // fp32, or fp16 when e_f16
   const float* t_pool;
   const int32_t* seg_ids;
   const int32_t* cu_segs;
   int32_t R, P, total_steps, H, dk, dv;
   int gate;
+  int e_f16;
   float* S_out;
   cudaStream_t stream;
 };

@@ -12,6 +12,8 @@
 //   the log-decay summed in fp64 (4,096 fp32 terms would cost 1e-5 in fp32).
 // diag_compose_kernel: the fold is element-wise, so every thread owns 4 float4s of S for the whole chain and streams
 //   the E_i of its request through registers, one step prefetched ahead: bound by reading E_i from HBM.
+#include <cuda_fp16.h>
+
 #include "common.cuh"
 
 namespace hypic {
@@ -224,9 +226,9 @@ int dg_dispatch(const DiagEncodeArgs& a) {
 constexpr int kDcThreads = 256;
 constexpr int kDcV4 = 4;  // float4s of S per thread: a CTA owns 4,096 consecutive elements of one (request, head)
 
-template <bool CHANNEL>
+template <bool CHANNEL, bool F16>
 __global__ void __launch_bounds__(kDcThreads)
-    diag_compose_kernel(const float* __restrict__ S_in, const float* __restrict__ E_pool,
+    diag_compose_kernel(const float* __restrict__ S_in, const void* __restrict__ E_pool,
                         const float* __restrict__ t_pool, const int32_t* __restrict__ seg_ids,
                         const int32_t* __restrict__ cu_segs, int H, int dk, int unit_v4, float* __restrict__ S_out) {
   const int tid = threadIdx.x;
@@ -250,11 +252,16 @@ __global__ void __launch_bounds__(kDcThreads)
   float4 e_nxt[kDcV4], t_nxt[kDcV4];
   auto fetch = [&](int j) {
     const size_t ph = (size_t)seg_ids[j] * H + h;
-    const float4* Ei = reinterpret_cast<const float4*>(E_pool) + ph * unit_v4;
 #pragma unroll
     for (int i = 0; i < kDcV4; ++i) {
       if (live[i]) {
-        e_nxt[i] = __ldcs(Ei + e4[i]);
+        if (F16) {  // fp16-stored end-states (the paper's cache precision): exact inputs; kept raw in
+                    // the prefetch registers and widened at use, so the load is not consumed one instruction later
+          const uint2 hv = __ldcs(reinterpret_cast<const uint2*>(E_pool) + ph * unit_v4 + e4[i]);
+          e_nxt[i] = make_float4(__uint_as_float(hv.x), __uint_as_float(hv.y), 0.f, 0.f);
+        } else {
+          e_nxt[i] = __ldcs(reinterpret_cast<const float4*>(E_pool) + ph * unit_v4 + e4[i]);
+        }
         if (CHANNEL) {
           t_nxt[i] = __ldg(reinterpret_cast<const float4*>(t_pool + ph * dk) + e4[i] % dk4);
         } else {
@@ -272,6 +279,12 @@ __global__ void __launch_bounds__(kDcThreads)
     if (j + 1 < j1) fetch(j + 1);
 #pragma unroll
     for (int i = 0; i < kDcV4; ++i) {
+      if (F16) {
+        const uint32_t w0 = __float_as_uint(e_cur[i].x), w1 = __float_as_uint(e_cur[i].y);
+        const float2 lo = __half22float2(*reinterpret_cast<const __half2*>(&w0));
+        const float2 hi = __half22float2(*reinterpret_cast<const __half2*>(&w1));
+        e_cur[i] = make_float4(lo.x, lo.y, hi.x, hi.y);
+      }
       x[i].x = fmaf(x[i].x, t_cur[i].x, e_cur[i].x);
       x[i].y = fmaf(x[i].y, t_cur[i].y, e_cur[i].y);
       x[i].z = fmaf(x[i].z, t_cur[i].z, e_cur[i].z);
@@ -300,12 +313,10 @@ int diag_compose(const DiagComposeArgs& a) {
   if (a.R == 0) return HYPIC_OK;
   const int unit_v4 = a.dv * a.dk / 4;
   dim3 grid((unit_v4 + kDcThreads * kDcV4 - 1) / (kDcThreads * kDcV4), a.H, a.R);
-  if (a.gate == HYPIC_GATE_CHANNEL)
-    diag_compose_kernel<true><<<grid, kDcThreads, 0, a.stream>>>(a.S_in, a.E_pool, a.t_pool, a.seg_ids, a.cu_segs, a.H,
-                                                                 a.dk, unit_v4, a.S_out);
-  else
-    diag_compose_kernel<false><<<grid, kDcThreads, 0, a.stream>>>(a.S_in, a.E_pool, a.t_pool, a.seg_ids, a.cu_segs, a.H,
-                                                                  a.dk, unit_v4, a.S_out);
+  const bool ch = a.gate == HYPIC_GATE_CHANNEL;
+  auto kern = a.e_f16 ? (ch ? diag_compose_kernel<true, true> : diag_compose_kernel<false, true>)
+                      : (ch ? diag_compose_kernel<true, false> : diag_compose_kernel<false, false>);
+  kern<<<grid, kDcThreads, 0, a.stream>>>(a.S_in, a.E_pool, a.t_pool, a.seg_ids, a.cu_segs, a.H, a.dk, unit_v4, a.S_out);
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
   return HYPIC_OK;

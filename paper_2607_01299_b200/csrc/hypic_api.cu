@@ -174,9 +174,9 @@ int hypic_diag_encode_impl_for(int32_t H, int32_t dk, int32_t dv, int kv_dtype, 
   return tensor_ok ? HYPIC_IMPL_TENSOR : HYPIC_IMPL_SIMT;
 }
 
-int hypic_diag_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,
-                       const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
-                       int32_t dv, int gate, float* S_out, void* stream) {
+static int diag_compose_call(const float* S_in, const void* E_pool, int e_f16, const float* t_pool, const int32_t* seg_ids,
+                             const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
+                             int32_t dv, int gate, float* S_out, void* stream) {
   g_launch_count = 0;
   if (R < 0 || P < 0 || total_steps < 0 || H <= 0 || dk <= 0 || dv <= 0) return HYPIC_ERR_INVALID_ARG;
   if (gate != HYPIC_GATE_SCALAR && gate != HYPIC_GATE_CHANNEL) return HYPIC_ERR_INVALID_ARG;
@@ -185,9 +185,21 @@ int hypic_diag_compose(const float* S_in, const float* E_pool, const float* t_po
   if (total_steps > 0 && (!E_pool || !t_pool || !seg_ids || P == 0)) return HYPIC_ERR_INVALID_ARG;
   if (!aligned16(S_in) || !aligned16(E_pool) || !aligned16(t_pool) || !aligned16(S_out)) return HYPIC_ERR_INVALID_ARG;
   if (dk % 4 != 0 || dk > 1024 || dv > 1024) return HYPIC_ERR_UNSUPPORTED;
-  DiagComposeArgs a{S_in, E_pool, t_pool, seg_ids, cu_segs, R, P, total_steps, H, dk, dv, gate, S_out,
+  DiagComposeArgs a{S_in, E_pool, t_pool, seg_ids, cu_segs, R, P, total_steps, H, dk, dv, gate, e_f16, S_out,
                     (cudaStream_t)stream};
   return diag_compose(a);
+}
+
+int hypic_diag_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,
+                       const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
+                       int32_t dv, int gate, float* S_out, void* stream) {
+  return diag_compose_call(S_in, E_pool, 0, t_pool, seg_ids, cu_segs, R, P, total_steps, H, dk, dv, gate, S_out, stream);
+}
+
+int hypic_diag_compose_f16(const float* S_in, const void* E_pool, const float* t_pool, const int32_t* seg_ids,
+                           const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
+                           int32_t dv, int gate, float* S_out, void* stream) {
+  return diag_compose_call(S_in, E_pool, 1, t_pool, seg_ids, cu_segs, R, P, total_steps, H, dk, dv, gate, S_out, stream);
 }
 
 int hypic_encode_impl_for(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate) {

@@ -645,6 +645,12 @@ def test_diag_compose_vs_oracle_and_sequential(gate, d):
     S3 = S_in.clone()
     hb.hypic_diag_compose(S3, E, tv, ids, cu, S_out=S3)
     assert torch.equal(S3, S)
+    # fp16-stored end-states are exact inputs: fold of the stored values to the fp32-input tolerance
+    Eh = hb.hypic_tuple_pack_f16(E)
+    Sh = hb.hypic_diag_compose(S_in, Eh, tv, ids, cu)
+    refh = oracle.diag_compose(S_in.cpu().numpy(), Eh.float().cpu().numpy(), tv.cpu().numpy(), ids.cpu().numpy(),
+                               cu.cpu().numpy())
+    check_E(Sh, refh, TOL_F32, "S_out (diag compose, fp16 end-states)")
     # all P segments in order from S_in[2] == the token recurrence over the concatenation
     all_ids = torch.arange(P, dtype=torch.int32, device="cuda")
     S_all = hb.hypic_diag_compose(S_in[2:3].contiguous(), E, tv, all_ids, torch.tensor([0, P], dtype=torch.int32,
