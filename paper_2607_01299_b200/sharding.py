@@ -8,6 +8,10 @@ communication is the timing reduction (max over ranks) that bench.py reports.
   (Eq. 9: min over assignments of the max per-worker token count).
 * ``head_range`` -- contiguous split of the head axis for compose-only workloads.
 * ``max_over_ranks`` -- device- or host-side MAX all-reduce of a timing, on whatever backend the group uses.
+* ``exchange_tuples`` -- the one real exchange step of segment parallelism (scatter workers
+  ship their segments' ``(T_C, S_{C|0})`` to where the state is assembled), in its data-parallel form: encode is sharded
+  by segments (LPT), compose by heads, so the tuples make one all-to-all between the two layouts.  Pure data movement
+  (``torch.distributed.all_to_all_single`` over NCCL on GPUs, gloo in the CPU tests); no arithmetic.
 """
 from __future__ import annotations
 
@@ -54,3 +58,53 @@ def max_over_ranks(value: float, device: Optional[torch.device] = None, group=No
     t = torch.tensor([float(value)], dtype=torch.float64, device=device if device is not None else "cpu")
     dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
     return float(t.item())
+
+
+def exchange_tuples(E_loc: torch.Tensor, T_loc: torch.Tensor, parts: Sequence[Sequence[int]], rank: int,
+                    world_size: int, group=None) -> Tuple[torch.Tensor, torch.Tensor]:
+    """From the segment-sharded layout of encode to the head-sharded layout of compose.
+
+    ``E_loc:[len(parts[rank]), H, dv, dk]`` and ``T_loc:[len(parts[rank]), H, dk, dk]`` are this rank's tuples, rows in
+    the order of ``parts[rank]`` (``lpt_partition``'s ascending segment indices).  Returns
+    ``(E:[n_seg, Hr, dv, dk], T:[n_seg, Hr, dk, dk])`` for ALL segments in global index order and this rank's heads
+    ``head_range(H, rank, world_size)``: exactly the pools ``hypic_compose`` takes with ``H = Hr``.
+    One all-to-all; rank ``s`` sends rank ``d`` the block ``[parts[s], heads of d]`` of both tensors."""
+    import torch.distributed as dist
+
+    n_loc, H, dv, dk = (int(x) for x in E_loc.shape)
+    if tuple(T_loc.shape) != (n_loc, H, dk, dk) or n_loc != len(parts[rank]):
+        raise ValueError("E_loc / T_loc do not match parts[rank]")
+    n_seg = sum(len(p) for p in parts)
+    hb, he = head_range(H, rank, world_size)
+    Hr = he - hb
+    per_head = dv * dk + dk * dk
+    if world_size == 1:
+        order = torch.as_tensor(list(parts[0]), dtype=torch.long, device=E_loc.device)
+        E = torch.empty_like(E_loc)
+        T = torch.empty_like(T_loc)
+        E[order], T[order] = E_loc, T_loc
+        return E, T
+    send_chunks, send_sizes = [], []
+    for d in range(world_size):
+        b, e = head_range(H, d, world_size)
+        blk = torch.cat([E_loc[:, b:e].reshape(n_loc, e - b, dv * dk), T_loc[:, b:e].reshape(n_loc, e - b, dk * dk)],
+                        dim=2)  # [n_loc, heads of d, per_head]
+        send_chunks.append(blk.reshape(-1))
+        send_sizes.append(n_loc * (e - b) * per_head)
+    recv_sizes = [len(parts[s]) * Hr * per_head for s in range(world_size)]
+    send = torch.cat(send_chunks)
+    recv = torch.empty(sum(recv_sizes), dtype=E_loc.dtype, device=E_loc.device)
+    dist.all_to_all_single(recv, send, output_split_sizes=recv_sizes, input_split_sizes=send_sizes, group=group)
+    E = torch.empty((n_seg, Hr, dv, dk), dtype=E_loc.dtype, device=E_loc.device)
+    T = torch.empty((n_seg, Hr, dk, dk), dtype=E_loc.dtype, device=E_loc.device)
+    off = 0
+    for s in range(world_size):
+        n_s = len(parts[s])
+        if n_s == 0:
+            continue
+        blk = recv[off:off + recv_sizes[s]].reshape(n_s, Hr, per_head)
+        off += recv_sizes[s]
+        idx = torch.as_tensor(list(parts[s]), dtype=torch.long, device=E_loc.device)
+        E[idx] = blk[:, :, :dv * dk].reshape(n_s, Hr, dv, dk)
+        T[idx] = blk[:, :, dv * dk:].reshape(n_s, Hr, dk, dk)
+    return E, T

@@ -44,11 +44,11 @@ def _free_port():
         return s.getsockname()[1]
 
 
-def _worker(rank, world, port, out_dir):
+def _worker(rank, world, port, out_dir, H=2):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
-        inp = wl.make_encode_inputs([70, 33, 129, 64, 5], 2, 16, 16, kv_dtype=torch.float32, seed=wl.seed_for(0, 9))
+        inp = wl.make_encode_inputs([70, 33, 129, 64, 5], H, 16, 16, kv_dtype=torch.float32, seed=wl.seed_for(0, 9))
         parts = sharding.lpt_partition(inp.seg_lens, world)
         mine = parts[rank]
         # every rank derives the same partition on its own
@@ -64,12 +64,20 @@ def _worker(rank, world, port, out_dir):
                                          np.array([0, sl.stop - sl.start], dtype=np.int32), gate=inp.gate)
             assert np.array_equal(E[0], E_all[s]) and np.array_equal(T[0], T_all[s])
         # compose is sharded by heads: my heads of the composed state equal the same heads of the full run
-        b, e = sharding.head_range(2, rank, world)
+        b, e = sharding.head_range(H, rank, world)
         ids = np.arange(5, dtype=np.int32)
         cu_r = np.array([0, 5], dtype=np.int32)
         S_full = oracle.compose(None, E_all, T_all, ids, cu_r)
         S_mine = oracle.compose(None, E_all[:, b:e], T_all[:, b:e], ids, cu_r)
         assert np.array_equal(S_mine, S_full[:, b:e])
+        # the exchange step of segment parallelism: my segments x all heads -> all segments x my heads, one all-to-all
+        E_loc = torch.from_numpy(np.ascontiguousarray(E_all[mine]))
+        T_loc = torch.from_numpy(np.ascontiguousarray(T_all[mine]))
+        E_x, T_x = sharding.exchange_tuples(E_loc, T_loc, parts, rank, world)
+        assert torch.equal(E_x, torch.from_numpy(np.ascontiguousarray(E_all[:, b:e])))
+        assert torch.equal(T_x, torch.from_numpy(np.ascontiguousarray(T_all[:, b:e])))
+        S_x = oracle.compose(None, E_x.numpy(), T_x.numpy(), ids, cu_r)
+        assert np.array_equal(S_x, S_full[:, b:e])
         # timing reduction: max over ranks
         t = sharding.max_over_ranks(10.0 + rank)
         assert t == 10.0 + world - 1
@@ -79,7 +87,22 @@ def _worker(rank, world, port, out_dir):
         dist.destroy_process_group()
 
 
+def test_exchange_tuples_single_rank_is_a_reorder():
+    E = torch.arange(3 * 2 * 4 * 4, dtype=torch.float32).reshape(3, 2, 4, 4)
+    T = -E.clone()
+    parts = [[0, 1, 2]]
+    E_x, T_x = sharding.exchange_tuples(E, T, parts, 0, 1)
+    assert torch.equal(E_x, E) and torch.equal(T_x, T)
+
+
 def test_two_rank_gloo_sharding(tmp_path):
     world = 2
     mp.spawn(_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    assert all((tmp_path / f"ok{r}").exists() for r in range(world))
+
+
+def test_three_rank_gloo_uneven_heads(tmp_path):
+    """3 ranks, 4 heads (2 + 1 + 1) and 5 segments (LPT gives 2 + 2 + 1): uneven on both axes of the all-to-all."""
+    world = 3
+    mp.spawn(_worker, args=(world, _free_port(), str(tmp_path), 4), nprocs=world, join=True)
     assert all((tmp_path / f"ok{r}").exists() for r in range(world))
