@@ -659,3 +659,28 @@ def test_diag_compose_vs_oracle_and_sequential(gate, d):
     seq = oracle.diag_sequential(S_in[2:3].cpu().numpy(), c.k, c.v, c.g, np.array([0, sum(lens)], dtype=np.int32),
                                  gate=c.gate)
     check_E(S_all, seq, TOL_F32, "encode -> compose vs sequential")
+
+
+def test_diag_compose_cfg4_lists_sampled_requests():
+    """The launch bench.py times for the scalar family's compose (cfg4's request lists over a pool of 1,024 end-states,
+    one scalar each), fp32 and fp16-stored end-states: sampled (request, head) chains against the oracle."""
+    E = wl.cfg4_pool_E(device="cuda")
+    gen = torch.Generator(device="cuda").manual_seed(wl.seed_for(6, 5))
+    t_pool = torch.rand((E.shape[0], 32), device="cuda", generator=gen) * 0.5 + 0.5
+    req = wl.cfg4_requests(device="cuda")
+    S = hb.hypic_diag_compose(req.S_in, E, t_pool, req.seg_ids, req.cu_segs)
+    Eh = hb.hypic_tuple_pack_f16(E)
+    Sh = hb.hypic_diag_compose(req.S_in, Eh, t_pool, req.seg_ids, req.cu_segs)
+    torch.cuda.synchronize()
+    assert torch.isfinite(S).all() and torch.isfinite(Sh).all()
+    ids_all, cu = req.seg_ids.cpu().numpy(), req.cu_segs.cpu().numpy()
+    for r, h in _sample_units(128, 32, 6, 13):
+        ids = torch.as_tensor(ids_all[cu[r]:cu[r + 1]], dtype=torch.long, device="cuda")
+        n = len(ids)
+        args = (np.arange(n, dtype=np.int32), np.array([0, n], dtype=np.int32))
+        s0 = req.S_in[r:r + 1, h:h + 1].cpu().numpy()
+        tp = t_pool[ids, h:h + 1].cpu().numpy()
+        ref = oracle.diag_compose(s0, E[ids, h:h + 1].cpu().numpy(), tp, *args)
+        check_E(S[r:r + 1, h:h + 1], ref, TOL_F32, "S_out (scalar family, cfg4 lists)")
+        refh = oracle.diag_compose(s0, Eh[ids, h:h + 1].float().cpu().numpy(), tp, *args)
+        check_E(Sh[r:r + 1, h:h + 1], refh, TOL_F32, "S_out (scalar family, fp16 end-states)")
