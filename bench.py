@@ -370,6 +370,34 @@ def time_extra_seam(hb, device, peaks, reps=20, w=8):
             "kernel_family": "simt"}
 
 
+def time_extra_forward(hb, device):
+    """hypic_forward_encode (encode folded into the forward) on one cfg2-shaped layer: fp32 CUDA-core
+    token recurrence over the stacked state [S ; T] (256 rows), 8 dk flop per row and token (decay, read, write,
+    read-out).  Bound by the fp32 pipe: peak = 148 SMs x 128 lanes x 2 flop x the SM clock under load."""
+    si = wl.make_seam_inputs([4096] * N_SEG, H, D, D, kv_dtype=torch.bfloat16, seed=wl.seed_for(7, 0), device=device)
+    e = si.enc
+
+    def one():
+        return hb.hypic_forward_encode(si.q, e.k, e.v, e.g, e.beta, e.cu_seqlens, e.gate)
+
+    one()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    one()
+    one()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 2
+    tfl = e.t_total * H * (2 * D) * D * 8 / (ms * 1e-3) / 1e12
+    peak = 148 * 128 * 2 * 1.92e9 / 1e12
+    return {"workload": "forward + encode in one pass, one cfg2-shaped layer (20 x 4096, H=32, bf16 q/k/v, fp32 arithmetic)",
+            "ms": ms, "tokens_per_s": e.t_total / (ms * 1e-3),
+            "roofline": {"bound": "alu", "achieved": tfl, "peak": peak, "unit": "TFLOP/s", "frac": tfl / peak,
+                         "traffic": None, "peak_source": "148 SMs x 128 fp32 lanes x 2 flop x 1.92 GHz (DESIGN.md 6.5e)"},
+            "kernel_family": "simt"}
+
+
 def time_extra_diag(hb, device, peaks, iters=16):
     """Scalar family (Table 1: RetNet / Mamba2-style scalar gate; compressed T_C of Table 3): hypic_diag_encode on one
     cfg2-shaped layer (20 x 4096 tokens, H = 32, bf16 k/v) and hypic_diag_compose on cfg4's request lists over a
@@ -589,6 +617,8 @@ def run_ours(args):
         extra["seam_window"] = time_extra_seam(hb, device, peaks)
         torch.cuda.empty_cache()
         extra["diag_family"] = time_extra_diag(hb, device, peaks)
+        torch.cuda.empty_cache()
+        extra["forward_encode"] = time_extra_forward(hb, device)
         extra["cfg2_compose"] = {"avg_launch_ms": cmp_avg, "compose_ops_per_s": N_SEG * H / (cmp_avg * 1e-3),
                                  "hbm_gbs": N_SEG * H * COMPOSE_BYTES_PER_STEP / (cmp_avg * 1e-3) / 1e9}
 

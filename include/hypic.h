@@ -160,6 +160,20 @@ int hypic_seam_window(const void* q, const void* k, const void* v, const float* 
                       int kv_dtype, int gate, const float* S_in, float* S_out, float* o, void* stream);
 
 /*
+ * hypic_forward_encode: the segment encode folded into the segment's own forward pass ("accumulating T_C
+ * is folded into the first segment prefill"): ONE pass over the tokens of every segment, started from the
+ * zero state, emits the per-token layer outputs  o[t,h,:] = S_t q_t together with the tuple
+ * (E, T) that hypic_segment_encode returns for the same inputs.  Arguments as hypic_segment_encode plus
+ *   q  [t_total, H, dk] kv_dtype        o  out [t_total, H, dv] fp32
+ * fp32 arithmetic on the CUDA cores (the token recurrence itself, rows of the stacked state [S ; T] in registers): the
+ * accurate form, bound by the fp32 pipe at about a tenth of the tensor family's encode rate; a tcgen05 version of
+ * this pass is not built.  Built envelope: dk in {64, 128}, dv in [1, 1024]; n_seg, H <= 65535.  No workspace.
+ */
+int hypic_forward_encode(const void* q, const void* k, const void* v, const float* g, const float* beta,
+                         const int32_t* cu_seqlens, int32_t n_seg, int32_t t_total, int32_t H, int32_t dk, int32_t dv,
+                         int kv_dtype, int gate, float* o, float* E, float* T, void* stream);
+
+/*
  * Scalar and diagonal families (Table 1; compressed transitions of PAPER.md:188-200 Table 3).
  * T_i = a_i I (RetNet / Lightning-2 with a constant a_i = gamma, Mamba2 with a data-dependent scalar) or diag(g_i)
  * (GLA); u_i = k_i v_i^T (no beta).  Row convention: S <- S diag(a_t) + v_t k_t^T, a_t = exp(g_t) (A2).

@@ -30,7 +30,7 @@ EXPORTS = (
     "hypic_status_string", "hypic_version", "hypic_last_launch_count", "hypic_encode_impl_for",
     "hypic_compose_impl_for", "hypic_debug_timeout_count", "hypic_envelope_violation_count", "hypic_compose_f16",
     "hypic_tuple_pack_f16", "hypic_seam_window", "hypic_diag_encode", "hypic_diag_compose",
-    "hypic_diag_encode_impl_for", "hypic_diag_compose_f16",
+    "hypic_diag_encode_impl_for", "hypic_diag_compose_f16", "hypic_forward_encode",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -76,6 +76,9 @@ def load_library() -> ctypes.CDLL:
     lib.hypic_diag_encode.restype = ctypes.c_int
     lib.hypic_diag_compose.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, ctypes.c_int, vp, vp]
     lib.hypic_diag_compose.restype = ctypes.c_int
+    lib.hypic_forward_encode.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, ctypes.c_int, ctypes.c_int, vp,
+                                         vp, vp, vp]
+    lib.hypic_forward_encode.restype = ctypes.c_int
     lib.hypic_diag_compose_f16.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, ctypes.c_int, vp, vp]
     lib.hypic_diag_compose_f16.restype = ctypes.c_int
     lib.hypic_diag_encode_impl_for.argtypes = [i32, i32, i32, ctypes.c_int, ctypes.c_int]
@@ -434,3 +437,44 @@ def hypic_diag_compose(S_in: Optional[torch.Tensor], E_pool: torch.Tensor, t_poo
     if rc != HYPIC_OK:
         raise HypicError(rc, "hypic_diag_compose")
     return S_out
+
+
+def hypic_forward_encode(q: torch.Tensor, k: torch.Tensor, v: torch.Tensor, g: torch.Tensor, beta: torch.Tensor,
+                         cu_seqlens: torch.Tensor, gate: int = HYPIC_GATE_SCALAR, *,
+                         stream: Optional[torch.cuda.Stream] = None) -> Tuple[torch.Tensor, torch.Tensor, torch.Tensor]:
+    """One pass per segment from the zero state: per-token outputs o:[Ttot,H,dv] and the tuple (E:[n_seg,H,dv,dk],
+    T:[n_seg,H,dk,dk]) of hypic_segment_encode, all fp32."""
+    lib = load_library()
+    for name, t in (("q", q), ("k", k), ("v", v), ("g", g), ("beta", beta), ("cu_seqlens", cu_seqlens)):
+        if not t.is_cuda:
+            raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if k.dim() != 3 or v.dim() != 3 or k.shape[:2] != v.shape[:2] or k.dtype != v.dtype or q.shape != k.shape \
+            or q.dtype != k.dtype:
+        raise ValueError("q, k:[Ttot,H,dk] and v:[Ttot,H,dv] must agree in Ttot, H and dtype")
+    t_total, H, dk = (int(x) for x in k.shape)
+    dv = int(v.shape[2])
+    if k.dtype == torch.bfloat16:
+        kv_dtype = HYPIC_DT_BF16
+    elif k.dtype == torch.float32:
+        kv_dtype = HYPIC_DT_F32
+    else:
+        raise ValueError(f"q/k/v must be bf16 or fp32, got {k.dtype}")
+    want_g = (t_total, H) if gate == HYPIC_GATE_SCALAR else (t_total, H, dk)
+    if tuple(g.shape) != want_g or tuple(beta.shape) != (t_total, H):
+        raise ValueError(f"g must be {want_g} and beta {(t_total, H)}")
+    n_seg = int(cu_seqlens.numel()) - 1
+    if n_seg < 0:
+        raise ValueError("cu_seqlens must have n_seg+1 >= 1 entries")
+    dev = k.device
+    o = torch.empty((t_total, H, dv), dtype=torch.float32, device=dev)
+    E = torch.empty((n_seg, H, dv, dk), dtype=torch.float32, device=dev)
+    T = torch.empty((n_seg, H, dk, dk), dtype=torch.float32, device=dev)
+    with torch.cuda.device(dev):
+        rc = lib.hypic_forward_encode(
+            _dev_ptr(q, "q"), _dev_ptr(k, "k"), _dev_ptr(v, "v"), _dev_ptr(g, "g", torch.float32),
+            _dev_ptr(beta, "beta", torch.float32), _dev_ptr(cu_seqlens, "cu_seqlens", torch.int32), n_seg, t_total, H,
+            dk, dv, kv_dtype, int(gate), _dev_ptr(o, "o", torch.float32), _dev_ptr(E, "E", torch.float32),
+            _dev_ptr(T, "T", torch.float32), _stream_handle(stream))
+    if rc != HYPIC_OK:
+        raise HypicError(rc, "hypic_forward_encode")
+    return o, E, T

@@ -67,6 +67,7 @@ struct SeamArgs {
   const float* S_in;
   float* S_out;
   float* o;
+  float* T_out;  // NULL: seam-window step; else forward-encode mode (rows of T appended to the state)
   cudaStream_t stream;
 };
 

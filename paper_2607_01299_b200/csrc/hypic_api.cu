@@ -142,7 +142,25 @@ int hypic_seam_window(const void* q, const void* k, const void* v, const float* 
     return HYPIC_ERR_INVALID_ARG;
   if (dk != 64 && dk != 128) return HYPIC_ERR_UNSUPPORTED;
   if (dv > 1024) return HYPIC_ERR_UNSUPPORTED;
-  SeamArgs a{q, k, v, g, beta, cu_tokens, R, t_total, H, dk, dv, kv_dtype, gate, S_in, S_out, o, (cudaStream_t)stream};
+  SeamArgs a{q, k, v, g, beta, cu_tokens, R, t_total, H, dk, dv, kv_dtype, gate, S_in, S_out, o, nullptr,
+             (cudaStream_t)stream};
+  return seam_simt(a);
+}
+
+int hypic_forward_encode(const void* q, const void* k, const void* v, const float* g, const float* beta,
+                         const int32_t* cu_seqlens, int32_t n_seg, int32_t t_total, int32_t H, int32_t dk, int32_t dv,
+                         int kv_dtype, int gate, float* o, float* E, float* T, void* stream) {
+  g_launch_count = 0;
+  const int vs = validate_encode_shape(n_seg, t_total, H, dk, dv, kv_dtype, gate);
+  if (vs != HYPIC_OK) return vs;
+  if (!cu_seqlens) return HYPIC_ERR_INVALID_ARG;
+  if (n_seg > 0 && (!E || !T)) return HYPIC_ERR_INVALID_ARG;
+  if (t_total > 0 && (!q || !k || !v || !g || !beta || !o)) return HYPIC_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(g) || !aligned16(beta) || !aligned16(o) ||
+      !aligned16(E) || !aligned16(T))
+    return HYPIC_ERR_INVALID_ARG;
+  SeamArgs a{q, k, v, g, beta, cu_seqlens, n_seg, t_total, H, dk, dv, kv_dtype, gate, nullptr, E, o, T,
+             (cudaStream_t)stream};
   return seam_simt(a);
 }
 

@@ -21,6 +21,11 @@
 //     ahead and converted / stored to shared memory when their turn comes, and o leaves through shared memory as
 //     whole rows.
 // One CTA = 128 threads; one item = 64 rows of one (request, head) unit.
+//
+// The same kernel is the fp32 "encode folded into the forward" pass (at cache
+// time the segment's normal prefill also accumulates T_C): with T_out given, the rows of the stacked state [S ; T] are
+// walked, T rows starting at the identity and taking no value term, so one pass over the tokens emits the per-token
+// outputs o, the end-state E (= S_out from a zero start) and T.
 #include <algorithm>
 #include <type_traits>
 
@@ -72,11 +77,12 @@ struct SeamRaw {
   float b, gs;
 };
 
-template <int DK, bool BF16, bool CHANNEL>
+template <int DK, bool BF16, bool CHANNEL, bool WITH_T>
 __global__ void __launch_bounds__(kSeamThreads, CHANNEL ? 3 : 4)
     seam_simt_kernel(const void* __restrict__ q, const void* __restrict__ k, const void* __restrict__ v,
                      const float* __restrict__ g, const float* __restrict__ beta, const int32_t* __restrict__ cu_tokens,
-                     int H, int dv, int n_blk, int n_items, const float* S_in, float* S_out, float* __restrict__ o) {
+                     int H, int dv, int n_blk, int n_items, const float* S_in, float* S_out, float* __restrict__ o,
+                     float* __restrict__ T_out) {
   constexpr int AW = CHANNEL ? DK : 1;
   constexpr int NJ = DK / 32;                   // float4s of a row owned by one lane
   constexpr int NV = kSeamTT * kSeamRows / kSeamThreads;
@@ -243,10 +249,17 @@ __global__ void __launch_bounds__(kSeamThreads, CHANNEL ? 3 : 4)
     cp_async_wait_all();
 #pragma unroll
     for (int i = 0; i < kSeamRT; ++i) {
-      const bool have = S_in && row0 + rloc0 + i < dv;
+      const int row = row0 + rloc0 + i;
+      const bool have = S_in && row < dv;
+      // forward-encode mode (T_out != NULL): rows [dv, dv + dk) are the rows of T, which start at the identity
+      const int m = (WITH_T && row >= dv) ? row - dv : -1;
 #pragma unroll
-      for (int j = 0; j < NJ; ++j)
-        x[i][j] = have ? xs[(i * NJ + j) * kSeamThreads + tid] : make_float4(0.f, 0.f, 0.f, 0.f);
+      for (int j = 0; j < NJ; ++j) {
+        const int c0 = 4 * (l + kSeamLanes * j);
+        x[i][j] = have ? xs[(i * NJ + j) * kSeamThreads + tid]
+                       : make_float4(m == c0 ? 1.f : 0.f, m == c0 + 1 ? 1.f : 0.f, m == c0 + 2 ? 1.f : 0.f,
+                                     m == c0 + 3 ? 1.f : 0.f);
+      }
     }
     if (next < n_items) prefetch_rows(next);  // every thread refills only the slots it has just read
     if (n_tiles == 0 && next < n_items) load_raw(raw, next, 0, nt_begin, nt_end);
@@ -365,8 +378,13 @@ __global__ void __launch_bounds__(kSeamThreads, CHANNEL ? 3 : 4)
 #pragma unroll
     for (int i = 0; i < kSeamRT; ++i) {
       const int row = row0 + rloc0 + i;
-      if (row < dv) {
-        float4* dst = reinterpret_cast<float4*>(S_out + ((size_t)unit * dv + row) * DK);
+      float* base = nullptr;
+      if (row < dv)
+        base = S_out + ((size_t)unit * dv + row) * DK;
+      else if (WITH_T && row < dv + DK)
+        base = T_out + ((size_t)unit * DK + (row - dv)) * DK;
+      if (base) {
+        float4* dst = reinterpret_cast<float4*>(base);
 #pragma unroll
         for (int j = 0; j < NJ; ++j) __stcs(dst + l + kSeamLanes * j, x[i][j]);
       }
@@ -376,15 +394,15 @@ __global__ void __launch_bounds__(kSeamThreads, CHANNEL ? 3 : 4)
   }
 }
 
-template <int DK, bool BF16, bool CHANNEL>
+template <int DK, bool BF16, bool CHANNEL, bool WITH_T>
 int seam_launch(const SeamArgs& a) {
-  const int n_blk = (a.dv + kSeamRows - 1) / kSeamRows;
+  const int n_blk = (a.dv + (WITH_T ? DK : 0) + kSeamRows - 1) / kSeamRows;  // rows of [S ; T]
   const long long n_items = (long long)n_blk * a.H * a.R;
   if (n_items > 0x7fffffffLL) return HYPIC_ERR_UNSUPPORTED;
   const DeviceInfo& di = device_info();
   if (!di.ok) return HYPIC_ERR_CUDA;
   constexpr int kDyn = kSeamRT * (DK / 32) * kSeamThreads * 16;  // prefetch buffer for the next item's rows
-  auto kern = seam_simt_kernel<DK, BF16, CHANNEL>;
+  auto kern = seam_simt_kernel<DK, BF16, CHANNEL, WITH_T>;
   static bool attr_set = false;  // per instantiation
   if (!attr_set) {
     HYPIC_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kDyn));
@@ -392,17 +410,17 @@ int seam_launch(const SeamArgs& a) {
   }
   const int grid = (int)std::min<long long>(n_items, (CHANNEL ? 3LL : 4LL) * di.sm_count);
   kern<<<grid, kSeamThreads, kDyn, a.stream>>>(a.q, a.k, a.v, a.g, a.beta, a.cu_tokens, a.H, a.dv, n_blk, (int)n_items,
-                                               a.S_in, a.S_out, a.o);
+                                               a.S_in, a.S_out, a.o, a.T_out);
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
   return HYPIC_OK;
 }
 
-template <int DK>
+template <int DK, bool WITH_T>
 int seam_dispatch(const SeamArgs& a) {
   const bool bf = a.kv_dtype == HYPIC_DT_BF16, ch = a.gate == HYPIC_GATE_CHANNEL;
-  if (bf) return ch ? seam_launch<DK, true, true>(a) : seam_launch<DK, true, false>(a);
-  return ch ? seam_launch<DK, false, true>(a) : seam_launch<DK, false, false>(a);
+  if (bf) return ch ? seam_launch<DK, true, true, WITH_T>(a) : seam_launch<DK, true, false, WITH_T>(a);
+  return ch ? seam_launch<DK, false, true, WITH_T>(a) : seam_launch<DK, false, false, WITH_T>(a);
 }
 
 }  // namespace
@@ -411,8 +429,8 @@ int seam_simt(const SeamArgs& a) {
   if (a.H > 65535 || a.R > 65535) return HYPIC_ERR_UNSUPPORTED;
   if (a.dv < 1 || a.dv > 1024) return HYPIC_ERR_UNSUPPORTED;
   if (a.R == 0) return HYPIC_OK;
-  if (a.dk == 128) return seam_dispatch<128>(a);
-  if (a.dk == 64) return seam_dispatch<64>(a);
+  if (a.dk == 128) return a.T_out ? seam_dispatch<128, true>(a) : seam_dispatch<128, false>(a);
+  if (a.dk == 64) return a.T_out ? seam_dispatch<64, true>(a) : seam_dispatch<64, false>(a);
   return HYPIC_ERR_UNSUPPORTED;
 }
 

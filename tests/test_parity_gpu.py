@@ -684,3 +684,33 @@ def test_diag_compose_cfg4_lists_sampled_requests():
         check_E(S[r:r + 1, h:h + 1], ref, TOL_F32, "S_out (scalar family, cfg4 lists)")
         refh = oracle.diag_compose(s0, Eh[ids, h:h + 1].float().cpu().numpy(), tp, *args)
         check_E(Sh[r:r + 1, h:h + 1], refh, TOL_F32, "S_out (scalar family, fp16 end-states)")
+
+
+# ------------------------------------------------------------------------------------------------ forward + encode in one pass
+@pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
+@pytest.mark.parametrize("kv,d,dv", [(torch.float32, 128, 128), (torch.bfloat16, 128, 128), (torch.float32, 64, 64),
+                                     (torch.bfloat16, 128, 72), (torch.float32, 64, 33)])
+def test_forward_encode_vs_oracle(gate, kv, d, dv):
+    """hypic_forward_encode: one pass emits o, E and T.  o against the oracle's token recurrence with
+    read-outs from the zero state (oracle.seam_window, pins W1-W4), (E, T) against oracle.segment_encode (pins P1-P10);
+    ragged segments incl. empty and 1-token ones, dv off the 64-row tile so that a CTA straddles the E / T boundary."""
+    lens = [70, 0, 1, 129, 16, 200]
+    si = wl.make_seam_inputs(lens, 3, d, dv, kv_dtype=kv, gate=gate, g_lo=-0.1, seed=wl.seed_for(7, 1), device="cuda")
+    e = si.enc
+    o, E, T = hb.hypic_forward_encode(si.q, e.k, e.v, e.g, e.beta, e.cu_seqlens, e.gate)
+    torch.cuda.synchronize()
+    assert hb.hypic_last_launch_count() == 1
+    c = e.cpu()
+    E_ref, T_ref = oracle.segment_encode(c.k, c.v, c.g, c.beta, c.cu_seqlens, gate=c.gate)
+    check_E(E, E_ref, TOL_F32, "E (forward-encode)")
+    check_T(T, T_ref, TOL_F32, "T (forward-encode)")
+    host = [t.float().cpu().numpy() for t in (si.q, e.k, e.v, e.g, e.beta)]
+    cu_h = e.cu_seqlens.cpu().numpy()
+    S_ref, o_ref = oracle.seam_window(None, *host, cu_h, gate=e.gate)
+    assert np.array_equal(S_ref, E_ref)  # the two oracle routes agree bit for bit on the end-state
+    _check_o(o, o_ref, cu_h, TOL_F32, _typical_readout(None, *host, cu_h, e.gate))
+    # and the tensor-family encode of the same inputs returns the same tuple within its own tolerance
+    if kv == torch.bfloat16 and d == 128 and dv == 128:
+        E2, T2 = hb.hypic_segment_encode(e.k, e.v, e.g, e.beta, e.cu_seqlens, e.gate)
+        check_E(E2, E.cpu().numpy(), TOL_BF16, "E (tensor family vs forward-encode)")
+        check_T(T2, T.cpu().numpy(), TOL_BF16, "T (tensor family vs forward-encode)")
