@@ -27,9 +27,19 @@ constexpr int kDtSmem = kDtOffBar + 128 + 1024;
 
 struct DtBars {
   uint64_t full[kDtStages], conv[kDtStages], free_[kDtStages], done;
+  double peer_g;  // split kernels: the peer CTA's total log-decay, written through distributed shared memory
   uint32_t tmem_base;
   int abort_flag;
 };
+
+__device__ __forceinline__ void cluster_arrive_release() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait_acquire() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+// store a double into the same shared-memory variable of CTA `rank` of this cluster
+__device__ __forceinline__ void st_cluster_f64(double* local_smem_ptr, uint32_t rank, double v) {
+  uint32_t remote;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(local_smem_ptr)), "r"(rank));
+  asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(remote), "d"(v) : "memory");
+}
 
 // Single-thread wait of the loader / issuer: mbarrier.try_wait already suspends the thread for a hardware-chosen time, so
 // a plain retry loop reacts within tens of cycles; s2_wait's __nanosleep back-off (measured here: the loader woke up
@@ -50,10 +60,15 @@ __device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
   asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
-__global__ void __launch_bounds__(kDtThreads, 3)
-    diag_scan_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
-                     const float* __restrict__ g, const int32_t* __restrict__ cu_seqlens, int H, float* __restrict__ E,
-                     float* __restrict__ tvec) {
+// kSplit = 2: the unit is shared by a cluster of two CTAs (blockIdx.z = rank): rank 1 streams the later half of the chunks
+// and writes its sum E_1 to the unit's place in E; rank 0 streams the earlier half with weights relative to ITS last
+// token, learns rank 1's total log-decay G_1 through distributed shared memory, and after the cluster barrier writes
+// E = exp(G_1) E_0 + E_1 in a fixed order (deterministic; no workspace, no atomics).  Twice the CTAs of half the length:
+// 2.9 waves of 32 chunks instead of 1.44 waves of 64 on the cfg2-shaped layer, and twice the parallelism when units are few.
+template <int kSplit>
+__device__ __forceinline__ void diag_scan_body(const CUtensorMap& tmK, const CUtensorMap& tmV, const float* __restrict__ g,
+                                               const int32_t* __restrict__ cu_seqlens, int H, float* E,
+                                               float* __restrict__ tvec) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   DtBars* bars = reinterpret_cast<DtBars*>(smem + kDtOffBar);
@@ -62,14 +77,13 @@ __global__ void __launch_bounds__(kDtThreads, 3)
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int h = blockIdx.x, s = blockIdx.y;
   const int seg_begin = cu_seqlens[s], seg_end = cu_seqlens[s + 1];
-  const int nc = (seg_end - seg_begin + kC - 1) / kC;
+  const int nc_tot = (seg_end - seg_begin + kC - 1) / kC;
+  const int rank = kSplit == 2 ? (int)blockIdx.z : 0;
+  const int c_lo = (kSplit == 2 && rank == 1) ? nc_tot / 2 : 0;           // this CTA's chunks [c_lo, c_hi) of the segment
+  const int c_hi = (kSplit == 2 && rank == 0) ? nc_tot / 2 : nc_tot;
+  const int nc = c_hi - c_lo;
   float* Eu = E + ((size_t)s * H + h) * kD * kD;
-
-  if (nc == 0) {  // empty segment: E = 0, tvec = 1
-    for (int i = tid; i < kD * kD / 4; i += kDtThreads) reinterpret_cast<float4*>(Eu)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (tid == 0) tvec[(size_t)s * H + h] = 1.f;
-    return;
-  }
+  // (an empty range runs no pipeline iteration and contributes E = 0, log-decay 0; nobody returns before the cluster barrier)
 
   if (warp == kDtConvWarps) tmem_alloc(&bars->tmem_base, 128);
   if (tid == 0) {
@@ -85,6 +99,10 @@ __global__ void __launch_bounds__(kDtThreads, 3)
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  if (kSplit == 2) {  // both CTAs of the pair are running before either touches the other's shared memory
+    cluster_arrive_release();
+    cluster_wait_acquire();
+  }
   const uint32_t tmem = bars->tmem_base;
   const uint32_t smem_base = smem_u32(smem);
 
@@ -98,7 +116,7 @@ __global__ void __launch_bounds__(kDtThreads, 3)
     auto load_g = [&](int i, float& ga, float& gb) {
       ga = gb = 0.f;
       if (i < nc) {
-        const int ta = seg_begin + (nc - 1 - i) * kC + 2 * lane;
+        const int ta = seg_begin + (c_hi - 1 - i) * kC + 2 * lane;
         if (ta < seg_end) ga = __ldg(g + (size_t)ta * H + h);
         if (ta + 1 < seg_end) gb = __ldg(g + (size_t)(ta + 1) * H + h);
       }
@@ -109,7 +127,7 @@ __global__ void __launch_bounds__(kDtThreads, 3)
 #pragma unroll 1
     for (int i = 0; i < nc; ++i) {
       const int st = i % kDtStages;
-      const int t0 = seg_begin + (nc - 1 - i) * kC;  // last chunk first
+      const int t0 = seg_begin + (c_hi - 1 - i) * kC;  // last chunk first
       const int ta = t0 + 2 * lane, tb = ta + 1;
       S2_STAMPW(kDtConvWarps + 1, 0, i, 2);
       const float ga = ga0, gb = gb0;
@@ -150,7 +168,14 @@ __global__ void __launch_bounds__(kDtThreads, 3)
     }
 #pragma unroll
     for (int d = 16; d > 0; d /= 2) lane_sum += __shfl_xor_sync(0xffffffffu, lane_sum, d);
-    if (lane == 0) tvec[(size_t)s * H + h] = (float)exp(lane_sum);
+    if (kSplit == 1) {
+      if (lane == 0) tvec[(size_t)s * H + h] = (float)exp(lane_sum);
+    } else {
+      if (rank == 1 && lane == 0) st_cluster_f64(&bars->peer_g, 0, lane_sum);  // into rank 0's shared memory
+      cluster_arrive_release();
+      cluster_wait_acquire();
+      if (rank == 0 && lane == 0) tvec[(size_t)s * H + h] = (float)exp(lane_sum + bars->peer_g);
+    }
   } else if (warp == kDtConvWarps) {
     // ----------------------------------------------------------------------------------------------- MMA issuer
     if (lane == 0) {
@@ -169,14 +194,18 @@ __global__ void __launch_bounds__(kDtThreads, 3)
         mma_commit(&bars->free_[st]);
         S2_STAMPW(kDtConvWarps, 2, i, 1);
       }
-      mma_commit(&bars->done);
+      if (nc > 0) mma_commit(&bars->done);
+    }
+    if (kSplit == 2) {
+      cluster_arrive_release();
+      cluster_wait_acquire();
     }
   } else {
     // ----------------------------------------------------------------------------------------------- converters
 #pragma unroll 1
     for (int i = 0; i < nc; ++i) {
       const int st = i % kDtStages;
-      const int t0 = seg_begin + (nc - 1 - i) * kC;
+      const int t0 = seg_begin + (c_hi - 1 - i) * kC;
       s2_wait_warp(&bars->full[st], (i / kDtStages) & 1, abort_flag, lane);
       S2_STAMPW(0, 1, i, 0);
       const float* w = sw + st * 64;
@@ -202,21 +231,48 @@ __global__ void __launch_bounds__(kDtThreads, 3)
       S2_STAMPW(0, 1, i, 1);
     }
     // ----------------------------------------------------------------------------------------------- epilogue
-    s2_wait_warp(&bars->done, 0, abort_flag, lane);
-    tc_fence_after();
+    if (nc > 0) {
+      s2_wait_warp(&bars->done, 0, abort_flag, lane);
+      tc_fence_after();
+    }
     const int q = warp & 3, hf = warp >> 2;  // TMEM lane quarter of this warp; column slice (two warps per quarter)
     const int row = 32 * q + lane;           // dv index = TMEM lane
     constexpr int kColsPerWarp = kD / (kDtConvWarps / 4);
     float4* dst = reinterpret_cast<float4*>(Eu + (size_t)row * kD + kColsPerWarp * hf);
+    float scale = 1.f;
+    if (kSplit == 2 && rank == 0) {
+      cluster_arrive_release();
+      cluster_wait_acquire();  // rank 1's E_1 is in global memory, its log-decay in bars->peer_g
+      scale = expf((float)bars->peer_g);
+    }
+    const bool add_peer = kSplit == 2 && rank == 0;
+    if (!(add_peer && nc == 0)) {  // (rank 0 with no chunks: E = E_1 is already in place)
 #pragma unroll 1
-    for (int cb = 0; cb < kColsPerWarp / 32; ++cb) {
-      uint32_t x[32];
-      tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + kColsPerWarp * hf + 32 * cb, x);
-      tmem_ld_wait();
+      for (int cb = 0; cb < kColsPerWarp / 32; ++cb) {
+        uint32_t x[32];
+        if (nc > 0) {
+          tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + kColsPerWarp * hf + 32 * cb, x);
+          tmem_ld_wait();
+        } else {
 #pragma unroll
-      for (int u = 0; u < 8; ++u)
-        dst[8 * cb + u] = make_float4(__uint_as_float(x[4 * u]), __uint_as_float(x[4 * u + 1]), __uint_as_float(x[4 * u + 2]),
-                                      __uint_as_float(x[4 * u + 3]));
+          for (int u = 0; u < 32; ++u) x[u] = 0u;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          float4 o4 = make_float4(__uint_as_float(x[4 * u]), __uint_as_float(x[4 * u + 1]), __uint_as_float(x[4 * u + 2]),
+                                  __uint_as_float(x[4 * u + 3]));
+          if (add_peer) {
+            const float4 p4 = dst[8 * cb + u];  // plain load: written by the peer CTA during this kernel
+            o4 = make_float4(fmaf(scale, o4.x, p4.x), fmaf(scale, o4.y, p4.y), fmaf(scale, o4.z, p4.z),
+                             fmaf(scale, o4.w, p4.w));
+          }
+          dst[8 * cb + u] = o4;
+        }
+      }
+    }
+    if (kSplit == 2 && rank == 1) {
+      cluster_arrive_release();  // E_1 written
+      cluster_wait_acquire();
     }
   }
   tc_fence_before();
@@ -224,6 +280,20 @@ __global__ void __launch_bounds__(kDtThreads, 3)
   if (warp == kDtConvWarps) tmem_dealloc(tmem, 128);
 }
 
+
+__global__ void __launch_bounds__(kDtThreads, 3)
+    diag_scan_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                     const float* __restrict__ g, const int32_t* __restrict__ cu_seqlens, int H, float* E,
+                     float* __restrict__ tvec) {
+  diag_scan_body<1>(tmK, tmV, g, cu_seqlens, H, E, tvec);
+}
+
+__global__ void __cluster_dims__(1, 1, 2) __launch_bounds__(kDtThreads, 3)
+    diag_scan_split2_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                            const float* __restrict__ g, const int32_t* __restrict__ cu_seqlens, int H, float* E,
+                            float* __restrict__ tvec) {
+  diag_scan_body<2>(tmK, tmV, g, cu_seqlens, H, E, tvec);
+}
 
 // ------------------------------------------------------------------------------------------------------------------
 // Diagonal family (GLA: T_i = diag(g_i)): the same reverse-streamed contraction with per-channel weights,

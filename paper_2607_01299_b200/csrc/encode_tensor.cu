@@ -215,6 +215,7 @@ int diag_encode_tensor(const DiagEncodeArgs& a) {
   static bool configured = false;
   if (!configured) {
     HYPIC_CUDA_OK(cudaFuncSetAttribute(diag_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDtSmem));
+    HYPIC_CUDA_OK(cudaFuncSetAttribute(diag_scan_split2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDtSmem));
     HYPIC_CUDA_OK(cudaFuncSetAttribute(diag_scan_ch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDtChSmem));
     configured = true;
   }
@@ -225,8 +226,21 @@ int diag_encode_tensor(const DiagEncodeArgs& a) {
   if (a.gate == HYPIC_GATE_CHANNEL)
     diag_scan_ch_kernel<<<dim3(a.H, a.n_seg), kDtThreads, kDtChSmem, a.stream>>>(tmK, tmV, a.g, a.cu_seqlens, a.H, a.E,
                                                                                 a.tvec);
-  else
-    diag_scan_kernel<<<dim3(a.H, a.n_seg), kDtThreads, kDtSmem, a.stream>>>(tmK, tmV, a.g, a.cu_seqlens, a.H, a.E, a.tvec);
+  else {
+    // pair-split only while the split CTAs still fit one wave (few units: twice the parallelism, half the chain length).
+    // With more units than that the split LOSES (measured on the cfg2-shaped layer, 640 units on 444 slots: 0.31 ms split
+    // vs 0.25 ms unsplit -- the pipeline fill / drain and the E_1 round trip are paid twice, and the unsplit tail wave runs
+    // faster than a full one anyway).
+    const DeviceInfo& di = device_info();
+    const long long slots = 3LL * (di.ok ? di.sm_count : 148), U = (long long)a.H * a.n_seg;
+    const bool split = 2 * U <= slots;
+    if (split)
+      diag_scan_split2_kernel<<<dim3(a.H, a.n_seg, 2), kDtThreads, kDtSmem, a.stream>>>(tmK, tmV, a.g, a.cu_seqlens, a.H,
+                                                                                       a.E, a.tvec);
+    else
+      diag_scan_kernel<<<dim3(a.H, a.n_seg), kDtThreads, kDtSmem, a.stream>>>(tmK, tmV, a.g, a.cu_seqlens, a.H, a.E,
+                                                                             a.tvec);
+  }
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
   return HYPIC_OK;

@@ -572,6 +572,18 @@ def test_diag_encode_ragged_segments(name, impl, gate, kv, d, dv):
     assert torch.all(E[1] == 0) and torch.all(tv[1] == 1)  # empty segment: E = 0, tvec = 1
 
 
+def test_diag_encode_tensor_unsplit_schedule():
+    """n_seg x H = 444 units: more than half a wave of 3 CTAs per SM, so the scalar-family kernel keeps one CTA per
+    unit (the ragged-segment tests, 27 units, take its cluster-pair split): all units against the oracle."""
+    lens = [70, 64, 1, 129, 130, 200, 63, 65, 0, 128, 192, 5]
+    inp = wl.make_encode_inputs(lens, 37, 128, 128, kv_dtype=torch.bfloat16, g_lo=-0.2, seed=wl.seed_for(6, 6), device="cuda")
+    E, tv = gpu_diag_encode(inp, hb.HYPIC_IMPL_TENSOR)
+    c = inp.cpu()
+    E_ref, t_ref = oracle.diag_encode(c.k, c.v, c.g, c.cu_seqlens, gate=c.gate)
+    check_E(E, E_ref, TOL_BF16, "E (scalar family, unsplit)")
+    _check_tvec(tv, t_ref, TOL_F32)
+
+
 def test_diag_encode_tensor_channel_gate_full_size_sampled_units():
     """Diagonal family (GLA) on the tcgen05 kernel at the bench shape (20 x 4096 tokens, H = 32, per-channel gate with a
     milder decay so that tvec stays representable): sampled units against the oracle, tvec of those units included."""
