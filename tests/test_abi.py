@@ -77,6 +77,37 @@ def test_argument_validation_needs_no_gpu(lib):
     assert comp(None, fake, fake, fake, fake, 1, 4, 2, 1, 64, 64, None, None) == b.HYPIC_ERR_INVALID_ARG
     assert comp(None, fake, fake, fake, fake, 1, 4, 2, 1, 48, 64, fake, None) == b.HYPIC_ERR_UNSUPPORTED
 
+    # the entry points added around the north-star pair validate the same way
+    seam = lib.hypic_seam_window
+    assert seam(fake, fake, fake, fake, fake, None, 1, 8, 1, 64, 64, 0, 0, None, fake, fake, None) == b.HYPIC_ERR_INVALID_ARG
+    assert seam(fake, fake, fake, fake, fake, fake, -1, 8, 1, 64, 64, 0, 0, None, fake, fake, None) == b.HYPIC_ERR_INVALID_ARG
+    assert seam(None, fake, fake, fake, fake, fake, 1, 8, 1, 64, 64, 0, 0, None, fake, fake, None) == b.HYPIC_ERR_INVALID_ARG
+    assert seam(fake, fake, fake, fake, fake, fake, 1, 8, 1, 64, 64, 0, 0, None, None, fake, None) == b.HYPIC_ERR_INVALID_ARG
+    assert seam(fake, fake, fake, fake, fake, fake, 1, 8, 1, 64, 64, 0, 0, odd, fake, fake, None) == b.HYPIC_ERR_INVALID_ARG
+    assert seam(fake, fake, fake, fake, fake, fake, 1, 8, 1, 80, 64, 0, 0, None, fake, fake, None) == b.HYPIC_ERR_UNSUPPORTED
+    fwd = lib.hypic_forward_encode
+    assert fwd(fake, fake, fake, fake, fake, None, 1, 8, 1, 64, 64, 0, 0, fake, fake, fake, None) == b.HYPIC_ERR_INVALID_ARG
+    assert fwd(fake, fake, fake, fake, fake, fake, 1, 8, 1, 64, 64, 0, 0, None, fake, fake, None) == b.HYPIC_ERR_INVALID_ARG
+    assert fwd(fake, fake, fake, fake, fake, fake, 1, 8, 1, 64, 64, 0, 0, fake, fake, None, None) == b.HYPIC_ERR_INVALID_ARG
+    assert fwd(fake, fake, fake, fake, fake, fake, 1, 8, 1, 64, 64, 3, 0, fake, fake, fake, None) == b.HYPIC_ERR_INVALID_ARG
+    denc = lib.hypic_diag_encode
+    assert denc(fake, fake, fake, None, 1, 8, 1, 64, 64, 0, 0, fake, fake, None) == b.HYPIC_ERR_INVALID_ARG
+    assert denc(fake, fake, fake, fake, 1, 8, 1, 64, 64, 0, 0, fake, None, None) == b.HYPIC_ERR_INVALID_ARG
+    assert denc(fake, fake, None, fake, 1, 8, 1, 64, 64, 0, 0, fake, fake, None) == b.HYPIC_ERR_INVALID_ARG
+    assert denc(fake, fake, fake, fake, 1, 8, 1, 96, 64, 0, 0, fake, fake, None) == b.HYPIC_ERR_UNSUPPORTED
+    for dcomp in (lib.hypic_diag_compose, lib.hypic_diag_compose_f16):
+        assert dcomp(None, fake, fake, fake, None, 1, 4, 2, 1, 64, 64, 0, fake, None) == b.HYPIC_ERR_INVALID_ARG
+        assert dcomp(None, fake, None, fake, fake, 1, 4, 2, 1, 64, 64, 0, fake, None) == b.HYPIC_ERR_INVALID_ARG
+        assert dcomp(None, fake, fake, fake, fake, 1, 4, 2, 1, 64, 64, 9, fake, None) == b.HYPIC_ERR_INVALID_ARG
+        assert dcomp(None, fake, fake, fake, fake, 1, 4, 2, 1, 66, 64, 0, fake, None) == b.HYPIC_ERR_UNSUPPORTED
+    cf16 = lib.hypic_compose_f16
+    assert cf16(None, fake, fake, fake, None, 1, 4, 2, 1, 128, 128, fake, None) == b.HYPIC_ERR_INVALID_ARG
+    assert cf16(None, fake, fake, fake, fake, 1, 4, 2, 1, 64, 64, fake, None) == b.HYPIC_ERR_UNSUPPORTED
+    assert lib.hypic_tuple_pack_f16(None, fake, 8, None) == b.HYPIC_ERR_INVALID_ARG
+    assert lib.hypic_diag_encode_impl_for(1, 96, 64, 0, 0) == -b.HYPIC_ERR_UNSUPPORTED
+    assert lib.hypic_diag_encode_impl_for(1, 128, 128, b.HYPIC_DT_BF16, 1) == b.HYPIC_IMPL_TENSOR
+    assert lib.hypic_diag_encode_impl_for(1, 64, 64, b.HYPIC_DT_F32, 0) == b.HYPIC_IMPL_SIMT
+
     assert lib.hypic_set_impl(42) == b.HYPIC_ERR_INVALID_ARG
     assert lib.hypic_set_impl(b.HYPIC_IMPL_AUTO) == b.HYPIC_OK
     assert lib.hypic_segment_encode_workspace(-1, 0, 1, 64, 64, 0, 0) == 0
