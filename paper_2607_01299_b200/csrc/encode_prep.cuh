@@ -157,31 +157,48 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
   }
   {  // a1: inclusive cumulative log-decay by a two-warp shuffle scan (warps 0 and 1 hold the 64 tokens)
     float gv = greg, bv = breg;
-    if (ci + 1 < kPrepChunksPerCta && metas[ci + 1].y > 0) prefetch(metas[ci + 1]);  // in flight during this chunk
+    if (!kCh && ci + 1 < kPrepChunksPerCta && metas[ci + 1].y > 0) prefetch(metas[ci + 1]);  // in flight during this chunk
     if (kCh) {
-      // per-channel gate: thread = channel c; G_j[c] = cumulative log-decay down the chunk's tokens; the K chunk is
-      // rewritten as K (.) Gamma (s_k) and K (/) Gamma (s_k2), both fp16 (Gamma in [e^-9, 1] inside the envelope)
+      // per-channel gate: thread = (channel pair 2p, 2p+1; token range [32 r, 32 r + 32)); G_j[c] = cumulative log-decay
+      // down the chunk's tokens; the K chunk is rewritten as K (.) Gamma (s_k) and K (/) Gamma (s_k2), both fp16 (Gamma
+      // in [e^-9, 1] inside the envelope).  All 32 log-decay loads of a thread are in flight together, and the two
+      // fp16 tiles are touched with 32-bit accesses (the first version, one thread per channel walking 64 tokens with
+      // four serialised load batches and 16-bit accesses, took 25,000 of the chunk's 35,000 cycles).
       if (tid < kC) s_b[tid] = bv;
-      __syncthreads();  // the K chunk is in s_k
+      const int p = tid & 63, rg = tid >> 6;
       const int t0c = metas[ci].x;
-      __half* k2 = reinterpret_cast<__half*>(s_k2);
-      float run = 0.f;
-#pragma unroll 1
-      for (int jb = 0; jb < kC; jb += 16) {
-        float gl[16];  // 16 independent loads in flight per thread
+      float2 gl[32];
 #pragma unroll
-        for (int i = 0; i < 16; ++i) gl[i] = (jb + i < valid) ? g[((size_t)(t0c + jb + i) * H + h) * kD + tid] : 0.f;
-#pragma unroll
-        for (int i = 0; i < 16; ++i) {
-          const int j = jb + i;
-          run += gl[i];
-          const float kv = __half2float(ks[j * kKsPitch + tid]);
-          const float e = __expf(run);
-          ks[j * kKsPitch + tid] = __float2half_rn(kv * e);
-          k2[j * kKsPitch + tid] = __float2half_rn(__fdividef(kv, e));
-        }
+      for (int i = 0; i < 32; ++i) {
+        const int j = 32 * rg + i;
+        gl[i] = (j < valid) ? __ldg(reinterpret_cast<const float2*>(g + ((size_t)(t0c + j) * H + h) * kD) + p)
+                            : make_float2(0.f, 0.f);
       }
-      s_g[tid] = run;
+      float r0 = 0.f, r1 = 0.f;
+#pragma unroll
+      for (int i = 0; i < 32; ++i) {  // inclusive prefix inside the range, in place
+        r0 += gl[i].x, r1 += gl[i].y;
+        gl[i] = make_float2(r0, r1);
+      }
+      float2* s_gt = reinterpret_cast<float2*>(s_m);  // totals of range 0 (s_m is free until the block merges)
+      if (rg == 0) s_gt[p] = make_float2(r0, r1);
+      __syncthreads();  // the K chunk is in s_k; the totals of range 0 are visible
+      const float2 base = rg ? s_gt[p] : make_float2(0.f, 0.f);
+      __half2* ks2 = reinterpret_cast<__half2*>(s_k);
+      __half2* k22 = reinterpret_cast<__half2*>(s_k2);
+#pragma unroll 8
+      for (int i = 0; i < 32; ++i) {
+        const int idx = ((32 * rg + i) * kKsPitch) / 2 + p;
+        const float2 kv = __half22float2(ks2[idx]);
+        const float G0 = base.x + gl[i].x, G1 = base.y + gl[i].y;
+        ks2[idx] = __floats2half2_rn(kv.x * __expf(G0), kv.y * __expf(G1));
+        k22[idx] = __floats2half2_rn(kv.x * __expf(-G0), kv.y * __expf(-G1));
+      }
+      if (rg == 1) {
+        s_g[2 * p] = base.x + r0;
+        s_g[2 * p + 1] = base.y + r1;
+      }
+      if (ci + 1 < kPrepChunksPerCta && metas[ci + 1].y > 0) prefetch(metas[ci + 1]);  // in flight during the rest
     } else {
       if (warp < 2) {
 #pragma unroll
@@ -222,7 +239,6 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
       *reinterpret_cast<uint4*>(out + kRecKt + off) = make_uint4(w[0], w[1], w[2], w[3]);
     }
   }
-
   // ---- a2: Gram K K^t, lower block triangle = 10 blocks of 16 x 16 (block row m, block column p <= m), dealt to the
   // warps as 3 + 2 + 3 + 2 so that no warp carries the whole last block row
   {
@@ -393,7 +409,6 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
         *reinterpret_cast<uint32_t*>(out + kRecW + off) = pack_f16(-wacc[nt][2 * hh], -wacc[nt][2 * hh + 1]);
       }
   }
-
   // ---- A_b = A diag(beta) as an fp16 B tile (K-major, 128B swizzle: row r, 16-byte chunk j8 at ((j8 ^ (r & 7)) * 16))
 #pragma unroll
   for (int it = 0; it < kC * 8 / kPrepThreads; ++it) {
