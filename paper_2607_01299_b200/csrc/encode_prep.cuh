@@ -110,6 +110,7 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
   uint8_t* s_k2 = reinterpret_cast<uint8_t*>(s_a);           // fp16 [64][kKsPitch]: exactly the size of s_a
   __shared__ __align__(16) float s_m[32 * kMPitch];         // temporaries of the block merges
   __shared__ __align__(16) float s_g[kCh ? kD : kC], s_b[kC], s_bg[kC];  // s_g: G_r per token (scalar) or G_C per channel
+  __shared__ __align__(16) float s_fc[kC];  // scalar gate: exp(-G_j), so that exp(G_r - G_j) = exp(G_r) exp(-G_j) costs no MUFU per entry of L
   __shared__ float s_wsum;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int gq = lane >> 2, tq = lane & 3;
@@ -214,6 +215,7 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
         s_g[tid] = gv;
         s_b[tid] = bv;
         s_bg[tid] = bv * expf(gv);
+        s_fc[tid] = expf(fminf(-gv, 80.f));  // <= e^9 inside the envelope; the clamp only keeps a violating chunk finite
       }
     }
   }
@@ -282,7 +284,8 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
       const int bi = blk < 3 ? 0 : (blk < 5 ? 1 : 2), bj = blk < 3 ? blk + 1 : (blk < 5 ? blk - 1 : 3);
       *reinterpret_cast<float4*>(s_a + (16 * bi + (e >> 2)) * kLPitch + 16 * bj + 4 * (e & 3)) = make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    // L_rj = beta_r exp(G_r - G_j) (k_r.k_j) for j < r, else 0
+    // L_rj = beta_r exp(G_r - G_j) (k_r.k_j) for j < r, else 0; the exponential is the product of two per-token factors
+    // prepared in a1 (one MUFU per token instead of one per entry, and no dependent LDS -> MUFU chain per entry)
 #pragma unroll
     for (int u = 0; u < 3; ++u) {
       if (u == 2 && nun < 3) continue;
@@ -290,13 +293,14 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
 #pragma unroll
       for (int hh = 0; hh < 2; ++hh) {
         const int r = 16 * mm + gq + 8 * hh;
-        const float br = s_b[r], gr = kCh ? 0.f : s_g[r];
+        const float br = kCh ? s_b[r] : s_bg[r];  // scalar gate: beta_r exp(G_r)
 #pragma unroll
         for (int nt = 0; nt < 2; ++nt) {
           const int j = 16 * pp + 8 * nt + 2 * tq;
+          const float2 fc = kCh ? make_float2(1.f, 1.f) : *reinterpret_cast<const float2*>(s_fc + j);
           float v0 = 0.f, v1 = 0.f;
-          if (j < r) v0 = br * (kCh ? 1.f : __expf(gr - s_g[j])) * acc[u][nt][2 * hh];
-          if (j + 1 < r) v1 = br * (kCh ? 1.f : __expf(gr - s_g[j + 1])) * acc[u][nt][2 * hh + 1];
+          if (j < r) v0 = br * fc.x * acc[u][nt][2 * hh];
+          if (j + 1 < r) v1 = br * fc.y * acc[u][nt][2 * hh + 1];
           *reinterpret_cast<float2*>(s_a + r * kLPitch + j) = make_float2(v0, v1);
         }
       }
