@@ -35,11 +35,11 @@ constexpr int kThreads = 608;         // warp 0 T producer, 1 MMA issuer, 2 E pr
 constexpr int kOffT = 0;
 constexpr int kOffE = kOffT + kNT * kTMat;
 constexpr int kOffXch = kOffE + kNE * kEQuarter;
-constexpr int kOffBar = kOffXch + 2048;
+constexpr int kOffBar = kOffXch + 4096;  // row maxima: one 2 KB exchange buffer per interleaved head
 constexpr int kSmemBytes = kOffBar + 512 + 1024;
 
 struct Bars {
-  uint64_t t_full[kNT], t_empty[kNT], e_full[kNE], e_empty[kNE], d_full, a_ready;
+  uint64_t t_full[kNT], t_empty[kNT], e_full[kNE], e_empty[kNE], d_full[2], a_ready[2];  // [head of the pair]
   uint32_t tmem_base;
   int abort_flag;
 };
@@ -105,6 +105,10 @@ int make_rows_tensor_map_f16(CUtensorMap* tm, const void* base, uint64_t rows) {
   return r == CUDA_SUCCESS ? HYPIC_OK : HYPIC_ERR_CUDA;
 }
 
+// kHeads = 2: the CTA folds heads h0, h0 + 1 of one request as two interleaved chains (they share the step list): while the
+// round-trip warps rewrite one head's state the tensor pipe multiplies the other's, instead of the strict
+// MMAs -> commit -> round trip -> barrier sequence of a single chain.  TMEM: 256 columns per head.
+template <int kHeads>
 __global__ void __launch_bounds__(kThreads, 1)
     compose_f16_kernel(const __grid_constant__ CUtensorMap tmE, const __grid_constant__ CUtensorMap tmT,
                        const float* __restrict__ S_in, const int32_t* __restrict__ seg_ids,
@@ -115,18 +119,20 @@ __global__ void __launch_bounds__(kThreads, 1)
   volatile int* abort_flag = &bars->abort_flag;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int unit = blockIdx.x;
-  const int r = unit / H, h = unit % H;
+  const int hp = H / kHeads;  // CTAs per request
+  const int r = blockIdx.x / hp, h0 = (blockIdx.x % hp) * kHeads;
   const int seg_begin = cu_segs[r];
   const int n = cu_segs[r + 1] - seg_begin;
   const size_t mat = (size_t)kD * kD;
 
-  if (warp == 0) tmem_alloc(&bars->tmem_base, 256);
+  if (warp == 0) tmem_alloc(&bars->tmem_base, 256 * kHeads);
   if (tid == 32) {
     for (int i = 0; i < kNT; ++i) { mbar_init(&bars->t_full[i], 1); mbar_init(&bars->t_empty[i], 1); }
     for (int i = 0; i < kNE; ++i) { mbar_init(&bars->e_full[i], 1); mbar_init(&bars->e_empty[i], 4); }
-    mbar_init(&bars->d_full, 1);
-    mbar_init(&bars->a_ready, 16);
+    for (int u = 0; u < 2; ++u) {
+      mbar_init(&bars->d_full[u], 1);
+      mbar_init(&bars->a_ready[u], 16);
+    }
     bars->abort_flag = 0;
     fence_barrier_init();
   }
@@ -134,14 +140,14 @@ __global__ void __launch_bounds__(kThreads, 1)
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = bars->tmem_base;
-  const uint32_t tD = tmem, tAhi = tmem + 128, tAlo = tmem + 192;  // D fp32 128 columns; S_hi, S_lo fp16 64 each
+  // per head u: D fp32 at columns [256 u, 256 u + 128); S_hi, S_lo fp16 at + 128, + 192 (64 columns each)
 
   if (warp == 0) {
     // ---------------------------------------------------------------- T producer: 32-row slabs, two boxes each
     if (lane == 0) {
       uint32_t it = 0;
-      for (int i = 0; i < n; ++i) {
-        const int row0 = (seg_ids[seg_begin + i] * H + h) * kD;
+      for (int i = 0; i < n * kHeads; ++i) {
+        const int row0 = (seg_ids[seg_begin + i / kHeads] * H + h0 + i % kHeads) * kD;
         const uint32_t slot = it % kNT, ph = (it / kNT) & 1;
         wait_or_abort(&bars->t_empty[slot], ph ^ 1, abort_flag);
         mbar_expect_tx(&bars->t_full[slot], kTMat);
@@ -158,10 +164,12 @@ __global__ void __launch_bounds__(kThreads, 1)
     if (lane == 0) {
       constexpr uint32_t idesc = make_idesc(0u, 128, 128, 0, 1);  // fp16, M = N = 128, A from TMEM, B MN-major
       uint32_t it = 0;
-      for (int i = 0; i < n; ++i) {
+      for (int v = 0; v < n * kHeads; ++v) {
+        const int i = v / kHeads, u = v % kHeads;
+        const uint32_t tD = tmem + 256 * u, tAhi = tD + 128, tAlo = tD + 192;
         const uint32_t slot = it % kNT, ph = (it / kNT) & 1;
         wait_or_abort(&bars->t_full[slot], ph, abort_flag);  // T runs ahead of the state: probe it first
-        wait_or_abort(&bars->a_ready, i & 1, abort_flag);
+        wait_or_abort(&bars->a_ready[u], i & 1, abort_flag);
         tc_fence_after();
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
@@ -177,15 +185,15 @@ __global__ void __launch_bounds__(kThreads, 1)
         }
         mma_commit(&bars->t_empty[slot]);
         ++it;
-        mma_commit(&bars->d_full);
+        mma_commit(&bars->d_full[u]);
       }
     }
   } else if (warp == 2) {
     // ---------------------------------------------------------------- E producer: per TMEM lane quarter, two boxes
     if (lane == 0) {
       uint32_t it = 0;
-      for (int i = 0; i < n; ++i) {
-        const int row0 = (seg_ids[seg_begin + i] * H + h) * kD;
+      for (int i = 0; i < n * kHeads; ++i) {
+        const int row0 = (seg_ids[seg_begin + i / kHeads] * H + h0 + i % kHeads) * kD;
         for (int q = 0; q < 4; ++q, ++it) {
           const uint32_t slot = it % kNE, ph = (it / kNE) & 1;
           wait_or_abort(&bars->e_empty[slot], ph ^ 1, abort_flag);
@@ -201,16 +209,24 @@ __global__ void __launch_bounds__(kThreads, 1)
     const int part = (warp - 3) >> 2;  // which 32 columns of the quarter this warp handles (4 warps per quarter)
     const uint32_t lane_base = (uint32_t)(32 * q) << 16;
     const int row = 32 * q + lane;
-    float* out_row = S_out + (size_t)unit * mat + (size_t)row * kD + 32 * part;
-    float* xch = reinterpret_cast<float*>(smem + kOffXch);
-    float unscale = 1.f;  // D of step s holds 2^-r_m (S T): r_m = this row's normalisation chosen after step s - 1
+    float unscale_u[kHeads];  // D of step s holds 2^-r_m (S T): r_m = this row's normalisation chosen after step s - 1
+#pragma unroll
+    for (int u = 0; u < kHeads; ++u) unscale_u[u] = 1.f;
     for (int s = -1; s < n; ++s) {
+#pragma unroll
+     for (int u = 0; u < kHeads; ++u) {
+      const size_t unit = (size_t)r * H + h0 + u;
+      const uint32_t tD = tmem + 256 * u, tAhi = tD + 128, tAlo = tD + 192;
+      float* out_row = S_out + unit * mat + (size_t)row * kD + 32 * part;
+      float* xch = reinterpret_cast<float*>(smem + kOffXch + 2048 * u);
+      float unscale = unscale_u[u];
       const bool last = (s == n - 1);
       float xv[32];
       if (s >= 0) {
-        const uint32_t eslot = (uint32_t)(4 * s + q) % kNE, eph = ((uint32_t)(4 * s + q) / kNE) & 1;
+        const uint32_t ev = (uint32_t)(4 * (kHeads * s + u) + q);
+        const uint32_t eslot = ev % kNE, eph = (ev / kNE) & 1;
         wait_or_abort(&bars->e_full[eslot], eph, abort_flag);  // E runs ahead: its probe overlaps the MMAs
-        wait_or_abort(&bars->d_full, s & 1, abort_flag);
+        wait_or_abort(&bars->d_full[u], s & 1, abort_flag);
         tc_fence_after();
         const uint8_t* eb = smem + kOffE + eslot * kEQuarter + (part >> 1) * (kEQuarter / 2) + lane * 128;
         uint32_t d[32];
@@ -230,7 +246,7 @@ __global__ void __launch_bounds__(kThreads, 1)
         __syncwarp();
         if (lane == 0) mbar_arrive(&bars->e_empty[eslot]);
       } else {
-        const float4* src = reinterpret_cast<const float4*>(S_in + (size_t)unit * mat + (size_t)row * kD + 32 * part);
+        const float4* src = reinterpret_cast<const float4*>(S_in + unit * mat + (size_t)row * kD + 32 * part);
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
           const float4 v = (S_in != nullptr) ? src[u] : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -254,7 +270,7 @@ __global__ void __launch_bounds__(kThreads, 1)
         int rs = (e == 0) ? 0 : e - 140;  // max in [2^(e-127), 2^(e-126)) -> 2^-rs max in [2^13, 2^14)
         rs = max(-100, min(100, rs));
         const float sc = __uint_as_float((uint32_t)(127 - rs) << 23);
-        unscale = __uint_as_float((uint32_t)(127 + rs) << 23);
+        unscale_u[u] = __uint_as_float((uint32_t)(127 + rs) << 23);
         uint32_t hi[16], lo[16];
 #pragma unroll
         for (int c = 0; c < 16; ++c) split_f16(xv[2 * c] * sc, xv[2 * c + 1] * sc, hi[c], lo[c]);
@@ -263,14 +279,15 @@ __global__ void __launch_bounds__(kThreads, 1)
         tmem_st_wait();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(&bars->a_ready);
+        if (lane == 0) mbar_arrive(&bars->a_ready[u]);
       }
+     }
     }
   }
 
   tc_fence_before();
   __syncthreads();
-  if (warp == 0) tmem_dealloc(tmem, 256);
+  if (warp == 0) tmem_dealloc(tmem, 256 * kHeads);
 }
 
 __global__ void pack_f16_kernel(const float* __restrict__ src, __half* __restrict__ dst, size_t n) {
@@ -293,7 +310,8 @@ int compose_f16(const ComposeF16Args& a) {
   if (a.R == 0) return HYPIC_OK;
   static bool configured = false;
   if (!configured) {
-    HYPIC_CUDA_OK(cudaFuncSetAttribute(compose_f16_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    HYPIC_CUDA_OK(cudaFuncSetAttribute(compose_f16_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    HYPIC_CUDA_OK(cudaFuncSetAttribute(compose_f16_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
     configured = true;
   }
   const long long units = (long long)a.R * a.H;
@@ -307,8 +325,12 @@ int compose_f16(const ComposeF16Args& a) {
     memset(&tmE, 0, sizeof(tmE));
     memset(&tmT, 0, sizeof(tmT));
   }
-  compose_f16_kernel<<<(unsigned)units, kThreads, kSmemBytes, a.stream>>>(tmE, tmT, a.S_in, a.seg_ids, a.cu_segs, a.H,
-                                                                         a.S_out);
+  if (a.H % 2 == 0)  // heads h, h + 1 of a request as two interleaved chains of one CTA
+    compose_f16_kernel<2><<<(unsigned)(units / 2), kThreads, kSmemBytes, a.stream>>>(tmE, tmT, a.S_in, a.seg_ids,
+                                                                                    a.cu_segs, a.H, a.S_out);
+  else
+    compose_f16_kernel<1><<<(unsigned)units, kThreads, kSmemBytes, a.stream>>>(tmE, tmT, a.S_in, a.seg_ids, a.cu_segs,
+                                                                              a.H, a.S_out);
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
   return HYPIC_OK;

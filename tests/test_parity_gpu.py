@@ -331,11 +331,12 @@ def test_tuple_pack_f16_is_ieee_rne():
     assert hb.hypic_tuple_pack_f16(torch.empty(0, device="cuda")).numel() == 0
 
 
-def test_compose_f16_pools_vs_oracle():
+@pytest.mark.parametrize("H", [3, 4])
+def test_compose_f16_pools_vs_oracle(H):
     """hypic_compose_f16: pools stored in fp16 (as the paper caches them) are exact inputs; the fold
     must match the fp64 compose of the same stored values to the fp32-input tolerance.  Near-unit pool (reading S9),
     lists of length 0, 1 and 39, repeated and unsorted ids, NULL and in-place S."""
-    P, H, d = 24, 3, 128
+    P, d = 24, 128  # H = 3: one chain per CTA; H = 4: heads h, h + 1 interleaved in one CTA
     pin = wl.near_unit_pool_inputs(P, H, device="cuda", d=d, kv_dtype=torch.float32)
     hb.hypic_set_impl(hb.HYPIC_IMPL_SIMT)
     E, T = hb.hypic_segment_encode(pin.k, pin.v, pin.g, pin.beta, pin.cu_seqlens, pin.gate)
