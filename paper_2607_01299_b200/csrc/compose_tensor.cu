@@ -45,11 +45,11 @@ constexpr int kOffHl = 0;
 constexpr int kOffRaw = kOffHl + kNHl * kHlBytes;
 constexpr int kOffE = kOffRaw + kNRaw * kSlabBytes;
 constexpr int kOffXch = kOffE + 4 * kESlotBytes;  // row maxima of the two column halves (round trip)
-constexpr int kOffBar = kOffXch + 1024;
+constexpr int kOffBar = kOffXch + 2048;  // one 1 KB exchange buffer per interleaved head
 constexpr int kSmemBytes = kOffBar + 256 + 1024;  // + barriers + alignment slack
 
 struct Bars {
-  uint64_t raw_full[kNRaw], raw_empty[kNRaw], hl_full[kNHl], hl_empty[kNHl], e_full[4], e_empty[4], d_full, a_ready;
+  uint64_t raw_full[kNRaw], raw_empty[kNRaw], hl_full[kNHl], hl_empty[kNHl], e_full[4], e_empty[4], d_full[2], a_ready[2];  // d_full, a_ready: [head of the pair]
   uint32_t tmem_base;
   int abort_flag;
 };
@@ -118,6 +118,10 @@ int make_rows_tensor_map(CUtensorMap* tm, const float* base, uint64_t rows) {
   return r == CUDA_SUCCESS ? HYPIC_OK : HYPIC_ERR_CUDA;
 }
 
+// kHeads = 2: the CTA folds heads h0, h0 + 1 of one request as two interleaved chains (they share the step list): while the
+// round-trip warps rewrite one head's state the tensor pipe multiplies the other's, instead of the strict
+// MMAs -> commit -> round trip -> barrier sequence of a single chain.  TMEM: 256 columns per head (512 = two heads).
+template <int kHeads>
 __global__ void __launch_bounds__(kThreads, 1)
     compose_tensor_kernel(const __grid_constant__ CUtensorMap tmE, const __grid_constant__ CUtensorMap tmS,
                           const float* __restrict__ S_in, const float* __restrict__ T_pool, const int32_t* __restrict__ seg_ids,
@@ -128,8 +132,8 @@ __global__ void __launch_bounds__(kThreads, 1)
   volatile int* abort_flag = &bars->abort_flag;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int unit = blockIdx.x;
-  const int r = unit / H, h = unit % H;
+  const int hp = H / kHeads;  // CTAs per request
+  const int r = blockIdx.x / hp, h0 = (blockIdx.x % hp) * kHeads;
   const int seg_begin = cu_segs[r];
   const int n = cu_segs[r + 1] - seg_begin;
   const size_t mat = (size_t)kD * kD;
@@ -139,8 +143,10 @@ __global__ void __launch_bounds__(kThreads, 1)
     for (int i = 0; i < kNRaw; ++i) { mbar_init(&bars->raw_full[i], 1); mbar_init(&bars->raw_empty[i], 4); }
     for (int i = 0; i < kNHl; ++i) { mbar_init(&bars->hl_full[i], 4); mbar_init(&bars->hl_empty[i], 1); }
     for (int i = 0; i < 4; ++i) { mbar_init(&bars->e_full[i], 1); mbar_init(&bars->e_empty[i], 2); }
-    mbar_init(&bars->d_full, 1);
-    mbar_init(&bars->a_ready, 8);
+    for (int u = 0; u < 2; ++u) {
+      mbar_init(&bars->d_full[u], 1);
+      mbar_init(&bars->a_ready[u], 8);
+    }
     bars->abort_flag = 0;
     fence_barrier_init();
   }
@@ -148,15 +154,15 @@ __global__ void __launch_bounds__(kThreads, 1)
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = bars->tmem_base;
-  const uint32_t tD = tmem, tAhi = tmem + 128, tAlo = tmem + 192;  // D fp32 128 columns; S_hi, S_lo fp16 64 each
+  // per head u: D fp32 at columns [256 u, 256 u + 128); S_hi, S_lo fp16 at + 128, + 192 (64 columns each)
 
   if (warp == 0) {
     // ---------------------------------------------------------------- T producer: 16 KB slabs into the raw ring
     if (lane == 0) {
       uint32_t it = 0;
-      for (int i = 0; i < n; ++i) {
-        const int id = seg_ids[seg_begin + i];
-        const float* Tg = T_pool + ((size_t)id * H + h) * mat;
+      for (int i = 0; i < n * kHeads; ++i) {
+        const int id = seg_ids[seg_begin + i / kHeads];
+        const float* Tg = T_pool + ((size_t)id * H + h0 + i % kHeads) * mat;
         for (int j = 0; j < 4; ++j, ++it) {
           const uint32_t slot = it % kNRaw, ph = (it / kNRaw) & 1;
           wait_or_abort(&bars->raw_empty[slot], ph ^ 1, abort_flag);
@@ -170,8 +176,10 @@ __global__ void __launch_bounds__(kThreads, 1)
     if (lane == 0) {
       constexpr uint32_t idesc = make_idesc(0u, 128, 128, 0, 1);  // fp16, M = N = 128, A from TMEM, B MN-major
       uint32_t it = 0;
-      for (int i = 0; i < n; ++i) {
-        wait_or_abort(&bars->a_ready, i & 1, abort_flag);
+      for (int v = 0; v < n * kHeads; ++v) {
+        const int i = v / kHeads, u = v % kHeads;
+        const uint32_t tD = tmem + 256 * u, tAhi = tD + 128, tAlo = tD + 192;
+        wait_or_abort(&bars->a_ready[u], i & 1, abort_flag);
         tc_fence_after();
         for (int j = 0; j < 4; ++j, ++it) {
           const uint32_t slot = it % kNHl, ph = (it / kNHl) & 1;
@@ -191,23 +199,24 @@ __global__ void __launch_bounds__(kThreads, 1)
           }
           mma_commit(&bars->hl_empty[slot]);
         }
-        mma_commit(&bars->d_full);
+        mma_commit(&bars->d_full[u]);
       }
     }
   } else if (warp == 2) {
     // ---------------------------------------------------------------- E producer: 4 TMA boxes (32 x 32 fp32) per slab
     if (lane < 4) {
       uint32_t ecount = 0;
-      for (int s = -1; s < n; ++s) {
+      for (int sv = -kHeads; sv < n * kHeads; ++sv) {
+        const int s = sv < 0 ? -1 : sv / kHeads, u = sv < 0 ? sv + kHeads : sv % kHeads;
         const CUtensorMap* tm;
         int row0;
         if (s < 0) {
           if (S_in == nullptr) continue;
           tm = &tmS;
-          row0 = unit * kD;
+          row0 = (r * H + h0 + u) * kD;
         } else {
           tm = &tmE;
-          row0 = (seg_ids[seg_begin + s] * H + h) * kD;
+          row0 = (seg_ids[seg_begin + s] * H + h0 + u) * kD;
         }
         for (int q = 0; q < 4; ++q) {
           wait_or_abort(&bars->e_empty[q], (ecount & 1) ^ 1, abort_flag);
@@ -222,7 +231,7 @@ __global__ void __launch_bounds__(kThreads, 1)
     // ---------------------------------------------------------------- converters: raw slab -> (hi, lo) tiles
     const int ctid = tid - 96;
     uint32_t it = 0;
-    for (int i = 0; i < n; ++i) {
+    for (int i = 0; i < n * kHeads; ++i) {
       for (int j = 0; j < 4; ++j, ++it) {
         const uint32_t rslot = it % kNRaw, rph = (it / kNRaw) & 1;
         const uint32_t hslot = it % kNHl, hph = (it / kNHl) & 1;
@@ -261,15 +270,21 @@ __global__ void __launch_bounds__(kThreads, 1)
     const uint32_t lane_base = (uint32_t)(32 * q) << 16;
     const int row = 32 * q + lane;
     const uint8_t* erow = smem + kOffE + q * kESlotBytes + lane * 128;
-    float* out_row = S_out + (size_t)unit * mat + (size_t)row * kD;
     uint32_t ecount = 0;
-    float* xch = reinterpret_cast<float*>(smem + kOffXch);
-    float unscale = 1.f;  // D of step s holds 2^(14 - r_m) (S T): r_m = this row's normalisation chosen after step s - 1
+    float unscale_u[kHeads];  // D of step s holds 2^(14 - r_m) (S T): r_m = this row's normalisation chosen after step s - 1
+#pragma unroll
+    for (int u = 0; u < kHeads; ++u) unscale_u[u] = 1.f;
     for (int s = -1; s < n; ++s) {
+#pragma unroll
+     for (int u = 0; u < kHeads; ++u) {
+      const uint32_t tD = tmem + 256 * u, tAhi = tD + 128, tAlo = tD + 192;
+      float* out_row = S_out + ((size_t)r * H + h0 + u) * mat + (size_t)row * kD;
+      float* xch = reinterpret_cast<float*>(smem + kOffXch + 1024 * u);
+      const float unscale = unscale_u[u];
       const bool have_e = (s >= 0) || (S_in != nullptr);
       const bool last = (s == n - 1);
       if (s >= 0) {
-        wait_or_abort(&bars->d_full, s & 1, abort_flag);
+        wait_or_abort(&bars->d_full[u], s & 1, abort_flag);
         tc_fence_after();
       }
       if (have_e) wait_or_abort(&bars->e_full[q], ecount & 1, abort_flag);
@@ -318,7 +333,7 @@ __global__ void __launch_bounds__(kThreads, 1)
         int r = (e == 0) ? 0 : e - 140;  // max in [2^(e-127), 2^(e-126)) -> 2^-r max in [2^13, 2^14)
         r = max(-100, min(100, r));
         const float sc = __uint_as_float((uint32_t)(127 - r) << 23);
-        unscale = __uint_as_float((uint32_t)(127 + r - 14) << 23);
+        unscale_u[u] = __uint_as_float((uint32_t)(127 + r - 14) << 23);
         uint32_t hi[32], lo[32];
 #pragma unroll
         for (int c = 0; c < 32; ++c) split_f16(xv[2 * c] * sc, xv[2 * c + 1] * sc, hi[c], lo[c]);
@@ -327,8 +342,9 @@ __global__ void __launch_bounds__(kThreads, 1)
         tmem_st_wait();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(&bars->a_ready);
+        if (lane == 0) mbar_arrive(&bars->a_ready[u]);
       }
+     }
     }
   }
 
@@ -346,7 +362,8 @@ int compose_tensor(const ComposeArgs& a) {
   if (a.R == 0) return HYPIC_OK;
   static bool configured = false;
   if (!configured) {
-    HYPIC_CUDA_OK(cudaFuncSetAttribute(compose_tensor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    HYPIC_CUDA_OK(cudaFuncSetAttribute(compose_tensor_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    HYPIC_CUDA_OK(cudaFuncSetAttribute(compose_tensor_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
     configured = true;
   }
   const long long units = (long long)a.R * a.H;
@@ -364,8 +381,12 @@ int compose_tensor(const ComposeArgs& a) {
     const int rc = make_rows_tensor_map(&tmS, a.S_in, (uint64_t)units * kD);
     if (rc != HYPIC_OK) return rc;
   }
-  compose_tensor_kernel<<<(unsigned)units, kThreads, kSmemBytes, a.stream>>>(tmE, tmS, a.S_in, a.T_pool, a.seg_ids,
-                                                                            a.cu_segs, a.H, a.S_out);
+  if (a.H % 2 == 0)  // heads h, h + 1 of a request as two interleaved chains of one CTA
+    compose_tensor_kernel<2><<<(unsigned)(units / 2), kThreads, kSmemBytes, a.stream>>>(tmE, tmS, a.S_in, a.T_pool,
+                                                                                       a.seg_ids, a.cu_segs, a.H, a.S_out);
+  else
+    compose_tensor_kernel<1><<<(unsigned)units, kThreads, kSmemBytes, a.stream>>>(tmE, tmS, a.S_in, a.T_pool, a.seg_ids,
+                                                                                 a.cu_segs, a.H, a.S_out);
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
   return HYPIC_OK;

@@ -133,11 +133,12 @@ def test_encode_degenerate_inputs(name, impl):
 
 # ------------------------------------------------------------------------------------------ compose
 @pytest.mark.parametrize("name,impl", IMPLS)
+@pytest.mark.parametrize("H", [3, 4])
 @pytest.mark.parametrize("d", [128, 64])
-def test_compose_near_unit_pool(name, impl, d):
+def test_compose_near_unit_pool(name, impl, d, H):
     """Reading S9: pool with ||T||_F = O(1..10) (short segments, weak decay), so S.T is not negligible; fp32
     pools vs fp64 compose of the same pools -> 1e-5.  Lists of length 0, 1 and up to 40; unsorted ids."""
-    P, H = 24, 3
+    P = 24  # H = 3: one chain per CTA in the tensor family; H = 4: heads h, h + 1 interleaved in one CTA
     pin = wl.near_unit_pool_inputs(P, H, device="cuda", d=d, kv_dtype=torch.float32)
     hb.hypic_set_impl(hb.HYPIC_IMPL_SIMT)
     E, T = hb.hypic_segment_encode(pin.k, pin.v, pin.g, pin.beta, pin.cu_seqlens, pin.gate)
