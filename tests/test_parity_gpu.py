@@ -728,3 +728,25 @@ def test_forward_encode_vs_oracle(gate, kv, d, dv):
         E2, T2 = hb.hypic_segment_encode(e.k, e.v, e.g, e.beta, e.cu_seqlens, e.gate)
         check_E(E2, E.cpu().numpy(), TOL_BF16, "E (tensor family vs forward-encode)")
         check_T(T2, T.cpu().numpy(), TOL_BF16, "T (tensor family vs forward-encode)")
+
+
+def test_compose_interleaved_heads_every_unit():
+    """R x H = 40 x 8 = 320 chains: enough for the tensor-family compose kernels to fold heads h, h + 1 of a request as
+    two interleaved chains of one CTA (below 2 x 148 units they run one chain per CTA).  Every unit against the oracle,
+    fp32 pools and fp16-stored pools; lists of length 0..12 with repeated, unsorted ids; NULL S_in as well."""
+    P, H, d, R = 16, 8, 128, 40
+    pin = wl.near_unit_pool_inputs(P, H, device="cuda", d=d, kv_dtype=torch.float32)
+    with impl_family(hb.HYPIC_IMPL_SIMT):
+        E, T = hb.hypic_segment_encode(pin.k, pin.v, pin.g, pin.beta, pin.cu_seqlens, pin.gate)
+    req = wl.make_compose_requests(R, P, H, d, d, n_lo=0, n_hi=12, seed=78, device="cuda", s_in_std=1.0)
+    ids, cu = req.seg_ids.cpu().numpy(), req.cu_segs.cpu().numpy()
+    for S_in in (req.S_in, None):
+        s_host = None if S_in is None else S_in.cpu().numpy()
+        S = gpu_compose(S_in, E, T, req.seg_ids, req.cu_segs, hb.HYPIC_IMPL_TENSOR)
+        check_E(S, oracle.compose(s_host, E.cpu().numpy(), T.cpu().numpy(), ids, cu), TOL_F32, "S_out (fp32 pools)")
+        Eh, Th = hb.hypic_tuple_pack_f16(E), hb.hypic_tuple_pack_f16(T)
+        Sh = hb.hypic_compose_f16(S_in, Eh, Th, req.seg_ids, req.cu_segs)
+        torch.cuda.synchronize()
+        check_E(Sh, oracle.compose(s_host, Eh.float().cpu().numpy(), Th.float().cpu().numpy(), ids, cu), TOL_F32,
+                "S_out (fp16 pools)")
+    assert hb.hypic_debug_timeout_count() == 0
