@@ -249,7 +249,7 @@ __global__ void __launch_bounds__(kDcThreads)
   }
   const int dk4 = dk / 4;
   const int j0 = cu_segs[r], j1 = cu_segs[r + 1];
-  float4 e_nxt[kDcV4], t_nxt[kDcV4];
+  float4 e_nxt[kDcV4], t_nxt[CHANNEL ? kDcV4 : 1];  // scalar family: one decay per step (t_nxt[0].x)
   auto fetch = [&](int j) {
     const size_t ph = (size_t)seg_ids[j] * H + h;
 #pragma unroll
@@ -262,20 +262,19 @@ __global__ void __launch_bounds__(kDcThreads)
         } else {
           e_nxt[i] = __ldcs(reinterpret_cast<const float4*>(E_pool) + ph * unit_v4 + e4[i]);
         }
-        if (CHANNEL) {
-          t_nxt[i] = __ldg(reinterpret_cast<const float4*>(t_pool + ph * dk) + e4[i] % dk4);
-        } else {
-          const float ts = __ldg(t_pool + ph);
-          t_nxt[i] = make_float4(ts, ts, ts, ts);
-        }
+        if (CHANNEL) t_nxt[i] = __ldg(reinterpret_cast<const float4*>(t_pool + ph * dk) + e4[i] % dk4);
       }
     }
+    if (!CHANNEL) t_nxt[0].x = __ldg(t_pool + ph);
   };
   if (j0 < j1) fetch(j0);
   for (int j = j0; j < j1; ++j) {
     float4 e_cur[kDcV4], t_cur[kDcV4];
 #pragma unroll
-    for (int i = 0; i < kDcV4; ++i) e_cur[i] = e_nxt[i], t_cur[i] = t_nxt[i];
+    for (int i = 0; i < kDcV4; ++i) {
+      e_cur[i] = e_nxt[i];
+      t_cur[i] = CHANNEL ? t_nxt[CHANNEL ? i : 0] : make_float4(t_nxt[0].x, t_nxt[0].x, t_nxt[0].x, t_nxt[0].x);
+    }
     if (j + 1 < j1) fetch(j + 1);
 #pragma unroll
     for (int i = 0; i < kDcV4; ++i) {
