@@ -318,7 +318,7 @@ __device__ __forceinline__ void sts32(uint32_t addr, uint32_t v) {
   asm volatile("st.shared.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 
-__global__ void __launch_bounds__(kDtThreads, 2)
+__global__ void __launch_bounds__(kDtThreads, 3)
     diag_scan_ch_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
                         const float* __restrict__ g, const int32_t* __restrict__ cu_seqlens, int H, float* __restrict__ E,
                         float* __restrict__ tvec) {
@@ -397,32 +397,26 @@ __global__ void __launch_bounds__(kDtThreads, 2)
     const int p = tid & 63, r = tid >> 6;
     double carry0 = 0.0, carry1 = 0.0;  // log-decay of all tokens after the current chunk, channels 2p and 2p + 1
     double dsum0 = 0.0, dsum1 = 0.0;    // this thread's tokens only, for tvec
-    float2 gn[16];
-    auto load_g = [&](int i) {
-      const int tb = seg_begin + (nc - 1 - i) * kC + 16 * r;
-#pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        gn[j] = make_float2(0.f, 0.f);
-        if (i < nc && tb + j < seg_end) gn[j] = __ldg(reinterpret_cast<const float2*>(g + ((size_t)(tb + j) * H + h) * kD) + p);
-      }
+    float2 gn[16];  // log-decays of this thread's 16 tokens x 2 channels of the current chunk; refilled in place, token
+                    // by token, with the next chunk's as soon as each has been used (prefetch without a second array)
+    auto load_g1 = [&](int i, int j) {
+      const int t = seg_begin + (nc - 1 - i) * kC + 16 * r + j;
+      return (i < nc && t < seg_end) ? __ldg(reinterpret_cast<const float2*>(g + ((size_t)t * H + h) * kD) + p)
+                                     : make_float2(0.f, 0.f);
     };
-    load_g(0);
+#pragma unroll
+    for (int j = 0; j < 16; ++j) gn[j] = load_g1(0, j);
     // K tile address of (token row 16 r + j, channel pair p): box p / 32, 128-byte rows, 16-byte chunks XOR-swizzled by row
     const uint32_t k_box = (uint32_t)(p >> 5) * 8192u, k_chunk = (uint32_t)((p & 31) >> 2), k_in = (uint32_t)(p & 3) * 4u;
 #pragma unroll 1
     for (int i = 0; i < nc; ++i) {
       const int st = i % kDtStages;
       const int t0 = seg_begin + (nc - 1 - i) * kC;
-      float lw0[16], lw1[16];
       float s0 = 0.f, s1 = 0.f;
 #pragma unroll
-      for (int j = 15; j >= 0; --j) {  // exclusive suffix sums inside this thread's 16 tokens
-        lw0[j] = s0, lw1[j] = s1;
-        s0 += gn[j].x, s1 += gn[j].y;
-        dsum0 += (double)gn[j].x, dsum1 += (double)gn[j].y;
-      }
+      for (int j = 0; j < 16; ++j) s0 += gn[j].x, s1 += gn[j].y;
+      dsum0 += (double)s0, dsum1 += (double)s1;  // 16-term fp32 sums, accumulated over the chunks in fp64
       xs->tot[i & 1][r][p] = make_float2(s0, s1);
-      load_g(i + 1);  // next chunk's log-decays: in flight during this chunk's conversion
       asm volatile("bar.sync 1, 256;" ::: "memory");
       float later0 = 0.f, later1 = 0.f, all0 = 0.f, all1 = 0.f;
 #pragma unroll
@@ -431,19 +425,21 @@ __global__ void __launch_bounds__(kDtThreads, 2)
         if (rr > r) later0 += t.x, later1 += t.y;
         all0 += t.x, all1 += t.y;
       }
-      const float b0 = (float)carry0 + later0, b1 = (float)carry1 + later1;
+      float run0 = (float)carry0 + later0, run1 = (float)carry1 + later1;  // log-weight of the range's LAST token
       carry0 += (double)all0, carry1 += (double)all1;
       s2_wait_warp(&bars->full[st], (i / kDtStages) & 1, abort_flag, lane);
       const uint32_t tile = smem_base + st * kDtStageBytes;
 #pragma unroll
-      for (int j = 0; j < 16; ++j) {
+      for (int j = 15; j >= 0; --j) {
         const int tr = 16 * r + j;
         const uint32_t addr = tile + k_box + (uint32_t)tr * 128u + ((k_chunk ^ (uint32_t)(tr & 7)) << 4) + k_in;
         const uint32_t x = lds32(addr);
         uint32_t y = 0u;
         if (t0 + tr < seg_end)
-          y = pack_f16(__uint_as_float(x << 16) * __expf(b0 + lw0[j]), __uint_as_float(x & 0xffff0000u) * __expf(b1 + lw1[j]));
+          y = pack_f16(__uint_as_float(x << 16) * __expf(run0), __uint_as_float(x & 0xffff0000u) * __expf(run1));
         sts32(addr, y);
+        run0 += gn[j].x, run1 += gn[j].y;  // weight of token j - 1: everything after it, token j included
+        gn[j] = load_g1(i + 1, j);         // next chunk's log-decays: in flight during the rest of this conversion
       }
       // V tile: bf16 -> fp16 in place, rows past the segment zeroed
 #pragma unroll
