@@ -52,6 +52,7 @@ struct Bars {
   uint64_t raw_full[kNRaw], raw_empty[kNRaw], hl_full[kNHl], hl_empty[kNHl], e_full[4], e_empty[4], d_full[2], a_ready[2];  // d_full, a_ready: [head of the pair]
   uint32_t tmem_base;
   int abort_flag;
+  int req_pick;  // LPT order: the request this CTA folds
 };
 
 __device__ __forceinline__ bool wait_or_abort(uint64_t* bar, uint32_t parity, volatile int* abort_flag) {
@@ -125,7 +126,7 @@ template <int kHeads>
 __global__ void __launch_bounds__(kThreads, 1)
     compose_tensor_kernel(const __grid_constant__ CUtensorMap tmE, const __grid_constant__ CUtensorMap tmS,
                           const float* __restrict__ S_in, const float* __restrict__ T_pool, const int32_t* __restrict__ seg_ids,
-                          const int32_t* __restrict__ cu_segs, int H, float* __restrict__ S_out) {
+                          const int32_t* __restrict__ cu_segs, int R, int H, float* __restrict__ S_out) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   Bars* bars = reinterpret_cast<Bars*>(smem + kOffBar);
@@ -133,7 +134,29 @@ __global__ void __launch_bounds__(kThreads, 1)
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int hp = H / kHeads;  // CTAs per request
-  const int r = blockIdx.x / hp, h0 = (blockIdx.x % hp) * kHeads;
+  // Longest lists first (the hardware hands out CTAs in index order, so the last CTAs set the tail of the launch): the
+  // request this CTA folds is the one whose list length has rank blockIdx.x / hp, ties by index.  Each CTA ranks the
+  // R <= 512 lengths itself from shared memory (a microsecond); beyond that, index order.
+  int r = blockIdx.x / hp;
+  if (R <= 512) {
+    int* s_len = reinterpret_cast<int*>(smem + kOffXch);  // free until the first round trip
+    int* s_pick = &bars->req_pick;
+    for (int t = threadIdx.x; t < R; t += kThreads) s_len[t] = cu_segs[t + 1] - cu_segs[t];
+    __syncthreads();
+    for (int t = threadIdx.x; t < R; t += kThreads) {
+      const int lt = s_len[t];
+      int rank = 0;
+      for (int j = 0; j < R; ++j) {
+        const int lj = s_len[j];
+        rank += (lj > lt || (lj == lt && j < t)) ? 1 : 0;
+      }
+      if (rank == r) *s_pick = t;
+    }
+    __syncthreads();
+    r = *s_pick;
+    __syncthreads();  // s_len is the exchange buffer of the round trip from here on
+  }
+  const int h0 = (blockIdx.x % hp) * kHeads;
   const int seg_begin = cu_segs[r];
   const int n = cu_segs[r + 1] - seg_begin;
   const size_t mat = (size_t)kD * kD;
@@ -386,10 +409,10 @@ int compose_tensor(const ComposeArgs& a) {
   const DeviceInfo& di = device_info();
   if (a.H % 2 == 0 && units >= 2LL * (di.ok ? di.sm_count : 148))
     compose_tensor_kernel<2><<<(unsigned)(units / 2), kThreads, kSmemBytes, a.stream>>>(tmE, tmS, a.S_in, a.T_pool,
-                                                                                       a.seg_ids, a.cu_segs, a.H, a.S_out);
+                                                                                       a.seg_ids, a.cu_segs, a.R, a.H, a.S_out);
   else
     compose_tensor_kernel<1><<<(unsigned)units, kThreads, kSmemBytes, a.stream>>>(tmE, tmS, a.S_in, a.T_pool, a.seg_ids,
-                                                                                 a.cu_segs, a.H, a.S_out);
+                                                                                 a.cu_segs, a.R, a.H, a.S_out);
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
   return HYPIC_OK;
