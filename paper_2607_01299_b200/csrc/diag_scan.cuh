@@ -60,6 +60,31 @@ __device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
   asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
+// Longest segments first (CTAs are handed out in index order, so the last ones set the tail of a launch with ragged
+// segments): the segment of rank blockIdx.y by length, ties by index; every CTA ranks the n_seg <= 512 lengths itself in
+// shared memory.  `scratch` (>= 2 KB + 4 B) is free until the pipeline starts; beyond 512 segments, index order.
+__device__ __forceinline__ int dt_pick_segment(const int32_t* __restrict__ cu_seqlens, int n_seg, int* scratch) {
+  int s = blockIdx.y;
+  if (n_seg > 512) return s;
+  int* s_len = scratch;
+  int* s_pick = scratch + 512;
+  for (int t = threadIdx.x; t < n_seg; t += blockDim.x) s_len[t] = cu_seqlens[t + 1] - cu_seqlens[t];
+  __syncthreads();
+  for (int t = threadIdx.x; t < n_seg; t += blockDim.x) {
+    const int lt = s_len[t];
+    int rank = 0;
+    for (int j = 0; j < n_seg; ++j) {
+      const int lj = s_len[j];
+      rank += (lj > lt || (lj == lt && j < t)) ? 1 : 0;
+    }
+    if (rank == s) *s_pick = t;
+  }
+  __syncthreads();
+  s = *s_pick;
+  __syncthreads();
+  return s;
+}
+
 // kSplit = 2: the unit is shared by a cluster of two CTAs (blockIdx.z = rank): rank 1 streams the later half of the chunks
 // and writes its sum E_1 to the unit's place in E; rank 0 streams the earlier half with weights relative to ITS last
 // token, learns rank 1's total log-decay G_1 through distributed shared memory, and after the cluster barrier writes
@@ -75,7 +100,8 @@ __device__ __forceinline__ void diag_scan_body(const CUtensorMap& tmK, const CUt
   float* sw = reinterpret_cast<float*>(smem + kDtOffW);
   volatile int* abort_flag = &bars->abort_flag;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int h = blockIdx.x, s = blockIdx.y;
+  const int h = blockIdx.x;
+  const int s = dt_pick_segment(cu_seqlens, (int)gridDim.y, reinterpret_cast<int*>(smem));  // stage 0 is still empty
   const int seg_begin = cu_seqlens[s], seg_end = cu_seqlens[s + 1];
   const int nc_tot = (seg_end - seg_begin + kC - 1) / kC;
   const int rank = kSplit == 2 ? (int)blockIdx.z : 0;
@@ -328,7 +354,8 @@ __global__ void __launch_bounds__(kDtThreads, 3)
   DtChShared* xs = reinterpret_cast<DtChShared*>(smem + kDtChOffX);
   volatile int* abort_flag = &bars->abort_flag;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int h = blockIdx.x, s = blockIdx.y;
+  const int h = blockIdx.x;
+  const int s = dt_pick_segment(cu_seqlens, (int)gridDim.y, reinterpret_cast<int*>(smem));  // stage 0 is still empty
   const int seg_begin = cu_seqlens[s], seg_end = cu_seqlens[s + 1];
   const int nc = (seg_end - seg_begin + kC - 1) / kC;
   float* Eu = E + ((size_t)s * H + h) * kD * kD;
