@@ -232,7 +232,9 @@ unsigned int hypic_debug_timeout_count(void);
  * cumulative log-decay of every 64-token chunk stays above -9 (gamma >= 1.2e-4 inside a chunk; the benchmark
  * distributions stay above -6.4) and that g and beta are finite.  Its prep kernel counts the (chunk, head) pairs that
  * break this since library load; such pairs may come out with a relative error above the family's tolerance, and the
- * caller should re-run the call with HYPIC_IMPL_SIMT, which has no such limit.  Synchronises the device; 0 = never
+ * caller should re-run the call with HYPIC_IMPL_SIMT, which has no such limit.  The tcgen05 kernels of hypic_diag_encode
+ * add to the same counter for every 64-token chunk (per warp of 64 or 512 log-decays) that holds a positive or non-finite
+ * log-decay (their fp16 weights exp(sum of later log-decays) must not exceed 1).  Synchronises the device; 0 = never
  * violated; 0xffffffff = the query itself failed.
  */
 unsigned int hypic_envelope_violation_count(void);

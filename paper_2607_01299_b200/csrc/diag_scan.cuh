@@ -159,6 +159,9 @@ __device__ __forceinline__ void diag_scan_body(const CUtensorMap& tmK, const CUt
       const float ga = ga0, gb = gb0;
       ga0 = ga1, gb0 = gb1;
       load_g(i + 2, ga1, gb1);
+      // envelope: the fp16 weights assume log-decays <= 0 (and finite); a chunk that breaks this is counted, like the dense
+      // family's violations (hypic_envelope_violation_count), and should be re-run on the fp32 kernel
+      if (__any_sync(0xffffffffu, !(ga <= 0.f) || !(gb <= 0.f)) && lane == 0) atomicAdd(&g_envelope_count_enc, 1u);
       S2_STAMPW(kDtConvWarps + 1, 0, i, 3);
       if (i >= kDtStages) {
         if (lane == 0) dt_wait(&bars->free_[st], ((i / kDtStages) & 1) ^ 1, abort_flag);
@@ -440,8 +443,13 @@ __global__ void __launch_bounds__(kDtThreads, 3)
       const int st = i % kDtStages;
       const int t0 = seg_begin + (nc - 1 - i) * kC;
       float s0 = 0.f, s1 = 0.f;
+      bool bad = false;  // envelope: log-decays <= 0 and finite (see the scalar kernel)
 #pragma unroll
-      for (int j = 0; j < 16; ++j) s0 += gn[j].x, s1 += gn[j].y;
+      for (int j = 0; j < 16; ++j) {
+        s0 += gn[j].x, s1 += gn[j].y;
+        bad = bad || !(gn[j].x <= 0.f) || !(gn[j].y <= 0.f);
+      }
+      if (__any_sync(0xffffffffu, bad) && lane == 0) atomicAdd(&g_envelope_count_enc, 1u);
       dsum0 += (double)s0, dsum1 += (double)s1;  // 16-term fp32 sums, accumulated over the chunks in fp64
       xs->tot[i & 1][r][p] = make_float2(s0, s1);
       asm volatile("bar.sync 1, 256;" ::: "memory");

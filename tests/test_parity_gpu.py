@@ -586,6 +586,28 @@ def test_diag_encode_tensor_unsplit_schedule():
     _check_tvec(tv, t_ref, TOL_F32)
 
 
+@pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
+def test_diag_encode_tensor_envelope_guard(gate):
+    """The tcgen05 kernels of the scalar / diagonal families assume log-decays <= 0; a call that breaks this is counted
+    (and the fp32 kernel handles it)."""
+    inp = wl.make_encode_inputs([200, 64], 2, 128, 128, kv_dtype=torch.bfloat16, gate=gate, g_lo=-0.1,
+                                seed=wl.seed_for(6, 7), device="cuda")
+    before = hb.hypic_envelope_violation_count()
+    gpu_diag_encode(inp, hb.HYPIC_IMPL_TENSOR)
+    assert hb.hypic_envelope_violation_count() == before  # inside the envelope: nothing counted
+    g_bad = inp.g.clone()
+    g_bad[70] = 0.5  # growth instead of decay on one token
+    bad = wl.EncodeInputs(k=inp.k, v=inp.v, g=g_bad, beta=inp.beta, cu_seqlens=inp.cu_seqlens, gate=inp.gate,
+                          seg_lens=inp.seg_lens)
+    gpu_diag_encode(bad, hb.HYPIC_IMPL_TENSOR)
+    assert hb.hypic_envelope_violation_count() > before
+    E, tv = gpu_diag_encode(bad, hb.HYPIC_IMPL_SIMT)  # the fp32 kernel has no such limit
+    c = bad.cpu()
+    E_ref, t_ref = oracle.diag_encode(c.k, c.v, c.g, c.cu_seqlens, gate=c.gate)
+    check_E(E, E_ref, TOL_F32, "E (fp32 kernel, growing gate)")
+    _check_tvec(tv, t_ref, TOL_F32)
+
+
 def test_diag_encode_tensor_channel_gate_full_size_sampled_units():
     """Diagonal family (GLA) on the tcgen05 kernel at the bench shape (20 x 4096 tokens, H = 32, per-channel gate with a
     milder decay so that tvec stays representable): sampled units against the oracle, tvec of those units included."""
