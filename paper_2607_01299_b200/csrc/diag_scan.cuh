@@ -333,7 +333,6 @@ __global__ void __cluster_dims__(1, 1, 2) __launch_bounds__(kDtThreads, 3)
 // memory (one named barrier per chunk), and folds exp(.) into its 16 x 2 entries of the K tile with 32-bit accesses.
 struct DtChShared {
   float2 tot[2][4][64];   // [chunk parity][token range][channel pair]: log-decay summed over the range
-  double dsum[4][64][2];  // end of the segment: fp64 partial sums per (range, pair, channel of the pair)
 };
 constexpr int kDtChOffX = kDtOffBar + 128;
 constexpr int kDtChSmem = kDtChOffX + (int)sizeof(DtChShared) + 1024;
@@ -426,7 +425,6 @@ __global__ void __launch_bounds__(kDtThreads, 3)
     static_assert(kDtConvWarps == 8, "thread map below: 64 channel pairs x 4 token ranges");
     const int p = tid & 63, r = tid >> 6;
     double carry0 = 0.0, carry1 = 0.0;  // log-decay of all tokens after the current chunk, channels 2p and 2p + 1
-    double dsum0 = 0.0, dsum1 = 0.0;    // this thread's tokens only, for tvec
     float2 gn[16];  // log-decays of this thread's 16 tokens x 2 channels of the current chunk; refilled in place, token
                     // by token, with the next chunk's as soon as each has been used (prefetch without a second array)
     auto load_g1 = [&](int i, int j) {
@@ -443,14 +441,11 @@ __global__ void __launch_bounds__(kDtThreads, 3)
       const int st = i % kDtStages;
       const int t0 = seg_begin + (nc - 1 - i) * kC;
       float s0 = 0.f, s1 = 0.f;
-      bool bad = false;  // envelope: log-decays <= 0 and finite (see the scalar kernel)
 #pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        s0 += gn[j].x, s1 += gn[j].y;
-        bad = bad || !(gn[j].x <= 0.f) || !(gn[j].y <= 0.f);
-      }
-      if (__any_sync(0xffffffffu, bad) && lane == 0) atomicAdd(&g_envelope_count_enc, 1u);
-      dsum0 += (double)s0, dsum1 += (double)s1;  // 16-term fp32 sums, accumulated over the chunks in fp64
+      for (int j = 0; j < 16; ++j) s0 += gn[j].x, s1 += gn[j].y;
+      // envelope: log-decays <= 0 and finite (see the scalar kernel): a NaN / inf shows in the sums, a positive one in the
+      // running maximum taken while the values are consumed below
+      float gmax = (fabsf(s0) + fabsf(s1) < 3.0e38f) ? -1.f : 1.f;
       xs->tot[i & 1][r][p] = make_float2(s0, s1);
       asm volatile("bar.sync 1, 256;" ::: "memory");
       float later0 = 0.f, later1 = 0.f, all0 = 0.f, all1 = 0.f;
@@ -474,8 +469,10 @@ __global__ void __launch_bounds__(kDtThreads, 3)
           y = pack_f16(__uint_as_float(x << 16) * __expf(run0), __uint_as_float(x & 0xffff0000u) * __expf(run1));
         sts32(addr, y);
         run0 += gn[j].x, run1 += gn[j].y;  // weight of token j - 1: everything after it, token j included
+        gmax = fmaxf(gmax, fmaxf(gn[j].x, gn[j].y));
         gn[j] = load_g1(i + 1, j);         // next chunk's log-decays: in flight during the rest of this conversion
       }
+      if (__any_sync(0xffffffffu, gmax > 0.f) && lane == 0) atomicAdd(&g_envelope_count_enc, 1u);
       // V tile: bf16 -> fp16 in place, rows past the segment zeroed
 #pragma unroll
       for (int it = 0; it < 4; ++it) {
@@ -493,15 +490,9 @@ __global__ void __launch_bounds__(kDtThreads, 3)
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars->conv[st]);
     }
-    // tvec: fp64 sums of the four token ranges of every channel
-    xs->dsum[r][p][0] = dsum0;
-    xs->dsum[r][p][1] = dsum1;
-    asm volatile("bar.sync 1, 256;" ::: "memory");
-    if (r == 0) {
-      const double a0 = xs->dsum[0][p][0] + xs->dsum[1][p][0] + xs->dsum[2][p][0] + xs->dsum[3][p][0];
-      const double a1 = xs->dsum[0][p][1] + xs->dsum[1][p][1] + xs->dsum[2][p][1] + xs->dsum[3][p][1];
-      *reinterpret_cast<float2*>(tv + 2 * p) = make_float2((float)exp(a0), (float)exp(a1));
-    }
+    // tvec: the carry is now the log-decay of the whole segment (64-term fp32 chunk sums accumulated in fp64; the four
+    // range-threads of a channel pair hold the same value)
+    if (r == 0) *reinterpret_cast<float2*>(tv + 2 * p) = make_float2((float)exp(carry0), (float)exp(carry1));
     // ----------------------------------------------------------------------------------------------- epilogue
     s2_wait_warp(&bars->done, 0, abort_flag, lane);
     tc_fence_after();
