@@ -255,6 +255,17 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
         for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x1[2 * j]), __uint_as_float(x1[2 * j + 1]));
         tmem_st16(tH + 16, hh);
       }
+      tmem_st_wait();  // Xh is in TMEM; the decayed X follows while (3) runs (only (4) needs it)
+      tc_fence_before();
+      named_bar_sync(5 + b, 256);  // the whole chain has written Xh
+      S2_STAMP(b, c, 1);
+      if (issuer) {
+        if (!kIsT) s2_wait_count(&bars->issued1_cnt, c, abort_flag);  // (1)_c is ahead of (3)_c in the tensor pipe
+        tc_fence_after();
+        s2_issue3(tmem, smem_base + st * kS2StageBytes, b);
+        mma_commit(&bars->m3_done[b]);
+      }
+      __syncwarp();
       if (kCh) {
         const float4* gv = reinterpret_cast<const float4*>(gt + 64 * hf);
 #pragma unroll
@@ -277,16 +288,6 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
       S2_STAMP(b, c, 6);
       tmem_st_wait();
     }
-    tc_fence_before();
-    named_bar_sync(5 + b, 256);  // the whole chain has written Xh / X
-    S2_STAMP(b, c, 1);
-    if (issuer) {
-      if (!kIsT) s2_wait_count(&bars->issued1_cnt, c, abort_flag);  // (1)_c is ahead of (3)_c in the tensor pipe
-      tc_fence_after();
-      s2_issue3(tmem, smem_base + st * kS2StageBytes, b);
-      mma_commit(&bars->m3_done[b]);
-    }
-    __syncwarp();
 
     // ---- epilogue: U''[:, j] = fp16(DY[:, j] d_j) -> TMEM (A operand of (4)); this thread: tokens [32 hf, 32 hf + 32)
     s2_wait_warp(&bars->m3_done[b], c & 1, abort_flag, lane);
