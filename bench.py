@@ -188,40 +188,52 @@ def run_reference(args):
 # GPU arm
 # ------------------------------------------------------------------------------------------------------------
 class Cfg2Request:
-    """One RAG-shaped request (cfg2) resident in HBM: per-layer inputs, (E, T) pools, composed state."""
+    """One RAG-shaped request (cfg2) resident in HBM: inputs, (E, T) pools and composed state of its layers.
 
-    def __init__(self, hb, n_layers: int, seed_base: int, device):
+    The layers are independent (BASELINE.json configs[2]), so ``fold`` of them at a time are laid out along the head
+    axis ([Ttot, fold*H, d]) and go through ONE hypic_segment_encode and ONE hypic_compose call:
+    head l*H + h of a group is head h of its l-th layer, each layer with its own seeded k/v/g/beta."""
+
+    def __init__(self, hb, n_layers: int, seed_base: int, device, fold: int = 1):
         self.hb = hb
-        self.layers = [wl.cfg2_layer(seed_base + l, device=device) for l in range(n_layers)]
-        self.E = [torch.empty((N_SEG, H, D, D), dtype=torch.float32, device=device) for _ in range(n_layers)]
-        self.T = [torch.empty((N_SEG, H, D, D), dtype=torch.float32, device=device) for _ in range(n_layers)]
-        self.S = [torch.empty((1, H, D, D), dtype=torch.float32, device=device) for _ in range(n_layers)]
+        self.fold = fold = max(1, min(fold, n_layers))
+        self.groups, self.sizes = [], []
+        for l0 in range(0, n_layers, fold):
+            ls = [wl.cfg2_layer(seed_base + l, device=device) for l in range(l0, min(l0 + fold, n_layers))]
+            self.groups.append(wl.fold_layers(ls) if len(ls) > 1 else ls[0])
+            self.sizes.append(len(ls))
+            del ls
+        mk = lambda n, G: torch.empty((n, G * H, D, D), dtype=torch.float32, device=device)
+        self.E = [mk(N_SEG, G) for G in self.sizes]
+        self.T = [mk(N_SEG, G) for G in self.sizes]
+        self.S = [mk(1, G) for G in self.sizes]
         self.ids = torch.arange(N_SEG, dtype=torch.int32, device=device)
         self.cu = torch.tensor([0, N_SEG], dtype=torch.int32, device=device)
-        need = hb.hypic_segment_encode_workspace(N_SEG, N_SEG * SEG_LEN, H, D, D, hb.HYPIC_DT_BF16, hb.HYPIC_GATE_SCALAR)
+        need = hb.hypic_segment_encode_workspace(N_SEG, N_SEG * SEG_LEN, fold * H, D, D, hb.HYPIC_DT_BF16,
+                                                 hb.HYPIC_GATE_SCALAR)
         self.ws = torch.empty(max(need, 16), dtype=torch.uint8, device=device)
         self.launches = 0
 
-    def encode(self, l, inp=None):
-        x = inp if inp is not None else self.layers[l]
-        self.hb.hypic_segment_encode(x.k, x.v, x.g, x.beta, x.cu_seqlens, x.gate, E=self.E[l], T=self.T[l],
+    def encode(self, i, inp=None):
+        x = inp if inp is not None else self.groups[i]
+        self.hb.hypic_segment_encode(x.k, x.v, x.g, x.beta, x.cu_seqlens, x.gate, E=self.E[i], T=self.T[i],
                                      workspace=self.ws)
         self.launches += self.hb.hypic_last_launch_count()
 
-    def compose(self, l):
-        self.hb.hypic_compose(None, self.E[l], self.T[l], self.ids, self.cu, total_steps=N_SEG, S_out=self.S[l])
+    def compose(self, i):
+        self.hb.hypic_compose(None, self.E[i], self.T[i], self.ids, self.cu, total_steps=N_SEG, S_out=self.S[i])
         self.launches += self.hb.hypic_last_launch_count()
 
     def step(self, events=None):
-        for l in range(len(self.layers)):
+        for i in range(len(self.groups)):
             if events is not None:
-                events[l][0].record()
-            self.encode(l)
+                events[i][0].record()
+            self.encode(i)
             if events is not None:
-                events[l][1].record()
-            self.compose(l)
+                events[i][1].record()
+            self.compose(i)
             if events is not None:
-                events[l][2].record()
+                events[i][2].record()
 
 
 def time_extra_cfg1(hb, device, peaks, reps=20):
@@ -508,12 +520,14 @@ def run_ours(args):
     L = args.layers
 
     # weak scaling: every rank owns one full request with its own seeds (layer index offset by rank)
-    req = Cfg2Request(hb, L, seed_base=L * rank, device=device)
+    req = Cfg2Request(hb, L, seed_base=L * rank, device=device, fold=args.fold)
+    NG = len(req.groups)
+    req_fold = req.fold
     for _ in range(args.warmup):
         req.step()
     torch.cuda.synchronize()
 
-    events = [[[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(L)] for _ in range(args.steps)]
+    events = [[[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(NG)] for _ in range(args.steps)]
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
@@ -540,13 +554,16 @@ def run_ours(args):
     value = tokens_per_step / (ms_step * 1e-3)
 
     # per-kernel durations measured live inside the timed region (CUDA events on the launching stream)
-    enc_ms = [ev[0].elapsed_time(ev[1]) for st in events for ev in st]
-    cmp_ms = [ev[1].elapsed_time(ev[2]) for st in events for ev in st]
-    enc_avg, cmp_avg = sum(enc_ms) / len(enc_ms), sum(cmp_ms) / len(cmp_ms)
-    th_per_launch = N_SEG * SEG_LEN * H
+    # (per call of `fold` layers; the last group may be smaller, so durations are normalised to one layer first)
+    enc_ms = [ev[0].elapsed_time(ev[1]) / req.sizes[i] for st in events for i, ev in enumerate(st)]
+    cmp_ms = [ev[1].elapsed_time(ev[2]) / req.sizes[i] for st in events for i, ev in enumerate(st)]
+    G = req.fold
+    enc_layer, cmp_layer = sum(enc_ms) / len(enc_ms), sum(cmp_ms) / len(cmp_ms)
+    enc_avg, cmp_avg = enc_layer * G, cmp_layer * G  # one launch of a full group
+    th_per_launch = N_SEG * SEG_LEN * H * G
     enc_family = hb.hypic_encode_impl_for(H, D, D, hb.HYPIC_DT_BF16, hb.HYPIC_GATE_SCALAR)
     enc_tflops = th_per_launch * ENC_FLOP_PER_TOKEN_HEAD / (enc_avg * 1e-3) / 1e12
-    enc_gbs = (th_per_launch * ENC_BYTES_PER_TOKEN_HEAD + N_SEG * H * COMPOSE_BYTES_PER_STEP) / (enc_avg * 1e-3) / 1e9
+    enc_gbs = (th_per_launch * ENC_BYTES_PER_TOKEN_HEAD + N_SEG * H * G * COMPOSE_BYTES_PER_STEP) / (enc_avg * 1e-3) / 1e9
     if enc_family == hb.HYPIC_IMPL_TENSOR:
         roofline = {"bound": "tensor", "achieved": enc_tflops, "peak": peaks["bf16_tflops_sustained"],
                     "unit": "TFLOP/s", "frac": enc_tflops / peaks["bf16_tflops_sustained"], "traffic": None,
@@ -558,12 +575,14 @@ def run_ours(args):
     fam = "tensor" if enc_family == hb.HYPIC_IMPL_TENSOR else "simt"
     tpath = os.path.join(ROOT, "profiles", "traffic.json")  # dram bytes per launch from the committed ncu capture
     if os.path.exists(tpath):
-        roofline["traffic"] = json.load(open(tpath)).get(f"encode_{fam}_cfg2_layer_dram_bytes")
+        per_layer = json.load(open(tpath)).get(f"encode_{fam}_cfg2_layer_dram_bytes")
+        roofline["traffic"] = None if per_layer is None else per_layer * G  # captured per layer, scaled to the launch
     roofline.update({"kernel": ("hypic_segment_encode = chunk_offsets_kernel + prep_kernel + scan2_kernel (tensor "
                                 "family; prep and scan share the call about evenly, see profiles/)") if fam == "tensor" else
                      "hypic_segment_encode = encode_simt_kernel (simt family)",
                      "units_per_launch": f"{th_per_launch} token-heads x {ENC_FLOP_PER_TOKEN_HEAD} flop",
-                     "avg_launch_ms": enc_avg, "share_of_step": enc_avg * L / ms_step,
+                     "avg_launch_ms": enc_avg, "layers_per_launch": G, "ms_per_layer": enc_layer,
+                     "share_of_step": enc_layer * L / ms_step,
                      "frac_of_bf16_burst_peak": enc_tflops / peaks["bf16_tflops"], "hbm_gbs": enc_gbs,
                      "hbm_frac": enc_gbs / peaks["hbm_gbs"]})
 
@@ -574,23 +593,24 @@ def run_ours(args):
         return 0
 
     # ---- end to end: pinned host inputs -> H2D -> C-ABI calls -> D2H of the composed state, every step
-    Le = min(L, args.e2e_layers)
-    host = []
-    for l in range(Le):
-        x = req.layers[l]
-        host.append([t.cpu().pin_memory() for t in (x.k, x.v, x.g, x.beta)])
-    stage = req.layers[0]
-    s_host = torch.empty((1, H, D, D), dtype=torch.float32).pin_memory()
-    h2d = sum(t.numel() * t.element_size() for t in host[0])
+    # (one folded group of Le layers per step, through the same two calls as the device-resident run)
+    if req.sizes[0] > args.e2e_layers:
+        del req
+        torch.cuda.empty_cache()
+        req = Cfg2Request(hb, args.e2e_layers, seed_base=L * rank, device=device, fold=args.e2e_layers)
+    Le = req.sizes[0]
+    stage = req.groups[0]
+    host = [t.cpu().pin_memory() for t in (stage.k, stage.v, stage.g, stage.beta)]
+    s_host = torch.empty((1, Le * H, D, D), dtype=torch.float32).pin_memory()
+    h2d = sum(t.numel() * t.element_size() for t in host)
     d2h = s_host.numel() * 4
 
     def e2e_step():
-        for l in range(Le):
-            for dst, src in zip((stage.k, stage.v, stage.g, stage.beta), host[l]):
-                dst.copy_(src, non_blocking=True)
-            req.encode(0, stage)
-            req.compose(0)
-            s_host.copy_(req.S[0], non_blocking=True)
+        for dst, src in zip((stage.k, stage.v, stage.g, stage.beta), host):
+            dst.copy_(src, non_blocking=True)
+        req.encode(0, stage)
+        req.compose(0)
+        s_host.copy_(req.S[0], non_blocking=True)
         torch.cuda.synchronize()
 
     e2e_step()
@@ -600,10 +620,11 @@ def run_ours(args):
     for _ in range(n_e2e):
         e2e_step()
     e2e_s = (time.perf_counter() - w0) / n_e2e
-    e2e = {"value": Le * N_SEG * SEG_LEN / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d * Le,
-           "d2h_bytes_per_step": d2h * Le, "layers_per_step": Le,
-           "note": "pinned host k/v/g/beta -> device per layer, encode + compose via the C ABI, composed S -> host"}
-    del host
+    e2e = {"value": Le * N_SEG * SEG_LEN / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "layers_per_step": Le,
+           "note": "pinned host k/v/g/beta of one folded group of layers -> device, encode + compose via the C ABI, "
+                   "composed S -> host"}
+    del host, stage
 
     extra = {}
     if not args.no_extra:
@@ -619,8 +640,9 @@ def run_ours(args):
         extra["diag_family"] = time_extra_diag(hb, device, peaks)
         torch.cuda.empty_cache()
         extra["forward_encode"] = time_extra_forward(hb, device)
-        extra["cfg2_compose"] = {"avg_launch_ms": cmp_avg, "compose_ops_per_s": N_SEG * H / (cmp_avg * 1e-3),
-                                 "hbm_gbs": N_SEG * H * COMPOSE_BYTES_PER_STEP / (cmp_avg * 1e-3) / 1e9}
+        extra["cfg2_compose"] = {"avg_launch_ms": cmp_avg, "layers_per_launch": G,
+                                 "compose_ops_per_s": N_SEG * H * G / (cmp_avg * 1e-3),
+                                 "hbm_gbs": N_SEG * H * G * COMPOSE_BYTES_PER_STEP / (cmp_avg * 1e-3) / 1e9}
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -636,7 +658,9 @@ def run_ours(args):
         "config": {"workload": "cfg2 (BASELINE.json configs[2]): RAG-shaped request, encode all segments then compose "
                                "per layer", "layers": L, "segments": N_SEG, "seg_len": SEG_LEN, "H": H, "dk": D,
                    "dv": D, "kv_dtype": "bf16", "gate": "scalar", "requests_per_gpu": 1,
-                   "l2": "inputs larger than L2 (1.35 GB per layer, own buffers per layer); no flush needed",
+                   "layers_per_call": req_fold, "layout": f"[Ttot, {req_fold} layers x {H} heads, d] (layers folded "
+                   "into the head axis, SURVEY.md 8(b); each layer keeps its own seeded inputs)",
+                   "l2": "inputs larger than L2 (1.35 GB per layer, own buffers per layer group); no flush needed",
                    "token_heads_per_s": value * H},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
         "extra": extra,
@@ -656,6 +680,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layers", type=int, default=36, help="linear layers of the cfg2 request (36 = as written)")
     ap.add_argument("--e2e-layers", type=int, default=4, help="layers per end-to-end step (bounds pinned host memory)")
+    ap.add_argument("--fold", type=int, default=4,
+                    help="independent layers folded into the head axis per library call (1 = one call per layer)")
     ap.add_argument("--no-extra", action="store_true", help="skip the cfg1 / cfg4 side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -130,6 +130,20 @@ def cfg2_layer(layer: int, device: str = "cpu", seg_len: int = 4096, n_seg: int 
                               beta_kind="sigmoid", seed=seed_for(2, layer), device=device)
 
 
+def fold_layers(layers: List[EncodeInputs]) -> EncodeInputs:
+    """Independent layers with the same packing, folded into the head axis ("fold layers into the
+    head axis when the caller's layout is [Ttot, layers*H, d]"): head l*H + h of the result is head h of layers[l].
+    Pure layout: values are copied, none is recomputed.  One call then covers all the folded layers."""
+    first = layers[0]
+    for x in layers[1:]:
+        if x.seg_lens != first.seg_lens or x.gate != first.gate or x.k.dtype != first.k.dtype:
+            raise ValueError("fold_layers: layers must share segment lengths, gate kind and dtype")
+    cat = lambda ts: torch.cat(ts, dim=1).contiguous()
+    return EncodeInputs(k=cat([x.k for x in layers]), v=cat([x.v for x in layers]), g=cat([x.g for x in layers]),
+                        beta=cat([x.beta for x in layers]), cu_seqlens=first.cu_seqlens, gate=first.gate,
+                        seg_lens=list(first.seg_lens))
+
+
 def cfg3_seg_lens(n_seg: int = 64, lo: int = 512, hi: int = 16384) -> List[int]:
     gen = torch.Generator()
     gen.manual_seed(seed_for(3, 999))

@@ -245,6 +245,32 @@ def test_cfg2_one_layer_sampled_units():
     check_E(S[0, [0, 13, 31]][:, None], ref, TOL_F32, "S_out")
 
 
+def test_cfg2_folded_layers_launch_configuration():
+    """cfg2 in the launch configuration bench.py times: 4 independent layers folded into the head axis (H = 128,
+    SURVEY.md 8(b)), full size (20 x 4096).  The folded call must reproduce the per-layer calls bit for bit (units
+    are independent), sampled units are checked against the oracle, and so is the folded composition."""
+    layers = [wl.cfg2_layer(l, "cuda") for l in range(4)]
+    inp = wl.fold_layers(layers)
+    E, T = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
+    for l in (0, 3):
+        E1, T1 = gpu_encode(layers[l], hb.HYPIC_IMPL_AUTO)
+        assert torch.equal(E[:, 32 * l:32 * l + 32], E1) and torch.equal(T[:, 32 * l:32 * l + 32], T1)
+        del E1, T1
+    del layers
+    units = [(0, 0), (19, 127)] + _sample_units(20, 128, 4, 5)
+    E_ref, T_ref = oracle_encode_units(inp, units)
+    si, hi = torch.tensor([u[0] for u in units]), torch.tensor([u[1] for u in units])
+    check_E(E[si, hi][:, None], E_ref, TOL_BF16)
+    check_T(T[si, hi][:, None], T_ref, TOL_BF16)
+    assert torch.isfinite(E).all() and torch.isfinite(T).all()
+    ids = torch.arange(20, dtype=torch.int32, device="cuda")
+    cu = torch.tensor([0, 20], dtype=torch.int32, device="cuda")
+    S = gpu_compose(None, E, T, ids, cu, hb.HYPIC_IMPL_AUTO)
+    hs = [0, 45, 96, 127]
+    ref = oracle_compose_units(None, E, T, ids, cu, [(0, h) for h in hs])
+    check_E(S[0, hs][:, None], ref, TOL_F32, "S_out (folded)")
+
+
 def test_cfg3_varlen_channel_gate_sampled_units():
     """cfg3 (64 varlen segments, per-channel gate) at a reduced head count to bound memory; sampled units
     including the shortest and the longest segment."""

@@ -106,3 +106,20 @@ def test_three_rank_gloo_uneven_heads(tmp_path):
     world = 3
     mp.spawn(_worker, args=(world, _free_port(), str(tmp_path), 4), nprocs=world, join=True)
     assert all((tmp_path / f"ok{r}").exists() for r in range(world))
+
+
+def test_fold_layers_is_a_pure_relayout():
+    """fold_layers: head l*H + h of the folded inputs is head h of layer l, bit for bit; the oracle on a folded unit
+    equals the oracle on the layer's own unit (layers stay independent)."""
+    layers = [wl.make_encode_inputs([70, 33], 2, 16, 16, kv_dtype=torch.float32, seed=wl.seed_for(0, 40 + l))
+              for l in range(3)]
+    f = wl.fold_layers(layers)
+    assert f.H == 6 and f.seg_lens == [70, 33] and f.k.is_contiguous()
+    for l, x in enumerate(layers):
+        for name in ("k", "v", "g", "beta"):
+            assert torch.equal(getattr(f, name)[:, 2 * l:2 * l + 2], getattr(x, name))
+    Ef, Tf = oracle.segment_encode(f.k.numpy(), f.v.numpy(), f.g.numpy(), f.beta.numpy(), f.cu_seqlens.numpy())
+    E1, T1 = oracle.segment_encode(layers[1].k.numpy(), layers[1].v.numpy(), layers[1].g.numpy(), layers[1].beta.numpy(),
+                           layers[1].cu_seqlens.numpy())
+    assert np.array_equal(Ef[:, 2:4], E1) and np.array_equal(Tf[:, 2:4], T1)
+
