@@ -575,8 +575,11 @@ def run_ours(args):
     fam = "tensor" if enc_family == hb.HYPIC_IMPL_TENSOR else "simt"
     tpath = os.path.join(ROOT, "profiles", "traffic.json")  # dram bytes per launch from the committed ncu capture
     if os.path.exists(tpath):
-        per_layer = json.load(open(tpath)).get(f"encode_{fam}_cfg2_layer_dram_bytes")
-        roofline["traffic"] = None if per_layer is None else per_layer * G  # captured per layer, scaled to the launch
+        tj = json.load(open(tpath))
+        per_layer = tj.get(f"encode_{fam}_cfg2_layer_dram_bytes")
+        # a capture of this very launch shape if there is one, else the per-layer capture scaled to the launch
+        roofline["traffic"] = tj.get(f"encode_{fam}_cfg2_fold{G}_dram_bytes",
+                                     None if per_layer is None else per_layer * G)
     roofline.update({"kernel": ("hypic_segment_encode = chunk_offsets_kernel + prep_kernel + scan2_kernel (tensor "
                                 "family; prep and scan share the call about evenly, see profiles/)") if fam == "tensor" else
                      "hypic_segment_encode = encode_simt_kernel (simt family)",
