@@ -60,6 +60,8 @@ def _load():
         lib.hypic_oracle_diag_sequential.restype = i32
         lib.hypic_oracle_diag_compose.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp]
         lib.hypic_oracle_diag_compose.restype = i32
+        lib.hypic_oracle_rope_compose.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, vp]
+        lib.hypic_oracle_rope_compose.restype = i32
         lib.hypic_oracle_compose.argtypes = [vp, vp, vp, i32, vp, vp, i32, i32, i32, i32, i32, vp]
         lib.hypic_oracle_compose.restype = i32
         _lib = lib
@@ -227,6 +229,30 @@ def diag_compose(S_in, E_pool, t_pool, seg_ids, cu_segs):
                                            gate, _ptr(S_out))
     if rc != 0:
         raise ValueError(f"hypic_oracle_diag_compose failed with code {rc}")
+    return S_out
+
+
+def rope_compose(S_in, E_pool, t_pool, seg_ids, cu_segs, pos, inv_freq):
+    """Scalar family with RoPE inside the layer: S <- t_i S + E_i R(p_i)^T, every row of the zero-start end-state
+    re-rotated like a key to the segment's global start position p_i (Eq. 7).
+    t_pool:[P,H]; pos:int32[len(seg_ids)]; inv_freq:[dk/2] (pair = columns c, c + dk/2)."""
+    E_pool = np.ascontiguousarray(E_pool, dtype=np.float64)
+    t_pool = np.ascontiguousarray(t_pool, dtype=np.float64)
+    inv_freq = np.ascontiguousarray(inv_freq, dtype=np.float64)
+    P, H, dv, dk = E_pool.shape
+    assert t_pool.shape == (P, H) and dk % 2 == 0 and inv_freq.shape == (dk // 2,)
+    ids, cu, pos = _i32(seg_ids), _i32(cu_segs), _i32(pos)
+    R = cu.shape[0] - 1
+    assert cu[0] == 0 and cu[-1] == ids.shape[0] and np.all(np.diff(cu) >= 0) and pos.shape == ids.shape
+    assert ids.size == 0 or (ids.min() >= 0 and ids.max() < P)
+    if S_in is not None:
+        S_in = np.ascontiguousarray(S_in, dtype=np.float64)
+        assert S_in.shape == (R, H, dv, dk)
+    S_out = np.empty((R, H, dv, dk), dtype=np.float64)
+    rc = _load().hypic_oracle_rope_compose(_ptr(S_in), _ptr(E_pool), _ptr(t_pool), _ptr(ids), _ptr(cu), _ptr(pos),
+                                           _ptr(inv_freq), R, H, dk, dv, _ptr(S_out))
+    if rc != 0:
+        raise ValueError(f"hypic_oracle_rope_compose failed with code {rc}")
     return S_out
 
 

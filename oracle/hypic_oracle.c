@@ -26,7 +26,7 @@
  *       of PAPER.md:86-90 (Eq. 2) after each step:  paper o_i = q_i^T S_i;  here o_t = S_t q_t
  *
  * There is no chunking, blocking, fusion or reordering here: one token at a time, one row at a time.
- * All pins are in tests/test_oracle_pins.py (P1..P10, W1..W4 and D1..D5 of DESIGN.md); no function here is "parity unpinned".
+ * All pins are in tests/test_oracle_pins.py (P1..P10, W1..W4, D1..D5 and R1..R3 of DESIGN.md); no function here is "parity unpinned".
  *
  * Build: gcc -O3 -march=native -fopenmp -shared -fPIC hypic_oracle.c -o libhypic_oracle.so -lm
  */
@@ -292,6 +292,49 @@ int hypic_oracle_diag_compose(const double* S_in, const double* E_pool, const do
       for (int i = 0; i < dv; ++i)
         for (int c = 0; c < dk; ++c)
           Su[(size_t)i * dk + c] = Su[(size_t)i * dk + c] * ti[tw == 1 ? 0 : c] + Ei[(size_t)i * dk + c];
+    }
+  }
+  return 0;
+}
+
+/*
+ * hypic_oracle_rope_compose: state RoPE re-rotation, PAPER.md:208-214 (Eq. 7), scalar family only (T_i = t_i I commutes
+ * with every rotation): "Hypic replaces each S_{C_i|0} in Equation (6) with R(p_i) S_{C_i|0}", p_i = the segment's
+ * global start position.  Row convention (reading A1): the keys run along the columns of the dv x dk state,
+ * so R(p) acts on every ROW of E_i as it acts on a key.  Pairing and angles (reading R1): column c < dk/2 is
+ * paired with column c + dk/2, angle phi_c = p * inv_freq[c]:
+ *     E'[i][c]        = E[i][c] cos(phi_c) - E[i][c + dk/2] sin(phi_c)
+ *     E'[i][c + dk/2] = E[i][c] sin(phi_c) + E[i][c + dk/2] cos(phi_c)
+ * then  S <- t_i S + E'_i  over the request's ordered ids.  pos:int32[cu_segs[R]] (one start position per list entry),
+ * inv_freq:double[dk/2], E_pool:[P,H,dv,dk], t_pool:[P,H], doubles.  Pins: R1-R3 of tests/test_oracle_pins.py.
+ */
+int hypic_oracle_rope_compose(const double* S_in, const double* E_pool, const double* t_pool, const int32_t* seg_ids,
+                              const int32_t* cu_segs, const int32_t* pos, const double* inv_freq, int R, int H, int dk,
+                              int dv, double* S_out) {
+  if (R < 0 || H <= 0 || dk <= 0 || (dk & 1) || dv <= 0 || !cu_segs || !S_out || !inv_freq) return 1;
+  const int half = dk / 2;
+  const long n_units = (long)R * H;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (long u = 0; u < n_units; ++u) {
+    const int r = (int)(u / H), h = (int)(u % H);
+    double* Su = S_out + (size_t)u * dv * dk;
+    if (S_in)
+      memcpy(Su, S_in + (size_t)u * dv * dk, sizeof(double) * (size_t)dv * dk);
+    else
+      memset(Su, 0, sizeof(double) * (size_t)dv * dk);
+    for (int j = cu_segs[r]; j < cu_segs[r + 1]; ++j) {
+      const size_t ph = (size_t)seg_ids[j] * H + h;
+      const double* Ei = E_pool + ph * dv * dk;
+      const double ti = t_pool[ph];
+      for (int c = 0; c < half; ++c) {
+        const double phi = (double)pos[j] * inv_freq[c];
+        const double cs = cos(phi), sn = sin(phi);
+        for (int i = 0; i < dv; ++i) {
+          const double a = Ei[(size_t)i * dk + c], b = Ei[(size_t)i * dk + c + half];
+          Su[(size_t)i * dk + c] = Su[(size_t)i * dk + c] * ti + (a * cs - b * sn);
+          Su[(size_t)i * dk + c + half] = Su[(size_t)i * dk + c + half] * ti + (a * sn + b * cs);
+        }
+      }
     }
   }
   return 0;

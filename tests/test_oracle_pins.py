@@ -538,3 +538,85 @@ def test_D5_diag_family_is_the_dense_family_without_erasure():
     np.testing.assert_allclose(E_dense, E_diag, rtol=0, atol=1e-6)
     kk = k[:, 0].astype(np.float64)
     np.testing.assert_allclose(T_dense[0, 0], t[0, 0] * (np.eye(dk) - kk.T @ kk), rtol=0, atol=1e-6)
+
+
+# ------------------------------------------------------------------------------------------------ state RoPE re-rotation
+def _rope_matrix(p, inv_freq):
+    """R(p) as an explicit dense dk x dk matrix of 2 x 2 rotation blocks on the pairs (c, c + dk/2): a different code
+    path from the oracle's column loop.  k_rot = R(p) k."""
+    half = len(inv_freq)
+    Rm = np.zeros((2 * half, 2 * half))
+    for c in range(half):
+        phi = p * inv_freq[c]
+        Rm[c, c] = Rm[c + half, c + half] = np.cos(phi)
+        Rm[c, c + half] = -np.sin(phi)
+        Rm[c + half, c] = np.sin(phi)
+    return Rm
+
+
+def _rope_keys(k, start, inv_freq):
+    """Keys of one stretch of tokens with RoPE applied at positions start, start + 1, ... (float64 [L,H,dk])."""
+    out = np.empty(k.shape, dtype=np.float64)
+    for t in range(k.shape[0]):
+        out[t] = k[t].astype(np.float64) @ _rope_matrix(start + t, inv_freq).T
+    return out
+
+
+def test_R1_eq7_rerotation_of_a_cached_end_state():
+    """PAPER.md:212 Eq. 7: S_{C|b} = R(b - a) S_{C|a} for a scalar transition.  The end state of a segment whose keys
+    were rotated from start position b equals the re-rotation (oracle.rope_compose, one step, t = 1) of the end state
+    computed from start position a; the rotation preserves the Frobenius norm; p = 0 is the identity."""
+    rng = np.random.default_rng(7100)
+    L, H, dk, dv = 23, 2, 8, 5
+    inv_freq = 10000.0 ** (-np.arange(dk // 2) / (dk // 2))
+    k, v, g, _ = _rand_inputs(L, H, dk, dv, GATE_SCALAR, rng, g_lo=-0.2, normalise=False)
+    a, b = 3, 1000
+    E_a, t_a = oracle.diag_encode(_rope_keys(k, a, inv_freq).astype(np.float32), v, g, _cu([L]), GATE_SCALAR)
+    E_b, _ = oracle.diag_encode(_rope_keys(k, b, inv_freq).astype(np.float32), v, g, _cu([L]), GATE_SCALAR)
+    one = np.ones_like(t_a)
+    ids, cu = np.zeros(1, dtype=np.int32), _cu([1])
+    rot = oracle.rope_compose(None, E_a, one, ids, cu, np.array([b - a], dtype=np.int32), inv_freq)
+    assert oracle.rel_fro(rot[0], E_b[0]) < 5e-7  # keys pass through float32 on the way into diag_encode
+    assert oracle.rel_fro(rot[0], E_a[0]) > 1e-2  # and the rotation is not a no-op
+    np.testing.assert_allclose(np.linalg.norm(rot), np.linalg.norm(E_a), rtol=1e-13)
+    same = oracle.rope_compose(None, E_a, one, ids, cu, np.zeros(1, dtype=np.int32), inv_freq)
+    np.testing.assert_array_equal(same[0], E_a[0])
+    # dense-matrix form of the same statement: every row of E is rotated like a key
+    for h in range(H):
+        np.testing.assert_allclose(rot[0, h], E_a[0, h] @ _rope_matrix(b - a, inv_freq).T, rtol=1e-12, atol=1e-14)
+
+
+@pytest.mark.parametrize("zero_start", [True, False])
+def test_R2_rope_compose_equals_sequential_with_global_positions(zero_start):
+    """replacing each S_{C_i|0} by R(p_i) S_{C_i|0} in Eq. 6, p_i = the segment's global start position,
+    reproduces the recurrence over the spliced sequence whose keys carry RoPE at their global positions."""
+    rng = np.random.default_rng(7200)
+    lens = [17, 1, 40, 0, 9]
+    H, dk, dv = 2, 8, 5
+    inv_freq = 10000.0 ** (-np.arange(dk // 2) / (dk // 2))
+    k, v, g, _ = _rand_inputs(sum(lens), H, dk, dv, GATE_SCALAR, rng, g_lo=-0.2, normalise=False)
+    starts = np.concatenate([[0], np.cumsum(lens)[:-1]]).astype(np.int32)
+    k_local = np.concatenate([_rope_keys(k[s:s + n], 0, inv_freq) for s, n in zip(starts, lens)]).astype(np.float32)
+    k_global = _rope_keys(k, 0, inv_freq).astype(np.float32)
+    E, t = oracle.diag_encode(k_local, v, g, _cu(lens), GATE_SCALAR)  # position-independent tuples (cache time)
+    S0 = None if zero_start else rng.standard_normal((1, H, dv, dk))
+    ids = np.arange(len(lens), dtype=np.int32)
+    S = oracle.rope_compose(S0, E, t, ids, _cu([len(lens)]), starts, inv_freq)
+    S_seq = oracle.diag_sequential(S0, k_global, v, g, _cu([sum(lens)]), GATE_SCALAR)
+    assert oracle.rel_fro(S, S_seq) < 5e-7
+    S_norot = oracle.diag_compose(S0, E, t, ids, _cu([len(lens)]))
+    assert oracle.rel_fro(S_norot, S_seq) > 1e-2  # without the re-rotation the cached states do not splice
+
+
+def test_R3_rope_compose_at_position_zero_is_diag_compose():
+    """p_i = 0 for every entry: R(0) = I, so the routine reduces to the scalar family's plain composition."""
+    rng = np.random.default_rng(7300)
+    P, H, dk, dv = 6, 3, 16, 4
+    E = rng.standard_normal((P, H, dv, dk))
+    t = rng.uniform(0.5, 1.0, (P, H))
+    ids = np.array([4, 0, 5, 2, 2, 1], dtype=np.int32)
+    cu = np.array([0, 4, 4, 6], dtype=np.int32)
+    S0 = rng.standard_normal((3, H, dv, dk))
+    inv_freq = 10000.0 ** (-np.arange(dk // 2) / (dk // 2))
+    S = oracle.rope_compose(S0, E, t, ids, cu, np.zeros(6, dtype=np.int32), inv_freq)
+    np.testing.assert_allclose(S, oracle.diag_compose(S0, E, t, ids, cu), rtol=1e-15, atol=0)
