@@ -198,6 +198,28 @@ int hypic_diag_encode(const void* k, const void* v, const float* g, const int32_
 int hypic_diag_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,
                        const int32_t* cu_segs, int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk,
                        int32_t dv, int gate, float* S_out, void* stream);
+/*
+ * hypic_rope_compose: state RoPE re-rotation (Eq. 7: S_{C|b} = R(b - a) S_{C|a}) for models of the
+ * scalar family that apply RoPE to K inside the linear layer.  T_i = t_i I commutes with every rotation, so a zero-start
+ * end-state cached from position 0 is valid at any position after one rotation; at reuse time each S_{C_i|0} of Eq. 6 is
+ * replaced by R(p_i) S_{C_i|0}, p_i = the segment's global start position in the spliced sequence:
+ *     S <- t_i S + E_i R(p_i)^T      over each request's ordered id list
+ * Row convention (keys along the dk columns): every ROW of E_i is rotated like a key.  Pairing (reading R1):
+ * column c < dk/2 with column c + dk/2, angle p_i * inv_freq[c]:
+ *     E'[:, c] = E[:, c] cos - E[:, c + dk/2] sin,    E'[:, c + dk/2] = E[:, c] sin + E[:, c + dk/2] cos.
+ *   S_in, E_pool [P,H,dv,dk] fp32, seg_ids, cu_segs, S_out as in hypic_diag_compose; t_pool [P,H] fp32 (scalar family)
+ *   pos       int32 [total_steps]   start position of every list entry (same indexing as seg_ids), >= 0
+ *   inv_freq  fp32 [dk/2]           angular frequency of pair c in radians per position (e.g. base^(-2c/dk))
+ *   workspace device, >= hypic_rope_compose_workspace(total_steps, dk) bytes, 16-byte aligned; holds the cos/sin table
+ *             of this call (angles are formed and reduced in fp64: an fp32 product p * w is off by p * 2^-24 rad)
+ * Device-side contents (seg_ids, cu_segs, pos) are trusted.  S_out may alias S_in exactly.  Built envelope: dk in
+ * {8, 16, 32, 64, 128}, dv in [1, 1024], H, R <= 65535.  HYPIC_ERR_WORKSPACE when the workspace is missing or too small.
+ */
+size_t hypic_rope_compose_workspace(int32_t total_steps, int32_t dk);
+int hypic_rope_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,
+                       const int32_t* cu_segs, const int32_t* pos, const float* inv_freq, int32_t R, int32_t P,
+                       int32_t total_steps, int32_t H, int32_t dk, int32_t dv, float* S_out, void* workspace,
+                       size_t workspace_bytes, void* stream);
 /* hypic_diag_compose_f16: hypic_diag_compose over end-states stored in fp16 (hypic_tuple_pack_f16 of hypic_diag_encode's
  * E; the paper's cache precision): E_pool [P,H,dv,dk] fp16, taken as exact inputs; t_pool stays fp32
  * (4 B or 4 dk B per tuple: there is nothing to save, and a decay product rounded to fp16 would cost 5e-4 per step). */

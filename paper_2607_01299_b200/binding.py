@@ -30,7 +30,8 @@ EXPORTS = (
     "hypic_status_string", "hypic_version", "hypic_last_launch_count", "hypic_encode_impl_for",
     "hypic_compose_impl_for", "hypic_debug_timeout_count", "hypic_envelope_violation_count", "hypic_compose_f16",
     "hypic_tuple_pack_f16", "hypic_seam_window", "hypic_diag_encode", "hypic_diag_compose",
-    "hypic_diag_encode_impl_for", "hypic_diag_compose_f16", "hypic_forward_encode",
+    "hypic_diag_encode_impl_for", "hypic_diag_compose_f16", "hypic_forward_encode", "hypic_rope_compose_workspace",
+    "hypic_rope_compose",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -81,6 +82,10 @@ def load_library() -> ctypes.CDLL:
     lib.hypic_forward_encode.restype = ctypes.c_int
     lib.hypic_diag_compose_f16.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, ctypes.c_int, vp, vp]
     lib.hypic_diag_compose_f16.restype = ctypes.c_int
+    lib.hypic_rope_compose_workspace.argtypes = [i32, i32]
+    lib.hypic_rope_compose_workspace.restype = sz
+    lib.hypic_rope_compose.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp, vp, sz, vp]
+    lib.hypic_rope_compose.restype = ctypes.c_int
     lib.hypic_diag_encode_impl_for.argtypes = [i32, i32, i32, ctypes.c_int, ctypes.c_int]
     lib.hypic_diag_encode_impl_for.restype = ctypes.c_int
     lib.hypic_status_string.argtypes = [ctypes.c_int]
@@ -436,6 +441,59 @@ def hypic_diag_compose(S_in: Optional[torch.Tensor], E_pool: torch.Tensor, t_poo
             _dev_ptr(S_out, "S_out", torch.float32), _stream_handle(stream))
     if rc != HYPIC_OK:
         raise HypicError(rc, "hypic_diag_compose")
+    return S_out
+
+
+def hypic_rope_compose_workspace(total_steps: int, dk: int) -> int:
+    return int(load_library().hypic_rope_compose_workspace(int(total_steps), int(dk)))
+
+
+def hypic_rope_compose(S_in: Optional[torch.Tensor], E_pool: torch.Tensor, t_pool: torch.Tensor,
+                       seg_ids: torch.Tensor, cu_segs: torch.Tensor, pos: torch.Tensor, inv_freq: torch.Tensor, *,
+                       total_steps: Optional[int] = None, S_out: Optional[torch.Tensor] = None,
+                       workspace: Optional[torch.Tensor] = None,
+                       stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """Scalar family with RoPE inside the layer (Eq. 7): S <- t_i S + E_i R(pos_i)^T over
+    seg_ids[cu_segs[r]:cu_segs[r+1]] from S_in[r,h] (None = 0).  E_pool:[P,H,dv,dk] fp32, t_pool:[P,H] fp32,
+    pos:int32[len(seg_ids)], inv_freq:fp32[dk/2].  A workspace is allocated when none is given."""
+    lib = load_library()
+    for name, t in (("E_pool", E_pool), ("t_pool", t_pool), ("seg_ids", seg_ids), ("cu_segs", cu_segs), ("pos", pos),
+                    ("inv_freq", inv_freq)):
+        if not t.is_cuda:
+            raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if E_pool.dim() != 4:
+        raise ValueError("E_pool:[P,H,dv,dk]")
+    P, H, dv, dk = (int(x) for x in E_pool.shape)
+    if tuple(t_pool.shape) != (P, H):
+        raise ValueError("t_pool must be [P,H] (scalar family only: a diagonal T does not commute with rotations)")
+    if tuple(inv_freq.shape) != (dk // 2,):
+        raise ValueError("inv_freq must be [dk/2]")
+    if pos.numel() != seg_ids.numel():
+        raise ValueError("pos must have one entry per seg_ids entry")
+    R = int(cu_segs.numel()) - 1
+    if R < 0:
+        raise ValueError("cu_segs must have R+1 >= 1 entries")
+    if total_steps is None:
+        total_steps = int(seg_ids.numel())
+    if S_in is not None and tuple(S_in.shape) != (R, H, dv, dk):
+        raise ValueError("S_in must be [R,H,dv,dk]")
+    if S_out is None:
+        S_out = torch.empty((R, H, dv, dk), dtype=torch.float32, device=E_pool.device)
+    if tuple(S_out.shape) != (R, H, dv, dk):
+        raise ValueError("S_out must be [R,H,dv,dk]")
+    need = hypic_rope_compose_workspace(total_steps, dk)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=E_pool.device)
+    with torch.cuda.device(E_pool.device):
+        rc = lib.hypic_rope_compose(
+            _dev_ptr(S_in, "S_in", torch.float32), _dev_ptr(E_pool, "E_pool", torch.float32),
+            _dev_ptr(t_pool, "t_pool", torch.float32), _dev_ptr(seg_ids, "seg_ids", torch.int32),
+            _dev_ptr(cu_segs, "cu_segs", torch.int32), _dev_ptr(pos, "pos", torch.int32),
+            _dev_ptr(inv_freq, "inv_freq", torch.float32), R, P, int(total_steps), H, dk, dv,
+            _dev_ptr(S_out, "S_out", torch.float32), _dev_ptr(workspace, "workspace", torch.uint8),
+            int(workspace.numel()), _stream_handle(stream))
+    if rc != HYPIC_OK:
+        raise HypicError(rc, "hypic_rope_compose")
     return S_out
 
 

@@ -96,12 +96,28 @@ struct DiagComposeArgs {
   cudaStream_t stream;
 };
 
+struct RopeComposeArgs {
+  const float* S_in;
+  const float* E_pool;
+  const float* t_pool;
+  const int32_t* seg_ids;
+  const int32_t* cu_segs;
+  const int32_t* pos;
+  const float* inv_freq;
+  int32_t R, P, total_steps, H, dk, dv;
+  float* S_out;
+  void* workspace;
+  cudaStream_t stream;
+};
+
 // Kernel families (each returns a hypic_status_t; UNSUPPORTED when the shape is outside its envelope).
 int encode_simt(const EncodeArgs& a);
 int compose_simt(const ComposeArgs& a);
 int seam_simt(const SeamArgs& a);
 int diag_encode(const DiagEncodeArgs& a);
 int diag_compose(const DiagComposeArgs& a);
+size_t rope_compose_workspace(int32_t total_steps, int32_t dk);
+int rope_compose(const RopeComposeArgs& a);
 bool diag_encode_tensor_shape_ok(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate);
 int diag_encode_tensor(const DiagEncodeArgs& a);
 bool encode_tensor_shape_ok(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate);

@@ -220,6 +220,29 @@ int hypic_diag_compose_f16(const float* S_in, const void* E_pool, const float* t
   return diag_compose_call(S_in, E_pool, 1, t_pool, seg_ids, cu_segs, R, P, total_steps, H, dk, dv, gate, S_out, stream);
 }
 
+size_t hypic_rope_compose_workspace(int32_t total_steps, int32_t dk) {
+  if (total_steps <= 0 || dk <= 0) return 0;
+  return rope_compose_workspace(total_steps, dk);
+}
+
+int hypic_rope_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,
+                       const int32_t* cu_segs, const int32_t* pos, const float* inv_freq, int32_t R, int32_t P,
+                       int32_t total_steps, int32_t H, int32_t dk, int32_t dv, float* S_out, void* workspace,
+                       size_t workspace_bytes, void* stream) {
+  g_launch_count = 0;
+  if (R < 0 || P < 0 || total_steps < 0 || H <= 0 || dk <= 0 || dv <= 0) return HYPIC_ERR_INVALID_ARG;
+  if (!cu_segs) return HYPIC_ERR_INVALID_ARG;
+  if (R > 0 && !S_out) return HYPIC_ERR_INVALID_ARG;
+  if (total_steps > 0 && (!E_pool || !t_pool || !seg_ids || !pos || !inv_freq || P == 0)) return HYPIC_ERR_INVALID_ARG;
+  if (!aligned16(S_in) || !aligned16(E_pool) || !aligned16(S_out) || !aligned16(workspace)) return HYPIC_ERR_INVALID_ARG;
+  if (dk % 8 != 0) return HYPIC_ERR_UNSUPPORTED;
+  if (total_steps > 0 && (!workspace || workspace_bytes < rope_compose_workspace(total_steps, dk)))
+    return HYPIC_ERR_WORKSPACE;
+  RopeComposeArgs a{S_in, E_pool, t_pool, seg_ids, cu_segs, pos, inv_freq, R, P, total_steps, H, dk, dv, S_out,
+                    workspace, (cudaStream_t)stream};
+  return rope_compose(a);
+}
+
 int hypic_encode_impl_for(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate) {
   const int vs = validate_encode_shape(0, 0, H, dk, dv, kv_dtype, gate);
   if (vs != HYPIC_OK) return -vs;

@@ -748,6 +748,110 @@ def test_diag_compose_cfg4_lists_sampled_requests():
         check_E(Sh[r:r + 1, h:h + 1], refh, TOL_F32, "S_out (scalar family, fp16 end-states)")
 
 
+# ------------------------------------------------------------------------------------------------ state RoPE re-rotation
+def _inv_freq(dk, device="cuda"):
+    return (10000.0 ** (-torch.arange(dk // 2, dtype=torch.float64) / (dk // 2))).float().to(device)
+
+
+@pytest.mark.parametrize("dk,dv", [(128, 128), (64, 64), (128, 33), (8, 5), (32, 1024)])
+def test_rope_compose_vs_oracle(dk, dv):
+    """hypic_rope_compose (Eq. 7): lists of length 0, 1 and 40 with repeated, unsorted ids and start
+    positions up to 2^20 (an fp32 angle would be off by 6e-2 rad there); NULL and in-place S; p = 0 equals
+    hypic_diag_compose bit for bit up to the rotation's own rounding (cos = 1, sin = 0: exactly)."""
+    P, H = 24, 3
+    gen = torch.Generator().manual_seed(4100 + dk + dv)
+    E = torch.randn((P, H, dv, dk), generator=gen).cuda()
+    t_pool = (torch.rand((P, H), generator=gen) * 0.5 + 0.5).cuda()
+    ids = torch.randint(0, P, (41,), generator=gen, dtype=torch.int32).cuda()
+    pos = torch.randint(0, 1 << 20, (41,), generator=gen, dtype=torch.int32).cuda()
+    cu = torch.tensor([0, 0, 1, 41], dtype=torch.int32, device="cuda")
+    w = _inv_freq(dk)
+    S_in = torch.randn((3, H, dv, dk), generator=gen).cuda()
+    S = hb.hypic_rope_compose(S_in, E, t_pool, ids, cu, pos, w)
+    torch.cuda.synchronize()
+    assert hb.hypic_last_launch_count() == 2
+    args = (E.cpu().numpy(), t_pool.cpu().numpy(), ids.cpu().numpy(), cu.cpu().numpy(), pos.cpu().numpy(),
+            w.cpu().numpy())
+    ref = oracle.rope_compose(S_in.cpu().numpy(), *args)
+    check_E(S, ref, TOL_F32, "S_out (rope compose)")
+    assert torch.equal(S[0], S_in[0])  # empty list: S_in is copied
+    S0 = hb.hypic_rope_compose(None, E, t_pool, ids, cu, pos, w)
+    check_E(S0, oracle.rope_compose(None, *args), TOL_F32, "S_out (NULL S_in)")
+    S3 = S_in.clone()
+    hb.hypic_rope_compose(S3, E, t_pool, ids, cu, pos, w, S_out=S3)
+    assert torch.equal(S3, S)
+    Sz = hb.hypic_rope_compose(S_in, E, t_pool, ids, cu, torch.zeros_like(pos), w)
+    assert torch.equal(Sz, hb.hypic_diag_compose(S_in, E, t_pool, ids, cu))
+    # the rotation matters: without it the result is far from the reference
+    assert oracle.rel_fro(hb.hypic_diag_compose(S_in, E, t_pool, ids, cu)[2].cpu().numpy(), ref[2]) > 1e-2
+
+
+def test_rope_compose_end_to_end_equals_spliced_sequence():
+    """Cache time: hypic_diag_encode of segments whose keys carry RoPE from position 0.  Reuse time: hypic_rope_compose
+    with the global start positions.  Must equal the oracle's token recurrence over the spliced sequence whose keys carry
+    RoPE at their global positions; bf16 k/v, so the bf16 tolerance."""
+    H, d = 2, 128
+    lens = [300, 64, 1000, 17, 555]
+    gen = torch.Generator().manual_seed(4200)
+    Ttot = sum(lens)
+    k = torch.nn.functional.normalize(torch.randn((Ttot, H, d), generator=gen, dtype=torch.float64), dim=-1)
+    v = torch.randn((Ttot, H, d), generator=gen).to(torch.bfloat16)
+    g = -0.05 * torch.rand((Ttot, H), generator=gen)
+    w = _inv_freq(d, "cpu")
+    starts = np.concatenate([[0], np.cumsum(lens)[:-1]])
+
+    def rope(kk, p0):  # keys at positions p0, p0 + 1, ...: pairs (c, c + d/2), angles in fp64
+        ang = (torch.arange(kk.shape[0], dtype=torch.float64) + p0)[:, None] * w.double()[None, :]
+        co, si = ang.cos()[:, None, :], ang.sin()[:, None, :]
+        a, b = kk[..., :d // 2], kk[..., d // 2:]
+        return torch.cat([a * co - b * si, a * si + b * co], dim=-1)
+
+    k_local = torch.cat([rope(k[s:s + n], 0) for s, n in zip(starts, lens)]).to(torch.bfloat16)
+    cu_tok = torch.tensor(np.concatenate([[0], np.cumsum(lens)]), dtype=torch.int32)
+    E, tv = hb.hypic_diag_encode(k_local.cuda(), v.cuda(), g.cuda(), cu_tok.cuda(), wl.GATE_SCALAR)
+    ids = torch.arange(len(lens), dtype=torch.int32, device="cuda")
+    cu = torch.tensor([0, len(lens)], dtype=torch.int32, device="cuda")
+    S_in = torch.randn((1, H, d, d), generator=gen).cuda()
+    S = hb.hypic_rope_compose(S_in, E, tv, ids, cu, torch.tensor(starts, dtype=torch.int32).cuda(), w.cuda())
+    # reference: the global keys are the rotation of the SAME bf16-rounded local keys (rotation and rounding do not
+    # commute, and the cached tuples were built from the rounded ones)
+    k_ref = torch.cat([_rerotate(k_local[s:s + n].double(), int(s), w) for s, n in zip(starts, lens)])
+    seq = oracle.diag_sequential(S_in.cpu().numpy(), k_ref.float().numpy(), v.float().numpy(), g.numpy(),
+                                 np.array([0, Ttot], dtype=np.int32), wl.GATE_SCALAR)
+    check_E(S, seq, TOL_BF16, "rope compose vs spliced sequence")
+
+
+def _rerotate(k_rot0, shift, w):
+    """Keys already rotated from position 0, moved to start position `shift` (R(a + t) = R(a) R(t)), fp64."""
+    d = k_rot0.shape[-1]
+    ang = shift * w.double()
+    co, si = ang.cos()[None, None, :], ang.sin()[None, None, :]
+    a, b = k_rot0[..., :d // 2], k_rot0[..., d // 2:]
+    return torch.cat([a * co - b * si, a * si + b * co], dim=-1)
+
+
+def test_rope_compose_cfg4_lists_sampled_requests():
+    """cfg4's request lists over a pool of 1,024 end-states (one scalar each) with start positions up to 131,072: sampled
+    (request, head) chains against the oracle."""
+    E = wl.cfg4_pool_E(device="cuda")
+    gen = torch.Generator(device="cuda").manual_seed(wl.seed_for(6, 7))
+    t_pool = torch.rand((E.shape[0], 32), device="cuda", generator=gen) * 0.5 + 0.5
+    req = wl.cfg4_requests(device="cuda")
+    pos = torch.randint(0, 131072, (req.n_steps,), device="cuda", generator=gen, dtype=torch.int32)
+    w = _inv_freq(128)
+    S = hb.hypic_rope_compose(req.S_in, E, t_pool, req.seg_ids, req.cu_segs, pos, w)
+    torch.cuda.synchronize()
+    assert torch.isfinite(S).all()
+    ids_all, cu, pos_all = req.seg_ids.cpu().numpy(), req.cu_segs.cpu().numpy(), pos.cpu().numpy()
+    for r, h in _sample_units(128, 32, 6, 17):
+        ids = torch.as_tensor(ids_all[cu[r]:cu[r + 1]], dtype=torch.long, device="cuda")
+        n = len(ids)
+        ref = oracle.rope_compose(req.S_in[r:r + 1, h:h + 1].cpu().numpy(), E[ids, h:h + 1].cpu().numpy(),
+                                  t_pool[ids, h:h + 1].cpu().numpy(), np.arange(n, dtype=np.int32),
+                                  np.array([0, n], dtype=np.int32), pos_all[cu[r]:cu[r + 1]], w.cpu().numpy())
+        check_E(S[r:r + 1, h:h + 1], ref, TOL_F32, "S_out (rope compose, cfg4 lists)")
+
+
 # ------------------------------------------------------------------------------------------------ forward + encode in one pass
 @pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
 @pytest.mark.parametrize("kv,d,dv", [(torch.float32, 128, 128), (torch.bfloat16, 128, 128), (torch.float32, 64, 64),
