@@ -469,6 +469,22 @@ def time_extra_diag(hb, device, peaks, iters=16):
     ms = e0.elapsed_time(e1)
     head_steps = sum(r.n_steps for r in reqs) * H
     gbs = (head_steps * (D * D * 4 + 4) + iters * 128 * H * 2 * D * D * 4) / (ms * 1e-3) / 1e9
+    # state RoPE re-rotation: the same lists, every entry with a start position < 131,072
+    inv_freq = (10000.0 ** (-torch.arange(D // 2, dtype=torch.float64) / (D // 2))).float().to(device)
+    poss = [torch.randint(0, 131072, (r.n_steps,), device=device, dtype=torch.int32) for r in reqs]
+    ws_r = torch.empty(max(hb.hypic_rope_compose_workspace(max(r.n_steps for r in reqs), D), 16), dtype=torch.uint8,
+                       device=device)
+    for i in range(3):
+        hb.hypic_rope_compose(reqs[i].S_in, E_pool, t_pool, reqs[i].seg_ids, reqs[i].cu_segs, poss[i], inv_freq,
+                              S_out=S_out, workspace=ws_r)
+    torch.cuda.synchronize()
+    e0.record()
+    for rq, ps in zip(reqs, poss):
+        hb.hypic_rope_compose(rq.S_in, E_pool, t_pool, rq.seg_ids, rq.cu_segs, ps, inv_freq, S_out=S_out, workspace=ws_r)
+    e1.record()
+    torch.cuda.synchronize()
+    ms_rope = e0.elapsed_time(e1)
+    gbs_rope = (head_steps * (D * D * 4 + 4) + iters * 128 * H * 2 * D * D * 4) / (ms_rope * 1e-3) / 1e9
     Eh = hb.hypic_tuple_pack_f16(E_pool)
     del E_pool
     for i in range(3):
@@ -497,6 +513,11 @@ def time_extra_diag(hb, device, peaks, iters=16):
                                 "roofline": {"bound": "hbm", "achieved": ch_gbs, "peak": peaks["hbm_gbs"],
                                              "unit": "GB/s", "frac": ch_gbs / peaks["hbm_gbs"], "traffic": None,
                                              "peak_source": peaks["source"]}},
+            "rope_compose": {"ms_total": ms_rope, "compose_ops_per_s": head_steps / (ms_rope * 1e-3),
+                             "note": "hypic_rope_compose: cos/sin table kernel + fold, per call",
+                             "roofline": {"bound": "hbm", "achieved": gbs_rope, "peak": peaks["hbm_gbs"],
+                                          "unit": "GB/s", "frac": gbs_rope / peaks["hbm_gbs"], "traffic": None,
+                                          "peak_source": peaks["source"]}},
             "compose": {"ms_total": ms, "compose_ops_per_s": head_steps / (ms * 1e-3),
                         "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                      "frac": gbs / peaks["hbm_gbs"], "traffic": None,
