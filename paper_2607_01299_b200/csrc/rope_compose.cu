@@ -34,7 +34,7 @@ __global__ void rope_table_kernel(const int32_t* __restrict__ pos, const float* 
   table[(size_t)j * 2 * half + half + c] = (float)s;
 }
 
-__global__ void __launch_bounds__(kRcThreads)
+__global__ void __launch_bounds__(kRcThreads, 3)  // 3 CTAs per SM like diag_compose_kernel: bytes in flight set the rate
     rope_compose_kernel(const float* __restrict__ S_in, const float* __restrict__ E_pool,
                         const float* __restrict__ t_pool, const int32_t* __restrict__ seg_ids,
                         const int32_t* __restrict__ cu_segs, const float* __restrict__ table, int H, int dk, int unit_v4,
