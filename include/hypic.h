@@ -220,6 +220,13 @@ int hypic_rope_compose(const float* S_in, const float* E_pool, const float* t_po
                        const int32_t* cu_segs, const int32_t* pos, const float* inv_freq, int32_t R, int32_t P,
                        int32_t total_steps, int32_t H, int32_t dk, int32_t dv, float* S_out, void* workspace,
                        size_t workspace_bytes, void* stream);
+/* hypic_rope_compose_f16: the same over end-states stored in fp16 (hypic_tuple_pack_f16 of hypic_diag_encode's E; the
+ * paper's cache precision): E_pool [P,H,dv,dk] fp16, taken as exact inputs and widened to fp32 before
+ * the rotation; everything else as hypic_rope_compose. */
+int hypic_rope_compose_f16(const float* S_in, const void* E_pool, const float* t_pool, const int32_t* seg_ids,
+                           const int32_t* cu_segs, const int32_t* pos, const float* inv_freq, int32_t R, int32_t P,
+                           int32_t total_steps, int32_t H, int32_t dk, int32_t dv, float* S_out, void* workspace,
+                           size_t workspace_bytes, void* stream);
 /* hypic_diag_compose_f16: hypic_diag_compose over end-states stored in fp16 (hypic_tuple_pack_f16 of hypic_diag_encode's
  * E; the paper's cache precision): E_pool [P,H,dv,dk] fp16, taken as exact inputs; t_pool stays fp32
  * (4 B or 4 dk B per tuple: there is nothing to save, and a decay product rounded to fp16 would cost 5e-4 per step). */

@@ -31,7 +31,7 @@ EXPORTS = (
     "hypic_compose_impl_for", "hypic_debug_timeout_count", "hypic_envelope_violation_count", "hypic_compose_f16",
     "hypic_tuple_pack_f16", "hypic_seam_window", "hypic_diag_encode", "hypic_diag_compose",
     "hypic_diag_encode_impl_for", "hypic_diag_compose_f16", "hypic_forward_encode", "hypic_rope_compose_workspace",
-    "hypic_rope_compose",
+    "hypic_rope_compose", "hypic_rope_compose_f16",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -86,6 +86,8 @@ def load_library() -> ctypes.CDLL:
     lib.hypic_rope_compose_workspace.restype = sz
     lib.hypic_rope_compose.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp, vp, sz, vp]
     lib.hypic_rope_compose.restype = ctypes.c_int
+    lib.hypic_rope_compose_f16.argtypes = list(lib.hypic_rope_compose.argtypes)
+    lib.hypic_rope_compose_f16.restype = ctypes.c_int
     lib.hypic_diag_encode_impl_for.argtypes = [i32, i32, i32, ctypes.c_int, ctypes.c_int]
     lib.hypic_diag_encode_impl_for.restype = ctypes.c_int
     lib.hypic_status_string.argtypes = [ctypes.c_int]
@@ -454,7 +456,8 @@ def hypic_rope_compose(S_in: Optional[torch.Tensor], E_pool: torch.Tensor, t_poo
                        workspace: Optional[torch.Tensor] = None,
                        stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
     """Scalar family with RoPE inside the layer (Eq. 7): S <- t_i S + E_i R(pos_i)^T over
-    seg_ids[cu_segs[r]:cu_segs[r+1]] from S_in[r,h] (None = 0).  E_pool:[P,H,dv,dk] fp32, t_pool:[P,H] fp32,
+    seg_ids[cu_segs[r]:cu_segs[r+1]] from S_in[r,h] (None = 0).  E_pool:[P,H,dv,dk] fp32 (or fp16:
+    hypic_rope_compose_f16), t_pool:[P,H] fp32,
     pos:int32[len(seg_ids)], inv_freq:fp32[dk/2].  A workspace is allocated when none is given."""
     lib = load_library()
     for name, t in (("E_pool", E_pool), ("t_pool", t_pool), ("seg_ids", seg_ids), ("cu_segs", cu_segs), ("pos", pos),
@@ -484,9 +487,11 @@ def hypic_rope_compose(S_in: Optional[torch.Tensor], E_pool: torch.Tensor, t_poo
     need = hypic_rope_compose_workspace(total_steps, dk)
     if workspace is None:
         workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=E_pool.device)
+    f16 = E_pool.dtype == torch.float16
+    fn = lib.hypic_rope_compose_f16 if f16 else lib.hypic_rope_compose
     with torch.cuda.device(E_pool.device):
-        rc = lib.hypic_rope_compose(
-            _dev_ptr(S_in, "S_in", torch.float32), _dev_ptr(E_pool, "E_pool", torch.float32),
+        rc = fn(
+            _dev_ptr(S_in, "S_in", torch.float32), _dev_ptr(E_pool, "E_pool", torch.float16 if f16 else torch.float32),
             _dev_ptr(t_pool, "t_pool", torch.float32), _dev_ptr(seg_ids, "seg_ids", torch.int32),
             _dev_ptr(cu_segs, "cu_segs", torch.int32), _dev_ptr(pos, "pos", torch.int32),
             _dev_ptr(inv_freq, "inv_freq", torch.float32), R, P, int(total_steps), H, dk, dv,

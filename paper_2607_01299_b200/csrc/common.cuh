@@ -98,7 +98,7 @@ struct DiagComposeArgs {
 
 struct RopeComposeArgs {
   const float* S_in;
-  const float* E_pool;
+  const void* E_pool;  // fp32, or fp16 when e_f16
   const float* t_pool;
   const int32_t* seg_ids;
   const int32_t* cu_segs;
@@ -107,6 +107,7 @@ struct RopeComposeArgs {
   int32_t R, P, total_steps, H, dk, dv;
   float* S_out;
   void* workspace;
+  int e_f16;
   cudaStream_t stream;
 };
 

@@ -225,10 +225,10 @@ size_t hypic_rope_compose_workspace(int32_t total_steps, int32_t dk) {
   return rope_compose_workspace(total_steps, dk);
 }
 
-int hypic_rope_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,
-                       const int32_t* cu_segs, const int32_t* pos, const float* inv_freq, int32_t R, int32_t P,
-                       int32_t total_steps, int32_t H, int32_t dk, int32_t dv, float* S_out, void* workspace,
-                       size_t workspace_bytes, void* stream) {
+static int rope_compose_call(const float* S_in, const void* E_pool, int e_f16, const float* t_pool,
+                             const int32_t* seg_ids, const int32_t* cu_segs, const int32_t* pos, const float* inv_freq,
+                             int32_t R, int32_t P, int32_t total_steps, int32_t H, int32_t dk, int32_t dv, float* S_out,
+                             void* workspace, size_t workspace_bytes, void* stream) {
   g_launch_count = 0;
   if (R < 0 || P < 0 || total_steps < 0 || H <= 0 || dk <= 0 || dv <= 0) return HYPIC_ERR_INVALID_ARG;
   if (!cu_segs) return HYPIC_ERR_INVALID_ARG;
@@ -239,8 +239,24 @@ int hypic_rope_compose(const float* S_in, const float* E_pool, const float* t_po
   if (total_steps > 0 && (!workspace || workspace_bytes < rope_compose_workspace(total_steps, dk)))
     return HYPIC_ERR_WORKSPACE;
   RopeComposeArgs a{S_in, E_pool, t_pool, seg_ids, cu_segs, pos, inv_freq, R, P, total_steps, H, dk, dv, S_out,
-                    workspace, (cudaStream_t)stream};
+                    workspace, e_f16, (cudaStream_t)stream};
   return rope_compose(a);
+}
+
+int hypic_rope_compose(const float* S_in, const float* E_pool, const float* t_pool, const int32_t* seg_ids,
+                       const int32_t* cu_segs, const int32_t* pos, const float* inv_freq, int32_t R, int32_t P,
+                       int32_t total_steps, int32_t H, int32_t dk, int32_t dv, float* S_out, void* workspace,
+                       size_t workspace_bytes, void* stream) {
+  return rope_compose_call(S_in, E_pool, 0, t_pool, seg_ids, cu_segs, pos, inv_freq, R, P, total_steps, H, dk, dv, S_out,
+                           workspace, workspace_bytes, stream);
+}
+
+int hypic_rope_compose_f16(const float* S_in, const void* E_pool, const float* t_pool, const int32_t* seg_ids,
+                           const int32_t* cu_segs, const int32_t* pos, const float* inv_freq, int32_t R, int32_t P,
+                           int32_t total_steps, int32_t H, int32_t dk, int32_t dv, float* S_out, void* workspace,
+                           size_t workspace_bytes, void* stream) {
+  return rope_compose_call(S_in, E_pool, 1, t_pool, seg_ids, cu_segs, pos, inv_freq, R, P, total_steps, H, dk, dv, S_out,
+                           workspace, workspace_bytes, stream);
 }
 
 int hypic_encode_impl_for(int32_t H, int32_t dk, int32_t dv, int kv_dtype, int gate) {

@@ -14,6 +14,8 @@
 //                        of S for the whole chain; the partner column c +- dk/2 of the same row sits dk/8 lanes away in
 //                        the same warp, so the pair is completed with one shuffle per float; E is streamed once
 //                        (HBM-bound: 4 dv dk bytes per head-step).
+#include <cuda_fp16.h>
+
 #include "common.cuh"
 
 namespace hypic {
@@ -34,8 +36,9 @@ __global__ void rope_table_kernel(const int32_t* __restrict__ pos, const float* 
   table[(size_t)j * 2 * half + half + c] = (float)s;
 }
 
+template <bool F16>  // F16: end-states stored in fp16 (the paper's cache precision), exact inputs
 __global__ void __launch_bounds__(kRcThreads, 3)  // 3 CTAs per SM like diag_compose_kernel: bytes in flight set the rate
-    rope_compose_kernel(const float* __restrict__ S_in, const float* __restrict__ E_pool,
+    rope_compose_kernel(const float* __restrict__ S_in, const void* __restrict__ E_pool,
                         const float* __restrict__ t_pool, const int32_t* __restrict__ seg_ids,
                         const int32_t* __restrict__ cu_segs, const float* __restrict__ table, int H, int dk, int unit_v4,
                         float* __restrict__ S_out) {
@@ -69,7 +72,16 @@ __global__ void __launch_bounds__(kRcThreads, 3)  // 3 CTAs per SM like diag_com
 #pragma unroll
     for (int i = 0; i < kRcV4; ++i) {
       e_nxt[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (live[i]) e_nxt[i] = __ldcs(reinterpret_cast<const float4*>(E_pool) + ph * unit_v4 + e4[i]);
+      if (live[i]) {
+        if (F16) {
+          const uint2 hv = __ldcs(reinterpret_cast<const uint2*>(E_pool) + ph * unit_v4 + e4[i]);
+          const float2 lo = __half22float2(*reinterpret_cast<const __half2*>(&hv.x));
+          const float2 hi = __half22float2(*reinterpret_cast<const __half2*>(&hv.y));
+          e_nxt[i] = make_float4(lo.x, lo.y, hi.x, hi.y);
+        } else {
+          e_nxt[i] = __ldcs(reinterpret_cast<const float4*>(E_pool) + ph * unit_v4 + e4[i]);
+        }
+      }
     }
     t_nxt = __ldg(t_pool + ph);
     cs_nxt = __ldg(reinterpret_cast<const float4*>(table + (size_t)j * dk + cpair));
@@ -126,7 +138,8 @@ int rope_compose(const RopeComposeArgs& a) {
   }
   const int unit_v4 = a.dv * a.dk / 4;
   dim3 grid((unit_v4 + kRcThreads * kRcV4 - 1) / (kRcThreads * kRcV4), a.H, a.R);
-  rope_compose_kernel<<<grid, kRcThreads, 0, a.stream>>>(a.S_in, a.E_pool, a.t_pool, a.seg_ids, a.cu_segs, table, a.H,
+  auto kern = a.e_f16 ? rope_compose_kernel<true> : rope_compose_kernel<false>;
+  kern<<<grid, kRcThreads, 0, a.stream>>>(a.S_in, a.E_pool, a.t_pool, a.seg_ids, a.cu_segs, table, a.H,
                                                          a.dk, unit_v4, a.S_out);
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());

@@ -100,15 +100,16 @@ def test_argument_validation_needs_no_gpu(lib):
         assert dcomp(None, fake, None, fake, fake, 1, 4, 2, 1, 64, 64, 0, fake, None) == b.HYPIC_ERR_INVALID_ARG
         assert dcomp(None, fake, fake, fake, fake, 1, 4, 2, 1, 64, 64, 9, fake, None) == b.HYPIC_ERR_INVALID_ARG
         assert dcomp(None, fake, fake, fake, fake, 1, 4, 2, 1, 66, 64, 0, fake, None) == b.HYPIC_ERR_UNSUPPORTED
-    rc_ = lib.hypic_rope_compose
     assert lib.hypic_rope_compose_workspace(10, 128) == 10 * 128 * 4 and lib.hypic_rope_compose_workspace(0, 128) == 0
-    assert rc_(None, fake, fake, fake, None, fake, fake, 1, 4, 2, 1, 64, 64, fake, fake, 1 << 20, None) == b.HYPIC_ERR_INVALID_ARG
-    assert rc_(None, fake, fake, fake, fake, None, fake, 1, 4, 2, 1, 64, 64, fake, fake, 1 << 20, None) == b.HYPIC_ERR_INVALID_ARG
-    assert rc_(None, fake, fake, fake, fake, fake, None, 1, 4, 2, 1, 64, 64, fake, fake, 1 << 20, None) == b.HYPIC_ERR_INVALID_ARG
-    assert rc_(None, fake, fake, fake, fake, fake, fake, 1, 4, 2, 1, 12, 64, fake, fake, 1 << 20, None) == b.HYPIC_ERR_UNSUPPORTED
-    assert rc_(None, fake, fake, fake, fake, fake, fake, 1, 4, 2, 1, 24, 64, fake, fake, 1 << 20, None) == b.HYPIC_ERR_UNSUPPORTED
-    assert rc_(None, fake, fake, fake, fake, fake, fake, 1, 4, 2, 1, 64, 64, fake, fake, 2 * 64 * 4 - 1, None) == b.HYPIC_ERR_WORKSPACE
-    assert rc_(None, fake, fake, fake, fake, fake, fake, 1, 4, 2, 1, 64, 64, fake, None, 0, None) == b.HYPIC_ERR_WORKSPACE
+    for rc_ in (lib.hypic_rope_compose, lib.hypic_rope_compose_f16):
+        big = 1 << 20
+        assert rc_(None, fake, fake, fake, None, fake, fake, 1, 4, 2, 1, 64, 64, fake, fake, big, None) == b.HYPIC_ERR_INVALID_ARG
+        assert rc_(None, fake, fake, fake, fake, None, fake, 1, 4, 2, 1, 64, 64, fake, fake, big, None) == b.HYPIC_ERR_INVALID_ARG
+        assert rc_(None, fake, fake, fake, fake, fake, None, 1, 4, 2, 1, 64, 64, fake, fake, big, None) == b.HYPIC_ERR_INVALID_ARG
+        assert rc_(None, fake, fake, fake, fake, fake, fake, 1, 4, 2, 1, 12, 64, fake, fake, big, None) == b.HYPIC_ERR_UNSUPPORTED
+        assert rc_(None, fake, fake, fake, fake, fake, fake, 1, 4, 2, 1, 24, 64, fake, fake, big, None) == b.HYPIC_ERR_UNSUPPORTED
+        assert rc_(None, fake, fake, fake, fake, fake, fake, 1, 4, 2, 1, 64, 64, fake, fake, 2 * 64 * 4 - 1, None) == b.HYPIC_ERR_WORKSPACE
+        assert rc_(None, fake, fake, fake, fake, fake, fake, 1, 4, 2, 1, 64, 64, fake, None, 0, None) == b.HYPIC_ERR_WORKSPACE
     cf16 = lib.hypic_compose_f16
     assert cf16(None, fake, fake, fake, None, 1, 4, 2, 1, 128, 128, fake, None) == b.HYPIC_ERR_INVALID_ARG
     assert cf16(None, fake, fake, fake, fake, 1, 4, 2, 1, 64, 64, fake, None) == b.HYPIC_ERR_UNSUPPORTED

@@ -782,6 +782,11 @@ def test_rope_compose_vs_oracle(dk, dv):
     assert torch.equal(S3, S)
     Sz = hb.hypic_rope_compose(S_in, E, t_pool, ids, cu, torch.zeros_like(pos), w)
     assert torch.equal(Sz, hb.hypic_diag_compose(S_in, E, t_pool, ids, cu))
+    # fp16-stored end-states are exact inputs: the fold of the stored values, to the fp32-input tolerance
+    Eh = hb.hypic_tuple_pack_f16(E)
+    Sh = hb.hypic_rope_compose(S_in, Eh, t_pool, ids, cu, pos, w)
+    refh = oracle.rope_compose(S_in.cpu().numpy(), Eh.float().cpu().numpy(), *args[1:])
+    check_E(Sh, refh, TOL_F32, "S_out (rope compose, fp16 end-states)")
     # the rotation matters: without it the result is far from the reference
     assert oracle.rel_fro(hb.hypic_diag_compose(S_in, E, t_pool, ids, cu)[2].cpu().numpy(), ref[2]) > 1e-2
 
