@@ -469,6 +469,19 @@ def time_extra_diag(hb, device, peaks, iters=16):
     ms = e0.elapsed_time(e1)
     head_steps = sum(r.n_steps for r in reqs) * H
     gbs = (head_steps * (D * D * 4 + 4) + iters * 128 * H * 2 * D * D * 4) / (ms * 1e-3) / 1e9
+    # diagonal family (GLA): the same lists with a dk-vector of decays per tuple
+    t_pool_ch = torch.rand((E_pool.shape[0], H, D), device=device) * 0.5 + 0.5
+    for i in range(3):
+        hb.hypic_diag_compose(reqs[i].S_in, E_pool, t_pool_ch, reqs[i].seg_ids, reqs[i].cu_segs, S_out=S_out)
+    torch.cuda.synchronize()
+    e0.record()
+    for rq in reqs:
+        hb.hypic_diag_compose(rq.S_in, E_pool, t_pool_ch, rq.seg_ids, rq.cu_segs, S_out=S_out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms_dch = e0.elapsed_time(e1)
+    gbs_dch = (head_steps * (D * D * 4 + 4 * D) + iters * 128 * H * 2 * D * D * 4) / (ms_dch * 1e-3) / 1e9
+    del t_pool_ch
     # state RoPE re-rotation: the same lists, every entry with a start position < 131,072
     inv_freq = (10000.0 ** (-torch.arange(D // 2, dtype=torch.float64) / (D // 2))).float().to(device)
     poss = [torch.randint(0, 131072, (r.n_steps,), device=device, dtype=torch.int32) for r in reqs]
@@ -513,6 +526,10 @@ def time_extra_diag(hb, device, peaks, iters=16):
                                 "roofline": {"bound": "hbm", "achieved": ch_gbs, "peak": peaks["hbm_gbs"],
                                              "unit": "GB/s", "frac": ch_gbs / peaks["hbm_gbs"], "traffic": None,
                                              "peak_source": peaks["source"]}},
+            "compose_diagonal": {"ms_total": ms_dch, "compose_ops_per_s": head_steps / (ms_dch * 1e-3),
+                                 "roofline": {"bound": "hbm", "achieved": gbs_dch, "peak": peaks["hbm_gbs"],
+                                              "unit": "GB/s", "frac": gbs_dch / peaks["hbm_gbs"], "traffic": None,
+                                              "peak_source": peaks["source"]}},
             "rope_compose": {"ms_total": ms_rope, "compose_ops_per_s": head_steps / (ms_rope * 1e-3),
                              "note": "hypic_rope_compose: cos/sin table kernel + fold, per call",
                              "roofline": {"bound": "hbm", "achieved": gbs_rope, "peak": peaks["hbm_gbs"],

@@ -226,8 +226,10 @@ int dg_dispatch(const DiagEncodeArgs& a) {
 constexpr int kDcThreads = 256;
 constexpr int kDcV4 = 4;  // float4s of S per thread: a CTA owns 4,096 consecutive elements of one (request, head)
 
-template <bool CHANNEL, bool F16>
-__global__ void __launch_bounds__(kDcThreads)
+// TSH (diagonal family): dk/4 divides the CTA width, so the four float4s a thread owns sit in the same columns and share
+// ONE float4 of the decay vector per step (otherwise each float4 fetches its own).
+template <bool CHANNEL, bool F16, bool TSH = false>
+__global__ void __launch_bounds__(kDcThreads, (CHANNEL && !TSH) ? 2 : 3)
     diag_compose_kernel(const float* __restrict__ S_in, const void* __restrict__ E_pool,
                         const float* __restrict__ t_pool, const int32_t* __restrict__ seg_ids,
                         const int32_t* __restrict__ cu_segs, int H, int dk, int unit_v4, float* __restrict__ S_out) {
@@ -249,7 +251,9 @@ __global__ void __launch_bounds__(kDcThreads)
   }
   const int dk4 = dk / 4;
   const int j0 = cu_segs[r], j1 = cu_segs[r + 1];
-  float4 e_nxt[kDcV4], t_nxt[CHANNEL ? kDcV4 : 1];  // scalar family: one decay per step (t_nxt[0].x)
+  constexpr int kTn = (CHANNEL && !TSH) ? kDcV4 : 1;
+  float4 e_nxt[kDcV4], t_nxt[kTn];  // scalar family: one decay per step (t_nxt[0].x)
+  const int tcol = tid % dk4;       // TSH: the float4 column all of this thread's float4s share
   auto fetch = [&](int j) {
     const size_t ph = (size_t)seg_ids[j] * H + h;
 #pragma unroll
@@ -262,10 +266,11 @@ __global__ void __launch_bounds__(kDcThreads)
         } else {
           e_nxt[i] = __ldcs(reinterpret_cast<const float4*>(E_pool) + ph * unit_v4 + e4[i]);
         }
-        if (CHANNEL) t_nxt[i] = __ldg(reinterpret_cast<const float4*>(t_pool + ph * dk) + e4[i] % dk4);
+        if (CHANNEL && !TSH) t_nxt[i] = __ldg(reinterpret_cast<const float4*>(t_pool + ph * dk) + e4[i] % dk4);
       }
     }
     if (!CHANNEL) t_nxt[0].x = __ldg(t_pool + ph);
+    if (CHANNEL && TSH) t_nxt[0] = __ldg(reinterpret_cast<const float4*>(t_pool + ph * dk) + tcol);
   };
   if (j0 < j1) fetch(j0);
   for (int j = j0; j < j1; ++j) {
@@ -273,7 +278,7 @@ __global__ void __launch_bounds__(kDcThreads)
 #pragma unroll
     for (int i = 0; i < kDcV4; ++i) {
       e_cur[i] = e_nxt[i];
-      t_cur[i] = CHANNEL ? t_nxt[CHANNEL ? i : 0] : make_float4(t_nxt[0].x, t_nxt[0].x, t_nxt[0].x, t_nxt[0].x);
+      t_cur[i] = CHANNEL ? t_nxt[kTn > 1 ? i : 0] : make_float4(t_nxt[0].x, t_nxt[0].x, t_nxt[0].x, t_nxt[0].x);
     }
     if (j + 1 < j1) fetch(j + 1);
 #pragma unroll
@@ -313,8 +318,11 @@ int diag_compose(const DiagComposeArgs& a) {
   const int unit_v4 = a.dv * a.dk / 4;
   dim3 grid((unit_v4 + kDcThreads * kDcV4 - 1) / (kDcThreads * kDcV4), a.H, a.R);
   const bool ch = a.gate == HYPIC_GATE_CHANNEL;
-  auto kern = a.e_f16 ? (ch ? diag_compose_kernel<true, true> : diag_compose_kernel<false, true>)
-                      : (ch ? diag_compose_kernel<true, false> : diag_compose_kernel<false, false>);
+  const bool tsh = ch && kDcThreads % (a.dk / 4) == 0;
+  auto kern = a.e_f16 ? (ch ? (tsh ? diag_compose_kernel<true, true, true> : diag_compose_kernel<true, true>)
+                            : diag_compose_kernel<false, true>)
+                      : (ch ? (tsh ? diag_compose_kernel<true, false, true> : diag_compose_kernel<true, false>)
+                            : diag_compose_kernel<false, false>);
   kern<<<grid, kDcThreads, 0, a.stream>>>(a.S_in, a.E_pool, a.t_pool, a.seg_ids, a.cu_segs, a.H, a.dk, unit_v4, a.S_out);
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());

@@ -723,6 +723,28 @@ def test_diag_compose_vs_oracle_and_sequential(gate, d):
     check_E(S_all, seq, TOL_F32, "encode -> compose vs sequential")
 
 
+@pytest.mark.parametrize("dk,dv", [(24, 5), (40, 64), (256, 3), (1024, 2)])
+@pytest.mark.parametrize("channel", [False, True])
+def test_diag_compose_general_widths(dk, dv, channel):
+    """hypic_diag_compose outside dk in {64, 128}: widths whose float4 count does not divide the CTA width take the
+    kernel's general decay-vector path (one float4 of tvec per owned float4), the others the shared one."""
+    P, H = 9, 2
+    gen = torch.Generator().manual_seed(5100 + dk + dv)
+    E = torch.randn((P, H, dv, dk), generator=gen).cuda()
+    tv = (torch.rand((P, H, dk) if channel else (P, H), generator=gen) * 0.5 + 0.5).cuda()
+    ids = torch.randint(0, P, (23,), generator=gen, dtype=torch.int32).cuda()
+    cu = torch.tensor([0, 3, 3, 23], dtype=torch.int32, device="cuda")
+    S_in = torch.randn((3, H, dv, dk), generator=gen).cuda()
+    S = hb.hypic_diag_compose(S_in, E, tv, ids, cu)
+    ref = oracle.diag_compose(S_in.cpu().numpy(), E.cpu().numpy(), tv.cpu().numpy(), ids.cpu().numpy(), cu.cpu().numpy())
+    check_E(S, ref, TOL_F32, "S_out (diag compose, general width)")
+    Eh = hb.hypic_tuple_pack_f16(E)
+    Sh = hb.hypic_diag_compose(S_in, Eh, tv, ids, cu)
+    refh = oracle.diag_compose(S_in.cpu().numpy(), Eh.float().cpu().numpy(), tv.cpu().numpy(), ids.cpu().numpy(),
+                               cu.cpu().numpy())
+    check_E(Sh, refh, TOL_F32, "S_out (diag compose, general width, fp16 end-states)")
+
+
 def test_diag_compose_cfg4_lists_sampled_requests():
     """The launch bench.py times for the scalar family's compose (cfg4's request lists over a pool of 1,024 end-states,
     one scalar each), fp32 and fp16-stored end-states: sampled (request, head) chains against the oracle."""
