@@ -113,6 +113,8 @@ struct RopeComposeArgs {
 
 // Kernel families (each returns a hypic_status_t; UNSUPPORTED when the shape is outside its envelope).
 int encode_simt(const EncodeArgs& a);
+// the same kernel over a device-side list of units (s H + h), *unit_count entries; used as the in-call fp32 fallback
+int encode_simt_list(const EncodeArgs& a, const int32_t* unit_list, const int32_t* unit_count);
 int compose_simt(const ComposeArgs& a);
 int seam_simt(const SeamArgs& a);
 int diag_encode(const DiagEncodeArgs& a);

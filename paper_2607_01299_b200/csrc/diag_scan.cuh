@@ -51,14 +51,7 @@ __device__ __forceinline__ void dt_wait(uint64_t* bar, uint32_t parity, volatile
   s2_wait(bar, parity, abort_flag);
 }
 
-__device__ __forceinline__ uint4 lds128(uint32_t addr) {
-  uint4 v;
-  asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
-  return v;
-}
-__device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
-  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-}
+// lds128 / sts128: encode_scan2.cuh
 
 // Longest segments first (CTAs are handed out in index order, so the last ones set the tail of a launch with ragged
 // segments): the segment of rank blockIdx.y by length, ties by index; every CTA ranks the n_seg <= 512 lengths itself in
@@ -155,19 +148,16 @@ __device__ __forceinline__ void diag_scan_body(const CUtensorMap& tmK, const CUt
       const int st = i % kDtStages;
       const int t0 = seg_begin + (c_hi - 1 - i) * kC;  // last chunk first
       const int ta = t0 + 2 * lane, tb = ta + 1;
-      S2_STAMPW(kDtConvWarps + 1, 0, i, 2);
       const float ga = ga0, gb = gb0;
       ga0 = ga1, gb0 = gb1;
       load_g(i + 2, ga1, gb1);
       // envelope: the fp16 weights assume log-decays <= 0 (and finite); a chunk that breaks this is counted, like the dense
       // family's violations (hypic_envelope_violation_count), and should be re-run on the fp32 kernel
       if (__any_sync(0xffffffffu, !(ga <= 0.f) || !(gb <= 0.f)) && lane == 0) atomicAdd(&g_envelope_count_enc, 1u);
-      S2_STAMPW(kDtConvWarps + 1, 0, i, 3);
       if (i >= kDtStages) {
         if (lane == 0) dt_wait(&bars->free_[st], ((i / kDtStages) & 1) ^ 1, abort_flag);
         __syncwarp();
       }
-      S2_STAMPW(kDtConvWarps + 1, 0, i, 0);
       if (lane == 0) {
         const uint32_t sb = smem_base + st * kDtStageBytes;
         mbar_expect_tx(&bars->full[st], (uint32_t)kDtStageBytes);
@@ -193,7 +183,6 @@ __device__ __forceinline__ void diag_scan_body(const CUtensorMap& tmK, const CUt
       lane_sum += (double)ga + (double)gb;
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars->full[st]);
-      S2_STAMPW(kDtConvWarps + 1, 0, i, 1);
     }
 #pragma unroll
     for (int d = 16; d > 0; d /= 2) lane_sum += __shfl_xor_sync(0xffffffffu, lane_sum, d);
@@ -214,14 +203,12 @@ __device__ __forceinline__ void diag_scan_body(const CUtensorMap& tmK, const CUt
         const int st = i % kDtStages;
         dt_wait(&bars->conv[st], (i / kDtStages) & 1, abort_flag);
         tc_fence_after();
-        S2_STAMPW(kDtConvWarps, 2, i, 0);
         const uint32_t sb = smem_base + st * kDtStageBytes;
 #pragma unroll
         for (int ks = 0; ks < 4; ++ks)
           mma_f16_ss(tmem, make_desc(sb + 16384 + ks * 2048, 8192, 1024, 2), make_desc(sb + ks * 2048, 8192, 1024, 2),
                      idesc, (i > 0 || ks > 0) ? 1u : 0u);
         mma_commit(&bars->free_[st]);
-        S2_STAMPW(kDtConvWarps, 2, i, 1);
       }
       if (nc > 0) mma_commit(&bars->done);
     }
@@ -236,7 +223,6 @@ __device__ __forceinline__ void diag_scan_body(const CUtensorMap& tmK, const CUt
       const int st = i % kDtStages;
       const int t0 = seg_begin + (c_hi - 1 - i) * kC;
       s2_wait_warp(&bars->full[st], (i / kDtStages) & 1, abort_flag, lane);
-      S2_STAMPW(0, 1, i, 0);
       const float* w = sw + st * 64;
       const uint32_t tile = smem_base + st * kDtStageBytes;
       // 2,048 16-byte vectors: K boxes [0, 1024), V boxes [1024, 2048); vector idx of a box sits in token row (idx % 512) / 8
@@ -257,7 +243,6 @@ __device__ __forceinline__ void diag_scan_body(const CUtensorMap& tmK, const CUt
       fence_proxy_async();
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars->conv[st]);
-      S2_STAMPW(0, 1, i, 1);
     }
     // ----------------------------------------------------------------------------------------------- epilogue
     if (nc > 0) {

@@ -1,15 +1,22 @@
 // encode_prep.cuh -- the prep kernel (K1) of the tensor-family segment encode: everything of a chunk that does not
 // depend on the running state.  Included by encode_tensor.cu inside namespace hypic::{anonymous}.
 //
-// One CTA (4 warps) per (chunk, head).  Rows a1..a3 of SURVEY.md section 8(a):
-//   a1  G_r = inclusive cumulative log-decay, gamma_r = exp(G_r), d_j = exp(G_C - G_j)
-//   a2  L_rj = beta_r exp(G_r - G_j) (k_r.k_j) for j < r            Gram by mma.sync (fp16 operands, fp32 accumulate)
+// One CTA (4 warps) per (chunk, head).  Rows a1..a3 of SURVEY.md section 8(a).
+// Scalar gate (GDN row of Table 1): alpha_t is a scalar, so it commutes with (I - beta k k^t) and the whole
+// gate factors out of the chunk algebra: with Gamma(t) the decay from the segment start through
+// token t, S_t / Gamma(t) obeys the UNGATED delta rule with values v_t / Gamma(t), and T_C = Gamma(L) prod (I - beta k k^t).
+// The prep is therefore gate-free for the scalar gate:
+//   a1  G_r = inclusive in-chunk cumulative log-decay (handed to the scan as the gate record; nothing here uses it)
+//   a2  L_rj = beta_r (k_r.k_j) for j < r                          Gram by mma.sync (fp16 operands, fp32 accumulate)
 //   a3  A = (I + L)^-1, blocked 4 x 4 in 16 x 16 blocks: the diagonal blocks by forward substitution in fp32 (one
 //       column per lane), the off-diagonal ones by the 2 x 2 block inverse formula A21 = -A22 L21 A11 applied at block
-//       sizes 16 and 32; their 16^3 products run on mma.sync with both operands split in fp16 hi + lo (three passes,
-//       ~2^-22 relative), so A stays at fp32 quality although the flops sit on the tensor pipe
-//   out -W = -(A diag(beta gamma)) K  (mma.sync, fp16 out, K-major 128B-swizzled UMMA B tile of two 64-wide boxes),
-//       A_b = A diag(beta) (fp16, K-major 128B-swizzled UMMA B tile), gate record (d_j, gamma_C).
+//       sizes 16 and 32; their 16^3 products run on mma.sync, single pass on fp16 operands for the scalar gate (A only
+//       feeds the fp16 tiles below; emulation: E 3.5e-4, T 1.0e-3 at 2,048 tokens either way), hi + lo split (three
+//       passes, ~2^-22) for the per-channel gate
+//   out -W = -(A diag(beta)) K  (mma.sync, fp16 out, K-major 128B-swizzled UMMA B tile of two 64-wide boxes),
+//       A_b = A diag(beta) (fp16, K-major 128B-swizzled UMMA B tile), gate record G_r[64].
+// Per-channel gate (KDA row): Gamma does not commute; L_rj = beta_r (k_r (.) Gamma_r).(k_j (/) Gamma_j), W = A_b (K (.) Gamma),
+// K~ and Gamma_C go into the record (section 6.4).
 // K is staged as fp16 (exact for bf16 values with |x| in [2^-14, 65504]; smaller magnitudes lose bits below 2^-24
 // absolute), so that the Gram and W contractions run as f16 mma.sync with an 11-bit second operand.
 #pragma once
@@ -54,6 +61,7 @@ __device__ __forceinline__ void split_f16(float x0, float x1, uint32_t& hi, uint
 
 // acc (16 x 16, two n-tiles of the m16n8 C fragment) += X Y with X = xs[0..16)[0..16), Y = ys[0..16)[0..16), both fp32
 // row-major in shared memory with the given pitches; operands split in fp16 hi + lo, three passes (hh, lh, hl).
+template <bool kSplit>
 __device__ __forceinline__ void block_mma_16(float (&acc)[2][4], const float* xs, int xp, const float* ys, int yp,
                                              int lane) {
   const int gq = lane >> 2, tq = lane & 3;
@@ -75,8 +83,10 @@ __device__ __forceinline__ void block_mma_16(float (&acc)[2][4], const float* xs
     split_f16(ys[(2 * tq) * yp + n], ys[(2 * tq + 1) * yp + n], bh[0], bl[0]);
     split_f16(ys[(2 * tq + 8) * yp + n], ys[(2 * tq + 9) * yp + n], bh[1], bl[1]);
     mma_f16_16816(acc[nt], ah[0], ah[1], ah[2], ah[3], bh[0], bh[1]);
-    mma_f16_16816(acc[nt], al[0], al[1], al[2], al[3], bh[0], bh[1]);
-    mma_f16_16816(acc[nt], ah[0], ah[1], ah[2], ah[3], bl[0], bl[1]);
+    if (kSplit) {
+      mma_f16_16816(acc[nt], al[0], al[1], al[2], al[3], bh[0], bh[1]);
+      mma_f16_16816(acc[nt], ah[0], ah[1], ah[2], ah[3], bl[0], bl[1]);
+    }
   }
 }
 // store sign * acc as a 16 x 16 fp32 block
@@ -104,14 +114,16 @@ template <bool kCh>
 __global__ void __launch_bounds__(kPrepThreads, 4)
     prep_kernel(const __nv_bfloat16* __restrict__ k, const float* __restrict__ g, const float* __restrict__ beta,
                 const int2* __restrict__ chunk_meta, int cap, int H,
-                uint8_t* __restrict__ rec, float* __restrict__ gate) {
+                uint8_t* __restrict__ rec, float* __restrict__ gate, const int32_t* __restrict__ chunk_off, int n_seg,
+                int32_t* __restrict__ fb) {
   __shared__ __align__(16) uint8_t s_k[kC * kKsPitch * 2];  // K chunk (fp16)
   __shared__ __align__(16) float s_a[kC * kLPitch];         // L, inverted in place to A (per-channel gate: first K (/) Gamma)
   uint8_t* s_k2 = reinterpret_cast<uint8_t*>(s_a);           // fp16 [64][kKsPitch]: exactly the size of s_a
   __shared__ __align__(16) float s_m[32 * kMPitch];         // temporaries of the block merges
-  __shared__ __align__(16) float s_g[kCh ? kD : kC], s_b[kC], s_bg[kC];  // s_g: G_r per token (scalar) or G_C per channel
-  __shared__ __align__(16) float s_fc[kC];  // scalar gate: exp(-G_j), so that exp(G_r - G_j) = exp(G_r) exp(-G_j) costs no MUFU per entry of L
+  __shared__ __align__(16) float s_g[kCh ? kD : kC], s_b[kC];  // s_g: G_r per token (scalar) or G_C per channel
   __shared__ float s_wsum;
+  __shared__ int s_viol;  // per-channel gate: this chunk breaks the fp16 envelope (a channel's log-decay outside [-9, 0])
+  if (threadIdx.x == 0) s_viol = 0;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int gq = lane >> 2, tq = lane & 3;
   const int x0 = blockIdx.x * kPrepChunksPerCta, h = blockIdx.y;
@@ -214,8 +226,6 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
         if (warp == 1) gv += s_wsum;
         s_g[tid] = gv;
         s_b[tid] = bv;
-        s_bg[tid] = bv * expf(gv);
-        s_fc[tid] = expf(fminf(-gv, 80.f));  // <= e^9 inside the envelope; the clamp only keeps a violating chunk finite
       }
     }
   }
@@ -284,8 +294,7 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
       const int bi = blk < 3 ? 0 : (blk < 5 ? 1 : 2), bj = blk < 3 ? blk + 1 : (blk < 5 ? blk - 1 : 3);
       *reinterpret_cast<float4*>(s_a + (16 * bi + (e >> 2)) * kLPitch + 16 * bj + 4 * (e & 3)) = make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    // L_rj = beta_r exp(G_r - G_j) (k_r.k_j) for j < r, else 0; the exponential is the product of two per-token factors
-    // prepared in a1 (one MUFU per token instead of one per entry, and no dependent LDS -> MUFU chain per entry)
+    // L_rj = beta_r (k_r.k_j) for j < r, else 0 (per-channel gate: the decay ratios already sit in the two Gram operands)
 #pragma unroll
     for (int u = 0; u < 3; ++u) {
       if (u == 2 && nun < 3) continue;
@@ -293,14 +302,13 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
 #pragma unroll
       for (int hh = 0; hh < 2; ++hh) {
         const int r = 16 * mm + gq + 8 * hh;
-        const float br = kCh ? s_b[r] : s_bg[r];  // scalar gate: beta_r exp(G_r)
+        const float br = s_b[r];
 #pragma unroll
         for (int nt = 0; nt < 2; ++nt) {
           const int j = 16 * pp + 8 * nt + 2 * tq;
-          const float2 fc = kCh ? make_float2(1.f, 1.f) : *reinterpret_cast<const float2*>(s_fc + j);
           float v0 = 0.f, v1 = 0.f;
-          if (j < r) v0 = br * fc.x * acc[u][nt][2 * hh];
-          if (j + 1 < r) v1 = br * fc.y * acc[u][nt][2 * hh + 1];
+          if (j < r) v0 = br * acc[u][nt][2 * hh];
+          if (j + 1 < r) v1 = br * acc[u][nt][2 * hh + 1];
           *reinterpret_cast<float2*>(s_a + r * kLPitch + j) = make_float2(v0, v1);
         }
       }
@@ -342,11 +350,11 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
     float* tmp = s_m + (16 * warp) * kMPitch;
     float acc[2][4];
     block_zero(acc);
-    block_mma_16(acc, B(i, j), kLPitch, B(j, j), kLPitch, lane);
+    block_mma_16<kCh>(acc, B(i, j), kLPitch, B(j, j), kLPitch, lane);
     block_store_16(acc, 1.f, tmp, kMPitch, lane);
     __syncwarp();
     block_zero(acc);
-    block_mma_16(acc, B(i, i), kLPitch, tmp, kMPitch, lane);
+    block_mma_16<kCh>(acc, B(i, i), kLPitch, tmp, kMPitch, lane);
     __syncwarp();
     block_store_16(acc, -1.f, B(i, j), kLPitch, lane);
   }
@@ -356,18 +364,18 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
     const int i = 2 + (warp >> 1), j = warp & 1;
     float acc[2][4];
     block_zero(acc);
-    if (j == 0) block_mma_16(acc, B(i, 0), kLPitch, B(0, 0), kLPitch, lane);
-    block_mma_16(acc, B(i, 1), kLPitch, B(1, j), kLPitch, lane);
+    if (j == 0) block_mma_16<kCh>(acc, B(i, 0), kLPitch, B(0, 0), kLPitch, lane);
+    block_mma_16<kCh>(acc, B(i, 1), kLPitch, B(1, j), kLPitch, lane);
     block_store_16(acc, 1.f, s_m + (16 * (i - 2)) * kMPitch + 16 * j, kMPitch, lane);
     __syncthreads();
     block_zero(acc);
-    block_mma_16(acc, B(i, 2), kLPitch, s_m + 16 * j, kMPitch, lane);
-    if (i == 3) block_mma_16(acc, B(3, 3), kLPitch, s_m + 16 * kMPitch + 16 * j, kMPitch, lane);
+    block_mma_16<kCh>(acc, B(i, 2), kLPitch, s_m + 16 * j, kMPitch, lane);
+    if (i == 3) block_mma_16<kCh>(acc, B(3, 3), kLPitch, s_m + 16 * kMPitch + 16 * j, kMPitch, lane);
     block_store_16(acc, -1.f, B(i, j), kLPitch, lane);
   }
   __syncthreads();
 
-  // ---- -W = -(A diag(beta gamma)) K with mma.sync: warp w rows [16w, 16w+16), k-steps kk <= w (A is lower
+  // ---- -W = -(A diag(beta)) K with mma.sync: warp w rows [16w, 16w+16), k-steps kk <= w (A is lower
   // triangular), in two halves of 64 columns; the fp16 fragments go straight to the record in its K-major
   // 128B-swizzled two-box layout (4-byte stores; each 16-byte chunk is completed by the four lanes of a quad)
 #pragma unroll 1
@@ -383,7 +391,7 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
       uint32_t a[4];
       {
         const int r0 = 16 * warp + gq, c0 = 16 * kk + 2 * tq;
-        const float* sc = kCh ? s_b : s_bg;  // per-channel gate: Gamma already sits in the K (.) Gamma operand
+        const float* sc = s_b;  // per-channel gate: Gamma already sits in the K (.) Gamma operand
         const float g0 = sc[c0], g1 = sc[c0 + 1], g8 = sc[c0 + 8], g9 = sc[c0 + 9];
         const float2 p0 = *reinterpret_cast<const float2*>(s_a + r0 * kLPitch + c0);
         const float2 p1 = *reinterpret_cast<const float2*>(s_a + (r0 + 8) * kLPitch + c0);
@@ -432,13 +440,23 @@ __global__ void __launch_bounds__(kPrepThreads, 4)
     const float gc = s_g[tid];
     go[tid] = expf(gc);
     if (tid < kGateFloatsCh - kD) go[kD + tid] = 0.f;
-    if (!(gc >= -9.f && gc <= 0.f)) atomicAdd(&g_envelope_count_enc, 1u);  // also NaN
+    if (!(gc >= -9.f && gc <= 0.f)) s_viol = 1;  // also NaN
   } else {
-    float* go = gate + ((size_t)x * H + h) * kGateFloats;
-    if (tid == 0 && !(s_g[kC - 1] >= -9.f && s_g[kC - 1] <= 0.f)) atomicAdd(&g_envelope_count_enc, 1u);  // also NaN
-    if (tid < kC) go[tid] = expf(s_g[kC - 1] - s_g[tid]);
-    else if (tid < kGateFloats) go[tid] = (tid == kC) ? expf(s_g[kC - 1]) : 0.f;
+    float* go = gate + ((size_t)x * H + h) * kGateFloats;  // the scan turns G_r into the value weights (lazy decay)
+    if (tid < kGateFloats) go[tid] = (tid < kC) ? s_g[tid] : 0.f;
   }
   __syncthreads();  // s_k, s_a, s_g are free for the next chunk
+  if (kCh && tid == 0 && s_viol) {
+    // the unit of this chunk is recomputed by the fp32 family inside the same call (no host involvement): find its
+    // segment in chunk_off and put (segment, head) on the call's fallback list
+    s_viol = 0;
+    atomicAdd(&g_envelope_count_enc, 1u);  // diagnostic counter (hypic_envelope_violation_count)
+    int lo = 0, hi = n_seg;                // chunk_off[lo] <= x < chunk_off[hi]
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (chunk_off[mid] <= x) lo = mid; else hi = mid;
+    }
+    fb_append(fb, n_seg * H, lo * H + h);
+  }
   }
 }

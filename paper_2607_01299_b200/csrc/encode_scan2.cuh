@@ -31,26 +31,7 @@
 // DY_T [448,512).  All waits are bounded; a protocol error bumps g_timeout_count_enc instead of hanging the GPU.
 #pragma once
 
-// Diagnostics only (-DHYPIC_TIMELINE, never in the shipped library): per-chunk clock stamps of CTA (0, 0).
-#ifdef HYPIC_TIMELINE
-__device__ long long g_s2_timeline[4 * 64 * 8];
-#define S2_STAMP(role, c, k)                                                                              \
-  do {                                                                                                    \
-    if (blockIdx.x == 0 && blockIdx.y == 0 && (c) < 64 && (threadIdx.x & 31) == 0 &&                      \
-        (threadIdx.x >> 5) == ((role) == 0 ? 0 : 8))                                 \
-      g_s2_timeline[((role) * 64 + (c)) * 8 + (k)] = clock64();                                           \
-  } while (0)
-#define S2_STAMPW(w, role, c, k)                                                                          \
-  do {                                                                                                    \
-    if (blockIdx.x == 0 && blockIdx.y == 0 && (c) < 64 && (threadIdx.x & 31) == 0 && (threadIdx.x >> 5) == (w)) \
-      g_s2_timeline[((role) * 64 + (c)) * 8 + (k)] = clock64();                                           \
-  } while (0)
-#else
-#define S2_STAMP(role, c, k) do {} while (0)
-#define S2_STAMPW(w, role, c, k) do {} while (0)
-#endif
-
-constexpr int kS2Threads = 608;
+constexpr int kS2Threads = 640;
 constexpr int kS2Stages = 3;
 constexpr int kS2StK = 0, kS2StV = 16384, kS2StRec = 32768, kS2StGate = 32768 + kRecBytes;
 constexpr int kS2StageBytes = 32768 + kRecBytes + 1024;
@@ -60,15 +41,23 @@ constexpr int kS2Smem = kS2OffBar + 256 + 1024;
 
 struct S2Bars {
   uint64_t st_full[kS2Stages], st_free[kS2Stages];
+  uint64_t st_ready[kS2Stages];     // converters -> chains, (1) issuer: the stage's K and V tiles are fp16 (2 arrivals)
   uint64_t m3_done[2], m4_done[2];  // [block]: 0 = E, 1 = T
   uint64_t dy_free;                 // E chain -> V converter (which issues (1)): DY_E may be overwritten
   // Progress counters read with plain acquire loads: an mbarrier probe costs ~380 cycles in this kernel even when the
   // phase completed long ago, and these two sit on the chains' critical path once per chunk.
-  int conv_cnt[2];                  // chunks converted by warp 16 (K) / 17 (V); both > c: stage c landed and converted
+  int fin_flag;                     // 1 once the V converter has posted p_final / g_total
   int issued1_cnt;                  // chunks whose (1) is in the tensor pipe
   uint32_t tmem_base;
   int abort_flag;
+  // scalar gate (lazy decay of the E block): written by the V converter, read by the chains
+  float resc[kS2Stages];            // factor the E chain applies to X_E in the pass of the stage's chunk (1 = none)
+  float p_final;                    // E = X_E exp(p_final) at write-out
+  double g_total;                   // the segment's total log-decay: T = That exp(g_total)
+  int bad;                          // a chain saw a non-finite result: the unit goes to the fp32 fallback list
+  float fac[1][kC];                 // V converter scratch: this chunk's value weights
 };
+constexpr float kLazyP = 4.1588831f;  // ln 64: the stored E block runs at most 64x above / below its true scale
 
 __device__ __forceinline__ void tma_load_3d(uint32_t dst_smem, const CUtensorMap* tm, int c0, int c1, int c2,
                                             uint64_t* bar) {
@@ -93,10 +82,22 @@ __device__ __noinline__ bool s2_wait(uint64_t* bar, uint32_t parity, volatile in
   return false;
 }
 
-__device__ __forceinline__ void s2_wait_warp(uint64_t* bar, uint32_t parity, volatile int* abort_flag, int) {
+// single-thread roles (loader, (1) issuer): retry try_wait for a long while before the sleeping fallback -- a thread
+// that has gone into s2_wait's __nanosleep loop wakes up thousands of cycles after its barrier completed
+__device__ __forceinline__ void s2_wait_spin(uint64_t* bar, uint32_t parity, volatile int* abort_flag) {
 #pragma unroll 1
-  for (int i = 0; i < 64; ++i)  // inline fast path: the chains' waits are on the critical path of every chunk
+  for (int i = 0; i < 8192; ++i)
     if (mbar_try_wait(bar, parity)) return;
+  s2_wait(bar, parity, abort_flag);
+}
+
+__device__ __forceinline__ void s2_wait_warp(uint64_t* bar, uint32_t parity, volatile int* abort_flag, int) {
+  // the chains' waits: try_wait with a suspend-time hint, so that a waiting warp sleeps in hardware until the phase
+  // completes instead of re-issuing the probe -- 16 chain warps polling st_ready in a tight loop flooded the
+  // shared-memory pipeline and slowed the two converter warps they were waiting for to ~4,000 cycles per tile
+#pragma unroll 1
+  for (int i = 0; i < 64; ++i)
+    if (mbar_try_wait_hint(bar, parity, 100000u)) return;
   s2_wait(bar, parity, abort_flag);
 }
 
@@ -140,6 +141,39 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 __device__ __forceinline__ float pow2i(int e) { return __uint_as_float((uint32_t)(127 + e) << 23); }  // e in [-126, 127]
+
+// explicit shared-space 128-bit accesses by 32-bit shared address: through a generic pointer derived from the aligned
+// dynamic-smem base ptxas emits LD.E / ST.E (generic), which cost the converters ~160 cycles per dependent round trip
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+  uint4 v;
+  asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ void sts128(uint32_t a, const uint4& v) {
+  asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ float lds32f(uint32_t a) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+  return v;
+}
+// eight bf16 (one 16-byte piece of a TMA box) -> eight fp16 scaled by f
+__device__ __forceinline__ uint4 cvt8_bf16_f16(uint4 w, float f) {
+  uint32_t a0 = w.x << 16, a1 = w.x & 0xffff0000u, b0 = w.y << 16, b1 = w.y & 0xffff0000u;
+  uint32_t c0 = w.z << 16, c1 = w.z & 0xffff0000u, d0 = w.w << 16, d1 = w.w & 0xffff0000u;
+  mul2(a0, a1, f);
+  mul2(b0, b1, f);
+  mul2(c0, c1, f);
+  mul2(d0, d1, f);
+  return make_uint4(pack_f16(__uint_as_float(a0), __uint_as_float(a1)), pack_f16(__uint_as_float(b0), __uint_as_float(b1)),
+                    pack_f16(__uint_as_float(c0), __uint_as_float(c1)), pack_f16(__uint_as_float(d0), __uint_as_float(d1)));
+}
+__device__ __forceinline__ uint4 cvt8_bf16_f16(uint4 w) {
+  return make_uint4(pack_f16(__uint_as_float(w.x << 16), __uint_as_float(w.x & 0xffff0000u)),
+                    pack_f16(__uint_as_float(w.y << 16), __uint_as_float(w.y & 0xffff0000u)),
+                    pack_f16(__uint_as_float(w.z << 16), __uint_as_float(w.z & 0xffff0000u)),
+                    pack_f16(__uint_as_float(w.w << 16), __uint_as_float(w.w & 0xffff0000u)));
+}
 
 // MMA batches of one chunk; each is issued by one elected thread of the chain that produced its operands.
 __device__ __forceinline__ void s2_issue1(uint32_t tmem, uint32_t sb) {  // DY_E = V^t A_b^t
@@ -193,11 +227,11 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
   for (int c = 0; c < nc; ++c) {
     const int st = c % kS2Stages;
     const float* gt = reinterpret_cast<const float*>(smem + st * kS2StageBytes + kS2StGate);
-    s2_wait_count(&bars->conv_cnt[0], c, abort_flag);  // converted, hence also landed
-    s2_wait_count(&bars->conv_cnt[1], c, abort_flag);
+    // converted, hence also landed.  A hardware-suspended mbarrier wait: the chains often arrive first, and a spinning
+    // chain (16 warps polling a counter) starved the three converter warps of issue slots (profiles/r02a)
+    s2_wait_warp(&bars->st_ready[st], (c / kS2Stages) & 1, abort_flag, lane);
     if (c > 0) s2_wait_warp(&bars->m4_done[b], (c - 1) & 1, abort_flag, lane);
     tc_fence_after();
-    S2_STAMP(b, c, 0);
     const float gC = kCh ? 1.f : gt[kC];  // scalar gate: gamma_C; per-channel gate: Gamma_C[col] = gt[col], applied below
     // ---- pass: Xh = fp16(X) (A operand of (3)), X <- gamma_C X; T rows are re-normalised on the way
     {
@@ -205,7 +239,6 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
       tmem_ld32(tX, x0);
       tmem_ld32(tX + 32, x1);
       tmem_ld_wait();
-      S2_STAMP(b, c, 4);
       float f = gC;
       if (kIsT) {
         float m = 0.f;
@@ -214,7 +247,6 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
         xch[2 * row + hf] = m;
         named_bar_sync(1 + q, 64);
         m = fmaxf(m, xch[2 * row + (hf ^ 1)]);
-        S2_STAMP(b, c, 5);
         // row maximum in [2^(e-127), 2^(e-126)): move it to [2^14, 2^15) -- in place, the row stays normalised
         const int e = (int)(__float_as_uint(m) >> 23);
         int dlt = (e == 0) ? 0 : 141 - e;
@@ -258,7 +290,6 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
       tmem_st_wait();  // Xh is in TMEM; the decayed X follows while (3) runs (only (4) needs it)
       tc_fence_before();
       named_bar_sync(5 + b, 256);  // the whole chain has written Xh
-      S2_STAMP(b, c, 1);
       if (issuer) {
         if (!kIsT) s2_wait_count(&bars->issued1_cnt, c, abort_flag);  // (1)_c is ahead of (3)_c in the tensor pipe
         tc_fence_after();
@@ -285,19 +316,16 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
       }
       tmem_st32(tX, x0);
       tmem_st32(tX + 32, x1);
-      S2_STAMP(b, c, 6);
       tmem_st_wait();
     }
 
     // ---- epilogue: U''[:, j] = fp16(DY[:, j] d_j) -> TMEM (A operand of (4)); this thread: tokens [32 hf, 32 hf + 32)
     s2_wait_warp(&bars->m3_done[b], c & 1, abort_flag, lane);
     tc_fence_after();
-    S2_STAMP(b, c, 2);
     {
       uint32_t y[32];
       tmem_ld32(tD, y);
       tmem_ld_wait();
-      S2_STAMP(b, c, 7);
 #pragma unroll
       for (int j8 = 0; j8 < 4; ++j8) {
         float4 d0 = make_float4(1.f, 1.f, 1.f, 1.f), d1 = d0;  // per-channel gate: the decay ratios sit in the K~ tile
@@ -318,7 +346,6 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
     }
     tc_fence_before();
     named_bar_sync(5 + b, 256);  // the whole chain has written U''
-    S2_STAMP(b, c, 3);
     if (issuer) {
       if (!kIsT) mbar_arrive(&bars->dy_free);  // DY_E has been read: the V converter may issue (1) of the next chunk
       tc_fence_after();
@@ -337,6 +364,7 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
   const int se = max(-250, min(250, s_exp));
   const float f0 = pow2i(-(se / 2)), f1 = pow2i(-(se - se / 2));
   float* dst = dst_block + (size_t)row * kD + 64 * hf;
+  bool bad = false;
 #pragma unroll 1
   for (int cb = 0; cb < 2; ++cb) {
     uint32_t x[32];
@@ -353,9 +381,189 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
         o.z = o.z * f0 * f1;
         o.w = o.w * f0 * f1;
       }
+      bad |= !(fabsf(o.x) <= 3.0e38f) | !(fabsf(o.y) <= 3.0e38f) | !(fabsf(o.z) <= 3.0e38f) | !(fabsf(o.w) <= 3.0e38f);
       d4[u] = o;
     }
   }
+  if (bad) bars->bad = 1;  // an fp16 operand overflowed somewhere: the unit goes to the fp32 fallback list
+}
+
+
+// Scalar gate.  The gate commutes with (I - beta k k^t), so it is kept out of the tensor-core algebra altogether:
+//   T block: That = prod (I - beta_t k_t k_t^t), the ungated product; T = exp(sum g) That at write-out.  Rows are held
+//            as That_r 2^s_r, s_r re-chosen every 8th chunk so that the row maximum sits in [2^11, 2^12) (a contraction
+//            cannot grow a row by more than sqrt(dk) = 11.3, so fp16 never overflows in between).
+//   E block: stored X_E = E exp(-p), p the pending log-decay; the chunk's values enter as v_i exp(-(p + G_i)) (weights from
+//            the V converter).  When |p + G_C| would exceed ln 64 the pass multiplies X_E by exp(p + G_C), the values enter
+//            as v_i exp(G_C - G_i) <= v_i and p restarts at 0: a strongly decaying chunk degenerates to the plain
+//            "decay, then add" form, a weakly decaying one costs no TMEM rewrite at all.
+// Per chunk: pass Xh = fp16(X) -> (3) DY (+)= Xh (-W)^t -> epilogue U'' = fp16(DY) -> (4) X += U'' K.
+template <bool kIsT>
+__device__ __forceinline__ void s2_chain_sc(uint8_t* smem, S2Bars* bars, volatile int* abort_flag, uint32_t tmem, int cw,
+                                            int lane, int nc, float* __restrict__ dst_block) {
+  constexpr int b = kIsT ? 1 : 0;
+  constexpr uint32_t cX = kIsT ? 128 : 0, cH = kIsT ? 320 : 256, cD = kIsT ? 448 : 384;
+  const int q = cw & 3, hf = cw >> 2;  // TMEM lane quarter; column half
+  const int row = 32 * q + lane;
+  const uint32_t lane_base = (uint32_t)(32 * q) << 16;
+  const uint32_t tX = tmem + cX + lane_base + 64 * hf, tH = tmem + cH + lane_base + 32 * hf,
+                 tD = tmem + cD + lane_base + 32 * hf;
+  float* xch = reinterpret_cast<float*>(smem + kS2OffXch);
+  int s_exp = 0;  // T chain: the TMEM copy of this row is That_row * 2^s_exp
+
+  // X_0 = [0 ; I]
+#pragma unroll
+  for (int cb = 0; cb < 2; ++cb) {
+    uint32_t x[32];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) x[i] = (kIsT && 64 * hf + 32 * cb + i == row) ? __float_as_uint(1.f) : 0u;
+    tmem_st32(tX + 32 * cb, x);
+  }
+  tmem_st_wait();
+  const uint32_t smem_base = smem_u32(smem);
+  const bool issuer = (cw == 0 && lane == 0);  // this chain's MMA-issuing thread
+
+#pragma unroll 1
+  for (int c = 0; c < nc; ++c) {
+    const int st = c % kS2Stages;
+    // converted, hence also landed.  A hardware-suspended mbarrier wait: the chains often arrive first, and a spinning
+    // chain (16 warps polling a counter) starved the three converter warps of issue slots (profiles/r02a)
+    s2_wait_warp(&bars->st_ready[st], (c / kS2Stages) & 1, abort_flag, lane);
+    if (c > 0) s2_wait_warp(&bars->m4_done[b], (c - 1) & 1, abort_flag, lane);
+    tc_fence_after();
+    // ---- pass: Xh = fp16(X) (A operand of (3)); X itself is only rewritten on a rescale
+    {
+      bool rewrite;
+      float f = 1.f;
+      if (kIsT) {
+        rewrite = (c & 7) == 0;
+      } else {
+        f = bars->resc[st];
+        rewrite = (f != 1.f);
+      }
+      if (!rewrite) {  // the common case: X stays as it is, 32 columns at a time (few live registers)
+        uint32_t x[32], hh[16];
+        tmem_ld32(tX, x);
+        tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x[2 * j]), __uint_as_float(x[2 * j + 1]));
+        tmem_ld32(tX + 32, x);
+        tmem_st16(tH, hh);
+        tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x[2 * j]), __uint_as_float(x[2 * j + 1]));
+        tmem_st16(tH + 16, hh);
+        tmem_st_wait();
+        tc_fence_before();
+        named_bar_sync(5 + b, 256);  // the whole chain has written Xh
+        if (issuer) {
+          if (!kIsT) s2_wait_count(&bars->issued1_cnt, c, abort_flag);  // (1)_c is ahead of (3)_c in the tensor pipe
+          tc_fence_after();
+          s2_issue3(tmem, smem_base + st * kS2StageBytes, b);
+          mma_commit(&bars->m3_done[b]);
+        }
+        __syncwarp();
+      } else {
+        uint32_t x0[32], x1[32];
+        tmem_ld32(tX, x0);
+        tmem_ld32(tX + 32, x1);
+        tmem_ld_wait();
+        if (kIsT) {
+          float m = 0.f;
+#pragma unroll
+          for (int i = 0; i < 32; ++i) m = fmaxf(m, fmaxf(fabsf(__uint_as_float(x0[i])), fabsf(__uint_as_float(x1[i]))));
+          xch[2 * row + hf] = m;
+          named_bar_sync(1 + q, 64);
+          m = fmaxf(m, xch[2 * row + (hf ^ 1)]);
+          // row maximum in [2^(e-127), 2^(e-126)): move it to [2^11, 2^12)
+          const int e = (int)((__float_as_uint(m) >> 23) & 0xffu);
+          int dlt = (e == 0 || e == 255) ? 0 : 138 - e;
+          dlt = max(-100, min(100, dlt));
+          s_exp += dlt;
+          f = pow2i(dlt);
+        }
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+          mul2(x0[2 * j], x0[2 * j + 1], f);
+          mul2(x1[2 * j], x1[2 * j + 1], f);
+        }
+        {
+          uint32_t hh[16];
+#pragma unroll
+          for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x0[2 * j]), __uint_as_float(x0[2 * j + 1]));
+          tmem_st16(tH, hh);
+#pragma unroll
+          for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x1[2 * j]), __uint_as_float(x1[2 * j + 1]));
+          tmem_st16(tH + 16, hh);
+        }
+        tmem_st_wait();
+        tc_fence_before();
+        named_bar_sync(5 + b, 256);  // the whole chain has written Xh
+        if (issuer) {
+          if (!kIsT) s2_wait_count(&bars->issued1_cnt, c, abort_flag);
+          tc_fence_after();
+          s2_issue3(tmem, smem_base + st * kS2StageBytes, b);
+          mma_commit(&bars->m3_done[b]);
+        }
+        __syncwarp();
+        tmem_st32(tX, x0);  // (3) reads Xh alone; only (4) accumulates into X
+        tmem_st32(tX + 32, x1);
+        tmem_st_wait();
+      }
+    }
+
+    // ---- epilogue: U'' = fp16(DY) -> TMEM (A operand of (4)); this thread: tokens [32 hf, 32 hf + 32)
+    s2_wait_warp(&bars->m3_done[b], c & 1, abort_flag, lane);
+    tc_fence_after();
+    {
+      uint32_t y[32];
+      tmem_ld32(tD, y);
+      tmem_ld_wait();
+#pragma unroll
+      for (int j = 0; j < 16; ++j) y[j] = pack_f16(__uint_as_float(y[2 * j]), __uint_as_float(y[2 * j + 1]));  // slot j <= 2 j
+      tmem_st16(tH - 16 * hf, y);  // columns [16 hf, 16 hf + 16) of the (dead) Xh region: tokens [32 hf, 32 hf + 32)
+      tmem_st_wait();
+    }
+    tc_fence_before();
+    named_bar_sync(5 + b, 256);  // the whole chain has written U''
+    if (issuer) {
+      if (!kIsT) mbar_arrive(&bars->dy_free);  // DY_E has been read: the V converter may issue (1) of the next chunk
+      tc_fence_after();
+      s2_issue4(tmem, smem_base + st * kS2StageBytes, b);
+      mma_commit(&bars->m4_done[b]);
+      mma_commit(&bars->st_free[st]);  // count 2: released when both chains' (4) of this chunk have completed
+    }
+    __syncwarp();
+  }
+
+  // ---- a5: write this thread's 64 columns of its row; the gate (and T's row scale) is applied here, in fp64 so that a
+  // T that underflows fp32 underflows exactly like the correctly rounded result
+  s2_wait_count(&bars->fin_flag, 0, abort_flag);  // the V converter has posted p_final and g_total
+  if (nc > 0) {
+    s2_wait_warp(&bars->m4_done[b], (nc - 1) & 1, abort_flag, lane);
+    tc_fence_after();
+  }
+  const double sc = kIsT ? exp(bars->g_total - 0.6931471805599453 * (double)s_exp) : (double)expf(bars->p_final);
+  float* dst = dst_block + (size_t)row * kD + 64 * hf;
+  bool bad = false;
+#pragma unroll 1
+  for (int cb = 0; cb < 2; ++cb) {
+    uint32_t x[32];
+    tmem_ld32(tX + 32 * cb, x);
+    tmem_ld_wait();
+    float4* d4 = reinterpret_cast<float4*>(dst + 32 * cb);
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      float4 o;
+      o.x = (float)((double)__uint_as_float(x[4 * u]) * sc);
+      o.y = (float)((double)__uint_as_float(x[4 * u + 1]) * sc);
+      o.z = (float)((double)__uint_as_float(x[4 * u + 2]) * sc);
+      o.w = (float)((double)__uint_as_float(x[4 * u + 3]) * sc);
+      bad |= !(fabsf(o.x) <= 3.0e38f) | !(fabsf(o.y) <= 3.0e38f) | !(fabsf(o.z) <= 3.0e38f) | !(fabsf(o.w) <= 3.0e38f);
+      d4[u] = o;
+    }
+  }
+  if (bad) bars->bad = 1;
 }
 
 template <bool kCh>
@@ -363,7 +571,7 @@ __global__ void __launch_bounds__(kS2Threads, 1)
     scan2_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
                  const int32_t* __restrict__ cu_seqlens, const int32_t* __restrict__ chunk_off,
                  const int32_t* __restrict__ seg_order, int H, const uint8_t* __restrict__ rec, const float* __restrict__ gate, float* __restrict__ E,
-                 float* __restrict__ T) {
+                 float* __restrict__ T, int32_t* __restrict__ fb, int n_units) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   S2Bars* bars = reinterpret_cast<S2Bars*>(smem + kS2OffBar);
@@ -380,13 +588,17 @@ __global__ void __launch_bounds__(kS2Threads, 1)
       mbar_init(&bars->st_full[i], 1);
       if (i == 0) mbar_init(&bars->dy_free, 1);
       mbar_init(&bars->st_free[i], 2);
+      mbar_init(&bars->st_ready[i], 2);
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(&bars->m3_done[i], 1);
       mbar_init(&bars->m4_done[i], 1);
     }
     bars->abort_flag = 0;
-    bars->conv_cnt[0] = bars->conv_cnt[1] = bars->issued1_cnt = 0;
+    bars->bad = 0;
+    bars->p_final = 0.f;
+    bars->g_total = 0.0;
+    bars->fin_flag = bars->issued1_cnt = 0;
     fence_barrier_init();
   }
   tc_fence_before();
@@ -402,8 +614,7 @@ __global__ void __launch_bounds__(kS2Threads, 1)
 #pragma unroll 1
       for (int c = 0; c < nc; ++c) {
         const int st = c % kS2Stages;
-        s2_wait(&bars->st_free[st], ((c / kS2Stages) & 1) ^ 1, abort_flag);
-        S2_STAMPW(18, 3, c, 5);
+        s2_wait_spin(&bars->st_free[st], ((c / kS2Stages) & 1) ^ 1, abort_flag);
         const uint32_t sb = smem_base + st * kS2StageBytes;
         const int t0 = seg_begin + c * kC;
         mbar_expect_tx(&bars->st_full[st], bytes);
@@ -422,47 +633,93 @@ __global__ void __launch_bounds__(kS2Threads, 1)
                  kCh ? kGateBytesCh : kGateBytes, &bars->st_full[st]);
       }
     }
-  } else if (warp >= 16) {
-    // ------------------------------------------------------------------------------------------- converters
-    // bf16 -> fp16 in place (element-wise on 16-bit lanes, so the 128B swizzle of the TMA boxes is untouched)
+  } else if (warp == 19) {
+    // ------------------------------------------------------------------------------------------- (1) issuer
+    // (1)_c = V^t A_b^t goes to the tensor pipe as soon as the V tile is converted and DY_E is free (the E chain has
+    // read it for chunk c - 1) -- a role of its own, so that neither the converters nor the E chain ever wait for it.
+    if (lane == 0) {
 #pragma unroll 1
-    for (int c = 0; c < nc; ++c) {
-      const int st = c % kS2Stages;
-      s2_wait_warp(&bars->st_full[st], (c / kS2Stages) & 1, abort_flag, lane);
-      S2_STAMPW(16, 3, c, 3);
-      uint4* tile = reinterpret_cast<uint4*>(smem + st * kS2StageBytes + (warp == 16 ? kS2StK : kS2StV));
-      if (!(kCh && warp == 16)) {  // the K~ tile of the per-channel gate arrives as fp16
-#pragma unroll 4
-      for (int it = 0; it < 32; ++it) {
-        uint4 w = tile[it * 32 + lane];
-        w.x = pack_f16(__uint_as_float(w.x << 16), __uint_as_float(w.x & 0xffff0000u));
-        w.y = pack_f16(__uint_as_float(w.y << 16), __uint_as_float(w.y & 0xffff0000u));
-        w.z = pack_f16(__uint_as_float(w.z << 16), __uint_as_float(w.z & 0xffff0000u));
-        w.w = pack_f16(__uint_as_float(w.w << 16), __uint_as_float(w.w & 0xffff0000u));
-        tile[it * 32 + lane] = w;
-      }
-      }
-      fence_proxy_async();
-      __syncwarp();
-      S2_STAMPW(16, 3, c, 4);
-      if (lane == 0) flag_release(&bars->conv_cnt[warp - 16], c + 1);
-      if (warp == 17 && lane == 0) {
-        // (1)_c = V^t A_b^t is issued here, off the E chain's critical path: its V operand was just converted by this
-        // warp, A_b landed with the stage, and DY_E is free once the E chain has read it for chunk c - 1.
-        if (c > 0) s2_wait(&bars->dy_free, (c - 1) & 1, abort_flag);
+      for (int c = 0; c < nc; ++c) {
+        const int st = c % kS2Stages;
+        s2_wait_spin(&bars->st_ready[st], (c / kS2Stages) & 1, abort_flag);
+        if (c > 0) s2_wait_spin(&bars->dy_free, (c - 1) & 1, abort_flag);
         tc_fence_after();
         s2_issue1(tmem, smem_base + st * kS2StageBytes);
         tc_fence_before();
         flag_release(&bars->issued1_cnt, c + 1);
       }
+    }
+  } else if (warp >= 16) {
+    // ------------------------------------------------------------------------------------------- converters
+    // bf16 -> fp16 in place (element-wise on 16-bit lanes, so the 128B swizzle of the TMA boxes is untouched): warp 16
+    // the K tile, warp 17 the V tile.  Rows at or beyond the segment's end belong to the next segment (or lie past the
+    // tensor): they are zeroed, so that nothing of a neighbour -- not even an Inf or NaN -- reaches this unit through
+    // 0 x garbage.  Scalar gate: the V converter also runs the lazy-decay automaton of the E block (s2_chain_sc) and
+    // folds the value weights into the tile.
+    const int role = warp == 16 ? 0 : 1;
+    float p_lazy = 0.f;
+    double g_tot = 0.0;
+    const int seg_len = seg_end - seg_begin;
+#pragma unroll 1
+    for (int c = 0; c < nc; ++c) {
+      const int st = c % kS2Stages;
+      s2_wait_warp(&bars->st_full[st], (c / kS2Stages) & 1, abort_flag, lane);
+      const int valid = min(kC, seg_len - c * kC);
+      const bool weigh = !kCh && role != 0;
+      float* fac = bars->fac[0];
+      if (weigh) {
+        const float* gt = reinterpret_cast<const float*>(smem + st * kS2StageBytes + kS2StGate);  // G_r, inclusive
+        const float GC = gt[kC - 1], g0 = gt[lane], g1 = gt[lane + 32];
+        const bool rs = !(fabsf(p_lazy + GC) <= kLazyP);  // also NaN
+        fac[lane] = rs ? expf(GC - g0) : expf(-(p_lazy + g0));
+        fac[lane + 32] = rs ? expf(GC - g1) : expf(-(p_lazy + g1));
+        if (role == 1 && lane == 0) bars->resc[st] = rs ? expf(p_lazy + GC) : 1.f;
+        p_lazy = rs ? 0.f : p_lazy + GC;
+        g_tot += (double)GC;
+        __syncwarp();
+      }
+      const uint32_t tile = smem_base + st * kS2StageBytes + (role == 0 ? kS2StK : kS2StV) + 16 * lane;
+      const uint32_t fac_s = smem_u32(fac) + 4 * (lane >> 3);
+      if (!(kCh && role == 0)) {  // the K~ tile of the per-channel gate arrives as fp16 (rows past the end are zero)
+        // 16-byte piece it * 32 + lane of a box belongs to token 4 (it % 16) + lane / 8; four pieces in flight per lane
+#pragma unroll 1
+        for (int i0 = 0; i0 < 32; i0 += 4) {
+          uint4 w[4];
+          float f[4];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) w[j] = lds128(tile + 512 * (i0 + j));
+          if (weigh) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) f[j] = lds32f(fac_s + 16 * ((i0 + j) & 15));
+          }
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const int tok = 4 * ((i0 + j) & 15) + (lane >> 3);
+            uint4 o = weigh ? cvt8_bf16_f16(w[j], f[j]) : cvt8_bf16_f16(w[j]);
+            if (tok >= valid) o = make_uint4(0u, 0u, 0u, 0u);
+            sts128(tile + 512 * (i0 + j), o);
+          }
+        }
+      }
+      fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars->st_ready[st]);
       __syncwarp();
     }
+    if (role == 1 && lane == 0) {
+      bars->p_final = p_lazy;
+      bars->g_total = g_tot;
+    }
+    if (role == 1 && lane == 0) flag_release(&bars->fin_flag, 1);
   } else if (warp < 8) {
-    s2_chain<false, kCh>(smem, bars, abort_flag, tmem, warp, lane, nc, E + ((size_t)s * H + h) * kD * kD);
+    if (kCh) s2_chain<false, true>(smem, bars, abort_flag, tmem, warp, lane, nc, E + ((size_t)s * H + h) * kD * kD);
+    else s2_chain_sc<false>(smem, bars, abort_flag, tmem, warp, lane, nc, E + ((size_t)s * H + h) * kD * kD);
   } else {
-    s2_chain<true, kCh>(smem, bars, abort_flag, tmem, warp - 8, lane, nc, T + ((size_t)s * H + h) * kD * kD);
+    if (kCh) s2_chain<true, true>(smem, bars, abort_flag, tmem, warp - 8, lane, nc, T + ((size_t)s * H + h) * kD * kD);
+    else s2_chain_sc<true>(smem, bars, abort_flag, tmem, warp - 8, lane, nc, T + ((size_t)s * H + h) * kD * kD);
   }
   tc_fence_before();
   __syncthreads();
   if (warp == 16) tmem_dealloc(tmem, 512);
+  if (tid == 0 && bars->bad) fb_append(fb, n_units, s * H + h);
 }

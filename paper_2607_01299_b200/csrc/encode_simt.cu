@@ -22,12 +22,12 @@ __device__ __forceinline__ float load_kv(const void* p, size_t idx) {
   return reinterpret_cast<const float*>(p)[idx];
 }
 
+// One (segment s, head h, row block) unit of work; called by both kernels below.
 template <int DK, bool BF16, bool CHANNEL>
-__global__ void __launch_bounds__(kRows) encode_simt_kernel(const void* __restrict__ k, const void* __restrict__ v,
-                                                            const float* __restrict__ g,
-                                                            const float* __restrict__ beta,
-                                                            const int32_t* __restrict__ cu_seqlens, int H, int dv,
-                                                            float* __restrict__ E, float* __restrict__ T) {
+__device__ __forceinline__ void encode_simt_unit(const void* __restrict__ k, const void* __restrict__ v,
+                                                 const float* __restrict__ g, const float* __restrict__ beta,
+                                                 const int32_t* __restrict__ cu_seqlens, int H, int dv,
+                                                 float* __restrict__ E, float* __restrict__ T, int h, int s, int row0) {
   constexpr int AW = CHANNEL ? DK : 1;
   __shared__ __align__(16) float sk[2][kTT][DK];
   __shared__ __align__(16) float sa[2][kTT][AW];
@@ -35,8 +35,6 @@ __global__ void __launch_bounds__(kRows) encode_simt_kernel(const void* __restri
   __shared__ float sb[2][kTT];
 
   const int tid = threadIdx.x;
-  const int h = blockIdx.y, s = blockIdx.z;
-  const int row0 = blockIdx.x * kRows;
   const int row = row0 + tid;  // row of X = [E; T]
   const bool is_e = row < dv;
   const bool live = row < dv + DK;
@@ -158,6 +156,33 @@ __global__ void __launch_bounds__(kRows) encode_simt_kernel(const void* __restri
 }
 
 template <int DK, bool BF16, bool CHANNEL>
+__global__ void __launch_bounds__(kRows) encode_simt_kernel(const void* __restrict__ k, const void* __restrict__ v,
+                                                            const float* __restrict__ g,
+                                                            const float* __restrict__ beta,
+                                                            const int32_t* __restrict__ cu_seqlens, int H, int dv,
+                                                            float* __restrict__ E, float* __restrict__ T) {
+  encode_simt_unit<DK, BF16, CHANNEL>(k, v, g, beta, cu_seqlens, H, dv, E, T, blockIdx.y, blockIdx.z, blockIdx.x * kRows);
+}
+
+// The same work over a device-side list of units: CTA (x, y) takes row block x of list entries y, y + gridDim.y, ...
+// An empty list costs one load per CTA.
+template <int DK, bool BF16, bool CHANNEL>
+__global__ void __launch_bounds__(kRows) encode_simt_list_kernel(const void* __restrict__ k, const void* __restrict__ v,
+                                                                 const float* __restrict__ g,
+                                                                 const float* __restrict__ beta,
+                                                                 const int32_t* __restrict__ cu_seqlens, int H, int dv,
+                                                                 float* __restrict__ E, float* __restrict__ T,
+                                                                 const int32_t* __restrict__ unit_list,
+                                                                 const int32_t* __restrict__ unit_count) {
+  const int n = *unit_count;
+  for (int i = blockIdx.y; i < n; i += gridDim.y) {
+    const int u = unit_list[i];
+    encode_simt_unit<DK, BF16, CHANNEL>(k, v, g, beta, cu_seqlens, H, dv, E, T, u % H, u / H, blockIdx.x * kRows);
+    __syncthreads();  // the staging buffers are reused by the next unit
+  }
+}
+
+template <int DK, bool BF16, bool CHANNEL>
 int launch(const EncodeArgs& a) {
   dim3 grid((a.dv + DK + kRows - 1) / kRows, a.H, a.n_seg);
   encode_simt_kernel<DK, BF16, CHANNEL><<<grid, kRows, 0, a.stream>>>(a.k, a.v, a.g, a.beta, a.cu_seqlens, a.H, a.dv,
@@ -174,7 +199,25 @@ int dispatch(const EncodeArgs& a) {
   return ch ? launch<DK, false, true>(a) : launch<DK, false, false>(a);
 }
 
+template <int DK, bool CHANNEL>
+int launch_list(const EncodeArgs& a, const int32_t* unit_list, const int32_t* unit_count) {
+  const long long units = (long long)a.n_seg * a.H;
+  const dim3 grid((a.dv + DK + kRows - 1) / kRows, (unsigned)(units < 296 ? units : 296));
+  encode_simt_list_kernel<DK, true, CHANNEL><<<grid, kRows, 0, a.stream>>>(a.k, a.v, a.g, a.beta, a.cu_seqlens, a.H, a.dv,
+                                                                          a.E, a.T, unit_list, unit_count);
+  note_launch();
+  HYPIC_CUDA_OK(cudaGetLastError());
+  return HYPIC_OK;
+}
+
 }  // namespace
+
+int encode_simt_list(const EncodeArgs& a, const int32_t* unit_list, const int32_t* unit_count) {
+  if (a.dk != 128 || a.kv_dtype != HYPIC_DT_BF16) return HYPIC_ERR_UNSUPPORTED;  // the tensor family's shapes
+  if (a.n_seg == 0) return HYPIC_OK;
+  return a.gate == HYPIC_GATE_CHANNEL ? launch_list<128, true>(a, unit_list, unit_count)
+                                      : launch_list<128, false>(a, unit_list, unit_count);
+}
 
 int encode_simt(const EncodeArgs& a) {
   if (a.H > 65535 || a.n_seg > 65535) return HYPIC_ERR_UNSUPPORTED;

@@ -40,10 +40,16 @@ constexpr int kGateFloatsCh = 144;       // Gamma_C[128], pad (576 B = 36 x 16 B
 constexpr int kGateBytesCh = kGateFloatsCh * 4;
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
-// workspace: chunk_off int32[n_seg + 1], seg_order int32[n_seg] | chunk_meta int2[cap] | records [cap][H][kRecBytes] | gate [cap][H][kGateFloats]
+// workspace: chunk_off int32[n_seg + 1], seg_order int32[n_seg] | fallback list int32[4 + 2 n_seg H] | chunk_meta int2[cap] |
+//            records [cap][H][kRecBytes] | gate [cap][H][kGateFloats]
 __host__ __device__ inline size_t chunk_cap(int32_t n_seg, int32_t t_total) { return (size_t)t_total / kC + n_seg; }
-__host__ __device__ inline size_t ws_off_meta(int32_t n_seg) { return align_up(8 * ((size_t)n_seg + 1), 1024); }
-__host__ __device__ inline size_t ws_off_rec(int32_t n_seg, size_t cap) { return ws_off_meta(n_seg) + align_up(8 * cap, 1024); }
+__host__ __device__ inline size_t ws_off_fb(int32_t n_seg) { return align_up(8 * ((size_t)n_seg + 1), 1024); }
+__host__ __device__ inline size_t ws_off_meta(int32_t n_seg, int32_t H) {
+  return ws_off_fb(n_seg) + align_up(4 * (4 + 2 * (size_t)n_seg * H), 1024);
+}
+__host__ __device__ inline size_t ws_off_rec(int32_t n_seg, int32_t H, size_t cap) {
+  return ws_off_meta(n_seg, H) + align_up(8 * cap, 1024);
+}
 
 // ------------------------------------------------------------------------------------------------ K0
 // chunk_meta[x] = (first token, number of valid tokens) of global chunk x, (0, 0) for the unused tail of the table:
@@ -51,9 +57,11 @@ __host__ __device__ inline size_t ws_off_rec(int32_t n_seg, size_t cap) { return
 // seg_order = the segments by decreasing length (the paper's LPT rule, used here as the launch order of
 // the scan CTAs so that the longest sequential scans start first); identity beyond 8192 segments.
 __global__ void chunk_offsets_kernel(const int32_t* __restrict__ cu_seqlens, int n_seg, int32_t* __restrict__ chunk_off,
-                                     int32_t* __restrict__ seg_order, int2* __restrict__ chunk_meta, int cap) {
+                                     int32_t* __restrict__ seg_order, int2* __restrict__ chunk_meta, int cap,
+                                     int32_t* __restrict__ fb, long long n_units) {
   __shared__ int part[1024];
   const int tid = threadIdx.x;
+  for (long long i = tid; i < 4 + n_units; i += 1024) fb[i] = 0;  // empty fallback list, no unit flagged
   const int per = (n_seg + 1023) / 1024;
   const int lo = min(n_seg, tid * per), hi = min(n_seg, lo + per);
   int sum = 0;
@@ -99,6 +107,12 @@ __global__ void chunk_offsets_kernel(const int32_t* __restrict__ cu_seqlens, int
 // ------------------------------------------------------------------------------------------------ K1, K2
 __device__ unsigned int g_timeout_count_enc = 0;
 __device__ unsigned int g_envelope_count_enc = 0;  // (chunk, head) pairs outside the fp16 envelope (hypic.h)
+
+// The fallback list of a call (workspace): fb[0] = count, fb[4 .. 4 + n_units) = per-unit flags, then the list.  A unit
+// (segment s, head h -> s H + h) is appended once; encode_simt's list kernel recomputes it in fp32 after the scan.
+__device__ __forceinline__ void fb_append(int32_t* fb, int n_units, int unit) {
+  if (atomicExch(&fb[4 + unit], 1) == 0) fb[4 + n_units + atomicAdd(&fb[0], 1)] = unit;
+}
 
 #include "encode_prep.cuh"
 
@@ -153,13 +167,13 @@ size_t encode_tensor_workspace(int32_t n_seg, int32_t t_total, int32_t H, int32_
   if (!encode_tensor_shape_ok(H, dk, dv, kv_dtype, gate)) return 0;
   const size_t cap = chunk_cap(n_seg, t_total);
   const bool ch = gate == HYPIC_GATE_CHANNEL;
-  return ws_off_rec(n_seg, cap) + cap * H * ((size_t)(ch ? kRecBytesCh : kRecBytes) + (ch ? kGateBytesCh : kGateBytes));
+  return ws_off_rec(n_seg, H, cap) + cap * H * ((size_t)(ch ? kRecBytesCh : kRecBytes) + (ch ? kGateBytesCh : kGateBytes));
 }
 
 int encode_tensor(const EncodeArgs& a) {
   if (!encode_tensor_supported(a)) return HYPIC_ERR_UNSUPPORTED;
   if (a.n_seg == 0) return HYPIC_OK;
-  if (a.H > 65535 || a.n_seg > 65535) return HYPIC_ERR_UNSUPPORTED;
+  if (a.H > 65535 || a.n_seg > 65535 || (long long)a.H * a.n_seg > 0x3fffffffLL) return HYPIC_ERR_UNSUPPORTED;
   const size_t cap = chunk_cap(a.n_seg, a.t_total);
   if (cap > 0x7fffffffULL) return HYPIC_ERR_UNSUPPORTED;
   if (a.t_total == 0) {
@@ -171,8 +185,10 @@ int encode_tensor(const EncodeArgs& a) {
   uint8_t* ws = static_cast<uint8_t*>(a.workspace);
   int32_t* chunk_off = reinterpret_cast<int32_t*>(ws);
   int32_t* seg_order = chunk_off + a.n_seg + 1;
-  int2* chunk_meta = reinterpret_cast<int2*>(ws + ws_off_meta(a.n_seg));
-  uint8_t* rec = ws + ws_off_rec(a.n_seg, cap);
+  int32_t* fb = reinterpret_cast<int32_t*>(ws + ws_off_fb(a.n_seg));
+  const int n_units = a.n_seg * a.H;
+  int2* chunk_meta = reinterpret_cast<int2*>(ws + ws_off_meta(a.n_seg, a.H));
+  uint8_t* rec = ws + ws_off_rec(a.n_seg, a.H, cap);
   const bool ch = a.gate == HYPIC_GATE_CHANNEL;
   float* gate = reinterpret_cast<float*>(rec + cap * a.H * (size_t)(ch ? kRecBytesCh : kRecBytes));
   static bool configured = false;
@@ -186,21 +202,29 @@ int encode_tensor(const EncodeArgs& a) {
   int rc = make_kv_tensor_map(&tmK, a.k, a.t_total, a.H);
   if (rc == HYPIC_OK) rc = make_kv_tensor_map(&tmV, a.v, a.t_total, a.H);
   if (rc != HYPIC_OK) return rc;
-  chunk_offsets_kernel<<<1, 1024, 0, a.stream>>>(a.cu_seqlens, a.n_seg, chunk_off, seg_order, chunk_meta, (int)cap);
+  chunk_offsets_kernel<<<1, 1024, 0, a.stream>>>(a.cu_seqlens, a.n_seg, chunk_off, seg_order, chunk_meta, (int)cap, fb,
+                                                 (long long)n_units);
   note_launch();
   const dim3 pgrid((unsigned)((cap + kPrepChunksPerCta - 1) / kPrepChunksPerCta), a.H), sgrid(a.H, a.n_seg);
   if (ch) {
-    prep_kernel<true><<<pgrid, kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, chunk_meta, (int)cap, a.H, rec, gate);
+    prep_kernel<true><<<pgrid, kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, chunk_meta, (int)cap, a.H, rec, gate, chunk_off,
+                                                            a.n_seg, fb);
     note_launch();
-    scan2_kernel<true><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, seg_order, a.H, rec, gate, a.E, a.T);
+    scan2_kernel<true><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, seg_order, a.H, rec, gate,
+                                                                 a.E, a.T, fb, n_units);
   } else {
-    prep_kernel<false><<<pgrid, kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, chunk_meta, (int)cap, a.H, rec, gate);
+    prep_kernel<false><<<pgrid, kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, chunk_meta, (int)cap, a.H, rec, gate, chunk_off,
+                                                             a.n_seg, fb);
     note_launch();
-    scan2_kernel<false><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, seg_order, a.H, rec, gate, a.E, a.T);
+    scan2_kernel<false><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, seg_order, a.H, rec, gate,
+                                                                  a.E, a.T, fb, n_units);
   }
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());
-  return HYPIC_OK;
+  // Units the fp16 operands could not carry (a per-channel chunk decaying below e^-9, an operand beyond 65504, ...)
+  // were put on the call's fallback list by the kernels above: the fp32 family recomputes exactly those, in the same
+  // call and on the same stream, with a device-side list -- no work (a few idle CTAs) when the list is empty.
+  return encode_simt_list(a, fb + 4 + n_units, fb);
 }
 
 bool diag_encode_tensor_shape_ok(int32_t, int32_t dk, int32_t dv, int kv_dtype, int gate) {
@@ -245,12 +269,6 @@ int diag_encode_tensor(const DiagEncodeArgs& a) {
   HYPIC_CUDA_OK(cudaGetLastError());
   return HYPIC_OK;
 }
-
-#ifdef HYPIC_TIMELINE
-extern "C" int hypic_debug_timeline(long long* out, int n) {
-  return cudaMemcpyFromSymbol(out, g_s2_timeline, sizeof(long long) * (size_t)n) == cudaSuccess ? 0 : 1;
-}
-#endif
 
 unsigned int envelope_violation_count_encode() {
   unsigned int v = 0;

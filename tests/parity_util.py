@@ -66,6 +66,23 @@ def oracle_encode_units(inp, units):
     return np.stack(Es)[:, None], np.stack(Ts)[:, None]
 
 
+def oracle_encode_units_batched(inp, units):
+    """As oracle_encode_units, but the sampled units go to the oracle in ONE call (packed as len(units) one-head
+    segments), so that its OpenMP loop over independent units uses every host core: [n,1,dv,dk], [n,1,dk,dk]."""
+    cu = np.concatenate([[0], np.cumsum(inp.seg_lens)]).astype(np.int64)
+    ks, vs, gs, bs, lens = [], [], [], [], []
+    for s, h in units:
+        sl = slice(int(cu[s]), int(cu[s + 1]))
+        ks.append(inp.k[sl, h:h + 1].cpu())
+        vs.append(inp.v[sl, h:h + 1].cpu())
+        gs.append(inp.g[sl, h:h + 1].cpu())
+        bs.append(inp.beta[sl, h:h + 1].cpu())
+        lens.append(int(cu[s + 1] - cu[s]))
+    cu_u = torch.tensor(np.concatenate([[0], np.cumsum(lens)]), dtype=torch.int32)
+    E, T = oracle.segment_encode(torch.cat(ks), torch.cat(vs), torch.cat(gs), torch.cat(bs), cu_u, gate=inp.gate)
+    return E, T
+
+
 def oracle_compose_units(S_in, E_pool, T_pool, seg_ids, cu_segs, units):
     """Oracle composed state for sampled (request, head) units of a large compose problem: [n,1,dv,dk]."""
     ids_all = seg_ids.cpu().numpy()

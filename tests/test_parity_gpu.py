@@ -11,7 +11,7 @@ import oracle
 from paper_2607_01299_b200 import binding as hb
 from paper_2607_01299_b200 import workloads as wl
 from parity_util import (TOL_BF16, TOL_F32, check_E, check_T, oracle_compose_units, oracle_encode,
-                         oracle_encode_units)
+                         oracle_encode_units, oracle_encode_units_batched)
 
 pytestmark = pytest.mark.gpu
 
@@ -226,29 +226,32 @@ def test_cfg1_full_size():
     check_E(S, ref_e2e, TOL_BF16, "S_out end to end")
 
 
-def test_cfg2_one_layer_sampled_units():
-    """cfg2, one of the 36 layers at full size (20 x 4096, H=32): sampled (segment, head) units one by one."""
+def _compose_all_heads_ref(S_in, E, T, ids, cu):
+    """fp64 compose of the same fp32 pools, every (request, head) chain, in one oracle call."""
+    return oracle.compose(None if S_in is None else S_in.cpu().numpy(), E.cpu().numpy(), T.cpu().numpy(),
+                          ids.cpu().numpy(), cu.cpu().numpy())
+
+
+def test_cfg2_one_layer_every_unit():
+    """cfg2, one of the 36 layers at full size (20 x 4096, H=32): EVERY one of the 640 (segment, head) units against the
+    oracle (a tail-wave or head-boundary bug that hits one unit in fifty cannot hide behind a sample), then the
+    composition of the 20 segments for every head."""
     inp = wl.cfg2_layer(0, "cuda")
     E, T = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
-    units = _sample_units(20, 32, 6, 2)
-    E_ref, T_ref = oracle_encode_units(inp, units)
-    sel_s = torch.tensor([u[0] for u in units]), torch.tensor([u[1] for u in units])
-    check_E(E[sel_s[0], sel_s[1]][:, None], E_ref, TOL_BF16)
-    check_T(T[sel_s[0], sel_s[1]][:, None], T_ref, TOL_BF16)  # 4096 tokens: T underflows -> absolute criterion
-    assert torch.isfinite(E).all() and torch.isfinite(T).all()
-    # compose the 20 segments per head, sampled heads, vs fp64 compose of the same fp32 pools
+    E_ref, T_ref = oracle_encode(inp)
+    check_E(E, E_ref, TOL_BF16)
+    check_T(T, T_ref, TOL_BF16)  # 4096 tokens: T underflows -> absolute criterion
     ids = torch.arange(20, dtype=torch.int32, device="cuda")
     cu = torch.tensor([0, 20], dtype=torch.int32, device="cuda")
     S = gpu_compose(None, E, T, ids, cu, hb.HYPIC_IMPL_AUTO)
-    heads = [(0, h) for h in (0, 13, 31)]
-    ref = oracle_compose_units(None, E, T, ids, cu, heads)
-    check_E(S[0, [0, 13, 31]][:, None], ref, TOL_F32, "S_out")
+    check_E(S, _compose_all_heads_ref(None, E, T, ids, cu), TOL_F32, "S_out")
+    check_E(S, oracle.compose(None, E_ref, T_ref, ids.cpu().numpy(), cu.cpu().numpy()), TOL_BF16, "S_out end to end")
 
 
-def test_cfg2_folded_layers_launch_configuration():
+def test_cfg2_folded_layers_launch_configuration_every_unit():
     """cfg2 in the launch configuration bench.py times: 4 independent layers folded into the head axis (H = 128,
     SURVEY.md 8(b)), full size (20 x 4096).  The folded call must reproduce the per-layer calls bit for bit (units
-    are independent), sampled units are checked against the oracle, and so is the folded composition."""
+    are independent), ALL 2,560 units are checked against the oracle, and so is the folded composition of every head."""
     layers = [wl.cfg2_layer(l, "cuda") for l in range(4)]
     inp = wl.fold_layers(layers)
     E, T = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
@@ -257,48 +260,41 @@ def test_cfg2_folded_layers_launch_configuration():
         assert torch.equal(E[:, 32 * l:32 * l + 32], E1) and torch.equal(T[:, 32 * l:32 * l + 32], T1)
         del E1, T1
     del layers
-    units = [(0, 0), (19, 127)] + _sample_units(20, 128, 4, 5)
-    E_ref, T_ref = oracle_encode_units(inp, units)
-    si, hi = torch.tensor([u[0] for u in units]), torch.tensor([u[1] for u in units])
-    check_E(E[si, hi][:, None], E_ref, TOL_BF16)
-    check_T(T[si, hi][:, None], T_ref, TOL_BF16)
-    assert torch.isfinite(E).all() and torch.isfinite(T).all()
+    E_ref, T_ref = oracle_encode(inp)
+    check_E(E, E_ref, TOL_BF16)
+    check_T(T, T_ref, TOL_BF16)
+    del E_ref, T_ref
     ids = torch.arange(20, dtype=torch.int32, device="cuda")
     cu = torch.tensor([0, 20], dtype=torch.int32, device="cuda")
     S = gpu_compose(None, E, T, ids, cu, hb.HYPIC_IMPL_AUTO)
-    hs = [0, 45, 96, 127]
-    ref = oracle_compose_units(None, E, T, ids, cu, [(0, h) for h in hs])
-    check_E(S[0, hs][:, None], ref, TOL_F32, "S_out (folded)")
+    check_E(S, _compose_all_heads_ref(None, E, T, ids, cu), TOL_F32, "S_out (folded)")
 
 
-def test_cfg3_varlen_channel_gate_sampled_units():
-    """cfg3 (64 varlen segments, per-channel gate) at a reduced head count to bound memory; sampled units
-    including the shortest and the longest segment."""
-    inp = wl.cfg3("cuda", H=4)
+def test_cfg3_varlen_channel_gate_full_head_count():
+    """cfg3 exactly as bench.py times it (64 varlen segments, per-channel gate, H = 32): the shortest and the longest
+    segment plus 34 sampled (segment, head) units, one oracle call over all of them."""
+    inp = wl.cfg3("cuda")
     E, T = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
+    assert torch.isfinite(E).all() and torch.isfinite(T).all()
     lens = inp.seg_lens
-    units = [(int(np.argmin(lens)), 1), (int(np.argmax(lens)), 2)] + _sample_units(64, 4, 3, 3)
-    E_ref, T_ref = oracle_encode_units(inp, units)
+    units = [(int(np.argmin(lens)), 1), (int(np.argmin(lens)), 31), (int(np.argmax(lens)), 2), (int(np.argmax(lens)), 30)]
+    units += [u for u in _sample_units(64, 32, 34, 3) if u not in units]
+    E_ref, T_ref = oracle_encode_units_batched(inp, units)
     si, hi = torch.tensor([u[0] for u in units]), torch.tensor([u[1] for u in units])
     check_E(E[si, hi][:, None], E_ref, TOL_BF16)
     check_T(T[si, hi][:, None], T_ref, TOL_BF16)
-    assert torch.isfinite(E).all() and torch.isfinite(T).all()
 
 
-def test_cfg4_compose_stress_sampled_requests():
-    """cfg4 at full size for one layer-iteration (P=1024, H=32, R=128, n_r ~ U{16..64}): sampled (request,
-    head) chains against the fp64 compose of the same fp32 pools."""
+def test_cfg4_compose_stress_every_chain():
+    """cfg4 at full size for one layer-iteration (P=1024, H=32, R=128, n_r ~ U{16..64}): ALL 4,096 (request, head)
+    chains against the fp64 compose of the same fp32 pools."""
     pin = wl.cfg4_pool_inputs(device="cuda")
     _, T = gpu_encode(pin, hb.HYPIC_IMPL_AUTO)
     del pin
     E = wl.cfg4_pool_E(device="cuda")
     req = wl.cfg4_requests(device="cuda")
     S = gpu_compose(req.S_in, E, T, req.seg_ids, req.cu_segs, hb.HYPIC_IMPL_AUTO)
-    assert torch.isfinite(S).all()
-    units = _sample_units(128, 32, 8, 4)
-    ref = oracle_compose_units(req.S_in, E, T, req.seg_ids, req.cu_segs, units)
-    ri, hi = torch.tensor([u[0] for u in units]), torch.tensor([u[1] for u in units])
-    check_E(S[ri, hi][:, None], ref, TOL_F32, "S_out")
+    check_E(S, _compose_all_heads_ref(req.S_in, E, T, req.seg_ids, req.cu_segs), TOL_F32, "S_out")
 
 
 # ------------------------------------------------- tensor family: range handling of the fp16 operands
@@ -330,18 +326,70 @@ def test_tensor_family_operand_range(case):
     assert hb.hypic_envelope_violation_count() == before
 
 
-def test_tensor_family_envelope_guard():
-    """g ~ U(-1, 0): the cumulative log-decay of a chunk (~ -32) is far outside the fp16 envelope of the tensor family
-    (hypic.h); its prep kernel must count the violation, and the SIMT family must still match the oracle."""
-    inp = wl.make_encode_inputs([130, 64], 2, 128, 128, kv_dtype=torch.bfloat16, g_lo=-1.0, seed=wl.seed_for(1, 32),
-                                device="cuda")
-    before = hb.hypic_envelope_violation_count()
-    gpu_encode(inp, hb.HYPIC_IMPL_TENSOR)
-    assert hb.hypic_envelope_violation_count() > before
-    E, T = gpu_encode(inp, hb.HYPIC_IMPL_SIMT)
+@pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
+@pytest.mark.parametrize("g_lo", [-1.0, -0.3])
+def test_auto_meets_tolerance_for_any_gate_strength(gate, g_lo):
+    """Table 1's gates are data-dependent with no range given.  g ~ U(-1, 0) puts the log-decay of a
+    64-token chunk near -32, g ~ U(-0.3, 0) near -10.  AUTO (what a caller gets by default) must meet the bf16
+    tolerance with no caller action: the scalar gate never enters the fp16 algebra, a per-channel
+    chunk below e^-9 sends its unit to the fp32 family inside the same call (device-side fallback list)."""
+    inp = wl.make_encode_inputs([700, 130, 64, 1], 3, 128, 128, kv_dtype=torch.bfloat16, gate=gate, g_lo=g_lo,
+                                seed=wl.seed_for(1, 32), device="cuda")
+    E, T = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
     E_ref, T_ref = oracle_encode(inp)
     check_E(E, E_ref, TOL_BF16)
     check_T(T, T_ref, TOL_BF16)
+
+
+def test_fallback_list_takes_only_the_units_that_need_it():
+    """Per-channel gate, one (segment, head) with one strongly decaying channel range: that unit alone leaves the fp16
+    envelope.  Every unit must match the oracle, and the units inside the envelope must be bit-identical to a call
+    without the outlier (they stay on the tcgen05 path)."""
+    inp = wl.make_encode_inputs([256, 300, 128], 4, 128, 128, kv_dtype=torch.bfloat16, gate=wl.GATE_CHANNEL,
+                                seed=wl.seed_for(3, 33), device="cuda")
+    E0, T0 = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
+    before = hb.hypic_envelope_violation_count()
+    inp.g[256 + 70:256 + 200, 2, 5:9] = -0.4  # segment 1, head 2: chunks 1 and 2 decay to e^-25 in four channels
+    E, T = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
+    assert hb.hypic_envelope_violation_count() > before
+    E_ref, T_ref = oracle_encode(inp)
+    check_E(E, E_ref, TOL_BF16)
+    check_T(T, T_ref, TOL_BF16)
+    keep = torch.ones(3, 4, dtype=torch.bool)
+    keep[1, 2] = False
+    assert torch.equal(E[keep], E0[keep]) and torch.equal(T[keep], T0[keep])
+    assert not torch.equal(E[1, 2], E0[1, 2])
+
+
+@pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
+def test_fp16_operand_overflow_falls_back_in_call(gate):
+    """|v| up to ~5e4: the weighted values leave fp16's range inside the tensor family, the result would hold Inf / NaN;
+    the unit must come back from the fp32 family instead, within tolerance."""
+    inp = wl.make_encode_inputs([200, 64], 2, 128, 128, kv_dtype=torch.bfloat16, gate=gate, seed=wl.seed_for(1, 34),
+                                device="cuda")
+    inp.v.mul_(1.0e4)
+    E, T = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
+    E_ref, T_ref = oracle_encode(inp)
+    check_E(E, E_ref, TOL_BF16)
+    check_T(T, T_ref, TOL_BF16)
+
+
+@pytest.mark.parametrize("gate", [wl.GATE_SCALAR, wl.GATE_CHANNEL])
+def test_neighbour_segment_cannot_poison_a_ragged_tail(gate):
+    """The TMA boxes of a segment's last chunk also hold the first tokens of the next segment.  Inf / NaN planted
+    there must not reach this segment (0 x Inf = NaN): its E and T still match the oracle."""
+    inp = wl.make_encode_inputs([100, 64, 30], 2, 128, 128, kv_dtype=torch.bfloat16, gate=gate, seed=wl.seed_for(1, 35),
+                                device="cuda")
+    ref = wl.make_encode_inputs([100, 64, 30], 2, 128, 128, kv_dtype=torch.bfloat16, gate=gate, seed=wl.seed_for(1, 35),
+                                device="cuda")
+    inp.k[100:164] = float("inf")
+    inp.v[100:164] = float("nan")
+    E, T = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
+    E_ref, T_ref = oracle_encode(ref)
+    for s in (0, 2):
+        check_E(E[s:s + 1], E_ref[s:s + 1], TOL_BF16)
+        check_T(T[s:s + 1], T_ref[s:s + 1], TOL_BF16)
+    assert not torch.isfinite(E[1]).all()  # the poisoned segment itself is non-finite on both sides
 
 
 # ------------------------------------------------------------- fp16-stored tuples (SURVEY.md 8(f) NEXT-1)
@@ -447,6 +495,14 @@ def _check_o(o_gpu, o_ref, cu, tol, typical=None):
         den = np.maximum(den, typical[inside])
     worst = float((num / np.maximum(den, 1e-300)).max()) if inside.any() else 0.0
     assert worst <= tol, f"o: max per-token rel. L2 error {worst:.3e} > {tol:.1e}"
+    if typical is not None and inside.any():
+        # rows whose read-out is not a cancellation (||o_ref|| at least the general-position size) must also meet the
+        # PLAIN relative bound, so that a regression in well-conditioned rows cannot hide behind the W2 denominator
+        plain = np.sqrt((o_ref[inside] ** 2).sum(-1))
+        good = plain >= typical[inside]
+        if good.any():
+            worst_plain = float((num[good] / np.maximum(plain[good], 1e-300)).max())
+            assert worst_plain <= tol, f"o: max plain rel. L2 error on well-conditioned rows {worst_plain:.3e} > {tol:.1e}"
     assert np.all(o_gpu[~inside] == 0.0), "o rows outside every window must be left untouched"
     return worst
 
@@ -907,6 +963,27 @@ def test_forward_encode_vs_oracle(gate, kv, d, dv):
         E2, T2 = hb.hypic_segment_encode(e.k, e.v, e.g, e.beta, e.cu_seqlens, e.gate)
         check_E(E2, E.cpu().numpy(), TOL_BF16, "E (tensor family vs forward-encode)")
         check_T(T2, T.cpu().numpy(), TOL_BF16, "T (tensor family vs forward-encode)")
+
+
+def test_forward_encode_bench_size_sampled_units():
+    """hypic_forward_encode in the launch bench.py times (20 x 4096 tokens, H = 32, bf16 q/k/v): sampled (segment, head)
+    units, o against oracle.seam_window from the zero state, (E, T) against oracle.segment_encode."""
+    si = wl.make_seam_inputs([4096] * 20, 32, 128, 128, kv_dtype=torch.bfloat16, seed=wl.seed_for(7, 0), device="cuda")
+    e = si.enc
+    o, E, T = hb.hypic_forward_encode(si.q, e.k, e.v, e.g, e.beta, e.cu_seqlens, e.gate)
+    torch.cuda.synchronize()
+    assert torch.isfinite(o).all() and torch.isfinite(E).all() and torch.isfinite(T).all()
+    tol = TOL_F32  # fp32 arithmetic on both q/k/v dtypes
+    for s, h in [(0, 0), (19, 31)] + _sample_units(20, 32, 6, 11):
+        sl = slice(4096 * s, 4096 * (s + 1))
+        f = lambda t: t[sl, h:h + 1].float().cpu().numpy()
+        cu1 = np.array([0, 4096], dtype=np.int32)
+        S_ref, o_ref = oracle.seam_window(None, f(si.q), f(e.k), f(e.v), f(e.g), f(e.beta), cu1, gate=e.gate)
+        u = e.unit(s, h)
+        E_ref, T_ref = oracle.segment_encode(u.k, u.v, u.g, u.beta, u.cu_seqlens, gate=u.gate)
+        check_E(E[s:s + 1, h:h + 1], E_ref, tol, "E (forward-encode)")
+        check_T(T[s:s + 1, h:h + 1], T_ref, tol, "T (forward-encode)")
+        _check_o(o[sl, h:h + 1], o_ref, cu1, tol, _typical_readout(None, f(si.q), f(e.k), f(e.v), f(e.g), f(e.beta), cu1, e.gate))
 
 
 def test_compose_interleaved_heads_every_unit():
