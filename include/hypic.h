@@ -280,6 +280,12 @@ int hypic_version(void);
  */
 int hypic_last_launch_count(void);
 
+/*
+ * hypic_last_cuda_error: the cudaError_t value behind the most recent HYPIC_ERR_CUDA returned on this thread
+ * (0 = none since load).  Pure host bookkeeping; diagnostics only.
+ */
+int hypic_last_cuda_error(void);
+
 #ifdef __cplusplus
 }
 #endif

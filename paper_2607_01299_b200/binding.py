@@ -27,7 +27,7 @@ HYPIC_IMPL_TENSOR = 2
 
 EXPORTS = (
     "hypic_set_impl", "hypic_get_impl", "hypic_segment_encode_workspace", "hypic_segment_encode", "hypic_compose",
-    "hypic_status_string", "hypic_version", "hypic_last_launch_count", "hypic_encode_impl_for",
+    "hypic_status_string", "hypic_version", "hypic_last_launch_count", "hypic_last_cuda_error", "hypic_encode_impl_for",
     "hypic_compose_impl_for", "hypic_debug_timeout_count", "hypic_envelope_violation_count", "hypic_compose_f16",
     "hypic_tuple_pack_f16", "hypic_seam_window", "hypic_diag_encode", "hypic_diag_compose",
     "hypic_diag_encode_impl_for", "hypic_diag_compose_f16", "hypic_forward_encode", "hypic_rope_compose_workspace",
@@ -42,7 +42,10 @@ _lib = None
 class HypicError(RuntimeError):
     def __init__(self, status: int, where: str):
         self.status = int(status)
-        super().__init__(f"{where} failed: status {status} ({hypic_status_string(status)})")
+        extra = ""
+        if self.status == HYPIC_ERR_CUDA and _lib is not None:
+            extra = f", cudaError {int(_lib.hypic_last_cuda_error())}"
+        super().__init__(f"{where} failed: status {status} ({hypic_status_string(status)}{extra})")
 
 
 def load_library() -> ctypes.CDLL:
@@ -96,6 +99,8 @@ def load_library() -> ctypes.CDLL:
     lib.hypic_version.restype = ctypes.c_int
     lib.hypic_last_launch_count.argtypes = []
     lib.hypic_last_launch_count.restype = ctypes.c_int
+    lib.hypic_last_cuda_error.argtypes = []
+    lib.hypic_last_cuda_error.restype = ctypes.c_int
     lib.hypic_encode_impl_for.argtypes = [i32, i32, i32, ctypes.c_int, ctypes.c_int]
     lib.hypic_encode_impl_for.restype = ctypes.c_int
     lib.hypic_compose_impl_for.argtypes = [i32, i32, i32]

@@ -12,10 +12,16 @@ namespace hypic {
 extern thread_local int g_launch_count;
 inline void note_launch(int n = 1) { g_launch_count += n; }
 
+// The CUDA error behind the most recent HYPIC_ERR_CUDA of this thread (hypic_last_cuda_error()).
+extern thread_local int g_last_cuda_error;
+
 #define HYPIC_CUDA_OK(expr)                        \
   do {                                             \
     cudaError_t _e = (expr);                       \
-    if (_e != cudaSuccess) return HYPIC_ERR_CUDA;  \
+    if (_e != cudaSuccess) {                       \
+      g_last_cuda_error = (int)_e;                 \
+      return HYPIC_ERR_CUDA;                       \
+    }                                              \
   } while (0)
 
 struct EncodeArgs {

@@ -86,8 +86,8 @@ __device__ __noinline__ bool s2_wait(uint64_t* bar, uint32_t parity, volatile in
 // that has gone into s2_wait's __nanosleep loop wakes up thousands of cycles after its barrier completed
 __device__ __forceinline__ void s2_wait_spin(uint64_t* bar, uint32_t parity, volatile int* abort_flag) {
 #pragma unroll 1
-  for (int i = 0; i < 8192; ++i)
-    if (mbar_try_wait(bar, parity)) return;
+  for (int i = 0; i < 256; ++i)
+    if (mbar_try_wait_hint(bar, parity, 20000u)) return;  // suspended in hardware until the phase completes (or 20 us)
   s2_wait(bar, parity, abort_flag);
 }
 

@@ -118,6 +118,8 @@ __device__ __forceinline__ void fb_append(int32_t* fb, int n_units, int unit) {
 
 #include "encode_scan2.cuh"
 
+#include "encode_scan3.cuh"
+
 #include "diag_scan.cuh"
 
 // k / v viewed as 3-D bf16 tensors [t_total][H][128]; box = 64 elements (128 B) x 1 head x 64 tokens, 128B swizzle:
@@ -166,8 +168,9 @@ size_t encode_tensor_workspace(int32_t n_seg, int32_t t_total, int32_t H, int32_
                                int gate) {
   if (!encode_tensor_shape_ok(H, dk, dv, kv_dtype, gate)) return 0;
   const size_t cap = chunk_cap(n_seg, t_total);
-  const bool ch = gate == HYPIC_GATE_CHANNEL;
-  return ws_off_rec(n_seg, H, cap) + cap * H * ((size_t)(ch ? kRecBytesCh : kRecBytes) + (ch ? kGateBytesCh : kGateBytes));
+  // scalar gate: one fused kernel, nothing but the chunk tables and the fallback list; per-channel gate: prep records
+  if (gate != HYPIC_GATE_CHANNEL) return ws_off_rec(n_seg, H, cap);
+  return ws_off_rec(n_seg, H, cap) + cap * H * ((size_t)kRecBytesCh + kGateBytesCh);
 }
 
 int encode_tensor(const EncodeArgs& a) {
@@ -193,7 +196,7 @@ int encode_tensor(const EncodeArgs& a) {
   float* gate = reinterpret_cast<float*>(rec + cap * a.H * (size_t)(ch ? kRecBytesCh : kRecBytes));
   static bool configured = false;
   if (!configured) {
-    HYPIC_CUDA_OK(cudaFuncSetAttribute(scan2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kS2Smem));
+    HYPIC_CUDA_OK(cudaFuncSetAttribute(scan3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kF_Smem));
     HYPIC_CUDA_OK(cudaFuncSetAttribute(scan2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kS2Smem));
     configured = true;
   }
@@ -213,11 +216,8 @@ int encode_tensor(const EncodeArgs& a) {
     scan2_kernel<true><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, seg_order, a.H, rec, gate,
                                                                  a.E, a.T, fb, n_units);
   } else {
-    prep_kernel<false><<<pgrid, kPrepThreads, 0, a.stream>>>(kp, a.g, a.beta, chunk_meta, (int)cap, a.H, rec, gate, chunk_off,
-                                                             a.n_seg, fb);
-    note_launch();
-    scan2_kernel<false><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, seg_order, a.H, rec, gate,
-                                                                  a.E, a.T, fb, n_units);
+    scan3_kernel<<<sgrid, kF_Threads, kF_Smem, a.stream>>>(tmK, tmV, a.g, a.beta, a.cu_seqlens, seg_order, a.H, a.E, a.T, fb,
+                                                           n_units);
   }
   note_launch();
   HYPIC_CUDA_OK(cudaGetLastError());

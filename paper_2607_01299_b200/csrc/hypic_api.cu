@@ -7,6 +7,7 @@
 namespace hypic {
 
 thread_local int g_launch_count = 0;
+thread_local int g_last_cuda_error = 0;
 static std::atomic<int> g_impl{HYPIC_IMPL_AUTO};
 
 const DeviceInfo& device_info() {
@@ -297,5 +298,7 @@ unsigned int hypic_debug_timeout_count(void) { return debug_timeout_count(); }
 unsigned int hypic_envelope_violation_count(void) { return envelope_violation_count_encode(); }
 
 int hypic_last_launch_count(void) { return g_launch_count; }
+
+int hypic_last_cuda_error(void) { return g_last_cuda_error; }
 
 }  // extern "C"
