@@ -33,7 +33,7 @@
 //   warp 0       loader     TMA boxes of K (4-deep ring, two chunks ahead of V) and V (2-deep ring)
 //   warp 1       gate       the chunk's g / beta, its cumulative log-decay and the lazy-decay automaton (a ring of 8
 //                           gate records)
-//   warp 2       (1) issuer (also zeroes the rows of a ragged last V tile that belong to the next segment)
+//   warp 2       V helper   zeroes the rows of a ragged last V tile that belong to the next segment, releases V to (1)
 //   warps 3-6    E chain    thread = row of E: pass Xh = fp16(X) (and the lazy rescale), epilogue U'' = fp16(DY);
 //                           one elected thread issues the chain's MMA batches (3), (4)
 //   warps 7-10   T chain    same for T, plus the row re-normalisation every 8th chunk
@@ -66,10 +66,10 @@ struct F_Bars {
   uint64_t out_full[kF_Slots], out_free[kF_Slots];  // producer group done (4 warps) / (1) and both (3) completed
   uint64_t gate_full[kF_GateSlots];                 // loader wrote the chunk's gate record
   uint64_t m3_done[2], m4_done[2];                  // [block]: 0 = E, 1 = T
-  uint64_t dy_for_t, dy_for_e;                      // the shared DY columns: E's epilogue has read them / T's has
+  uint64_t dy_for_t, dy_for_e;                      // the shared DY columns: E's epilogue has read them / T's has (128 arrivals)
+  uint64_t v_ok[kF_VStages];                        // the V tile has landed and a ragged tail is zeroed
   uint64_t acc_done[2];                             // [producer group]: its MMAs into ACC have completed
   int acc_lock;                                     // ACC is taken (one producer group at a time)
-  int issued1_cnt;                                  // chunks whose (1) is in the tensor pipe
   int fin_flag;                                     // the loader has posted p_final / g_total
   uint32_t tmem_base;
   int abort_flag;
@@ -230,34 +230,46 @@ __device__ __noinline__ void f_chain(const bool kIsT, uint8_t* smem, F_Bars* bar
       tc_fence_before();
       named_bar_sync(1 + b, 128);  // the whole chain has written Xh
       if (issuer) {
-        // the DY columns are shared: E's (3) follows (1) of this chunk (which waited for T's previous epilogue), T's (3)
-        // follows E's epilogue of this chunk
-        if (!kIsT) s2_wait_count(&bars->issued1_cnt, c, abort_flag);
-        else s2_wait_spin(&bars->dy_for_t, c & 1, abort_flag);
-        tc_fence_after();
+        // The DY columns are shared by the two chains in turn.  E: (1) and (3) of this chunk go to the tensor pipe in one
+        // burst once T's epilogue of the previous chunk has read DY; T: (3) follows E's epilogue of this chunk.
+        if (!kIsT) {
+          if (c > 0) s2_wait_spin(&bars->dy_for_e, (c - 1) & 1, abort_flag);
+          s2_wait_spin(&bars->v_ok[slot], (c >> 1) & 1, abort_flag);
+          tc_fence_after();
+          f_issue1(tmem, smem_base + kF_OffV + slot * 2 * kTileB, out);
+        } else {
+          s2_wait_spin(&bars->dy_for_t, c & 1, abort_flag);
+          tc_fence_after();
+        }
         f_issue3(tmem, out, b);
         mma_commit(&bars->m3_done[b]);
-        mma_commit(&bars->out_free[slot]);  // count 3: (1) and both chains' (3) have read the slot
+        mma_commit(&bars->out_free[slot]);  // count 2: both chains' (3) -- and with E's, (1) -- have read the slot
+        if (!kIsT) mma_commit(&bars->v_free[slot]);
       }
       __syncwarp();
     }
-    // ---- epilogue: U'' = fp16(DY) -> TMEM (A operand of (4)), tokens [32 cb, 32 cb + 32) -> columns [16 cb, 16 cb + 16)
+    // ---- epilogue: U'' = fp16(DY) -> TMEM (A operand of (4)), tokens [32 cb, 32 cb + 32) -> columns [16 cb, 16 cb + 16).
+    // DY is handed to the other chain as soon as this thread's loads have completed (128 arrivals), before the conversion.
     s2_wait_warp(&bars->m3_done[b], c & 1, abort_flag, lane);
     tc_fence_after();
-#pragma unroll 1
-    for (int cb = 0; cb < 2; ++cb) {
-      uint32_t y[32];
-      tmem_ld32(tD + 32 * cb, y);
+    {
+      uint32_t y0[32], y1[32];
+      tmem_ld32(tD, y0);
+      tmem_ld32(tD + 32, y1);
       tmem_ld_wait();
+      tc_fence_before();
+      mbar_arrive(kIsT ? &bars->dy_for_e : &bars->dy_for_t);
 #pragma unroll
-      for (int j = 0; j < 16; ++j) y[j] = pack_f16(__uint_as_float(y[2 * j]), __uint_as_float(y[2 * j + 1]));  // slot j <= 2 j
-      tmem_st16(tH + 16 * cb, y);
+      for (int j = 0; j < 16; ++j) y0[j] = pack_f16(__uint_as_float(y0[2 * j]), __uint_as_float(y0[2 * j + 1]));  // slot j <= 2 j
+      tmem_st16(tH, y0);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) y1[j] = pack_f16(__uint_as_float(y1[2 * j]), __uint_as_float(y1[2 * j + 1]));
+      tmem_st16(tH + 16, y1);
     }
     tmem_st_wait();
     tc_fence_before();
     named_bar_sync(1 + b, 128);  // the whole chain has written U''
     if (issuer) {
-      mbar_arrive(kIsT ? &bars->dy_for_e : &bars->dy_for_t);  // DY has been read: the other chain's turn
       tc_fence_after();
       f_issue4(tmem, smem_base + kF_OffK + kst * 2 * kTileB, b);
       mma_commit(&bars->m4_done[b]);
@@ -537,15 +549,17 @@ __global__ void __launch_bounds__(kF_Threads, 1)  // 18 warps = 5 on two of the 
     }
     for (int i = 0; i < kF_Slots; ++i) {
       mbar_init(&bars->out_full[i], 4);
-      mbar_init(&bars->out_free[i], 3);
+      mbar_init(&bars->out_free[i], 2);
     }
     for (int i = 0; i < kF_GateSlots; ++i) mbar_init(&bars->gate_full[i], 1);
     for (int i = 0; i < 2; ++i) {
       mbar_init(&bars->m3_done[i], 1);
       mbar_init(&bars->m4_done[i], 1);
     }
-    mbar_init(&bars->dy_for_t, 1);
-    mbar_init(&bars->dy_for_e, 1);
+    mbar_init(&bars->dy_for_t, 128);
+    mbar_init(&bars->dy_for_e, 128);
+    mbar_init(&bars->v_ok[0], 1);
+    mbar_init(&bars->v_ok[1], 1);
     mbar_init(&bars->acc_done[0], 1);
     mbar_init(&bars->acc_done[1], 1);
     bars->acc_lock = 0;
@@ -553,7 +567,7 @@ __global__ void __launch_bounds__(kF_Threads, 1)  // 18 warps = 5 on two of the 
     bars->bad = 0;
     bars->p_final = 0.f;
     bars->g_total = 0.0;
-    bars->fin_flag = bars->issued1_cnt = 0;
+    bars->fin_flag = 0;
     fence_barrier_init();
   }
   tc_fence_before();
@@ -648,10 +662,10 @@ __global__ void __launch_bounds__(kF_Threads, 1)  // 18 warps = 5 on two of the 
       flag_release(&bars->fin_flag, 1);
     }
   } else if (warp == kF_WIssuer) {
-    // ------------------------------------------------------------------------------------------- (1) issuer
-    // all 32 lanes walk the chunks (every phase of v_full is waited for in order: a parity wait must never skip one);
-    // lane 0 issues.  The ragged last chunk's V box also holds tokens of the next segment: this warp zeroes those rows
-    // first, so that nothing of a neighbour -- not even an Inf or NaN -- reaches the unit through 0 x garbage.
+    // ------------------------------------------------------------------------------------------- V helper
+    // Walks the V tiles in order (every phase of v_full is waited for: a parity wait must never skip one).  The ragged
+    // last chunk's V box also holds tokens of the next segment: this warp zeroes those rows, so that nothing of a
+    // neighbour -- not even an Inf or NaN -- reaches the unit through 0 x garbage; then the tile is released to (1).
 #pragma unroll 1
     for (int c = 0; c < nc; ++c) {
       const int slot = c & 1;
@@ -665,16 +679,7 @@ __global__ void __launch_bounds__(kF_Threads, 1)  // 18 warps = 5 on two of the 
         fence_proxy_async();
       }
       __syncwarp();
-      if (lane == 0) {
-        s2_wait_spin(&bars->out_full[slot], (c >> 1) & 1, abort_flag);
-        if (c > 0) s2_wait_spin(&bars->dy_for_e, (c - 1) & 1, abort_flag);  // T's epilogue of chunk c - 1 has read DY
-        tc_fence_after();
-        f_issue1(tmem, vt, smem_base + kF_OffOut + slot * kF_OutBytes);
-        mma_commit(&bars->v_free[slot]);
-        mma_commit(&bars->out_free[slot]);
-        tc_fence_before();
-        flag_release(&bars->issued1_cnt, c + 1);
-      }
+      if (lane == 0) mbar_arrive(&bars->v_ok[slot]);
       __syncwarp();
     }
   } else if (warp >= kF_WProd) {
