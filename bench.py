@@ -602,10 +602,13 @@ def run_ours(args):
     enc_family = hb.hypic_encode_impl_for(H, D, D, hb.HYPIC_DT_BF16, hb.HYPIC_GATE_SCALAR)
     enc_tflops = th_per_launch * ENC_FLOP_PER_TOKEN_HEAD / (enc_avg * 1e-3) / 1e12
     enc_gbs = (th_per_launch * ENC_BYTES_PER_TOKEN_HEAD + N_SEG * H * G * COMPOSE_BYTES_PER_STEP) / (enc_avg * 1e-3) / 1e9
+    # fractions are reported against the BURST figure (a kernel timed alone), the sustained one beside it
     if enc_family == hb.HYPIC_IMPL_TENSOR:
-        roofline = {"bound": "tensor", "achieved": enc_tflops, "peak": peaks["bf16_tflops_sustained"],
-                    "unit": "TFLOP/s", "frac": enc_tflops / peaks["bf16_tflops_sustained"], "traffic": None,
-                    "peak_kind": f"bf16 dense, sustained, {peaks['source']} (burst {peaks['bf16_tflops']})"}
+        roofline = {"bound": "tensor", "achieved": enc_tflops, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
+                    "frac": enc_tflops / peaks["bf16_tflops"], "traffic": None,
+                    "peak_kind": f"bf16 dense, burst, {peaks['source']}",
+                    "peak_sustained": peaks["bf16_tflops_sustained"],
+                    "frac_sustained": enc_tflops / peaks["bf16_tflops_sustained"]}
     else:
         roofline = {"bound": "alu", "achieved": enc_tflops, "peak": FP32_ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
                     "frac": enc_tflops / FP32_ALU_PEAK_TFLOPS, "traffic": None,
@@ -618,10 +621,13 @@ def run_ours(args):
         # a capture of this very launch shape if there is one, else the per-layer capture scaled to the launch
         roofline["traffic"] = tj.get(f"encode_{fam}_cfg2_fold{G}_dram_bytes",
                                      None if per_layer is None else per_layer * G)
-    roofline.update({"kernel": ("hypic_segment_encode = chunk_offsets_kernel + prep_kernel + scan2_kernel (tensor "
-                                "family; prep and scan share the call about evenly, see profiles/)") if fam == "tensor" else
+        roofline["traffic_source"] = tj.get("source", "profiles/traffic.json (a committed ncu capture, not this run)")
+    alg_bytes = th_per_launch * ENC_BYTES_PER_TOKEN_HEAD + N_SEG * H * G * COMPOSE_BYTES_PER_STEP
+    roofline.update({"kernel": ("hypic_segment_encode = chunk_offsets_kernel + scan3_kernel (tensor family, scalar gate: "
+                                "one fused tcgen05 kernel; the fp32 fallback-list kernel runs empty)") if fam == "tensor" else
                      "hypic_segment_encode = encode_simt_kernel (simt family)",
                      "units_per_launch": f"{th_per_launch} token-heads x {ENC_FLOP_PER_TOKEN_HEAD} flop",
+                     "algorithmic_bytes_per_launch": alg_bytes,
                      "avg_launch_ms": enc_avg, "layers_per_launch": G, "ms_per_layer": enc_layer,
                      "share_of_step": enc_layer * L / ms_step,
                      "frac_of_bf16_burst_peak": enc_tflops / peaks["bf16_tflops"], "hbm_gbs": enc_gbs,
@@ -684,6 +690,22 @@ def run_ours(args):
         extra["cfg2_compose"] = {"avg_launch_ms": cmp_avg, "layers_per_launch": G,
                                  "compose_ops_per_s": N_SEG * H * G / (cmp_avg * 1e-3),
                                  "hbm_gbs": N_SEG * H * G * COMPOSE_BYTES_PER_STEP / (cmp_avg * 1e-3) / 1e9}
+        # the compose half of BASELINE.json's metric and the other configs, where the driver keeps them (it drops "extra")
+        c4 = extra["cfg4_compose"]
+        roofline["compose"] = {"workload": extra["cfg4_compose"]["workload"], "ms_total": c4["ms_total"],
+                               "head_steps": extra["cfg4_compose"]["head_steps"],
+                               "compose_ops_per_s": c4["compose_ops_per_s"], "bound": "hbm",
+                               "achieved": c4["roofline"]["achieved"], "peak": c4["roofline"]["peak"], "unit": "GB/s",
+                               "frac": c4["roofline"]["frac"],
+                               "traffic_source": "profiles/traffic.json: compose_tensor_cfg4_dram_bytes_per_head_step"}
+        c3 = extra["cfg3_encode"]
+        roofline["cfg3_encode"] = {"ms": c3["ms"], "tokens_per_s": c3["tokens_per_s"], "bound": "hbm",
+                                   "achieved": c3["roofline"]["achieved"], "peak": c3["roofline"]["peak"], "unit": "GB/s",
+                                   "frac": c3["roofline"]["frac"],
+                                   "tc_frac_of_bf16_burst_peak": c3["tc_frac_of_bf16_burst_peak"]}
+        c1 = extra["cfg1"]
+        roofline["cfg1"] = {"ms": c1["ms"], "tokens_per_s": c1["tokens_per_s"],
+                            "tc_frac_of_bf16_burst_peak": c1["tc_frac_of_bf16_burst_peak"]}
 
     cpu = None
     if not args.no_cpu_baseline:
