@@ -88,6 +88,18 @@ __device__ __forceinline__ uint32_t pack_bf16_rn(float lo, float hi) {
   return *reinterpret_cast<uint32_t*>(&p);
 }
 
+// Waits of the background roles (producers, loader, gate, V helper): they run chunks ahead of the chains, so a late
+// wake-up costs nothing, while a tight probe loop takes issue slots from the warps on the critical path (ncu: half of
+// all executed instructions were mbarrier probes).
+__device__ __forceinline__ void f_wait_lazy(uint64_t* bar, uint32_t parity, volatile int* abort_flag) {
+#pragma unroll 1
+  for (int i = 0; i < 200000; ++i) {
+    if (mbar_try_wait(bar, parity)) return;
+    __nanosleep(500);
+  }
+  s2_wait(bar, parity, abort_flag);
+}
+
 // ---- MMA batches (one elected thread each)
 constexpr uint32_t kF_DY = 384, kF_ACC = 448;
 __device__ __forceinline__ void f_issue1(uint32_t tmem, uint32_t v_tile, uint32_t out) {  // DY = V^t (A_b f)^t, bf16 hi + lo
@@ -452,7 +464,7 @@ __device__ __forceinline__ void f_produce(uint8_t* smem, F_Bars* bars, volatile 
   named_bar_sync(3 + gi, 128);
 
   // the output slot is free once (1) and both (3) of chunk c - 2 have completed
-  if (c >= kF_Slots) s2_wait_warp(&bars->out_free[c & 1], ((c >> 1) - 1) & 1, abort_flag, lane);
+  if (c >= kF_Slots) f_wait_lazy(&bars->out_free[c & 1], ((c >> 1) - 1) & 1, abort_flag);
 
   // ---- A_b = A diag(beta) as an fp16 B tile (the B operand of the W contraction; it borrows the upper half of the
   // slot's W tile, which is only written once that contraction has completed) and A_b f = A diag(beta f) as a bf16
@@ -587,7 +599,7 @@ __global__ void __launch_bounds__(kF_Threads, 1)  // 18 warps = 5 on two of the 
         if (c < nc) {
           const int kst = c % kF_KStages;
           const int t0 = seg_begin + c * kC;
-          if (c >= kF_KStages) s2_wait_spin(&bars->k_free[kst], ((c / kF_KStages) - 1) & 1, abort_flag);
+          if (c >= kF_KStages) f_wait_lazy(&bars->k_free[kst], ((c / kF_KStages) - 1) & 1, abort_flag);
           mbar_expect_tx(&bars->k_full[kst], 2 * kTileB);
           tma_load_3d(smem_base + kF_OffK + kst * 2 * kTileB, &tmK, 0, h, t0, &bars->k_full[kst]);
           tma_load_3d(smem_base + kF_OffK + kst * 2 * kTileB + 8192, &tmK, 64, h, t0, &bars->k_full[kst]);
@@ -596,7 +608,7 @@ __global__ void __launch_bounds__(kF_Threads, 1)  // 18 warps = 5 on two of the 
         if (cv >= 0) {
           const int vst = cv & 1;
           const int t0 = seg_begin + cv * kC;
-          if (cv >= kF_VStages) s2_wait_spin(&bars->v_free[vst], ((cv >> 1) - 1) & 1, abort_flag);
+          if (cv >= kF_VStages) f_wait_lazy(&bars->v_free[vst], ((cv >> 1) - 1) & 1, abort_flag);
           mbar_expect_tx(&bars->v_full[vst], 2 * kTileB);
           tma_load_3d(smem_base + kF_OffV + vst * 2 * kTileB, &tmV, 0, h, t0, &bars->v_full[vst]);
           tma_load_3d(smem_base + kF_OffV + vst * 2 * kTileB + 8192, &tmV, 64, h, t0, &bars->v_full[vst]);
@@ -631,7 +643,7 @@ __global__ void __launch_bounds__(kF_Threads, 1)  // 18 warps = 5 on two of the 
       float g0 = gn0, g1 = gn1;
       const float b0 = bn0, b1 = bn1;
       if (c + 1 < nc) fetch(c + 1);
-      s2_wait_warp(&bars->k_full[c % kF_KStages], (c / kF_KStages) & 1, abort_flag, lane);  // pacing only
+      f_wait_lazy(&bars->k_full[c % kF_KStages], (c / kF_KStages) & 1, abort_flag);  // pacing only
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {  // inclusive scans of the two token halves
         const float u0 = __shfl_up_sync(0xffffffffu, g0, o), u1 = __shfl_up_sync(0xffffffffu, g1, o);
@@ -671,7 +683,7 @@ __global__ void __launch_bounds__(kF_Threads, 1)  // 18 warps = 5 on two of the 
       const int slot = c & 1;
       const int valid = min(kC, seg_len - c * kC);
       const uint32_t vt = smem_base + kF_OffV + slot * 2 * kTileB;
-      s2_wait_warp(&bars->v_full[slot], (c >> 1) & 1, abort_flag, lane);
+      f_wait_lazy(&bars->v_full[slot], (c >> 1) & 1, abort_flag);
       if (valid < kC) {
 #pragma unroll 1
         for (int p = lane; p < 1024; p += 32)  // 16-byte piece p of the tile: token (p % 512) / 8
@@ -688,8 +700,8 @@ __global__ void __launch_bounds__(kF_Threads, 1)  // 18 warps = 5 on two of the 
 #pragma unroll 1
     for (int c = gi; c < nc; c += 2) {
       const int kst = c % kF_KStages;
-      s2_wait_warp(&bars->gate_full[c & (kF_GateSlots - 1)], (c / kF_GateSlots) & 1, abort_flag, lane);
-      s2_wait_warp(&bars->k_full[kst], (c / kF_KStages) & 1, abort_flag, lane);
+      f_wait_lazy(&bars->gate_full[c & (kF_GateSlots - 1)], (c / kF_GateSlots) & 1, abort_flag);
+      f_wait_lazy(&bars->k_full[kst], (c / kF_KStages) & 1, abort_flag);
       f_produce(smem, bars, abort_flag, tmem, gi, gtid, warp & 3, c, min(kC, seg_len - c * kC),
                 smem_base + kF_OffK + kst * 2 * kTileB, smem_base + kF_OffOut + (c & 1) * kF_OutBytes);
     }
