@@ -541,6 +541,100 @@ def time_extra_diag(hb, device, peaks, iters=16):
                                      "peak_source": peaks["source"]}}}
 
 
+
+def run_strong(args):
+    """--scaling strong: segment parallelism on devices (Eq. 9).  ONE cfg2 request:
+    its 20 segments are LPT-sharded over the ranks; per group of folded layers every rank encodes its shard in two calls
+    (finalize-and-ship: the first call's tuples are exchanged on a side stream while the second call runs), the tuples
+    make an all-to-all (NCCL) to the head-sharded layout and every rank composes its heads."""
+    from paper_2607_01299_b200 import binding as hb
+    from paper_2607_01299_b200 import segment_parallel as sp
+    from paper_2607_01299_b200 import sharding
+
+    rank, local_rank, world = dist_env()
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")  # so that a scaling run can count the ranks of the communicator
+        os.environ.setdefault("NCCL_DEBUG_FILE", os.path.join(ROOT, "gpurun_out", "nccl_rank%h_%p.log"))
+        os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+    hb.load_library()
+    peaks = load_peaks()
+    L, fold = args.layers, max(1, min(args.fold, args.layers))
+    lens = [SEG_LEN] * N_SEG
+    parts, groups_all = sp.plan(lens, world, 2)
+    shards, sizes = [], []
+    for l0 in range(0, L, fold):
+        ls = [wl.cfg2_layer(l, device=device) for l in range(l0, min(l0 + fold, L))]  # the SAME request on every rank
+        full = wl.fold_layers(ls) if len(ls) > 1 else ls[0]
+        del ls
+        shards.append([sp.take_segments(full, groups_all[g][rank]) for g in range(2)])
+        sizes.append(full.H // H)
+        del full
+        torch.cuda.empty_cache()
+    ids = torch.arange(N_SEG, dtype=torch.int32, device=device)
+    cu = torch.tensor([0, N_SEG], dtype=torch.int32, device=device)
+    comm = torch.cuda.Stream(device)
+
+    def step():
+        sent = 0
+        for my in shards:
+            res = sp.encode_exchange_compose(hb, my, groups_all, N_SEG, rank, world, ids, cu, group=None, comm_stream=comm)
+            sent += res.exchanged_bytes
+        return sent
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for _ in range(args.steps):
+        sent = step()
+    t1.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_step = t0.elapsed_time(t1) / args.steps
+    if dist is not None:
+        ms_step = sharding.max_over_ranks(ms_step, device=device)
+        sent_all = torch.tensor([float(sent)], dtype=torch.float64, device=device)
+        dist.all_reduce(sent_all)
+        sent = int(sent_all.item())
+    if rank == 0:
+        tokens = L * N_SEG * SEG_LEN  # ONE request, whatever the number of ranks
+        my_tokens = sum(lens[i] for i in parts[0])
+        tfl = tokens * H * ENC_FLOP_PER_TOKEN_HEAD / (ms_step * 1e-3) / 1e12
+        line = {"metric": METRIC, "value": tokens / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong",
+                "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                "config": {"workload": "cfg2 (BASELINE.json configs[2]): ONE RAG-shaped request, segment-parallel",
+                           "layers": L, "segments": N_SEG, "seg_len": SEG_LEN, "H": H, "dk": D, "dv": D,
+                           "parallelism": f"segments LPT-sharded over {world} ranks (Eq. 9), 2 encode calls per rank and "
+                                          "group (finalize-and-ship), all-to-all of (T_C, S_C|0) to head-sharded compose",
+                           "segments_of_rank0": len(parts[0]), "tokens_of_rank0": my_tokens,
+                           "exchanged_bytes_per_step": sent, "layers_per_call": fold,
+                           "l2": "inputs larger than L2; no flush needed"},
+                "clocks": clocks, "e2e": None, "gpu_launches": None,
+                "roofline": {"bound": "tensor", "achieved": tfl / world, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
+                             "frac": tfl / world / peaks["bf16_tflops"], "traffic": None,
+                             "note": "whole step (encode + exchange + compose) per GPU, algorithmic encode flops"},
+                "cpu_baseline": None}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
 def run_ours(args):
     from paper_2607_01299_b200 import binding as hb
 
@@ -745,12 +839,18 @@ def main():
     ap.add_argument("--e2e-layers", type=int, default=4, help="layers per end-to-end step (bounds pinned host memory)")
     ap.add_argument("--fold", type=int, default=4,
                     help="independent layers folded into the head axis per library call (1 = one call per layer)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="weak: one private cfg2 request per rank (default); strong: ONE request, its segments LPT-sharded "
+                         "over the ranks, tuples exchanged by one all-to-all per group, compose sharded by heads "
+                         "(segment parallelism, PAPER.md:246-267)")
     ap.add_argument("--no-extra", action="store_true", help="skip the cfg1 / cfg4 side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
+    if args.scaling == "strong":
+        return run_strong(args)
     return run_ours(args)
 
 

@@ -61,27 +61,39 @@ def max_over_ranks(value: float, device: Optional[torch.device] = None, group=No
 
 
 def exchange_tuples(E_loc: torch.Tensor, T_loc: torch.Tensor, parts: Sequence[Sequence[int]], rank: int,
-                    world_size: int, group=None) -> Tuple[torch.Tensor, torch.Tensor]:
+                    world_size: int, group=None, out: Optional[Tuple[torch.Tensor, torch.Tensor]] = None,
+                    n_seg: Optional[int] = None, via_host: bool = False) -> Tuple[torch.Tensor, torch.Tensor]:
     """From the segment-sharded layout of encode to the head-sharded layout of compose.
 
     ``E_loc:[len(parts[rank]), H, dv, dk]`` and ``T_loc:[len(parts[rank]), H, dk, dk]`` are this rank's tuples, rows in
     the order of ``parts[rank]`` (``lpt_partition``'s ascending segment indices).  Returns
     ``(E:[n_seg, Hr, dv, dk], T:[n_seg, Hr, dk, dk])`` for ALL segments in global index order and this rank's heads
     ``head_range(H, rank, world_size)``: exactly the pools ``hypic_compose`` takes with ``H = Hr``.
-    One all-to-all; rank ``s`` sends rank ``d`` the block ``[parts[s], heads of d]`` of both tensors."""
+    One all-to-all; rank ``s`` sends rank ``d`` the block ``[parts[s], heads of d]`` of both tensors.
+
+    ``out = (E, T)`` with ``n_seg`` rows: fill these buffers instead of new ones, so that several calls -- one per
+    finished group of segments, ``parts`` then being the group's share of every rank (finalize-and-ship,
+    PAPER.md:265-267) -- assemble one pool.  ``via_host``: stage the blocks through host memory (a ``gloo`` group with
+    device tensors: ranks that share one GPU in a test cannot form an NCCL communicator)."""
     import torch.distributed as dist
 
     n_loc, H, dv, dk = (int(x) for x in E_loc.shape)
     if tuple(T_loc.shape) != (n_loc, H, dk, dk) or n_loc != len(parts[rank]):
         raise ValueError("E_loc / T_loc do not match parts[rank]")
-    n_seg = sum(len(p) for p in parts)
+    if n_seg is None:
+        n_seg = sum(len(p) for p in parts)
     hb, he = head_range(H, rank, world_size)
     Hr = he - hb
     per_head = dv * dk + dk * dk
+    if out is not None:
+        E, T = out
+        if tuple(E.shape) != (n_seg, Hr, dv, dk) or tuple(T.shape) != (n_seg, Hr, dk, dk):
+            raise ValueError("out buffers must be [n_seg, Hr, dv, dk] and [n_seg, Hr, dk, dk]")
+    else:
+        E = torch.empty((n_seg, Hr, dv, dk), dtype=E_loc.dtype, device=E_loc.device)
+        T = torch.empty((n_seg, Hr, dk, dk), dtype=E_loc.dtype, device=E_loc.device)
     if world_size == 1:
         order = torch.as_tensor(list(parts[0]), dtype=torch.long, device=E_loc.device)
-        E = torch.empty_like(E_loc)
-        T = torch.empty_like(T_loc)
         E[order], T[order] = E_loc, T_loc
         return E, T
     send_chunks, send_sizes = [], []
@@ -93,10 +105,14 @@ def exchange_tuples(E_loc: torch.Tensor, T_loc: torch.Tensor, parts: Sequence[Se
         send_sizes.append(n_loc * (e - b) * per_head)
     recv_sizes = [len(parts[s]) * Hr * per_head for s in range(world_size)]
     send = torch.cat(send_chunks)
-    recv = torch.empty(sum(recv_sizes), dtype=E_loc.dtype, device=E_loc.device)
-    dist.all_to_all_single(recv, send, output_split_sizes=recv_sizes, input_split_sizes=send_sizes, group=group)
-    E = torch.empty((n_seg, Hr, dv, dk), dtype=E_loc.dtype, device=E_loc.device)
-    T = torch.empty((n_seg, Hr, dk, dk), dtype=E_loc.dtype, device=E_loc.device)
+    if via_host:
+        send_h = send.cpu()
+        recv_h = torch.empty(sum(recv_sizes), dtype=E_loc.dtype)
+        dist.all_to_all_single(recv_h, send_h, output_split_sizes=recv_sizes, input_split_sizes=send_sizes, group=group)
+        recv = recv_h.to(E_loc.device)
+    else:
+        recv = torch.empty(sum(recv_sizes), dtype=E_loc.dtype, device=E_loc.device)
+        dist.all_to_all_single(recv, send, output_split_sizes=recv_sizes, input_split_sizes=send_sizes, group=group)
     off = 0
     for s in range(world_size):
         n_s = len(parts[s])

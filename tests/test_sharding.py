@@ -10,6 +10,7 @@ import torch.distributed as dist
 import torch.multiprocessing as mp
 
 import oracle
+from paper_2607_01299_b200 import segment_parallel as sp
 from paper_2607_01299_b200 import sharding
 from paper_2607_01299_b200 import workloads as wl
 
@@ -123,3 +124,62 @@ def test_fold_layers_is_a_pure_relayout():
                            layers[1].cu_seqlens.numpy())
     assert np.array_equal(Ef[:, 2:4], E1) and np.array_equal(Tf[:, 2:4], T1)
 
+
+
+# ------------------------------------------------------------------ segment parallelism: plan, groups, grouped exchange
+def test_plan_groups_cover_every_segment_once():
+    lens = wl.cfg3_seg_lens()
+    for world in (1, 2, 3):
+        for n_groups in (1, 2, 4):
+            parts, groups_all = sp.plan(lens, world, n_groups)
+            assert len(groups_all) == n_groups and all(len(g) == world for g in groups_all)
+            for r in range(world):
+                mine = sorted(i for g in groups_all for i in g[r])
+                assert mine == parts[r]
+            # longest first: the first group of a rank holds its longest segment
+            for r in range(world):
+                if parts[r]:
+                    longest = max(parts[r], key=lambda i: (lens[i], -i))
+                    assert longest in groups_all[0][r]
+
+
+def test_take_segments_is_pure_indexing():
+    inp = wl.make_encode_inputs([7, 0, 5, 9], 2, 8, 8, kv_dtype=torch.float32, seed=3)
+    sub = sp.take_segments(inp, [3, 0])
+    assert sub.seg_lens == [9, 7] and sub.cu_seqlens.tolist() == [0, 9, 16]
+    assert torch.equal(sub.k[:9], inp.k[12:21]) and torch.equal(sub.k[9:], inp.k[:7])
+    assert torch.equal(sub.g[:9], inp.g[12:21]) and torch.equal(sub.beta[9:], inp.beta[:7])
+    empty = sp.take_segments(inp, [])
+    assert empty.n_seg == 0 and empty.t_total == 0
+
+
+def _worker_groups(rank, world, port, out_dir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        H = 3
+        inp = wl.make_encode_inputs([70, 33, 129, 64, 5, 90], H, 16, 16, kv_dtype=torch.float32, seed=wl.seed_for(0, 11))
+        E_all, T_all = oracle.segment_encode(inp.k, inp.v, inp.g, inp.beta, inp.cu_seqlens, gate=inp.gate)
+        parts, groups_all = sp.plan(inp.seg_lens, world, 3)
+        b, e = sharding.head_range(H, rank, world)
+        E = torch.full((6, e - b, 16, 16), float("nan"))
+        T = torch.full((6, e - b, 16, 16), float("nan"))
+        for g in range(3):  # one exchange per finished group, all filling the same pools
+            mine = groups_all[g][rank]
+            E_loc = torch.from_numpy(np.ascontiguousarray(E_all[mine])).float().reshape(len(mine), H, 16, 16)
+            T_loc = torch.from_numpy(np.ascontiguousarray(T_all[mine])).float().reshape(len(mine), H, 16, 16)
+            sharding.exchange_tuples(E_loc, T_loc, groups_all[g], rank, world, out=(E, T), n_seg=6)
+        assert torch.equal(E, torch.from_numpy(np.ascontiguousarray(E_all[:, b:e])).float())
+        assert torch.equal(T, torch.from_numpy(np.ascontiguousarray(T_all[:, b:e])).float())
+        with open(os.path.join(out_dir, f"ok{rank}"), "w") as f:
+            f.write("ok")
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_rank_gloo_grouped_exchange(tmp_path):
+    """Finalize-and-ship: three exchanges, one per finished group (one of them empty on a rank), assemble
+    the same head-sharded pools as the single all-to-all."""
+    world = 2
+    mp.spawn(_worker_groups, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    assert all((tmp_path / f"ok{r}").exists() for r in range(world))
