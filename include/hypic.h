@@ -82,10 +82,13 @@ size_t hypic_segment_encode_workspace(int32_t n_seg, int32_t t_total, int32_t H,
  *            (may be NULL when that is 0).  Contents are undefined before and after the call.
  *
  * A zero-length segment yields E = 0, T = I.  n_seg = 0 or t_total = 0 with n_seg > 0 are valid.
- * Built envelope: dk in {64, 128}; dv in [1, 1024] for the SIMT family, dv = dk = 128 for the tensor family
- * (bf16 k/v, scalar or per-channel gate; its tensor-core operands are fp16, so it additionally assumes finite |k|, |v| <= 65504 and
- * beta |k|^2 within the stable range of the recurrence and a per-chunk log-decay >= -9, see
- * hypic_envelope_violation_count -- callers outside that range select HYPIC_IMPL_SIMT);
+ * Built envelope (shapes): dk in {64, 128}; dv in [1, 1024] for the SIMT family (fp32 CUDA cores), dv = dk = 128 with
+ * bf16 k/v for the tensor family (tcgen05; scalar or per-channel gate), which HYPIC_IMPL_AUTO takes whenever the shape
+ * allows.  Values: any finite inputs.  The tensor family computes with 16-bit operands; what those cannot carry -- a
+ * per-channel chunk whose log-decay leaves [-9, 0], weighted values or states beyond fp16's range -- is detected on the
+ * device per (segment, head) unit, and exactly those units are recomputed by the fp32 family inside the same call, on the
+ * same stream, with no host synchronisation and no caller action (the scalar gate never enters the 16-bit algebra, so it
+ * has no log-decay limit at all).  hypic_envelope_violation_count remains as a diagnostic counter.
  * H, n_seg, lengths arbitrary.  Inputs are only read; E and T are fully overwritten.
  */
 int hypic_segment_encode(const void* k, const void* v, const float* g, const float* beta,
@@ -257,14 +260,13 @@ int hypic_compose_impl_for(int32_t H, int32_t dk, int32_t dv);
 unsigned int hypic_debug_timeout_count(void);
 
 /*
- * hypic_envelope_violation_count: the tensor-family encode computes in fp16 operands and therefore assumes that the
- * cumulative log-decay of every 64-token chunk stays above -9 (gamma >= 1.2e-4 inside a chunk; the benchmark
- * distributions stay above -6.4) and that g and beta are finite.  Its prep kernel counts the (chunk, head) pairs that
- * break this since library load; such pairs may come out with a relative error above the family's tolerance, and the
- * caller should re-run the call with HYPIC_IMPL_SIMT, which has no such limit.  The tcgen05 kernels of hypic_diag_encode
- * add to the same counter for every 64-token chunk (per warp of 64 or 512 log-decays) that holds a positive or non-finite
- * log-decay (their fp16 weights exp(sum of later log-decays) must not exceed 1).  Synchronises the device; 0 = never
- * violated; 0xffffffff = the query itself failed.
+ * hypic_envelope_violation_count: diagnostics.  The per-channel tensor-family encode counts the (chunk, head) pairs whose
+ * per-channel log-decay leaves [-9, 0] since library load (their units are recomputed in fp32 inside the same call, see
+ * hypic_segment_encode; nothing is left to the caller).  The tcgen05 kernels of hypic_diag_encode add to the same
+ * counter for every 64-token chunk that holds a positive or non-finite log-decay (their fp16 weights exp(sum of later
+ * log-decays) must not exceed 1; Table 1's gates are <= 1, so such inputs are outside the method's range -- that call
+ * has no workspace, so there the caller re-runs with HYPIC_IMPL_SIMT).  Synchronises the device; 0 = never;
+ * 0xffffffff = the query itself failed.
  */
 unsigned int hypic_envelope_violation_count(void);
 
