@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 #include "../../include/hypic.h"
 
 namespace hypic {
@@ -147,7 +149,19 @@ unsigned int debug_timeout_count_encode();
 unsigned int envelope_violation_count_encode();
 unsigned int debug_timeout_count();  // bounded-wait expiries in the tensor kernels since load (0 = healthy)
 
-// Device properties cached per process (SM count, opt-in shared memory).
+// Per-device one-time setup (cudaFuncSetAttribute is per device): `mask` holds one bit per device ordinal (< 64; beyond
+// that the setup simply runs on every call).  Concurrent first calls may both run the setup, which is idempotent.
+inline bool needs_device_setup(std::atomic<unsigned long long>& mask, int* dev_out) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) dev = 0;
+  *dev_out = dev;
+  return dev >= 64 || ((mask.load(std::memory_order_acquire) >> dev) & 1ull) == 0;
+}
+inline void device_setup_done(std::atomic<unsigned long long>& mask, int dev) {
+  if (dev < 64) mask.fetch_or(1ull << dev, std::memory_order_release);
+}
+
+// Device properties of the CURRENT device, cached per device ordinal (SM count, opt-in shared memory).
 struct DeviceInfo {
   int ok;  // 0 = not queried / failed
   int device;

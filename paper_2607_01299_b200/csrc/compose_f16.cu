@@ -112,8 +112,8 @@ int make_rows_tensor_map_f16(CUtensorMap* tm, const void* base, uint64_t rows) {
 template <int kHeads>
 __global__ void __launch_bounds__(kThreads, 1)
     compose_f16_kernel(const __grid_constant__ CUtensorMap tmE, const __grid_constant__ CUtensorMap tmT,
-                       const float* __restrict__ S_in, const int32_t* __restrict__ seg_ids,
-                       const int32_t* __restrict__ cu_segs, int R, int H, float* __restrict__ S_out) {
+                       const float* S_in /* may alias S_out */, const int32_t* __restrict__ seg_ids,
+                       const int32_t* __restrict__ cu_segs, int R, int H, float* S_out) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   Bars* bars = reinterpret_cast<Bars*>(smem + kOffBar);
@@ -331,11 +331,12 @@ bool compose_f16_shape_ok(int32_t, int32_t dk, int32_t dv) { return dk == kD && 
 int compose_f16(const ComposeF16Args& a) {
   if (!compose_f16_shape_ok(a.H, a.dk, a.dv)) return HYPIC_ERR_UNSUPPORTED;
   if (a.R == 0) return HYPIC_OK;
-  static bool configured = false;
-  if (!configured) {
+  static std::atomic<unsigned long long> configured{0};
+  int cfg_dev = 0;
+  if (needs_device_setup(configured, &cfg_dev)) {
     HYPIC_CUDA_OK(cudaFuncSetAttribute(compose_f16_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
     HYPIC_CUDA_OK(cudaFuncSetAttribute(compose_f16_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
-    configured = true;
+    device_setup_done(configured, cfg_dev);
   }
   const long long units = (long long)a.R * a.H;
   if (units > 0x7fffffffLL) return HYPIC_ERR_UNSUPPORTED;

@@ -16,12 +16,12 @@ constexpr int kBM = 128;       // rows of S per CTA
 constexpr int kSlab = 16;      // rows of T per staged slab
 
 template <int DK>
-__global__ void __launch_bounds__(kThreads) compose_simt_kernel(const float* __restrict__ S_in,
+__global__ void __launch_bounds__(kThreads) compose_simt_kernel(const float* S_in,  /* may alias S_out: no __restrict__, no read-only path */
                                                                 const float* __restrict__ E_pool,
                                                                 const float* __restrict__ T_pool,
                                                                 const int32_t* __restrict__ seg_ids,
                                                                 const int32_t* __restrict__ cu_segs, int H, int dv,
-                                                                float* __restrict__ S_out) {
+                                                                float* S_out) {
   constexpr int NJ = DK / 16;     // output columns per thread
   constexpr int LDS_ = kBM + 4;   // padded leading dimension of the transposed state
   extern __shared__ __align__(16) float smem[];
@@ -118,11 +118,12 @@ __global__ void __launch_bounds__(kThreads) compose_simt_kernel(const float* __r
 template <int DK>
 int launch(const ComposeArgs& a) {
   const size_t smem = (size_t)(DK * (kBM + 4) + 2 * kSlab * DK) * sizeof(float);
-  static bool configured = false;
-  if (!configured) {
+  static std::atomic<unsigned long long> configured{0};
+  int cfg_dev = 0;
+  if (needs_device_setup(configured, &cfg_dev)) {
     HYPIC_CUDA_OK(cudaFuncSetAttribute(compose_simt_kernel<DK>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)smem));
-    configured = true;
+    device_setup_done(configured, cfg_dev);
   }
   dim3 grid((a.dv + kBM - 1) / kBM, a.H, a.R);
   compose_simt_kernel<DK><<<grid, kThreads, smem, a.stream>>>(a.S_in, a.E_pool, a.T_pool, a.seg_ids, a.cu_segs, a.H,

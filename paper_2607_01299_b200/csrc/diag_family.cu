@@ -230,9 +230,9 @@ constexpr int kDcV4 = 4;  // float4s of S per thread: a CTA owns 4,096 consecuti
 // ONE float4 of the decay vector per step (otherwise each float4 fetches its own).
 template <bool CHANNEL, bool F16, bool TSH = false>
 __global__ void __launch_bounds__(kDcThreads, (CHANNEL && !TSH) ? 2 : 3)
-    diag_compose_kernel(const float* __restrict__ S_in, const void* __restrict__ E_pool,
+    diag_compose_kernel(const float* S_in /* may alias S_out */, const void* __restrict__ E_pool,
                         const float* __restrict__ t_pool, const int32_t* __restrict__ seg_ids,
-                        const int32_t* __restrict__ cu_segs, int H, int dk, int unit_v4, float* __restrict__ S_out) {
+                        const int32_t* __restrict__ cu_segs, int H, int dk, int unit_v4, float* S_out) {
   const int tid = threadIdx.x;
   const int h = blockIdx.y, r = blockIdx.z;
   const size_t unit = (size_t)r * H + h;
@@ -247,7 +247,7 @@ __global__ void __launch_bounds__(kDcThreads, (CHANNEL && !TSH) ? 2 : 3)
 #pragma unroll
   for (int i = 0; i < kDcV4; ++i) {
     x[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (live[i] && S_in) x[i] = __ldg(reinterpret_cast<const float4*>(S_in) + unit * unit_v4 + e4[i]);
+    if (live[i] && S_in) x[i] = *(reinterpret_cast<const float4*>(S_in) + unit * unit_v4 + e4[i]);  // plain load: S_out may alias S_in
   }
   const int dk4 = dk / 4;
   const int j0 = cu_segs[r], j1 = cu_segs[r + 1];

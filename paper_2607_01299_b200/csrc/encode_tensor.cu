@@ -194,11 +194,12 @@ int encode_tensor(const EncodeArgs& a) {
   uint8_t* rec = ws + ws_off_rec(a.n_seg, a.H, cap);
   const bool ch = a.gate == HYPIC_GATE_CHANNEL;
   float* gate = reinterpret_cast<float*>(rec + cap * a.H * (size_t)(ch ? kRecBytesCh : kRecBytes));
-  static bool configured = false;
-  if (!configured) {
+  static std::atomic<unsigned long long> configured{0};
+  int cfg_dev = 0;
+  if (needs_device_setup(configured, &cfg_dev)) {
     HYPIC_CUDA_OK(cudaFuncSetAttribute(scan3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kF_Smem));
     HYPIC_CUDA_OK(cudaFuncSetAttribute(scan2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kS2Smem));
-    configured = true;
+    device_setup_done(configured, cfg_dev);
   }
   const auto* kp = static_cast<const __nv_bfloat16*>(a.k);
   CUtensorMap tmK, tmV;
@@ -236,12 +237,13 @@ int diag_encode_tensor(const DiagEncodeArgs& a) {
   if (!diag_encode_tensor_shape_ok(a.H, a.dk, a.dv, a.kv_dtype, a.gate) || a.t_total <= 0) return HYPIC_ERR_UNSUPPORTED;
   if (a.n_seg == 0) return HYPIC_OK;
   if (a.H > 65535 || a.n_seg > 65535) return HYPIC_ERR_UNSUPPORTED;
-  static bool configured = false;
-  if (!configured) {
+  static std::atomic<unsigned long long> configured{0};
+  int cfg_dev = 0;
+  if (needs_device_setup(configured, &cfg_dev)) {
     HYPIC_CUDA_OK(cudaFuncSetAttribute(diag_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDtSmem));
     HYPIC_CUDA_OK(cudaFuncSetAttribute(diag_scan_split2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDtSmem));
     HYPIC_CUDA_OK(cudaFuncSetAttribute(diag_scan_ch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDtChSmem));
-    configured = true;
+    device_setup_done(configured, cfg_dev);
   }
   CUtensorMap tmK, tmV;
   int rc = make_kv_tensor_map(&tmK, a.k, a.t_total, a.H);

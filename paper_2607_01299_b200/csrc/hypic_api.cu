@@ -11,21 +11,26 @@ thread_local int g_last_cuda_error = 0;
 static std::atomic<int> g_impl{HYPIC_IMPL_AUTO};
 
 const DeviceInfo& device_info() {
-  static DeviceInfo info = [] {
-    DeviceInfo d{};
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return d;
-    cudaDeviceProp p;
-    if (cudaGetDeviceProperties(&p, dev) != cudaSuccess) return d;
-    d.device = dev;
-    d.sm_count = p.multiProcessorCount;
-    d.cc_major = p.major;
-    d.cc_minor = p.minor;
-    d.max_smem_optin = (int)p.sharedMemPerBlockOptin;
-    d.ok = 1;
-    return d;
-  }();
-  return info;
+  static DeviceInfo infos[64];
+  static std::atomic<unsigned long long> known{0};
+  static thread_local DeviceInfo scratch;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) dev = 0;
+  DeviceInfo* d = (dev >= 0 && dev < 64) ? &infos[dev] : &scratch;
+  if (dev >= 0 && dev < 64 && ((known.load(std::memory_order_acquire) >> dev) & 1ull)) return *d;
+  DeviceInfo t{};
+  cudaDeviceProp p;
+  if (cudaGetDeviceProperties(&p, dev) == cudaSuccess) {
+    t.device = dev;
+    t.sm_count = p.multiProcessorCount;
+    t.cc_major = p.major;
+    t.cc_minor = p.minor;
+    t.max_smem_optin = (int)p.sharedMemPerBlockOptin;
+    t.ok = 1;
+  }
+  *d = t;  // concurrent first calls write the same values
+  if (dev >= 0 && dev < 64 && t.ok) known.fetch_or(1ull << dev, std::memory_order_release);
+  return *d;
 }
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
