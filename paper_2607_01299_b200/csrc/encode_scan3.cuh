@@ -100,43 +100,119 @@ __device__ __forceinline__ void f_wait_lazy(uint64_t* bar, uint32_t parity, vola
   s2_wait(bar, parity, abort_flag);
 }
 
-// ---- MMA batches (one elected thread each)
 constexpr uint32_t kF_DY = 384, kF_ACC = 448;
-__device__ __forceinline__ void f_issue1(uint32_t tmem, uint32_t v_tile, uint32_t out) {  // DY = V^t (A_b f)^t, bf16 hi + lo
-  constexpr uint32_t id1 = make_idesc(1u, 128, 64, 1, 0);  // bf16, A MN-major (V tile), B K-major (A_b f)
-#pragma unroll
-  for (int ks = 0; ks < 8; ++ks)
-    mma_f16_ss(tmem + kF_DY, make_desc(v_tile + (ks & 3) * 2048, 8192, 1024, 2),
-               make_desc(out + (ks < 4 ? kF_OutHi : kF_OutLo) + (ks & 3) * 32, 16, 1024, 2), id1, ks > 0);
+// ---- MMA bursts.  Each is ONE asm block executed by a whole converged warp (warp-uniform control flow): one elected lane
+// issues, descriptors and TMEM addresses advance inside the block, and the commits ride along.  Issued from a
+// lane-divergent branch (`if (lane == 0)`), ptxas wraps every tcgen05.mma in an ELECT / R2UR.BROADCAST x 5 / branch
+// loop of ~21 dependent instructions -- ~100 cycles of issue time per MMA, 44 MMAs per chunk; in this form the
+// UTCHMMAs come out back to back on the uniform datapath.
+// Descriptor arithmetic: the low 14 bits hold (address >> 4); steps used: 16 rows of a 128-byte-row tile = 2048 B =
+// +128, 32 B inside a row = +2, the next 64-column box = 8192 B = +512.
+#define F_MMA_TS "@P tcgen05.mma.cta_group::1.kind::f16 [%0], [at], bd, %3, Q;\n\t"
+#define F_MMA_SS "@P tcgen05.mma.cta_group::1.kind::f16 [%0], ad, bd, %3, Q;\n\t"
+#define F_COMMIT(n) "@P tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%" #n "];\n\t"
+// (3): DY (+)= Xh_b (-W)^t -- A = Xh from TMEM (8 columns per k-step), B = the slot's W^t tile (MN-major, negated by the
+// instruction descriptor); then commits to m3_done and to the slot's out_free, and to v_free for the E chain.
+__device__ __forceinline__ void f_issue3(uint32_t d_tmem, uint32_t a_tmem, uint32_t w_tile, uint32_t acc_first,
+                                         uint64_t* bar0, uint64_t* bar1, uint64_t* bar2) {
+  constexpr uint32_t id3 = make_idesc(0u, 128, 64, 0, 1, 0, 1);
+  const uint64_t bd0 = make_desc(w_tile, 8192, 1024, 2);
+  const uint32_t b2 = bar2 ? smem_u32(bar2) : 0u;
+  asm volatile(
+      "{\n\t.reg .pred P, Q, R;\n\t.reg .b64 bd;\n\t.reg .b32 at;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "setp.ne.b32 Q, %4, 0;\n\tsetp.ne.b32 R, %7, 0;\n\tand.pred R, R, P;\n\t"
+      "mov.b64 bd, %2;\n\tmov.b32 at, %1;\n\t" F_MMA_TS
+      "setp.ne.b32 Q, 1, 0;\n\t"
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      F_COMMIT(5) F_COMMIT(6)
+      "@R tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%7];\n\t"
+      "}" ::"r"(d_tmem), "r"(a_tmem), "l"(bd0), "r"(id3), "r"(acc_first), "r"(smem_u32(bar0)), "r"(smem_u32(bar1)), "r"(b2)
+      : "memory");
 }
-__device__ __forceinline__ void f_issue3(uint32_t tmem, uint32_t out, int b) {  // DY (+)= Xh_b (-W)^t
-  constexpr uint32_t id3 = make_idesc(0u, 128, 64, 0, 1, 0, 1);  // fp16, A from TMEM, B = W^t tile MN-major, negated
-#pragma unroll
-  for (int ks = 0; ks < 8; ++ks)
-    mma_f16_ts(tmem + kF_DY, tmem + 256 + 64 * b + 8 * ks, make_desc(out + kF_OutW + ks * 2048, 8192, 1024, 2), id3,
-               (b == 0 || ks > 0) ? 1u : 0u);
-}
-__device__ __forceinline__ void f_issue4(uint32_t tmem, uint32_t k_tile, int b) {  // X_b += U''_b K
+// (4): X_b += U''_b K -- A = U'' from TMEM, B = the K tile (MN-major, two 64-column boxes); commits to m4_done, k_free
+__device__ __forceinline__ void f_issue4(uint32_t d_tmem, uint32_t a_tmem, uint32_t k_tile, uint64_t* bar0, uint64_t* bar1) {
   constexpr uint32_t id4 = make_idesc(0u, 128, 128, 0, 1);
-#pragma unroll
-  for (int ks = 0; ks < 4; ++ks)
-    mma_f16_ts(tmem + 128 * b, tmem + 256 + 64 * b + 8 * ks, make_desc(k_tile + ks * 2048, 8192, 1024, 2), id4, 1u);
+  const uint64_t bd0 = make_desc(k_tile, 8192, 1024, 2);
+  asm volatile(
+      "{\n\t.reg .pred P, Q;\n\t.reg .b64 bd;\n\t.reg .b32 at;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "setp.ne.b32 Q, 1, 0;\n\t"
+      "mov.b64 bd, %2;\n\tmov.b32 at, %1;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      F_COMMIT(4) F_COMMIT(5)
+      "}" ::"r"(d_tmem), "r"(a_tmem), "l"(bd0), "r"(id4), "r"(smem_u32(bar0)), "r"(smem_u32(bar1))
+      : "memory");
 }
-__device__ __forceinline__ void f_issue_gram(uint32_t tmem, uint32_t k_tile) {  // ACC[0:64, 0:64] = K K^t
-  // M = 128: the A rows 64..127 run on into whatever follows the 64-row box (valid shared memory); their results land in
-  // TMEM lanes 64..127 and are never read.  An M = 64 instruction costs the same tensor time.
+// (1): DY = V^t (A_b f)^t on bf16 operands -- A = the V tile (MN-major, +128 per 16 tokens), B = the hi tile then the lo
+// tile of A_b diag(f) (K-major, +2 per 16 tokens; lo = hi + 8192 B); no commit: (3) of the same chunk follows
+__device__ __forceinline__ void f_issue1(uint32_t d_tmem, uint32_t v_tile, uint32_t hi_tile) {
+  constexpr uint32_t id1 = make_idesc(1u, 128, 64, 1, 0);
+  const uint64_t ad0 = make_desc(v_tile, 8192, 1024, 2), bd0 = make_desc(hi_tile, 16, 1024, 2);
+  asm volatile(
+      "{\n\t.reg .pred P, Q;\n\t.reg .b64 ad, bd;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "setp.ne.b32 Q, 0, 0;\n\t"
+      "mov.b64 ad, %1;\n\tmov.b64 bd, %2;\n\t" F_MMA_SS
+      "setp.ne.b32 Q, 1, 0;\n\t"
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      "mov.b64 ad, %1;\n\tadd.s64 bd, bd, 506;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      "}" ::"r"(d_tmem), "l"(ad0), "l"(bd0), "r"(id1)
+      : "memory");
+}
+// (G): ACC[0:64, 0:64] = K K^t -- A = B = the fp16 K tile, K-major, two 64-column boxes.  M = 128: the A rows 64..127 run
+// on into whatever follows the 64-row box (valid shared memory); their results land in TMEM lanes 64..127 and are never
+// read.  An M = 64 instruction costs the same tensor time.  Commits to the group's acc_done.
+__device__ __forceinline__ void f_issue_gram(uint32_t d_tmem, uint32_t k_tile, uint64_t* bar0) {
   constexpr uint32_t idg = make_idesc(0u, 128, 64, 0, 0);
-#pragma unroll
-  for (int ks = 0; ks < 8; ++ks) {
-    const uint64_t d = make_desc(k_tile + (ks >> 2) * 8192 + (ks & 3) * 32, 16, 1024, 2);
-    mma_f16_ss(tmem + kF_ACC, d, d, idg, ks > 0);
-  }
+  const uint64_t d0 = make_desc(k_tile, 16, 1024, 2);
+  asm volatile(
+      "{\n\t.reg .pred P, Q;\n\t.reg .b64 ad, bd;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "setp.ne.b32 Q, 0, 0;\n\t"
+      "mov.b64 ad, %1;\n\tmov.b64 bd, %1;\n\t" F_MMA_SS
+      "setp.ne.b32 Q, 1, 0;\n\t"
+      "add.s64 ad, ad, 2;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 2;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 2;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 506;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 2;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 2;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 2;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      F_COMMIT(2)
+      "}" ::"r"(d_tmem), "l"(d0), "r"(smem_u32(bar0)), "r"(idg)
+      : "memory");
 }
-__device__ __forceinline__ void f_issue_w(uint32_t tmem, uint32_t k_tile, uint32_t ab_tile) {  // ACC = K^t A_b^t = W^t
-  constexpr uint32_t idw = make_idesc(0u, 128, 64, 1, 0);  // fp16, A = K tile MN-major, B = A_b K-major
-#pragma unroll
-  for (int ks = 0; ks < 4; ++ks)
-    mma_f16_ss(tmem + kF_ACC, make_desc(k_tile + ks * 2048, 8192, 1024, 2), make_desc(ab_tile + ks * 32, 16, 1024, 2), idw, ks > 0);
+// (W): ACC = K^t A_b^t = W^t -- A = the K tile MN-major (+128 per 16 tokens), B = the A_b tile K-major (+2); commits to
+// the group's acc_done
+__device__ __forceinline__ void f_issue_w(uint32_t d_tmem, uint32_t k_tile, uint32_t ab_tile, uint64_t* bar0) {
+  constexpr uint32_t idw = make_idesc(0u, 128, 64, 1, 0);
+  const uint64_t ad0 = make_desc(k_tile, 8192, 1024, 2), bd0 = make_desc(ab_tile, 16, 1024, 2);
+  asm volatile(
+      "{\n\t.reg .pred P, Q;\n\t.reg .b64 ad, bd;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "setp.ne.b32 Q, 0, 0;\n\t"
+      "mov.b64 ad, %1;\n\tmov.b64 bd, %2;\n\t" F_MMA_SS
+      "setp.ne.b32 Q, 1, 0;\n\t"
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      F_COMMIT(4)
+      "}" ::"r"(d_tmem), "l"(ad0), "l"(bd0), "r"(idw), "r"(smem_u32(bar0))
+      : "memory");
 }
 // ACC lock (one thread per producer group)
 __device__ __forceinline__ void f_acc_acquire(int* lock) {
@@ -166,7 +242,7 @@ __device__ __noinline__ void f_chain(const bool kIsT, uint8_t* smem, F_Bars* bar
   const uint32_t smem_base = smem_u32(smem);
   const float* gate_ring = reinterpret_cast<const float*>(smem + kF_OffGate);
   int s_exp = 0;  // T chain: the TMEM copy of this row is That_row * 2^s_exp
-  const bool issuer = (cw == (kIsT ? kF_WChainT : kF_WChainE) && lane == 0);
+  const bool issue_warp = (cw == (kIsT ? kF_WChainT : kF_WChainE));  // warp-uniform: the bursts elect their lane
 
   // X_0 = [0 ; I]
 #pragma unroll
@@ -241,24 +317,22 @@ __device__ __noinline__ void f_chain(const bool kIsT, uint8_t* smem, F_Bars* bar
       tmem_st_wait();
       tc_fence_before();
       named_bar_sync(1 + b, 128);  // the whole chain has written Xh
-      if (issuer) {
+      if (issue_warp) {
         // The DY columns are shared by the two chains in turn.  E: (1) and (3) of this chunk go to the tensor pipe in one
         // burst once T's epilogue of the previous chunk has read DY; T: (3) follows E's epilogue of this chunk.
         if (!kIsT) {
-          if (c > 0) s2_wait_spin(&bars->dy_for_e, (c - 1) & 1, abort_flag);
-          s2_wait_spin(&bars->v_ok[slot], (c >> 1) & 1, abort_flag);
+          if (c > 0) s2_wait_warp(&bars->dy_for_e, (c - 1) & 1, abort_flag, lane);
+          s2_wait_warp(&bars->v_ok[slot], (c >> 1) & 1, abort_flag, lane);
           tc_fence_after();
-          f_issue1(tmem, smem_base + kF_OffV + slot * 2 * kTileB, out);
+          f_issue1(tmem + kF_DY, smem_base + kF_OffV + slot * 2 * kTileB, out + kF_OutHi);
         } else {
-          s2_wait_spin(&bars->dy_for_t, c & 1, abort_flag);
+          s2_wait_warp(&bars->dy_for_t, c & 1, abort_flag, lane);
           tc_fence_after();
         }
-        f_issue3(tmem, out, b);
-        mma_commit(&bars->m3_done[b]);
-        mma_commit(&bars->out_free[slot]);  // count 2: both chains' (3) -- and with E's, (1) -- have read the slot
-        if (!kIsT) mma_commit(&bars->v_free[slot]);
+        // commits: m3_done; out_free (count 2: both chains' (3) -- and with E's, (1) -- have read the slot); E: v_free
+        f_issue3(tmem + kF_DY, tmem + cH, out + kF_OutW, kIsT ? 0u : 1u, &bars->m3_done[b], &bars->out_free[slot],
+                 kIsT ? nullptr : &bars->v_free[slot]);
       }
-      __syncwarp();
     }
     // ---- epilogue: U'' = fp16(DY) -> TMEM (A operand of (4)), tokens [32 cb, 32 cb + 32) -> columns [16 cb, 16 cb + 16).
     // DY is handed to the other chain as soon as this thread's loads have completed (128 arrivals), before the conversion.
@@ -281,13 +355,11 @@ __device__ __noinline__ void f_chain(const bool kIsT, uint8_t* smem, F_Bars* bar
     tmem_st_wait();
     tc_fence_before();
     named_bar_sync(1 + b, 128);  // the whole chain has written U''
-    if (issuer) {
+    if (issue_warp) {
       tc_fence_after();
-      f_issue4(tmem, smem_base + kF_OffK + kst * 2 * kTileB, b);
-      mma_commit(&bars->m4_done[b]);
-      mma_commit(&bars->k_free[kst]);  // count 2: both chains' (4) of this chunk have completed
+      // commits: m4_done; k_free (count 2: both chains' (4) of this chunk have completed)
+      f_issue4(tmem + cX, tmem + cH, smem_base + kF_OffK + kst * 2 * kTileB, &bars->m4_done[b], &bars->k_free[kst]);
     }
-    __syncwarp();
   }
 
   // ---- a5: write this thread's row; the gate (and T's row scale) is applied here, in fp64, so that a T that underflows
@@ -360,11 +432,11 @@ __device__ __forceinline__ void f_produce(uint8_t* smem, F_Bars* bars, volatile 
   named_bar_sync(3 + gi, 128);
 
   // ---- a2: Gram on the tensor pipe, then L_rj = beta_r Gram_rj (j < r) into s_a (the upper triangle as zeros)
-  if (gtid == 0) {
-    f_acc_acquire(&bars->acc_lock);
+  if (wq == 0) {
+    if (lane == 0) f_acc_acquire(&bars->acc_lock);
+    __syncwarp();
     tc_fence_after();
-    f_issue_gram(tmem, kt);
-    mma_commit(&bars->acc_done[gi]);
+    f_issue_gram(tmem + kF_ACC, kt, &bars->acc_done[gi]);
   }
   if (wq < 2) {  // Gram rows 0..63 sit in TMEM lanes 0..63: the two warps of the group that reach them
     s2_wait_warp(&bars->acc_done[gi], (2 * it) & 1, abort_flag, lane);
@@ -500,11 +572,11 @@ __device__ __forceinline__ void f_produce(uint8_t* smem, F_Bars* bars, volatile 
 
   // ---- W^t = K^t A_b^t on the tensor pipe: thread = dk index c' holds W[0..63][c']; packed as token pairs into row c'
   // of the slot's W tile ([dk][token], 128-byte rows, 128B swizzle: the MN-major B operand of (3))
-  if (gtid == 0) {
-    f_acc_acquire(&bars->acc_lock);
+  if (wq == 0) {
+    if (lane == 0) f_acc_acquire(&bars->acc_lock);
+    __syncwarp();
     tc_fence_after();
-    f_issue_w(tmem, kt, ab_tile);
-    mma_commit(&bars->acc_done[gi]);
+    f_issue_w(tmem + kF_ACC, kt, ab_tile, &bars->acc_done[gi]);
   }
   s2_wait_warp(&bars->acc_done[gi], (2 * it + 1) & 1, abort_flag, lane);
   tc_fence_after();
