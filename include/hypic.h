@@ -38,7 +38,8 @@ typedef enum {
   HYPIC_ERR_INVALID_ARG = 1, /* null / negative / inconsistent host-visible argument */
   HYPIC_ERR_UNSUPPORTED = 2, /* shape or dtype outside the built envelope (see each call) */
   HYPIC_ERR_WORKSPACE = 3,   /* workspace NULL or smaller than *_workspace() says */
-  HYPIC_ERR_CUDA = 4         /* a CUDA runtime/driver call failed (no device, launch error, ...) */
+  HYPIC_ERR_CUDA = 4,        /* a CUDA runtime/driver call failed (no device, launch error, ...) */
+  HYPIC_ERR_STATIC_SCRATCH = 5 /* hypic_segment_encode_static: the problem needs more scratch than the built-in array */
 } hypic_status_t;
 
 typedef enum { HYPIC_DT_F32 = 0, HYPIC_DT_BF16 = 1 } hypic_dtype_t;          /* dtype of k and v */
@@ -95,6 +96,28 @@ int hypic_segment_encode(const void* k, const void* v, const float* g, const flo
                          const int32_t* cu_seqlens, int32_t n_seg, int32_t t_total, int32_t H, int32_t dk,
                          int32_t dv, int kv_dtype, int gate, float* E, float* T, void* workspace,
                          size_t workspace_bytes, void* stream);
+
+/*
+ * hypic_segment_encode_static: hypic_segment_encode (same operation, Eq. 8; same arguments, layouts,
+ * envelope, results and error codes) for callers that cannot allocate device memory -- code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc.  The call takes NO workspace and allocates nothing (no
+ * cudaMalloc / cudaFree / allocating library routine): its scratch is a file-scope device array inside the library of
+ * hypic_static_scratch_bytes() = 4 MiB, held by every GPU that loads the library until the process exits.
+ *   - HYPIC_ERR_STATIC_SCRATCH when hypic_segment_encode_workspace(...) for these arguments exceeds
+ *     hypic_static_scratch_bytes() (the scalar-gate tensor family needs ~1 KB + 8 n_seg H + 8 (t_total / 64 + n_seg)
+ *     bytes: ~33 KB for four folded cfg2 layers; the per-channel gate's prep records, 40 KB per chunk and head, do not
+ *     fit beyond ~100 chunk-heads -- use hypic_segment_encode with a caller-owned workspace there).  Nothing is launched.
+ *   - The array is shared by every call on the device and keeps the previous call's contents; the call's first kernel
+ *     clears what must start at zero.  Calls that OVERLAP on the GPU (different streams without ordering between
+ *     them) race on it: issue them on one stream, or order the streams with events.  hypic_segment_encode with
+ *     caller-owned workspaces has no such restriction.
+ *   - The array's device address is looked up once per device (cudaGetSymbolAddress with that device current) on the
+ *     first call there; HYPIC_ERR_CUDA (hypic_last_cuda_error) if that fails.
+ */
+size_t hypic_static_scratch_bytes(void);
+int hypic_segment_encode_static(const void* k, const void* v, const float* g, const float* beta,
+                                const int32_t* cu_seqlens, int32_t n_seg, int32_t t_total, int32_t H, int32_t dk,
+                                int32_t dv, int kv_dtype, int gate, float* E, float* T, void* stream);
 
 /*
  * hypic_compose: for every request r and head h, fold  S <- S T_i + E_i  (Eq. 6, evaluated as

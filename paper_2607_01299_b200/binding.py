@@ -17,6 +17,7 @@ HYPIC_ERR_INVALID_ARG = 1
 HYPIC_ERR_UNSUPPORTED = 2
 HYPIC_ERR_WORKSPACE = 3
 HYPIC_ERR_CUDA = 4
+HYPIC_ERR_STATIC_SCRATCH = 5
 HYPIC_DT_F32 = 0
 HYPIC_DT_BF16 = 1
 HYPIC_GATE_SCALAR = 0
@@ -31,7 +32,7 @@ EXPORTS = (
     "hypic_compose_impl_for", "hypic_debug_timeout_count", "hypic_envelope_violation_count", "hypic_compose_f16",
     "hypic_tuple_pack_f16", "hypic_seam_window", "hypic_diag_encode", "hypic_diag_compose",
     "hypic_diag_encode_impl_for", "hypic_diag_compose_f16", "hypic_forward_encode", "hypic_rope_compose_workspace",
-    "hypic_rope_compose", "hypic_rope_compose_f16",
+    "hypic_rope_compose", "hypic_rope_compose_f16", "hypic_static_scratch_bytes", "hypic_segment_encode_static",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -67,6 +68,11 @@ def load_library() -> ctypes.CDLL:
     lib.hypic_segment_encode.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, ctypes.c_int, ctypes.c_int, vp,
                                          vp, vp, sz, vp]
     lib.hypic_segment_encode.restype = ctypes.c_int
+    lib.hypic_static_scratch_bytes.argtypes = []
+    lib.hypic_static_scratch_bytes.restype = sz
+    lib.hypic_segment_encode_static.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, ctypes.c_int, ctypes.c_int,
+                                                vp, vp, vp]
+    lib.hypic_segment_encode_static.restype = ctypes.c_int
     lib.hypic_compose.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp, vp]
     lib.hypic_compose.restype = ctypes.c_int
     lib.hypic_compose_f16.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp, vp]
@@ -223,6 +229,44 @@ def hypic_segment_encode(k: torch.Tensor, v: torch.Tensor, g: torch.Tensor, beta
             ws_bytes, _stream_handle(stream))
     if rc != HYPIC_OK:
         raise HypicError(rc, "hypic_segment_encode")
+    return E, T
+
+
+def hypic_static_scratch_bytes() -> int:
+    return int(load_library().hypic_static_scratch_bytes())
+
+
+def hypic_segment_encode_static(k: torch.Tensor, v: torch.Tensor, g: torch.Tensor, beta: torch.Tensor,
+                                cu_seqlens: torch.Tensor, gate: int, E: torch.Tensor, T: torch.Tensor, *,
+                                stream: Optional[torch.cuda.Stream] = None) -> Tuple[torch.Tensor, torch.Tensor]:
+    """hypic_segment_encode without a workspace and without any allocation: the scratch is a 4 MiB static device array
+    inside the library (include/hypic.h).  E:[n_seg,H,dv,dk] and T:[n_seg,H,dk,dk] fp32 are the CALLER's (this wrapper
+    allocates nothing either); raises HypicError(HYPIC_ERR_STATIC_SCRATCH) when the problem does not fit.  Calls that
+    overlap on the GPU race on the array."""
+    lib = load_library()
+    for name, t in (("k", k), ("v", v), ("g", g), ("beta", beta), ("cu_seqlens", cu_seqlens), ("E", E), ("T", T)):
+        if not t.is_cuda:
+            raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if k.dim() != 3 or v.dim() != 3 or k.shape[:2] != v.shape[:2] or k.dtype != v.dtype:
+        raise ValueError("k:[Ttot,H,dk] and v:[Ttot,H,dv] must agree in Ttot, H and dtype")
+    t_total, H, dk = (int(x) for x in k.shape)
+    dv = int(v.shape[2])
+    if k.dtype not in (torch.bfloat16, torch.float32):
+        raise ValueError(f"k/v must be bf16 or fp32, got {k.dtype}")
+    kv_dtype = HYPIC_DT_BF16 if k.dtype == torch.bfloat16 else HYPIC_DT_F32
+    want_g = (t_total, H) if gate == HYPIC_GATE_SCALAR else (t_total, H, dk)
+    if tuple(g.shape) != want_g or tuple(beta.shape) != (t_total, H):
+        raise ValueError(f"g must be {want_g} and beta {(t_total, H)}; got {tuple(g.shape)}, {tuple(beta.shape)}")
+    n_seg = int(cu_seqlens.numel()) - 1
+    if n_seg < 0 or tuple(E.shape) != (n_seg, H, dv, dk) or tuple(T.shape) != (n_seg, H, dk, dk):
+        raise ValueError("cu_seqlens / E / T have the wrong shape")
+    with torch.cuda.device(k.device):
+        rc = lib.hypic_segment_encode_static(
+            _dev_ptr(k, "k"), _dev_ptr(v, "v"), _dev_ptr(g, "g", torch.float32), _dev_ptr(beta, "beta", torch.float32),
+            _dev_ptr(cu_seqlens, "cu_seqlens", torch.int32), n_seg, t_total, H, dk, dv, kv_dtype, int(gate),
+            _dev_ptr(E, "E", torch.float32), _dev_ptr(T, "T", torch.float32), _stream_handle(stream))
+    if rc != HYPIC_OK:
+        raise HypicError(rc, "hypic_segment_encode_static")
     return E, T
 
 

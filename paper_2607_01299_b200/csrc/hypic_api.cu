@@ -292,6 +292,7 @@ const char* hypic_status_string(int status) {
     case HYPIC_ERR_UNSUPPORTED: return "unsupported shape or dtype";
     case HYPIC_ERR_WORKSPACE: return "workspace missing or too small";
     case HYPIC_ERR_CUDA: return "CUDA error";
+    case HYPIC_ERR_STATIC_SCRATCH: return "problem needs more scratch than the built-in static array holds (hypic_static_scratch_bytes)";
     default: return "unknown status";
   }
 }
