@@ -62,6 +62,7 @@ constexpr int kF_Smem = kF_OffBar + 512 + 1024;
 
 struct F_Bars {
   uint64_t k_full[kF_KStages], k_free[kF_KStages];  // TMA landed / both chains' (4) of the stage's chunk completed
+  uint64_t k_ready[kF_KStages];                     // the stage's K tile has been converted to fp16 (and a ragged tail zeroed)
   uint64_t v_full[kF_VStages], v_free[kF_VStages];  // TMA landed / (1) of the stage's chunk completed
   uint64_t out_full[kF_Slots], out_free[kF_Slots];  // producer group done (4 warps) / (1) and both (3) completed
   uint64_t gate_full[kF_GateSlots];                 // loader wrote the chunk's gate record
@@ -408,27 +409,12 @@ __device__ __forceinline__ void f_produce(uint8_t* smem, F_Bars* bars, volatile 
   const uint32_t acc_t = tmem + kF_ACC + ((uint32_t)(32 * wq) << 16);
   const int it = c >> 1;  // this group's chunk counter: phase of acc_done is 2 it (Gram), 2 it + 1 (W)
 
-  // ---- K tile bf16 -> fp16 in place (16-byte pieces; piece p of a box: row = token p / 8), rows past the segment zeroed
-#pragma unroll 1
-  for (int i0 = 0; i0 < 8; i0 += 4) {
-    uint4 w[4];
-#pragma unroll
-    for (int j = 0; j < 4; ++j) w[j] = lds128(kt + 16 * (gtid + 128 * (i0 + j)));
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const int tok = ((gtid + 128 * (i0 + j)) & 511) >> 3;
-      uint4 o = cvt8_bf16_f16(w[j]);
-      if (tok >= valid) o = make_uint4(0u, 0u, 0u, 0u);
-      sts128(kt + 16 * (gtid + 128 * (i0 + j)), o);
-    }
-  }
   if (gtid < kC) {  // beta and the value weights f_j of the lazy decay
     const float bj = gr[kC + gtid], Gj = gr[gtid];
     const float p_old = gr[2 * kC], GC = gr[2 * kC + 2], rs = gr[2 * kC + 3];
     s_b[gtid] = bj;
     s_bf[gtid] = bj * (rs != 0.f ? expf(GC - Gj) : expf(-(p_old + Gj)));
   }
-  fence_proxy_async();  // the fp16 K tile must be visible to the tensor pipe's reads
   named_bar_sync(3 + gi, 128);
 
   // ---- a2: Gram on the tensor pipe, then L_rj = beta_r Gram_rj (j < r) into s_a (the upper triangle as zeros)
@@ -626,6 +612,7 @@ __global__ void __launch_bounds__(kF_Threads, 1)  // 18 warps = 5 on two of the 
     for (int i = 0; i < kF_KStages; ++i) {
       mbar_init(&bars->k_full[i], 1);
       mbar_init(&bars->k_free[i], 2);
+      mbar_init(&bars->k_ready[i], 1);
     }
     for (int i = 0; i < kF_VStages; ++i) {
       mbar_init(&bars->v_full[i], 1);
@@ -746,25 +733,53 @@ __global__ void __launch_bounds__(kF_Threads, 1)  // 18 warps = 5 on two of the 
       flag_release(&bars->fin_flag, 1);
     }
   } else if (warp == kF_WIssuer) {
-    // ------------------------------------------------------------------------------------------- V helper
-    // Walks the V tiles in order (every phase of v_full is waited for: a parity wait must never skip one).  The ragged
-    // last chunk's V box also holds tokens of the next segment: this warp zeroes those rows, so that nothing of a
-    // neighbour -- not even an Inf or NaN -- reaches the unit through 0 x garbage; then the tile is released to (1).
+    // ------------------------------------------------------------------------------------------- converter
+    // Walks the tiles in the loader's order (K of chunk c, then V of chunk c - 2; every phase of k_full / v_full is waited
+    // for: a parity wait must never skip one).  K: bf16 -> fp16 in place (element-wise on 16-bit lanes, so the 128B swizzle
+    // of the TMA boxes is untouched), two chunks ahead of the producers' need.  V stays bf16.  The ragged last chunk's
+    // boxes also hold tokens of the next segment: those rows are zeroed in both tiles, so that nothing of a neighbour --
+    // not even an Inf or NaN -- reaches the unit through 0 x garbage.
 #pragma unroll 1
-    for (int c = 0; c < nc; ++c) {
-      const int slot = c & 1;
-      const int valid = min(kC, seg_len - c * kC);
-      const uint32_t vt = smem_base + kF_OffV + slot * 2 * kTileB;
-      f_wait_lazy(&bars->v_full[slot], (c >> 1) & 1, abort_flag);
-      if (valid < kC) {
+    for (int c = 0; c < nc + 2; ++c) {
+      if (c < nc) {
+        const int kst = c % kF_KStages;
+        const int valid = min(kC, seg_len - c * kC);
+        const uint32_t kt = smem_base + kF_OffK + kst * 2 * kTileB;
+        f_wait_lazy(&bars->k_full[kst], (c / kF_KStages) & 1, abort_flag);
 #pragma unroll 1
-        for (int p = lane; p < 1024; p += 32)  // 16-byte piece p of the tile: token (p % 512) / 8
-          if (((p & 511) >> 3) >= valid) sts128(vt + 16 * p, make_uint4(0u, 0u, 0u, 0u));
-        fence_proxy_async();
+        for (int i0 = 0; i0 < 32; i0 += 8) {  // 16-byte piece p of the tile: token (p % 512) / 8
+          uint4 w[8];
+#pragma unroll
+          for (int j = 0; j < 8; ++j) w[j] = lds128(kt + 16 * (lane + 32 * (i0 + j)));
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            const int p = lane + 32 * (i0 + j);
+            uint4 o = cvt8_bf16_f16(w[j]);
+            if (((p & 511) >> 3) >= valid) o = make_uint4(0u, 0u, 0u, 0u);
+            sts128(kt + 16 * p, o);
+          }
+        }
+        fence_proxy_async();  // the fp16 K tile must be visible to the tensor pipe's reads
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars->k_ready[kst]);
+        __syncwarp();
       }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&bars->v_ok[slot]);
-      __syncwarp();
+      const int cv = c - 2;
+      if (cv >= 0) {
+        const int slot = cv & 1;
+        const int valid = min(kC, seg_len - cv * kC);
+        const uint32_t vt = smem_base + kF_OffV + slot * 2 * kTileB;
+        f_wait_lazy(&bars->v_full[slot], (cv >> 1) & 1, abort_flag);
+        if (valid < kC) {
+#pragma unroll 1
+          for (int p = lane; p < 1024; p += 32)
+            if (((p & 511) >> 3) >= valid) sts128(vt + 16 * p, make_uint4(0u, 0u, 0u, 0u));
+          fence_proxy_async();
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars->v_ok[slot]);
+        __syncwarp();
+      }
     }
   } else if (warp >= kF_WProd) {
     // ------------------------------------------------------------------------------------------- producers
@@ -773,7 +788,7 @@ __global__ void __launch_bounds__(kF_Threads, 1)  // 18 warps = 5 on two of the 
     for (int c = gi; c < nc; c += 2) {
       const int kst = c % kF_KStages;
       f_wait_lazy(&bars->gate_full[c & (kF_GateSlots - 1)], (c / kF_GateSlots) & 1, abort_flag);
-      f_wait_lazy(&bars->k_full[kst], (c / kF_KStages) & 1, abort_flag);
+      f_wait_lazy(&bars->k_ready[kst], (c / kF_KStages) & 1, abort_flag);
       f_produce(smem, bars, abort_flag, tmem, gi, gtid, warp & 3, c, min(kC, seg_len - c * kC),
                 smem_base + kF_OffK + kst * 2 * kTileB, smem_base + kF_OffOut + (c & 1) * kF_OutBytes);
     }
