@@ -717,7 +717,7 @@ def run_ours(args):
                                      None if per_layer is None else per_layer * G)
         roofline["traffic_source"] = tj.get("source", "profiles/traffic.json (a committed ncu capture, not this run)")
     alg_bytes = th_per_launch * ENC_BYTES_PER_TOKEN_HEAD + N_SEG * H * G * COMPOSE_BYTES_PER_STEP
-    roofline.update({"kernel": ("hypic_segment_encode = chunk_offsets_kernel + scan3_kernel (tensor family, scalar gate: "
+    roofline.update({"kernel": ("hypic_segment_encode = chunk_offsets_kernel + scan4_kernel (tensor family, scalar gate: "
                                 "one fused tcgen05 kernel; the fp32 fallback-list kernel runs empty)") if fam == "tensor" else
                      "hypic_segment_encode = encode_simt_kernel (simt family)",
                      "units_per_launch": f"{th_per_launch} token-heads x {ENC_FLOP_PER_TOKEN_HEAD} flop",

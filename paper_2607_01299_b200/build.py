@@ -21,7 +21,7 @@ OBJ_DIR = os.path.join(HERE, "build")
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
     "--expt-relaxed-constexpr", "-I", INCLUDE,
-]
+] + os.environ.get("HYPIC_NVCC_EXTRA", "").split()
 
 
 def _nvcc() -> str:

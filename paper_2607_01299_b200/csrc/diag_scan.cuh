@@ -327,7 +327,7 @@ __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(addr));
   return v;
 }
-// sts32: encode_scan3.cuh
+// sts32: encode_scan4.cuh
 
 __global__ void __launch_bounds__(kDtThreads, 3)
     diag_scan_ch_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,

@@ -1,0 +1,778 @@
+// encode_scan4.cuh -- the fused segment-encode kernel of the tensor family, scalar gate (GDN row of Table 1),
+// in the REVERSE (suffix-product) chunk form.  Included by encode_tensor.cu inside namespace hypic::{anonymous}; uses the
+// helpers of encode_prep.cuh / encode_scan2.cuh.
+//
+// One CTA per (segment, head) does rows a0..a5 of SURVEY.md section 8(a), walking the segment's 64-token chunks LAST CHUNK
+// FIRST.  Algebra.  The scalar gate commutes with (I - beta k k^t): with w_t = exp(sum_{s > t} g_s) the
+// decay a token's contribution still sees,
+//     T_C = exp(sum g) prod_t (I - beta_t k_t k_t^t)            (ordered, first token leftmost; Eq. 4)
+//     E   = sum_t w_t beta_t v_t k_t^t prod_{s > t} (I - beta_s k_s k_s^t)
+// and per chunk c the ungated WY/UT form gives  prod_{t in c} (I - beta k k^t) = P_c = I - K^t A_b^t K,  with
+//     L_rj = beta_r (k_r . k_j) (j < r),  A = (I + L)^-1,  A_b = A diag(beta),  W' = A_b^t K  (all state-independent),
+// and the chunk's own end state  V^t diag(w) A_b^t K.  With the SUFFIX product R_c = P_{c+1} ... P_n (R_n = I):
+//     Y_c = W'_c R_c             (64 x dk)     the only product that reads the state
+//     R_{c-1} = R_c - K_c^t Y_c                 T = exp(sum g) R_0
+//     E += (diag(w) V_c)^t Y_c                  E is a pure accumulator: never read back, never rescaled
+// Against the forward form (X = [E ; T] <- X + ([U^t ; 0] - X W^t) K: two 128-row blocks through two dependent
+// contractions each) the state-reading product is one M = 128 block instead of two, the value contraction V^t A_b^t
+// disappears, E needs no fp16 copy of itself, and the weights w_t <= 1 are known when a chunk arrives, so there is no
+// decay bookkeeping at all (no envelope, no lazy rescale): 28 MMAs per chunk instead of 44.
+//
+// The state is held transposed, R^t, so that TMEM lane j = column j of R: columns evolve independently under the left
+// multiplication by P_c, each lane carries its own power-of-two scale (re-chosen every 8th chunk, maximum to
+// [2^11, 2^12)) and the contractions have the shapes
+//     (3') DY   = Rh W'^t          M = 128 (j), N = 64 (token), K = 128: A = Rh = fp16(R^t) from TMEM, B = the W' tile
+//     (4') R^t -= U'' K            M = 128 (j), N = 128, K = 64:        A = U'' = fp16(DY) from TMEM, B = the K tile
+//     (5)  E   += V^t (w Y)        M = 128 (dv), N = 128 (j), K = 64:   A = the V tile (MN-major), B = fY tile (shared)
+// with fY[j][t] = fp16(w_t 2^-s_j DY[j][t]) written by the epilogue threads as a K-major B tile.
+// Producer groups (G) Gram = K K^t and (W) W'^t = K^t A_b on tcgen05 as before; the blocked UT inverse on mma.sync.
+//
+// TMEM columns: R^t [0,128), E [128,256), Rh / U'' [256,320), DY [320,384), ACC0 [384,448), ACC1 [448,512) (one
+// accumulator per producer group: no lock).
+//
+// 16 warps (512 threads, 128 registers each):
+//   warps 0-3    chain      thread = lane j: pass Rh = fp16(R^t), epilogue U'' / fY; warp 0 issues (3'), (4'), (5)
+//   warp 4       loader     TMA boxes of K (6-deep ring, two chunks ahead of V) and V (2-deep ring)
+//   warp 5       gate       the chunk's g / beta, the weights w_t (suffix scan), a ring of 8 gate records
+//   warp 6, 7    converters K / V tile bf16 -> fp16 in place; the rows of the ragged last tile zeroed
+//   warps 8-11   producer group 0 (even iterations), warps 12-15 producer group 1 (odd iterations)
+#pragma once
+
+constexpr int kR_Groups = 2;
+constexpr int kR_Threads = 32 * (8 + 4 * kR_Groups);
+constexpr int kR_WChain = 0, kR_WLoader = 4, kR_WGate = 5, kR_WConv = 6, kR_WConvV = 7, kR_WProd = 8;
+constexpr int kR_KStages = 6, kR_VStages = 2, kR_GateSlots = 8;
+constexpr int kR_OffK = 0;                                        // 4 x 16 KB: K tile, two 64-column boxes [token][64]
+constexpr int kR_OffV = kR_OffK + kR_KStages * 2 * kTileB;        // 2 x 16 KB: V tile (bf16 as it arrives)
+constexpr int kR_OffOut = kR_OffV + kR_VStages * 2 * kTileB;      // one 16 KB W' tile per producer group
+constexpr int kR_OffFy = kR_OffOut + kR_Groups * 2 * kTileB;      // 16 KB: fY tile [j][token]
+constexpr int kR_OffAb = kR_OffFy + 2 * kTileB;                   // one 8 KB A_b tile per producer group
+constexpr int kR_OffScr = kR_OffAb + kR_Groups * kTileB;          // producer scratch per group
+constexpr int kR_ScrL = 0;                                        // fp16 L [64][64]: 128-byte rows, 16-byte pieces ^ (row & 7)
+constexpr int kR_DPitch = 48;                                     // bytes per row of a 16 x 16 fp16 block (conflict-free ldmatrix)
+constexpr int kR_ScrD = kTileB;                                   // fp16 D_i = (I + L_ii)^-1, 4 x [16][24]
+constexpr int kR_ScrT = kR_ScrD + 4 * 16 * kR_DPitch;             // fp16 temporaries of the strips, one [16][24] per warp
+constexpr int kR_ScrB = kR_ScrT + 4 * 16 * kR_DPitch;             // fp32 [64] beta
+constexpr int kR_ScrBytes = kR_ScrB + 256;
+constexpr int kR_OffGate = kR_OffScr + kR_Groups * kR_ScrBytes;   // 8 x gate record: w_t[64], beta_t[64]
+constexpr int kR_GateFloats = 2 * kC;
+constexpr int kR_OffBar = kR_OffGate + kR_GateSlots * kR_GateFloats * 4;
+constexpr int kR_Smem = kR_OffBar + 512 + 1024;
+constexpr uint32_t kR_ColR = 0, kR_ColE = 128, kR_ColH = 256, kR_ColDY = 320, kR_ColACC = 384;
+
+struct R_Bars {
+  uint64_t k_full[kR_KStages], k_free[kR_KStages];  // TMA landed / (4') of the stage's chunk completed
+  uint64_t k_ready[kR_KStages];                     // the stage's K tile is fp16 (and a ragged tail zeroed)
+  uint64_t v_full[kR_VStages], v_free[kR_VStages];  // TMA landed / (5) of the stage's chunk completed
+  uint64_t v_ok[kR_VStages];                        // the V tile has landed and a ragged tail is zeroed
+  uint64_t out_full[kR_Groups], out_free[kR_Groups];  // the group's W' tile is written (4 warps) / (3') has read it
+  uint64_t gate_full[kR_GateSlots];                 // the gate warp wrote the chunk's record
+  uint64_t m3_done, m4_done, e_done;                // (3') / (4') / (5) of the current chunk completed
+  uint64_t acc_done[kR_Groups];                     // the group's MMAs into its ACC have completed
+  int fin_flag;                                     // the gate warp has posted g_total
+  uint32_t tmem_base;
+  int abort_flag;
+  int bad;
+  double g_total;
+};
+static_assert(sizeof(R_Bars) <= 512, "barrier block");
+
+__device__ __forceinline__ void sts32(uint32_t a, uint32_t v) { asm volatile("st.shared.b32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+
+// Waits of the background roles (producers, loader, gate, converters): they run chunks ahead of the chain, so a late
+// wake-up costs nothing, while a tight probe loop takes issue slots from the warps on the critical path.
+__device__ __forceinline__ void f_wait_lazy(uint64_t* bar, uint32_t parity, volatile int* abort_flag) {
+#pragma unroll 1
+  for (int i = 0; i < 200000; ++i) {
+    if (mbar_try_wait(bar, parity)) return;
+    __nanosleep(500);
+  }
+  s2_wait(bar, parity, abort_flag);
+}
+
+// ---- MMA bursts.  Each is ONE asm block executed by a whole converged warp (warp-uniform control flow): one elected lane
+// issues, descriptors and TMEM addresses advance inside the block, and the commits ride along.  Issued from a
+// lane-divergent branch (`if (lane == 0)`), ptxas wraps every tcgen05.mma in an ELECT / R2UR.BROADCAST x 5 / branch
+// loop of ~21 dependent instructions -- ~100 cycles of issue time per MMA; in this form the UTCHMMAs come out back to
+// back on the uniform datapath.
+// Descriptor arithmetic: the low 14 bits hold (address >> 4); steps used: 16 rows of a 128-byte-row tile = 2048 B =
+// +128, 32 B inside a row = +2, the next 64-column box = 8192 B = +512.
+#define F_MMA_TS "@P tcgen05.mma.cta_group::1.kind::f16 [%0], [at], bd, %3, Q;\n\t"
+#define F_MMA_SS "@P tcgen05.mma.cta_group::1.kind::f16 [%0], ad, bd, %3, Q;\n\t"
+#define F_COMMIT(n) "@P tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%" #n "];\n\t"
+// (G): ACC[0:64, 0:64] = K K^t -- A = B = the fp16 K tile, K-major, two 64-column boxes.  M = 128: the A rows 64..127 run
+// on into whatever follows the 64-row box (valid shared memory); their results land in TMEM lanes 64..127 and are never
+// read.  An M = 64 instruction costs the same tensor time.  Commits to the group's acc_done.
+__device__ __forceinline__ void f_issue_gram(uint32_t d_tmem, uint32_t k_tile, uint64_t* bar0) {
+  constexpr uint32_t idg = make_idesc(0u, 128, 64, 0, 0);
+  const uint64_t d0 = make_desc(k_tile, 16, 1024, 2);
+  asm volatile(
+      "{\n\t.reg .pred P, Q;\n\t.reg .b64 ad, bd;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "setp.ne.b32 Q, 0, 0;\n\t"
+      "mov.b64 ad, %1;\n\tmov.b64 bd, %1;\n\t" F_MMA_SS
+      "setp.ne.b32 Q, 1, 0;\n\t"
+      "add.s64 ad, ad, 2;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 2;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 2;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 506;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 2;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 2;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 2;\n\tmov.b64 bd, ad;\n\t" F_MMA_SS
+      F_COMMIT(2)
+      "}" ::"r"(d_tmem), "l"(d0), "r"(smem_u32(bar0)), "r"(idg)
+      : "memory");
+}
+// (3'): DY = Rh W'^t -- A = Rh from TMEM (8 columns per k-step), B = the W' tile [dk][token] (MN-major); commits to
+// m3_done and to the group's out_free
+__device__ __forceinline__ void r_issue3(uint32_t d_tmem, uint32_t a_tmem, uint32_t w_tile, uint64_t* bar0, uint64_t* bar1) {
+  constexpr uint32_t id3 = make_idesc(0u, 128, 64, 0, 1);
+  const uint64_t bd0 = make_desc(w_tile, 8192, 1024, 2);
+  asm volatile(
+      "{\n\t.reg .pred P, Q;\n\t.reg .b64 bd;\n\t.reg .b32 at;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "setp.ne.b32 Q, 0, 0;\n\t"
+      "mov.b64 bd, %2;\n\tmov.b32 at, %1;\n\t" F_MMA_TS
+      "setp.ne.b32 Q, 1, 0;\n\t"
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      F_COMMIT(4) F_COMMIT(5)
+      "}" ::"r"(d_tmem), "r"(a_tmem), "l"(bd0), "r"(id3), "r"(smem_u32(bar0)), "r"(smem_u32(bar1))
+      : "memory");
+}
+// (4'): R^t -= U'' K -- A = U'' from TMEM, B = the K tile (MN-major, two 64-column boxes), negated by the instruction
+// descriptor; commits to m4_done and k_free
+__device__ __forceinline__ void r_issue4(uint32_t d_tmem, uint32_t a_tmem, uint32_t k_tile, uint64_t* bar0, uint64_t* bar1) {
+  constexpr uint32_t id4 = make_idesc(0u, 128, 128, 0, 1, 0, 1);
+  const uint64_t bd0 = make_desc(k_tile, 8192, 1024, 2);
+  asm volatile(
+      "{\n\t.reg .pred P, Q;\n\t.reg .b64 bd;\n\t.reg .b32 at;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "setp.ne.b32 Q, 1, 0;\n\t"
+      "mov.b64 bd, %2;\n\tmov.b32 at, %1;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      "add.s64 bd, bd, 128;\n\tadd.s32 at, at, 8;\n\t" F_MMA_TS
+      F_COMMIT(4) F_COMMIT(5)
+      "}" ::"r"(d_tmem), "r"(a_tmem), "l"(bd0), "r"(id4), "r"(smem_u32(bar0)), "r"(smem_u32(bar1))
+      : "memory");
+}
+// (5): E (+)= V^t fY^t -- A = the fp16 V tile (MN-major, +128 per 16 tokens), B = the fY tile [j][token] (K-major fp16, +2
+// per 16 tokens); commits to v_free and e_done.  (A kind::f16 instruction with a bf16 A and an fp16 B operand -- V as TMA
+// delivers it -- is an illegal instruction on sm_100a: hence the V converter warp.)
+__device__ __forceinline__ void r_issue5(uint32_t d_tmem, uint32_t v_tile, uint32_t fy_tile, uint32_t acc_first, uint64_t* bar0,
+                                         uint64_t* bar1) {
+  constexpr uint32_t id5 = make_idesc(0u, 128, 128, 1, 0);
+  const uint64_t ad0 = make_desc(v_tile, 8192, 1024, 2), bd0 = make_desc(fy_tile, 16, 1024, 2);
+  asm volatile(
+      "{\n\t.reg .pred P, Q;\n\t.reg .b64 ad, bd;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "setp.ne.b32 Q, %4, 0;\n\t"
+      "mov.b64 ad, %1;\n\tmov.b64 bd, %2;\n\t" F_MMA_SS
+      "setp.ne.b32 Q, 1, 0;\n\t"
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      F_COMMIT(5) F_COMMIT(6)
+      "}" ::"r"(d_tmem), "l"(ad0), "l"(bd0), "r"(id5), "r"(acc_first), "r"(smem_u32(bar0)), "r"(smem_u32(bar1))
+      : "memory");
+}
+// (W'): ACC = K^t A_b = W'^t -- A = the K tile MN-major (+128 per 16 tokens), B = the A_b tile [j][r] read MN-major
+// (+128 per 16 rows j); commits to the group's acc_done
+__device__ __forceinline__ void r_issue_w(uint32_t d_tmem, uint32_t k_tile, uint32_t ab_tile, uint64_t* bar0) {
+  constexpr uint32_t idw = make_idesc(0u, 128, 64, 1, 1);
+  const uint64_t ad0 = make_desc(k_tile, 8192, 1024, 2), bd0 = make_desc(ab_tile, 8192, 1024, 2);
+  asm volatile(
+      "{\n\t.reg .pred P, Q;\n\t.reg .b64 ad, bd;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "setp.ne.b32 Q, 0, 0;\n\t"
+      "mov.b64 ad, %1;\n\tmov.b64 bd, %2;\n\t" F_MMA_SS
+      "setp.ne.b32 Q, 1, 0;\n\t"
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 128;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 128;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 128;\n\t" F_MMA_SS
+      F_COMMIT(4)
+      "}" ::"r"(d_tmem), "l"(ad0), "l"(bd0), "r"(idw), "r"(smem_u32(bar0))
+      : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------------- chain
+__device__ __forceinline__ void r_chain(uint8_t* smem, R_Bars* bars, volatile int* abort_flag, uint32_t tmem, int cw, int lane,
+                                        int nc, float* __restrict__ E_dst, float* __restrict__ T_dst) {
+  const int wq = cw & 3;  // a warp reaches the TMEM lane quarter warp id % 4; the chain's four warps cover all four
+  const int row = 32 * wq + lane;
+  const uint32_t lane_base = (uint32_t)(32 * wq) << 16;
+  const uint32_t tR = tmem + kR_ColR + lane_base, tE = tmem + kR_ColE + lane_base, tH = tmem + kR_ColH + lane_base,
+                 tD = tmem + kR_ColDY + lane_base;
+  const uint32_t smem_base = smem_u32(smem);
+  const uint32_t fy_row = smem_base + kR_OffFy + (row >> 3) * 1024 + (row & 7) * 128;
+  const uint32_t gate_base = smem_base + kR_OffGate;
+  int s_exp = 0;        // the TMEM copy of this lane is (column `row` of R) * 2^s_exp
+  float unscale = 1.f;  // 2^-s_exp (0 once the column has shrunk below the fp32 range: its contributions to E vanish)
+  const bool issue_warp = (cw == kR_WChain);  // warp-uniform: the bursts elect their lane
+
+  // R_n^t = I
+#pragma unroll
+  for (int cb = 0; cb < 4; ++cb) {
+    uint32_t x[32];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) x[i] = (32 * cb + i == row) ? __float_as_uint(1.f) : 0u;
+    tmem_st32(tR + 32 * cb, x);
+  }
+  tmem_st_wait();
+
+#pragma unroll 1
+  for (int it = 0; it < nc; ++it) {
+    const int gi = it % kR_Groups, kst = it % kR_KStages, vst = it % kR_VStages;
+    s2_wait_warp(&bars->out_full[gi], (it / kR_Groups) & 1, abort_flag, lane);  // W' and the fp16 K tile are in place
+    if (it > 0) s2_wait_warp(&bars->m4_done, (it - 1) & 1, abort_flag, lane);
+    tc_fence_after();
+    // ---- pass: Rh = fp16(R^t), 32 columns at a time; R^t itself is only rewritten when the lane's scale is re-chosen
+    {
+      float f = 1.f;
+      const bool rewrite = (it & 7) == 0;
+      if (rewrite) {  // the whole column of R lives in this thread: maximum -> power-of-two scale
+        float m = 0.f;
+#pragma unroll 1
+        for (int cb = 0; cb < 4; ++cb) {
+          uint32_t x[32];
+          tmem_ld32(tR + 32 * cb, x);
+          tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 32; ++i) m = fmaxf(m, fabsf(__uint_as_float(x[i])));
+        }
+        const int e = (int)((__float_as_uint(m) >> 23) & 0xffu);  // maximum in [2^(e-127), 2^(e-126))
+        int dlt = (e == 0 || e == 255) ? 0 : 138 - e;             // -> [2^11, 2^12)
+        dlt = max(-100, min(100, dlt));
+        s_exp += dlt;
+        f = pow2i(dlt);
+        unscale = (s_exp > 126) ? 0.f : pow2i(max(-126, -s_exp));
+      }
+      {
+        uint32_t xa[32], xb[32], hh[16];
+        tmem_ld32(tR, xa);
+#pragma unroll
+        for (int cb = 0; cb < 4; cb += 2) {  // the next 32 columns are in flight while these are converted
+          tmem_ld_wait();
+          tmem_ld32(tR + 32 * (cb + 1), xb);
+          if (rewrite) {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) mul2(xa[2 * j], xa[2 * j + 1], f);
+            tmem_st32(tR + 32 * cb, xa);  // (3') reads Rh alone; (4') of this chunk is issued after the chain barrier below
+          }
+#pragma unroll
+          for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(xa[2 * j]), __uint_as_float(xa[2 * j + 1]));
+          tmem_st16(tH + 16 * cb, hh);
+          tmem_ld_wait();
+          if (cb + 2 < 4) tmem_ld32(tR + 32 * (cb + 2), xa);
+          if (rewrite) {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) mul2(xb[2 * j], xb[2 * j + 1], f);
+            tmem_st32(tR + 32 * (cb + 1), xb);
+          }
+#pragma unroll
+          for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(xb[2 * j]), __uint_as_float(xb[2 * j + 1]));
+          tmem_st16(tH + 16 * (cb + 1), hh);
+        }
+      }
+      tmem_st_wait();
+      tc_fence_before();
+      named_bar_sync(1, 128);  // the whole chain has written Rh
+      if (issue_warp) {
+        tc_fence_after();
+        r_issue3(tmem + kR_ColDY, tmem + kR_ColH, smem_base + kR_OffOut + gi * 2 * kTileB, &bars->m3_done, &bars->out_free[gi]);
+      }
+    }
+    // ---- epilogue: U'' = fp16(DY) -> TMEM (A operand of (4')), tokens [32 cb, 32 cb + 32) -> columns [16 cb, 16 cb + 16);
+    // fY = fp16(w_t 2^-s DY) -> row `row` of the shared fY tile (B operand of (5); 128-byte rows, 128B swizzle).  The tile
+    // is single-buffered: (5) of the previous chunk sits in front of this chunk's (3') in the in-order tensor pipe, so it
+    // has completed when m3_done fires.
+    s2_wait_warp(&bars->m3_done, it & 1, abort_flag, lane);
+    tc_fence_after();
+    {
+      const uint32_t gw = gate_base + (it & (kR_GateSlots - 1)) * kR_GateFloats * 4;
+#pragma unroll
+      for (int hb = 0; hb < 2; ++hb) {
+        uint32_t y[32], u[16];
+        uint4 wq4[8];
+        tmem_ld32(tD + 32 * hb, y);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) wq4[q] = lds128(gw + (32 * hb + 4 * q) * 4);  // the 32 weights, under the TMEM load
+        tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 16; ++j) u[j] = pack_f16(__uint_as_float(y[2 * j]), __uint_as_float(y[2 * j + 1]));
+        tmem_st16(tH + 16 * hb, u);
+#pragma unroll
+        for (int p8 = 0; p8 < 4; ++p8) {  // tokens 32 hb + 8 p8 .. + 7 -> 16-byte piece 4 hb + p8 of the row
+          uint32_t wv[8] = {wq4[2 * p8].x, wq4[2 * p8].y, wq4[2 * p8].z, wq4[2 * p8].w,
+                            wq4[2 * p8 + 1].x, wq4[2 * p8 + 1].y, wq4[2 * p8 + 1].z, wq4[2 * p8 + 1].w};
+          uint32_t o[4];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            mul2(wv[2 * q], wv[2 * q + 1], unscale);
+            mul2v(y[8 * p8 + 2 * q], y[8 * p8 + 2 * q + 1], __uint_as_float(wv[2 * q]), __uint_as_float(wv[2 * q + 1]));
+            o[q] = pack_f16(__uint_as_float(y[8 * p8 + 2 * q]), __uint_as_float(y[8 * p8 + 2 * q + 1]));
+          }
+          sts128(fy_row + (((4 * hb + p8) ^ (row & 7)) << 4), make_uint4(o[0], o[1], o[2], o[3]));
+        }
+      }
+    }
+    tmem_st_wait();
+    tc_fence_before();
+    fence_proxy_async();     // the fY tile must be visible to the tensor pipe's reads
+    named_bar_sync(1, 128);  // the whole chain has written U'' and fY
+    if (issue_warp) {
+      tc_fence_after();
+      r_issue4(tmem + kR_ColR, tmem + kR_ColH, smem_base + kR_OffK + kst * 2 * kTileB, &bars->m4_done, &bars->k_free[kst]);
+      s2_wait_warp(&bars->v_ok[vst], (it / kR_VStages) & 1, abort_flag, lane);
+      tc_fence_after();
+      r_issue5(tmem + kR_ColE, smem_base + kR_OffV + vst * 2 * kTileB, smem_base + kR_OffFy, it > 0 ? 1u : 0u,
+                       &bars->v_free[vst], &bars->e_done);
+    }
+  }
+
+  // ---- a5.  T = exp(sum g) R_0: lane j holds column j of R, so for every row i the chain's 128 threads write 512
+  // contiguous bytes; the gate and the lane's scale are applied in fp64, so that a T that underflows fp32 underflows
+  // exactly like the correctly rounded result.  E: thread = row of the accumulator.
+  s2_wait_count(&bars->fin_flag, 0, abort_flag);  // the gate warp has posted g_total
+  if (nc > 0) {
+    s2_wait_warp(&bars->e_done, (nc - 1) & 1, abort_flag, lane);  // the last (5), and with it every MMA before it
+    tc_fence_after();
+  }
+  bool bad = false;
+  {
+    const double sc = exp(bars->g_total - 0.6931471805599453 * (double)s_exp);
+#pragma unroll 1
+    for (int cb = 0; cb < 4; ++cb) {
+      uint32_t x[32];
+      tmem_ld32(tR + 32 * cb, x);
+      tmem_ld_wait();
+#pragma unroll
+      for (int i = 0; i < 32; ++i) {
+        const float o = (float)((double)__uint_as_float(x[i]) * sc);
+        bad |= !(fabsf(o) <= 3.0e38f);
+        T_dst[(size_t)(32 * cb + i) * kD + row] = o;
+      }
+    }
+  }
+  {
+    float* dst = E_dst + (size_t)row * kD;
+#pragma unroll 1
+    for (int cb = 0; cb < 4; ++cb) {
+      uint32_t x[32];
+      if (nc > 0) {
+        tmem_ld32(tE + 32 * cb, x);
+        tmem_ld_wait();
+      } else {
+#pragma unroll
+        for (int i = 0; i < 32; ++i) x[i] = 0u;
+      }
+      float4* d4 = reinterpret_cast<float4*>(dst + 32 * cb);
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        float4 o;
+        o.x = __uint_as_float(x[4 * u]);
+        o.y = __uint_as_float(x[4 * u + 1]);
+        o.z = __uint_as_float(x[4 * u + 2]);
+        o.w = __uint_as_float(x[4 * u + 3]);
+        bad |= !(fabsf(o.x) <= 3.0e38f) | !(fabsf(o.y) <= 3.0e38f) | !(fabsf(o.z) <= 3.0e38f) | !(fabsf(o.w) <= 3.0e38f);
+        d4[u] = o;
+      }
+    }
+  }
+  if (bad) bars->bad = 1;  // an fp16 operand overflowed somewhere: the unit goes to the fp32 fallback list
+}
+
+// ---------------------------------------------------------------------------------------------------- producers
+__device__ __forceinline__ void sts16(uint32_t a, uint16_t v) { asm volatile("st.shared.b16 [%0], %1;" ::"r"(a), "h"(v) : "memory"); }
+__device__ __forceinline__ uint16_t f16_bits(float x) { return __half_as_ushort(__float2half_rn(x)); }
+__device__ __forceinline__ float f16lo(uint32_t w) { return __half2float(__ushort_as_half((uint16_t)(w & 0xffffu))); }
+__device__ __forceinline__ float f16hi(uint32_t w) { return __half2float(__ushort_as_half((uint16_t)(w >> 16))); }
+
+// One chunk of the state-independent half, by one group of four warps (gtid = 0..127; `wq` = the TMEM lane quarter the
+// warp can reach):
+//   G  Gram = K K^t (tcgen05) of the fp16 K tile `kt`; L_rj = beta_r Gram_rj (j < r) as an fp16 tile in shared memory
+//   D  warp w: D_w = (I + L_ww)^-1 by forward substitution (fp32, lane = column), stored as fp16
+//   S  warp j: block column j of A_b = (I + L)^-1 diag(beta):  A_b[jj] = D_j diag(beta_j),
+//      A_b[ij] = -D_i sum_{k=j}^{i-1} L_ik A_b[kj]  (i > j; a right scaling commutes with the recursion).  A block column
+//      depends only on L, the D_i and its own earlier blocks, so the four warps run without a barrier; operands come from
+//      shared memory by ldmatrix, products are single-pass fp16 mma.sync (A_b only feeds a 16-bit tile).
+//   W  W'^t = K^t A_b (tcgen05) -> the MN-major W' tile of (3') in the group's output slot.
+// `it` = the chunk's iteration (the group's own counter is it / kR_Groups).
+__device__ __forceinline__ void r_produce(uint8_t* smem, R_Bars* bars, volatile int* abort_flag, uint32_t tmem, int gi, int gtid,
+                                          int wq, int it, uint32_t kt, uint32_t out
+                                          ) {
+  const int warp = gtid >> 5, lane = gtid & 31;
+  const uint32_t smem_base = smem_u32(smem);
+  const uint32_t scr = smem_base + kR_OffScr + gi * kR_ScrBytes;
+  const uint32_t s_l = scr + kR_ScrL, s_d = scr + kR_ScrD, s_t = scr + kR_ScrT + warp * 16 * kR_DPitch, s_b = scr + kR_ScrB;
+  const uint32_t ab_tile = smem_base + kR_OffAb + gi * kTileB;
+  const uint32_t gr = smem_base + kR_OffGate + (it & (kR_GateSlots - 1)) * kR_GateFloats * 4;
+  const uint32_t acc_col = tmem + kR_ColACC + 64 * gi;
+  const uint32_t acc_t = acc_col + ((uint32_t)(32 * wq) << 16);
+  const int itg = it / kR_Groups;  // phase of acc_done is 2 itg (Gram), 2 itg + 1 (W')
+
+  if (gtid < kC) sts32(s_b + 4 * gtid, __float_as_uint(lds32f(gr + 4 * (kC + gtid))));
+  tc_fence_before();
+  named_bar_sync(3 + gi, 128);  // beta is in place; every warp's TMEM reads of ACC for the group's previous chunk are done
+
+  // ---- G: Gram on the tensor pipe, then L as an fp16 tile (the upper triangle as zeros)
+  if (wq == 0) {
+    tc_fence_after();
+    f_issue_gram(acc_col, kt, &bars->acc_done[gi]);
+  }
+  if (wq < 2) {  // Gram rows 0..63 sit in TMEM lanes 0..63: the two warps of the group that reach them
+    s2_wait_warp(&bars->acc_done[gi], (2 * itg) & 1, abort_flag, lane);
+    tc_fence_after();
+    const int r = 32 * wq + lane;
+    const float br = lds32f(s_b + 4 * r);
+#pragma unroll 1
+    for (int cb = 0; cb < 2; ++cb) {
+      uint32_t x[32];
+      tmem_ld32(acc_t + 32 * cb, x);
+      tmem_ld_wait();
+#pragma unroll
+      for (int p8 = 0; p8 < 4; ++p8) {
+        const int j = 32 * cb + 8 * p8;
+        uint32_t o[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+          o[q] = pack_f16((j + 2 * q < r) ? br * __uint_as_float(x[8 * p8 + 2 * q]) : 0.f,
+                          (j + 2 * q + 1 < r) ? br * __uint_as_float(x[8 * p8 + 2 * q + 1]) : 0.f);
+        sts128(s_l + r * 128 + (((4 * cb + p8) ^ (r & 7)) << 4), make_uint4(o[0], o[1], o[2], o[3]));
+      }
+    }
+    tc_fence_before();
+  }
+  named_bar_sync(3 + gi, 128);
+
+  // ---- D: diagonal block `warp`, lane c (and its twin c + 16) = column c: a_r = delta_rc - sum_{j < r} L_rj a_j
+  {
+    const int cc = lane & 15;
+    float a[16];
+    uint4 lo[16], hi[8];  // row r of the block: 16 halves = pieces 2 warp, 2 warp + 1 of row 16 warp + r
+#pragma unroll
+    for (int r = 1; r < 16; ++r) {
+      const int R = 16 * warp + r;
+      lo[r] = lds128(s_l + R * 128 + (((2 * warp) ^ (R & 7)) << 4));
+      if (r > 8) hi[r - 8] = lds128(s_l + R * 128 + (((2 * warp + 1) ^ (R & 7)) << 4));
+    }
+    a[0] = (cc == 0) ? 1.f : 0.f;
+#pragma unroll
+    for (int r = 1; r < 16; ++r) {
+      const uint32_t w[8] = {lo[r].x, lo[r].y, lo[r].z, lo[r].w, r > 8 ? hi[r - 8].x : 0u, r > 8 ? hi[r - 8].y : 0u,
+                             r > 8 ? hi[r - 8].z : 0u, r > 8 ? hi[r - 8].w : 0u};
+      float p0 = (r == cc) ? 1.f : 0.f, p1 = 0.f;
+#pragma unroll
+      for (int j = 0; j < r; ++j) {
+        const float l = (j & 1) ? f16hi(w[j >> 1]) : f16lo(w[j >> 1]);
+        if (j & 1) p1 = fmaf(-l, a[j], p1);
+        else p0 = fmaf(-l, a[j], p0);
+      }
+      a[r] = p0 + p1;
+    }
+    // lanes 0..15 store D (for the strips' left factors), their twins store A_b[ww] = D diag(beta)
+    if (lane < 16) {
+#pragma unroll
+      for (int r = 0; r < 16; ++r) sts16(s_d + warp * 16 * kR_DPitch + r * kR_DPitch + 2 * cc, f16_bits(a[r]));
+    } else {
+      const float bc = lds32f(s_b + 4 * (16 * warp + cc));
+#pragma unroll
+      for (int r = 0; r < 16; ++r) {
+        const int R = 16 * warp + r;
+        sts16(ab_tile + R * 128 + (((2 * warp + (cc >> 3)) ^ (R & 7)) << 4) + 2 * (cc & 7), f16_bits(a[r] * bc));
+      }
+    }
+  }
+  named_bar_sync(3 + gi, 128);
+
+  // ---- S: block column `warp` of A_b
+  {
+    const int j = warp;
+    const int lrow = (lane & 7) + ((lane >> 3) & 1) * 8, lhi = lane >> 4;  // ldmatrix.x4: this lane's row / 8-column half
+    const int gq = lane >> 2, tq = lane & 3;
+#pragma unroll 1
+    for (int i = j + 1; i < 4; ++i) {
+      float acc[2][4];
+      block_zero(acc);
+#pragma unroll 1
+      for (int k = j; k < i; ++k) {  // acc += L_ik A_b[kj]
+        uint32_t af[4], bf[4];
+        const int Ra = 16 * i + lrow, Rb = 16 * k + lrow;
+        ldmatrix_x4(af, s_l + Ra * 128 + (((2 * k + lhi) ^ (Ra & 7)) << 4));
+        ldmatrix_x4_trans(bf, ab_tile + Rb * 128 + (((2 * j + lhi) ^ (Rb & 7)) << 4));
+        mma_f16_16816(acc[0], af[0], af[1], af[2], af[3], bf[0], bf[1]);
+        mma_f16_16816(acc[1], af[0], af[1], af[2], af[3], bf[2], bf[3]);
+      }
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt) {
+        sts32(s_t + gq * kR_DPitch + 2 * (8 * nt + 2 * tq), pack_f16(acc[nt][0], acc[nt][1]));
+        sts32(s_t + (gq + 8) * kR_DPitch + 2 * (8 * nt + 2 * tq), pack_f16(acc[nt][2], acc[nt][3]));
+      }
+      __syncwarp();
+      {  // A_b[ij] = -D_i tmp
+        uint32_t af[4], bf[4];
+        ldmatrix_x4(af, s_d + i * 16 * kR_DPitch + lrow * kR_DPitch + 16 * lhi);
+        ldmatrix_x4_trans(bf, s_t + lrow * kR_DPitch + 16 * lhi);
+        block_zero(acc);
+        mma_f16_16816(acc[0], af[0], af[1], af[2], af[3], bf[0], bf[1]);
+        mma_f16_16816(acc[1], af[0], af[1], af[2], af[3], bf[2], bf[3]);
+      }
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt) {
+        const int R0 = 16 * i + gq, R1 = R0 + 8;
+        sts32(ab_tile + R0 * 128 + (((2 * j + nt) ^ (R0 & 7)) << 4) + 4 * tq, pack_f16(-acc[nt][0], -acc[nt][1]));
+        sts32(ab_tile + R1 * 128 + (((2 * j + nt) ^ (R1 & 7)) << 4) + 4 * tq, pack_f16(-acc[nt][2], -acc[nt][3]));
+      }
+      __syncwarp();
+    }
+  }
+  fence_proxy_async();  // the A_b tile must be visible to the tensor pipe's reads
+  named_bar_sync(3 + gi, 128);
+
+  // ---- W: W'^t = K^t A_b on the tensor pipe: thread = dk index c' holds W'[0..63][c']; packed as token pairs into row
+  // c' of the slot's W' tile ([dk][token], 128-byte rows, 128B swizzle: the MN-major B operand of (3'))
+  if (wq == 0) {
+    tc_fence_after();
+    r_issue_w(acc_col, kt, ab_tile, &bars->acc_done[gi]);
+  }
+  s2_wait_warp(&bars->acc_done[gi], (2 * itg + 1) & 1, abort_flag, lane);
+  // the group's output slot is free once (3') of its previous chunk has completed
+  if (it >= kR_Groups) s2_wait_warp(&bars->out_free[gi], (itg - 1) & 1, abort_flag, lane);
+  tc_fence_after();
+  {
+    const int cr = 32 * wq + lane;  // dk index = TMEM lane
+    const uint32_t wrow = out + (cr >> 3) * 1024 + (cr & 7) * 128;
+#pragma unroll 1
+    for (int cb = 0; cb < 2; ++cb) {
+      uint32_t x[32];
+      tmem_ld32(acc_t + 32 * cb, x);
+      tmem_ld_wait();
+#pragma unroll
+      for (int p8 = 0; p8 < 4; ++p8) {  // tokens 32 cb + 8 p8 .. + 7 -> 16-byte piece 4 cb + p8 of the row
+        const uint4 o = make_uint4(pack_f16(__uint_as_float(x[8 * p8 + 0]), __uint_as_float(x[8 * p8 + 1])),
+                                   pack_f16(__uint_as_float(x[8 * p8 + 2]), __uint_as_float(x[8 * p8 + 3])),
+                                   pack_f16(__uint_as_float(x[8 * p8 + 4]), __uint_as_float(x[8 * p8 + 5])),
+                                   pack_f16(__uint_as_float(x[8 * p8 + 6]), __uint_as_float(x[8 * p8 + 7])));
+        sts128(wrow + (((4 * cb + p8) ^ (cr & 7)) << 4), o);
+      }
+    }
+  }
+  tc_fence_before();
+  fence_proxy_async();
+  __syncwarp();
+  if (lane == 0) mbar_arrive(&bars->out_full[gi]);  // count 4: one arrival per warp of the group
+}
+
+// ---------------------------------------------------------------------------------------------------- kernel
+__global__ void __launch_bounds__(kR_Threads, 1)
+    scan4_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                 const float* __restrict__ g, const float* __restrict__ beta, const int32_t* __restrict__ cu_seqlens,
+                 const int32_t* __restrict__ seg_order, int H, float* __restrict__ E, float* __restrict__ T,
+                 int32_t* __restrict__ fb, int n_units) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  R_Bars* bars = reinterpret_cast<R_Bars*>(smem + kR_OffBar);
+  volatile int* abort_flag = &bars->abort_flag;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int h = blockIdx.x, s = seg_order[blockIdx.y];  // longest segments first
+  const int seg_begin = cu_seqlens[s], seg_end = cu_seqlens[s + 1];
+  const int seg_len = seg_end - seg_begin;
+  const int nc = (seg_len + kC - 1) / kC;
+  const int last_valid = seg_len - (nc - 1) * kC;  // tokens of the ragged last chunk = the FIRST iteration
+
+  if (warp == kR_WLoader) tmem_alloc(&bars->tmem_base, 512);
+  if (tid == 0) {
+    for (int i = 0; i < kR_KStages; ++i) {
+      mbar_init(&bars->k_full[i], 1);
+      mbar_init(&bars->k_free[i], 1);
+      mbar_init(&bars->k_ready[i], 1);
+    }
+    for (int i = 0; i < kR_VStages; ++i) {
+      mbar_init(&bars->v_full[i], 1);
+      mbar_init(&bars->v_free[i], 1);
+      mbar_init(&bars->v_ok[i], 1);
+    }
+    for (int i = 0; i < kR_Groups; ++i) {
+      mbar_init(&bars->out_full[i], 4);
+      mbar_init(&bars->out_free[i], 1);
+      mbar_init(&bars->acc_done[i], 1);
+    }
+    for (int i = 0; i < kR_GateSlots; ++i) mbar_init(&bars->gate_full[i], 1);
+    mbar_init(&bars->m3_done, 1);
+    mbar_init(&bars->m4_done, 1);
+    mbar_init(&bars->e_done, 1);
+    bars->abort_flag = 0;
+    bars->bad = 0;
+    bars->g_total = 0.0;
+    bars->fin_flag = 0;
+    fence_barrier_init();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = bars->tmem_base;
+  const uint32_t smem_base = smem_u32(smem);
+
+  if (warp == kR_WLoader) {
+    // ------------------------------------------------------------------------------------------- loader
+    // Iteration it = chunk nc - 1 - it: its K tile, then the V tile of iteration it - 2 (the producers need K two
+    // iterations before (5) needs V).  One lane, nothing but waits and TMA issues.
+    if (lane == 0) {
+#pragma unroll 1
+      for (int it = 0; it < nc + 2; ++it) {
+        if (it < nc) {
+          const int kst = it % kR_KStages;
+          const int t0 = seg_begin + (nc - 1 - it) * kC;
+          if (it >= kR_KStages) f_wait_lazy(&bars->k_free[kst], ((it / kR_KStages) - 1) & 1, abort_flag);
+          mbar_expect_tx(&bars->k_full[kst], 2 * kTileB);
+          tma_load_3d(smem_base + kR_OffK + kst * 2 * kTileB, &tmK, 0, h, t0, &bars->k_full[kst]);
+          tma_load_3d(smem_base + kR_OffK + kst * 2 * kTileB + 8192, &tmK, 64, h, t0, &bars->k_full[kst]);
+        }
+        const int iv = it - 2;
+        if (iv >= 0) {
+          const int vst = iv % kR_VStages;
+          const int t0 = seg_begin + (nc - 1 - iv) * kC;
+          if (iv >= kR_VStages) f_wait_lazy(&bars->v_free[vst], ((iv / kR_VStages) - 1) & 1, abort_flag);
+          mbar_expect_tx(&bars->v_full[vst], 2 * kTileB);
+          tma_load_3d(smem_base + kR_OffV + vst * 2 * kTileB, &tmV, 0, h, t0, &bars->v_full[vst]);
+          tma_load_3d(smem_base + kR_OffV + vst * 2 * kTileB + 8192, &tmV, 64, h, t0, &bars->v_full[vst]);
+        }
+      }
+    }
+  } else if (warp == kR_WGate) {
+    // ------------------------------------------------------------------------------------------- gate
+    // All 32 lanes, always converged.  Lanes t, t + 32 own tokens t, t + 32 of the chunk; the next iteration's g / beta
+    // are in flight while this one is scanned.  w_t = exp(G_after + sum_{s > t in chunk} g_s), G_after = the log-decay of
+    // all later chunks (fp64 running sum).  Paced by the chunk's K tile landing, so the 8-slot ring cannot be lapped.
+    float* gate_ring = reinterpret_cast<float*>(smem + kR_OffGate);
+    double g_after = 0.0;
+    float gn0 = 0.f, gn1 = 0.f, bn0 = 0.f, bn1 = 0.f;
+    auto fetch = [&](int it) {
+      const int c = nc - 1 - it;
+      const int t0 = seg_begin + c * kC, valid = min(kC, seg_len - c * kC);
+      gn0 = gn1 = bn0 = bn1 = 0.f;  // tokens past the segment's end: g = 0, beta = 0 (exact no-ops)
+      if (lane < valid) {
+        gn0 = g[(size_t)(t0 + lane) * H + h];
+        bn0 = beta[(size_t)(t0 + lane) * H + h];
+      }
+      if (lane + 32 < valid) {
+        gn1 = g[(size_t)(t0 + lane + 32) * H + h];
+        bn1 = beta[(size_t)(t0 + lane + 32) * H + h];
+      }
+    };
+    if (nc > 0) fetch(0);
+#pragma unroll 1
+    for (int it = 0; it < nc; ++it) {
+      const float o0 = gn0, o1 = gn1, b0 = bn0, b1 = bn1;
+      float g0 = o0, g1 = o1;
+      if (it + 1 < nc) fetch(it + 1);
+      f_wait_lazy(&bars->k_full[it % kR_KStages], (it / kR_KStages) & 1, abort_flag);  // pacing only
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {  // inclusive suffix scans of the two token halves
+        const float u0 = __shfl_down_sync(0xffffffffu, g0, o), u1 = __shfl_down_sync(0xffffffffu, g1, o);
+        if (lane + o < 32) g0 += u0, g1 += u1;
+      }
+      g0 += __shfl_sync(0xffffffffu, g1, 0);  // the upper half's tokens all come after the lower half's
+      const float GC = __shfl_sync(0xffffffffu, g0, 0);
+      const float ga = (float)g_after;
+      float* gr = gate_ring + (it & (kR_GateSlots - 1)) * kR_GateFloats;
+      gr[lane] = expf(ga + (g0 - o0));
+      gr[lane + 32] = expf(ga + (g1 - o1));
+      gr[kC + lane] = b0;
+      gr[kC + lane + 32] = b1;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars->gate_full[it & (kR_GateSlots - 1)]);
+      g_after += (double)GC;
+    }
+    if (lane == 0) {
+      bars->g_total = g_after;
+      flag_release(&bars->fin_flag, 1);
+    }
+  } else if (warp == kR_WConv) {
+    // ------------------------------------------------------------------------------------------- converter
+    // Walks the tiles in the loader's order (every phase of k_full / v_full is waited for: a parity wait must never skip
+    // one).  K: bf16 -> fp16 in place (element-wise on 16-bit lanes, so the 128B swizzle of the TMA boxes is untouched),
+    // ahead of the producers' need; the V converter does the same for V (a kind::f16 MMA cannot mix a bf16 and an fp16
+    // operand).  The ragged last chunk (the first iteration) also holds tokens of the next segment: those rows are
+    // zeroed in both tiles, so that nothing of a neighbour -- not even an Inf or NaN -- reaches the unit through
+    // 0 x garbage.
+#pragma unroll 1
+    for (int it = 0; it < nc; ++it) {
+      const int kst = it % kR_KStages;
+      const int valid = it == 0 ? last_valid : kC;
+      const uint32_t kt = smem_base + kR_OffK + kst * 2 * kTileB;
+      f_wait_lazy(&bars->k_full[kst], (it / kR_KStages) & 1, abort_flag);
+#pragma unroll 1
+      for (int i0 = 0; i0 < 32; i0 += 8) {  // 16-byte piece p of the tile: token (p % 512) / 8
+        uint4 w[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) w[j] = lds128(kt + 16 * (lane + 32 * (i0 + j)));
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const int p = lane + 32 * (i0 + j);
+          uint4 o = cvt8_bf16_f16(w[j]);
+          if (((p & 511) >> 3) >= valid) o = make_uint4(0u, 0u, 0u, 0u);
+          sts128(kt + 16 * p, o);
+        }
+      }
+      fence_proxy_async();  // the fp16 K tile must be visible to the tensor pipe's reads
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars->k_ready[kst]);
+      __syncwarp();
+    }
+  } else if (warp == kR_WConvV) {
+    // ------------------------------------------------------------------------------------------- V converter
+#pragma unroll 1
+    for (int iv = 0; iv < nc; ++iv) {
+      const int vst = iv % kR_VStages;
+      const int valid = iv == 0 ? last_valid : kC;
+      const uint32_t vt = smem_base + kR_OffV + vst * 2 * kTileB;
+      f_wait_lazy(&bars->v_full[vst], (iv / kR_VStages) & 1, abort_flag);
+#pragma unroll 1
+      for (int i0 = 0; i0 < 32; i0 += 8) {
+        uint4 w[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) w[j] = lds128(vt + 16 * (lane + 32 * (i0 + j)));
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const int p = lane + 32 * (i0 + j);
+          uint4 o = cvt8_bf16_f16(w[j]);
+          if (((p & 511) >> 3) >= valid) o = make_uint4(0u, 0u, 0u, 0u);
+          sts128(vt + 16 * p, o);
+        }
+      }
+      fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars->v_ok[vst]);
+      __syncwarp();
+    }
+  } else if (warp >= kR_WProd) {
+    // ------------------------------------------------------------------------------------------- producers
+    const int gi = (warp - kR_WProd) >> 2, gtid = tid - 32 * kR_WProd - 128 * gi;
+    // the blocks above the diagonal of the group's A_b tile are never written: zero the tile once
+    for (int p = gtid; p < kTileB / 16; p += 128) sts128(smem_base + kR_OffAb + gi * kTileB + 16 * p, make_uint4(0u, 0u, 0u, 0u));
+    named_bar_sync(3 + gi, 128);
+#pragma unroll 1
+    for (int it = gi; it < nc; it += kR_Groups) {
+      const int kst = it % kR_KStages;
+      f_wait_lazy(&bars->gate_full[it & (kR_GateSlots - 1)], (it / kR_GateSlots) & 1, abort_flag);
+      f_wait_lazy(&bars->k_ready[kst], (it / kR_KStages) & 1, abort_flag);
+      r_produce(smem, bars, abort_flag, tmem, gi, gtid, warp & 3, it, smem_base + kR_OffK + kst * 2 * kTileB,
+                smem_base + kR_OffOut + gi * 2 * kTileB
+                );
+    }
+  } else {
+    r_chain(smem, bars, abort_flag, tmem, warp, lane, nc, E + ((size_t)s * H + h) * kD * kD,
+                    T + ((size_t)s * H + h) * kD * kD);
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == kR_WLoader) tmem_dealloc(tmem, 512);
+  if (tid == 0 && bars->bad) fb_append(fb, n_units, s * H + h);
+}

@@ -1,20 +1,18 @@
 // encode_tensor.cu -- tcgen05/TMEM segment encode: bf16 k/v, scalar gate, dk = dv = 128 (HYPIC_IMPL_TENSOR).
 //
 // Rows a0..a5 of SURVEY.md section 8(a), chunked (C = 64 tokens) WY/UT form of the token recurrence
-// (Eq. 2, Table 1 GDN row PAPER.md:61; T_C and S_{C|0} of PAPER.md:118-126).  Per chunk, with
-// G_r the in-chunk inclusive cumulative log-decay, gamma_r = exp(G_r), d_j = exp(G_C - G_j):
-//     L_rj = beta_r exp(G_r - G_j) (k_r.k_j)  (j < r),   A = (I + L)^-1,   A_b = A diag(beta),
-//     W = A_b diag(gamma) K  (C x dk),   U^ = A_b V  (C x dv),
-//     X <- gamma_C X + ([U^t ; 0] - X W^t) diag(d) K          for the stacked state X = [E ; T].
-// Three launches:
-//   K0 chunk_offsets : prefix sum of ceil(L_s / 64) (cu_seqlens lives on the device; no host sync).
-//   K1 prep          : per (chunk, head), state-independent: Gram (mma.sync), L, A = (I + L)^-1 by a blocked inverse,
-//                      -W (mma.sync, fp16 out) and A_b (fp16), stored as ready-made K-major 128B-swizzled
-//                      UMMA B tiles, plus the gate record (d_j, gamma_C)  (encode_prep.cuh).
-//   K2 scan          : one CTA per (segment, head), sequential over chunks, both row blocks of X resident in TMEM;
-//                      every state contraction is a tcgen05.mma (see encode_scan2.cuh).
+// (Eq. 2, Table 1 GDN / KDA rows PAPER.md:61; T_C and S_{C|0} of PAPER.md:118-126).
+//   Scalar gate (GDN): K0 chunk_offsets + ONE fused kernel, scan4_kernel (encode_scan4.cuh): the gate commutes with the
+//     delta rule's factors, so the chunk algebra is gate-free and runs in the reverse (suffix-product) form.
+//   Per-channel gate (KDA): K0 + K1 prep_kernel<1> (encode_prep.cuh: Gram, L, A = (I + L)^-1 by a blocked inverse, -W and
+//     A_b as ready-made UMMA B tiles plus the gate record, in HBM) + K2 scan2_kernel<1> (encode_scan2.cuh: one CTA per
+//     (segment, head), sequential over chunks, both row blocks of X = [E ; T] resident in TMEM).
+//   Units the fp16 operands cannot carry go to a device-side list that the fp32 family recomputes inside the same call.
 #include <cuda.h>
 #include <cuda_fp16.h>
+#ifdef HYPIC_PROF
+#include <stdio.h>
+#endif
 #include <stdlib.h>
 
 #include "common.cuh"
@@ -118,7 +116,7 @@ __device__ __forceinline__ void fb_append(int32_t* fb, int n_units, int unit) {
 
 #include "encode_scan2.cuh"
 
-#include "encode_scan3.cuh"
+#include "encode_scan4.cuh"
 
 #include "diag_scan.cuh"
 
@@ -197,7 +195,7 @@ int encode_tensor(const EncodeArgs& a) {
   static std::atomic<unsigned long long> configured{0};
   int cfg_dev = 0;
   if (needs_device_setup(configured, &cfg_dev)) {
-    HYPIC_CUDA_OK(cudaFuncSetAttribute(scan3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kF_Smem));
+    HYPIC_CUDA_OK(cudaFuncSetAttribute(scan4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kR_Smem));
     HYPIC_CUDA_OK(cudaFuncSetAttribute(scan2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kS2Smem));
     device_setup_done(configured, cfg_dev);
   }
@@ -217,7 +215,7 @@ int encode_tensor(const EncodeArgs& a) {
     scan2_kernel<true><<<sgrid, kS2Threads, kS2Smem, a.stream>>>(tmK, tmV, a.cu_seqlens, chunk_off, seg_order, a.H, rec, gate,
                                                                  a.E, a.T, fb, n_units);
   } else {
-    scan3_kernel<<<sgrid, kF_Threads, kF_Smem, a.stream>>>(tmK, tmV, a.g, a.beta, a.cu_seqlens, seg_order, a.H, a.E, a.T, fb,
+    scan4_kernel<<<sgrid, kR_Threads, kR_Smem, a.stream>>>(tmK, tmV, a.g, a.beta, a.cu_seqlens, seg_order, a.H, a.E, a.T, fb,
                                                            n_units);
   }
   note_launch();
