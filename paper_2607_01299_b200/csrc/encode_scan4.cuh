@@ -39,8 +39,8 @@
 #pragma once
 
 constexpr int kR_Groups = 2;
-constexpr int kR_Threads = 32 * (8 + 4 * kR_Groups);
-constexpr int kR_WChain = 0, kR_WLoader = 4, kR_WGate = 5, kR_WConv = 6, kR_WConvV = 7, kR_WProd = 8;
+constexpr int kR_Threads = 32 * (12 + 4 * kR_Groups);
+constexpr int kR_WChain = 0, kR_WLoader = 8, kR_WGate = 9, kR_WConv = 10, kR_WConvV = 11, kR_WProd = 12;
 constexpr int kR_KStages = 6, kR_VStages = 2, kR_GateSlots = 8;
 constexpr int kR_OffK = 0;                                        // 4 x 16 KB: K tile, two 64-column boxes [token][64]
 constexpr int kR_OffV = kR_OffK + kR_KStages * 2 * kTileB;        // 2 x 16 KB: V tile (bf16 as it arrives)
@@ -50,13 +50,14 @@ constexpr int kR_OffAb = kR_OffFy + 2 * kTileB;                   // one 8 KB A_
 constexpr int kR_OffScr = kR_OffAb + kR_Groups * kTileB;          // producer scratch per group
 constexpr int kR_ScrL = 0;                                        // fp16 L [64][64]: 128-byte rows, 16-byte pieces ^ (row & 7)
 constexpr int kR_DPitch = 48;                                     // bytes per row of a 16 x 16 fp16 block (conflict-free ldmatrix)
-constexpr int kR_ScrD = kTileB;                                   // fp16 D_i = (I + L_ii)^-1, 4 x [16][24]
-constexpr int kR_ScrT = kR_ScrD + 4 * 16 * kR_DPitch;             // fp16 temporaries of the strips, one [16][24] per warp
+constexpr int kR_ScrD = kTileB;                                   // fp16 D_i^t, D_i = (I + L_ii)^-1, 4 x [16][24]
+constexpr int kR_ScrT = kR_ScrD + 4 * 16 * kR_DPitch;             // (unused)
 constexpr int kR_ScrB = kR_ScrT + 4 * 16 * kR_DPitch;             // fp32 [64] beta
 constexpr int kR_ScrBytes = kR_ScrB + 256;
 constexpr int kR_OffGate = kR_OffScr + kR_Groups * kR_ScrBytes;   // 8 x gate record: w_t[64], beta_t[64]
 constexpr int kR_GateFloats = 2 * kC;
-constexpr int kR_OffBar = kR_OffGate + kR_GateSlots * kR_GateFloats * 4;
+constexpr int kR_OffXch = kR_OffGate + kR_GateSlots * kR_GateFloats * 4;  // fp32 [2][128]: lane maxima of the chain halves
+constexpr int kR_OffBar = kR_OffXch + 1024;
 constexpr int kR_Smem = kR_OffBar + 512 + 1024;
 constexpr uint32_t kR_ColR = 0, kR_ColE = 128, kR_ColH = 256, kR_ColDY = 320, kR_ColACC = 384;
 
@@ -76,6 +77,7 @@ struct R_Bars {
   double g_total;
 };
 static_assert(sizeof(R_Bars) <= 512, "barrier block");
+static_assert(kR_Smem <= 232448, "227 KB of shared memory per CTA");
 
 __device__ __forceinline__ void sts32(uint32_t a, uint32_t v) { asm volatile("st.shared.b32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 
@@ -182,46 +184,48 @@ __device__ __forceinline__ void r_issue5(uint32_t d_tmem, uint32_t v_tile, uint3
       "}" ::"r"(d_tmem), "l"(ad0), "l"(bd0), "r"(id5), "r"(acc_first), "r"(smem_u32(bar0)), "r"(smem_u32(bar1))
       : "memory");
 }
-// (W'): ACC = K^t A_b = W'^t -- A = the K tile MN-major (+128 per 16 tokens), B = the A_b tile [j][r] read MN-major
-// (+128 per 16 rows j); commits to the group's acc_done
+// (W'): ACC = K^t A_b = W'^t -- A = the K tile MN-major (+128 per 16 tokens), B = the A_b^t tile [r][j] K-major (+2 per
+// 16 rows j of A_b); commits to the group's acc_done
 __device__ __forceinline__ void r_issue_w(uint32_t d_tmem, uint32_t k_tile, uint32_t ab_tile, uint64_t* bar0) {
-  constexpr uint32_t idw = make_idesc(0u, 128, 64, 1, 1);
-  const uint64_t ad0 = make_desc(k_tile, 8192, 1024, 2), bd0 = make_desc(ab_tile, 8192, 1024, 2);
+  constexpr uint32_t idw = make_idesc(0u, 128, 64, 1, 0);
+  const uint64_t ad0 = make_desc(k_tile, 8192, 1024, 2), bd0 = make_desc(ab_tile, 16, 1024, 2);
   asm volatile(
       "{\n\t.reg .pred P, Q;\n\t.reg .b64 ad, bd;\n\t"
       "elect.sync _|P, 0xffffffff;\n\t"
       "setp.ne.b32 Q, 0, 0;\n\t"
       "mov.b64 ad, %1;\n\tmov.b64 bd, %2;\n\t" F_MMA_SS
       "setp.ne.b32 Q, 1, 0;\n\t"
-      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 128;\n\t" F_MMA_SS
-      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 128;\n\t" F_MMA_SS
-      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 128;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
+      "add.s64 ad, ad, 128;\n\tadd.s64 bd, bd, 2;\n\t" F_MMA_SS
       F_COMMIT(4)
       "}" ::"r"(d_tmem), "l"(ad0), "l"(bd0), "r"(idw), "r"(smem_u32(bar0))
       : "memory");
 }
 
 // ---------------------------------------------------------------------------------------------------- chain
+// Eight warps: warp cw reaches the TMEM lane quarter cw % 4; the two warps of a quarter split the columns (pass: 64 columns
+// of R^t each; epilogue: 32 tokens of DY each), so that every phase is one TMEM load deep.
 __device__ __forceinline__ void r_chain(uint8_t* smem, R_Bars* bars, volatile int* abort_flag, uint32_t tmem, int cw, int lane,
                                         int nc, float* __restrict__ E_dst, float* __restrict__ T_dst) {
-  const int wq = cw & 3;  // a warp reaches the TMEM lane quarter warp id % 4; the chain's four warps cover all four
+  const int wq = cw & 3, hf = cw >> 2;
   const int row = 32 * wq + lane;
   const uint32_t lane_base = (uint32_t)(32 * wq) << 16;
-  const uint32_t tR = tmem + kR_ColR + lane_base, tE = tmem + kR_ColE + lane_base, tH = tmem + kR_ColH + lane_base,
-                 tD = tmem + kR_ColDY + lane_base;
+  const uint32_t tR = tmem + kR_ColR + lane_base + 64 * hf, tE = tmem + kR_ColE + lane_base + 64 * hf,
+                 tH = tmem + kR_ColH + lane_base, tD = tmem + kR_ColDY + lane_base + 32 * hf;
   const uint32_t smem_base = smem_u32(smem);
   const uint32_t fy_row = smem_base + kR_OffFy + (row >> 3) * 1024 + (row & 7) * 128;
   const uint32_t gate_base = smem_base + kR_OffGate;
+  const uint32_t xch = smem_base + kR_OffXch;  // fp32 [2][128]: the two halves' column maxima of a lane
   int s_exp = 0;        // the TMEM copy of this lane is (column `row` of R) * 2^s_exp
   float unscale = 1.f;  // 2^-s_exp (0 once the column has shrunk below the fp32 range: its contributions to E vanish)
-  const bool issue_warp = (cw == kR_WChain);  // warp-uniform: the bursts elect their lane
 
   // R_n^t = I
 #pragma unroll
-  for (int cb = 0; cb < 4; ++cb) {
+  for (int cb = 0; cb < 2; ++cb) {
     uint32_t x[32];
 #pragma unroll
-    for (int i = 0; i < 32; ++i) x[i] = (32 * cb + i == row) ? __float_as_uint(1.f) : 0u;
+    for (int i = 0; i < 32; ++i) x[i] = (64 * hf + 32 * cb + i == row) ? __float_as_uint(1.f) : 0u;
     tmem_st32(tR + 32 * cb, x);
   }
   tmem_st_wait();
@@ -232,113 +236,96 @@ __device__ __forceinline__ void r_chain(uint8_t* smem, R_Bars* bars, volatile in
     s2_wait_warp(&bars->out_full[gi], (it / kR_Groups) & 1, abort_flag, lane);  // W' and the fp16 K tile are in place
     if (it > 0) s2_wait_warp(&bars->m4_done, (it - 1) & 1, abort_flag, lane);
     tc_fence_after();
-    // ---- pass: Rh = fp16(R^t), 32 columns at a time; R^t itself is only rewritten when the lane's scale is re-chosen
+    // ---- pass: Rh = fp16(R^t), this thread's 64 columns; R^t itself is only rewritten when the lane's scale is re-chosen
     {
-      float f = 1.f;
-      const bool rewrite = (it & 7) == 0;
-      if (rewrite) {  // the whole column of R lives in this thread: maximum -> power-of-two scale
+      uint32_t xa[32], xb[32], hh[16];
+      tmem_ld32(tR, xa);
+      tmem_ld32(tR + 32, xb);
+      tmem_ld_wait();
+      if ((it & 7) == 0) {  // lane maximum over both halves -> power-of-two scale (the same in both threads of the lane)
         float m = 0.f;
-#pragma unroll 1
-        for (int cb = 0; cb < 4; ++cb) {
-          uint32_t x[32];
-          tmem_ld32(tR + 32 * cb, x);
-          tmem_ld_wait();
 #pragma unroll
-          for (int i = 0; i < 32; ++i) m = fmaxf(m, fabsf(__uint_as_float(x[i])));
-        }
+        for (int i = 0; i < 32; ++i) m = fmaxf(m, fmaxf(fabsf(__uint_as_float(xa[i])), fabsf(__uint_as_float(xb[i]))));
+        sts32(xch + 4 * (128 * hf + row), __float_as_uint(m));
+        named_bar_sync(2, 256);
+        m = fmaxf(m, lds32f(xch + 4 * (128 * (hf ^ 1) + row)));
         const int e = (int)((__float_as_uint(m) >> 23) & 0xffu);  // maximum in [2^(e-127), 2^(e-126))
         int dlt = (e == 0 || e == 255) ? 0 : 138 - e;             // -> [2^11, 2^12)
         dlt = max(-100, min(100, dlt));
         s_exp += dlt;
-        f = pow2i(dlt);
+        const float f = pow2i(dlt);
         unscale = (s_exp > 126) ? 0.f : pow2i(max(-126, -s_exp));
-      }
-      {
-        uint32_t xa[32], xb[32], hh[16];
-        tmem_ld32(tR, xa);
 #pragma unroll
-        for (int cb = 0; cb < 4; cb += 2) {  // the next 32 columns are in flight while these are converted
-          tmem_ld_wait();
-          tmem_ld32(tR + 32 * (cb + 1), xb);
-          if (rewrite) {
-#pragma unroll
-            for (int j = 0; j < 16; ++j) mul2(xa[2 * j], xa[2 * j + 1], f);
-            tmem_st32(tR + 32 * cb, xa);  // (3') reads Rh alone; (4') of this chunk is issued after the chain barrier below
-          }
-#pragma unroll
-          for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(xa[2 * j]), __uint_as_float(xa[2 * j + 1]));
-          tmem_st16(tH + 16 * cb, hh);
-          tmem_ld_wait();
-          if (cb + 2 < 4) tmem_ld32(tR + 32 * (cb + 2), xa);
-          if (rewrite) {
-#pragma unroll
-            for (int j = 0; j < 16; ++j) mul2(xb[2 * j], xb[2 * j + 1], f);
-            tmem_st32(tR + 32 * (cb + 1), xb);
-          }
-#pragma unroll
-          for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(xb[2 * j]), __uint_as_float(xb[2 * j + 1]));
-          tmem_st16(tH + 16 * (cb + 1), hh);
+        for (int j = 0; j < 16; ++j) {
+          mul2(xa[2 * j], xa[2 * j + 1], f);
+          mul2(xb[2 * j], xb[2 * j + 1], f);
         }
+        tmem_st32(tR, xa);  // (3') reads Rh alone; (4') of this chunk is issued after the chain barrier below
+        tmem_st32(tR + 32, xb);
       }
-      tmem_st_wait();
-      tc_fence_before();
-      named_bar_sync(1, 128);  // the whole chain has written Rh
-      if (issue_warp) {
-        tc_fence_after();
-        r_issue3(tmem + kR_ColDY, tmem + kR_ColH, smem_base + kR_OffOut + gi * 2 * kTileB, &bars->m3_done, &bars->out_free[gi]);
-      }
+#pragma unroll
+      for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(xa[2 * j]), __uint_as_float(xa[2 * j + 1]));
+      tmem_st16(tH + 32 * hf, hh);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(xb[2 * j]), __uint_as_float(xb[2 * j + 1]));
+      tmem_st16(tH + 32 * hf + 16, hh);
     }
-    // ---- epilogue: U'' = fp16(DY) -> TMEM (A operand of (4')), tokens [32 cb, 32 cb + 32) -> columns [16 cb, 16 cb + 16);
-    // fY = fp16(w_t 2^-s DY) -> row `row` of the shared fY tile (B operand of (5); 128-byte rows, 128B swizzle).  The tile
-    // is single-buffered: (5) of the previous chunk sits in front of this chunk's (3') in the in-order tensor pipe, so it
-    // has completed when m3_done fires.
+    tmem_st_wait();
+    tc_fence_before();
+    named_bar_sync(1, 256);  // the whole chain has written Rh
+    if (cw == 0) {
+      tc_fence_after();
+      r_issue3(tmem + kR_ColDY, tmem + kR_ColH, smem_base + kR_OffOut + gi * 2 * kTileB, &bars->m3_done, &bars->out_free[gi]);
+    }
+    // ---- epilogue, this thread's 32 tokens: U'' = fp16(DY) -> TMEM (A operand of (4')), tokens [32 hf, 32 hf + 32) ->
+    // columns [16 hf, 16 hf + 16); fY = fp16(w_t 2^-s DY) -> row `row` of the shared fY tile (B operand of (5); 128-byte
+    // rows, 128B swizzle).  The tile is single-buffered: (5) of the previous chunk sits in front of this chunk's (3') in
+    // the in-order tensor pipe, so it has completed when m3_done fires.
     s2_wait_warp(&bars->m3_done, it & 1, abort_flag, lane);
     tc_fence_after();
     {
-      const uint32_t gw = gate_base + (it & (kR_GateSlots - 1)) * kR_GateFloats * 4;
+      const uint32_t gw = gate_base + ((it & (kR_GateSlots - 1)) * kR_GateFloats + 32 * hf) * 4;
+      uint32_t y[32], u[16];
+      uint4 wq4[8];
+      tmem_ld32(tD, y);
 #pragma unroll
-      for (int hb = 0; hb < 2; ++hb) {
-        uint32_t y[32], u[16];
-        uint4 wq4[8];
-        tmem_ld32(tD + 32 * hb, y);
+      for (int q = 0; q < 8; ++q) wq4[q] = lds128(gw + 16 * q);  // the 32 weights, under the TMEM load
+      tmem_ld_wait();
 #pragma unroll
-        for (int q = 0; q < 8; ++q) wq4[q] = lds128(gw + (32 * hb + 4 * q) * 4);  // the 32 weights, under the TMEM load
-        tmem_ld_wait();
+      for (int j = 0; j < 16; ++j) u[j] = pack_f16(__uint_as_float(y[2 * j]), __uint_as_float(y[2 * j + 1]));
+      tmem_st16(tH + 16 * hf, u);
 #pragma unroll
-        for (int j = 0; j < 16; ++j) u[j] = pack_f16(__uint_as_float(y[2 * j]), __uint_as_float(y[2 * j + 1]));
-        tmem_st16(tH + 16 * hb, u);
+      for (int p8 = 0; p8 < 4; ++p8) {  // tokens 32 hf + 8 p8 .. + 7 -> 16-byte piece 4 hf + p8 of the row
+        uint32_t wv[8] = {wq4[2 * p8].x, wq4[2 * p8].y, wq4[2 * p8].z, wq4[2 * p8].w,
+                          wq4[2 * p8 + 1].x, wq4[2 * p8 + 1].y, wq4[2 * p8 + 1].z, wq4[2 * p8 + 1].w};
+        uint32_t o[4];
 #pragma unroll
-        for (int p8 = 0; p8 < 4; ++p8) {  // tokens 32 hb + 8 p8 .. + 7 -> 16-byte piece 4 hb + p8 of the row
-          uint32_t wv[8] = {wq4[2 * p8].x, wq4[2 * p8].y, wq4[2 * p8].z, wq4[2 * p8].w,
-                            wq4[2 * p8 + 1].x, wq4[2 * p8 + 1].y, wq4[2 * p8 + 1].z, wq4[2 * p8 + 1].w};
-          uint32_t o[4];
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            mul2(wv[2 * q], wv[2 * q + 1], unscale);
-            mul2v(y[8 * p8 + 2 * q], y[8 * p8 + 2 * q + 1], __uint_as_float(wv[2 * q]), __uint_as_float(wv[2 * q + 1]));
-            o[q] = pack_f16(__uint_as_float(y[8 * p8 + 2 * q]), __uint_as_float(y[8 * p8 + 2 * q + 1]));
-          }
-          sts128(fy_row + (((4 * hb + p8) ^ (row & 7)) << 4), make_uint4(o[0], o[1], o[2], o[3]));
+        for (int q = 0; q < 4; ++q) {
+          mul2(wv[2 * q], wv[2 * q + 1], unscale);
+          mul2v(y[8 * p8 + 2 * q], y[8 * p8 + 2 * q + 1], __uint_as_float(wv[2 * q]), __uint_as_float(wv[2 * q + 1]));
+          o[q] = pack_f16(__uint_as_float(y[8 * p8 + 2 * q]), __uint_as_float(y[8 * p8 + 2 * q + 1]));
         }
+        sts128(fy_row + (((4 * hf + p8) ^ (row & 7)) << 4), make_uint4(o[0], o[1], o[2], o[3]));
       }
     }
     tmem_st_wait();
     tc_fence_before();
     fence_proxy_async();     // the fY tile must be visible to the tensor pipe's reads
-    named_bar_sync(1, 128);  // the whole chain has written U'' and fY
-    if (issue_warp) {
+    named_bar_sync(1, 256);  // the whole chain has written U'' and fY
+    if (cw == 0) {
       tc_fence_after();
       r_issue4(tmem + kR_ColR, tmem + kR_ColH, smem_base + kR_OffK + kst * 2 * kTileB, &bars->m4_done, &bars->k_free[kst]);
+    } else if (cw == 1) {  // (5) is off the critical path: a second warp issues it while (4') runs
       s2_wait_warp(&bars->v_ok[vst], (it / kR_VStages) & 1, abort_flag, lane);
       tc_fence_after();
       r_issue5(tmem + kR_ColE, smem_base + kR_OffV + vst * 2 * kTileB, smem_base + kR_OffFy, it > 0 ? 1u : 0u,
-                       &bars->v_free[vst], &bars->e_done);
+               &bars->v_free[vst], &bars->e_done);
     }
   }
 
-  // ---- a5.  T = exp(sum g) R_0: lane j holds column j of R, so for every row i the chain's 128 threads write 512
+  // ---- a5.  T = exp(sum g) R_0: lane j holds column j of R, so for every row i a quarter's 32 threads write 128
   // contiguous bytes; the gate and the lane's scale are applied in fp64, so that a T that underflows fp32 underflows
-  // exactly like the correctly rounded result.  E: thread = row of the accumulator.
+  // exactly like the correctly rounded result.  E: thread = half a row of the accumulator.
   s2_wait_count(&bars->fin_flag, 0, abort_flag);  // the gate warp has posted g_total
   if (nc > 0) {
     s2_wait_warp(&bars->e_done, (nc - 1) & 1, abort_flag, lane);  // the last (5), and with it every MMA before it
@@ -348,7 +335,7 @@ __device__ __forceinline__ void r_chain(uint8_t* smem, R_Bars* bars, volatile in
   {
     const double sc = exp(bars->g_total - 0.6931471805599453 * (double)s_exp);
 #pragma unroll 1
-    for (int cb = 0; cb < 4; ++cb) {
+    for (int cb = 0; cb < 2; ++cb) {
       uint32_t x[32];
       tmem_ld32(tR + 32 * cb, x);
       tmem_ld_wait();
@@ -356,14 +343,14 @@ __device__ __forceinline__ void r_chain(uint8_t* smem, R_Bars* bars, volatile in
       for (int i = 0; i < 32; ++i) {
         const float o = (float)((double)__uint_as_float(x[i]) * sc);
         bad |= !(fabsf(o) <= 3.0e38f);
-        T_dst[(size_t)(32 * cb + i) * kD + row] = o;
+        T_dst[(size_t)(64 * hf + 32 * cb + i) * kD + row] = o;
       }
     }
   }
   {
-    float* dst = E_dst + (size_t)row * kD;
+    float* dst = E_dst + (size_t)row * kD + 64 * hf;
 #pragma unroll 1
-    for (int cb = 0; cb < 4; ++cb) {
+    for (int cb = 0; cb < 2; ++cb) {
       uint32_t x[32];
       if (nc > 0) {
         tmem_ld32(tE + 32 * cb, x);
@@ -389,43 +376,44 @@ __device__ __forceinline__ void r_chain(uint8_t* smem, R_Bars* bars, volatile in
 }
 
 // ---------------------------------------------------------------------------------------------------- producers
+__device__ __forceinline__ void ldmatrix_x1(uint32_t& r, uint32_t saddr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x1.shared.b16 {%0}, [%1];" : "=r"(r) : "r"(saddr));
+}
+__device__ __forceinline__ void ldmatrix_x1_trans(uint32_t& r, uint32_t saddr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x1.trans.shared.b16 {%0}, [%1];" : "=r"(r) : "r"(saddr));
+}
 __device__ __forceinline__ void sts16(uint32_t a, uint16_t v) { asm volatile("st.shared.b16 [%0], %1;" ::"r"(a), "h"(v) : "memory"); }
 __device__ __forceinline__ uint16_t f16_bits(float x) { return __half_as_ushort(__float2half_rn(x)); }
 __device__ __forceinline__ float f16lo(uint32_t w) { return __half2float(__ushort_as_half((uint16_t)(w & 0xffffu))); }
 __device__ __forceinline__ float f16hi(uint32_t w) { return __half2float(__ushort_as_half((uint16_t)(w >> 16))); }
 
 // One chunk of the state-independent half, by one group of four warps (gtid = 0..127; `wq` = the TMEM lane quarter the
-// warp can reach):
-//   G  Gram = K K^t (tcgen05) of the fp16 K tile `kt`; L_rj = beta_r Gram_rj (j < r) as an fp16 tile in shared memory
-//   D  warp w: D_w = (I + L_ww)^-1 by forward substitution (fp32, lane = column), stored as fp16
-//   S  warp j: block column j of A_b = (I + L)^-1 diag(beta):  A_b[jj] = D_j diag(beta_j),
-//      A_b[ij] = -D_i sum_{k=j}^{i-1} L_ik A_b[kj]  (i > j; a right scaling commutes with the recursion).  A block column
+// warp can reach).  The chunk's Gram = K K^t has been issued to the group's ACC already (by the previous call, or by the
+// producer loop for the group's first chunk), and the chunk's beta sits in the scratch:
+//   G  L_rj = beta_r Gram_rj (j < r) as an fp16 tile in shared memory
+//   D  warp w: D_w = (I + L_ww)^-1 by forward substitution (fp32, lane = column), stored transposed as fp16
+//   S  warp j: block row j of A_b^t = diag(beta) (I + L)^-t:  A_b^t[jj] = diag(beta_j) D_j^t,
+//      A_b^t[ji] = -(sum_{k=j}^{i-1} A_b^t[jk] L_ik^t) D_i^t  (i > j; a left scaling commutes with the recursion).  A block row
 //      depends only on L, the D_i and its own earlier blocks, so the four warps run without a barrier; operands come from
-//      shared memory by ldmatrix, products are single-pass fp16 mma.sync (A_b only feeds a 16-bit tile).
-//   W  W'^t = K^t A_b (tcgen05) -> the MN-major W' tile of (3') in the group's output slot.
+//      shared memory by ldmatrix, the sum feeds the second product from registers (C fragment -> A fragment), products
+//      are single-pass fp16 mma.sync (A_b only feeds a 16-bit tile).
+//   W  W'^t = K^t A_b (tcgen05) -> the MN-major W' tile of (3') in the group's output slot
+// and then the Gram of the group's next chunk (`kt_next` != 0) is issued, so that it runs under the next call's waits.
 // `it` = the chunk's iteration (the group's own counter is it / kR_Groups).
 __device__ __forceinline__ void r_produce(uint8_t* smem, R_Bars* bars, volatile int* abort_flag, uint32_t tmem, int gi, int gtid,
-                                          int wq, int it, uint32_t kt, uint32_t out
+                                          int wq, int it, int nc, uint32_t kt, uint32_t out
                                           ) {
   const int warp = gtid >> 5, lane = gtid & 31;
   const uint32_t smem_base = smem_u32(smem);
   const uint32_t scr = smem_base + kR_OffScr + gi * kR_ScrBytes;
-  const uint32_t s_l = scr + kR_ScrL, s_d = scr + kR_ScrD, s_t = scr + kR_ScrT + warp * 16 * kR_DPitch, s_b = scr + kR_ScrB;
+  const uint32_t s_l = scr + kR_ScrL, s_d = scr + kR_ScrD, s_b = scr + kR_ScrB;
   const uint32_t ab_tile = smem_base + kR_OffAb + gi * kTileB;
-  const uint32_t gr = smem_base + kR_OffGate + (it & (kR_GateSlots - 1)) * kR_GateFloats * 4;
   const uint32_t acc_col = tmem + kR_ColACC + 64 * gi;
   const uint32_t acc_t = acc_col + ((uint32_t)(32 * wq) << 16);
   const int itg = it / kR_Groups;  // phase of acc_done is 2 itg (Gram), 2 itg + 1 (W')
 
-  if (gtid < kC) sts32(s_b + 4 * gtid, __float_as_uint(lds32f(gr + 4 * (kC + gtid))));
-  tc_fence_before();
-  named_bar_sync(3 + gi, 128);  // beta is in place; every warp's TMEM reads of ACC for the group's previous chunk are done
-
-  // ---- G: Gram on the tensor pipe, then L as an fp16 tile (the upper triangle as zeros)
-  if (wq == 0) {
-    tc_fence_after();
-    f_issue_gram(acc_col, kt, &bars->acc_done[gi]);
-  }
+  if (it >= 0) {
+  // ---- G: L as an fp16 tile (the upper triangle as zeros): row r = 128 bytes, 16-byte pieces swizzled with r & 7
   if (wq < 2) {  // Gram rows 0..63 sit in TMEM lanes 0..63: the two warps of the group that reach them
     s2_wait_warp(&bars->acc_done[gi], (2 * itg) & 1, abort_flag, lane);
     tc_fence_after();
@@ -451,23 +439,22 @@ __device__ __forceinline__ void r_produce(uint8_t* smem, R_Bars* bars, volatile 
   }
   named_bar_sync(3 + gi, 128);
 
-  // ---- D: diagonal block `warp`, lane c (and its twin c + 16) = column c: a_r = delta_rc - sum_{j < r} L_rj a_j
+  // ---- D: diagonal block `warp` = [[L11, 0], [L21, L22]] in 8 x 8 blocks.  D1 = (I + L11)^-1 and D2 = (I + L22)^-1 by
+  // forward substitution (fp32; lanes 0..7 = the columns of D1, lanes 8..15 = those of D2, lanes 16..31 their twins), then
+  // D21^t = -(D1^t L21^t) D2^t by two mma.sync on the block-diagonal D^t (zero sub-blocks contribute nothing).  Stored:
+  // D^t as fp16 (the strips' right factors) and A_b^t[ww] = diag(beta) D^t into the tile.
   {
-    const int cc = lane & 15;
-    float a[16];
-    uint4 lo[16], hi[8];  // row r of the block: 16 halves = pieces 2 warp, 2 warp + 1 of row 16 warp + r
+    const int g = (lane >> 3) & 1, c = lane & 7;
+    const int Rb = 16 * warp + 8 * g;  // first row / column of this lane's 8 x 8 block
+    float a[8];
+    uint4 lw[8];
 #pragma unroll
-    for (int r = 1; r < 16; ++r) {
-      const int R = 16 * warp + r;
-      lo[r] = lds128(s_l + R * 128 + (((2 * warp) ^ (R & 7)) << 4));
-      if (r > 8) hi[r - 8] = lds128(s_l + R * 128 + (((2 * warp + 1) ^ (R & 7)) << 4));
-    }
-    a[0] = (cc == 0) ? 1.f : 0.f;
+    for (int r = 1; r < 8; ++r) lw[r] = lds128(s_l + (Rb + r) * 128 + (((2 * warp + g) ^ ((Rb + r) & 7)) << 4));
+    a[0] = (c == 0) ? 1.f : 0.f;
 #pragma unroll
-    for (int r = 1; r < 16; ++r) {
-      const uint32_t w[8] = {lo[r].x, lo[r].y, lo[r].z, lo[r].w, r > 8 ? hi[r - 8].x : 0u, r > 8 ? hi[r - 8].y : 0u,
-                             r > 8 ? hi[r - 8].z : 0u, r > 8 ? hi[r - 8].w : 0u};
-      float p0 = (r == cc) ? 1.f : 0.f, p1 = 0.f;
+    for (int r = 1; r < 8; ++r) {
+      const uint32_t w[4] = {lw[r].x, lw[r].y, lw[r].z, lw[r].w};
+      float p0 = (r == c) ? 1.f : 0.f, p1 = 0.f;
 #pragma unroll
       for (int j = 0; j < r; ++j) {
         const float l = (j & 1) ? f16hi(w[j >> 1]) : f16lo(w[j >> 1]);
@@ -476,63 +463,83 @@ __device__ __forceinline__ void r_produce(uint8_t* smem, R_Bars* bars, volatile 
       }
       a[r] = p0 + p1;
     }
-    // lanes 0..15 store D (for the strips' left factors), their twins store A_b[ww] = D diag(beta)
-    if (lane < 16) {
-#pragma unroll
-      for (int r = 0; r < 16; ++r) sts16(s_d + warp * 16 * kR_DPitch + r * kR_DPitch + 2 * cc, f16_bits(a[r]));
-    } else {
-      const float bc = lds32f(s_b + 4 * (16 * warp + cc));
-#pragma unroll
-      for (int r = 0; r < 16; ++r) {
-        const int R = 16 * warp + r;
-        sts16(ab_tile + R * 128 + (((2 * warp + (cc >> 3)) ^ (R & 7)) << 4) + 2 * (cc & 7), f16_bits(a[r] * bc));
-      }
+    // the lane holds column c of D_g = row c of D_g^t: eight contiguous halves
+    const int R = Rb + c;
+    const float br = lds32f(s_b + 4 * (16 * warp + (lane >> 2)));  // beta of row 16 warp + gq (the merge's stores)
+    const float sc = lane < 16 ? 1.f : lds32f(s_b + 4 * R);
+    const uint32_t dst = lane < 16 ? s_d + (16 * warp + 8 * g + c) * kR_DPitch + 16 * g
+                                   : ab_tile + R * 128 + (((2 * warp + g) ^ (R & 7)) << 4);
+    sts128(dst, make_uint4(pack_f16(a[0] * sc, a[1] * sc), pack_f16(a[2] * sc, a[3] * sc), pack_f16(a[4] * sc, a[5] * sc),
+                           pack_f16(a[6] * sc, a[7] * sc)));
+    __syncwarp();
+    {
+      const int lrow = (lane & 7) + ((lane >> 3) & 1) * 8, lhi = lane >> 4, gq = lane >> 2, tq = lane & 3;
+      uint32_t af[4], b0, b1;
+      float p[4] = {0.f, 0.f, 0.f, 0.f}, q[4] = {0.f, 0.f, 0.f, 0.f};
+      ldmatrix_x4(af, s_d + (16 * warp + lrow) * kR_DPitch + 16 * lhi);  // block-diagonal D^t (a stale D21^t meets zeros)
+      const int Rl = 16 * warp + 8 + (lane & 7);
+      ldmatrix_x1(b0, s_l + Rl * 128 + (((2 * warp) ^ (Rl & 7)) << 4));   // L21 as the B operand L21^t, n = 8..15, k = 0..7
+      ldmatrix_x1_trans(b1, s_d + (16 * warp + 8 + (lane & 7)) * kR_DPitch + 16);  // D2^t, k = 8..15, n = 8..15
+      mma_f16_16816(p, af[0], af[1], af[2], af[3], b0, 0u);                 // P[:, 8..15] = D^t[:, 0..7] L21^t
+      mma_f16_16816(q, 0u, 0u, pack_f16(p[0], p[1]), pack_f16(p[2], p[3]), 0u, b1);  // Q[:, 8..15] = P[:, 8..15] D2^t
+      const int R0 = 16 * warp + gq;
+      sts32(s_d + R0 * kR_DPitch + 16 + 4 * tq, pack_f16(-q[0], -q[1]));
+      sts32(ab_tile + R0 * 128 + (((2 * warp + 1) ^ (R0 & 7)) << 4) + 4 * tq, pack_f16(-q[0] * br, -q[1] * br));
     }
   }
   named_bar_sync(3 + gi, 128);
 
-  // ---- S: block column `warp` of A_b
+  // ---- S: block row `warp` of A_b^t.  Running sums Q_i = sum_k A_b^t[jk] L_ik^t for every later block i are kept in
+  // registers and every product is issued as soon as its left factor exists, so that the dependent chain is two mma.sync
+  // per block (the last term of the sum, then D_i^t) and no result goes through shared memory on its way to the next
+  // product (C fragment -> A fragment).
   {
     const int j = warp;
-    const int lrow = (lane & 7) + ((lane >> 3) & 1) * 8, lhi = lane >> 4;  // ldmatrix.x4: this lane's row / 8-column half
+    const int lrow = (lane & 7) + ((lane >> 3) & 1) * 8, lhi = lane >> 4;   // ldmatrix.x4, A-operand order of the four 8 x 8
+    const int brow = (lane & 7) + ((lane >> 4) << 3), bhi = (lane >> 3) & 1;  // B-operand order (n-tile major)
     const int gq = lane >> 2, tq = lane & 3;
-#pragma unroll 1
-    for (int i = j + 1; i < 4; ++i) {
-      float acc[2][4];
-      block_zero(acc);
-#pragma unroll 1
-      for (int k = j; k < i; ++k) {  // acc += L_ik A_b[kj]
-        uint32_t af[4], bf[4];
-        const int Ra = 16 * i + lrow, Rb = 16 * k + lrow;
-        ldmatrix_x4(af, s_l + Ra * 128 + (((2 * k + lhi) ^ (Ra & 7)) << 4));
-        ldmatrix_x4_trans(bf, ab_tile + Rb * 128 + (((2 * j + lhi) ^ (Rb & 7)) << 4));
-        mma_f16_16816(acc[0], af[0], af[1], af[2], af[3], bf[0], bf[1]);
-        mma_f16_16816(acc[1], af[0], af[1], af[2], af[3], bf[2], bf[3]);
+    float q[4][2][4];
+#pragma unroll
+    for (int i = 1; i < 4; ++i) block_zero(q[i]);
+    uint32_t cur[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      if (k < j) continue;  // warp-uniform
+      if (k == j) {
+        const int Ra = 16 * j + lrow;
+        ldmatrix_x4(cur, ab_tile + Ra * 128 + (((2 * j + lhi) ^ (Ra & 7)) << 4));  // the diagonal block of phase D
       }
 #pragma unroll
-      for (int nt = 0; nt < 2; ++nt) {
-        sts32(s_t + gq * kR_DPitch + 2 * (8 * nt + 2 * tq), pack_f16(acc[nt][0], acc[nt][1]));
-        sts32(s_t + (gq + 8) * kR_DPitch + 2 * (8 * nt + 2 * tq), pack_f16(acc[nt][2], acc[nt][3]));
+      for (int i = k + 1; i < 4; ++i) {  // Q_i += A_b^t[jk] L_ik^t
+        uint32_t bf[4];
+        const int Rl = 16 * i + brow;
+        ldmatrix_x4(bf, s_l + Rl * 128 + (((2 * k + bhi) ^ (Rl & 7)) << 4));
+        mma_f16_16816(q[i][0], cur[0], cur[1], cur[2], cur[3], bf[0], bf[1]);
+        mma_f16_16816(q[i][1], cur[0], cur[1], cur[2], cur[3], bf[2], bf[3]);
       }
-      __syncwarp();
-      {  // A_b[ij] = -D_i tmp
-        uint32_t af[4], bf[4];
-        ldmatrix_x4(af, s_d + i * 16 * kR_DPitch + lrow * kR_DPitch + 16 * lhi);
-        ldmatrix_x4_trans(bf, s_t + lrow * kR_DPitch + 16 * lhi);
+      {  // A_b^t[j, k + 1] = -Q_{k+1} D_{k+1}^t
+        const int i = k + 1;
+        const uint32_t a0 = pack_f16(q[i][0][0], q[i][0][1]), a1 = pack_f16(q[i][0][2], q[i][0][3]);
+        const uint32_t a2 = pack_f16(q[i][1][0], q[i][1][1]), a3 = pack_f16(q[i][1][2], q[i][1][3]);
+        uint32_t bf[4];
+        float acc[2][4];
+        ldmatrix_x4_trans(bf, s_d + (i * 16 + lrow) * kR_DPitch + 16 * lhi);
         block_zero(acc);
-        mma_f16_16816(acc[0], af[0], af[1], af[2], af[3], bf[0], bf[1]);
-        mma_f16_16816(acc[1], af[0], af[1], af[2], af[3], bf[2], bf[3]);
+        mma_f16_16816(acc[0], a0, a1, a2, a3, bf[0], bf[1]);
+        mma_f16_16816(acc[1], a0, a1, a2, a3, bf[2], bf[3]);
+        cur[0] = pack_f16(-acc[0][0], -acc[0][1]);
+        cur[1] = pack_f16(-acc[0][2], -acc[0][3]);
+        cur[2] = pack_f16(-acc[1][0], -acc[1][1]);
+        cur[3] = pack_f16(-acc[1][2], -acc[1][3]);
+        const int R0 = 16 * j + gq, R1 = R0 + 8;
+        sts32(ab_tile + R0 * 128 + (((2 * i) ^ (R0 & 7)) << 4) + 4 * tq, cur[0]);
+        sts32(ab_tile + R1 * 128 + (((2 * i) ^ (R1 & 7)) << 4) + 4 * tq, cur[1]);
+        sts32(ab_tile + R0 * 128 + (((2 * i + 1) ^ (R0 & 7)) << 4) + 4 * tq, cur[2]);
+        sts32(ab_tile + R1 * 128 + (((2 * i + 1) ^ (R1 & 7)) << 4) + 4 * tq, cur[3]);
       }
-#pragma unroll
-      for (int nt = 0; nt < 2; ++nt) {
-        const int R0 = 16 * i + gq, R1 = R0 + 8;
-        sts32(ab_tile + R0 * 128 + (((2 * j + nt) ^ (R0 & 7)) << 4) + 4 * tq, pack_f16(-acc[nt][0], -acc[nt][1]));
-        sts32(ab_tile + R1 * 128 + (((2 * j + nt) ^ (R1 & 7)) << 4) + 4 * tq, pack_f16(-acc[nt][2], -acc[nt][3]));
-      }
-      __syncwarp();
     }
   }
-  fence_proxy_async();  // the A_b tile must be visible to the tensor pipe's reads
+  fence_proxy_async();  // the A_b^t tile must be visible to the tensor pipe's reads
   named_bar_sync(3 + gi, 128);
 
   // ---- W: W'^t = K^t A_b on the tensor pipe: thread = dk index c' holds W'[0..63][c']; packed as token pairs into row
@@ -541,9 +548,9 @@ __device__ __forceinline__ void r_produce(uint8_t* smem, R_Bars* bars, volatile 
     tc_fence_after();
     r_issue_w(acc_col, kt, ab_tile, &bars->acc_done[gi]);
   }
-  s2_wait_warp(&bars->acc_done[gi], (2 * itg + 1) & 1, abort_flag, lane);
   // the group's output slot is free once (3') of its previous chunk has completed
   if (it >= kR_Groups) s2_wait_warp(&bars->out_free[gi], (itg - 1) & 1, abort_flag, lane);
+  s2_wait_warp(&bars->acc_done[gi], (2 * itg + 1) & 1, abort_flag, lane);
   tc_fence_after();
   {
     const int cr = 32 * wq + lane;  // dk index = TMEM lane
@@ -567,6 +574,42 @@ __device__ __forceinline__ void r_produce(uint8_t* smem, R_Bars* bars, volatile 
   fence_proxy_async();
   __syncwarp();
   if (lane == 0) mbar_arrive(&bars->out_full[gi]);  // count 4: one arrival per warp of the group
+  }
+
+  // ---- the group's next chunk: its beta into the scratch, its Gram onto the tensor pipe
+  const int itn = it + kR_Groups;
+  if (itn < nc) {
+    s2_wait_warp(&bars->gate_full[itn & (kR_GateSlots - 1)], (itn / kR_GateSlots) & 1, abort_flag, lane);
+    if (gtid < kC)
+      sts32(s_b + 4 * gtid, __float_as_uint(lds32f(smem_base + kR_OffGate + ((itn & (kR_GateSlots - 1)) * kR_GateFloats + kC + gtid) * 4)));
+    named_bar_sync(3 + gi, 128);  // every warp's TMEM reads of ACC are done; beta is in place
+    if (wq == 0) {
+      const int ksn = itn % kR_KStages;
+      s2_wait_warp(&bars->k_ready[ksn], (itn / kR_KStages) & 1, abort_flag, lane);
+      tc_fence_after();
+      f_issue_gram(acc_col, smem_base + kR_OffK + ksn * 2 * kTileB, &bars->acc_done[gi]);
+    }
+  }
+}
+
+// One 64 x 128 tile (two TMA boxes) bf16 -> fp16 in place, rows at or beyond `valid` zeroed; one warp.  Element-wise on
+// 16-bit lanes, so the 128B swizzle of the boxes is untouched.  Shared by the K and the V converter warps (one copy of the
+// code: the kernel's hot loops have to fit the 32 KB instruction cache).
+__device__ __noinline__ void r_convert_tile(uint32_t tile, int valid, int lane) {
+#pragma unroll 1
+  for (int i0 = 0; i0 < 32; i0 += 4) {  // 16-byte piece p of the tile: token (p % 512) / 8
+    uint4 w[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) w[j] = lds128(tile + 16 * (lane + 32 * (i0 + j)));
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int p = lane + 32 * (i0 + j);
+      uint4 o = cvt8_bf16_f16(w[j]);
+      if (((p & 511) >> 3) >= valid) o = make_uint4(0u, 0u, 0u, 0u);
+      sts128(tile + 16 * p, o);
+    }
+  }
+  fence_proxy_async();  // the fp16 tile must be visible to the tensor pipe's reads
 }
 
 // ---------------------------------------------------------------------------------------------------- kernel
@@ -708,20 +751,7 @@ __global__ void __launch_bounds__(kR_Threads, 1)
       const int valid = it == 0 ? last_valid : kC;
       const uint32_t kt = smem_base + kR_OffK + kst * 2 * kTileB;
       f_wait_lazy(&bars->k_full[kst], (it / kR_KStages) & 1, abort_flag);
-#pragma unroll 1
-      for (int i0 = 0; i0 < 32; i0 += 8) {  // 16-byte piece p of the tile: token (p % 512) / 8
-        uint4 w[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j) w[j] = lds128(kt + 16 * (lane + 32 * (i0 + j)));
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const int p = lane + 32 * (i0 + j);
-          uint4 o = cvt8_bf16_f16(w[j]);
-          if (((p & 511) >> 3) >= valid) o = make_uint4(0u, 0u, 0u, 0u);
-          sts128(kt + 16 * p, o);
-        }
-      }
-      fence_proxy_async();  // the fp16 K tile must be visible to the tensor pipe's reads
+      r_convert_tile(kt, valid, lane);
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars->k_ready[kst]);
       __syncwarp();
@@ -734,20 +764,7 @@ __global__ void __launch_bounds__(kR_Threads, 1)
       const int valid = iv == 0 ? last_valid : kC;
       const uint32_t vt = smem_base + kR_OffV + vst * 2 * kTileB;
       f_wait_lazy(&bars->v_full[vst], (iv / kR_VStages) & 1, abort_flag);
-#pragma unroll 1
-      for (int i0 = 0; i0 < 32; i0 += 8) {
-        uint4 w[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j) w[j] = lds128(vt + 16 * (lane + 32 * (i0 + j)));
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const int p = lane + 32 * (i0 + j);
-          uint4 o = cvt8_bf16_f16(w[j]);
-          if (((p & 511) >> 3) >= valid) o = make_uint4(0u, 0u, 0u, 0u);
-          sts128(vt + 16 * p, o);
-        }
-      }
-      fence_proxy_async();
+      r_convert_tile(vt, valid, lane);
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars->v_ok[vst]);
       __syncwarp();
@@ -757,13 +774,12 @@ __global__ void __launch_bounds__(kR_Threads, 1)
     const int gi = (warp - kR_WProd) >> 2, gtid = tid - 32 * kR_WProd - 128 * gi;
     // the blocks above the diagonal of the group's A_b tile are never written: zero the tile once
     for (int p = gtid; p < kTileB / 16; p += 128) sts128(smem_base + kR_OffAb + gi * kTileB + 16 * p, make_uint4(0u, 0u, 0u, 0u));
+    for (int p = gtid; p < kR_ScrBytes / 16; p += 128) sts128(smem_base + kR_OffScr + gi * kR_ScrBytes + 16 * p, make_uint4(0u, 0u, 0u, 0u));
     named_bar_sync(3 + gi, 128);
 #pragma unroll 1
-    for (int it = gi; it < nc; it += kR_Groups) {
-      const int kst = it % kR_KStages;
-      f_wait_lazy(&bars->gate_full[it & (kR_GateSlots - 1)], (it / kR_GateSlots) & 1, abort_flag);
-      f_wait_lazy(&bars->k_ready[kst], (it / kR_KStages) & 1, abort_flag);
-      r_produce(smem, bars, abort_flag, tmem, gi, gtid, warp & 3, it, smem_base + kR_OffK + kst * 2 * kTileB,
+    for (int it = gi - kR_Groups; it < nc; it += kR_Groups) {  // the first pass only primes the group's first chunk
+      const int kst = (it + kR_KStages) % kR_KStages;
+      r_produce(smem, bars, abort_flag, tmem, gi, gtid, warp & 3, it, nc, smem_base + kR_OffK + kst * 2 * kTileB,
                 smem_base + kR_OffOut + gi * 2 * kTileB
                 );
     }
