@@ -10,9 +10,6 @@
 //   Units the fp16 operands cannot carry go to a device-side list that the fp32 family recomputes inside the same call.
 #include <cuda.h>
 #include <cuda_fp16.h>
-#ifdef HYPIC_PROF
-#include <stdio.h>
-#endif
 #include <stdlib.h>
 
 #include "common.cuh"
