@@ -837,7 +837,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layers", type=int, default=36, help="linear layers of the cfg2 request (36 = as written)")
     ap.add_argument("--e2e-layers", type=int, default=4, help="layers per end-to-end step (bounds pinned host memory)")
-    ap.add_argument("--fold", type=int, default=4,
+    ap.add_argument("--fold", type=int, default=6,
                     help="independent layers folded into the head axis per library call (1 = one call per layer)")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="weak: one private cfg2 request per rank (default); strong: ONE request, its segments LPT-sharded "

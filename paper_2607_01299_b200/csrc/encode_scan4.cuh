@@ -294,6 +294,13 @@ __device__ __forceinline__ void r_chain(uint8_t* smem, R_Bars* bars, volatile in
 #pragma unroll
       for (int j = 0; j < 16; ++j) u[j] = pack_f16(__uint_as_float(y[2 * j]), __uint_as_float(y[2 * j + 1]));
       tmem_st16(tH + 16 * hf, u);
+      tmem_st_wait();
+      tc_fence_before();
+      named_bar_sync(1, 256);  // the whole chain has written U'': (4') goes out first, fY is formed while it runs
+      if (cw == 0) {
+        tc_fence_after();
+        r_issue4(tmem + kR_ColR, tmem + kR_ColH, smem_base + kR_OffK + kst * 2 * kTileB, &bars->m4_done, &bars->k_free[kst]);
+      }
 #pragma unroll
       for (int p8 = 0; p8 < 4; ++p8) {  // tokens 32 hf + 8 p8 .. + 7 -> 16-byte piece 4 hf + p8 of the row
         uint32_t wv[8] = {wq4[2 * p8].x, wq4[2 * p8].y, wq4[2 * p8].z, wq4[2 * p8].w,
@@ -308,14 +315,9 @@ __device__ __forceinline__ void r_chain(uint8_t* smem, R_Bars* bars, volatile in
         sts128(fy_row + (((4 * hf + p8) ^ (row & 7)) << 4), make_uint4(o[0], o[1], o[2], o[3]));
       }
     }
-    tmem_st_wait();
-    tc_fence_before();
     fence_proxy_async();     // the fY tile must be visible to the tensor pipe's reads
-    named_bar_sync(1, 256);  // the whole chain has written U'' and fY
-    if (cw == 0) {
-      tc_fence_after();
-      r_issue4(tmem + kR_ColR, tmem + kR_ColH, smem_base + kR_OffK + kst * 2 * kTileB, &bars->m4_done, &bars->k_free[kst]);
-    } else if (cw == 1) {  // (5) is off the critical path: a second warp issues it while (4') runs
+    named_bar_sync(2, 256);  // the whole chain has written fY
+    if (cw == 1) {  // (5) is off the critical path: a second warp issues it while (4') runs
       s2_wait_warp(&bars->v_ok[vst], (it / kR_VStages) & 1, abort_flag, lane);
       tc_fence_after();
       r_issue5(tmem + kR_ColE, smem_base + kR_OffV + vst * 2 * kTileB, smem_base + kR_OffFy, it > 0 ? 1u : 0u,

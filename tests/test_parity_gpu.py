@@ -249,13 +249,14 @@ def test_cfg2_one_layer_every_unit():
 
 
 def test_cfg2_folded_layers_launch_configuration_every_unit():
-    """cfg2 in the launch configuration bench.py times: 4 independent layers folded into the head axis (H = 128,
-    SURVEY.md 8(b)), full size (20 x 4096).  The folded call must reproduce the per-layer calls bit for bit (units
-    are independent), ALL 2,560 units are checked against the oracle, and so is the folded composition of every head."""
-    layers = [wl.cfg2_layer(l, "cuda") for l in range(4)]
+    """cfg2 in the launch configuration bench.py times: 6 independent layers folded into the head axis (H = 192,
+    SURVEY.md 8(b); bench.py's --fold default: 3,840 units = 25.9 waves on 148 SMs), full size (20 x 4096).  The folded
+    call must reproduce the per-layer calls bit for bit (units are independent), ALL 3,840 units are checked against the
+    oracle, and so is the folded composition of every head."""
+    layers = [wl.cfg2_layer(l, "cuda") for l in range(6)]
     inp = wl.fold_layers(layers)
     E, T = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
-    for l in (0, 3):
+    for l in (0, 5):
         E1, T1 = gpu_encode(layers[l], hb.HYPIC_IMPL_AUTO)
         assert torch.equal(E[:, 32 * l:32 * l + 32], E1) and torch.equal(T[:, 32 * l:32 * l + 32], T1)
         del E1, T1
