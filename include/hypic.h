@@ -86,8 +86,9 @@ size_t hypic_segment_encode_workspace(int32_t n_seg, int32_t t_total, int32_t H,
  * Built envelope (shapes): dk in {64, 128}; dv in [1, 1024] for the SIMT family (fp32 CUDA cores), dv = dk = 128 with
  * bf16 k/v for the tensor family (tcgen05; scalar or per-channel gate), which HYPIC_IMPL_AUTO takes whenever the shape
  * allows.  Values: any finite inputs.  The tensor family computes with 16-bit operands; what those cannot carry -- a
- * per-channel chunk whose log-decay leaves [-9, 0], weighted values or states beyond fp16's range -- is detected on the
- * device per (segment, head) unit, and exactly those units are recomputed by the fp32 family inside the same call, on the
+ * per-channel chunk whose log-decay leaves [-9, 0], values or states beyond fp16's range, a scalar-gate unit of more
+ * than 8,192 tokens whose T is still representable (sum g > -72: the 16-bit rounding walk would leave the 3e-3 tolerance
+ * of T there) -- is detected on the device per (segment, head) unit, and exactly those units are recomputed by the fp32 family inside the same call, on the
  * same stream, with no host synchronisation and no caller action (the scalar gate never enters the 16-bit algebra, so it
  * has no log-decay limit at all).  hypic_envelope_violation_count remains as a diagnostic counter.
  * H, n_seg, lengths arbitrary.  Inputs are only read; E and T are fully overwritten.

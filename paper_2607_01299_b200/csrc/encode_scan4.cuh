@@ -59,6 +59,7 @@ constexpr int kR_GateFloats = 2 * kC;
 constexpr int kR_OffXch = kR_OffGate + kR_GateSlots * kR_GateFloats * 4;  // fp32 [2][128]: lane maxima of the chain halves
 constexpr int kR_OffBar = kR_OffXch + 1024;
 constexpr int kR_Smem = kR_OffBar + 512 + 1024;
+constexpr int kR_MaxChunksFp16 = 128;  // 8,192 tokens: beyond, a representable T leaves the 3e-3 tolerance
 constexpr uint32_t kR_ColR = 0, kR_ColE = 128, kR_ColH = 256, kR_ColDY = 320, kR_ColACC = 384;
 
 struct R_Bars {
@@ -374,7 +375,11 @@ __device__ __forceinline__ void r_chain(uint8_t* smem, R_Bars* bars, volatile in
       }
     }
   }
-  if (bad) bars->bad = 1;  // an fp16 operand overflowed somewhere: the unit goes to the fp32 fallback list
+  // The rounding of the fp16 operands is a random walk over the chunks: T is off by ~1.4e-3 after 4,096 tokens, 2.2e-3 after
+  // 8,192 and 3.0e-3 (the tolerance) after 16,384.  A longer unit whose T is still representable (a gate too weak to
+  // push it below the 1e-30 floor of DESIGN.md reading S6; ||R|| <= sqrt(dk)) is recomputed by the fp32 family.
+  if (nc > kR_MaxChunksFp16 && bars->g_total > -72.0) bad = true;
+  if (bad) bars->bad = 1;  // ... or an fp16 operand overflowed somewhere: the unit goes to the fp32 fallback list
 }
 
 // ---------------------------------------------------------------------------------------------------- producers
