@@ -420,7 +420,9 @@ __device__ __forceinline__ void r_produce(uint8_t* smem, R_Bars* bars, volatile 
   const int itg = it / kR_Groups;  // phase of acc_done is 2 itg (Gram), 2 itg + 1 (W')
 
   if (it >= 0) {
-  // ---- G: L as an fp16 tile (the upper triangle as zeros): row r = 128 bytes, 16-byte pieces swizzled with r & 7
+  // ---- G: diag(beta) Gram as an fp16 tile: row r = 128 bytes, 16-byte pieces swizzled with r & 7.  Only its strictly
+  // lower triangle (= L) is ever read: the substitutions stop at j < r, the merges and strips take blocks below the
+  // diagonal -- so nothing is masked here.
   if (wq < 2) {  // Gram rows 0..63 sit in TMEM lanes 0..63: the two warps of the group that reach them
     s2_wait_warp(&bars->acc_done[gi], (2 * itg) & 1, abort_flag, lane);
     tc_fence_after();
@@ -433,12 +435,12 @@ __device__ __forceinline__ void r_produce(uint8_t* smem, R_Bars* bars, volatile 
       tmem_ld_wait();
 #pragma unroll
       for (int p8 = 0; p8 < 4; ++p8) {
-        const int j = 32 * cb + 8 * p8;
         uint32_t o[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
-          o[q] = pack_f16((j + 2 * q < r) ? br * __uint_as_float(x[8 * p8 + 2 * q]) : 0.f,
-                          (j + 2 * q + 1 < r) ? br * __uint_as_float(x[8 * p8 + 2 * q + 1]) : 0.f);
+        for (int q = 0; q < 4; ++q) {
+          mul2(x[8 * p8 + 2 * q], x[8 * p8 + 2 * q + 1], br);
+          o[q] = pack_f16(__uint_as_float(x[8 * p8 + 2 * q]), __uint_as_float(x[8 * p8 + 2 * q + 1]));
+        }
         sts128(s_l + r * 128 + (((4 * cb + p8) ^ (r & 7)) << 4), make_uint4(o[0], o[1], o[2], o[3]));
       }
     }
