@@ -14,6 +14,7 @@ from parity_util import (per_unit_rel, TOL_BF16, TOL_F32, check_E, check_T, orac
                          oracle_encode_units, oracle_encode_units_batched)
 
 pytestmark = pytest.mark.gpu
+T_FLOOR_TEST = 1e-30  # reading S6: below this norm T is compared absolutely
 
 IMPLS = [("auto", hb.HYPIC_IMPL_AUTO), ("simt", hb.HYPIC_IMPL_SIMT), ("tensor", hb.HYPIC_IMPL_TENSOR)]
 
@@ -386,6 +387,34 @@ def test_fallback_list_takes_only_the_units_that_need_it():
     keep[1, 2] = False
     assert torch.equal(E[keep], E0[keep]) and torch.equal(T[keep], T0[keep])
     assert not torch.equal(E[1, 2], E0[1, 2])
+
+
+def test_tensor_encode_random_ragged_mixes_are_reproducible_and_match_the_fp32_family():
+    """24 random mixes of segment counts, head counts, lengths (empty, shorter than a chunk, ragged, up to 2,100 tokens)
+    and gate strengths through the fused tensor kernel: every call reproduces itself bit for bit (the kernel pipelines
+    six warp roles through some forty barriers), and matches the fp32 SIMT family -- itself checked against the oracle
+    above -- within the bf16 tolerance on every unit."""
+    rng = np.random.default_rng(123)
+
+    def rel(a, b):
+        num = (a.double() - b.double()).flatten(2).norm(dim=-1)
+        den = b.double().flatten(2).norm(dim=-1)
+        return float(torch.where(den > T_FLOOR_TEST, num / den.clamp_min(1e-300), num).max())
+
+    for trial in range(24):
+        n_seg, H, mode = int(rng.integers(1, 40)), int(rng.integers(1, 9)), trial % 4
+        lens = [int(x) for x in rng.integers(0, [700, 130, 2100, 66][mode], n_seg)]
+        if sum(lens) == 0:
+            lens[0] = 5
+        inp = wl.make_encode_inputs(lens, H, 128, 128, kv_dtype=torch.bfloat16, g_lo=[-0.05, -0.5, -0.01, -0.1][mode],
+                                    seed=wl.seed_for(1, 100 + trial), device="cuda")
+        E1, T1 = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
+        E2, T2 = gpu_encode(inp, hb.HYPIC_IMPL_AUTO)
+        assert torch.equal(E1, E2) and torch.equal(T1, T2), f"trial {trial}: two runs differ"
+        Es, Ts = gpu_encode(inp, hb.HYPIC_IMPL_SIMT)
+        eE, eT = rel(E1, Es), rel(T1, Ts)
+        assert eE <= TOL_BF16 and eT <= TOL_BF16, f"trial {trial}: E {eE:.2e} T {eT:.2e} (H={H}, lens={lens[:8]}...)"
+    assert hb.hypic_debug_timeout_count() == 0
 
 
 def test_long_weakly_gated_segments_stay_within_tolerance():
