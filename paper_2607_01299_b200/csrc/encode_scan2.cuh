@@ -95,6 +95,7 @@ __device__ __forceinline__ void s2_wait_warp(uint64_t* bar, uint32_t parity, vol
   // the chains' waits: try_wait with a suspend-time hint, so that a waiting warp sleeps in hardware until the phase
   // completes instead of re-issuing the probe -- 16 chain warps polling st_ready in a tight loop flooded the
   // shared-memory pipeline and slowed the two converter warps they were waiting for to ~4,000 cycles per tile
+  if (mbar_test_wait(bar, parity)) return;  // already complete: the plain probe is cheaper than a suspending one
 #pragma unroll 1
   for (int i = 0; i < 64; ++i)
     if (mbar_try_wait_hint(bar, parity, 100000u)) return;

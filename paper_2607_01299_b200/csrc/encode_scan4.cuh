@@ -800,5 +800,7 @@ __global__ void __launch_bounds__(kR_Threads, 1)
   tc_fence_before();
   __syncthreads();
   if (warp == kR_WLoader) tmem_dealloc(tmem, 512);
-  if (tid == 0 && bars->bad) fb_append(fb, n_units, s * H + h);
+  // A unit whose operands overflowed -- or whose CTA ran into a wait that expired (a protocol error; counted in
+  // hypic_debug_timeout_count) -- is recomputed by the fp32 family inside the same call: no silent garbage.
+  if (tid == 0 && (bars->bad || bars->abort_flag)) fb_append(fb, n_units, s * H + h);
 }
