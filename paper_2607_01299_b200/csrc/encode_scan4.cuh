@@ -235,8 +235,13 @@ __device__ __forceinline__ void r_chain(uint8_t* smem, R_Bars* bars, volatile in
 #pragma unroll 1
   for (int it = 0; it < nc; ++it) {
     const int gi = it % kR_Groups, kst = it % kR_KStages, vst = it % kR_VStages;
-    s2_wait_warp(&bars->out_full[gi], (it / kR_Groups) & 1, abort_flag, lane);  // W' and the fp16 K tile are in place
-    if (it > 0) s2_wait_warp(&bars->m4_done, (it - 1) & 1, abort_flag, lane);
+    // One warp probes the mbarriers, the others wait at a named barrier behind it: a probe costs 200-300 cycles of a
+    // busy shared-memory pipe here, eight of them at once only add traffic (and power).
+    if (cw == 0) {
+      s2_wait_warp(&bars->out_full[gi], (it / kR_Groups) & 1, abort_flag, lane);  // W' and the fp16 K tile are in place
+      if (it > 0) s2_wait_warp(&bars->m4_done, (it - 1) & 1, abort_flag, lane);
+    }
+    named_bar_sync(5, 256);
     tc_fence_after();
     // ---- pass: Rh = fp16(R^t), this thread's 64 columns; R^t itself is only rewritten when the lane's scale is re-chosen
     {
@@ -283,7 +288,8 @@ __device__ __forceinline__ void r_chain(uint8_t* smem, R_Bars* bars, volatile in
     // columns [16 hf, 16 hf + 16); fY = fp16(w_t 2^-s DY) -> row `row` of the shared fY tile (B operand of (5); 128-byte
     // rows, 128B swizzle).  The tile is single-buffered: (5) of the previous chunk sits in front of this chunk's (3') in
     // the in-order tensor pipe, so it has completed when m3_done fires.
-    s2_wait_warp(&bars->m3_done, it & 1, abort_flag, lane);
+    if (cw == 0) s2_wait_warp(&bars->m3_done, it & 1, abort_flag, lane);
+    named_bar_sync(5, 256);
     tc_fence_after();
     {
       const uint32_t gw = gate_base + ((it & (kR_GateSlots - 1)) * kR_GateFloats + 32 * hf) * 4;
@@ -425,7 +431,8 @@ __device__ __forceinline__ void r_produce(uint8_t* smem, R_Bars* bars, volatile 
   // lower triangle (= L) is ever read: the substitutions stop at j < r, the merges and strips take blocks below the
   // diagonal -- so nothing is masked here.
   {  // M = 64: Gram row r sits in TMEM lane (r % 16) + 32 (r / 16): lanes 0..15 of every warp's quarter
-    s2_wait_warp(&bars->acc_done[gi], (2 * itg) & 1, abort_flag, lane);
+    if (wq == 0) s2_wait_warp(&bars->acc_done[gi], (2 * itg) & 1, abort_flag, lane);  // one warp probes, the group follows
+    named_bar_sync(3 + gi, 128);
     tc_fence_after();
     const int r = 16 * wq + (lane & 15);
     const float br = lds32f(s_b + 4 * r);
@@ -558,9 +565,12 @@ __device__ __forceinline__ void r_produce(uint8_t* smem, R_Bars* bars, volatile 
     tc_fence_after();
     r_issue_w(acc_col, kt, ab_tile, &bars->acc_done[gi]);
   }
-  // the group's output slot is free once (3') of its previous chunk has completed
-  if (it >= kR_Groups) s2_wait_warp(&bars->out_free[gi], (itg - 1) & 1, abort_flag, lane);
-  s2_wait_warp(&bars->acc_done[gi], (2 * itg + 1) & 1, abort_flag, lane);
+  if (wq == 0) {
+    // the group's output slot is free once (3') of its previous chunk has completed
+    if (it >= kR_Groups) s2_wait_warp(&bars->out_free[gi], (itg - 1) & 1, abort_flag, lane);
+    s2_wait_warp(&bars->acc_done[gi], (2 * itg + 1) & 1, abort_flag, lane);
+  }
+  named_bar_sync(3 + gi, 128);
   tc_fence_after();
   {
     const int cr = 32 * wq + lane;  // dk index = TMEM lane
@@ -589,9 +599,10 @@ __device__ __forceinline__ void r_produce(uint8_t* smem, R_Bars* bars, volatile 
   // ---- the group's next chunk: its beta into the scratch, its Gram onto the tensor pipe
   const int itn = it + kR_Groups;
   if (itn < nc) {
-    s2_wait_warp(&bars->gate_full[itn & (kR_GateSlots - 1)], (itn / kR_GateSlots) & 1, abort_flag, lane);
-    if (gtid < kC)
+    if (gtid < kC) {
+      s2_wait_warp(&bars->gate_full[itn & (kR_GateSlots - 1)], (itn / kR_GateSlots) & 1, abort_flag, lane);
       sts32(s_b + 4 * gtid, __float_as_uint(lds32f(smem_base + kR_OffGate + ((itn & (kR_GateSlots - 1)) * kR_GateFloats + kC + gtid) * 4)));
+    }
     named_bar_sync(3 + gi, 128);  // every warp's TMEM reads of ACC are done; beta is in place
     if (wq == 0) {
       const int ksn = itn % kR_KStages;
