@@ -25,25 +25,29 @@
 //     (4') R^t -= U'' K            M = 128 (j), N = 128, K = 64:        A = U'' = fp16(DY) from TMEM, B = the K tile
 //     (5)  E   += V^t (w Y)        M = 128 (dv), N = 128 (j), K = 64:   A = the V tile (MN-major), B = fY tile (shared)
 // with fY[j][t] = fp16(w_t 2^-s_j DY[j][t]) written by the epilogue threads as a K-major B tile.
-// Producer groups (G) Gram = K K^t and (W) W'^t = K^t A_b on tcgen05 as before; the blocked UT inverse on mma.sync.
+// Producer groups: (G) Gram = K K^t (M = 64) and (W) W'^t = K^t A_b on tcgen05; the blocked UT inverse on mma.sync.
 //
 // TMEM columns: R^t [0,128), E [128,256), Rh / U'' [256,320), DY [320,384), ACC0 [384,448), ACC1 [448,512) (one
 // accumulator per producer group: no lock).
 //
-// 16 warps (512 threads, 128 registers each):
-//   warps 0-3    chain      thread = lane j: pass Rh = fp16(R^t), epilogue U'' / fY; warp 0 issues (3'), (4'), (5)
-//   warp 4       loader     TMA boxes of K (6-deep ring, two chunks ahead of V) and V (2-deep ring)
-//   warp 5       gate       the chunk's g / beta, the weights w_t (suffix scan), a ring of 8 gate records
-//   warp 6, 7    converters K / V tile bf16 -> fp16 in place; the rows of the ragged last tile zeroed
-//   warps 8-11   producer group 0 (even iterations), warps 12-15 producer group 1 (odd iterations)
+// 20 warps (640 threads, 96 registers each):
+//   warps 0-7    chain      two warps per TMEM lane quarter: thread = (lane j, half): pass Rh = fp16(R^t) on 64 of the 128
+//                           columns, epilogue U'' / fY on 32 of the 64 tokens; warp 0 probes the mbarriers for the others
+//                           (they follow at a named barrier) and issues (3'), (4'); warp 1 issues (5)
+//   warp 8       loader     TMA boxes of K (6-deep ring, two chunks ahead of V) and V (2-deep ring)
+//   warp 9       gate       the chunk's g / beta, the weights w_t (suffix scan), a ring of 8 gate records
+//   warps 10, 11 converters K / V tile bf16 -> fp16 in place; the rows of the ragged last tile zeroed
+//   warps 12-15  producer group 0 (even iterations), warps 16-19 producer group 1 (odd iterations)
+// Named barriers: 1 (chain: Rh written / U'' written), 2 (chain: fY written; lane maxima exchanged), 5 (chain: behind the
+// probing warp), 3 + group (producers).
 #pragma once
 
 constexpr int kR_Groups = 2;
 constexpr int kR_Threads = 32 * (12 + 4 * kR_Groups);
 constexpr int kR_WChain = 0, kR_WLoader = 8, kR_WGate = 9, kR_WConv = 10, kR_WConvV = 11, kR_WProd = 12;
 constexpr int kR_KStages = 6, kR_VStages = 2, kR_GateSlots = 8;
-constexpr int kR_OffK = 0;                                        // 4 x 16 KB: K tile, two 64-column boxes [token][64]
-constexpr int kR_OffV = kR_OffK + kR_KStages * 2 * kTileB;        // 2 x 16 KB: V tile (bf16 as it arrives)
+constexpr int kR_OffK = 0;                                        // 6 x 16 KB: K tile, two 64-column boxes [token][64]
+constexpr int kR_OffV = kR_OffK + kR_KStages * 2 * kTileB;        // 2 x 16 KB: V tile (converted to fp16 in place)
 constexpr int kR_OffOut = kR_OffV + kR_VStages * 2 * kTileB;      // one 16 KB W' tile per producer group
 constexpr int kR_OffFy = kR_OffOut + kR_Groups * 2 * kTileB;      // 16 KB: fY tile [j][token]
 constexpr int kR_OffAb = kR_OffFy + 2 * kTileB;                   // one 8 KB A_b tile per producer group
