@@ -390,183 +390,8 @@ __device__ __forceinline__ void s2_chain(uint8_t* smem, S2Bars* bars, volatile i
 }
 
 
-// Scalar gate.  The gate commutes with (I - beta k k^t), so it is kept out of the tensor-core algebra altogether:
-//   T block: That = prod (I - beta_t k_t k_t^t), the ungated product; T = exp(sum g) That at write-out.  Rows are held
-//            as That_r 2^s_r, s_r re-chosen every 8th chunk so that the row maximum sits in [2^11, 2^12) (a contraction
-//            cannot grow a row by more than sqrt(dk) = 11.3, so fp16 never overflows in between).
-//   E block: stored X_E = E exp(-p), p the pending log-decay; the chunk's values enter as v_i exp(-(p + G_i)) (weights from
-//            the V converter).  When |p + G_C| would exceed ln 64 the pass multiplies X_E by exp(p + G_C), the values enter
-//            as v_i exp(G_C - G_i) <= v_i and p restarts at 0: a strongly decaying chunk degenerates to the plain
-//            "decay, then add" form, a weakly decaying one costs no TMEM rewrite at all.
-// Per chunk: pass Xh = fp16(X) -> (3) DY (+)= Xh (-W)^t -> epilogue U'' = fp16(DY) -> (4) X += U'' K.
-template <bool kIsT>
-__device__ __forceinline__ void s2_chain_sc(uint8_t* smem, S2Bars* bars, volatile int* abort_flag, uint32_t tmem, int cw,
-                                            int lane, int nc, float* __restrict__ dst_block) {
-  constexpr int b = kIsT ? 1 : 0;
-  constexpr uint32_t cX = kIsT ? 128 : 0, cH = kIsT ? 320 : 256, cD = kIsT ? 448 : 384;
-  const int q = cw & 3, hf = cw >> 2;  // TMEM lane quarter; column half
-  const int row = 32 * q + lane;
-  const uint32_t lane_base = (uint32_t)(32 * q) << 16;
-  const uint32_t tX = tmem + cX + lane_base + 64 * hf, tH = tmem + cH + lane_base + 32 * hf,
-                 tD = tmem + cD + lane_base + 32 * hf;
-  float* xch = reinterpret_cast<float*>(smem + kS2OffXch);
-  int s_exp = 0;  // T chain: the TMEM copy of this row is That_row * 2^s_exp
-
-  // X_0 = [0 ; I]
-#pragma unroll
-  for (int cb = 0; cb < 2; ++cb) {
-    uint32_t x[32];
-#pragma unroll
-    for (int i = 0; i < 32; ++i) x[i] = (kIsT && 64 * hf + 32 * cb + i == row) ? __float_as_uint(1.f) : 0u;
-    tmem_st32(tX + 32 * cb, x);
-  }
-  tmem_st_wait();
-  const uint32_t smem_base = smem_u32(smem);
-  const bool issuer = (cw == 0 && lane == 0);  // this chain's MMA-issuing thread
-
-#pragma unroll 1
-  for (int c = 0; c < nc; ++c) {
-    const int st = c % kS2Stages;
-    // converted, hence also landed.  A hardware-suspended mbarrier wait: the chains often arrive first, and a spinning
-    // chain (16 warps polling a counter) starved the three converter warps of issue slots (profiles/r02a)
-    s2_wait_warp(&bars->st_ready[st], (c / kS2Stages) & 1, abort_flag, lane);
-    if (c > 0) s2_wait_warp(&bars->m4_done[b], (c - 1) & 1, abort_flag, lane);
-    tc_fence_after();
-    // ---- pass: Xh = fp16(X) (A operand of (3)); X itself is only rewritten on a rescale
-    {
-      bool rewrite;
-      float f = 1.f;
-      if (kIsT) {
-        rewrite = (c & 7) == 0;
-      } else {
-        f = bars->resc[st];
-        rewrite = (f != 1.f);
-      }
-      if (!rewrite) {  // the common case: X stays as it is, 32 columns at a time (few live registers)
-        uint32_t x[32], hh[16];
-        tmem_ld32(tX, x);
-        tmem_ld_wait();
-#pragma unroll
-        for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x[2 * j]), __uint_as_float(x[2 * j + 1]));
-        tmem_ld32(tX + 32, x);
-        tmem_st16(tH, hh);
-        tmem_ld_wait();
-#pragma unroll
-        for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x[2 * j]), __uint_as_float(x[2 * j + 1]));
-        tmem_st16(tH + 16, hh);
-        tmem_st_wait();
-        tc_fence_before();
-        named_bar_sync(5 + b, 256);  // the whole chain has written Xh
-        if (issuer) {
-          if (!kIsT) s2_wait_count(&bars->issued1_cnt, c, abort_flag);  // (1)_c is ahead of (3)_c in the tensor pipe
-          tc_fence_after();
-          s2_issue3(tmem, smem_base + st * kS2StageBytes, b);
-          mma_commit(&bars->m3_done[b]);
-        }
-        __syncwarp();
-      } else {
-        uint32_t x0[32], x1[32];
-        tmem_ld32(tX, x0);
-        tmem_ld32(tX + 32, x1);
-        tmem_ld_wait();
-        if (kIsT) {
-          float m = 0.f;
-#pragma unroll
-          for (int i = 0; i < 32; ++i) m = fmaxf(m, fmaxf(fabsf(__uint_as_float(x0[i])), fabsf(__uint_as_float(x1[i]))));
-          xch[2 * row + hf] = m;
-          named_bar_sync(1 + q, 64);
-          m = fmaxf(m, xch[2 * row + (hf ^ 1)]);
-          // row maximum in [2^(e-127), 2^(e-126)): move it to [2^11, 2^12)
-          const int e = (int)((__float_as_uint(m) >> 23) & 0xffu);
-          int dlt = (e == 0 || e == 255) ? 0 : 138 - e;
-          dlt = max(-100, min(100, dlt));
-          s_exp += dlt;
-          f = pow2i(dlt);
-        }
-#pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          mul2(x0[2 * j], x0[2 * j + 1], f);
-          mul2(x1[2 * j], x1[2 * j + 1], f);
-        }
-        {
-          uint32_t hh[16];
-#pragma unroll
-          for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x0[2 * j]), __uint_as_float(x0[2 * j + 1]));
-          tmem_st16(tH, hh);
-#pragma unroll
-          for (int j = 0; j < 16; ++j) hh[j] = pack_f16(__uint_as_float(x1[2 * j]), __uint_as_float(x1[2 * j + 1]));
-          tmem_st16(tH + 16, hh);
-        }
-        tmem_st_wait();
-        tc_fence_before();
-        named_bar_sync(5 + b, 256);  // the whole chain has written Xh
-        if (issuer) {
-          if (!kIsT) s2_wait_count(&bars->issued1_cnt, c, abort_flag);
-          tc_fence_after();
-          s2_issue3(tmem, smem_base + st * kS2StageBytes, b);
-          mma_commit(&bars->m3_done[b]);
-        }
-        __syncwarp();
-        tmem_st32(tX, x0);  // (3) reads Xh alone; only (4) accumulates into X
-        tmem_st32(tX + 32, x1);
-        tmem_st_wait();
-      }
-    }
-
-    // ---- epilogue: U'' = fp16(DY) -> TMEM (A operand of (4)); this thread: tokens [32 hf, 32 hf + 32)
-    s2_wait_warp(&bars->m3_done[b], c & 1, abort_flag, lane);
-    tc_fence_after();
-    {
-      uint32_t y[32];
-      tmem_ld32(tD, y);
-      tmem_ld_wait();
-#pragma unroll
-      for (int j = 0; j < 16; ++j) y[j] = pack_f16(__uint_as_float(y[2 * j]), __uint_as_float(y[2 * j + 1]));  // slot j <= 2 j
-      tmem_st16(tH - 16 * hf, y);  // columns [16 hf, 16 hf + 16) of the (dead) Xh region: tokens [32 hf, 32 hf + 32)
-      tmem_st_wait();
-    }
-    tc_fence_before();
-    named_bar_sync(5 + b, 256);  // the whole chain has written U''
-    if (issuer) {
-      if (!kIsT) mbar_arrive(&bars->dy_free);  // DY_E has been read: the V converter may issue (1) of the next chunk
-      tc_fence_after();
-      s2_issue4(tmem, smem_base + st * kS2StageBytes, b);
-      mma_commit(&bars->m4_done[b]);
-      mma_commit(&bars->st_free[st]);  // count 2: released when both chains' (4) of this chunk have completed
-    }
-    __syncwarp();
-  }
-
-  // ---- a5: write this thread's 64 columns of its row; the gate (and T's row scale) is applied here, in fp64 so that a
-  // T that underflows fp32 underflows exactly like the correctly rounded result
-  s2_wait_count(&bars->fin_flag, 0, abort_flag);  // the V converter has posted p_final and g_total
-  if (nc > 0) {
-    s2_wait_warp(&bars->m4_done[b], (nc - 1) & 1, abort_flag, lane);
-    tc_fence_after();
-  }
-  const double sc = kIsT ? exp(bars->g_total - 0.6931471805599453 * (double)s_exp) : (double)expf(bars->p_final);
-  float* dst = dst_block + (size_t)row * kD + 64 * hf;
-  bool bad = false;
-#pragma unroll 1
-  for (int cb = 0; cb < 2; ++cb) {
-    uint32_t x[32];
-    tmem_ld32(tX + 32 * cb, x);
-    tmem_ld_wait();
-    float4* d4 = reinterpret_cast<float4*>(dst + 32 * cb);
-#pragma unroll
-    for (int u = 0; u < 8; ++u) {
-      float4 o;
-      o.x = (float)((double)__uint_as_float(x[4 * u]) * sc);
-      o.y = (float)((double)__uint_as_float(x[4 * u + 1]) * sc);
-      o.z = (float)((double)__uint_as_float(x[4 * u + 2]) * sc);
-      o.w = (float)((double)__uint_as_float(x[4 * u + 3]) * sc);
-      bad |= !(fabsf(o.x) <= 3.0e38f) | !(fabsf(o.y) <= 3.0e38f) | !(fabsf(o.z) <= 3.0e38f) | !(fabsf(o.w) <= 3.0e38f);
-      d4[u] = o;
-    }
-  }
-  if (bad) bars->bad = 1;
-}
-
+// (The scalar gate no longer runs through this kernel: encode_scan4.cuh.  scan2_kernel is instantiated for the
+// per-channel gate only.)
 template <bool kCh>
 __global__ void __launch_bounds__(kS2Threads, 1)
     scan2_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
@@ -713,11 +538,9 @@ __global__ void __launch_bounds__(kS2Threads, 1)
     }
     if (role == 1 && lane == 0) flag_release(&bars->fin_flag, 1);
   } else if (warp < 8) {
-    if (kCh) s2_chain<false, true>(smem, bars, abort_flag, tmem, warp, lane, nc, E + ((size_t)s * H + h) * kD * kD);
-    else s2_chain_sc<false>(smem, bars, abort_flag, tmem, warp, lane, nc, E + ((size_t)s * H + h) * kD * kD);
+    s2_chain<false, true>(smem, bars, abort_flag, tmem, warp, lane, nc, E + ((size_t)s * H + h) * kD * kD);
   } else {
-    if (kCh) s2_chain<true, true>(smem, bars, abort_flag, tmem, warp - 8, lane, nc, T + ((size_t)s * H + h) * kD * kD);
-    else s2_chain_sc<true>(smem, bars, abort_flag, tmem, warp - 8, lane, nc, T + ((size_t)s * H + h) * kD * kD);
+    s2_chain<true, true>(smem, bars, abort_flag, tmem, warp - 8, lane, nc, T + ((size_t)s * H + h) * kD * kD);
   }
   tc_fence_before();
   __syncthreads();
