@@ -405,10 +405,12 @@ int compose_tensor(const ComposeArgs& a) {
     const int rc = make_rows_tensor_map(&tmS, a.S_in, (uint64_t)units * kD);
     if (rc != HYPIC_OK) return rc;
   }
-  // heads h, h + 1 of a request as two interleaved chains of one CTA -- once there are enough units to keep every SM busy
-  // that way; with fewer (cfg2: 32 chains) one chain per CTA on twice the SMs is the faster schedule (0.076 vs 0.113 ms)
+  // heads h, h + 1 of a request as two interleaved chains of one CTA -- once one chain per CTA no longer fits one wave
+  // (a pair takes 1.5 x the time of a single chain, a second wave 2 x: cfg2 with six folded layers, 192 chains, 0.147 ms
+  // as singles); with fewer (one cfg2 layer: 32 chains) one chain per CTA on twice the SMs is the faster schedule (0.076 vs
+  // 0.113 ms)
   const DeviceInfo& di = device_info();
-  if (a.H % 2 == 0 && units >= 2LL * (di.ok ? di.sm_count : 148))
+  if (a.H % 2 == 0 && units > (long long)(di.ok ? di.sm_count : 148))
     compose_tensor_kernel<2><<<(unsigned)(units / 2), kThreads, kSmemBytes, a.stream>>>(tmE, tmS, a.S_in, a.T_pool,
                                                                                        a.seg_ids, a.cu_segs, a.R, a.H, a.S_out);
   else

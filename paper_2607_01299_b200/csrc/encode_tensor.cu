@@ -53,7 +53,7 @@ __host__ __device__ inline size_t ws_off_rec(int32_t n_seg, int32_t H, size_t ca
 // the scan CTAs so that the longest sequential scans start first); identity beyond 8192 segments.
 __global__ void chunk_offsets_kernel(const int32_t* __restrict__ cu_seqlens, int n_seg, int32_t* __restrict__ chunk_off,
                                      int32_t* __restrict__ seg_order, int2* __restrict__ chunk_meta, int cap,
-                                     int32_t* __restrict__ fb, long long n_units) {
+                                     int32_t* __restrict__ fb, long long n_units, int need_meta) {
   __shared__ int part[1024];
   const int tid = threadIdx.x;
   for (long long i = tid; i < 4 + n_units; i += 1024) fb[i] = 0;  // empty fallback list, no unit flagged
@@ -61,30 +61,44 @@ __global__ void chunk_offsets_kernel(const int32_t* __restrict__ cu_seqlens, int
   const int lo = min(n_seg, tid * per), hi = min(n_seg, lo + per);
   int sum = 0;
   for (int s = lo; s < hi; ++s) sum += (cu_seqlens[s + 1] - cu_seqlens[s] + kC - 1) / kC;
-  part[tid] = sum;
-  __syncthreads();
-  if (tid == 0) {
-    int run = 0;
-    for (int i = 0; i < 1024; ++i) {
-      const int v = part[i];
-      part[i] = run;
-      run += v;
+  {  // exclusive prefix sum of the 1,024 partial counts: warp scans, then a scan of the 32 warp totals
+    const int lane = tid & 31, warp = tid >> 5;
+    int incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int up = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += up;
     }
-    chunk_off[n_seg] = run;
+    __shared__ int wtot[32];
+    if (lane == 31) wtot[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+      int w = wtot[lane];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int up = __shfl_up_sync(0xffffffffu, w, o);
+        if (lane >= o) w += up;
+      }
+      wtot[lane] = w;  // inclusive
+      if (lane == 31) chunk_off[n_seg] = w;
+    }
+    __syncthreads();
+    part[tid] = incl - sum + (warp > 0 ? wtot[warp - 1] : 0);
   }
-  __syncthreads();
   int run = part[tid];
   for (int s = lo; s < hi; ++s) {
     chunk_off[s] = run;
     const int b = cu_seqlens[s], e = cu_seqlens[s + 1];
     const int n = (e - b + kC - 1) / kC;
-    for (int c = 0; c < n; ++c) chunk_meta[run + c] = make_int2(b + c * kC, min(kC, e - b - c * kC));
+    if (need_meta)
+      for (int c = 0; c < n; ++c) chunk_meta[run + c] = make_int2(b + c * kC, min(kC, e - b - c * kC));
     run += n;
   }
   __shared__ int total;
   if (tid == 1023) total = run;  // the last thread ends at the grand total
   __syncthreads();
-  for (int x = total + tid; x < cap; x += 1024) chunk_meta[x] = make_int2(0, 0);
+  if (need_meta)
+    for (int x = total + tid; x < cap; x += 1024) chunk_meta[x] = make_int2(0, 0);
   for (int sg = tid; sg < n_seg; sg += 1024) {
     int rank = sg;
     if (n_seg <= 8192) {
@@ -202,7 +216,7 @@ int encode_tensor(const EncodeArgs& a) {
   if (rc == HYPIC_OK) rc = make_kv_tensor_map(&tmV, a.v, a.t_total, a.H);
   if (rc != HYPIC_OK) return rc;
   chunk_offsets_kernel<<<1, 1024, 0, a.stream>>>(a.cu_seqlens, a.n_seg, chunk_off, seg_order, chunk_meta, (int)cap, fb,
-                                                 (long long)n_units);
+                                                 (long long)n_units, ch ? 1 : 0);  // the fused scalar-gate kernel needs no chunk table
   note_launch();
   const dim3 pgrid((unsigned)((cap + kPrepChunksPerCta - 1) / kPrepChunksPerCta), a.H), sgrid(a.H, a.n_seg);
   if (ch) {
