@@ -1,7 +1,8 @@
 """Build libhypic.so in-tree with nvcc for sm_100a (``python -m paper_2607_01299_b200.build``).
 
 The shared object lands next to this file (git-ignored, but it travels to the GPU box with the snapshot).
-nvcc cross-compiles without a GPU.  Nothing here touches ``oracle/``.
+nvcc cross-compiles without a GPU.  Nothing here touches ``oracle/``.  Extra nvcc flags (e.g. a -D switch of a diagnostic
+build) can be passed through the environment variable ``HYPIC_NVCC_EXTRA``; they enter the dependency digest.
 """
 from __future__ import annotations
 
